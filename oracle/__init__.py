@@ -1,0 +1,272 @@
+"""CPU oracle -- TEST INFRASTRUCTURE ONLY (see md_oracle.c header).
+
+Thin ctypes access to oracle/liboracle.so plus the velocity-Verlet driver loop written in the order of
+DESIGN.md "The path".  Imports nothing from the CUDA package; only tests/, __graft_entry__.smoke()
+and bench.py's cpu_baseline / --impl reference legs may import this.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+_dp = C.POINTER(C.c_double)
+_u32p = C.POINTER(C.c_uint32)
+_i32p = C.POINTER(C.c_int32)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build.build())
+        L.orc_neighbor_pairs.restype = C.c_uint64
+        L.orc_needs_rebuild.restype = C.c_int
+        L.orc_dpd_theta.restype = C.c_double
+        L.orc_dpd_theta.argtypes = [C.c_uint32, C.c_uint32, C.c_uint64, C.c_uint64]
+        _lib = L
+    return _lib
+
+
+def _d(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(_dp)
+
+
+def _u(a):
+    a = np.ascontiguousarray(a, dtype=np.uint32)
+    return a, a.ctypes.data_as(_u32p)
+
+
+def _box(box):
+    b = np.ascontiguousarray(np.broadcast_to(np.asarray(box, dtype=np.float64), (3,)))
+    return b, b.ctypes.data_as(_dp)
+
+
+def wrap(pos, box, image=None):
+    pos = np.array(pos, dtype=np.float64, order="C")
+    b, bp = _box(box)
+    ip = image.ctypes.data_as(_i32p) if image is not None else None
+    lib().orc_wrap(pos.ctypes.data_as(_dp), ip, C.c_uint64(pos.shape[0]), bp)
+    return pos
+
+
+def cell_dims(box, r_list):
+    b, bp = _box(box)
+    dims = np.zeros(3, dtype=np.uint32)
+    lib().orc_cell_dims(bp, C.c_double(r_list), dims.ctypes.data_as(_u32p))
+    return dims
+
+
+def cell_assign(pos, box, r_list):
+    pos, pp = _d(pos)
+    b, bp = _box(box)
+    N = pos.shape[0]
+    cell = np.zeros(N, dtype=np.uint32)
+    dims = np.zeros(3, dtype=np.uint32)
+    lib().orc_cell_assign(pp, C.c_uint64(N), bp, C.c_double(r_list), cell.ctypes.data_as(_u32p),
+                          dims.ctypes.data_as(_u32p))
+    return cell, dims
+
+
+def neighbor_pairs(pos, box, r_list):
+    """All unordered tag pairs (a<b) within r_list, shape (n_pairs, 2), lexicographically sorted."""
+    pos, pp = _d(pos)
+    b, bp = _box(box)
+    N = pos.shape[0]
+    n = lib().orc_neighbor_pairs(pp, C.c_uint64(N), bp, C.c_double(r_list), None, C.c_uint64(0))
+    pairs = np.zeros((n, 2), dtype=np.uint32)
+    n2 = lib().orc_neighbor_pairs(pp, C.c_uint64(N), bp, C.c_double(r_list), pairs.ctypes.data_as(_u32p),
+                                  C.c_uint64(n))
+    assert n2 == n
+    return pairs
+
+
+def needs_rebuild(pos, pos_ref, box, r_buff) -> bool:
+    pos, pp = _d(pos)
+    ref, rp = _d(pos_ref)
+    b, bp = _box(box)
+    return bool(lib().orc_needs_rebuild(pp, rp, C.c_uint64(pos.shape[0]), bp, C.c_double(r_buff)))
+
+
+def forces_lj(pos, box, rc, epsilon=1.0, sigma=1.0, energy_shift=1):
+    pos, pp = _d(pos)
+    b, bp = _box(box)
+    N = pos.shape[0]
+    F = np.zeros((N, 3))
+    E = np.zeros(N)
+    lib().orc_forces_lj(pp, C.c_uint64(N), bp, C.c_double(rc), C.c_double(epsilon), C.c_double(sigma),
+                        C.c_int(energy_shift), F.ctypes.data_as(_dp), E.ctypes.data_as(_dp))
+    return F, E
+
+
+def philox4x32_10(ctr, key):
+    c, cp = _u(ctr)
+    k, kp = _u(key)
+    out = np.zeros(4, dtype=np.uint32)
+    lib().orc_philox4x32_10(cp, kp, out.ctypes.data_as(_u32p))
+    return out
+
+
+def dpd_theta(tag_a, tag_b, step, seed) -> float:
+    return float(lib().orc_dpd_theta(int(tag_a), int(tag_b), int(step), int(seed)))
+
+
+def forces_dpd(pos, vel, box, rc, A, gamma, kT, dt, step, seed):
+    pos, pp = _d(pos)
+    vel, vp = _d(vel)
+    b, bp = _box(box)
+    N = pos.shape[0]
+    F = np.zeros((N, 3))
+    lib().orc_forces_dpd(pp, vp, C.c_uint64(N), bp, C.c_double(rc), C.c_double(A), C.c_double(gamma),
+                         C.c_double(kT), C.c_double(dt), C.c_uint64(step), C.c_uint64(seed),
+                         F.ctypes.data_as(_dp))
+    return F
+
+
+def forces_bonds(pos, box, bonds, k, r0, force=None, energy=None):
+    """Accumulates into force/energy (fresh zero arrays if None); returns (force, energy)."""
+    pos, pp = _d(pos)
+    b, bp = _box(box)
+    N = pos.shape[0]
+    bonds = np.ascontiguousarray(bonds, dtype=np.uint32).reshape(-1, 2)
+    ta, tap = _u(bonds[:, 0])
+    tb, tbp = _u(bonds[:, 1])
+    F = np.zeros((N, 3)) if force is None else force
+    E = np.zeros(N) if energy is None else energy
+    assert F.flags.c_contiguous and F.dtype == np.float64
+    lib().orc_forces_bonds(pp, C.c_uint64(N), bp, tap, tbp, C.c_uint64(bonds.shape[0]), C.c_double(k),
+                           C.c_double(r0), F.ctypes.data_as(_dp), E.ctypes.data_as(_dp))
+    return F, E
+
+
+def vv_half1(pos, vel, image, force, box, dt, mass=None):
+    """In place on pos, vel, image (C-contiguous float64 / int32 arrays)."""
+    b, bp = _box(box)
+    N = pos.shape[0]
+    for a in (pos, vel, force):
+        assert a.flags.c_contiguous and a.dtype == np.float64
+    mp = None
+    if mass is not None:
+        mass, mp = _d(mass)
+    ip = image.ctypes.data_as(_i32p) if image is not None else None
+    lib().orc_vv_half1(pos.ctypes.data_as(_dp), vel.ctypes.data_as(_dp), ip, force.ctypes.data_as(_dp), mp,
+                       C.c_uint64(N), bp, C.c_double(dt))
+
+
+def vv_half2(vel, force, dt, mass=None):
+    N = vel.shape[0]
+    assert vel.flags.c_contiguous and force.flags.c_contiguous
+    mp = None
+    if mass is not None:
+        mass, mp = _d(mass)
+    lib().orc_vv_half2(vel.ctypes.data_as(_dp), force.ctypes.data_as(_dp), mp, C.c_uint64(N), C.c_double(dt))
+
+
+def probe_nlist(pos, box, r_list, probes, row_stride=512):
+    pos, pp = _d(pos)
+    b, bp = _box(box)
+    pr, prp = _u(probes)
+    M = pr.shape[0]
+    counts = np.zeros(M, dtype=np.uint32)
+    nbrs = np.full((M, row_stride), 0xFFFFFFFF, dtype=np.uint32)
+    lib().orc_probe_nlist(pp, C.c_uint64(pos.shape[0]), bp, C.c_double(r_list), prp, C.c_uint64(M),
+                          counts.ctypes.data_as(_u32p), nbrs.ctypes.data_as(_u32p), C.c_uint64(row_stride))
+    return counts, nbrs
+
+
+def probe_forces_lj(pos, box, rc, probes, epsilon=1.0, sigma=1.0, energy_shift=1):
+    pos, pp = _d(pos)
+    b, bp = _box(box)
+    pr, prp = _u(probes)
+    M = pr.shape[0]
+    F = np.zeros((M, 3))
+    E = np.zeros(M)
+    lib().orc_probe_forces_lj(pp, C.c_uint64(pos.shape[0]), bp, C.c_double(rc), C.c_double(epsilon),
+                              C.c_double(sigma), C.c_int(energy_shift), prp, C.c_uint64(M),
+                              F.ctypes.data_as(_dp), E.ctypes.data_as(_dp))
+    return F, E
+
+
+def probe_forces_dpd(pos, vel, box, rc, A, gamma, kT, dt, step, seed, probes):
+    pos, pp = _d(pos)
+    vel, vp = _d(vel)
+    b, bp = _box(box)
+    pr, prp = _u(probes)
+    M = pr.shape[0]
+    F = np.zeros((M, 3))
+    lib().orc_probe_forces_dpd(pp, vp, C.c_uint64(pos.shape[0]), bp, C.c_double(rc), C.c_double(A),
+                               C.c_double(gamma), C.c_double(kT), C.c_double(dt), C.c_uint64(step),
+                               C.c_uint64(seed), prp, C.c_uint64(M), F.ctypes.data_as(_dp))
+    return F
+
+
+# ------------------------------------------------------------------------------------------------------
+# The step loop, in the order of DESIGN.md "The path" (S6a -> S3 -> [S1,S2] -> S4 (+S5) -> S6b).
+# ------------------------------------------------------------------------------------------------------
+class Sim:
+    """Plain MD driver on top of the O(N^2) routines.
+
+    what: dict with any of
+       lj    = dict(epsilon, sigma, energy_shift)
+       dpd   = dict(A, gamma, kT, seed)
+       bonds = dict(k, r0)  (+ self.bonds array)
+    Forces never depend on a neighbour list here (all pairs); the rebuild trigger (O3) is evaluated
+    only to log WHEN the CUDA path must rebuild.
+    """
+
+    def __init__(self, pos, vel, box, rc, r_buff, what, bonds=None, mass=None, step0=0):
+        self.box = np.ascontiguousarray(np.broadcast_to(np.asarray(box, dtype=np.float64), (3,)))
+        self.pos = wrap(pos, self.box)
+        self.vel = np.array(vel, dtype=np.float64, order="C")
+        self.N = self.pos.shape[0]
+        self.image = np.zeros((self.N, 3), dtype=np.int32)
+        self.rc, self.r_buff = float(rc), float(r_buff)
+        self.what = what
+        self.bonds = bonds
+        self.mass = mass
+        self.step = int(step0)
+        self.pos_ref = self.pos.copy()
+        self.rebuild_steps = []
+        self.force = None
+        self.energy = None
+
+    def compute_forces(self, dt, step):
+        F = np.zeros((self.N, 3))
+        E = np.zeros(self.N)
+        if "lj" in self.what:
+            p = self.what["lj"]
+            F, E = forces_lj(self.pos, self.box, self.rc, p.get("epsilon", 1.0), p.get("sigma", 1.0),
+                             p.get("energy_shift", 1))
+        if "dpd" in self.what:
+            p = self.what["dpd"]
+            F = F + forces_dpd(self.pos, self.vel, self.box, self.rc, p["A"], p["gamma"], p["kT"], dt, step,
+                               p["seed"])
+        if "bonds" in self.what:
+            p = self.what["bonds"]
+            F = np.ascontiguousarray(F)
+            forces_bonds(self.pos, self.box, self.bonds, p["k"], p["r0"], F, E)
+        self.force, self.energy = np.ascontiguousarray(F), E
+        return self.force
+
+    def run(self, n_steps, dt):
+        if self.force is None:
+            self.compute_forces(dt, self.step)          # DESIGN.md R16: F(t0) before the first half-kick
+        for _ in range(n_steps):
+            vv_half1(self.pos, self.vel, self.image, self.force, self.box, dt, self.mass)
+            if needs_rebuild(self.pos, self.pos_ref, self.box, self.r_buff):
+                self.pos_ref = self.pos.copy()
+                self.rebuild_steps.append(self.step + 1)
+            self.compute_forces(dt, self.step + 1)      # DESIGN.md R15: hash counter = step being completed
+            vv_half2(self.vel, self.force, dt, self.mass)
+            self.step += 1
+        return self
+
+    def kinetic_energy(self):
+        m = 1.0 if self.mass is None else np.asarray(self.mass)[:, None]
+        return 0.5 * float(np.sum(m * self.vel * self.vel))
+
+    def potential_energy(self):
+        return float(np.sum(self.energy))
