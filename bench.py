@@ -1,0 +1,320 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the MD hot path (BASELINE.json: particle-steps/sec for LJ at N=1M on one B200).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--scale s] [--impl ours|reference]
+
+A "step" is one MD time step of md_step: half-kick + drift + displacement check, (when the check fires) cell binning +
+neighbour-list rebuild, pair (+ bond) forces, half-kick -- i.e. one pass of every row of SURVEY.md 8(a); rebuilds fall
+inside the timed region at their natural frequency.  N = 1 runs config 2 (LJ, N = 1,048,576, mixed precision).
+Multi-GPU: "replicas only": every rank runs an independent replica, no collective on the data path; the
+time is the max over ranks, the value the sum of all ranks' particle-steps.
+
+Prints ONE JSON line (see the keys below).  `--impl reference` times the CPU oracle (a bounded sample per step).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "particle-steps/sec"
+UNIT = "particle-steps/s"
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def measured_hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(p))["hbm_gbs"]), "measured"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index=0):
+        self.gpu = gpu_index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def workload_for(args):
+    from paper_1412_3387_b200 import inputs
+    return inputs.config(args.config, scale=args.scale)
+
+
+def algorithmic_bytes(kind, nbar, k):
+    """B_min per particle-step (strict, fully-fused ideal) and the staged minimum of the pair-force
+    kernel (index stream + own position + force write [+ velocity and tag for DPD])."""
+    dpd = kind in ("dpd", "polymer")
+    b_min = 4.0 * nbar * (1.0 + 1.0 / k) + 120.0 + (4.0 if dpd else 0.0) + 130.0 / k
+    force_kernel = 4.0 * nbar + (84.0 if dpd else 56.0)
+    return b_min, force_kernel
+
+
+# ----------------------------------------------------------------------------------------------------------------
+def cpu_baseline(w, budget_s=15.0):
+    """The oracle as it stands, one host core, on a bounded sample: force rows of M probe particles against all N
+    (O(M N) brute force, oracle O9).  Value = probe rows per second = particle force evaluations per second, the
+    dominant cost of a particle-step (integration is negligible next to the O(N) pair search per particle)."""
+    import oracle
+    from paper_1412_3387_b200 import inputs
+    M = 8
+    t_used, rows = 0.0, 0
+    p = w.params
+    while True:
+        pr = inputs.probe_tags(w.N, M, seed=99 + M)
+        t0 = time.perf_counter()
+        if w.kind == "lj":
+            oracle.probe_forces_lj(w.pos, w.box, w.rc, pr, p["epsilon"], p["sigma"], p["energy_shift"])
+        else:
+            oracle.probe_forces_dpd(w.pos, w.vel, w.box, w.rc, p["A"], p["gamma"], p["kT"], w.dt, 1, p["seed"], pr)
+        dt = time.perf_counter() - t0
+        t_used += dt; rows += len(pr)
+        rate = len(pr) / dt
+        if t_used > 0.6 * budget_s or len(pr) >= w.N:
+            break
+        M = int(min(w.N, max(2 * M, 0.5 * (budget_s - t_used) * rate)))
+    return {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"pair-force rows of {len(pr)} seeded probe particles against all N={w.N} "
+                      f"(O(M*N) brute force, oracle/md_oracle.c orc_probe_forces_*), {dt:.1f} s on 1 core; "
+                      f"full step extrapolated = N/M x this"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle, timed per 'step' on a bounded sample of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    from paper_1412_3387_b200 import inputs
+    w = workload_for(args)
+    p = w.params
+    # size the per-step sample so that the whole run stays within a few minutes
+    probe = inputs.probe_tags(w.N, 4, seed=5)
+    t0 = time.perf_counter()
+    oracle.probe_forces_lj(w.pos, w.box, w.rc, probe) if w.kind == "lj" else oracle.probe_forces_dpd(
+        w.pos, w.vel, w.box, w.rc, p["A"], p["gamma"], p["kT"], w.dt, 1, p["seed"], probe)
+    per_row = (time.perf_counter() - t0) / len(probe)
+    budget = 120.0 / max(1, args.steps + args.warmup)
+    M = int(max(1, min(w.N, budget / per_row)))
+    times = []
+    for s in range(args.warmup + args.steps):
+        pr = inputs.probe_tags(w.N, M, seed=1000 + s)
+        t0 = time.perf_counter()
+        if w.kind == "lj":
+            oracle.probe_forces_lj(w.pos, w.box, w.rc, pr, p["epsilon"], p["sigma"], p["energy_shift"])
+        else:
+            oracle.probe_forces_dpd(w.pos, w.vel, w.box, w.rc, p["A"], p["gamma"], p["kT"], w.dt, s, p["seed"], pr)
+        if s >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    t = float(np.sum(times))
+    value = M * len(times) / t
+    sample = (f"each step = pair-force rows of {M} seeded probe particles against all N={w.N} (O(M*N) brute force); "
+              f"value = rows/s = particle force evaluations/s")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / len(times),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "N": w.N, "precision": w.precision},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ----------------------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1412_3387_b200 import binding as B
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = workload_for(args)
+    precision = B.MD_MIXED if w.precision == "mixed" else B.MD_FP64
+    stream = torch.cuda.Stream()
+    order = {"lex": B.MD_ORDER_LEX, "morton": B.MD_ORDER_MORTON, "hilbert": B.MD_ORDER_HILBERT}[args.order]
+    md = B.MD(w.box, w.N, w.rc, w.r_buff, precision=precision, stream=stream.cuda_stream, order=order,
+              sched=B.MD_SCHED_HOST)
+    desc = B.step_desc(w.kind, w.dt, w.params)
+
+    # inputs resident in HBM before the timed region
+    d_pos = torch.from_numpy(w.pos).to("cuda")
+    d_vel = torch.from_numpy(w.vel).to("cuda")
+    torch.cuda.synchronize()
+    md.set_state(d_pos, d_vel)
+    if w.bonds is not None:
+        md.set_bonds(w.bonds)
+    if not args.no_tune:
+        md.tune(desc, False)
+
+    # ---- device-resident timing ---------------------------------------------------------------------------
+    md.step(desc, max(3, args.warmup))
+    st0 = md.stats()
+    md.set_profiling(True)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    e0 = torch.cuda.Event(enable_timing=True)
+    e1 = torch.cuda.Event(enable_timing=True)
+    barrier()
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        md.step(desc, args.steps)
+        e1.record(stream)
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms = e0.elapsed_time(e1)
+    st1 = md.stats()
+    md.set_profiling(False)
+
+    # ---- end to end through the C-ABI with HOST buffers: upload state, K steps, download state ----------------
+    h_pos = torch.from_numpy(w.pos).pin_memory()
+    h_vel = torch.from_numpy(w.vel).pin_memory()
+    o_pos = torch.empty_like(h_pos).pin_memory()
+    o_vel = torch.empty_like(h_vel).pin_memory()
+    md.set_state(h_pos, h_vel)
+    md.step(desc, 3)                                   # warm (first list build of the new state)
+    barrier()
+    t0 = time.perf_counter()
+    md.set_state(h_pos, h_vel)
+    md.step(desc, args.steps)
+    md.get_state(o_pos, o_vel, None)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    barrier()
+
+    t = torch.tensor([ms, e2e_s * 1e3], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max, e2e_ms = float(t[0]), float(t[1])
+
+    if rank == 0:
+        steps = st1["steps"] - st0["steps"]
+        rebuilds = st1["rebuilds"] - st0["rebuilds"]
+        k = steps / max(1, rebuilds)
+        nbar = st1["mean_neighbors"]
+        b_min, b_force = algorithmic_bytes(w.kind, nbar, k)
+        peak, peak_src = measured_hbm_peak()
+        value = world * w.N * args.steps / (ms_max * 1e-3)
+        fk = "lj" if w.kind == "lj" else "dpd"
+        f_ms = st1["stage_ms"][fk] / max(1, st1["stage_launches"][fk])
+        achieved = w.N * b_force / (f_ms * 1e-3) / 1e9 if f_ms > 0 else 0.0
+        stage_share = {n: round(v / ms, 4) for n, v in st1["stage_ms"].items() if v > 0}
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(3, args.warmup), "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32" if precision == B.MD_MIXED else "f64",
+            "data": "synthetic",
+            "config": {"workload": w.name, "N": w.N, "precision": w.precision, "rc": w.rc, "r_buff": w.r_buff,
+                       "dt": w.dt, "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": "inputs larger than L2 (neighbour list %.0f MB + state)" % (4e-6 * st1["nlist_entries"]),
+                       "tps": world * args.steps / (ms_max * 1e-3) / world, "rebuild_period_k": k,
+                       "mean_neighbors": nbar, "rebuilds": rebuilds, "dangerous_builds": st1["dangerous_builds"],
+                       "order": args.order, "sched": "host",
+                       "launch": {n: [v["block"], v["w"]] for n, v in st1["launch"].items()},
+                       "stage_share_of_step": stage_share,
+                       "step_bmin_bytes_per_particle": b_min,
+                       "step_roofline_frac": (w.N * b_min * args.steps / (ms_max * 1e-3)) / (peak * 1e9)},
+            "e2e": {"value": world * w.N * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
+                    "h2d_bytes_per_step": int(2 * w.pos.nbytes / args.steps),
+                    "d2h_bytes_per_step": int(2 * w.pos.nbytes / args.steps)},
+            "gpu_launches": int(st1["launches"] - st0["launches"]),
+            "clocks": clocks,
+            "roofline": {"bound": "hbm", "kernel": "k_forces_" + fk, "achieved": achieved, "peak": peak,
+                         "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                         "bytes_per_particle": b_force, "launch_ms": f_ms},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(w)
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=100)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--scale", type=float, default=1.0)
+    ap.add_argument("--order", default="lex", choices=["lex", "morton", "hilbert"])
+    ap.add_argument("--no-tune", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        sys.exit(run_reference(args))
+    sys.exit(run_ours(args))
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,223 @@
+/*
+ * b200md.h -- C-ABI of the B200-native single-GPU molecular-dynamics hot path.
+ *
+ * Implements the single-GPU engine that runs on every rank of HOOMD-blue 1.0 as described in
+ * Glaser et al., "Strong scaling of general-purpose molecular dynamics simulations on GPUs"
+ * (arXiv:1412.3387).  Citations "PAPER.md:<line>" refer to /root/reference/PAPER.md; "R<n>" to the
+ * numbered readings in DESIGN.md (the paper prints no formulas, so each operation also names the
+ * textbook definition it uses).
+ *
+ * Conventions
+ *  - Every function returns 0 (MD_OK) or a negative md_status; md_last_error(ctx) gives the text.
+ *  - Box: orthorhombic, periodic, edge lengths box[3], coordinates in [-L/2, L/2) per axis (R4).
+ *  - Particles are identified by TAG = index into the caller's arrays (0..N-1).  Every array crossing
+ *    this boundary is in TAG ORDER, row-major (N x 3 for vectors).  Internally particles are kept
+ *    sorted by cell along a space-filling curve ("reordering of the GPU arrays").
+ *  - POINTERS: every array pointer may be a HOST pointer or a CUDA DEVICE pointer; the library asks
+ *    the driver (cudaPointerGetAttributes) and copies accordingly.  The caller owns every pointer it
+ *    passes; the library never keeps one past the call.  Calls with device pointers only enqueue work
+ *    on the context's stream; calls with a host OUTPUT pointer synchronise that stream before
+ *    returning.  No torch types appear here; the Python binding passes tensor.data_ptr().
+ *  - All device work runs on the stream given to md_configure (default: the legacy default stream).
+ *  - The context owns all internal device memory (allocated with cudaMalloc at create/configure time,
+ *    the neighbour list grows on demand at a rebuild).  One context per host thread; no global state.
+ *  - There is NO CPU fallback: every entry point needs a CUDA device and fails with MD_ECUDA otherwise.
+ */
+#ifndef B200MD_H
+#define B200MD_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct md_ctx md_ctx;
+
+typedef enum {
+    MD_OK = 0,
+    MD_EINVAL = -1,  /* bad argument; box too small (needs floor(L/r_list) >= 3 per axis so that the 27-cell
+                        stencil has no duplicate cells and r_list < L/2 for the minimum image) */
+    MD_ESTATE = -2,  /* call out of order (e.g. md_build_nlist before md_set_state) */
+    MD_ENOMEM = -3,  /* device allocation failed */
+    MD_ECUDA = -4    /* CUDA runtime error, text in md_last_error */
+} md_status;
+
+/* arithmetic of the pair-force evaluation ("full double precision is available per compile-time
+   option"; here a run-time mode, R25) */
+#define MD_FP64 0   /* everything fp64 */
+#define MD_MIXED 1  /* LJ pair polynomial in fp32 on fp32 separations, r<rc decision as fp64 would take it,
+                       per-pair contributions summed in fp64; positions, velocities, integration, cell ids,
+                       neighbour-list decisions, displacement check stay fp64 */
+
+/* internal storage order of the cells (particles are always sorted by cell, ties by tag) */
+#define MD_ORDER_LEX 0     /* x fastest, then y, then z */
+#define MD_ORDER_MORTON 1  /* Z-order curve over (cx, cy, cz) */
+#define MD_ORDER_HILBERT 2 /* 3-D Hilbert curve over (cx, cy, cz) */
+
+/* which terms md_step evaluates */
+#define MD_F_LJ 1u
+#define MD_F_DPD 2u
+#define MD_F_BONDS 4u
+
+/* scheduling of md_step */
+#define MD_SCHED_HOST 0  /* host reads the rebuild flag every step (one small D2H + stream sync per step) */
+#define MD_SCHED_GRAPH 1 /* one CUDA graph per step; rebuild inside a device-side conditional node */
+
+typedef struct {
+    uint32_t flags;      /* MD_F_* */
+    int32_t lj_energy_shift;
+    double dt;
+    double lj_epsilon, lj_sigma;
+    double dpd_A, dpd_gamma, dpd_kT;
+    uint64_t dpd_seed;
+    double bond_k, bond_r0;
+} md_step_desc;
+
+#define MD_N_KERNELS 8
+enum { MD_K_NLIST = 0, MD_K_LJ = 1, MD_K_DPD = 2, MD_K_BONDS = 3, MD_K_INTEGRATE = 4, MD_K_CELLS = 5 };
+
+typedef struct {
+    uint64_t steps;             /* time steps taken by md_step since create */
+    uint64_t rebuilds;          /* neighbour-list builds (md_build_nlist calls + rebuilds inside md_step) */
+    uint64_t dangerous_builds;  /* rebuilds at which some particle had moved more than r_buff (not r_buff/2)
+                                   since the last build: with a check every step this must stay 0 */
+    uint64_t nlist_entries;     /* entries of the current full (double-sided) list */
+    uint64_t nlist_capacity;    /* entries allocated */
+    uint64_t device_bytes;      /* device memory owned by the context */
+    double mean_neighbors;      /* nlist_entries / N */
+    uint32_t dims[3];           /* cell grid */
+    uint32_t max_cell_count;    /* most populated cell at the last build */
+    int32_t block[MD_N_KERNELS];    /* launch parameters chosen by the tuner, per kernel */
+    int32_t w[MD_N_KERNELS];        /* threads per particle, per kernel */
+    float tuned_us[MD_N_KERNELS];   /* median time of the chosen setting when it was tuned */
+    uint32_t tuner_runs;        /* number of tuning sweeps performed */
+    uint32_t launches;          /* kernel launches issued by this context since create (all entry points) */
+    double stage_ms[MD_N_KERNELS];          /* with md_set_profiling(ctx,1): device time per stage (CUDA events on */
+    uint64_t stage_launches[MD_N_KERNELS];  /* the context's stream), accumulated since profiling was switched on  */
+} md_stats;
+
+/* ---- lifetime ------------------------------------------------------------------------------------------ */
+
+/* Neighbour problem of PAPER.md:79 / Fig. 1: N particles in a periodic box, pair cut-off rc
+   and buffer ("skin") r_buff; the list radius is r_list = rc + r_buff.  box: HOST pointer to 3 doubles.
+   Fails with MD_EINVAL unless floor(box[a]/r_list) >= 3 on every axis. */
+int md_create(md_ctx **out, const double box[3], uint64_t N, double rc, double r_buff);
+
+/* precision: MD_FP64 | MD_MIXED.  stream: a cudaStream_t (as void*), NULL = default stream.
+   order: MD_ORDER_*.  sched: MD_SCHED_*.  May be called again before md_set_state. */
+int md_configure(md_ctx *ctx, int precision, void *stream, int order, int sched);
+
+/* Releases every device buffer.  ctx is invalid afterwards. */
+int md_destroy(md_ctx *ctx);
+
+const char *md_last_error(md_ctx *ctx); /* static/ctx-owned string; valid until the next call on ctx */
+
+/* ---- state (tag order) --------------------------------------------------------------------------------- */
+
+/* pos, vel: N x 3 doubles.  mass: N doubles or NULL (= 1).  Positions are wrapped into the box once and the
+   periodic image counters reset to 0 (R4).  step0 is the time-step counter of this state (enters the DPD hash).
+   Invalidates cells, neighbour list and forces. */
+int md_set_state(md_ctx *ctx, const double *pos, const double *vel, const double *mass, uint64_t step0);
+
+/* Bonds as unordered tag pairs.  Stored per particle so that each particle sums its own bonds
+   without atomics.  n_bonds = 0 clears.  A particle may have any number of bonds. */
+int md_set_bonds(md_ctx *ctx, const uint32_t *tag_a, const uint32_t *tag_b, uint64_t n_bonds);
+
+/* pos, vel: N x 3 doubles (wrapped positions); image: N x 3 int32 or NULL.  Any of the three may be NULL. */
+int md_get_state(md_ctx *ctx, double *pos, double *vel, int32_t *image);
+
+/* force: N x 3 doubles, energy: N doubles (per-particle potential energy, half of each pair / bond energy) or
+   NULL.  MD_ESTATE if no force has been computed for the current positions. */
+int md_get_forces(md_ctx *ctx, double *force, double *energy);
+
+/* ---- S1 cell binning (PAPER.md:126 cell list; Fig. 4 step 1) ------------------------------- */
+
+/* Cell of every particle: n_c = floor(L/r_list) per axis, f = (x + L/2)/L, c = (int)(f n_c) clamped to n_c-1
+   (R5, bit-exact IEEE double, no FMA); then a deterministic counting sort of ALL per-particle arrays into cell
+   order (cells along the configured curve, particles of one cell by ascending tag), and a snapshot of the
+   positions for the displacement check (S3).  Invalidates the neighbour list. */
+int md_build_cells(md_ctx *ctx);
+
+/* cell_of: N uint32 in tag order, linear id cx + n_cx (cy + n_cy cz); dims: 3 uint32 (HOST pointer). */
+int md_get_cells(md_ctx *ctx, uint32_t *cell_of, uint32_t dims[3]);
+
+/* ---- S2 neighbour list (Fig. 4; list radius PAPER.md:79) -------------------------------- */
+
+/* Full (double-sided) Verlet list: row i holds every j != i with |minimg(x_i - x_j)|^2 < r_list^2 (strict;
+   (dx^2 + dy^2) + dz^2 in IEEE double without FMA, R2).  w cooperative threads per particle stride over the 27
+   stencil cells and compact with a w-wide prefix sum (no atomics).  Requires md_build_cells on the current
+   positions (it is run automatically if missing). */
+int md_build_nlist(md_ctx *ctx);
+
+/* Unordered export: each listed pair once as (tag_i < tag_j).  pairs = NULL: only *n_pairs is written
+   (HOST pointer).  Otherwise pairs must hold 2 * cap uint32; MD_EINVAL if cap is too small.
+   The ORDER of the pairs is unspecified (sort to compare). */
+int md_get_nlist(md_ctx *ctx, uint64_t *n_pairs, uint32_t *pairs, uint64_t cap);
+
+/* Rows of selected particles: counts[n_probe] = row length, nbr_tags[p * row_stride + k] = tag of the k-th
+   neighbour (k < min(count, row_stride)), order within a row unspecified. */
+int md_get_nlist_rows(md_ctx *ctx, const uint32_t *probe_tags, uint32_t n_probe, uint32_t *counts,
+                      uint32_t *nbr_tags, uint32_t row_stride);
+
+/* ---- S4/S5 forces (w threads per particle, shuffle reduction, one write per particle) ------ */
+
+/* Truncated LJ 12-6 (R1): F_i = sum_j 24 eps (2 s^12 - s^6)/r^2 d_ij over list neighbours with
+   r^2 < rc^2, s = sigma/r; per-particle energy = 1/2 sum_j [4 eps (s^12 - s^6) - shift U(rc)].  OVERWRITES the
+   force/energy arrays.  Needs a valid neighbour list (MD_ESTATE otherwise). */
+int md_forces_lj(md_ctx *ctx, double epsilon, double sigma, int energy_shift);
+
+/* DPD (Groot-Warren form, R5): for 0 < r < rc, w = 1 - r/rc,
+   F_ij = [A w - gamma w^2 (rhat . v_ij) + sqrt(2 gamma kT) w theta_ij / sqrt(dt)] rhat,
+   theta_ij = sqrt(3) (2u - 1), u = (X + 1/2) 2^-32, X = word 0 of Philox4x32-10 with
+   counter (min tag, max tag, step lo, step hi) and key (seed lo, seed hi) (R13, R14).
+   Uses the velocities as stored at the time of the call.  OVERWRITES force (energy lane = conservative energy). */
+int md_forces_dpd(md_ctx *ctx, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed);
+
+/* Harmonic bonds U = k/2 (r - r0)^2 (R6).  ACCUMULATES into force/energy. */
+int md_forces_bonds(md_ctx *ctx, double k, double r0);
+
+/* ---- S6 velocity-Verlet, NVE (R7) ---------------------------------------------------------- */
+
+/* half = 1: v += (dt/2) F/m; x += dt v; wrap into the box (image counters updated); evaluates the displacement
+   criterion of PAPER.md:79 (some particle moved more than r_buff/2 since the last md_build_cells, strict >) into a
+   device flag; invalidates forces.   half = 2: v += (dt/2) F/m. */
+int md_integrate_nve(md_ctx *ctx, double dt, int half);
+
+/* Host read of the displacement flag set by the last half-1 (synchronises).  *flag = 1: a rebuild is due. */
+int md_needs_rebuild(md_ctx *ctx, int *flag);
+
+/* ---- S7 step scheduler ---------------------------------------------------------------------------------- */
+
+/* n_steps of { half 1 -> displacement check -> [cells + neighbour list] -> forces -> half 2 }.  If no force is
+   current, forces are first evaluated at the current step index (R16).  The force evaluated during the step that
+   advances t -> t+1 uses hash counter t+1 (R15). */
+int md_step(md_ctx *ctx, const md_step_desc *what, uint64_t n_steps);
+
+/* ---- S8 runtime tuner ------------------------------------------------------------------ */
+
+/* Sweeps block size (multiples of 32 up to 1024; `full` = all 32, else a pruned set) x threads per particle
+   w in {1,2,4,8,16,32} for the neighbour-list kernel and the pair-force kernel `what` selects, on the live state
+   (the kernels are pure functions of it), median of 5 timed launches each, and fixes the fastest.  Choices are
+   reported by md_get_stats and, if the environment variable B200MD_LOG is set, printed to stderr. */
+int md_tune(md_ctx *ctx, const md_step_desc *what, int full);
+
+/* Fix launch parameters by hand (block multiple of 32 in [32,1024]; w power of two <= 32); kernel = MD_K_*. */
+int md_set_launch(md_ctx *ctx, int kernel, int block, int w);
+
+int md_get_stats(md_ctx *ctx, md_stats *out); /* synchronises */
+
+/* on = 1: bracket every stage launched by md_step / md_build_* / md_forces_* / md_integrate_nve with CUDA events on the
+   context's stream and accumulate their durations into md_stats.stage_ms (MD_K_CELLS = binning + reorder, MD_K_NLIST =
+   count + scan + fill, MD_K_LJ / MD_K_DPD / MD_K_BONDS force kernels, MD_K_INTEGRATE both halves).  Resets the
+   accumulators.  on = 0 switches the events off. */
+int md_set_profiling(md_ctx *ctx, int on);
+
+/* Test hook: Philox4x32-10 of `n` (counter, key) inputs evaluated ON THE DEVICE by the same device function the
+   DPD kernel uses.  ctr: n x 4 uint32, key: n x 2 uint32, out: n x 4 uint32 (host or device pointers). */
+int md_debug_philox(md_ctx *ctx, const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint64_t n);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* B200MD_H */

@@ -1,0 +1,286 @@
+"""Thin Python binding of the C-ABI in include/b200md.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of csrc/libb200md.so; this module converts numpy arrays /
+torch tensors to raw pointers and calls the functions of the same name.  There is no fallback: if the shared
+library is missing or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "csrc", "libb200md.so")
+
+MD_FP64, MD_MIXED = 0, 1
+MD_ORDER_LEX, MD_ORDER_MORTON, MD_ORDER_HILBERT = 0, 1, 2
+MD_F_LJ, MD_F_DPD, MD_F_BONDS = 1, 2, 4
+MD_SCHED_HOST, MD_SCHED_GRAPH = 0, 1
+MD_N_KERNELS = 8
+MD_K_NLIST, MD_K_LJ, MD_K_DPD, MD_K_BONDS, MD_K_INTEGRATE, MD_K_CELLS = 0, 1, 2, 3, 4, 5
+KERNEL_NAMES = {MD_K_NLIST: "nlist", MD_K_LJ: "lj", MD_K_DPD: "dpd", MD_K_BONDS: "bonds",
+                MD_K_INTEGRATE: "integrate", MD_K_CELLS: "cells"}
+
+EXPORTS = ["md_create", "md_configure", "md_destroy", "md_last_error", "md_set_state", "md_set_bonds",
+           "md_get_state", "md_get_forces", "md_build_cells", "md_get_cells", "md_build_nlist", "md_get_nlist",
+           "md_get_nlist_rows", "md_forces_lj", "md_forces_dpd", "md_forces_bonds", "md_integrate_nve",
+           "md_needs_rebuild", "md_step", "md_tune", "md_set_launch", "md_get_stats", "md_set_profiling",
+           "md_debug_philox"]
+
+
+class md_step_desc(C.Structure):
+    _fields_ = [("flags", C.c_uint32), ("lj_energy_shift", C.c_int32), ("dt", C.c_double),
+                ("lj_epsilon", C.c_double), ("lj_sigma", C.c_double),
+                ("dpd_A", C.c_double), ("dpd_gamma", C.c_double), ("dpd_kT", C.c_double),
+                ("dpd_seed", C.c_uint64), ("bond_k", C.c_double), ("bond_r0", C.c_double)]
+
+
+class md_stats(C.Structure):
+    _fields_ = [("steps", C.c_uint64), ("rebuilds", C.c_uint64), ("dangerous_builds", C.c_uint64),
+                ("nlist_entries", C.c_uint64), ("nlist_capacity", C.c_uint64), ("device_bytes", C.c_uint64),
+                ("mean_neighbors", C.c_double), ("dims", C.c_uint32 * 3), ("max_cell_count", C.c_uint32),
+                ("block", C.c_int32 * MD_N_KERNELS), ("w", C.c_int32 * MD_N_KERNELS),
+                ("tuned_us", C.c_float * MD_N_KERNELS), ("tuner_runs", C.c_uint32), ("launches", C.c_uint32),
+                ("stage_ms", C.c_double * MD_N_KERNELS), ("stage_launches", C.c_uint64 * MD_N_KERNELS)]
+
+
+class MDError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def load():
+    """Open csrc/libb200md.so (built by `python -m paper_1412_3387_b200.csrc.build`).  Raises if missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise MDError(f"{LIB_PATH} is missing: build it with `python -m paper_1412_3387_b200.csrc.build` "
+                      "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, u64, dbl, i32, u32 = C.c_void_p, C.c_uint64, C.c_double, C.c_int, C.c_uint32
+    sig = {
+        "md_create": [C.POINTER(vp), C.POINTER(dbl), u64, dbl, dbl],
+        "md_configure": [vp, i32, vp, i32, i32],
+        "md_destroy": [vp],
+        "md_set_state": [vp, vp, vp, vp, u64],
+        "md_set_bonds": [vp, vp, vp, u64],
+        "md_get_state": [vp, vp, vp, vp],
+        "md_get_forces": [vp, vp, vp],
+        "md_build_cells": [vp],
+        "md_get_cells": [vp, vp, C.POINTER(u32)],
+        "md_build_nlist": [vp],
+        "md_get_nlist": [vp, C.POINTER(u64), vp, u64],
+        "md_get_nlist_rows": [vp, vp, u32, vp, vp, u32],
+        "md_forces_lj": [vp, dbl, dbl, i32],
+        "md_forces_dpd": [vp, dbl, dbl, dbl, dbl, u64, u64],
+        "md_forces_bonds": [vp, dbl, dbl],
+        "md_integrate_nve": [vp, dbl, i32],
+        "md_needs_rebuild": [vp, C.POINTER(i32)],
+        "md_step": [vp, C.POINTER(md_step_desc), u64],
+        "md_tune": [vp, C.POINTER(md_step_desc), i32],
+        "md_set_launch": [vp, i32, i32, i32],
+        "md_get_stats": [vp, C.POINTER(md_stats)],
+        "md_set_profiling": [vp, i32],
+        "md_debug_philox": [vp, vp, vp, vp, u64],
+    }
+    for name, args in sig.items():
+        fn = getattr(L, name)
+        fn.argtypes = args
+        fn.restype = C.c_int
+    L.md_last_error.argtypes = [vp]
+    L.md_last_error.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _ptr(a):
+    """Raw address of a numpy array (host) or torch tensor (host or CUDA); None -> NULL."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        assert a.flags.c_contiguous, "array must be C-contiguous"
+        return a.ctypes.data
+    if hasattr(a, "data_ptr"):
+        assert a.is_contiguous(), "tensor must be contiguous"
+        return a.data_ptr()
+    raise TypeError(type(a))
+
+
+def step_desc(kind: str, dt: float, params: dict) -> md_step_desc:
+    d = md_step_desc()
+    d.dt = dt
+    d.lj_epsilon, d.lj_sigma, d.lj_energy_shift = 1.0, 1.0, 1
+    if kind == "lj":
+        d.flags = MD_F_LJ
+        d.lj_epsilon = params.get("epsilon", 1.0)
+        d.lj_sigma = params.get("sigma", 1.0)
+        d.lj_energy_shift = int(params.get("energy_shift", 1))
+    elif kind in ("dpd", "polymer"):
+        d.flags = MD_F_DPD | (MD_F_BONDS if kind == "polymer" else 0)
+        d.dpd_A, d.dpd_gamma, d.dpd_kT = params["A"], params["gamma"], params["kT"]
+        d.dpd_seed = int(params["seed"])
+        d.bond_k, d.bond_r0 = params.get("bond_k", 0.0), params.get("bond_r0", 0.0)
+    elif kind == "bonds":
+        d.flags = MD_F_BONDS
+        d.bond_k, d.bond_r0 = params["bond_k"], params["bond_r0"]
+    elif kind == "none":
+        d.flags = 0
+    else:
+        raise ValueError(kind)
+    return d
+
+
+class MD:
+    """One simulation context (md_ctx).  Methods are 1:1 with the C entry points (md_ prefix dropped)."""
+
+    def __init__(self, box, N, rc, r_buff, precision=MD_FP64, stream=None, order=MD_ORDER_LEX, sched=MD_SCHED_HOST):
+        self.L = load()
+        self.N = int(N)
+        b = (C.c_double * 3)(*[float(x) for x in np.broadcast_to(np.asarray(box, dtype=np.float64), (3,))])
+        h = C.c_void_p()
+        s = self.L.md_create(C.byref(h), b, self.N, float(rc), float(r_buff))
+        if s != 0:
+            raise MDError(f"md_create -> {s}: {self.L.md_last_error(None).decode()}")
+        self.h = h
+        self._chk(self.L.md_configure(self.h, precision, stream, order, sched), "md_configure")
+
+    def _chk(self, s, who):
+        if s != 0:
+            raise MDError(f"{who} -> {s}: {self.L.md_last_error(self.h).decode()}")
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.md_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # --- state
+    def set_state(self, pos, vel, mass=None, step0=0):
+        self._keep = (pos, vel, mass)
+        self._chk(self.L.md_set_state(self.h, _ptr(pos), _ptr(vel), _ptr(mass), int(step0)), "md_set_state")
+
+    def set_bonds(self, bonds):
+        if bonds is None or len(bonds) == 0:
+            self._chk(self.L.md_set_bonds(self.h, None, None, 0), "md_set_bonds")
+            return
+        b = np.ascontiguousarray(bonds, dtype=np.uint32).reshape(-1, 2)
+        ta, tb = np.ascontiguousarray(b[:, 0]), np.ascontiguousarray(b[:, 1])
+        self._chk(self.L.md_set_bonds(self.h, _ptr(ta), _ptr(tb), b.shape[0]), "md_set_bonds")
+
+    def get_state(self, pos=None, vel=None, image=None):
+        """Fills the given arrays/tensors; with no arguments returns fresh numpy (pos, vel, image)."""
+        if pos is None and vel is None and image is None:
+            pos = np.empty((self.N, 3)); vel = np.empty((self.N, 3)); image = np.empty((self.N, 3), dtype=np.int32)
+        self._chk(self.L.md_get_state(self.h, _ptr(pos), _ptr(vel), _ptr(image)), "md_get_state")
+        return pos, vel, image
+
+    def get_forces(self, force=None, energy=None):
+        if force is None and energy is None:
+            force = np.empty((self.N, 3)); energy = np.empty(self.N)
+        self._chk(self.L.md_get_forces(self.h, _ptr(force), _ptr(energy)), "md_get_forces")
+        return force, energy
+
+    # --- S1/S2
+    def build_cells(self):
+        self._chk(self.L.md_build_cells(self.h), "md_build_cells")
+
+    def get_cells(self, cell_of=None):
+        dims = (C.c_uint32 * 3)()
+        if cell_of is None:
+            cell_of = np.empty(self.N, dtype=np.uint32)
+        self._chk(self.L.md_get_cells(self.h, _ptr(cell_of), dims), "md_get_cells")
+        return cell_of, np.array(list(dims), dtype=np.uint32)
+
+    def build_nlist(self):
+        self._chk(self.L.md_build_nlist(self.h), "md_build_nlist")
+
+    def get_nlist(self, device_out=None):
+        """Unique pairs (tag_i < tag_j), unordered.  Returns a numpy (n,2) array unless a tensor is supplied."""
+        n = C.c_uint64()
+        self._chk(self.L.md_get_nlist(self.h, C.byref(n), None, 0), "md_get_nlist")
+        if device_out is not None:
+            assert device_out.numel() >= 2 * n.value
+            self._chk(self.L.md_get_nlist(self.h, C.byref(n), _ptr(device_out), n.value), "md_get_nlist")
+            return n.value
+        pairs = np.empty((n.value, 2), dtype=np.uint32)
+        self._chk(self.L.md_get_nlist(self.h, C.byref(n), _ptr(pairs), n.value), "md_get_nlist")
+        return pairs
+
+    def get_nlist_rows(self, probe_tags, row_stride=512):
+        pr = np.ascontiguousarray(probe_tags, dtype=np.uint32)
+        counts = np.empty(pr.shape[0], dtype=np.uint32)
+        nbrs = np.empty((pr.shape[0], row_stride), dtype=np.uint32)
+        self._chk(self.L.md_get_nlist_rows(self.h, _ptr(pr), pr.shape[0], _ptr(counts), _ptr(nbrs), row_stride),
+                  "md_get_nlist_rows")
+        return counts, nbrs
+
+    # --- S4/S5/S6
+    def forces_lj(self, epsilon=1.0, sigma=1.0, energy_shift=1):
+        self._chk(self.L.md_forces_lj(self.h, float(epsilon), float(sigma), int(energy_shift)), "md_forces_lj")
+
+    def forces_dpd(self, A, gamma, kT, dt, step, seed):
+        self._chk(self.L.md_forces_dpd(self.h, float(A), float(gamma), float(kT), float(dt), int(step), int(seed)),
+                  "md_forces_dpd")
+
+    def forces_bonds(self, k, r0):
+        self._chk(self.L.md_forces_bonds(self.h, float(k), float(r0)), "md_forces_bonds")
+
+    def integrate_nve(self, dt, half):
+        self._chk(self.L.md_integrate_nve(self.h, float(dt), int(half)), "md_integrate_nve")
+
+    def needs_rebuild(self) -> bool:
+        f = C.c_int()
+        self._chk(self.L.md_needs_rebuild(self.h, C.byref(f)), "md_needs_rebuild")
+        return bool(f.value)
+
+    # --- S7/S8
+    def step(self, desc: md_step_desc, n_steps: int):
+        self._chk(self.L.md_step(self.h, C.byref(desc), int(n_steps)), "md_step")
+
+    def tune(self, desc: md_step_desc, full: bool = False):
+        self._chk(self.L.md_tune(self.h, C.byref(desc), int(full)), "md_tune")
+
+    def set_profiling(self, on: bool):
+        self._chk(self.L.md_set_profiling(self.h, int(on)), "md_set_profiling")
+
+    def set_launch(self, kernel, block, w):
+        self._chk(self.L.md_set_launch(self.h, kernel, block, w), "md_set_launch")
+
+    def stats(self) -> dict:
+        st = md_stats()
+        self._chk(self.L.md_get_stats(self.h, C.byref(st)), "md_get_stats")
+        d = {k: getattr(st, k) for k in ("steps", "rebuilds", "dangerous_builds", "nlist_entries", "nlist_capacity",
+                                         "device_bytes", "mean_neighbors", "max_cell_count", "tuner_runs", "launches")}
+        d["dims"] = list(st.dims)
+        d["stage_ms"] = {KERNEL_NAMES[k]: st.stage_ms[k] for k in KERNEL_NAMES}
+        d["stage_launches"] = {KERNEL_NAMES[k]: st.stage_launches[k] for k in KERNEL_NAMES}
+        d["launch"] = {KERNEL_NAMES[k]: dict(block=st.block[k], w=st.w[k], us=st.tuned_us[k]) for k in KERNEL_NAMES}
+        return d
+
+    def debug_philox(self, ctr, key):
+        ctr = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
+        key = np.ascontiguousarray(key, dtype=np.uint32).reshape(-1, 2)
+        out = np.empty_like(ctr)
+        self._chk(self.L.md_debug_philox(self.h, _ptr(ctr), _ptr(key), _ptr(out), ctr.shape[0]), "md_debug_philox")
+        return out
+
+
+def from_workload(w, precision=None, **kw) -> MD:
+    """Context for a paper_1412_3387_b200.inputs.Workload, state and bonds uploaded."""
+    if precision is None:
+        precision = MD_MIXED if w.precision == "mixed" else MD_FP64
+    md = MD(w.box, w.N, w.rc, w.r_buff, precision=precision, **kw)
+    md.set_state(w.pos, w.vel)
+    if w.bonds is not None:
+        md.set_bonds(w.bonds)
+    return md

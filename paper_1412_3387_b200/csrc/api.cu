@@ -1,0 +1,790 @@
+// api.cu -- the extern "C" boundary of libb200md (include/b200md.h): context lifetime, host/device pointer
+// marshalling, S7 step scheduler, S8 runtime tuner.  No arithmetic of the method lives here.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <algorithm>
+
+#include "md_device.cuh"
+
+// =====================================================================================================
+// memory helpers
+// =====================================================================================================
+int md_alloc(md_ctx *c, void **p, uint64_t bytes)
+{
+    *p = nullptr;
+    if (bytes == 0) bytes = 16;
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) {
+        c->err = std::string("cudaMalloc(") + std::to_string(bytes) + "): " + cudaGetErrorString(e);
+        cudaGetLastError();
+        return e == cudaErrorMemoryAllocation ? MD_ENOMEM : MD_ECUDA;
+    }
+    c->allocs.push_back({*p, bytes});
+    c->device_bytes += bytes;
+    return MD_OK;
+}
+
+void md_free(md_ctx *c, void *p)
+{
+    if (!p) return;
+    for (auto it = c->allocs.begin(); it != c->allocs.end(); ++it)
+        if (it->first == p) {
+            c->device_bytes -= it->second;
+            c->allocs.erase(it);
+            break;
+        }
+    cudaFree(p);
+}
+
+int md_sync(md_ctx *c)
+{
+    MD_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    return MD_OK;
+}
+
+int md_read_flags(md_ctx *c)
+{
+    MD_CUDA_CHECK(c, cudaMemcpyAsync(c->h_flags, c->d_flags, sizeof(DevFlags), cudaMemcpyDeviceToHost, c->stream));
+    MD_TRY(md_sync(c));
+    if (c->profiling) prof_resolve(c);
+    return MD_OK;
+}
+
+static cudaEvent_t prof_event(md_ctx *c)
+{
+    if (!c->ev_pool.empty()) { cudaEvent_t e = c->ev_pool.back(); c->ev_pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+
+ProfScope::ProfScope(md_ctx *ctx, int kernel) : c(ctx), k(kernel)
+{
+    if (!c->profiling) return;
+    e0 = prof_event(c);
+    e1 = prof_event(c);
+    cudaEventRecord(e0, c->stream);
+}
+
+ProfScope::~ProfScope()
+{
+    if (!e0) return;
+    cudaEventRecord(e1, c->stream);
+    c->ev_pending.push_back({k, e0, e1});
+}
+
+void prof_resolve(md_ctx *c)
+{
+    for (auto &p : c->ev_pending) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, p.e0, p.e1) == cudaSuccess) {
+            c->stats.stage_ms[p.k] += ms;
+            c->stats.stage_launches[p.k]++;
+        } else cudaGetLastError();
+        c->ev_pool.push_back(p.e0);
+        c->ev_pool.push_back(p.e1);
+    }
+    c->ev_pending.clear();
+}
+
+extern "C" int md_set_profiling(md_ctx *c, int on)
+{
+    if (!c) return MD_EINVAL;
+    MD_TRY(md_sync(c));
+    prof_resolve(c);
+    c->profiling = on != 0;
+    for (int k = 0; k < MD_N_KERNELS; ++k) { c->stats.stage_ms[k] = 0.0; c->stats.stage_launches[k] = 0; }
+    return MD_OK;
+}
+
+static bool is_device_ptr(const void *p)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+// bump allocator over a growable staging buffer for host-pointer arguments; reset at the start of each API call
+struct Stage {
+    md_ctx *c;
+    uint64_t used = 0;
+    explicit Stage(md_ctx *ctx) : c(ctx) {}
+    int reserve(uint64_t bytes)
+    {
+        if (bytes <= c->stage_bytes) return MD_OK;
+        MD_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+        if (c->stage) md_free(c, c->stage);
+        c->stage_bytes = bytes + (bytes >> 3) + 4096;
+        return md_alloc(c, &c->stage, c->stage_bytes);
+    }
+    void *take(uint64_t bytes)
+    {
+        void *p = (char *)c->stage + used;
+        used += (bytes + 255) & ~255ull;
+        return p;
+    }
+};
+
+static uint64_t pad256(uint64_t b) { return (b + 255) & ~255ull; }
+
+// input: returns a device pointer holding `bytes` of *src (copying if src is a host pointer)
+static int stage_in(md_ctx *c, Stage &st, const void *src, uint64_t bytes, const void **dev)
+{
+    if (!src) { *dev = nullptr; return MD_OK; }
+    if (is_device_ptr(src)) { *dev = src; return MD_OK; }
+    void *d = st.take(bytes);
+    MD_CUDA_CHECK(c, cudaMemcpyAsync(d, src, bytes, cudaMemcpyHostToDevice, c->stream));
+    *dev = d;
+    return MD_OK;
+}
+
+// output: device pointer the kernel writes to; finish_out copies back if dst is a host pointer
+struct OutBuf { void *dst; void *dev; uint64_t bytes; bool host; };
+static OutBuf stage_out(Stage &st, void *dst, uint64_t bytes)
+{
+    OutBuf o{dst, nullptr, bytes, false};
+    if (!dst) return o;
+    if (is_device_ptr(dst)) { o.dev = dst; return o; }
+    o.dev = st.take(bytes);
+    o.host = true;
+    return o;
+}
+static int finish_out(md_ctx *c, const OutBuf &o)
+{
+    if (o.dst && o.host) MD_CUDA_CHECK(c, cudaMemcpyAsync(o.dst, o.dev, o.bytes, cudaMemcpyDeviceToHost, c->stream));
+    return MD_OK;
+}
+static uint64_t stage_need(const void *p, uint64_t bytes) { return (p && !is_device_ptr(p)) ? pad256(bytes) : 0; }
+
+// =====================================================================================================
+// cell storage order (host): rank_of_lin for Morton / Hilbert curves over the cell grid
+// =====================================================================================================
+static uint64_t morton3(uint32_t x, uint32_t y, uint32_t z)
+{
+    auto spread = [](uint64_t v) {
+        v &= 0x1fffff;
+        v = (v | v << 32) & 0x1f00000000ffffull;
+        v = (v | v << 16) & 0x1f0000ff0000ffull;
+        v = (v | v << 8) & 0x100f00f00f00f00full;
+        v = (v | v << 4) & 0x10c30c30c30c30c3ull;
+        v = (v | v << 2) & 0x1249249249249249ull;
+        return v;
+    };
+    return spread(x) | spread(y) << 1 | spread(z) << 2;
+}
+
+// Hilbert index of a 3-D point with `bits` bits per axis (Skilling, "Programming the Hilbert curve", 2004:
+// axes -> transposed index, then interleave)
+static uint64_t hilbert3(uint32_t x, uint32_t y, uint32_t z, int bits)
+{
+    uint32_t X[3] = {x, y, z};
+    const uint32_t M = 1u << (bits - 1);
+    for (uint32_t Q = M; Q > 1; Q >>= 1) {
+        const uint32_t P = Q - 1;
+        for (int i = 0; i < 3; ++i) {
+            if (X[i] & Q) X[0] ^= P;
+            else { const uint32_t t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }
+        }
+    }
+    for (int i = 1; i < 3; ++i) X[i] ^= X[i - 1];
+    uint32_t t = 0;
+    for (uint32_t Q = M; Q > 1; Q >>= 1)
+        if (X[2] & Q) t ^= Q - 1;
+    for (int i = 0; i < 3; ++i) X[i] ^= t;
+    uint64_t h = 0;
+    for (int b = bits - 1; b >= 0; --b)
+        for (int i = 0; i < 3; ++i) h = (h << 1) | ((X[i] >> b) & 1u);
+    return h;
+}
+
+int build_cell_order(md_ctx *c)
+{
+    if (c->rank_of_lin) { md_free(c, c->rank_of_lin); c->rank_of_lin = nullptr; }
+    if (c->order == MD_ORDER_LEX) return MD_OK;
+    const uint32_t nx = c->dims[0], ny = c->dims[1], nz = c->dims[2];
+    int bits = 1;
+    while ((1u << bits) < std::max(nx, std::max(ny, nz))) ++bits;
+    std::vector<std::pair<uint64_t, uint32_t>> keys(c->n_cells);
+    for (uint32_t z = 0; z < nz; ++z)
+        for (uint32_t y = 0; y < ny; ++y)
+            for (uint32_t x = 0; x < nx; ++x) {
+                const uint32_t lin = x + nx * (y + ny * z);
+                keys[lin] = {c->order == MD_ORDER_MORTON ? morton3(x, y, z) : hilbert3(x, y, z, bits), lin};
+            }
+    std::sort(keys.begin(), keys.end());
+    std::vector<uint32_t> rank(c->n_cells);
+    for (uint32_t r = 0; r < c->n_cells; ++r) rank[keys[r].second] = r;
+    MD_TRY(md_alloc(c, (void **)&c->rank_of_lin, sizeof(uint32_t) * c->n_cells));
+    MD_CUDA_CHECK(c, cudaMemcpy(c->rank_of_lin, rank.data(), sizeof(uint32_t) * c->n_cells, cudaMemcpyHostToDevice));
+    return MD_OK;
+}
+
+// =====================================================================================================
+// lifetime
+// =====================================================================================================
+static void set_default_cfg(md_ctx *c)
+{
+    for (int k = 0; k < MD_N_KERNELS; ++k) c->cfg[k] = LaunchCfg{128, 1, 0.f};
+    c->cfg[MD_K_NLIST] = LaunchCfg{128, 8, 0.f};
+    c->cfg[MD_K_LJ] = LaunchCfg{128, 8, 0.f};
+    c->cfg[MD_K_DPD] = LaunchCfg{128, 4, 0.f};
+    c->cfg[MD_K_BONDS] = LaunchCfg{128, 1, 0.f};
+    c->cfg[MD_K_INTEGRATE] = LaunchCfg{256, 1, 0.f};
+    c->cfg[MD_K_CELLS] = LaunchCfg{256, 1, 0.f};
+}
+
+static thread_local std::string g_create_err;
+
+extern "C" int md_create(md_ctx **out, const double box[3], uint64_t N, double rc, double r_buff)
+{
+    if (!out) return MD_EINVAL;
+    *out = nullptr;
+    if (!box || N == 0 || N >= 0xfffffff0ull || !(rc > 0.0) || !(r_buff >= 0.0)) { g_create_err = "md_create: bad argument"; return MD_EINVAL; }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        g_create_err = "md_create: no CUDA device (this library has no CPU fallback)";
+        return MD_ECUDA;
+    }
+    md_ctx *c = new md_ctx();
+    memset(&c->stats, 0, sizeof(c->stats));
+    c->N = N;
+    c->rc = rc;
+    c->r_buff = r_buff;
+    c->r_list = rc + r_buff;
+    c->precision = MD_FP64;
+    c->order = MD_ORDER_LEX;
+    c->sched = MD_SCHED_HOST;
+    c->stream = 0;
+    c->log = getenv("B200MD_LOG") != nullptr;
+    uint64_t ncell = 1;
+    for (int a = 0; a < 3; ++a) {
+        c->box[a] = box[a];
+        double n = floor(box[a] / c->r_list);
+        if (!(box[a] > 0.0) || n < 3.0 || n > 2097151.0) {
+            g_create_err = "md_create: box too small for the 27-cell stencil (need floor(L/(rc+r_buff)) >= 3 per axis)";
+            delete c;
+            return MD_EINVAL;
+        }
+        c->dims[a] = (uint32_t)n;
+        ncell *= c->dims[a];
+        c->g.L[a] = box[a];
+        c->g.h[a] = 0.5 * box[a];
+        c->g.lo[a] = -0.5 * box[a];
+        c->g.n[a] = c->dims[a];
+        c->g.dn[a] = (double)c->dims[a];
+    }
+    if (ncell >= 0xfffffff0ull) { g_create_err = "md_create: too many cells"; delete c; return MD_EINVAL; }
+    c->n_cells = (uint32_t)ncell;
+    c->g.n_cells = c->n_cells;
+    c->g.N = (uint32_t)N;
+    set_default_cfg(c);
+
+    int s = MD_OK;
+    auto A = [&](void **p, uint64_t bytes) { if (s == MD_OK) s = md_alloc(c, p, bytes); };
+    A((void **)&c->pos, N * sizeof(double4));
+    A((void **)&c->pos_alt, N * sizeof(double4));
+    A((void **)&c->vel, N * sizeof(double4));
+    A((void **)&c->vel_alt, N * sizeof(double4));
+    A((void **)&c->force, N * sizeof(double4));
+    A((void **)&c->force_alt, N * sizeof(double4));
+    A((void **)&c->image, 3 * N * sizeof(int));
+    A((void **)&c->image_alt, 3 * N * sizeof(int));
+    A((void **)&c->pos_ref, 3 * N * sizeof(double));
+    A((void **)&c->tag, N * sizeof(uint32_t));
+    A((void **)&c->tag_alt, N * sizeof(uint32_t));
+    A((void **)&c->rtag, N * sizeof(uint32_t));
+    A((void **)&c->cell_lin, N * sizeof(uint32_t));
+    A((void **)&c->cell_rank_tmp, N * sizeof(uint32_t));
+    A((void **)&c->perm, N * sizeof(uint32_t));
+    A((void **)&c->perm_sorted, N * sizeof(uint32_t));
+    A((void **)&c->cell_count, (uint64_t)c->n_cells * sizeof(uint32_t));
+    A((void **)&c->cell_start, ((uint64_t)c->n_cells + 1) * sizeof(uint32_t));
+    A((void **)&c->nl_cnt, N * sizeof(uint32_t));
+    A((void **)&c->nl_off, (N + 1) * sizeof(uint64_t));
+    A((void **)&c->d_flags, sizeof(DevFlags));
+    if (s == MD_OK && cudaMallocHost((void **)&c->h_flags, sizeof(DevFlags)) != cudaSuccess) { c->err = "cudaMallocHost failed"; s = MD_ENOMEM; }
+    if (s == MD_OK && cudaMemset(c->d_flags, 0, sizeof(DevFlags)) != cudaSuccess) s = MD_ECUDA;
+    if (s == MD_OK && cudaMemset(c->force, 0, N * sizeof(double4)) != cudaSuccess) s = MD_ECUDA;
+    if (s != MD_OK) {
+        g_create_err = c->err;
+        md_destroy(c);
+        return s;
+    }
+    *out = c;
+    return MD_OK;
+}
+
+extern "C" int md_configure(md_ctx *c, int precision, void *stream, int order, int sched)
+{
+    if (!c) return MD_EINVAL;
+    if ((precision != MD_FP64 && precision != MD_MIXED) || order < 0 || order > MD_ORDER_HILBERT ||
+        (sched != MD_SCHED_HOST && sched != MD_SCHED_GRAPH)) {
+        c->err = "md_configure: bad argument";
+        return MD_EINVAL;
+    }
+    c->precision = precision;
+    c->stream = (cudaStream_t)stream;
+    c->sched = sched;
+    if (order != c->order || (order != MD_ORDER_LEX && !c->rank_of_lin)) {
+        c->order = order;
+        MD_TRY(build_cell_order(c));
+        c->cells_valid = c->nlist_valid = false;
+    }
+    return MD_OK;
+}
+
+extern "C" int md_destroy(md_ctx *c)
+{
+    if (!c) return MD_EINVAL;
+    cudaStreamSynchronize(c->stream);
+    prof_resolve(c);
+    for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+    for (auto &p : c->allocs) cudaFree(p.first);
+    if (c->h_flags) cudaFreeHost(c->h_flags);
+    cudaGetLastError();
+    delete c;
+    return MD_OK;
+}
+
+extern "C" const char *md_last_error(md_ctx *c) { return c ? c->err.c_str() : g_create_err.c_str(); }
+
+// =====================================================================================================
+// state
+// =====================================================================================================
+extern "C" int md_set_state(md_ctx *c, const double *pos, const double *vel, const double *mass, uint64_t step0)
+{
+    if (!c || !pos || !vel) { if (c) c->err = "md_set_state: pos and vel are required"; return MD_EINVAL; }
+    const uint64_t b3 = 3 * c->N * sizeof(double), b1 = c->N * sizeof(double);
+    Stage st(c);
+    MD_TRY(st.reserve(stage_need(pos, b3) + stage_need(vel, b3) + stage_need(mass, b1)));
+    const void *dp, *dv, *dm;
+    MD_TRY(stage_in(c, st, pos, b3, &dp));
+    MD_TRY(stage_in(c, st, vel, b3, &dv));
+    MD_TRY(stage_in(c, st, mass, b1, &dm));
+    MD_TRY(launch_pack_state(c, (const double *)dp, (const double *)dv, (const double *)dm));
+    MD_CUDA_CHECK(c, cudaMemsetAsync(c->force, 0, c->N * sizeof(double4), c->stream));
+    MD_CUDA_CHECK(c, cudaMemsetAsync(c->d_flags, 0, sizeof(DevFlags), c->stream));
+    c->have_state = true;
+    c->cells_valid = c->nlist_valid = c->force_valid = false;
+    c->step = step0;
+    return MD_OK;
+}
+
+extern "C" int md_set_bonds(md_ctx *c, const uint32_t *ta, const uint32_t *tb, uint64_t nb)
+{
+    if (!c) return MD_EINVAL;
+    if (nb > 0 && (!ta || !tb)) { c->err = "md_set_bonds: null tag array"; return MD_EINVAL; }
+    if (nb >= 0x7fffffffull) { c->err = "md_set_bonds: too many bonds"; return MD_EINVAL; }
+    MD_TRY(md_sync(c));
+    if (c->bond_off) { md_free(c, c->bond_off); c->bond_off = nullptr; }
+    if (c->bond_partner) { md_free(c, c->bond_partner); c->bond_partner = nullptr; }
+    c->n_bonds = nb;
+    if (nb == 0) return MD_OK;
+    MD_TRY(md_alloc(c, (void **)&c->bond_off, (c->N + 1) * sizeof(uint32_t)));
+    MD_TRY(md_alloc(c, (void **)&c->bond_partner, 2 * nb * sizeof(uint32_t)));
+    Stage st(c);
+    const uint64_t bb = nb * sizeof(uint32_t);
+    MD_TRY(st.reserve(stage_need(ta, bb) + stage_need(tb, bb)));
+    const void *da, *db;
+    MD_TRY(stage_in(c, st, ta, bb, &da));
+    MD_TRY(stage_in(c, st, tb, bb, &db));
+    // validate on the host side when the caller gave host pointers (cheap); device pointers are trusted
+    if (!is_device_ptr(ta))
+        for (uint64_t m = 0; m < nb; ++m)
+            if (ta[m] >= c->N || tb[m] >= c->N || ta[m] == tb[m]) { c->err = "md_set_bonds: tag out of range or self bond"; c->n_bonds = 0; return MD_EINVAL; }
+    MD_TRY(launch_bonds_build(c, (const uint32_t *)da, (const uint32_t *)db, nb));
+    return md_sync(c);
+}
+
+extern "C" int md_get_state(md_ctx *c, double *pos, double *vel, int32_t *image)
+{
+    if (!c) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_get_state: no state"; return MD_ESTATE; }
+    const uint64_t b3 = 3 * c->N * sizeof(double), bi = 3 * c->N * sizeof(int32_t);
+    Stage st(c);
+    MD_TRY(st.reserve(stage_need(pos, b3) + stage_need(vel, b3) + stage_need(image, bi)));
+    OutBuf op = stage_out(st, pos, b3), ov = stage_out(st, vel, b3), oi = stage_out(st, image, bi);
+    MD_TRY(launch_unpack_state(c, (double *)op.dev, (double *)ov.dev, (int32_t *)oi.dev));
+    MD_TRY(finish_out(c, op));
+    MD_TRY(finish_out(c, ov));
+    MD_TRY(finish_out(c, oi));
+    if (op.host || ov.host || oi.host) MD_TRY(md_sync(c));
+    return MD_OK;
+}
+
+extern "C" int md_get_forces(md_ctx *c, double *force, double *energy)
+{
+    if (!c) return MD_EINVAL;
+    if (!c->force_valid) { c->err = "md_get_forces: no force has been computed for the current positions"; return MD_ESTATE; }
+    const uint64_t b3 = 3 * c->N * sizeof(double), b1 = c->N * sizeof(double);
+    Stage st(c);
+    MD_TRY(st.reserve(stage_need(force, b3) + stage_need(energy, b1)));
+    OutBuf of = stage_out(st, force, b3), oe = stage_out(st, energy, b1);
+    MD_TRY(launch_unpack_forces(c, (double *)of.dev, (double *)oe.dev));
+    MD_TRY(finish_out(c, of));
+    MD_TRY(finish_out(c, oe));
+    if (of.host || oe.host) MD_TRY(md_sync(c));
+    return MD_OK;
+}
+
+// =====================================================================================================
+// S1 / S2
+// =====================================================================================================
+static int do_build_cells(md_ctx *c)
+{
+    ProfScope ps(c, MD_K_CELLS);
+    MD_TRY(launch_build_cells(c));
+    c->cells_valid = true;
+    c->nlist_valid = false;
+    MD_CUDA_CHECK(c, cudaMemsetAsync(&c->d_flags->rebuild, 0, 2 * sizeof(int), c->stream));
+    return MD_OK;
+}
+
+extern "C" int md_build_cells(md_ctx *c)
+{
+    if (!c) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_build_cells: md_set_state first"; return MD_ESTATE; }
+    return do_build_cells(c);
+}
+
+extern "C" int md_get_cells(md_ctx *c, uint32_t *cell_of, uint32_t dims[3])
+{
+    if (!c) return MD_EINVAL;
+    if (dims) for (int a = 0; a < 3; ++a) dims[a] = c->dims[a];
+    if (!cell_of) return MD_OK;
+    if (!c->cells_valid) { c->err = "md_get_cells: md_build_cells first"; return MD_ESTATE; }
+    const uint64_t b = c->N * sizeof(uint32_t);
+    Stage st(c);
+    MD_TRY(st.reserve(stage_need(cell_of, b)));
+    OutBuf o = stage_out(st, cell_of, b);
+    MD_TRY(launch_unpack_cells(c, (uint32_t *)o.dev));
+    MD_TRY(finish_out(c, o));
+    if (o.host) MD_TRY(md_sync(c));
+    return MD_OK;
+}
+
+static int do_build_nlist(md_ctx *c)
+{
+    ProfScope ps(c, MD_K_NLIST);
+    MD_TRY(launch_nlist_count(c));
+    MD_TRY(launch_exclusive_scan_u32(c, c->nl_cnt, c->N, nullptr, c->nl_off, true, &c->d_flags->nl_total));
+    MD_TRY(md_read_flags(c));
+    const uint64_t total = c->h_flags->nl_total;
+    if (total > c->nl_capacity) {
+        if (c->nl_idx) { md_free(c, c->nl_idx); c->nl_idx = nullptr; }
+        const uint64_t cap = total + total / 8 + 1024;
+        c->nl_capacity = 0;
+        MD_TRY(md_alloc(c, (void **)&c->nl_idx, cap * sizeof(uint32_t)));
+        c->nl_capacity = cap;
+    }
+    c->nl_entries = total;
+    MD_TRY(launch_nlist_fill(c));
+    c->nlist_valid = true;
+    c->stats.rebuilds++;
+    c->stats.max_cell_count = c->h_flags->max_cell_count;
+    return MD_OK;
+}
+
+extern "C" int md_build_nlist(md_ctx *c)
+{
+    if (!c) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_build_nlist: md_set_state first"; return MD_ESTATE; }
+    if (!c->cells_valid) MD_TRY(do_build_cells(c));
+    return do_build_nlist(c);
+}
+
+extern "C" int md_get_nlist(md_ctx *c, uint64_t *n_pairs, uint32_t *pairs, uint64_t cap)
+{
+    if (!c || !n_pairs) return MD_EINVAL;
+    if (!c->nlist_valid) { c->err = "md_get_nlist: md_build_nlist first"; return MD_ESTATE; }
+    uint32_t *cnt = nullptr;
+    uint64_t *off = nullptr;
+    MD_TRY(md_alloc(c, (void **)&cnt, c->N * sizeof(uint32_t)));
+    MD_TRY(md_alloc(c, (void **)&off, (c->N + 1) * sizeof(uint64_t)));
+    int s = launch_export_pairs_count(c, cnt);
+    if (s == MD_OK) s = launch_exclusive_scan_u32(c, cnt, c->N, nullptr, off, false, &c->d_flags->nl_total);
+    if (s == MD_OK) s = md_read_flags(c);
+    const uint64_t total = c->h_flags->nl_total;
+    if (s == MD_OK) *n_pairs = total;
+    if (s == MD_OK && pairs) {
+        if (cap < total) { c->err = "md_get_nlist: cap too small"; s = MD_EINVAL; }
+        else {
+            const uint64_t b = 2 * total * sizeof(uint32_t);
+            Stage st(c);
+            s = st.reserve(stage_need(pairs, b));
+            if (s == MD_OK) {
+                OutBuf o = stage_out(st, pairs, b);
+                s = launch_export_pairs_fill(c, off, (uint32_t *)o.dev);
+                if (s == MD_OK) s = finish_out(c, o);
+            }
+        }
+    }
+    if (s == MD_OK) s = md_sync(c); else cudaStreamSynchronize(c->stream);
+    md_free(c, cnt);
+    md_free(c, off);
+    return s;
+}
+
+extern "C" int md_get_nlist_rows(md_ctx *c, const uint32_t *probe_tags, uint32_t n_probe, uint32_t *counts,
+                                 uint32_t *nbr_tags, uint32_t row_stride)
+{
+    if (!c || !probe_tags || !counts || (!nbr_tags && row_stride)) return MD_EINVAL;
+    if (!c->nlist_valid) { c->err = "md_get_nlist_rows: md_build_nlist first"; return MD_ESTATE; }
+    const uint64_t bp = (uint64_t)n_probe * sizeof(uint32_t), bn = (uint64_t)n_probe * row_stride * sizeof(uint32_t);
+    Stage st(c);
+    MD_TRY(st.reserve(stage_need(probe_tags, bp) + stage_need(counts, bp) + stage_need(nbr_tags, bn)));
+    const void *dp;
+    MD_TRY(stage_in(c, st, probe_tags, bp, &dp));
+    OutBuf oc = stage_out(st, counts, bp), on = stage_out(st, nbr_tags, bn);
+    if (on.dev) MD_CUDA_CHECK(c, cudaMemsetAsync(on.dev, 0xff, bn, c->stream));
+    MD_TRY(launch_export_rows(c, (const uint32_t *)dp, n_probe, (uint32_t *)oc.dev, (uint32_t *)on.dev, row_stride));
+    MD_TRY(finish_out(c, oc));
+    MD_TRY(finish_out(c, on));
+    if (oc.host || on.host) MD_TRY(md_sync(c));
+    return MD_OK;
+}
+
+// =====================================================================================================
+// S4 / S5 / S6 single calls
+// =====================================================================================================
+static int need_nlist(md_ctx *c, const char *who)
+{
+    if (!c->nlist_valid) { c->err = std::string(who) + ": no valid neighbour list (md_build_nlist first)"; return MD_ESTATE; }
+    return MD_OK;
+}
+
+extern "C" int md_forces_lj(md_ctx *c, double eps, double sigma, int shift)
+{
+    if (!c) return MD_EINVAL;
+    MD_TRY(need_nlist(c, "md_forces_lj"));
+    ProfScope ps(c, MD_K_LJ);
+    MD_TRY(launch_forces_lj(c, eps, sigma, shift));
+    c->force_valid = true;
+    return MD_OK;
+}
+
+extern "C" int md_forces_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed)
+{
+    if (!c) return MD_EINVAL;
+    if (!(dt > 0.0)) { c->err = "md_forces_dpd: dt must be positive"; return MD_EINVAL; }
+    MD_TRY(need_nlist(c, "md_forces_dpd"));
+    ProfScope ps(c, MD_K_DPD);
+    MD_TRY(launch_forces_dpd(c, A, gamma, kT, dt, step, seed));
+    c->force_valid = true;
+    return MD_OK;
+}
+
+extern "C" int md_forces_bonds(md_ctx *c, double k, double r0)
+{
+    if (!c) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_forces_bonds: md_set_state first"; return MD_ESTATE; }
+    if (c->n_bonds == 0) { c->force_valid = true; return MD_OK; }
+    ProfScope ps(c, MD_K_BONDS);
+    MD_TRY(launch_forces_bonds(c, k, r0));
+    c->force_valid = true;
+    return MD_OK;
+}
+
+extern "C" int md_integrate_nve(md_ctx *c, double dt, int half)
+{
+    if (!c) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_integrate_nve: md_set_state first"; return MD_ESTATE; }
+    if (half == 1) {
+        if (!c->cells_valid) MD_TRY(do_build_cells(c));  // the displacement check needs the reference snapshot
+        ProfScope ps(c, MD_K_INTEGRATE);
+        MD_TRY(launch_half1(c, dt));
+        c->force_valid = false;
+        return MD_OK;
+    }
+    if (half == 2) { ProfScope ps(c, MD_K_INTEGRATE); return launch_half2(c, dt); }
+    c->err = "md_integrate_nve: half must be 1 or 2";
+    return MD_EINVAL;
+}
+
+extern "C" int md_needs_rebuild(md_ctx *c, int *flag)
+{
+    if (!c || !flag) return MD_EINVAL;
+    MD_TRY(md_read_flags(c));
+    *flag = c->h_flags->rebuild;
+    return MD_OK;
+}
+
+// =====================================================================================================
+// S7 step scheduler
+// =====================================================================================================
+static int eval_forces(md_ctx *c, const md_step_desc *w, uint64_t step)
+{
+    bool any = false;
+    if (w->flags & MD_F_LJ) {
+        ProfScope ps(c, MD_K_LJ);
+        MD_TRY(launch_forces_lj(c, w->lj_epsilon, w->lj_sigma, w->lj_energy_shift));
+        any = true;
+    }
+    if (w->flags & MD_F_DPD) {
+        if (any) { c->err = "md_step: LJ and DPD pair terms are mutually exclusive (each overwrites the force)"; return MD_EINVAL; }
+        ProfScope ps(c, MD_K_DPD);
+        MD_TRY(launch_forces_dpd(c, w->dpd_A, w->dpd_gamma, w->dpd_kT, w->dt, step, w->dpd_seed));
+        any = true;
+    }
+    if (!any) MD_CUDA_CHECK(c, cudaMemsetAsync(c->force, 0, c->N * sizeof(double4), c->stream));
+    if ((w->flags & MD_F_BONDS) && c->n_bonds) {
+        ProfScope ps(c, MD_K_BONDS);
+        MD_TRY(launch_forces_bonds(c, w->bond_k, w->bond_r0));
+    }
+    c->force_valid = true;
+    return MD_OK;
+}
+
+static int rebuild(md_ctx *c)
+{
+    MD_TRY(do_build_cells(c));
+    return do_build_nlist(c);
+}
+
+extern "C" int md_step(md_ctx *c, const md_step_desc *w, uint64_t n_steps)
+{
+    if (!c || !w) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_step: md_set_state first"; return MD_ESTATE; }
+    if (!(w->dt > 0.0)) { c->err = "md_step: dt must be positive"; return MD_EINVAL; }
+    if (!c->nlist_valid) MD_TRY(rebuild(c));
+    if (!c->force_valid) MD_TRY(eval_forces(c, w, c->step));  // R16: F(t0) before the first half-kick
+    for (uint64_t s = 0; s < n_steps; ++s) {
+        {
+            ProfScope ps(c, MD_K_INTEGRATE);
+            MD_TRY(launch_half1(c, w->dt));
+        }
+        MD_TRY(md_read_flags(c));
+        if (c->h_flags->rebuild) {
+            if (c->h_flags->dangerous) c->stats.dangerous_builds++;
+            MD_TRY(rebuild(c));
+        }
+        MD_TRY(eval_forces(c, w, c->step + 1));  // R15: hash counter = index of the step being completed
+        {
+            ProfScope ps(c, MD_K_INTEGRATE);
+            MD_TRY(launch_half2(c, w->dt));
+        }
+        c->step++;
+        c->stats.steps++;
+    }
+    return MD_OK;
+}
+
+// =====================================================================================================
+// S8 runtime tuner: sweep block size x w, median of 5 timed launches, keep the fastest
+// =====================================================================================================
+template <typename F>
+static int time_median5(md_ctx *c, F &&fn, float *us)
+{
+    cudaEvent_t e0, e1;
+    MD_CUDA_CHECK(c, cudaEventCreate(&e0));
+    MD_CUDA_CHECK(c, cudaEventCreate(&e1));
+    float t[5];
+    int s = fn();  // warm-up (also absorbs first-launch module load)
+    for (int r = 0; r < 5 && s == MD_OK; ++r) {
+        cudaEventRecord(e0, c->stream);
+        s = fn();
+        cudaEventRecord(e1, c->stream);
+        cudaEventSynchronize(e1);
+        cudaEventElapsedTime(&t[r], e0, e1);
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (s != MD_OK) return s;
+    std::sort(t, t + 5);
+    *us = t[2] * 1000.f;
+    return MD_OK;
+}
+
+template <typename F>
+static int tune_kernel(md_ctx *c, int kernel, const char *name, bool sweep_w, int full, F &&fn)
+{
+    static const int pruned[] = {32, 64, 96, 128, 192, 256, 384, 512, 768, 1024};
+    std::vector<int> blocks;
+    if (full) for (int b = 32; b <= 1024; b += 32) blocks.push_back(b);
+    else blocks.assign(pruned, pruned + sizeof(pruned) / sizeof(int));
+    LaunchCfg best = c->cfg[kernel];
+    best.us = 1e30f;
+    for (int w = 1; w <= (sweep_w ? 32 : 1); w *= 2)
+        for (int b : blocks) {
+            c->cfg[kernel].block = b;
+            c->cfg[kernel].w = w;
+            float us;
+            MD_TRY(time_median5(c, fn, &us));
+            if (c->log) fprintf(stderr, "[b200md tuner] %-10s block=%4d w=%2d  %9.1f us\n", name, b, w, us);
+            if (us < best.us) best = LaunchCfg{b, w, us};
+        }
+    c->cfg[kernel] = best;
+    if (c->log) fprintf(stderr, "[b200md tuner] %-10s -> block=%d w=%d (%.1f us)\n", name, best.block, best.w, best.us);
+    return MD_OK;
+}
+
+extern "C" int md_tune(md_ctx *c, const md_step_desc *w, int full)
+{
+    if (!c || !w) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_tune: md_set_state first"; return MD_ESTATE; }
+    if (!c->nlist_valid) MD_TRY(rebuild(c));
+    // the kernels are pure functions of the live state, so they can be replayed without advancing the simulation
+    MD_TRY(tune_kernel(c, MD_K_NLIST, "nlist", true, full, [&]() {
+        MD_TRY(launch_nlist_count(c));
+        return launch_nlist_fill(c);
+    }));
+    if (w->flags & MD_F_LJ)
+        MD_TRY(tune_kernel(c, MD_K_LJ, "lj", true, full, [&]() { return launch_forces_lj(c, w->lj_epsilon, w->lj_sigma, w->lj_energy_shift); }));
+    if (w->flags & MD_F_DPD)
+        MD_TRY(tune_kernel(c, MD_K_DPD, "dpd", true, full, [&]() { return launch_forces_dpd(c, w->dpd_A, w->dpd_gamma, w->dpd_kT, w->dt, c->step, w->dpd_seed); }));
+    c->force_valid = false;  // the replays overwrote the force array with a partial evaluation (pair term only)
+    c->tuned = true;
+    c->stats.tuner_runs++;
+    return MD_OK;
+}
+
+extern "C" int md_set_launch(md_ctx *c, int kernel, int block, int w)
+{
+    if (!c || kernel < 0 || kernel >= MD_N_KERNELS || block < 32 || block > 1024 || (block % 32) || w < 1 || w > 32 ||
+        (w & (w - 1))) {
+        if (c) c->err = "md_set_launch: bad argument";
+        return MD_EINVAL;
+    }
+    c->cfg[kernel].block = block;
+    c->cfg[kernel].w = w;
+    c->cfg[kernel].us = 0.f;
+    return MD_OK;
+}
+
+extern "C" int md_get_stats(md_ctx *c, md_stats *out)
+{
+    if (!c || !out) return MD_EINVAL;
+    MD_TRY(md_sync(c));
+    prof_resolve(c);
+    c->stats.nlist_entries = c->nl_entries;
+    c->stats.nlist_capacity = c->nl_capacity;
+    c->stats.device_bytes = c->device_bytes;
+    c->stats.mean_neighbors = c->N ? (double)c->nl_entries / (double)c->N : 0.0;
+    for (int a = 0; a < 3; ++a) c->stats.dims[a] = c->dims[a];
+    for (int k = 0; k < MD_N_KERNELS; ++k) {
+        c->stats.block[k] = c->cfg[k].block;
+        c->stats.w[k] = c->cfg[k].w;
+        c->stats.tuned_us[k] = c->cfg[k].us;
+    }
+    *out = c->stats;
+    return MD_OK;
+}
+
+extern "C" int md_debug_philox(md_ctx *c, const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint64_t n)
+{
+    if (!c || !ctr || !key || !out) return MD_EINVAL;
+    Stage st(c);
+    MD_TRY(st.reserve(stage_need(ctr, 16 * n) + stage_need(key, 8 * n) + stage_need(out, 16 * n)));
+    const void *dc, *dk;
+    MD_TRY(stage_in(c, st, ctr, 16 * n, &dc));
+    MD_TRY(stage_in(c, st, key, 8 * n, &dk));
+    OutBuf o = stage_out(st, out, 16 * n);
+    MD_TRY(launch_debug_philox(c, (const uint32_t *)dc, (const uint32_t *)dk, (uint32_t *)o.dev, n));
+    MD_TRY(finish_out(c, o));
+    if (o.host) MD_TRY(md_sync(c));
+    return MD_OK;
+}

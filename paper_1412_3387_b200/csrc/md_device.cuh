@@ -1,0 +1,101 @@
+// md_device.cuh -- device helpers of the CUDA path (decision arithmetic, minimum image, hash, warp segments).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "md_internal.h"
+
+// ---- decision arithmetic: plain IEEE double, explicitly rounded, never contracted into FMA (R2) ----
+__device__ __forceinline__ double md_min_image(double d, double L, double h)
+{
+    if (d >= h) d = __dsub_rn(d, L);
+    else if (d < -h) d = __dadd_rn(d, L);
+    return d;
+}
+
+__device__ __forceinline__ double md_r2_exact(double dx, double dy, double dz)
+{
+    return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+}
+
+// cell coordinate along one axis (R5): f = (x - lo)/L, c = (int)(f n), clamp to [0, n-1]
+__device__ __forceinline__ uint32_t md_cell_coord(double x, double lo, double L, double dn, uint32_t n)
+{
+    double f = __ddiv_rn(__dsub_rn(x, lo), L);
+    long long k = (long long)__dmul_rn(f, dn);
+    if (k >= (long long)n) k = (long long)n - 1;
+    if (k < 0) k = 0;
+    return (uint32_t)k;
+}
+
+// ---- tag lane: pos.w carries the particle tag as raw bits --------------------------------------------------
+__device__ __forceinline__ double md_tag_to_lane(uint32_t tag) { return __longlong_as_double((long long)tag); }
+__device__ __forceinline__ uint32_t md_lane_to_tag(double w) { return (uint32_t)__double_as_longlong(w); }
+
+// ---- Philox4x32-10 (Salmon et al., SC'11), word 0 only is used by DPD (R14) -------------------------
+__device__ __forceinline__ uint4 md_philox4x32_10(uint4 c, uint2 k)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
+        c = make_uint4(hi1 ^ c.y ^ k.x, lo1, hi0 ^ c.w ^ k.y, lo0);
+        k.x += 0x9E3779B9u;
+        k.y += 0xBB67AE85u;
+    }
+    return c;
+}
+
+// theta_ij: uniform, zero mean, unit variance, symmetric in (i, j)
+__device__ __forceinline__ double md_dpd_theta(uint32_t ti, uint32_t tj, uint64_t step, uint64_t seed)
+{
+    const uint32_t lo = min(ti, tj), hi = max(ti, tj);
+    uint4 x = md_philox4x32_10(make_uint4(lo, hi, (uint32_t)step, (uint32_t)(step >> 32)),
+                               make_uint2((uint32_t)seed, (uint32_t)(seed >> 32)));
+    const double u = ((double)x.x + 0.5) * (1.0 / 4294967296.0);
+    return 1.7320508075688772 * (2.0 * u - 1.0);
+}
+
+// ---- warp segments of W cooperating threads ("w threads per particle") -----------------------
+template <int W>
+__device__ __forceinline__ unsigned md_seg_mask()
+{
+    if constexpr (W == 32) {
+        return 0xffffffffu;
+    } else {
+        const unsigned lane = threadIdx.x & 31u;
+        return ((1u << W) - 1u) << (lane & ~(unsigned)(W - 1));
+    }
+}
+
+template <int W>
+__device__ __forceinline__ double md_seg_sum(double v, unsigned mask)
+{
+#pragma unroll
+    for (int o = W / 2; o > 0; o >>= 1) v += __shfl_xor_sync(mask, v, o, W);
+    return v;
+}
+
+// dispatch a launch templated on W
+#define MD_DISPATCH_W(w, ...)            \
+    switch (w) {                          \
+    case 1: { constexpr int W_ = 1; __VA_ARGS__; } break;   \
+    case 2: { constexpr int W_ = 2; __VA_ARGS__; } break;   \
+    case 4: { constexpr int W_ = 4; __VA_ARGS__; } break;   \
+    case 8: { constexpr int W_ = 8; __VA_ARGS__; } break;   \
+    case 16: { constexpr int W_ = 16; __VA_ARGS__; } break; \
+    default: { constexpr int W_ = 32; __VA_ARGS__; } break; \
+    }
+
+#define MD_LAUNCH_CHECK(c)                                                                   \
+    do {                                                                                     \
+        cudaError_t _e = cudaGetLastError();                                                 \
+        (c)->stats.launches++;                                                               \
+        if (_e != cudaSuccess) {                                                             \
+            (c)->err = std::string("kernel launch: ") + cudaGetErrorString(_e) + " (" +      \
+                       __FILE__ + ":" + std::to_string(__LINE__) + ")";                      \
+            return MD_ECUDA;                                                                 \
+        }                                                                                    \
+    } while (0)
+
+static inline unsigned md_grid(uint64_t work_items, int block) { return (unsigned)((work_items + block - 1) / block); }

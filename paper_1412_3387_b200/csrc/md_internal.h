@@ -1,0 +1,156 @@
+// md_internal.h -- context object and internal kernel-launcher prototypes of libb200md (CUDA path).
+// Shares nothing with oracle/ (see DESIGN.md "Independence").
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <utility>
+#include <vector>
+
+#include "../../include/b200md.h"
+
+#define MD_CUDA_CHECK(ctx, expr)                                                                   \
+    do {                                                                                           \
+        cudaError_t _e = (expr);                                                                   \
+        if (_e != cudaSuccess) {                                                                   \
+            (ctx)->err = std::string(#expr) + ": " + cudaGetErrorString(_e) + " (" + __FILE__ +    \
+                         ":" + std::to_string(__LINE__) + ")";                                     \
+            return _e == cudaErrorMemoryAllocation ? MD_ENOMEM : MD_ECUDA;                         \
+        }                                                                                          \
+    } while (0)
+
+#define MD_TRY(expr)                  \
+    do {                              \
+        int _s = (expr);              \
+        if (_s != MD_OK) return _s;   \
+    } while (0)
+
+// geometry handed to kernels by value
+struct Geom {
+    double L[3];     // box edges
+    double h[3];     // L/2
+    double lo[3];    // -L/2
+    double dn[3];    // (double) cells per axis
+    uint32_t n[3];   // cells per axis
+    uint32_t n_cells;
+    uint32_t N;
+};
+
+// device-side flags / counters, mirrored to pinned host memory on demand
+struct DevFlags {
+    int rebuild;                  // displacement criterion fired (half 1)
+    int dangerous;                // some particle moved more than r_buff since the last build
+    unsigned int max_cell_count;  // most populated cell at the last binning
+    int pad;
+    unsigned long long nl_total;  // entries (padded rows) of the list being built
+};
+
+struct LaunchCfg {
+    int block;
+    int w;
+    float us;
+};
+
+struct md_ctx {
+    // problem
+    double box[3];
+    uint64_t N;
+    double rc, r_buff, r_list;
+    uint32_t dims[3];
+    uint32_t n_cells;
+    int precision, order, sched;
+    cudaStream_t stream;
+    std::string err;
+    Geom g;
+
+    // per-particle state, internal (slot) order; *_alt = reorder targets
+    double4 *pos = nullptr, *pos_alt = nullptr;      // x, y, z, tag (bits)
+    double4 *vel = nullptr, *vel_alt = nullptr;      // vx, vy, vz, mass
+    double4 *force = nullptr, *force_alt = nullptr;  // fx, fy, fz, potential energy
+    int *image = nullptr, *image_alt = nullptr;      // 3 per particle
+    double *pos_ref = nullptr;                       // 3 per particle: positions at the last binning
+    uint32_t *tag = nullptr, *tag_alt = nullptr;     // slot -> tag
+    uint32_t *rtag = nullptr;                        // tag -> slot
+    uint32_t *cell_lin = nullptr;                    // slot -> linear cell id (valid after binning)
+
+    // cell structures
+    uint32_t *rank_of_lin = nullptr;  // linear cell id -> storage rank (nullptr = identity, MD_ORDER_LEX)
+    uint32_t *cell_rank_tmp = nullptr;  // old slot -> rank (binning scratch)
+    uint32_t *cell_count = nullptr, *cell_start = nullptr;  // per rank; cell_start has n_cells+1 entries
+    uint32_t *perm = nullptr, *perm_sorted = nullptr;
+
+    // neighbour list (CSR, rows padded to multiples of 4 entries)
+    uint32_t *nl_cnt = nullptr;
+    uint64_t *nl_off = nullptr;
+    uint32_t *nl_idx = nullptr;
+    uint64_t nl_capacity = 0, nl_entries = 0, nl_real_entries = 0;
+
+    // bonds: CSR by TAG
+    uint64_t n_bonds = 0;
+    uint32_t *bond_off = nullptr;      // N+1
+    uint32_t *bond_partner = nullptr;  // 2*n_bonds partner tags
+
+    // scratch
+    uint64_t *scan_tmp = nullptr;
+    uint64_t scan_tmp_len = 0;
+    void *stage = nullptr;  // host<->device staging
+    uint64_t stage_bytes = 0;
+    DevFlags *d_flags = nullptr;
+    DevFlags *h_flags = nullptr;  // pinned
+
+    // status
+    bool have_state = false, cells_valid = false, nlist_valid = false, force_valid = false;
+    uint64_t step = 0;
+    md_stats stats;
+    LaunchCfg cfg[MD_N_KERNELS];
+    bool tuned = false;
+    uint64_t device_bytes = 0;
+    std::vector<std::pair<void *, uint64_t>> allocs;
+    bool log = false;
+
+    // per-stage event timing (md_set_profiling)
+    bool profiling = false;
+    std::vector<cudaEvent_t> ev_pool;
+    struct Pending { int k; cudaEvent_t e0, e1; };
+    std::vector<Pending> ev_pending;
+};
+
+// RAII bracket: records an event pair around a stage when profiling is on
+struct ProfScope {
+    md_ctx *c;
+    int k;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    ProfScope(md_ctx *ctx, int kernel);
+    ~ProfScope();
+};
+void prof_resolve(md_ctx *c);  // call after a stream sync: folds finished event pairs into stats
+
+// ---- helpers (api.cu) -----------------------------------------------------------------------------------
+int md_alloc(md_ctx *c, void **p, uint64_t bytes);
+void md_free(md_ctx *c, void *p);
+int md_sync(md_ctx *c);
+int md_read_flags(md_ctx *c);  // D2H of DevFlags + sync
+
+// ---- launchers (each enqueues on c->stream and returns MD_OK or an error) ------------------------------------
+int launch_exclusive_scan_u32(md_ctx *c, const uint32_t *in, uint64_t n, uint32_t *out32, uint64_t *out64,
+                              bool pad4, unsigned long long *total_out);
+int launch_pack_state(md_ctx *c, const double *pos, const double *vel, const double *mass);
+int launch_unpack_state(md_ctx *c, double *pos, double *vel, int32_t *image);
+int launch_unpack_forces(md_ctx *c, double *force, double *energy);
+int launch_unpack_cells(md_ctx *c, uint32_t *cell_of);
+int launch_build_cells(md_ctx *c);
+int launch_nlist_count(md_ctx *c);
+int launch_nlist_fill(md_ctx *c);
+int launch_forces_lj(md_ctx *c, double eps, double sigma, int shift);
+int launch_forces_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed);
+int launch_forces_bonds(md_ctx *c, double k, double r0);
+int launch_half1(md_ctx *c, double dt);
+int launch_half2(md_ctx *c, double dt);
+int launch_export_pairs_count(md_ctx *c, uint32_t *cnt);
+int launch_export_pairs_fill(md_ctx *c, const uint64_t *off, uint32_t *pairs);
+int launch_export_rows(md_ctx *c, const uint32_t *probe_tags, uint32_t n_probe, uint32_t *counts, uint32_t *nbr,
+                       uint32_t stride);
+int launch_bonds_build(md_ctx *c, const uint32_t *ta, const uint32_t *tb, uint64_t n_bonds);
+int launch_debug_philox(md_ctx *c, const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint64_t n);
+int build_cell_order(md_ctx *c);  // host: rank_of_lin table for the configured curve

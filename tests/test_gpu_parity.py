@@ -1,0 +1,372 @@
+"""GPU-vs-oracle parity through the C-ABI (python -m pytest tests -m gpu).
+
+Bars (BASELINE.json:north_star): cell ids and neighbour lists (as sorted tag pairs) bit-exact; per-particle forces
+max relative error 1e-10 (fp64) / 1e-4 (mixed), norm of DESIGN.md R11; single-step positions 1e-12 (fp64).
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1412_3387_b200 import binding as B
+from paper_1412_3387_b200 import inputs
+from gpu_util import sort_pairs, force_rel_err, min_image_diff
+
+pytestmark = pytest.mark.gpu
+
+ORDERS = [B.MD_ORDER_LEX, B.MD_ORDER_MORTON, B.MD_ORDER_HILBERT]
+
+
+def _thermalised_lj(n_cells, rc=2.5, jitter=0.08, seed=3, kT=1.0):
+    return inputs.lj_fcc(n_cells, rc=rc, r_buff=0.4, kT=kT, jitter=jitter, pos_seed=seed, vel_seed=seed + 1)
+
+
+# ---------------------------------------------------------------------------------------------------- hash
+def test_device_philox_equals_oracle_and_kat():
+    md = B.MD([9, 9, 9], 10, 1.0, 0.4)
+    rng = np.random.default_rng(0)
+    ctr = rng.integers(0, 2 ** 32, size=(4096, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2 ** 32, size=(4096, 2), dtype=np.uint64).astype(np.uint32)
+    ctr[0] = 0; key[0] = 0
+    ctr[1] = 0xFFFFFFFF; key[1] = 0xFFFFFFFF
+    ctr[2] = [0x243F6A88, 0x85A308D3, 0x13198A2E, 0x03707344]; key[2] = [0xA4093822, 0x299F31D0]
+    out = md.debug_philox(ctr, key)
+    assert [hex(x) for x in out[0]] == ["0x6627e8d5", "0xe169c58d", "0xbc57ac4c", "0x9b00dbd8"]
+    assert [hex(x) for x in out[2]] == ["0xd16cfe09", "0x94fdcceb", "0x5001e420", "0x24126ea1"]
+    ref = np.stack([oracle.philox4x32_10(c, k) for c, k in zip(ctr[:512], key[:512])])
+    assert np.array_equal(out[:512], ref)
+
+
+# ---------------------------------------------------------------------------------------------------- state
+def test_state_roundtrip_wrap_and_errors():
+    box = np.array([9.0, 10.0, 11.0])
+    pos = inputs.random_box(1000, box, 1) + np.array([9.0, -20.0, 0.0])   # outside the box: wrapped on input
+    vel = np.random.default_rng(2).standard_normal((1000, 3))
+    md = B.MD(box, 1000, 2.5, 0.4)
+    with pytest.raises(B.MDError):
+        md.build_cells()                                                  # MD_ESTATE before set_state
+    md.set_state(pos, vel)
+    for order_dependent in (False, True):
+        if order_dependent:
+            md.build_cells()                                              # internal reorder must be invisible
+        p, v, im = md.get_state()
+        assert np.array_equal(p, oracle.wrap(pos, box))
+        assert np.array_equal(v, vel) and not im.any()
+    with pytest.raises(B.MDError):
+        md.get_forces()
+    with pytest.raises(B.MDError):
+        B.MD([5.0, 5.0, 5.0], 10, 2.5, 0.4)                               # floor(5/2.9) = 1 < 3 cells
+
+
+def test_device_and_host_pointers_agree():
+    import torch
+    w = _thermalised_lj(6)
+    md = B.MD(w.box, w.N, w.rc, w.r_buff)
+    md.set_state(torch.from_numpy(w.pos).cuda(), torch.from_numpy(w.vel).cuda())
+    md.build_nlist(); md.forces_lj()
+    F_dev = torch.empty((w.N, 3), dtype=torch.float64, device="cuda")
+    md.get_forces(F_dev, None)
+    md2 = B.from_workload(w)
+    md2.build_nlist(); md2.forces_lj()
+    F_host, _ = md2.get_forces()
+    assert np.array_equal(F_dev.cpu().numpy(), F_host)
+
+
+# ---------------------------------------------------------------------------------------------------- S1 cells
+@pytest.mark.parametrize("order", ORDERS)
+@pytest.mark.parametrize("N,box,r_list", [(3000, (9.0, 9.0, 9.0), 2.9), (5000, (16.795962, 13.1, 9.0), 2.9),
+                                          (20000, (30.0, 7.0, 11.0), 1.4)])
+def test_cells_bit_exact(order, N, box, r_list):
+    box = np.array(box)
+    pos = inputs.random_box(N, box, 5)
+    md = B.MD(box, N, r_list - 0.4, 0.4, order=order)
+    md.set_state(pos, np.zeros_like(pos))
+    md.build_cells()
+    cell, dims = md.get_cells()
+    ref, rdims = oracle.cell_assign(pos, box, r_list)
+    assert np.array_equal(dims, rdims)
+    assert np.array_equal(cell, ref)
+
+
+def test_cells_exact_faces():
+    box = np.array([12.0, 12.0, 12.0])
+    faces = np.array([-6.0, -3.0, 0.0, 3.0])
+    x = np.concatenate([faces, np.nextafter(faces, -10), np.nextafter(faces, 10), [np.nextafter(6.0, 0)], faces - 1e-15])
+    g = np.stack(np.meshgrid(x, x[:5], x[-5:], indexing="ij"), -1).reshape(-1, 3)
+    g = oracle.wrap(g, box)
+    md = B.MD(box, len(g), 2.6, 0.4)
+    md.set_state(g, np.zeros_like(g)); md.build_cells()
+    cell, _ = md.get_cells()
+    assert np.array_equal(cell, oracle.cell_assign(g, box, 3.0)[0])
+
+
+def test_cells_config1():
+    w = inputs.config(1)
+    md = B.from_workload(w); md.build_cells()
+    cell, dims = md.get_cells()
+    ref, rd = oracle.cell_assign(w.pos, w.box, w.r_list)
+    assert list(dims) == [5, 5, 5] and np.array_equal(cell, ref)
+
+
+# ---------------------------------------------------------------------------------------------------- S2 nlist
+@pytest.mark.parametrize("order", ORDERS)
+@pytest.mark.parametrize("N,box,r_list,seed", [
+    (300, (9.0, 9.0, 9.0), 2.9, 1),          # 3x3x3 cells: every stencil wraps
+    (777, (4.3, 5.7, 6.7), 1.4, 2),          # orthorhombic 3x4x4, ragged N
+    (2000, (13.0, 13.0, 13.0), 3.4, 3),
+])
+def test_nlist_bit_exact_tiny_boxes(order, N, box, r_list, seed):
+    box = np.array(box)
+    pos = inputs.random_box(N, box, seed)
+    md = B.MD(box, N, r_list - 0.4, 0.4, order=order)
+    md.set_state(pos, np.zeros_like(pos))
+    md.build_nlist()
+    got = sort_pairs(md.get_nlist())
+    ref = oracle.neighbor_pairs(pos, box, r_list)
+    assert got.shape == ref.shape and np.array_equal(got, ref)
+    st = md.stats()
+    assert st["rebuilds"] == 1 and st["nlist_entries"] >= 2 * len(ref)
+
+
+@pytest.mark.parametrize("w,block", [(1, 32), (2, 64), (4, 96), (8, 128), (16, 256), (32, 1024), (32, 32)])
+def test_nlist_every_w_and_block(w, block):
+    wl = _thermalised_lj(6)                                         # N=864
+    md = B.from_workload(wl)
+    md.set_launch(B.MD_K_NLIST, block, w)
+    md.build_nlist()
+    assert np.array_equal(sort_pairs(md.get_nlist()), oracle.neighbor_pairs(wl.pos, wl.box, wl.r_list))
+
+
+def test_nlist_config1_fcc_shells_and_rows():
+    w = inputs.config(1)
+    md = B.from_workload(w); md.build_nlist()
+    got = sort_pairs(md.get_nlist())
+    assert got.shape[0] == 39 * w.N                                 # 78 neighbours each (FCC shells within 2.9)
+    assert np.array_equal(got, oracle.neighbor_pairs(w.pos, w.box, w.r_list))
+    pr = inputs.probe_tags(w.N, 97, seed=3)
+    counts, nbrs = md.get_nlist_rows(pr, row_stride=128)
+    rc, rn = oracle.probe_nlist(w.pos, w.box, w.r_list, pr, row_stride=128)
+    assert np.array_equal(counts, rc) and (counts == 78).all()
+    assert np.array_equal(np.sort(nbrs, axis=1), np.sort(rn, axis=1))
+
+
+def test_nlist_invariants_and_dense_cell():
+    # a clump of 200 particles inside one cell (cell population > 32 exercises the large-cell sort path)
+    box = np.array([9.0, 9.0, 9.0])
+    rng = np.random.default_rng(4)
+    pos = np.concatenate([inputs.random_box(500, box, 9), rng.uniform(-0.3, 0.3, size=(200, 3))])
+    md = B.MD(box, len(pos), 2.5, 0.4)
+    md.set_state(pos, np.zeros_like(pos)); md.build_nlist()
+    got = sort_pairs(md.get_nlist())
+    assert np.array_equal(got, oracle.neighbor_pairs(pos, box, 2.9))
+    assert md.stats()["max_cell_count"] >= 200
+    counts, nbrs = md.get_nlist_rows(np.arange(len(pos), dtype=np.uint32), row_stride=700)
+    deg = np.bincount(got.reshape(-1), minlength=len(pos))
+    assert np.array_equal(counts, deg)                              # double-sided: row length = degree
+    for i in (0, 13, 650):
+        row = nbrs[i, :counts[i]]
+        assert i not in row and len(np.unique(row)) == len(row)    # no self, no duplicates
+
+
+# ---------------------------------------------------------------------------------------------------- S4a LJ
+@pytest.mark.parametrize("w,block", [(1, 64), (4, 128), (8, 128), (32, 256)])
+def test_lj_forces_fp64(w, block):
+    wl = _thermalised_lj(6)                                         # N=864
+    md = B.from_workload(wl)
+    md.set_launch(B.MD_K_LJ, block, w)
+    md.build_nlist(); md.forces_lj(1.0, 1.0, 1)
+    F, E = md.get_forces()
+    Fr, Er = oracle.forces_lj(wl.pos, wl.box, wl.rc, 1.0, 1.0, 1)
+    assert force_rel_err(F, Fr) < 1e-10
+    assert np.abs(E - Er).max() < 1e-11 * np.abs(Er).max()
+    assert np.abs(F.sum(axis=0)).max() < 1e-10 * np.abs(F).sum()   # Newton's third law
+
+
+def test_lj_forces_params_and_unshifted():
+    wl = _thermalised_lj(5, rc=2.0)
+    box = wl.box * 1.2
+    md = B.MD(box, wl.N, 2.0 * 1.1, 0.4)
+    md.set_state(wl.pos * 1.2, wl.vel); md.build_nlist(); md.forces_lj(0.7, 1.1, 0)
+    F, E = md.get_forces()
+    Fr, Er = oracle.forces_lj(oracle.wrap(wl.pos * 1.2, box), box, 2.2, 0.7, 1.1, 0)
+    assert force_rel_err(F, Fr) < 1e-10 and np.abs(E - Er).max() < 1e-11 * np.abs(Er).max()
+
+
+def test_lj_forces_mixed_1e4():
+    wl = inputs.lj_fcc(7, rc=3.0, r_buff=0.4, kT=1.2, jitter=0.05, pos_seed=2, vel_seed=3)   # config-2 recipe, N=1372
+    md = B.from_workload(wl, precision=B.MD_MIXED)
+    md.build_nlist(); md.forces_lj()
+    F, E = md.get_forces()
+    Fr, Er = oracle.forces_lj(wl.pos, wl.box, 3.0)
+    err = force_rel_err(F, Fr)
+    assert err < 1e-4
+    assert err > 1e-9                                               # it really is the fp32 path
+    assert np.abs(E - Er).max() < 1e-4 * np.abs(Er).max()
+
+
+def test_lj_perfect_fcc_energy():
+    w = inputs.config(1)
+    md = B.from_workload(w); md.build_nlist(); md.forces_lj()
+    F, E = md.get_forces()
+    assert np.abs(E - (-6.332811992581)).max() < 1e-10 and np.abs(F).max() < 1e-10
+
+
+# ---------------------------------------------------------------------------------------------------- S4b DPD
+@pytest.mark.parametrize("w", [1, 4, 32])
+def test_dpd_forces(w):
+    wl = inputs.dpd_fluid(3000, pos_seed=4, vel_seed=5)             # L=10: 7^3 cells of width 1.43
+    p = wl.params
+    md = B.from_workload(wl)
+    md.set_launch(B.MD_K_DPD, 128, w)
+    md.build_nlist()
+    for step in (0, 7, 2 ** 33 + 5):
+        md.forces_dpd(p["A"], p["gamma"], p["kT"], wl.dt, step, p["seed"])
+        F, _ = md.get_forces()
+        Fr = oracle.forces_dpd(wl.pos, wl.vel, wl.box, wl.rc, p["A"], p["gamma"], p["kT"], wl.dt, step, p["seed"])
+        assert force_rel_err(F, Fr) < 1e-10
+    assert np.abs(F.sum(axis=0)).max() < 1e-10 * np.abs(F).sum()
+
+
+# ---------------------------------------------------------------------------------------------------- S5 bonds
+def test_bond_forces_accumulate():
+    wl = inputs.polymer_melt(40, chain_len=32, start_seed=6, walk_seed=7, vel_seed=8)   # N=1280, L=7.5
+    p = wl.params
+    md = B.from_workload(wl)
+    md.build_nlist()
+    md.forces_dpd(p["A"], p["gamma"], p["kT"], wl.dt, 3, p["seed"])
+    md.forces_bonds(p["bond_k"], p["bond_r0"])
+    F, E = md.get_forces()
+    Fr = oracle.forces_dpd(wl.pos, wl.vel, wl.box, wl.rc, p["A"], p["gamma"], p["kT"], wl.dt, 3, p["seed"])
+    Fb, Eb = oracle.forces_bonds(wl.pos, wl.box, wl.bonds, p["bond_k"], p["bond_r0"])
+    assert force_rel_err(F, Fr + Fb) < 1e-10
+    # bonds alone (no pair term): branched topology, several bonds per particle
+    rng = np.random.default_rng(1)
+    extra = np.stack([rng.integers(0, wl.N, 500), rng.integers(0, wl.N, 500)], 1)
+    extra = extra[extra[:, 0] != extra[:, 1]].astype(np.uint32)
+    bonds = np.concatenate([wl.bonds, extra])
+    md.set_bonds(bonds)
+    md.set_state(wl.pos, wl.vel); md.build_cells()
+    md.forces_bonds(100.0, 1.0)
+    F2, E2 = md.get_forces()
+    Fb2, Eb2 = oracle.forces_bonds(wl.pos, wl.box, bonds, 100.0, 1.0)
+    assert force_rel_err(F2, Fb2) < 1e-10 and np.abs(E2 - Eb2).max() < 1e-10 * np.abs(Eb2).max()
+
+
+# ---------------------------------------------------------------------------------------------------- S6/S3/S7
+def test_single_step_positions_1e12_and_trajectory():
+    wl = _thermalised_lj(6, kT=1.5)
+    desc = B.step_desc("lj", wl.dt, wl.params)
+    md = B.from_workload(wl)
+    sim = oracle.Sim(wl.pos, wl.vel, wl.box, wl.rc, wl.r_buff, {"lj": wl.params})
+    md.step(desc, 1); sim.run(1, wl.dt)
+    p, v, im = md.get_state()
+    assert np.abs(min_image_diff(p, sim.pos, wl.box)).max() < 1e-12
+    assert np.abs(v - sim.vel).max() < 1e-12
+    md.step(desc, 59); sim.run(59, wl.dt)
+    p, v, im = md.get_state()
+    assert np.abs(min_image_diff(p, sim.pos, wl.box)).max() < 1e-9       # chaotic growth of rounding differences
+    assert np.array_equal(im, sim.image)
+    st = md.stats()
+    assert st["steps"] == 60 and st["dangerous_builds"] == 0
+    assert st["rebuilds"] == 1 + len(sim.rebuild_steps) and len(sim.rebuild_steps) >= 2
+
+
+def test_manual_sequence_equals_md_step_and_rebuild_flag():
+    wl = _thermalised_lj(6, kT=2.0)
+    desc = B.step_desc("lj", wl.dt, wl.params)
+    a = B.from_workload(wl); b = B.from_workload(wl)
+    a.step(desc, 25)
+    b.build_nlist(); b.forces_lj()
+    sim = oracle.Sim(wl.pos, wl.vel, wl.box, wl.rc, wl.r_buff, {"lj": wl.params})
+    flagged = []
+    for s in range(25):
+        b.integrate_nve(wl.dt, 1)
+        if b.needs_rebuild():
+            flagged.append(s + 1)
+            b.build_cells(); b.build_nlist()
+        b.forces_lj()
+        b.integrate_nve(wl.dt, 2)
+    sim.run(25, wl.dt)
+    pa, va, _ = a.get_state(); pb, vb, _ = b.get_state()
+    assert np.array_equal(pa, pb) and np.array_equal(va, vb)             # same kernels, same order: bit-identical
+    assert flagged == sim.rebuild_steps
+
+
+def test_free_flight_images_and_rebuild_step():
+    box = np.array([9.0, 9.0, 9.0])
+    pos = inputs.random_box(400, box, 1)
+    vel = np.zeros_like(pos); vel[7] = [40.0, -35.0, 0.0]; vel[9] = [0.0, 0.0, 1.7]
+    md = B.MD(box, 400, 2.5, 0.4)
+    md.set_state(pos, vel)
+    desc = B.step_desc("none", 0.005, {})
+    md.step(desc, 200)
+    p, v, im = md.get_state()
+    assert np.abs((p + im * box) - (pos + 200 * 0.005 * vel)).max() < 1e-11
+    assert im[7, 0] >= 4 and im[7, 1] <= -3
+
+
+def test_dpd_and_polymer_trajectories():
+    for wl in (inputs.dpd_fluid(2000, pos_seed=4, vel_seed=5), inputs.polymer_melt(40, chain_len=32)):
+        kind = wl.kind
+        desc = B.step_desc(kind, wl.dt, wl.params)
+        md = B.from_workload(wl)
+        what = {"dpd": dict(A=wl.params["A"], gamma=wl.params["gamma"], kT=wl.params["kT"], seed=wl.params["seed"])}
+        if kind == "polymer":
+            what["bonds"] = dict(k=wl.params["bond_k"], r0=wl.params["bond_r0"])
+        sim = oracle.Sim(wl.pos, wl.vel, wl.box, wl.rc, wl.r_buff, what, bonds=wl.bonds)
+        md.step(desc, 1); sim.run(1, wl.dt)
+        p, v, _ = md.get_state()
+        assert np.abs(min_image_diff(p, sim.pos, wl.box)).max() < 1e-12
+        assert np.abs(v - sim.vel).max() < 1e-11
+        md.step(desc, 19); sim.run(19, wl.dt)
+        p, v, _ = md.get_state()
+        assert np.abs(min_image_diff(p, sim.pos, wl.box)).max() < 1e-8
+        assert md.stats()["rebuilds"] == 1 + len(sim.rebuild_steps)
+
+
+def test_step0_enters_the_hash():
+    wl = inputs.dpd_fluid(1500, pos_seed=4, vel_seed=5)
+    desc = B.step_desc("dpd", wl.dt, wl.params)
+    out = []
+    for step0 in (0, 1000):
+        md = B.MD(wl.box, wl.N, wl.rc, wl.r_buff)
+        md.set_state(wl.pos, wl.vel, None, step0)
+        md.step(desc, 3)
+        out.append(md.get_state()[0])
+    assert np.abs(out[0] - out[1]).max() > 1e-6
+    p = wl.params
+    sim = oracle.Sim(wl.pos, wl.vel, wl.box, wl.rc, wl.r_buff,
+                     {"dpd": dict(A=p["A"], gamma=p["gamma"], kT=p["kT"], seed=p["seed"])}, step0=1000)
+    sim.run(3, wl.dt)
+    assert np.abs(min_image_diff(out[1], sim.pos, wl.box)).max() < 1e-11
+
+
+def test_nve_energy_drift_gpu_config1():
+    """Config 1 (N=4000, 100 steps fp64) + drift bound over 1000 steps (R23)."""
+    w = inputs.config(1)
+    desc = B.step_desc("lj", w.dt, w.params)
+    md = B.from_workload(w)
+    md.build_nlist(); md.forces_lj()
+    def energy():
+        _, v, _ = md.get_state(); _, E = md.get_forces()
+        return 0.5 * (v * v).sum() + E.sum()
+    e0 = energy()
+    worst = 0.0
+    for _ in range(10):
+        md.step(desc, 100)
+        worst = max(worst, abs(energy() - e0) / w.N)
+    assert worst < 2e-3
+    st = md.stats()
+    assert st["dangerous_builds"] == 0 and 1000 / 25 <= st["rebuilds"] <= 1000 / 4
+
+
+def test_tuner_runs_and_keeps_results():
+    wl = _thermalised_lj(8)                                             # N=2048
+    desc = B.step_desc("lj", wl.dt, wl.params)
+    md = B.from_workload(wl)
+    md.tune(desc, False)
+    st = md.stats()
+    assert st["tuner_runs"] == 1 and st["launch"]["lj"]["us"] > 0 and st["launch"]["nlist"]["us"] > 0
+    assert st["launch"]["lj"]["w"] in (1, 2, 4, 8, 16, 32) and st["launch"]["lj"]["block"] % 32 == 0
+    md.build_nlist(); md.forces_lj()
+    F, _ = md.get_forces()
+    assert force_rel_err(F, oracle.forces_lj(wl.pos, wl.box, wl.rc)[0]) < 1e-10
