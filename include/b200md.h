@@ -51,9 +51,11 @@ typedef enum {
                        neighbour-list decisions, displacement check stay fp64 */
 
 /* internal storage order of the cells (particles are always sorted by cell, ties by tag) */
-#define MD_ORDER_LEX 0     /* x fastest, then y, then z */
-#define MD_ORDER_MORTON 1  /* Z-order curve over (cx, cy, cz) */
-#define MD_ORDER_HILBERT 2 /* 3-D Hilbert curve over (cx, cy, cz) */
+#define MD_ORDER_LEX 0     /* x fastest, then y, then z; general list kernels (32-bit indices, L1/L2 gathers) */
+#define MD_ORDER_MORTON 1  /* Z-order curve over (cx, cy, cz); enables the tile kernels: one CTA per brick of cells,
+                              stencil staged in shared memory, 16-bit list entries (the fast path, default of the
+                              Python binding); falls back to the general kernels if a tile exceeds shared memory */
+#define MD_ORDER_HILBERT 2 /* 3-D Hilbert curve over (cx, cy, cz); general list kernels */
 
 /* which terms md_step evaluates */
 #define MD_F_LJ 1u
@@ -201,6 +203,14 @@ int md_step(md_ctx *ctx, const md_step_desc *what, uint64_t n_steps);
    (the kernels are pure functions of it), median of 5 timed launches each, and fixes the fastest.  Choices are
    reported by md_get_stats and, if the environment variable B200MD_LOG is set, printed to stderr. */
 int md_tune(md_ctx *ctx, const md_step_desc *what, int full);
+
+/* Options of the tile path (MD_ORDER_MORTON).  MD_OPT_TILE_BRICK: edge of the cell brick one CTA owns, 1, 2 or 4
+   (0 = choose from the density); invalidates cells and list.  MD_OPT_ACC_BLOCK (MD_MIXED only): 1 = every pair's
+   fp32 contribution is widened and added in fp64; 8 (default) = contributions of 8 consecutive list entries are summed
+   in fp32, the block sum is widened and added in fp64 (R25). */
+#define MD_OPT_TILE_BRICK 1
+#define MD_OPT_ACC_BLOCK 2
+int md_set_option(md_ctx *ctx, int option, int64_t value);
 
 /* Fix launch parameters by hand (block multiple of 32 in [32,1024]; w power of two <= 32); kernel = MD_K_*. */
 int md_set_launch(md_ctx *ctx, int kernel, int block, int w);

@@ -18,6 +18,7 @@ MD_FP64, MD_MIXED = 0, 1
 MD_ORDER_LEX, MD_ORDER_MORTON, MD_ORDER_HILBERT = 0, 1, 2
 MD_F_LJ, MD_F_DPD, MD_F_BONDS = 1, 2, 4
 MD_SCHED_HOST, MD_SCHED_GRAPH = 0, 1
+MD_OPT_TILE_BRICK, MD_OPT_ACC_BLOCK = 1, 2
 MD_N_KERNELS = 8
 MD_K_NLIST, MD_K_LJ, MD_K_DPD, MD_K_BONDS, MD_K_INTEGRATE, MD_K_CELLS = 0, 1, 2, 3, 4, 5
 KERNEL_NAMES = {MD_K_NLIST: "nlist", MD_K_LJ: "lj", MD_K_DPD: "dpd", MD_K_BONDS: "bonds",
@@ -26,7 +27,7 @@ KERNEL_NAMES = {MD_K_NLIST: "nlist", MD_K_LJ: "lj", MD_K_DPD: "dpd", MD_K_BONDS:
 EXPORTS = ["md_create", "md_configure", "md_destroy", "md_last_error", "md_set_state", "md_set_bonds",
            "md_get_state", "md_get_forces", "md_build_cells", "md_get_cells", "md_build_nlist", "md_get_nlist",
            "md_get_nlist_rows", "md_forces_lj", "md_forces_dpd", "md_forces_bonds", "md_integrate_nve",
-           "md_needs_rebuild", "md_step", "md_tune", "md_set_launch", "md_get_stats", "md_set_profiling",
+           "md_needs_rebuild", "md_step", "md_tune", "md_set_option", "md_set_launch", "md_get_stats", "md_set_profiling",
            "md_debug_philox"]
 
 
@@ -84,6 +85,7 @@ def load():
         "md_step": [vp, C.POINTER(md_step_desc), u64],
         "md_tune": [vp, C.POINTER(md_step_desc), i32],
         "md_set_launch": [vp, i32, i32, i32],
+        "md_set_option": [vp, i32, C.c_int64],
         "md_get_stats": [vp, C.POINTER(md_stats)],
         "md_set_profiling": [vp, i32],
         "md_debug_philox": [vp, vp, vp, vp, u64],
@@ -138,7 +140,7 @@ def step_desc(kind: str, dt: float, params: dict) -> md_step_desc:
 class MD:
     """One simulation context (md_ctx).  Methods are 1:1 with the C entry points (md_ prefix dropped)."""
 
-    def __init__(self, box, N, rc, r_buff, precision=MD_FP64, stream=None, order=MD_ORDER_LEX, sched=MD_SCHED_HOST):
+    def __init__(self, box, N, rc, r_buff, precision=MD_FP64, stream=None, order=MD_ORDER_MORTON, sched=MD_SCHED_HOST):
         self.L = load()
         self.N = int(N)
         b = (C.c_double * 3)(*[float(x) for x in np.broadcast_to(np.asarray(box, dtype=np.float64), (3,))])
@@ -252,6 +254,9 @@ class MD:
 
     def set_profiling(self, on: bool):
         self._chk(self.L.md_set_profiling(self.h, int(on)), "md_set_profiling")
+
+    def set_option(self, option, value):
+        self._chk(self.L.md_set_option(self.h, int(option), int(value)), "md_set_option")
 
     def set_launch(self, kernel, block, w):
         self._chk(self.L.md_set_launch(self.h, kernel, block, w), "md_set_launch")

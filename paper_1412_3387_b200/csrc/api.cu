@@ -200,9 +200,23 @@ static uint64_t hilbert3(uint32_t x, uint32_t y, uint32_t z, int bits)
     return h;
 }
 
+static uint32_t choose_brick(md_ctx *c)
+{
+    if (c->tile_B_forced) return (uint32_t)c->tile_B_forced;
+    const double ppc = (double)c->N / (double)c->n_cells;
+    // aim at a few hundred home particles per tile, but keep at least ~2 tiles per SM
+    uint32_t B = ppc >= 48.0 ? 1u : (ppc >= 4.0 ? 2u : 4u);
+    while (B > 1 && (double)c->n_cells / (double)(B * B * B) < 300.0) B >>= 1;
+    return B;
+}
+
 int build_cell_order(md_ctx *c)
 {
-    if (c->rank_of_lin) { md_free(c, c->rank_of_lin); c->rank_of_lin = nullptr; }
+    for (uint32_t **p : {&c->rank_of_lin, &c->lin_of_rank, &c->tile_cell_begin, &c->tile_origin})
+        if (*p) { md_free(c, *p); *p = nullptr; }
+    if (c->tile_base) { md_free(c, c->tile_base); c->tile_base = nullptr; }
+    c->use_tiles = false;
+    c->n_tiles = 0;
     if (c->order == MD_ORDER_LEX) return MD_OK;
     const uint32_t nx = c->dims[0], ny = c->dims[1], nz = c->dims[2];
     int bits = 1;
@@ -215,10 +229,42 @@ int build_cell_order(md_ctx *c)
                 keys[lin] = {c->order == MD_ORDER_MORTON ? morton3(x, y, z) : hilbert3(x, y, z, bits), lin};
             }
     std::sort(keys.begin(), keys.end());
-    std::vector<uint32_t> rank(c->n_cells);
-    for (uint32_t r = 0; r < c->n_cells; ++r) rank[keys[r].second] = r;
+    std::vector<uint32_t> rank(c->n_cells), lin_of_rank(c->n_cells);
+    for (uint32_t r = 0; r < c->n_cells; ++r) { rank[keys[r].second] = r; lin_of_rank[r] = keys[r].second; }
     MD_TRY(md_alloc(c, (void **)&c->rank_of_lin, sizeof(uint32_t) * c->n_cells));
     MD_CUDA_CHECK(c, cudaMemcpy(c->rank_of_lin, rank.data(), sizeof(uint32_t) * c->n_cells, cudaMemcpyHostToDevice));
+    if (c->order != MD_ORDER_MORTON) return MD_OK;
+
+    // tiles: bricks of B^3 cells = runs of equal (Morton key >> 3 log2 B), contiguous in rank order
+    const uint32_t B = choose_brick(c);
+    int lb = 0;
+    while ((1u << lb) < B) ++lb;
+    std::vector<uint32_t> begin, origin;
+    uint64_t prev = ~0ull;
+    for (uint32_t r = 0; r < c->n_cells; ++r) {
+        const uint64_t brick = keys[r].first >> (3 * lb);
+        if (brick != prev) {
+            prev = brick;
+            begin.push_back(r);
+            const uint32_t lin = keys[r].second;
+            const uint32_t x = lin % nx, y = (lin / nx) % ny, z = lin / (nx * ny);
+            origin.push_back((x >> lb) << lb);
+            origin.push_back((y >> lb) << lb);
+            origin.push_back((z >> lb) << lb);
+        }
+    }
+    c->n_tiles = (uint32_t)begin.size();
+    begin.push_back(c->n_cells);
+    c->tile_B = B;
+    MD_TRY(md_alloc(c, (void **)&c->lin_of_rank, sizeof(uint32_t) * c->n_cells));
+    MD_TRY(md_alloc(c, (void **)&c->tile_cell_begin, sizeof(uint32_t) * begin.size()));
+    MD_TRY(md_alloc(c, (void **)&c->tile_origin, sizeof(uint32_t) * origin.size()));
+    MD_TRY(md_alloc(c, (void **)&c->tile_base, sizeof(unsigned long long) * c->n_tiles));
+    MD_CUDA_CHECK(c, cudaMemcpy(c->lin_of_rank, lin_of_rank.data(), sizeof(uint32_t) * c->n_cells, cudaMemcpyHostToDevice));
+    MD_CUDA_CHECK(c, cudaMemcpy(c->tile_cell_begin, begin.data(), sizeof(uint32_t) * begin.size(), cudaMemcpyHostToDevice));
+    MD_CUDA_CHECK(c, cudaMemcpy(c->tile_origin, origin.data(), sizeof(uint32_t) * origin.size(), cudaMemcpyHostToDevice));
+    if (!c->row_off) MD_TRY(md_alloc(c, (void **)&c->row_off, c->N * sizeof(uint32_t)));
+    c->use_tiles = true;
     return MD_OK;
 }
 
@@ -467,13 +513,8 @@ extern "C" int md_get_cells(md_ctx *c, uint32_t *cell_of, uint32_t dims[3])
     return MD_OK;
 }
 
-static int do_build_nlist(md_ctx *c)
+static int ensure_nl32(md_ctx *c, uint64_t total)
 {
-    ProfScope ps(c, MD_K_NLIST);
-    MD_TRY(launch_nlist_count(c));
-    MD_TRY(launch_exclusive_scan_u32(c, c->nl_cnt, c->N, nullptr, c->nl_off, true, &c->d_flags->nl_total));
-    MD_TRY(md_read_flags(c));
-    const uint64_t total = c->h_flags->nl_total;
     if (total > c->nl_capacity) {
         if (c->nl_idx) { md_free(c, c->nl_idx); c->nl_idx = nullptr; }
         const uint64_t cap = total + total / 8 + 1024;
@@ -481,11 +522,81 @@ static int do_build_nlist(md_ctx *c)
         MD_TRY(md_alloc(c, (void **)&c->nl_idx, cap * sizeof(uint32_t)));
         c->nl_capacity = cap;
     }
+    return MD_OK;
+}
+
+static int build_nlist_general(md_ctx *c)
+{
+    MD_TRY(launch_nlist_count(c));
+    MD_TRY(launch_exclusive_scan_u32(c, c->nl_cnt, c->N, nullptr, c->nl_off, true, &c->d_flags->nl_total));
+    MD_TRY(md_read_flags(c));
+    const uint64_t total = c->h_flags->nl_total;
+    MD_TRY(ensure_nl32(c, total));
     c->nl_entries = total;
     MD_TRY(launch_nlist_fill(c));
+    c->nl_is_tile = false;
+    return MD_OK;
+}
+
+static int build_nlist_tiles(md_ctx *c, bool *done)
+{
+    *done = false;
+    MD_TRY(tile_measure(c));
+    MD_TRY(md_read_flags(c));
+    c->tile_max_home = c->h_flags->max_home;
+    c->tile_max_staged = c->h_flags->max_staged;
+    if (c->nl16_capacity == 0) {
+        double vol = c->box[0] * c->box[1] * c->box[2];
+        double nbar = (double)c->N / vol * 4.18879020478639 * c->r_list * c->r_list * c->r_list;
+        uint64_t cap = (uint64_t)((double)c->N * (nbar + 8.0) * 1.15) + 4096;
+        MD_TRY(md_alloc(c, (void **)&c->nl16, cap * sizeof(uint16_t)));
+        c->nl16_capacity = cap;
+    }
+    for (int attempt = 0; attempt < 2; ++attempt) {
+        bool fits = false;
+        MD_TRY(launch_tile_build(c, &fits));
+        if (!fits) return MD_OK;  // largest tile exceeds shared memory: general path
+        MD_TRY(md_read_flags(c));
+        const uint64_t need = c->h_flags->cursor;
+        if (need <= c->nl16_capacity) {
+            c->nl_entries = need;
+            c->nl_is_tile = true;
+            c->nl32_decoded = false;
+            *done = true;
+            return MD_OK;
+        }
+        md_free(c, c->nl16);
+        c->nl16 = nullptr;
+        c->nl16_capacity = 0;
+        const uint64_t cap = need + need / 8 + 4096;
+        MD_TRY(md_alloc(c, (void **)&c->nl16, cap * sizeof(uint16_t)));
+        c->nl16_capacity = cap;
+    }
+    c->err = "neighbour list: capacity still too small after growing";
+    return MD_ECUDA;
+}
+
+static int do_build_nlist(md_ctx *c)
+{
+    ProfScope ps(c, MD_K_NLIST);
+    bool done = false;
+    if (c->use_tiles) MD_TRY(build_nlist_tiles(c, &done));
+    if (!done) MD_TRY(build_nlist_general(c));
     c->nlist_valid = true;
     c->stats.rebuilds++;
     c->stats.max_cell_count = c->h_flags->max_cell_count;
+    return MD_OK;
+}
+
+// exports read the general 32-bit CSR; a tile list is decoded into it on demand
+static int ensure_decoded(md_ctx *c)
+{
+    if (!c->nl_is_tile || c->nl32_decoded) return MD_OK;
+    MD_TRY(launch_exclusive_scan_u32(c, c->nl_cnt, c->N, nullptr, c->nl_off, true, &c->d_flags->nl_total));
+    MD_TRY(md_read_flags(c));
+    MD_TRY(ensure_nl32(c, c->h_flags->nl_total));
+    MD_TRY(launch_tile_decode(c));
+    c->nl32_decoded = true;
     return MD_OK;
 }
 
@@ -501,6 +612,7 @@ extern "C" int md_get_nlist(md_ctx *c, uint64_t *n_pairs, uint32_t *pairs, uint6
 {
     if (!c || !n_pairs) return MD_EINVAL;
     if (!c->nlist_valid) { c->err = "md_get_nlist: md_build_nlist first"; return MD_ESTATE; }
+    MD_TRY(ensure_decoded(c));
     uint32_t *cnt = nullptr;
     uint64_t *off = nullptr;
     MD_TRY(md_alloc(c, (void **)&cnt, c->N * sizeof(uint32_t)));
@@ -534,6 +646,7 @@ extern "C" int md_get_nlist_rows(md_ctx *c, const uint32_t *probe_tags, uint32_t
 {
     if (!c || !probe_tags || !counts || (!nbr_tags && row_stride)) return MD_EINVAL;
     if (!c->nlist_valid) { c->err = "md_get_nlist_rows: md_build_nlist first"; return MD_ESTATE; }
+    MD_TRY(ensure_decoded(c));
     const uint64_t bp = (uint64_t)n_probe * sizeof(uint32_t), bn = (uint64_t)n_probe * row_stride * sizeof(uint32_t);
     Stage st(c);
     MD_TRY(st.reserve(stage_need(probe_tags, bp) + stage_need(counts, bp) + stage_need(nbr_tags, bn)));
@@ -551,6 +664,18 @@ extern "C" int md_get_nlist_rows(md_ctx *c, const uint32_t *probe_tags, uint32_t
 // =====================================================================================================
 // S4 / S5 / S6 single calls
 // =====================================================================================================
+// pair kernels: tile path when the current list is a tile list, else the general list kernels
+static int pair_lj(md_ctx *c, double eps, double sigma, int shift)
+{
+    if (c->nl_is_tile) return launch_tile_lj(c, eps, sigma, shift);
+    return launch_forces_lj(c, eps, sigma, shift);
+}
+static int pair_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed)
+{
+    if (c->nl_is_tile) return launch_tile_dpd(c, A, gamma, kT, dt, step, seed);
+    return launch_forces_dpd(c, A, gamma, kT, dt, step, seed);
+}
+
 static int need_nlist(md_ctx *c, const char *who)
 {
     if (!c->nlist_valid) { c->err = std::string(who) + ": no valid neighbour list (md_build_nlist first)"; return MD_ESTATE; }
@@ -562,7 +687,7 @@ extern "C" int md_forces_lj(md_ctx *c, double eps, double sigma, int shift)
     if (!c) return MD_EINVAL;
     MD_TRY(need_nlist(c, "md_forces_lj"));
     ProfScope ps(c, MD_K_LJ);
-    MD_TRY(launch_forces_lj(c, eps, sigma, shift));
+    MD_TRY(pair_lj(c, eps, sigma, shift));
     c->force_valid = true;
     return MD_OK;
 }
@@ -573,7 +698,7 @@ extern "C" int md_forces_dpd(md_ctx *c, double A, double gamma, double kT, doubl
     if (!(dt > 0.0)) { c->err = "md_forces_dpd: dt must be positive"; return MD_EINVAL; }
     MD_TRY(need_nlist(c, "md_forces_dpd"));
     ProfScope ps(c, MD_K_DPD);
-    MD_TRY(launch_forces_dpd(c, A, gamma, kT, dt, step, seed));
+    MD_TRY(pair_dpd(c, A, gamma, kT, dt, step, seed));
     c->force_valid = true;
     return MD_OK;
 }
@@ -621,13 +746,13 @@ static int eval_forces(md_ctx *c, const md_step_desc *w, uint64_t step)
     bool any = false;
     if (w->flags & MD_F_LJ) {
         ProfScope ps(c, MD_K_LJ);
-        MD_TRY(launch_forces_lj(c, w->lj_epsilon, w->lj_sigma, w->lj_energy_shift));
+        MD_TRY(pair_lj(c, w->lj_epsilon, w->lj_sigma, w->lj_energy_shift));
         any = true;
     }
     if (w->flags & MD_F_DPD) {
         if (any) { c->err = "md_step: LJ and DPD pair terms are mutually exclusive (each overwrites the force)"; return MD_EINVAL; }
         ProfScope ps(c, MD_K_DPD);
-        MD_TRY(launch_forces_dpd(c, w->dpd_A, w->dpd_gamma, w->dpd_kT, w->dt, step, w->dpd_seed));
+        MD_TRY(pair_dpd(c, w->dpd_A, w->dpd_gamma, w->dpd_kT, w->dt, step, w->dpd_seed));
         any = true;
     }
     if (!any) MD_CUDA_CHECK(c, cudaMemsetAsync(c->force, 0, c->N * sizeof(double4), c->stream));
@@ -728,18 +853,48 @@ extern "C" int md_tune(md_ctx *c, const md_step_desc *w, int full)
     if (!c->have_state) { c->err = "md_tune: md_set_state first"; return MD_ESTATE; }
     if (!c->nlist_valid) MD_TRY(rebuild(c));
     // the kernels are pure functions of the live state, so they can be replayed without advancing the simulation
-    MD_TRY(tune_kernel(c, MD_K_NLIST, "nlist", true, full, [&]() {
-        MD_TRY(launch_nlist_count(c));
-        return launch_nlist_fill(c);
-    }));
+    if (c->nl_is_tile) {
+        // tile build: w is fixed at 32 (one ballot word per 32 candidates); only the block size is swept
+        MD_TRY(tune_kernel(c, MD_K_NLIST, "nlist/tile", false, full, [&]() {
+            bool fits;
+            return launch_tile_build(c, &fits);
+        }));
+        c->cfg[MD_K_NLIST].w = 32;
+    } else {
+        MD_TRY(tune_kernel(c, MD_K_NLIST, "nlist", true, full, [&]() {
+            MD_TRY(launch_nlist_count(c));
+            return launch_nlist_fill(c);
+        }));
+    }
     if (w->flags & MD_F_LJ)
-        MD_TRY(tune_kernel(c, MD_K_LJ, "lj", true, full, [&]() { return launch_forces_lj(c, w->lj_epsilon, w->lj_sigma, w->lj_energy_shift); }));
+        MD_TRY(tune_kernel(c, MD_K_LJ, c->nl_is_tile ? "lj/tile" : "lj", true, full, [&]() { return pair_lj(c, w->lj_epsilon, w->lj_sigma, w->lj_energy_shift); }));
     if (w->flags & MD_F_DPD)
-        MD_TRY(tune_kernel(c, MD_K_DPD, "dpd", true, full, [&]() { return launch_forces_dpd(c, w->dpd_A, w->dpd_gamma, w->dpd_kT, w->dt, c->step, w->dpd_seed); }));
+        MD_TRY(tune_kernel(c, MD_K_DPD, c->nl_is_tile ? "dpd/tile" : "dpd", true, full, [&]() { return pair_dpd(c, w->dpd_A, w->dpd_gamma, w->dpd_kT, w->dt, c->step, w->dpd_seed); }));
     c->force_valid = false;  // the replays overwrote the force array with a partial evaluation (pair term only)
     c->tuned = true;
     c->stats.tuner_runs++;
     return MD_OK;
+}
+
+extern "C" int md_set_option(md_ctx *c, int option, int64_t value)
+{
+    if (!c) return MD_EINVAL;
+    switch (option) {
+    case MD_OPT_TILE_BRICK:
+        if (value != 0 && value != 1 && value != 2 && value != 4) { c->err = "md_set_option: brick must be 0 (auto), 1, 2 or 4"; return MD_EINVAL; }
+        c->tile_B_forced = (int)value;
+        MD_TRY(md_sync(c));
+        MD_TRY(build_cell_order(c));
+        c->cells_valid = c->nlist_valid = false;
+        return MD_OK;
+    case MD_OPT_ACC_BLOCK:
+        if (value != 1 && value != 8) { c->err = "md_set_option: accumulation block must be 1 or 8"; return MD_EINVAL; }
+        c->acc_block = (int)value;
+        return MD_OK;
+    default:
+        c->err = "md_set_option: unknown option";
+        return MD_EINVAL;
+    }
 }
 
 extern "C" int md_set_launch(md_ctx *c, int kernel, int block, int w)

@@ -28,6 +28,15 @@ __device__ __forceinline__ uint32_t md_cell_coord(double x, double lo, double L,
     return (uint32_t)k;
 }
 
+// fast reciprocal: fp32 = MUFU.RCP (about 1 ulp), fp64 = IEEE division
+__device__ __forceinline__ float md_rcp(float x)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ double md_rcp(double x) { return 1.0 / x; }
+
 // ---- tag lane: pos.w carries the particle tag as raw bits --------------------------------------------------
 __device__ __forceinline__ double md_tag_to_lane(uint32_t tag) { return __longlong_as_double((long long)tag); }
 __device__ __forceinline__ uint32_t md_lane_to_tag(double w) { return (uint32_t)__double_as_longlong(w); }

@@ -42,8 +42,11 @@ struct DevFlags {
     int rebuild;                  // displacement criterion fired (half 1)
     int dangerous;                // some particle moved more than r_buff since the last build
     unsigned int max_cell_count;  // most populated cell at the last binning
+    unsigned int max_home;        // largest tile: home particles
+    unsigned int max_staged;      // largest tile: staged (stencil) particles
     int pad;
-    unsigned long long nl_total;  // entries (padded rows) of the list being built
+    unsigned long long nl_total;  // entries (padded rows) of the list being built (general path)
+    unsigned long long cursor;    // entries reserved by the tile build (may exceed the capacity: grow + rebuild)
 };
 
 struct LaunchCfg {
@@ -85,6 +88,19 @@ struct md_ctx {
     uint64_t *nl_off = nullptr;
     uint32_t *nl_idx = nullptr;
     uint64_t nl_capacity = 0, nl_entries = 0, nl_real_entries = 0;
+
+    // tile path (tiles.cu): bricks of tile_B^3 cells, Morton cell order, 16-bit staged indices
+    bool use_tiles = false;     // configured (MD_ORDER_MORTON)
+    bool nl_is_tile = false;    // the current list is a tile list
+    bool nl32_decoded = false;  // nl_off/nl_idx hold the decoded copy of the current tile list (exports)
+    uint32_t tile_B = 1, n_tiles = 0;
+    int tile_B_forced = 0, acc_block = 8;
+    uint32_t *tile_cell_begin = nullptr, *tile_origin = nullptr, *lin_of_rank = nullptr;
+    uint32_t tile_max_home = 0, tile_max_staged = 0;
+    uint16_t *nl16 = nullptr;
+    uint64_t nl16_capacity = 0;
+    unsigned long long *tile_base = nullptr;
+    uint32_t *row_off = nullptr;
 
     // bonds: CSR by TAG
     uint64_t n_bonds = 0;
@@ -153,4 +169,11 @@ int launch_export_rows(md_ctx *c, const uint32_t *probe_tags, uint32_t n_probe, 
                        uint32_t stride);
 int launch_bonds_build(md_ctx *c, const uint32_t *ta, const uint32_t *tb, uint64_t n_bonds);
 int launch_debug_philox(md_ctx *c, const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint64_t n);
-int build_cell_order(md_ctx *c);  // host: rank_of_lin table for the configured curve
+int build_cell_order(md_ctx *c);  // host: rank_of_lin table for the configured curve (+ tile tables for Morton)
+// tiles.cu
+int tile_measure(md_ctx *c);
+int launch_tile_build(md_ctx *c, bool *fits);
+int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift);
+int launch_tile_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed);
+bool tile_forces_fit(md_ctx *c, bool dpd);
+int launch_tile_decode(md_ctx *c);

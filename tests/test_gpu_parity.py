@@ -370,3 +370,100 @@ def test_tuner_runs_and_keeps_results():
     md.build_nlist(); md.forces_lj()
     F, _ = md.get_forces()
     assert force_rel_err(F, oracle.forces_lj(wl.pos, wl.box, wl.rc)[0]) < 1e-10
+
+
+# ---------------------------------------------------------------------------------------------------- tile path
+@pytest.mark.parametrize("brick", [1, 2, 4])
+def test_tile_bricks_lists_and_forces(brick):
+    """MD_ORDER_MORTON tile kernels (staged stencil, 16-bit entries) for every brick size, odd and small grids."""
+    # LJ, 5x5x5 cells (odd: partial bricks), fp64 and mixed
+    wl = inputs.lj_fcc(9, rc=2.5, r_buff=0.4, kT=1.0, jitter=0.08, pos_seed=5, vel_seed=6)     # N=2916, L=15.1
+    ref_pairs = oracle.neighbor_pairs(wl.pos, wl.box, wl.r_list)
+    Fr, Er = oracle.forces_lj(wl.pos, wl.box, wl.rc)
+    for prec, tol in ((B.MD_FP64, 1e-10), (B.MD_MIXED, 1e-4)):
+        md = B.from_workload(wl, precision=prec)
+        md.set_option(B.MD_OPT_TILE_BRICK, brick)
+        md.set_state(wl.pos, wl.vel)
+        md.build_nlist()
+        assert np.array_equal(sort_pairs(md.get_nlist()), ref_pairs)
+        md.forces_lj()
+        F, E = md.get_forces()
+        assert force_rel_err(F, Fr) < tol
+        assert np.abs(E - Er).max() < tol * 10 * np.abs(Er).max()
+    # DPD, 7x7x7 cells
+    wd = inputs.dpd_fluid(3000, pos_seed=4, vel_seed=5)
+    p = wd.params
+    md = B.from_workload(wd)
+    md.set_option(B.MD_OPT_TILE_BRICK, brick)
+    md.set_state(wd.pos, wd.vel)
+    md.build_nlist()
+    assert np.array_equal(sort_pairs(md.get_nlist()), oracle.neighbor_pairs(wd.pos, wd.box, wd.r_list))
+    md.forces_dpd(p["A"], p["gamma"], p["kT"], wd.dt, 11, p["seed"])
+    F, _ = md.get_forces()
+    Fd = oracle.forces_dpd(wd.pos, wd.vel, wd.box, wd.rc, p["A"], p["gamma"], p["kT"], wd.dt, 11, p["seed"])
+    assert force_rel_err(F, Fd) < 1e-10
+
+
+def test_tile_3x3x3_grid_every_image():
+    """Smallest legal grid: the (B+2)^3 stencil of a brick wraps onto itself, every staged cell is an image."""
+    box = np.array([9.0, 9.3, 10.0])
+    pos = inputs.random_box(900, box, 12)
+    for brick in (1, 2):
+        for prec in (B.MD_FP64, B.MD_MIXED):
+            md = B.MD(box, 900, 2.5, 0.4, precision=prec)
+            md.set_option(B.MD_OPT_TILE_BRICK, brick)
+            md.set_state(pos, np.zeros_like(pos)); md.build_nlist()
+            assert np.array_equal(sort_pairs(md.get_nlist()), oracle.neighbor_pairs(pos, box, 2.9))
+            md.forces_lj()
+            F, _ = md.get_forces()
+            assert force_rel_err(F, oracle.forces_lj(pos, box, 2.5)[0]) < (1e-10 if prec == B.MD_FP64 else 1e-4)
+
+
+def test_mixed_accumulation_blocks_agree():
+    wl = inputs.lj_fcc(7, rc=3.0, r_buff=0.4, kT=1.2, jitter=0.05, pos_seed=2, vel_seed=3)
+    Fr, _ = oracle.forces_lj(wl.pos, wl.box, 3.0)
+    errs = []
+    for blk in (1, 8):
+        md = B.from_workload(wl, precision=B.MD_MIXED)
+        md.set_option(B.MD_OPT_ACC_BLOCK, blk)
+        md.build_nlist(); md.forces_lj()
+        errs.append(force_rel_err(md.get_forces()[0], Fr))
+    assert max(errs) < 1e-4
+
+
+def test_tile_guard_band_pairs_at_the_cutoff():
+    """Pairs placed within 1e-7 of r_list and of rc (inside the fp32 guard band) take the exact fp64 decision."""
+    wl = inputs.lj_fcc(8, rc=2.5, r_buff=0.4)                                # perfect FCC, N=2048, L=13.4
+    pos, box = wl.pos.copy(), wl.box
+    rng = np.random.default_rng(3)
+    used = np.zeros(wl.N, dtype=bool)
+    n_made = 0
+    for i in rng.permutation(wl.N):
+        if used[i]:
+            continue
+        d = pos - pos[i]
+        d -= box * np.rint(d / box)
+        r = np.sqrt((d * d).sum(1))
+        target = 2.5 if n_made % 2 else 2.9
+        cand = np.nonzero((np.abs(r - target) < 0.2) & ~used)[0]             # FCC shells at 2.375, 2.656, 2.909
+        if len(cand) == 0:
+            continue
+        j = cand[0]
+        # neighbours of i and j must stay put, or earlier pairs would move
+        used[np.nonzero(r < 3.2)[0]] = True
+        dj = pos - pos[j]; dj -= box * np.rint(dj / box)
+        used[np.nonzero(np.sqrt((dj * dj).sum(1)) < 3.2)[0]] = True
+        pos[j] = pos[i] + d[j] / r[j] * (target + rng.uniform(-1e-7, 1e-7))
+        n_made += 1
+    assert n_made >= 20
+    pos = oracle.wrap(pos, box)
+    ref_pairs = oracle.neighbor_pairs(pos, box, 2.9)
+    Fr = oracle.forces_lj(pos, box, 2.5)[0]
+    for prec in (B.MD_FP64, B.MD_MIXED):
+        md = B.MD(box, len(pos), 2.5, 0.4, precision=prec)
+        md.set_state(pos, np.zeros_like(pos)); md.build_nlist()
+        assert np.array_equal(sort_pairs(md.get_nlist()), ref_pairs)
+        md.forces_lj()
+        F, _ = md.get_forces()
+        # a wrongly included / excluded pair at rc changes a force by |F(rc)| = 0.039: far above either tolerance
+        assert np.abs(F - Fr).max() < 2e-3
