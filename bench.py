@@ -307,7 +307,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--scale", type=float, default=1.0)
-    ap.add_argument("--order", default="lex", choices=["lex", "morton", "hilbert"])
+    ap.add_argument("--order", default="morton", choices=["lex", "morton", "hilbert"])
     ap.add_argument("--no-tune", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -169,7 +169,7 @@ int md_get_nlist_rows(md_ctx *ctx, const uint32_t *probe_tags, uint32_t n_probe,
    force/energy arrays.  Needs a valid neighbour list (MD_ESTATE otherwise). */
 int md_forces_lj(md_ctx *ctx, double epsilon, double sigma, int energy_shift);
 
-/* DPD (Groot-Warren form, R5): for 0 < r < rc, w = 1 - r/rc,
+/* DPD (Groot-Warren form, R9): for 0 < r < rc, w = 1 - r/rc,
    F_ij = [A w - gamma w^2 (rhat . v_ij) + sqrt(2 gamma kT) w theta_ij / sqrt(dt)] rhat,
    theta_ij = sqrt(3) (2u - 1), u = (X + 1/2) 2^-32, X = word 0 of Philox4x32-10 with
    counter (min tag, max tag, step lo, step hi) and key (seed lo, seed hi) (R13, R14).

@@ -15,7 +15,7 @@
  *
  * The paper prints no formula for LJ, DPD, harmonic bonds or velocity-Verlet (it names them,
  * PAPER.md:63, and cites refs [1], [41], [42]); the forms below are the textbook definitions as read
- * in DESIGN.md "Readings" (R1..R20), each function says which.
+ * in DESIGN.md "Readings" (R1..R27), each function says which.
  *
  * Pins (tests/test_oracle_*.py, all run without a GPU):
  *   orc_philox4x32_10     known-answer vectors (tests/golden/philox4x32_10_kat.txt)
@@ -214,7 +214,7 @@ double orc_dpd_theta(uint32_t tag_a, uint32_t tag_b, uint64_t step, uint64_t see
 
 /* ------------------------------------------------------------------------------------------------
  * O5 DPD pair force (named PAPER.md:63; drag needs neighbour velocities and the random term needs
- * global particle IDs; formula = Groot-Warren, R5):
+ * global particle IDs; formula = Groot-Warren, R9):
  *   pair with 0 < r < rc:  w = 1 - r/rc, rhat = d/r, d = minimg(x_a - x_b)
  *   F = [A w - gamma w^2 (rhat . (v_a - v_b)) + sqrt(2 gamma kT) w theta_ab / sqrt(dt)] rhat
  *   on a, -F on b.  force is OVERWRITTEN.

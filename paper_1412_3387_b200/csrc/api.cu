@@ -274,8 +274,8 @@ int build_cell_order(md_ctx *c)
 static void set_default_cfg(md_ctx *c)
 {
     for (int k = 0; k < MD_N_KERNELS; ++k) c->cfg[k] = LaunchCfg{128, 1, 0.f};
-    c->cfg[MD_K_NLIST] = LaunchCfg{128, 8, 0.f};
-    c->cfg[MD_K_LJ] = LaunchCfg{128, 8, 0.f};
+    c->cfg[MD_K_NLIST] = LaunchCfg{256, 8, 0.f};
+    c->cfg[MD_K_LJ] = LaunchCfg{256, 2, 0.f};
     c->cfg[MD_K_DPD] = LaunchCfg{128, 4, 0.f};
     c->cfg[MD_K_BONDS] = LaunchCfg{128, 1, 0.f};
     c->cfg[MD_K_INTEGRATE] = LaunchCfg{256, 1, 0.f};

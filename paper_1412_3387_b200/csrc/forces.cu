@@ -92,7 +92,7 @@ int launch_forces_lj(md_ctx *c, double eps, double sigma, int shift)
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// DPD (R5, R13-R15): conservative + drag + pairwise random force; fp64; needs neighbour velocities
+// DPD (R9, R13-R15): conservative + drag + pairwise random force; fp64; needs neighbour velocities
 // and tags.
 // ------------------------------------------------------------------------------------------------------------
 struct DPDParams {
