@@ -214,7 +214,6 @@ int build_cell_order(md_ctx *c)
 {
     for (uint32_t **p : {&c->rank_of_lin, &c->lin_of_rank, &c->tile_cell_begin, &c->tile_origin})
         if (*p) { md_free(c, *p); *p = nullptr; }
-    if (c->tile_base) { md_free(c, c->tile_base); c->tile_base = nullptr; }
     c->use_tiles = false;
     c->n_tiles = 0;
     if (c->order == MD_ORDER_LEX) return MD_OK;
@@ -259,11 +258,9 @@ int build_cell_order(md_ctx *c)
     MD_TRY(md_alloc(c, (void **)&c->lin_of_rank, sizeof(uint32_t) * c->n_cells));
     MD_TRY(md_alloc(c, (void **)&c->tile_cell_begin, sizeof(uint32_t) * begin.size()));
     MD_TRY(md_alloc(c, (void **)&c->tile_origin, sizeof(uint32_t) * origin.size()));
-    MD_TRY(md_alloc(c, (void **)&c->tile_base, sizeof(unsigned long long) * c->n_tiles));
     MD_CUDA_CHECK(c, cudaMemcpy(c->lin_of_rank, lin_of_rank.data(), sizeof(uint32_t) * c->n_cells, cudaMemcpyHostToDevice));
     MD_CUDA_CHECK(c, cudaMemcpy(c->tile_cell_begin, begin.data(), sizeof(uint32_t) * begin.size(), cudaMemcpyHostToDevice));
     MD_CUDA_CHECK(c, cudaMemcpy(c->tile_origin, origin.data(), sizeof(uint32_t) * origin.size(), cudaMemcpyHostToDevice));
-    if (!c->row_off) MD_TRY(md_alloc(c, (void **)&c->row_off, c->N * sizeof(uint32_t)));
     c->use_tiles = true;
     return MD_OK;
 }
@@ -462,10 +459,15 @@ extern "C" int md_get_state(md_ctx *c, double *pos, double *vel, int32_t *image)
     return MD_OK;
 }
 
+static int eval_forces(md_ctx *c, const md_step_desc *w, uint64_t step, bool energy);
+
 extern "C" int md_get_forces(md_ctx *c, double *force, double *energy)
 {
     if (!c) return MD_EINVAL;
     if (!c->force_valid) { c->err = "md_get_forces: no force has been computed for the current positions"; return MD_ESTATE; }
+    // md_step evaluates LJ forces without the per-particle energies; the forces are a pure function of the current
+    // state, so the same evaluation is repeated with the energy lane switched on when it is asked for
+    if (energy && !c->energy_valid && c->last_from_step) MD_TRY(eval_forces(c, &c->last_desc, c->last_force_step, true));
     const uint64_t b3 = 3 * c->N * sizeof(double), b1 = c->N * sizeof(double);
     Stage st(c);
     MD_TRY(st.reserve(stage_need(force, b3) + stage_need(energy, b1)));
@@ -538,6 +540,8 @@ static int build_nlist_general(md_ctx *c)
     return MD_OK;
 }
 
+static uint32_t round16(double x) { return (uint32_t)((uint64_t)(x + 15.0) / 16 * 16); }
+
 static int build_nlist_tiles(md_ctx *c, bool *done)
 {
     *done = false;
@@ -545,21 +549,21 @@ static int build_nlist_tiles(md_ctx *c, bool *done)
     MD_TRY(md_read_flags(c));
     c->tile_max_home = c->h_flags->max_home;
     c->tile_max_staged = c->h_flags->max_staged;
-    if (c->nl16_capacity == 0) {
-        double vol = c->box[0] * c->box[1] * c->box[2];
-        double nbar = (double)c->N / vol * 4.18879020478639 * c->r_list * c->r_list * c->r_list;
-        uint64_t cap = (uint64_t)((double)c->N * (nbar + 8.0) * 1.15) + 4096;
-        MD_TRY(md_alloc(c, (void **)&c->nl16, cap * sizeof(uint16_t)));
-        c->nl16_capacity = cap;
+    if (c->nl_stride == 0) {
+        // row stride from the mean density: 1.35 n + 24 covers the fluctuations of liquids and ideal gases at the
+        // configured densities; a longer row is detected by the build kernel and the stride grows
+        const double vol = c->box[0] * c->box[1] * c->box[2];
+        const double nbar = (double)c->N / vol * 4.18879020478639 * c->r_list * c->r_list * c->r_list;
+        c->nl_stride = round16(1.35 * nbar + 24.0);
     }
-    for (int attempt = 0; attempt < 2; ++attempt) {
+    for (int attempt = 0; attempt < 3; ++attempt) {
+        if (!c->nl16) MD_TRY(md_alloc(c, (void **)&c->nl16, c->N * (uint64_t)c->nl_stride * sizeof(uint16_t)));
         bool fits = false;
         MD_TRY(launch_tile_build(c, &fits));
         if (!fits) return MD_OK;  // largest tile exceeds shared memory: general path
         MD_TRY(md_read_flags(c));
-        const uint64_t need = c->h_flags->cursor;
-        if (need <= c->nl16_capacity) {
-            c->nl_entries = need;
+        if (c->h_flags->nl_overflow == 0) {
+            c->nl_entries = c->h_flags->nl_total;
             c->nl_is_tile = true;
             c->nl32_decoded = false;
             *done = true;
@@ -567,12 +571,10 @@ static int build_nlist_tiles(md_ctx *c, bool *done)
         }
         md_free(c, c->nl16);
         c->nl16 = nullptr;
-        c->nl16_capacity = 0;
-        const uint64_t cap = need + need / 8 + 4096;
-        MD_TRY(md_alloc(c, (void **)&c->nl16, cap * sizeof(uint16_t)));
-        c->nl16_capacity = cap;
+        c->nl_stride = round16(1.25 * c->h_flags->nl_overflow + 16.0);
+        if (c->log) fprintf(stderr, "[b200md] neighbour row stride grows to %u entries\n", c->nl_stride);
     }
-    c->err = "neighbour list: capacity still too small after growing";
+    c->err = "neighbour list: row stride still too small after growing";
     return MD_ECUDA;
 }
 
@@ -588,14 +590,18 @@ static int do_build_nlist(md_ctx *c)
     return MD_OK;
 }
 
-// exports read the general 32-bit CSR; a tile list is decoded into it on demand
+// exports read the general 32-bit CSR; a tile list is decoded into it on demand (exact filter, see tiles.cu)
 static int ensure_decoded(md_ctx *c)
 {
-    if (!c->nl_is_tile || c->nl32_decoded) return MD_OK;
-    MD_TRY(launch_exclusive_scan_u32(c, c->nl_cnt, c->N, nullptr, c->nl_off, true, &c->d_flags->nl_total));
+    if (!c->nl_is_tile) { c->nl_cnt_exp = c->nl_cnt; return MD_OK; }
+    if (c->nl32_decoded) return MD_OK;
+    if (!c->nl_cnt32) MD_TRY(md_alloc(c, (void **)&c->nl_cnt32, c->N * sizeof(uint32_t)));
+    MD_TRY(launch_tile_decode(c, false, c->nl_cnt32));
+    MD_TRY(launch_exclusive_scan_u32(c, c->nl_cnt32, c->N, nullptr, c->nl_off, false, &c->d_flags->nl_total));
     MD_TRY(md_read_flags(c));
     MD_TRY(ensure_nl32(c, c->h_flags->nl_total));
-    MD_TRY(launch_tile_decode(c));
+    MD_TRY(launch_tile_decode(c, true, nullptr));
+    c->nl_cnt_exp = c->nl_cnt32;
     c->nl32_decoded = true;
     return MD_OK;
 }
@@ -665,9 +671,9 @@ extern "C" int md_get_nlist_rows(md_ctx *c, const uint32_t *probe_tags, uint32_t
 // S4 / S5 / S6 single calls
 // =====================================================================================================
 // pair kernels: tile path when the current list is a tile list, else the general list kernels
-static int pair_lj(md_ctx *c, double eps, double sigma, int shift)
+static int pair_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
 {
-    if (c->nl_is_tile) return launch_tile_lj(c, eps, sigma, shift);
+    if (c->nl_is_tile) return launch_tile_lj(c, eps, sigma, shift, energy);
     return launch_forces_lj(c, eps, sigma, shift);
 }
 static int pair_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed)
@@ -687,8 +693,9 @@ extern "C" int md_forces_lj(md_ctx *c, double eps, double sigma, int shift)
     if (!c) return MD_EINVAL;
     MD_TRY(need_nlist(c, "md_forces_lj"));
     ProfScope ps(c, MD_K_LJ);
-    MD_TRY(pair_lj(c, eps, sigma, shift));
-    c->force_valid = true;
+    MD_TRY(pair_lj(c, eps, sigma, shift, true));
+    c->force_valid = c->energy_valid = true;
+    c->last_from_step = false;
     return MD_OK;
 }
 
@@ -699,7 +706,8 @@ extern "C" int md_forces_dpd(md_ctx *c, double A, double gamma, double kT, doubl
     MD_TRY(need_nlist(c, "md_forces_dpd"));
     ProfScope ps(c, MD_K_DPD);
     MD_TRY(pair_dpd(c, A, gamma, kT, dt, step, seed));
-    c->force_valid = true;
+    c->force_valid = c->energy_valid = true;
+    c->last_from_step = false;
     return MD_OK;
 }
 
@@ -741,12 +749,12 @@ extern "C" int md_needs_rebuild(md_ctx *c, int *flag)
 // =====================================================================================================
 // S7 step scheduler
 // =====================================================================================================
-static int eval_forces(md_ctx *c, const md_step_desc *w, uint64_t step)
+static int eval_forces(md_ctx *c, const md_step_desc *w, uint64_t step, bool energy)
 {
     bool any = false;
     if (w->flags & MD_F_LJ) {
         ProfScope ps(c, MD_K_LJ);
-        MD_TRY(pair_lj(c, w->lj_epsilon, w->lj_sigma, w->lj_energy_shift));
+        MD_TRY(pair_lj(c, w->lj_epsilon, w->lj_sigma, w->lj_energy_shift, energy));
         any = true;
     }
     if (w->flags & MD_F_DPD) {
@@ -761,6 +769,11 @@ static int eval_forces(md_ctx *c, const md_step_desc *w, uint64_t step)
         MD_TRY(launch_forces_bonds(c, w->bond_k, w->bond_r0));
     }
     c->force_valid = true;
+    // only the tile LJ kernel skips the per-particle energies
+    c->energy_valid = energy || !((w->flags & MD_F_LJ) && c->nl_is_tile);
+    c->last_desc = *w;
+    c->last_force_step = step;
+    c->last_from_step = true;
     return MD_OK;
 }
 
@@ -776,7 +789,7 @@ extern "C" int md_step(md_ctx *c, const md_step_desc *w, uint64_t n_steps)
     if (!c->have_state) { c->err = "md_step: md_set_state first"; return MD_ESTATE; }
     if (!(w->dt > 0.0)) { c->err = "md_step: dt must be positive"; return MD_EINVAL; }
     if (!c->nlist_valid) MD_TRY(rebuild(c));
-    if (!c->force_valid) MD_TRY(eval_forces(c, w, c->step));  // R16: F(t0) before the first half-kick
+    if (!c->force_valid) MD_TRY(eval_forces(c, w, c->step, false));  // R16: F(t0) before the first half-kick
     for (uint64_t s = 0; s < n_steps; ++s) {
         {
             ProfScope ps(c, MD_K_INTEGRATE);
@@ -787,7 +800,7 @@ extern "C" int md_step(md_ctx *c, const md_step_desc *w, uint64_t n_steps)
             if (c->h_flags->dangerous) c->stats.dangerous_builds++;
             MD_TRY(rebuild(c));
         }
-        MD_TRY(eval_forces(c, w, c->step + 1));  // R15: hash counter = index of the step being completed
+        MD_TRY(eval_forces(c, w, c->step + 1, false));  // R15: hash counter = index of the step being completed
         {
             ProfScope ps(c, MD_K_INTEGRATE);
             MD_TRY(launch_half2(c, w->dt));
@@ -867,7 +880,7 @@ extern "C" int md_tune(md_ctx *c, const md_step_desc *w, int full)
         }));
     }
     if (w->flags & MD_F_LJ)
-        MD_TRY(tune_kernel(c, MD_K_LJ, c->nl_is_tile ? "lj/tile" : "lj", true, full, [&]() { return pair_lj(c, w->lj_epsilon, w->lj_sigma, w->lj_energy_shift); }));
+        MD_TRY(tune_kernel(c, MD_K_LJ, c->nl_is_tile ? "lj/tile" : "lj", true, full, [&]() { return pair_lj(c, w->lj_epsilon, w->lj_sigma, w->lj_energy_shift, false); }));
     if (w->flags & MD_F_DPD)
         MD_TRY(tune_kernel(c, MD_K_DPD, c->nl_is_tile ? "dpd/tile" : "dpd", true, full, [&]() { return pair_dpd(c, w->dpd_A, w->dpd_gamma, w->dpd_kT, w->dt, c->step, w->dpd_seed); }));
     c->force_valid = false;  // the replays overwrote the force array with a partial evaluation (pair term only)

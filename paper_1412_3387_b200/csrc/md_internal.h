@@ -45,8 +45,9 @@ struct DevFlags {
     unsigned int max_home;        // largest tile: home particles
     unsigned int max_staged;      // largest tile: staged (stencil) particles
     int pad;
-    unsigned long long nl_total;  // entries (padded rows) of the list being built (general path)
-    unsigned long long cursor;    // entries reserved by the tile build (may exceed the capacity: grow + rebuild)
+    unsigned long long nl_total;  // entries of the list being built (general path: padded rows; tile path: sum of row lengths)
+    unsigned int nl_overflow;     // tile build: longest row if it exceeds the row stride (host grows the stride, rebuilds)
+    unsigned int pad2;
 };
 
 struct LaunchCfg {
@@ -87,7 +88,8 @@ struct md_ctx {
     uint32_t *nl_cnt = nullptr;
     uint64_t *nl_off = nullptr;
     uint32_t *nl_idx = nullptr;
-    uint64_t nl_capacity = 0, nl_entries = 0, nl_real_entries = 0;
+    uint64_t nl_capacity = 0, nl_entries = 0;
+    uint32_t *nl_cnt_exp = nullptr;  // row lengths of the decoded / general CSR that the exports read
 
     // tile path (tiles.cu): bricks of tile_B^3 cells, Morton cell order, 16-bit staged indices
     bool use_tiles = false;     // configured (MD_ORDER_MORTON)
@@ -97,10 +99,10 @@ struct md_ctx {
     int tile_B_forced = 0, acc_block = 8;
     uint32_t *tile_cell_begin = nullptr, *tile_origin = nullptr, *lin_of_rank = nullptr;
     uint32_t tile_max_home = 0, tile_max_staged = 0;
-    uint16_t *nl16 = nullptr;
-    uint64_t nl16_capacity = 0;
-    unsigned long long *tile_base = nullptr;
-    uint32_t *row_off = nullptr;
+    uint16_t *nl16 = nullptr;        // fixed-stride rows: row of slot i starts at nl16 + i * nl_stride
+    uint32_t nl_stride = 0;          // entries per row, multiple of 16
+    uint32_t nl_shift = 0;           // entry = staged index << nl_shift
+    uint32_t *nl_cnt32 = nullptr;    // exact row lengths of the decoded list (exports)
 
     // bonds: CSR by TAG
     uint64_t n_bonds = 0;
@@ -117,6 +119,10 @@ struct md_ctx {
 
     // status
     bool have_state = false, cells_valid = false, nlist_valid = false, force_valid = false;
+    bool energy_valid = false;  // the energy lane of `force` belongs to the current forces (md_step skips energies)
+    md_step_desc last_desc;     // what the current forces were evaluated with (re-evaluation with energies on demand)
+    uint64_t last_force_step = 0;
+    bool last_from_step = false;
     uint64_t step = 0;
     md_stats stats;
     LaunchCfg cfg[MD_N_KERNELS];
@@ -173,7 +179,7 @@ int build_cell_order(md_ctx *c);  // host: rank_of_lin table for the configured 
 // tiles.cu
 int tile_measure(md_ctx *c);
 int launch_tile_build(md_ctx *c, bool *fits);
-int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift);
+int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy);
 int launch_tile_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed);
 bool tile_forces_fit(md_ctx *c, bool dpd);
-int launch_tile_decode(md_ctx *c);
+int launch_tile_decode(md_ctx *c, bool fill, uint32_t *cnt32);

@@ -128,14 +128,14 @@ __global__ void k_pairs_fill(const uint32_t *__restrict__ nl_cnt, const uint64_t
 
 int launch_export_pairs_count(md_ctx *c, uint32_t *cnt)
 {
-    k_pairs_count<<<md_grid(c->N, 128), 128, 0, c->stream>>>(c->nl_cnt, c->nl_off, c->nl_idx, c->tag, (uint32_t)c->N, cnt);
+    k_pairs_count<<<md_grid(c->N, 128), 128, 0, c->stream>>>(c->nl_cnt_exp, c->nl_off, c->nl_idx, c->tag, (uint32_t)c->N, cnt);
     MD_LAUNCH_CHECK(c);
     return MD_OK;
 }
 
 int launch_export_pairs_fill(md_ctx *c, const uint64_t *off, uint32_t *pairs)
 {
-    k_pairs_fill<<<md_grid(c->N, 128), 128, 0, c->stream>>>(c->nl_cnt, c->nl_off, c->nl_idx, c->tag, (uint32_t)c->N, off,
+    k_pairs_fill<<<md_grid(c->N, 128), 128, 0, c->stream>>>(c->nl_cnt_exp, c->nl_off, c->nl_idx, c->tag, (uint32_t)c->N, off,
                                                            pairs);
     MD_LAUNCH_CHECK(c);
     return MD_OK;
@@ -160,7 +160,7 @@ int launch_export_rows(md_ctx *c, const uint32_t *probe_tags, uint32_t n_probe, 
                        uint32_t stride)
 {
     if (n_probe == 0) return MD_OK;
-    k_rows<<<n_probe, 64, 0, c->stream>>>(probe_tags, n_probe, c->rtag, c->nl_cnt, c->nl_off, c->nl_idx, c->tag,
+    k_rows<<<n_probe, 64, 0, c->stream>>>(probe_tags, n_probe, c->rtag, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->tag,
                                           (uint32_t)c->N, counts, nbr, stride);
     MD_LAUNCH_CHECK(c);
     return MD_OK;

@@ -4,23 +4,27 @@
 // range of particles ("home" particles) and one CTA owns it.  The CTA stages every particle of the (B+2)^3 stencil
 // cells in shared memory as coordinates RELATIVE to the brick centre with the periodic image already applied
 // ("Look up cell neighbors"; north_star "cell-neighbor stencils staged in shared memory").  Consequences:
-//   * neighbour-list entries are 16-bit indices into the staged block, not 32-bit global indices: the index stream,
+//   * neighbour-list entries are 16-bit references into the staged block, not 32-bit global indices: the index stream,
 //     which dominates the algorithmic HBM bytes, is halved;
 //   * every neighbour gather is a shared-memory load, never an L2/HBM access;
 //   * no minimum-image arithmetic per pair: the image is applied once per staged particle;
-//   * in MD_MIXED the staged coordinates are fp32 and small (|x| < ~2 cell widths), so separations keep ~1e-7
-//     absolute accuracy although absolute coordinates would not (hard part 3).
-// Decisions (r^2 < r_list^2 at build time, r^2 < rc^2 in the force kernels) are taken on the staged coordinates only
-// when they are outside a guard band around the threshold that bounds the staging error; inside the band the pair
-// is re-tested with the exact fp64 expression of DESIGN.md R2 on the global positions, so lists and cut-off
-// decisions are those of the plain definition, bit for bit.
+//   * the staged coordinates are small (|x| < ~2.5 cell widths), so fp32 separations keep ~1e-6 absolute accuracy
+//     although absolute fp32 coordinates would not (hard part 3).
 //
-// Neighbour-list build (Fig. 4) with w = 32: a warp strides over the 9 x-runs of the 27 stencil
-// cells, one ballot per 32 candidates (Fig. 4 steps 2-3), for BUILD_P home particles of one cell at a time (the
-// candidate is loaded once and tested against BUILD_P particles held in registers).  The ballot words are kept in
-// shared memory; per chunk of particles the CTA scans the row lengths, reserves the rows in the global array with ONE
-// atomicAdd (placement only: content and order of every row are deterministic) and writes the rows compacted by
-// popc prefix sums (steps 4-8), one lane per ballot word: no second distance pass, no per-entry atomics.
+// Neighbour list (Fig. 4), w = 32: a warp strides over the 9 x-runs of the 27 stencil cells, one
+// ballot per 32 candidates (Fig. 4 steps 2-3) for BUILD_P home particles of one cell at a time (a candidate is loaded
+// once and tested against BUILD_P particles held in registers).  The distance test is the fp32 dot-product form
+// |b|^2 - 2 a.b < R^2 - |a|^2 (three FFMA per candidate, |b|^2 staged with the record) against R^2 = r_list^2 + guard,
+// where the guard bounds the fp32 error: the stored list is therefore a SUPERSET of the exact list by at most the
+// pairs inside the guard band (relative width ~1e-5), which is a valid Verlet list (it only has to
+// contain every pair that can come within r_cut before the next rebuild).  Hits are compacted with popc prefix sums
+// of the ballot (steps 4-7) into a row assembled in shared memory and written out with 16-byte stores; rows have a
+// fixed stride, so there is no count pass, no scan, no reservation and no atomic anywhere, and every warp works
+// independently of the others.  The EXPORTED list (md_get_nlist / md_get_nlist_rows) is filtered with the exact fp64
+// expression of DESIGN.md R2 on the positions the list was built from, so it equals the plain definition bit for bit.
+//
+// Force kernels take the r < rc decision on the staged coordinates only outside a guard band around rc^2; inside
+// the band the pair is re-tested with the exact fp64 expression on the global positions (R26).
 #include <algorithm>
 #include <type_traits>
 
@@ -33,6 +37,8 @@ struct TileParams {
     uint32_t B;        // brick edge in cells
     uint32_t nsc_max;  // (B+2)^3
     uint32_t n_tiles;
+    uint32_t stride;   // entries per neighbour row (multiple of 16)
+    uint32_t shift;    // list entry = staged index << shift (4: byte offset of a float4 record; 0: plain index)
     const uint32_t *tile_cell_begin;  // [n_tiles+1] first cell rank of each tile
     const uint32_t *tile_origin;      // [3 n_tiles] lowest cell coordinate of the brick
     const uint32_t *lin_of_rank;      // cell rank -> linear id
@@ -51,6 +57,7 @@ struct TileSmem {
     uint32_t *sstart;   // [nsc+1] staged index of the first particle of each staged cell
     uint32_t *hc_sc;    // [B^3]   staged-cell index of each home cell
     uint32_t *hc_first; // [B^3+1] first home particle (tile-local) of each home cell
+    uint32_t *hc_task;  // [B^3+1] first build task of each home cell (build kernel only)
     double *cgeo;       // [nsc*6] per staged cell: centre inside the box (3), centre of its image rel. brick centre (3)
     char *rest;         // records etc.
 };
@@ -58,7 +65,7 @@ struct TileSmem {
 __host__ __device__ inline size_t tile_header_bytes(uint32_t B)
 {
     const size_t nsc = (size_t)(B + 2) * (B + 2) * (B + 2), nhc = (size_t)B * B * B;
-    size_t b = sizeof(uint32_t) * (nsc + (nsc + 1) + nhc + (nhc + 1));
+    size_t b = sizeof(uint32_t) * (nsc + (nsc + 1) + nhc + 2 * (nhc + 1));
     b = (b + 15) & ~(size_t)15;
     b += sizeof(double) * 6 * nsc;
     return (b + 15) & ~(size_t)15;
@@ -72,7 +79,8 @@ __device__ __forceinline__ TileSmem tile_carve(char *smem, uint32_t B)
     t.sstart = t.gstart + nsc;
     t.hc_sc = t.sstart + nsc + 1;
     t.hc_first = t.hc_sc + nhc;
-    size_t b = sizeof(uint32_t) * (nsc + (nsc + 1) + nhc + (nhc + 1));
+    t.hc_task = t.hc_first + nhc + 1;
+    size_t b = sizeof(uint32_t) * (nsc + (nsc + 1) + nhc + 2 * (nhc + 1));
     b = (b + 15) & ~(size_t)15;
     t.cgeo = (double *)(smem + b);
     t.rest = smem + tile_header_bytes(B);
@@ -172,28 +180,47 @@ __device__ __forceinline__ uint32_t tile_staged_of_home(const TileSmem &h, uint3
     return h.sstart[h.hc_sc[hc]] + (p - h.hc_first[hc]);
 }
 
+// global slot of staged index s
+__device__ __forceinline__ uint32_t tile_global_of_staged(const TileSmem &h, uint32_t n_sc, uint32_t s)
+{
+    const uint32_t sc = tile_cell_of_staged(h, n_sc, s);
+    return h.gstart[sc] + (s - h.sstart[sc]);
+}
+
 template <typename R4> struct RecTraits;
 template <> struct RecTraits<float4> {
     typedef float real;
-    static __device__ __forceinline__ float4 make(double x, double y, double z, double w) { return make_float4((float)x, (float)y, (float)z, 0.f); }
-    static __device__ __forceinline__ float4 far(float s) { return make_float4(s * 1e15f, s * 1e15f, s * 1e15f, 0.f); }
+    // w = |r|^2 of the ROUNDED coordinates (the build kernel's dot-product test)
+    static __device__ __forceinline__ float4 make(double x, double y, double z, double w)
+    {
+        const float fx = (float)x, fy = (float)y, fz = (float)z;
+        return make_float4(fx, fy, fz, fx * fx + fy * fy + fz * fz);
+    }
+    static __device__ __forceinline__ float4 far() { return make_float4(1e15f, 1e15f, 1e15f, 3e30f); }
 };
 template <> struct RecTraits<double4> {
     typedef double real;
     static __device__ __forceinline__ double4 make(double x, double y, double z, double w) { return make_double4(x, y, z, w); }
-    static __device__ __forceinline__ double4 far(double s) { return make_double4(s * 1e150, s * 1e150, s * 1e150, 0.0); }
+    static __device__ __forceinline__ double4 far() { return make_double4(1e150, 1e150, 1e150, 0.0); }
 };
 
 // stage every stencil particle: coordinates relative to the brick centre, periodic image applied.
 // x_staged = c_s + minimg(x - C_w): C_w = centre of the particle's cell inside the box, c_s = centre of that cell's
 // image relative to the brick centre.  |x - C_w| <= w/2 + drift << L/2, so this also undoes an integrator wrap.
+// scell: [max_staged] scratch, staged cell of each staged record (filled here; replaces a search per record).
 template <typename R4, bool WITH_VEL>
 __device__ __forceinline__ void tile_stage(const Geom &g, const TileCtx &tc, const TileSmem &h,
                                            const double4 *__restrict__ pos, const double4 *__restrict__ vel, R4 *rec,
-                                           double4 *svel)
+                                           double4 *svel, uint8_t *scell)
 {
+    const uint32_t lane = threadIdx.x & 31u, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (uint32_t sc = wid; sc < tc.n_sc; sc += nw) {
+        const uint32_t b = h.sstart[sc], e = h.sstart[sc + 1];
+        for (uint32_t s = b + lane; s < e; s += 32) scell[s] = (uint8_t)sc;
+    }
+    __syncthreads();
     for (uint32_t s = threadIdx.x; s < tc.n_staged; s += blockDim.x) {
-        const uint32_t sc = tile_cell_of_staged(h, tc.n_sc, s);
+        const uint32_t sc = scell[s];
         const uint32_t gi = h.gstart[sc] + (s - h.sstart[sc]);
         const double4 p = pos[gi];
         const double *cg = h.cgeo + 6 * sc;
@@ -203,17 +230,10 @@ __device__ __forceinline__ void tile_stage(const Geom &g, const TileCtx &tc, con
         rec[s] = RecTraits<R4>::make(x, y, z, p.w);
         if (WITH_VEL) svel[s] = vel[gi];
     }
-    if (threadIdx.x == 0) rec[tc.n_staged] = RecTraits<R4>::far(1);  // dummy record for row padding
+    if (threadIdx.x == 0) rec[tc.n_staged] = RecTraits<R4>::far();  // dummy record: row padding, out-of-run lanes
 }
 
-// global slot of staged index s
-__device__ __forceinline__ uint32_t tile_global_of_staged(const TileSmem &h, uint32_t n_sc, uint32_t s)
-{
-    const uint32_t sc = tile_cell_of_staged(h, n_sc, s);
-    return h.gstart[sc] + (s - h.sstart[sc]);
-}
-
-// the plain definition on the global (wrapped) positions: exact fp64, no FMA (R2, R8)
+// the plain definition on global (wrapped) positions: exact fp64, no FMA (R2, R8)
 __device__ __noinline__ double tile_exact_r2_impl(const double4 *__restrict__ pos, double Lx, double Ly, double Lz,
                                                   uint32_t gi, uint32_t gj)
 {
@@ -252,177 +272,141 @@ __global__ void k_tile_sizes(TileParams tp, Geom g, unsigned int *max_home, unsi
 }
 
 // ===============================================================================================================
-// S2 neighbour-list build, one CTA per tile
+// S2 neighbour-list build, one CTA per tile, one warp per task of P home particles of one cell
 // ===============================================================================================================
-template <typename R4>
-__global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build(TileParams tp, Geom g, const double4 *__restrict__ pos,
-                                                               typename RecTraits<R4>::real thr_in,
-                                                               typename RecTraits<R4>::real thr_out, double rl2_exact,
-                                                               uint32_t wpr /* ballot words per x-run */,
-                                                               uint32_t max_staged, unsigned long long *cursor,
-                                                               unsigned long long capacity, uint32_t *row_off,
-                                                               uint32_t *nl_cnt, uint16_t *nl16)
+__device__ __forceinline__ unsigned md_lanemask_lt()
 {
-    typedef typename RecTraits<R4>::real real;
+    unsigned m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+
+template <int P>
+__global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build(TileParams tp, Geom g, const double4 *__restrict__ pos,
+                                                               float thr_out /* r_list^2 + guard */,
+                                                               uint32_t max_staged, uint32_t *__restrict__ nl_cnt,
+                                                               uint16_t *__restrict__ nl16, DevFlags *flags)
+{
     extern __shared__ __align__(16) char smem_raw[];
     const TileSmem h = tile_carve(smem_raw, tp.B);
-    R4 *rec = (R4 *)h.rest;
+    float4 *rec = (float4 *)h.rest;
     const uint32_t nw = blockDim.x >> 5;
-    const uint32_t chunk = nw * BUILD_P;  // home particles per chunk
-    uint32_t *counts = (uint32_t *)(h.rest + sizeof(R4) * (max_staged + 1));  // [chunk] counts, then row offsets
-    uint32_t *words = counts + chunk;                                         // [chunk * 9 * wpr]
-    __shared__ unsigned long long s_base;
-    __shared__ uint32_t s_ok;
+    uint16_t *rowbuf = (uint16_t *)(h.rest + sizeof(float4) * (max_staged + 1));  // [nw][P][stride], 16-byte aligned
+    uint8_t *scell = (uint8_t *)(rowbuf + (size_t)nw * P * tp.stride);            // [max_staged]
 
     TileCtx tc;
     tile_setup(tp, g, blockIdx.x, h, tc);
-    tile_stage<R4, false>(g, tc, h, pos, nullptr, rec, nullptr);
+    tile_stage<float4, false>(g, tc, h, pos, nullptr, rec, nullptr, scell);
+    if (threadIdx.x < 32) {  // first task of each home cell: exclusive scan of ceil(count / P), n_hc <= 64
+        uint32_t carry = 0;
+        for (uint32_t base = 0; base <= tc.n_hc; base += 32) {
+            const uint32_t hc = base + threadIdx.x;
+            const uint32_t v = hc < tc.n_hc ? (h.hc_first[hc + 1] - h.hc_first[hc] + P - 1) / P : 0u;
+            uint32_t inc = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t u = __shfl_up_sync(0xffffffffu, inc, o);
+                if ((int)threadIdx.x >= o) inc += u;
+            }
+            if (hc <= tc.n_hc) h.hc_task[hc] = carry + inc - v;
+            carry += __shfl_sync(0xffffffffu, inc, 31);
+        }
+    }
     __syncthreads();
 
     const unsigned lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;
-    const uint32_t wpp = 9 * wpr;
+    const unsigned lt = md_lanemask_lt();
+    const uint32_t n_tasks = h.hc_task[tc.n_hc];
+    const uint32_t stride = tp.stride;
+    const uint32_t dummy_ent = tc.n_staged << tp.shift;
+    uint16_t *rb = rowbuf + (size_t)wid * P * stride;
+    unsigned long long total = 0;
+    uint32_t worst = 0;
 
-    // tasks: groups of BUILD_P consecutive particles of one home cell
-    uint32_t n_tasks = 0;
-    for (uint32_t hc = 0; hc < tc.n_hc; ++hc) n_tasks += (h.hc_first[hc + 1] - h.hc_first[hc] + BUILD_P - 1) / BUILD_P;
-
-    for (uint32_t task0 = 0; task0 < n_tasks; task0 += nw) {
-        // ---- pass A: hit masks (Fig. 4 steps 1-3); warp `wid` takes task task0 + wid
-        const uint32_t task = task0 + wid;
-        uint32_t hc = 0, p0 = 0, np = 0;  // home cell, first particle (tile-local), particles in this task
-        if (task < n_tasks) {
-            uint32_t t = task;
-            for (hc = 0; hc < tc.n_hc; ++hc) {
-                const uint32_t nt = (h.hc_first[hc + 1] - h.hc_first[hc] + BUILD_P - 1) / BUILD_P;
-                if (t < nt) break;
-                t -= nt;
+    for (uint32_t task = wid; task < n_tasks; task += nw) {
+        // home cell of the task (binary search over hc_task), first particle, particles in this task
+        uint32_t hc = 0;
+        {
+            uint32_t lo = 0, hi = tc.n_hc;
+            while (hi - lo > 1) {
+                const uint32_t mid = (lo + hi) >> 1;
+                if (h.hc_task[mid] <= task) lo = mid; else hi = mid;
             }
-            p0 = h.hc_first[hc] + t * BUILD_P;
-            np = min((uint32_t)BUILD_P, h.hc_first[hc + 1] - p0);
+            hc = lo;
         }
-        uint32_t cnt[BUILD_P];
+        const uint32_t p0 = h.hc_first[hc] + (task - h.hc_task[hc]) * P;
+        const uint32_t np = min((uint32_t)P, h.hc_first[hc + 1] - p0);
+        const uint32_t sch = h.hc_sc[hc];
+        const uint32_t ixh = sch % tc.sx, iyh = (sch / tc.sx) % tc.sy, izh = sch / (tc.sx * tc.sy);
+        const uint32_t self0 = h.sstart[sch] + (p0 - h.hc_first[hc]);
+        // hit <=> |b|^2 - 2 a.b < thr - |a|^2
+        float ax[P], ay[P], az[P], th[P];
+        uint32_t cnt[P];
 #pragma unroll
-        for (int q = 0; q < BUILD_P; ++q) cnt[q] = 0;
-        if (np > 0) {
-            const uint32_t sch = h.hc_sc[hc];
-            const uint32_t ixh = sch % tc.sx, iyh = (sch / tc.sx) % tc.sy, izh = sch / (tc.sx * tc.sy);
-            const uint32_t self0 = h.sstart[sch] + (p0 - h.hc_first[hc]);
-            R4 me[BUILD_P];
-#pragma unroll
-            for (int q = 0; q < BUILD_P; ++q) me[q] = (uint32_t)q < np ? rec[self0 + q] : RecTraits<R4>::far(-1);
-            uint32_t *wp = words + (size_t)wid * BUILD_P * wpp;
+        for (int q = 0; q < P; ++q) {
+            const float4 m = rec[self0 + min((uint32_t)q, np - 1)];
+            ax[q] = -2.f * m.x; ay[q] = -2.f * m.y; az[q] = -2.f * m.z;
+            th[q] = (uint32_t)q < np ? thr_out - m.w : -3e38f;  // absent particles never hit
+            cnt[q] = 0;
+        }
 #pragma unroll 1
-            for (int run = 0; run < 9; ++run) {
-                const uint32_t iy = iyh + (run % 3) - 1, iz = izh + (run / 3) - 1;
-                const uint32_t sc0 = (ixh - 1) + tc.sx * (iy + tc.sy * iz);
-                const uint32_t b = h.sstart[sc0], e = h.sstart[sc0 + 3];
-                uint32_t k = run * wpr;
-                for (uint32_t base = b; base < e; base += 32, ++k) {
-                    const uint32_t j = base + lane;
-                    const bool valid = j < e;
-                    const R4 pj = rec[valid ? j : tc.n_staged];  // past the run: the far-away dummy record
-                    unsigned bal[BUILD_P];
+        for (int run = 0; run < 9; ++run) {
+            const uint32_t iy = iyh + (run % 3) - 1, iz = izh + (run / 3) - 1;
+            const uint32_t sc0 = (ixh - 1) + tc.sx * (iy + tc.sy * iz);
+            const uint32_t b = h.sstart[sc0], e = h.sstart[sc0 + 3];
+#pragma unroll 1
+            for (uint32_t base = b; base < e; base += 32) {
+                const uint32_t j = base + lane;
+                const float4 pj = rec[j < e ? j : tc.n_staged];  // past the run: the far-away dummy record
+                unsigned bal[P];
 #pragma unroll
-                    for (int q = 0; q < BUILD_P; ++q) {
-                        const real dx = me[q].x - pj.x, dy = me[q].y - pj.y, dz = me[q].z - pj.z;
-                        const real r2 = dx * dx + dy * dy + dz * dz;
-                        bool hit = r2 < thr_in && j != self0 + q;
-                        if (r2 >= thr_in && r2 < thr_out && j != self0 + q) {
-                            // guard band: decide with the exact definition
-                            const uint32_t scj = j >= h.sstart[sc0 + 2] ? sc0 + 2 : (j >= h.sstart[sc0 + 1] ? sc0 + 1 : sc0);
-                            const uint32_t gj = h.gstart[scj] + (j - h.sstart[scj]);
-                            hit = tile_exact_r2(pos, g, tc.g0 + p0 + q, gj) < rl2_exact;
-                        }
-                        bal[q] = __ballot_sync(0xffffffffu, hit);
+                for (int q = 0; q < P; ++q) {
+                    float t = fmaf(ax[q], pj.x, pj.w);
+                    t = fmaf(ay[q], pj.y, t);
+                    t = fmaf(az[q], pj.z, t);
+                    bal[q] = __ballot_sync(0xffffffffu, t < th[q]);
+                }
+                if (self0 + (P - 1) - base < 32u + (P - 1)) {  // this group of 32 holds some of the task's own particles
+#pragma unroll
+                    for (int q = 0; q < P; ++q) {
+                        const uint32_t d = self0 + q - base;
+                        if (d < 32u) bal[q] &= ~(1u << d);
+                    }
+                }
+                const uint16_t ent = (uint16_t)(j << tp.shift);
+#pragma unroll
+                for (int q = 0; q < P; ++q) {
+                    if (bal[q]) {
+                        const uint32_t o = cnt[q] + __popc(bal[q] & lt);
+                        if (((bal[q] >> lane) & 1u) && o < stride) rb[q * stride + o] = ent;
                         cnt[q] += __popc(bal[q]);
                     }
-                    if (lane < BUILD_P) {
-                        unsigned v = bal[0];
-#pragma unroll
-                        for (int q = 1; q < BUILD_P; ++q) v = lane == (unsigned)q ? bal[q] : v;
-                        wp[lane * wpp + k] = v;
-                    }
-                }
-                for (; k < (uint32_t)(run + 1) * wpr; ++k)
-                    if (lane < BUILD_P) wp[lane * wpp + k] = 0u;
-            }
-        }
-        if (lane < BUILD_P) {
-            uint32_t v = cnt[0];
-#pragma unroll
-            for (int q = 1; q < BUILD_P; ++q) v = lane == (unsigned)q ? cnt[q] : v;
-            counts[wid * BUILD_P + lane] = lane < np ? v : 0u;
-        }
-        __syncthreads();
-
-        // ---- row offsets of the chunk (rows padded to 8 entries = 16 bytes), one reservation per chunk
-        if (wid == 0) {
-            uint32_t carry = 0;
-            for (uint32_t base = 0; base < chunk; base += 32) {
-                const uint32_t c = base + lane < chunk ? counts[base + lane] : 0u;
-                const uint32_t v = (c + 7u) >> 3;
-                uint32_t inc = v;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const uint32_t u = __shfl_up_sync(0xffffffffu, inc, o);
-                    if ((int)lane >= o) inc += u;
-                }
-                if (base + lane < chunk) counts[base + lane] = (carry + inc - v) | (c << 20);  // offset | count
-                carry += __shfl_sync(0xffffffffu, inc, 31);
-            }
-            if (lane == 0) {
-                const unsigned long long tot = 8ull * carry;
-                const unsigned long long bb = atomicAdd(cursor, tot);
-                s_base = bb;
-                s_ok = (bb + tot <= capacity) ? 1u : 0u;  // no room: host sees cursor > capacity, grows, rebuilds
-            }
-        }
-        __syncthreads();
-
-        // ---- pass B: compacted write (Fig. 4 steps 4-8): warp per particle, lane per ballot word
-        if (s_ok && np > 0) {
-            const uint32_t sch = h.hc_sc[hc];
-            const uint32_t ixh = sch % tc.sx, iyh = (sch / tc.sx) % tc.sy, izh = sch / (tc.sx * tc.sy);
-            for (uint32_t q = 0; q < np; ++q) {
-                const uint32_t oc = counts[wid * BUILD_P + q];
-                const uint32_t off8 = oc & 0xfffffu, n_tot = oc >> 20;
-                const unsigned long long row0 = s_base + 8ull * off8;
-                uint16_t *row = nl16 + row0;
-                const uint32_t *wp = words + ((size_t)wid * BUILD_P + q) * wpp;
-                uint32_t carry = 0;
-                for (uint32_t wbase = 0; wbase < wpp; wbase += 32) {
-                    const uint32_t wi = wbase + lane;
-                    unsigned bits = wi < wpp ? wp[wi] : 0u;
-                    const uint32_t c = __popc(bits);
-                    uint32_t inc = c;
-#pragma unroll
-                    for (int o = 1; o < 32; o <<= 1) {
-                        const uint32_t u = __shfl_up_sync(0xffffffffu, inc, o);
-                        if ((int)lane >= o) inc += u;
-                    }
-                    uint32_t o = carry + inc - c;
-                    if (bits) {
-                        const uint32_t run = wi / wpr, k = wi - run * wpr;
-                        const uint32_t iy = iyh + (run % 3) - 1, iz = izh + (run / 3) - 1;
-                        const uint32_t sc0 = (ixh - 1) + tc.sx * (iy + tc.sy * iz);
-                        const uint32_t jb = h.sstart[sc0] + 32u * k;
-                        while (bits) {
-                            const uint32_t bpos = __ffs(bits) - 1;
-                            bits &= bits - 1;
-                            row[o++] = (uint16_t)(jb + bpos);
-                        }
-                    }
-                    carry += __shfl_sync(0xffffffffu, inc, 31);
-                }
-                const uint32_t padded = (n_tot + 7u) & ~7u;
-                if (n_tot + lane < padded) row[n_tot + lane] = (uint16_t)tc.n_staged;  // dummy record (far away)
-                if (lane == 0) {
-                    row_off[tc.g0 + p0 + q] = (uint32_t)(row0 >> 3);
-                    nl_cnt[tc.g0 + p0 + q] = n_tot;
                 }
             }
         }
-        __syncthreads();
+        __syncwarp();
+        // rows: pad to 8 entries with the dummy record, copy out with 16-byte stores
+#pragma unroll
+        for (int q = 0; q < P; ++q) {
+            if ((uint32_t)q < np) {
+                worst = max(worst, cnt[q]);
+                const uint32_t n = min(cnt[q], stride);
+                const uint32_t nv = (n + 7u) >> 3;
+                uint16_t *r = rb + q * stride;
+                if (lane < 8 && n + lane < 8 * nv) r[n + lane] = (uint16_t)dummy_ent;
+                __syncwarp();
+                uint4 *dst = (uint4 *)(nl16 + (size_t)(tc.g0 + p0 + q) * stride);
+                const uint4 *src = (const uint4 *)r;
+                for (uint32_t v = lane; v < nv; v += 32) dst[v] = src[v];
+                if (lane == 0) nl_cnt[tc.g0 + p0 + q] = n;
+                total += n;
+            }
+        }
+        __syncwarp();
+    }
+    if (lane == 0) {
+        if (total) atomicAdd(&flags->nl_total, total);
+        if (worst > stride) atomicMax(&flags->nl_overflow, worst);
     }
 }
 
@@ -434,9 +418,16 @@ struct LJTile {
     double thr_in, thr_out;  // rc^2 -+ guard
 };
 
-template <int W, bool MIXED, int ACC_BLOCK>
+// record referenced by a list entry: PRE = the entry is (staged index << 4), i.e. the byte offset of a float4 record
+template <typename R4, bool PRE>
+__device__ __forceinline__ R4 tile_rec(const R4 *rec, uint32_t ent)
+{
+    if (PRE) return *(const R4 *)((const char *)rec + (size_t)ent * (sizeof(R4) / 16));
+    return rec[ent];
+}
+
+template <int W, bool MIXED, int ACC_BLOCK, bool ENERGY, bool PRE>
 __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj(TileParams tp, Geom g, const double4 *__restrict__ pos,
-                                                            const uint32_t *__restrict__ row_off,
                                                             const uint32_t *__restrict__ nl_cnt,
                                                             const uint16_t *__restrict__ nl16, LJTile lj,
                                                             uint32_t max_staged, double4 *__restrict__ force)
@@ -446,10 +437,11 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj(TileParams tp, Geom 
     extern __shared__ __align__(16) char smem_raw[];
     const TileSmem h = tile_carve(smem_raw, tp.B);
     R4 *rec = (R4 *)h.rest;
+    uint8_t *scell = (uint8_t *)(h.rest + sizeof(R4) * (max_staged + 1));
 
     TileCtx tc;
     tile_setup(tp, g, blockIdx.x, h, tc);
-    tile_stage<R4, false>(g, tc, h, pos, nullptr, rec, nullptr);
+    tile_stage<R4, false>(g, tc, h, pos, nullptr, rec, nullptr, scell);
     __syncthreads();
 
     const unsigned lane = threadIdx.x & (W - 1);
@@ -457,47 +449,54 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj(TileParams tp, Geom 
     const uint32_t n_groups = blockDim.x / W;
     const real thr_in = (real)lj.thr_in, thr_out = (real)lj.thr_out;
     const real sig2 = (real)lj.sig2, eps24 = (real)lj.eps24, eps4 = (real)lj.eps4, uc = (real)lj.uc;
+    const uint32_t stride8 = tp.stride >> 3;
 
     for (uint32_t p = threadIdx.x / W; p < tc.n_home; p += n_groups) {
         const uint32_t hc = tile_home_cell(h, tc.n_hc, p);
         const R4 me = rec[tile_staged_of_home(h, hc, p)];
         const uint32_t cnt = nl_cnt[tc.g0 + p];
         const uint32_t nblk = (cnt + 7u) >> 3;
-        const uint4 *row = (const uint4 *)(nl16 + 8ull * row_off[tc.g0 + p]);
+        const uint4 *row = (const uint4 *)nl16 + (size_t)(tc.g0 + p) * stride8;
         double fx = 0.0, fy = 0.0, fz = 0.0, en = 0.0;
+        uint4 q = lane < nblk ? __ldg(row + lane) : make_uint4(0, 0, 0, 0);
         for (uint32_t b = lane; b < nblk; b += W) {
-            const uint4 q = __ldg(row + b);
+            const uint4 qn = b + W < nblk ? __ldg(row + b + W) : q;  // prefetch the next block of 8 entries
             const uint32_t qq[4] = {q.x, q.y, q.z, q.w};
             real ax = 0, ay = 0, az = 0, ae = 0;
 #pragma unroll
             for (int e = 0; e < 8; ++e) {
-                const uint32_t j = (qq[e >> 1] >> ((e & 1) * 16)) & 0xffffu;
-                const R4 pj = rec[j];
+                const uint32_t ent = (e & 1) ? (qq[e >> 1] >> 16) : (qq[e >> 1] & 0xffffu);
+                const R4 pj = tile_rec<R4, PRE>(rec, ent);
                 const real dx = me.x - pj.x, dy = me.y - pj.y, dz = me.z - pj.z;
                 const real r2 = dx * dx + dy * dy + dz * dz;
                 bool in = r2 < thr_in;
                 if (!in && r2 < thr_out) {  // guard band around rc^2: the plain fp64 definition decides (R26)
+                    const uint32_t j = PRE ? ent >> 4 : ent;
                     in = tile_exact_r2(pos, g, tc.g0 + p, tile_global_of_staged(h, tc.n_sc, j)) < lj.rc2_exact;
                 }
                 const real rinv2 = md_rcp(r2);
                 const real s2 = sig2 * rinv2;
                 const real s6 = s2 * s2 * s2;
                 real f = eps24 * s6 * ((real)2 * s6 - (real)1) * rinv2;
-                real u = (real)0.5 * (eps4 * s6 * (s6 - (real)1) - uc);
                 f = in ? f : (real)0;
-                u = in ? u : (real)0;
-                ax += f * dx; ay += f * dy; az += f * dz; ae += u;
+                ax += f * dx; ay += f * dy; az += f * dz;
+                if (ENERGY) {
+                    real u = (real)0.5 * (eps4 * s6 * (s6 - (real)1) - uc);
+                    ae += in ? u : (real)0;
+                }
                 if (MIXED && ((e + 1) % ACC_BLOCK == 0)) {  // widen the fp32 block sum, accumulate in fp64
-                    fx += (double)ax; fy += (double)ay; fz += (double)az; en += (double)ae;
-                    ax = ay = az = ae = 0;
+                    fx += (double)ax; fy += (double)ay; fz += (double)az;
+                    ax = ay = az = 0;
+                    if (ENERGY) { en += (double)ae; ae = 0; }
                 }
             }
             if (!MIXED) { fx += ax; fy += ay; fz += az; en += ae; }
+            q = qn;
         }
         fx = md_seg_sum<W>(fx, seg_mask);
         fy = md_seg_sum<W>(fy, seg_mask);
         fz = md_seg_sum<W>(fz, seg_mask);
-        en = md_seg_sum<W>(en, seg_mask);
+        if (ENERGY) en = md_seg_sum<W>(en, seg_mask);
         if (lane == 0) force[tc.g0 + p] = make_double4(fx, fy, fz, en);
     }
 }
@@ -513,7 +512,6 @@ struct DPDTile {
 template <int W>
 __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_dpd(TileParams tp, Geom g, const double4 *__restrict__ pos,
                                                              const double4 *__restrict__ vel,
-                                                             const uint32_t *__restrict__ row_off,
                                                              const uint32_t *__restrict__ nl_cnt,
                                                              const uint16_t *__restrict__ nl16, DPDTile dp,
                                                              uint32_t max_staged, double4 *__restrict__ force)
@@ -522,16 +520,19 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_dpd(TileParams tp, Geom
     const TileSmem h = tile_carve(smem_raw, tp.B);
     double4 *rec = (double4 *)h.rest;
     double4 *svel = rec + (max_staged + 1);
+    uint8_t *scell = (uint8_t *)(svel + (max_staged + 1));
 
     TileCtx tc;
     tile_setup(tp, g, blockIdx.x, h, tc);
-    tile_stage<double4, true>(g, tc, h, pos, vel, rec, svel);
+    tile_stage<double4, true>(g, tc, h, pos, vel, rec, svel, scell);
     if (threadIdx.x == 0) svel[tc.n_staged] = make_double4(0, 0, 0, 1);
     __syncthreads();
 
     const unsigned lane = threadIdx.x & (W - 1);
     const unsigned seg_mask = md_seg_mask<W>();
     const uint32_t n_groups = blockDim.x / W;
+    const uint32_t stride8 = tp.stride >> 3;
+    const uint32_t sh = tp.shift;
 
     for (uint32_t p = threadIdx.x / W; p < tc.n_home; p += n_groups) {
         const uint32_t hc = tile_home_cell(h, tc.n_hc, p);
@@ -541,14 +542,14 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_dpd(TileParams tp, Geom
         const uint32_t ti = md_lane_to_tag(me.w);
         const uint32_t cnt = nl_cnt[tc.g0 + p];
         const uint32_t nblk = (cnt + 7u) >> 3;
-        const uint4 *row = (const uint4 *)(nl16 + 8ull * row_off[tc.g0 + p]);
+        const uint4 *row = (const uint4 *)nl16 + (size_t)(tc.g0 + p) * stride8;
         double fx = 0.0, fy = 0.0, fz = 0.0, en = 0.0;
         for (uint32_t b = lane; b < nblk; b += W) {
             const uint4 q = __ldg(row + b);
             const uint32_t qq[4] = {q.x, q.y, q.z, q.w};
 #pragma unroll
             for (int e = 0; e < 8; ++e) {
-                const uint32_t j = (qq[e >> 1] >> ((e & 1) * 16)) & 0xffffu;
+                const uint32_t j = ((qq[e >> 1] >> ((e & 1) * 16)) & 0xffffu) >> sh;
                 const double4 pj = rec[j];
                 const double dx = me.x - pj.x, dy = me.y - pj.y, dz = me.z - pj.z;
                 const double r2 = dx * dx + dy * dy + dz * dz;
@@ -577,22 +578,48 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_dpd(TileParams tp, Geom
 }
 
 // ===============================================================================================================
-// decode the 16-bit tile list into the general 32-bit CSR (exports / parity read-back only)
+// decode the 16-bit tile list into the general 32-bit CSR (exports / parity read-back only).  The stored list is a
+// guard-band superset; here every entry is tested with the exact fp64 expression (R2) on the positions the
+// list was built from (pos_ref, the snapshot taken at the binning), so the exported list is the plain definition.
+// FILL = false: exact row lengths into cnt32;  FILL = true: global slots into nl_idx at nl_off.
 // ===============================================================================================================
-__global__ void k_tile_decode(TileParams tp, Geom g, const uint32_t *__restrict__ row_off,
-                              const uint32_t *__restrict__ nl_cnt, const uint16_t *__restrict__ nl16,
-                              const uint64_t *__restrict__ nl_off, uint32_t *nl_idx)
+template <bool FILL>
+__global__ void k_tile_decode(TileParams tp, Geom g, const double *__restrict__ pos_ref,
+                              const uint32_t *__restrict__ nl_cnt, const uint16_t *__restrict__ nl16, double rl2,
+                              uint32_t *__restrict__ cnt32, const uint64_t *__restrict__ nl_off, uint32_t *nl_idx)
 {
     extern __shared__ __align__(16) char smem_raw[];
     const TileSmem h = tile_carve(smem_raw, tp.B);
     TileCtx tc;
     tile_setup(tp, g, blockIdx.x, h, tc);
     const unsigned lane = threadIdx.x & 31u, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const unsigned lt = md_lanemask_lt();
     for (uint32_t p = wid; p < tc.n_home; p += nw) {
-        const uint32_t cnt = nl_cnt[tc.g0 + p];
-        const uint16_t *row = nl16 + 8ull * row_off[tc.g0 + p];
-        uint32_t *out = nl_idx + nl_off[tc.g0 + p];
-        for (uint32_t k = lane; k < cnt; k += 32) out[k] = tile_global_of_staged(h, tc.n_sc, row[k]);
+        const uint32_t gi = tc.g0 + p;
+        const uint32_t cnt = nl_cnt[gi];
+        const uint16_t *row = nl16 + (size_t)gi * tp.stride;
+        const double xi = pos_ref[3ull * gi], yi = pos_ref[3ull * gi + 1], zi = pos_ref[3ull * gi + 2];
+        uint32_t *out = FILL ? nl_idx + nl_off[gi] : nullptr;
+        uint32_t n = 0;
+        for (uint32_t k0 = 0; k0 < cnt; k0 += 32) {
+            const uint32_t k = k0 + lane;
+            bool keep = false;
+            uint32_t gj = 0;
+            if (k < cnt) {
+                const uint32_t s = (uint32_t)row[k] >> tp.shift;
+                if (s < tc.n_staged) {
+                    gj = tile_global_of_staged(h, tc.n_sc, s);
+                    const double dx = md_min_image(__dsub_rn(xi, pos_ref[3ull * gj]), g.L[0], g.h[0]);
+                    const double dy = md_min_image(__dsub_rn(yi, pos_ref[3ull * gj + 1]), g.L[1], g.h[1]);
+                    const double dz = md_min_image(__dsub_rn(zi, pos_ref[3ull * gj + 2]), g.L[2], g.h[2]);
+                    keep = md_r2_exact(dx, dy, dz) < rl2;
+                }
+            }
+            const unsigned bal = __ballot_sync(0xffffffffu, keep);
+            if (FILL && keep) out[n + __popc(bal & lt)] = gj;
+            n += __popc(bal);
+        }
+        if (!FILL && lane == 0) cnt32[gi] = n;
     }
 }
 
@@ -605,6 +632,8 @@ static TileParams make_tp(md_ctx *c)
     tp.B = c->tile_B;
     tp.nsc_max = (c->tile_B + 2) * (c->tile_B + 2) * (c->tile_B + 2);
     tp.n_tiles = c->n_tiles;
+    tp.stride = c->nl_stride;
+    tp.shift = c->nl_shift;
     tp.tile_cell_begin = c->tile_cell_begin;
     tp.tile_origin = c->tile_origin;
     tp.lin_of_rank = c->lin_of_rank;
@@ -614,7 +643,8 @@ static TileParams make_tp(md_ctx *c)
     return tp;
 }
 
-// bound on |r2_staged - r2_true| for staged coordinates of magnitude <= E, separations <= R (see file header)
+// bound on |r2_staged - r2_true| for staged coordinates of magnitude <= E per axis, separations <= R
+// direct form (force kernels): r2 = dx^2 + dy^2 + dz^2 on rounded coordinates
 static double guard_fp32(double E, double R)
 {
     const double u = 5.9604644775390625e-08;  // 2^-24
@@ -626,6 +656,15 @@ static double guard_fp64(double E, double R)
     const double u = 1.1102230246251565e-16;  // 2^-53
     const double delta = 6.0 * E * u + u * R;
     return 4.0 * (2.0 * 1.7320508075688772 * R * delta + 3.0 * delta * delta + 4.0 * u * R * R);
+}
+// dot-product form (build kernel): t = |b|^2 - 2 a.b, compared with thr - |a|^2, all fp32.  Coordinates are rounded
+// once (error E u each, i.e. <= 2 sqrt(3) R E u on r^2 as above); then |a|^2, |b|^2 (<= 3 E^2 each, 3 roundings), the
+// three FFMA of the dot product (partial sums <= 9 E^2) and the final subtraction each add <= u times their magnitude:
+// generously 40 E^2 u in total.
+static double guard_dot_fp32(double E, double R)
+{
+    const double u = 5.9604644775390625e-08;
+    return guard_fp32(E, R) + 40.0 * E * E * u;
 }
 static double tile_extent(md_ctx *c)
 {
@@ -639,6 +678,7 @@ static size_t tile_smem_common(md_ctx *c, size_t rec_bytes, bool with_vel)
     size_t s = tile_header_bytes(c->tile_B);
     s += rec_bytes * (c->tile_max_staged + 1);
     if (with_vel) s += sizeof(double4) * (c->tile_max_staged + 1);
+    s += (c->tile_max_staged + 16) & ~(size_t)15;  // staged-cell table of tile_stage
     return s;
 }
 
@@ -659,41 +699,55 @@ static int set_smem(md_ctx *c, K kernel, size_t bytes)
 
 static const size_t TILE_SMEM_LIMIT = 227 * 1024 - 64;
 
+// entries are pre-shifted byte offsets when every staged index (and the dummy) fits in 12 bits
+static uint32_t tile_shift(md_ctx *c) { return c->tile_max_staged + 1 < 4096 ? 4u : 0u; }
+
 // returns MD_OK and sets *fits = false if the largest tile does not fit in shared memory (caller falls back)
 int launch_tile_build(md_ctx *c, bool *fits)
 {
-    const bool f32 = c->precision == MD_MIXED;
     const uint32_t ms = c->tile_max_staged;
-    const uint32_t wpr = std::max(1u, (3 * c->h_flags->max_cell_count + 31) / 32);
     const int block = std::min(c->cfg[MD_K_NLIST].block, TILE_MAX_BLOCK);
-    const uint32_t chunk = (uint32_t)(block / 32) * BUILD_P;
-    size_t smem = tile_smem_common(c, f32 ? sizeof(float4) : sizeof(double4), false);
-    smem += sizeof(uint32_t) * chunk;                     // counts / row offsets
-    smem += sizeof(uint32_t) * (size_t)chunk * 9 * wpr;   // ballot words
-    // row offset and count share one word in the chunk scan: 20 bits of offset (units of 8), 12 bits of count
-    const bool packable = (uint64_t)chunk * ((27ull * c->h_flags->max_cell_count + 7) / 8) < (1u << 20) &&
-                          27ull * c->h_flags->max_cell_count < 4096;
-    *fits = smem <= TILE_SMEM_LIMIT && ms < 65535 && packable;
+    const uint32_t nw = (uint32_t)block / 32;
+    size_t smem = tile_smem_common(c, sizeof(float4), false);
+    smem += sizeof(uint16_t) * (size_t)nw * BUILD_P * c->nl_stride;  // row assembly buffers
+    *fits = smem <= TILE_SMEM_LIMIT && ms < 65535 && c->tile_B <= 4;
     if (!*fits) return MD_OK;
+    c->nl_shift = tile_shift(c);
     const double R = c->r_list * 1.001, E = tile_extent(c), rl2 = c->r_list * c->r_list;
-    MD_CUDA_CHECK(c, cudaMemsetAsync(&c->d_flags->cursor, 0, sizeof(unsigned long long), c->stream));
+    MD_CUDA_CHECK(c, cudaMemsetAsync(&c->d_flags->nl_total, 0, sizeof(unsigned long long), c->stream));
+    MD_CUDA_CHECK(c, cudaMemsetAsync(&c->d_flags->nl_overflow, 0, sizeof(unsigned int), c->stream));
     TileParams tp = make_tp(c);
-    if (f32) {
-        const double gd = guard_fp32(E, R);
-        MD_TRY(set_smem(c, k_tile_build<float4>, smem));
-        k_tile_build<float4><<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->pos, (float)(rl2 - gd), (float)(rl2 + gd), rl2, wpr, ms,
-                                                                    &c->d_flags->cursor, c->nl16_capacity, c->row_off, c->nl_cnt, c->nl16);
-    } else {
-        const double gd = guard_fp64(E, R);
-        MD_TRY(set_smem(c, k_tile_build<double4>, smem));
-        k_tile_build<double4><<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->pos, rl2 - gd, rl2 + gd, rl2, wpr, ms,
-                                                                     &c->d_flags->cursor, c->nl16_capacity, c->row_off, c->nl_cnt, c->nl16);
-    }
+    const double gd = guard_dot_fp32(E, R);
+    MD_TRY(set_smem(c, k_tile_build<BUILD_P>, smem));
+    k_tile_build<BUILD_P><<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->pos, (float)(rl2 + gd), ms, c->nl_cnt, c->nl16,
+                                                                 c->d_flags);
     MD_LAUNCH_CHECK(c);
     return MD_OK;
 }
 
-int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift)
+template <int W, bool MIXED, int ACC, bool ENERGY>
+static int launch_lj_pre(md_ctx *c, const TileParams &tp, const LJTile &p, int block, size_t smem)
+{
+    if (c->nl_shift) {
+        MD_TRY(set_smem(c, k_tile_lj<W, MIXED, ACC, ENERGY, true>, smem));
+        k_tile_lj<W, MIXED, ACC, ENERGY, true><<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->pos, c->nl_cnt, c->nl16, p,
+                                                                                     c->tile_max_staged, c->force);
+    } else {
+        MD_TRY(set_smem(c, k_tile_lj<W, MIXED, ACC, ENERGY, false>, smem));
+        k_tile_lj<W, MIXED, ACC, ENERGY, false><<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->pos, c->nl_cnt, c->nl16, p,
+                                                                                      c->tile_max_staged, c->force);
+    }
+    return MD_OK;
+}
+
+template <int W, bool MIXED, int ACC>
+static int launch_lj_energy(md_ctx *c, const TileParams &tp, const LJTile &p, int block, size_t smem, bool energy)
+{
+    if (energy) return launch_lj_pre<W, MIXED, ACC, true>(c, tp, p, block, smem);
+    return launch_lj_pre<W, MIXED, ACC, false>(c, tp, p, block, smem);
+}
+
+int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
 {
     LaunchCfg cf = c->cfg[MD_K_LJ];
     cf.block = std::min(cf.block, TILE_MAX_BLOCK);
@@ -716,19 +770,10 @@ int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift)
     TileParams tp = make_tp(c);
     MD_DISPATCH_W(cf.w, {
         if (mixed) {
-            if (c->acc_block == 1) {
-                MD_TRY(set_smem(c, k_tile_lj<W_, true, 1>, smem));
-                k_tile_lj<W_, true, 1><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->row_off, c->nl_cnt, c->nl16, p,
-                                                                               c->tile_max_staged, c->force);
-            } else {
-                MD_TRY(set_smem(c, k_tile_lj<W_, true, 8>, smem));
-                k_tile_lj<W_, true, 8><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->row_off, c->nl_cnt, c->nl16, p,
-                                                                               c->tile_max_staged, c->force);
-            }
+            if (c->acc_block == 1) MD_TRY((launch_lj_energy<W_, true, 1>(c, tp, p, cf.block, smem, energy)));
+            else MD_TRY((launch_lj_energy<W_, true, 8>(c, tp, p, cf.block, smem, energy)));
         } else {
-            MD_TRY(set_smem(c, k_tile_lj<W_, false, 8>, smem));
-            k_tile_lj<W_, false, 8><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->row_off, c->nl_cnt, c->nl16, p,
-                                                                            c->tile_max_staged, c->force);
+            MD_TRY((launch_lj_energy<W_, false, 8>(c, tp, p, cf.block, smem, energy)));
         }
     });
     MD_LAUNCH_CHECK(c);
@@ -755,7 +800,7 @@ int launch_tile_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uin
     TileParams tp = make_tp(c);
     MD_DISPATCH_W(cf.w, {
         MD_TRY(set_smem(c, k_tile_dpd<W_>, smem));
-        k_tile_dpd<W_><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->vel, c->row_off, c->nl_cnt, c->nl16, p,
+        k_tile_dpd<W_><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->vel, c->nl_cnt, c->nl16, p,
                                                                c->tile_max_staged, c->force);
     });
     MD_LAUNCH_CHECK(c);
@@ -768,10 +813,17 @@ bool tile_forces_fit(md_ctx *c, bool dpd)
     return tile_smem_common(c, rec, dpd) <= TILE_SMEM_LIMIT;
 }
 
-int launch_tile_decode(md_ctx *c)
+// pass 1 (fill = false): exact row lengths into cnt32; pass 2 (fill = true): slots into nl_idx at nl_off
+int launch_tile_decode(md_ctx *c, bool fill, uint32_t *cnt32)
 {
     const size_t smem = tile_header_bytes(c->tile_B);
-    k_tile_decode<<<c->n_tiles, 256, smem, c->stream>>>(make_tp(c), c->g, c->row_off, c->nl_cnt, c->nl16, c->nl_off, c->nl_idx);
+    const double rl2 = c->r_list * c->r_list;
+    if (fill)
+        k_tile_decode<true><<<c->n_tiles, 256, smem, c->stream>>>(make_tp(c), c->g, c->pos_ref, c->nl_cnt, c->nl16, rl2, nullptr,
+                                                                 c->nl_off, c->nl_idx);
+    else
+        k_tile_decode<false><<<c->n_tiles, 256, smem, c->stream>>>(make_tp(c), c->g, c->pos_ref, c->nl_cnt, c->nl16, rl2, cnt32,
+                                                                  nullptr, nullptr);
     MD_LAUNCH_CHECK(c);
     return MD_OK;
 }
