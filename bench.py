@@ -211,6 +211,10 @@ def run_ours(args):
     md.set_state(d_pos, d_vel)
     if w.bonds is not None:
         md.set_bonds(w.bonds)
+    for spec in args.launch:                       # e.g. --launch lj=256,4 nlist=768,32 (fixes a kernel's block, w)
+        name, val = spec.split("=")
+        blk, ww = (int(x) for x in val.split(","))
+        md.set_launch({v: k for k, v in B.KERNEL_NAMES.items()}[name], blk, ww)
     if not args.no_tune:
         md.tune(desc, False)
 
@@ -309,6 +313,7 @@ def main():
     ap.add_argument("--scale", type=float, default=1.0)
     ap.add_argument("--order", default="morton", choices=["lex", "morton", "hilbert"])
     ap.add_argument("--no-tune", action="store_true")
+    ap.add_argument("--launch", nargs="*", default=[], help="kernel=block,w (with --no-tune)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
