@@ -201,7 +201,7 @@ def run_ours(args):
     stream = torch.cuda.Stream()
     order = {"lex": B.MD_ORDER_LEX, "morton": B.MD_ORDER_MORTON, "hilbert": B.MD_ORDER_HILBERT}[args.order]
     md = B.MD(w.box, w.N, w.rc, w.r_buff, precision=precision, stream=stream.cuda_stream, order=order,
-              sched=B.MD_SCHED_HOST)
+              sched=B.MD_SCHED_SYNC if args.sync_sched else B.MD_SCHED_SPECULATIVE)
     desc = B.step_desc(w.kind, w.dt, w.params)
 
     # inputs resident in HBM before the timed region
@@ -281,7 +281,9 @@ def run_ours(args):
                        "l2": "inputs larger than L2 (neighbour list %.0f MB + state)" % (4e-6 * st1["nlist_entries"]),
                        "tps": world * args.steps / (ms_max * 1e-3) / world, "rebuild_period_k": k,
                        "mean_neighbors": nbar, "rebuilds": rebuilds, "dangerous_builds": st1["dangerous_builds"],
-                       "order": args.order, "sched": "host",
+                       "order": args.order, "sched": "sync" if args.sync_sched else "speculative",
+                       "speculative_forces": st1["speculative_forces"] - st0["speculative_forces"],
+                       "wasted_forces": st1["wasted_forces"] - st0["wasted_forces"],
                        "launch": {n: [v["block"], v["w"]] for n, v in st1["launch"].items()},
                        "stage_share_of_step": stage_share,
                        "step_bmin_bytes_per_particle": b_min,
@@ -313,6 +315,7 @@ def main():
     ap.add_argument("--scale", type=float, default=1.0)
     ap.add_argument("--order", default="morton", choices=["lex", "morton", "hilbert"])
     ap.add_argument("--no-tune", action="store_true")
+    ap.add_argument("--sync-sched", action="store_true", help="MD_SCHED_SYNC instead of the speculative scheduler")
     ap.add_argument("--launch", nargs="*", default=[], help="kernel=block,w (with --no-tune)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -63,8 +63,10 @@ typedef enum {
 #define MD_F_BONDS 4u
 
 /* scheduling of md_step */
-#define MD_SCHED_HOST 0  /* host reads the rebuild flag every step (one small D2H + stream sync per step) */
-#define MD_SCHED_GRAPH 1 /* one CUDA graph per step; rebuild inside a device-side conditional node */
+#define MD_SCHED_SYNC 0        /* the host waits for the rebuild flag of half 1 before it enqueues the forces */
+#define MD_SCHED_SPECULATIVE 1 /* default: forces are enqueued before the flag arrives whenever no rebuild is predicted
+                                  (PAPER.md:122); if the flag says "rebuild" they are discarded and evaluated again on
+                                  the new list.  Results are identical in both modes */
 
 typedef struct {
     uint32_t flags;      /* MD_F_* */
@@ -97,6 +99,8 @@ typedef struct {
     uint32_t launches;          /* kernel launches issued by this context since create (all entry points) */
     double stage_ms[MD_N_KERNELS];          /* with md_set_profiling(ctx,1): device time per stage (CUDA events on */
     uint64_t stage_launches[MD_N_KERNELS];  /* the context's stream), accumulated since profiling was switched on  */
+    uint64_t speculative_forces;            /* force evaluations enqueued before the rebuild flag was known ...     */
+    uint64_t wasted_forces;                 /* ... and how many of them were discarded because a rebuild was due    */
 } md_stats;
 
 /* ---- lifetime ------------------------------------------------------------------------------------------ */

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "csrc", "libb200md.so")
 MD_FP64, MD_MIXED = 0, 1
 MD_ORDER_LEX, MD_ORDER_MORTON, MD_ORDER_HILBERT = 0, 1, 2
 MD_F_LJ, MD_F_DPD, MD_F_BONDS = 1, 2, 4
-MD_SCHED_HOST, MD_SCHED_GRAPH = 0, 1
+MD_SCHED_SYNC, MD_SCHED_SPECULATIVE = 0, 1
 MD_OPT_TILE_BRICK, MD_OPT_ACC_BLOCK = 1, 2
 MD_N_KERNELS = 8
 MD_K_NLIST, MD_K_LJ, MD_K_DPD, MD_K_BONDS, MD_K_INTEGRATE, MD_K_CELLS = 0, 1, 2, 3, 4, 5
@@ -44,7 +44,8 @@ class md_stats(C.Structure):
                 ("mean_neighbors", C.c_double), ("dims", C.c_uint32 * 3), ("max_cell_count", C.c_uint32),
                 ("block", C.c_int32 * MD_N_KERNELS), ("w", C.c_int32 * MD_N_KERNELS),
                 ("tuned_us", C.c_float * MD_N_KERNELS), ("tuner_runs", C.c_uint32), ("launches", C.c_uint32),
-                ("stage_ms", C.c_double * MD_N_KERNELS), ("stage_launches", C.c_uint64 * MD_N_KERNELS)]
+                ("stage_ms", C.c_double * MD_N_KERNELS), ("stage_launches", C.c_uint64 * MD_N_KERNELS),
+                ("speculative_forces", C.c_uint64), ("wasted_forces", C.c_uint64)]
 
 
 class MDError(RuntimeError):
@@ -140,7 +141,7 @@ def step_desc(kind: str, dt: float, params: dict) -> md_step_desc:
 class MD:
     """One simulation context (md_ctx).  Methods are 1:1 with the C entry points (md_ prefix dropped)."""
 
-    def __init__(self, box, N, rc, r_buff, precision=MD_FP64, stream=None, order=MD_ORDER_MORTON, sched=MD_SCHED_HOST):
+    def __init__(self, box, N, rc, r_buff, precision=MD_FP64, stream=None, order=MD_ORDER_MORTON, sched=MD_SCHED_SPECULATIVE):
         self.L = load()
         self.N = int(N)
         b = (C.c_double * 3)(*[float(x) for x in np.broadcast_to(np.asarray(box, dtype=np.float64), (3,))])
@@ -265,7 +266,8 @@ class MD:
         st = md_stats()
         self._chk(self.L.md_get_stats(self.h, C.byref(st)), "md_get_stats")
         d = {k: getattr(st, k) for k in ("steps", "rebuilds", "dangerous_builds", "nlist_entries", "nlist_capacity",
-                                         "device_bytes", "mean_neighbors", "max_cell_count", "tuner_runs", "launches")}
+                                         "device_bytes", "mean_neighbors", "max_cell_count", "tuner_runs", "launches",
+                                         "speculative_forces", "wasted_forces")}
         d["dims"] = list(st.dims)
         d["stage_ms"] = {KERNEL_NAMES[k]: st.stage_ms[k] for k in KERNEL_NAMES}
         d["stage_launches"] = {KERNEL_NAMES[k]: st.stage_launches[k] for k in KERNEL_NAMES}

@@ -90,6 +90,28 @@ void prof_resolve(md_ctx *c)
     c->ev_pending.clear();
 }
 
+// folds the event pairs that have completed (no synchronisation), keeps the rest pending
+void prof_resolve_ready(md_ctx *c)
+{
+    size_t keep = 0;
+    for (size_t i = 0; i < c->ev_pending.size(); ++i) {
+        auto p = c->ev_pending[i];
+        if (cudaEventQuery(p.e1) == cudaSuccess) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, p.e0, p.e1) == cudaSuccess) {
+                c->stats.stage_ms[p.k] += ms;
+                c->stats.stage_launches[p.k]++;
+            } else cudaGetLastError();
+            c->ev_pool.push_back(p.e0);
+            c->ev_pool.push_back(p.e1);
+        } else {
+            cudaGetLastError();
+            c->ev_pending[keep++] = p;
+        }
+    }
+    c->ev_pending.resize(keep);
+}
+
 extern "C" int md_set_profiling(md_ctx *c, int on)
 {
     if (!c) return MD_EINVAL;
@@ -300,7 +322,7 @@ extern "C" int md_create(md_ctx **out, const double box[3], uint64_t N, double r
     c->r_list = rc + r_buff;
     c->precision = MD_FP64;
     c->order = MD_ORDER_LEX;
-    c->sched = MD_SCHED_HOST;
+    c->sched = MD_SCHED_SPECULATIVE;
     c->stream = 0;
     c->log = getenv("B200MD_LOG") != nullptr;
     uint64_t ncell = 1;
@@ -365,7 +387,7 @@ extern "C" int md_configure(md_ctx *c, int precision, void *stream, int order, i
 {
     if (!c) return MD_EINVAL;
     if ((precision != MD_FP64 && precision != MD_MIXED) || order < 0 || order > MD_ORDER_HILBERT ||
-        (sched != MD_SCHED_HOST && sched != MD_SCHED_GRAPH)) {
+        (sched != MD_SCHED_SYNC && sched != MD_SCHED_SPECULATIVE)) {
         c->err = "md_configure: bad argument";
         return MD_EINVAL;
     }
@@ -387,6 +409,7 @@ extern "C" int md_destroy(md_ctx *c)
     prof_resolve(c);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     for (auto &p : c->allocs) cudaFree(p.first);
+    if (c->ev_flags) cudaEventDestroy(c->ev_flags);
     if (c->h_flags) cudaFreeHost(c->h_flags);
     cudaGetLastError();
     delete c;
@@ -488,6 +511,8 @@ static int do_build_cells(md_ctx *c)
     MD_TRY(launch_build_cells(c));
     c->cells_valid = true;
     c->nlist_valid = false;
+    c->steps_since_build = 0;
+    c->last_d2 = 0.f;
     MD_CUDA_CHECK(c, cudaMemsetAsync(&c->d_flags->rebuild, 0, 2 * sizeof(int), c->stream));
     return MD_OK;
 }
@@ -729,7 +754,8 @@ extern "C" int md_integrate_nve(md_ctx *c, double dt, int half)
     if (half == 1) {
         if (!c->cells_valid) MD_TRY(do_build_cells(c));  // the displacement check needs the reference snapshot
         ProfScope ps(c, MD_K_INTEGRATE);
-        MD_TRY(launch_half1(c, dt));
+        MD_TRY(launch_half1(c, dt, false));
+        c->steps_since_build++;
         c->force_valid = false;
         return MD_OK;
     }
@@ -783,31 +809,66 @@ static int rebuild(md_ctx *c)
     return do_build_nlist(c);
 }
 
+// Step loop.  The displacement criterion is decided on the device by half 1; the host needs the flag to
+// know whether to enqueue a rebuild.  As in the paper (forces are computed speculatively while the
+// criterion is being checked) the force kernels are enqueued BEFORE the host waits for the flag whenever a rebuild
+// is not expected at this step, so the device never idles on the round trip; if the flag then says "rebuild", the
+// speculative forces are discarded and evaluated again on the new list.  Whether a rebuild is expected is predicted
+// from the largest displacement of the previous step and its observed growth per step; a wrong prediction costs time
+// only, never correctness (the flag is always read before the forces are used).  Inside the loop the second
+// half-kick of a step and the first of the next are one launch (bit-identical to the two separate kernels).
 extern "C" int md_step(md_ctx *c, const md_step_desc *w, uint64_t n_steps)
 {
     if (!c || !w) return MD_EINVAL;
     if (!c->have_state) { c->err = "md_step: md_set_state first"; return MD_ESTATE; }
     if (!(w->dt > 0.0)) { c->err = "md_step: dt must be positive"; return MD_EINVAL; }
+    if (n_steps == 0) return MD_OK;
     if (!c->nlist_valid) MD_TRY(rebuild(c));
     if (!c->force_valid) MD_TRY(eval_forces(c, w, c->step, false));  // R16: F(t0) before the first half-kick
+    if (!c->ev_flags) MD_CUDA_CHECK(c, cudaEventCreateWithFlags(&c->ev_flags, cudaEventDisableTiming));
+    const double thr2 = 0.25 * c->r_buff * c->r_buff;
     for (uint64_t s = 0; s < n_steps; ++s) {
-        {
+        if (s == 0) {
             ProfScope ps(c, MD_K_INTEGRATE);
-            MD_TRY(launch_half1(c, w->dt));
+            MD_TRY(launch_half1(c, w->dt, false));
         }
-        MD_TRY(md_read_flags(c));
+        c->steps_since_build++;
+        MD_CUDA_CHECK(c, cudaMemcpyAsync(c->h_flags, c->d_flags, sizeof(DevFlags), cudaMemcpyDeviceToHost, c->stream));
+        MD_CUDA_CHECK(c, cudaEventRecord(c->ev_flags, c->stream));
+        // predicted largest displacement of this step: last one seen + the observed growth per step (with margin)
+        const double d_prev = sqrt((double)c->last_d2);
+        const bool speculate = c->sched != MD_SCHED_SYNC && d_prev + 1.5 * c->d2_rate < 0.5 * c->r_buff;
+        if (speculate) {
+            MD_TRY(eval_forces(c, w, c->step + 1, false));  // R15: hash counter = index of the step being completed
+            c->stats.speculative_forces++;
+        }
+        MD_CUDA_CHECK(c, cudaEventSynchronize(c->ev_flags));
+        if (c->profiling) prof_resolve_ready(c);
+        {
+            float d2;
+            memcpy(&d2, &c->h_flags->max_d2[c->d2_slot], sizeof(float));
+            c->last_d2 = d2;
+            const double d = sqrt((double)d2);
+            if (c->steps_since_build > 0) c->d2_rate = d / (double)c->steps_since_build;
+        }
         if (c->h_flags->rebuild) {
             if (c->h_flags->dangerous) c->stats.dangerous_builds++;
+            if (speculate) c->stats.wasted_forces++;
             MD_TRY(rebuild(c));
+            MD_TRY(eval_forces(c, w, c->step + 1, false));
+        } else if (!speculate) {
+            MD_TRY(eval_forces(c, w, c->step + 1, false));
         }
-        MD_TRY(eval_forces(c, w, c->step + 1, false));  // R15: hash counter = index of the step being completed
+        (void)thr2;
         {
             ProfScope ps(c, MD_K_INTEGRATE);
-            MD_TRY(launch_half2(c, w->dt));
+            if (s + 1 < n_steps) MD_TRY(launch_half1(c, w->dt, true));  // half 2 of this step + half 1 of the next
+            else MD_TRY(launch_half2(c, w->dt));
         }
         c->step++;
         c->stats.steps++;
     }
+    c->force_valid = true;
     return MD_OK;
 }
 

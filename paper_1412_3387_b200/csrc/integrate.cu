@@ -1,39 +1,52 @@
 // integrate.cu -- S6 velocity-Verlet NVE (R7) and S3 displacement check.
 #include "md_device.cuh"
 
-// half 1: v += (dt/2) F/m ; x += dt v ; wrap ; displacement since the last binning vs (r_buff/2)^2
+// half 1: v += (dt/2) F/m ; x += dt v ; wrap ; displacement since the last binning vs (r_buff/2)^2.
+// FUSED: the second half-kick of the previous step is applied first (same force, same operations in the same order
+// as k_half2 followed by k_half1, so the result is bit-identical to the two separate launches).
+// The largest squared displacement of the step goes to flags->max_d2[slot] (float bits; the host uses it to
+// predict the step at which the criterion will fire, see md_step); the other slot is cleared for the next step.
+template <bool FUSED>
 __global__ void k_half1(double4 *__restrict__ pos, double4 *__restrict__ vel, const double4 *__restrict__ force,
                         int *__restrict__ image, const double *__restrict__ pos_ref, Geom g, double dt, double half_dt,
-                        double thr2, double danger2, DevFlags *flags)
+                        double thr2, double danger2, DevFlags *flags, int slot)
 {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= g.N) return;
-    double4 p = pos[i];
-    double4 v = vel[i];
-    const double4 f = force[i];
-    const double m = v.w;
-    double x[3] = {p.x, p.y, p.z};
-    double u[3] = {v.x, v.y, v.z};
-    const double ff[3] = {f.x, f.y, f.z};
-    double d2 = 0.0;
+    float d2f = 0.f;
+    if (i < g.N) {
+        double4 p = pos[i];
+        double4 v = vel[i];
+        const double4 f = force[i];
+        const double m = v.w;
+        double x[3] = {p.x, p.y, p.z};
+        double u[3] = {v.x, v.y, v.z};
+        const double ff[3] = {f.x, f.y, f.z};
+        double d2 = 0.0;
 #pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        // same operation order as the definition: v + ((dt/2) F)/m ; x + dt v   (no FMA: positions parity 1e-12
-        // does not need it, but it keeps single steps bit-comparable with a plain CPU evaluation)
-        u[a] = __dadd_rn(u[a], __ddiv_rn(__dmul_rn(half_dt, ff[a]), m));
-        double xn = __dadd_rn(x[a], __dmul_rn(dt, u[a]));
-        if (xn >= g.h[a]) { xn = __dsub_rn(xn, g.L[a]); image[3ull * i + a] += 1; }
-        else if (xn < -g.h[a]) { xn = __dadd_rn(xn, g.L[a]); image[3ull * i + a] -= 1; }
-        x[a] = xn;
-        const double d = md_min_image(__dsub_rn(xn, pos_ref[3ull * i + a]), g.L[a], g.h[a]);
-        d2 = a == 0 ? __dmul_rn(d, d) : __dadd_rn(d2, __dmul_rn(d, d));
+        for (int a = 0; a < 3; ++a) {
+            // same operation order as the definition: v + ((dt/2) F)/m ; x + dt v   (no FMA: positions parity 1e-12
+            // does not need it, but it keeps single steps bit-comparable with a plain CPU evaluation)
+            const double kick = __ddiv_rn(__dmul_rn(half_dt, ff[a]), m);
+            if (FUSED) u[a] = __dadd_rn(u[a], kick);
+            u[a] = __dadd_rn(u[a], kick);
+            double xn = __dadd_rn(x[a], __dmul_rn(dt, u[a]));
+            if (xn >= g.h[a]) { xn = __dsub_rn(xn, g.L[a]); image[3ull * i + a] += 1; }
+            else if (xn < -g.h[a]) { xn = __dadd_rn(xn, g.L[a]); image[3ull * i + a] -= 1; }
+            x[a] = xn;
+            const double d = md_min_image(__dsub_rn(xn, pos_ref[3ull * i + a]), g.L[a], g.h[a]);
+            d2 = a == 0 ? __dmul_rn(d, d) : __dadd_rn(d2, __dmul_rn(d, d));
+        }
+        pos[i] = make_double4(x[0], x[1], x[2], p.w);
+        vel[i] = make_double4(u[0], u[1], u[2], m);
+        if (d2 > thr2) {
+            flags->rebuild = 1;  // benign race: every writer stores the same value
+            if (d2 > danger2) flags->dangerous = 1;
+        }
+        d2f = __double2float_ru(d2);
     }
-    pos[i] = make_double4(x[0], x[1], x[2], p.w);
-    vel[i] = make_double4(u[0], u[1], u[2], m);
-    if (d2 > thr2) {
-        flags->rebuild = 1;  // benign race: every writer stores the same value
-        if (d2 > danger2) flags->dangerous = 1;
-    }
+    const unsigned wmax = __reduce_max_sync(0xffffffffu, __float_as_uint(d2f));  // non-negative floats order as uints
+    if ((threadIdx.x & 31u) == 0 && wmax > flags->max_d2[slot]) atomicMax(&flags->max_d2[slot], wmax);
+    if (i == 0) flags->max_d2[slot ^ 1] = 0u;
 }
 
 __global__ void k_half2(double4 *__restrict__ vel, const double4 *__restrict__ force, uint32_t N, double half_dt)
@@ -48,12 +61,19 @@ __global__ void k_half2(double4 *__restrict__ vel, const double4 *__restrict__ f
     vel[i] = v;
 }
 
-int launch_half1(md_ctx *c, double dt)
+int launch_half1(md_ctx *c, double dt, bool fused)
 {
     const LaunchCfg &cf = c->cfg[MD_K_INTEGRATE];
     const double t = 0.5 * c->r_buff;
-    k_half1<<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->pos, c->vel, c->force, c->image, c->pos_ref, c->g, dt,
-                                                                0.5 * dt, t * t, c->r_buff * c->r_buff, c->d_flags);
+    c->d2_slot ^= 1;
+    if (fused)
+        k_half1<true><<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->pos, c->vel, c->force, c->image, c->pos_ref, c->g,
+                                                                         dt, 0.5 * dt, t * t, c->r_buff * c->r_buff,
+                                                                         c->d_flags, c->d2_slot);
+    else
+        k_half1<false><<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->pos, c->vel, c->force, c->image, c->pos_ref, c->g,
+                                                                          dt, 0.5 * dt, t * t, c->r_buff * c->r_buff,
+                                                                          c->d_flags, c->d2_slot);
     MD_LAUNCH_CHECK(c);
     return MD_OK;
 }

@@ -48,6 +48,8 @@ struct DevFlags {
     unsigned long long nl_total;  // entries of the list being built (general path: padded rows; tile path: sum of row lengths)
     unsigned int nl_overflow;     // tile build: longest row if it exceeds the row stride (host grows the stride, rebuilds)
     unsigned int pad2;
+    unsigned int max_d2[2];       // float bits of the largest squared displacement since the last binning, written by
+                                  // half 1 into the slot of the step's parity (the other slot is cleared)
 };
 
 struct LaunchCfg {
@@ -124,6 +126,11 @@ struct md_ctx {
     uint64_t last_force_step = 0;
     bool last_from_step = false;
     uint64_t step = 0;
+    int d2_slot = 0;                 // DevFlags::max_d2 slot of the last half 1
+    float last_d2 = 0.f;             // largest squared displacement seen at the last flag read-back
+    double d2_rate = 0.0;            // observed growth of the largest displacement per step (rebuild predictor)
+    uint64_t steps_since_build = 0;  // half-1 steps since the last binning
+    cudaEvent_t ev_flags = nullptr;  // recorded after the asynchronous flag read-back of md_step
     md_stats stats;
     LaunchCfg cfg[MD_N_KERNELS];
     bool tuned = false;
@@ -146,6 +153,7 @@ struct ProfScope {
     ProfScope(md_ctx *ctx, int kernel);
     ~ProfScope();
 };
+void prof_resolve_ready(md_ctx *c);  // no sync: folds the pairs that have completed
 void prof_resolve(md_ctx *c);  // call after a stream sync: folds finished event pairs into stats
 
 // ---- helpers (api.cu) -----------------------------------------------------------------------------------
@@ -167,7 +175,7 @@ int launch_nlist_fill(md_ctx *c);
 int launch_forces_lj(md_ctx *c, double eps, double sigma, int shift);
 int launch_forces_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed);
 int launch_forces_bonds(md_ctx *c, double k, double r0);
-int launch_half1(md_ctx *c, double dt);
+int launch_half1(md_ctx *c, double dt, bool fused);  // fused: preceded by the previous step's half 2
 int launch_half2(md_ctx *c, double dt);
 int launch_export_pairs_count(md_ctx *c, uint32_t *cnt);
 int launch_export_pairs_fill(md_ctx *c, const uint64_t *off, uint32_t *pairs);
