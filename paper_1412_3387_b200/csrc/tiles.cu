@@ -26,12 +26,15 @@
 // Force kernels take the r < rc decision on the staged coordinates only outside a guard band around rc^2; inside
 // the band the pair is re-tested with the exact fp64 expression on the global positions (R26).
 #include <algorithm>
+#include <cstdlib>
 #include <type_traits>
 
 #include "md_device.cuh"
 
 constexpr int TILE_MAX_BLOCK = 512;  // __launch_bounds__ of the tile kernels (up to 128 registers per thread)
 constexpr int BUILD_P = 4;           // home particles per warp task in the build kernel
+constexpr uint32_t N_DUMMY = 8;      // far-away dummy records after the staged ones, one per bank class (row padding)
+constexpr uint32_t RB_EXTRA = 96;    // build kernel: row assembly buffers hold this many entries more than a stored row
 
 struct TileParams {
     uint32_t B;        // brick edge in cells
@@ -211,7 +214,7 @@ template <> struct RecTraits<double4> {
 template <typename R4, bool WITH_VEL>
 __device__ __forceinline__ void tile_stage(const Geom &g, const TileCtx &tc, const TileSmem &h,
                                            const double4 *__restrict__ pos, const double4 *__restrict__ vel, R4 *rec,
-                                           double4 *svel, uint8_t *scell)
+                                           double4 *svel, uint8_t *scell, double scale = 1.0)
 {
     const uint32_t lane = threadIdx.x & 31u, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     for (uint32_t sc = wid; sc < tc.n_sc; sc += nw) {
@@ -227,10 +230,10 @@ __device__ __forceinline__ void tile_stage(const Geom &g, const TileCtx &tc, con
         const double x = cg[3] + md_min_image(p.x - cg[0], g.L[0], g.h[0]);
         const double y = cg[4] + md_min_image(p.y - cg[1], g.L[1], g.h[1]);
         const double z = cg[5] + md_min_image(p.z - cg[2], g.L[2], g.h[2]);
-        rec[s] = RecTraits<R4>::make(x, y, z, p.w);
+        rec[s] = RecTraits<R4>::make(x * scale, y * scale, z * scale, p.w);
         if (WITH_VEL) svel[s] = vel[gi];
     }
-    if (threadIdx.x == 0) rec[tc.n_staged] = RecTraits<R4>::far();  // dummy record: row padding, out-of-run lanes
+    if (threadIdx.x < N_DUMMY) rec[tc.n_staged + threadIdx.x] = RecTraits<R4>::far();  // dummy records: row padding
 }
 
 // the plain definition on global (wrapped) positions: exact fp64, no FMA (R2, R8)
@@ -291,8 +294,9 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build(TileParams tp, Ge
     const TileSmem h = tile_carve(smem_raw, tp.B);
     float4 *rec = (float4 *)h.rest;
     const uint32_t nw = blockDim.x >> 5;
-    uint16_t *rowbuf = (uint16_t *)(h.rest + sizeof(float4) * (max_staged + 1));  // [nw][P][stride], 16-byte aligned
-    uint8_t *scell = (uint8_t *)(rowbuf + (size_t)nw * P * tp.stride);            // [max_staged]
+    uint16_t *rowbuf = (uint16_t *)(h.rest + sizeof(float4) * (max_staged + N_DUMMY));  // [nw][P][stride + RB_EXTRA]
+    uint32_t *scratch = (uint32_t *)(rowbuf + (size_t)nw * P * (tp.stride + RB_EXTRA));  // [nw][P][24]
+    uint8_t *scell = (uint8_t *)(scratch + nw * P * 24);                                 // [max_staged]
 
     TileCtx tc;
     tile_setup(tp, g, blockIdx.x, h, tc);
@@ -317,9 +321,13 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build(TileParams tp, Ge
     const unsigned lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;
     const unsigned lt = md_lanemask_lt();
     const uint32_t n_tasks = h.hc_task[tc.n_hc];
-    const uint32_t stride = tp.stride;
-    const uint32_t dummy_ent = tc.n_staged << tp.shift;
-    uint16_t *rb = rowbuf + (size_t)wid * P * stride;
+    const uint32_t stride = tp.stride, rcap = tp.stride + RB_EXTRA;
+    // bank classes (see the layout note above k_tile_lj3): candidates are visited in groups of 32 aligned to 8 staged
+    // indices, so the class (staged index & 7) of a lane's candidate is the constant lane & 7
+    const uint32_t cls = lane & 7u;
+    const unsigned cmask_lt = (0x01010101u << cls) & lt, cmask = 0x01010101u << cls;
+    uint16_t *rb = rowbuf + (size_t)wid * P * rcap;
+    uint32_t *scr = scratch + wid * P * 24;  // per warp and row: n_c[8], first hole H_c[8], first overflow entry O_c[8]
     unsigned long long total = 0;
     uint32_t worst = 0;
 
@@ -341,13 +349,13 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build(TileParams tp, Ge
         const uint32_t self0 = h.sstart[sch] + (p0 - h.hc_first[hc]);
         // hit <=> |b|^2 - 2 a.b < thr - |a|^2
         float ax[P], ay[P], az[P], th[P];
-        uint32_t cnt[P];
+        uint32_t cntc[P];  // entries of this lane's class found so far, per home particle
 #pragma unroll
         for (int q = 0; q < P; ++q) {
             const float4 m = rec[self0 + min((uint32_t)q, np - 1)];
             ax[q] = -2.f * m.x; ay[q] = -2.f * m.y; az[q] = -2.f * m.z;
             th[q] = (uint32_t)q < np ? thr_out - m.w : -3e38f;  // absent particles never hit
-            cnt[q] = 0;
+            cntc[q] = 0;
         }
 #pragma unroll 1
         for (int run = 0; run < 9; ++run) {
@@ -355,9 +363,9 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build(TileParams tp, Ge
             const uint32_t sc0 = (ixh - 1) + tc.sx * (iy + tc.sy * iz);
             const uint32_t b = h.sstart[sc0], e = h.sstart[sc0 + 3];
 #pragma unroll 1
-            for (uint32_t base = b; base < e; base += 32) {
+            for (uint32_t base = b & ~7u; base < e; base += 32) {
                 const uint32_t j = base + lane;
-                const float4 pj = rec[j < e ? j : tc.n_staged];  // past the run: the far-away dummy record
+                const float4 pj = rec[(j >= b && j < e) ? j : tc.n_staged];  // outside the run: a far-away dummy record
                 unsigned bal[P];
 #pragma unroll
                 for (int q = 0; q < P; ++q) {
@@ -377,37 +385,92 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build(TileParams tp, Ge
 #pragma unroll
                 for (int q = 0; q < P; ++q) {
                     if (bal[q]) {
-                        const uint32_t o = cnt[q] + __popc(bal[q] & lt);
-                        if (((bal[q] >> lane) & 1u) && o < stride) rb[q * stride + o] = ent;
-                        cnt[q] += __popc(bal[q]);
+                        // k-th entry of class c goes to block k, slot (c - k - rot) & 7 (Fig. 4 steps 4-7 per class)
+                        const uint32_t k = cntc[q] + __popc(bal[q] & cmask_lt);
+                        const uint32_t o = 8u * k + ((cls - k - 4u * ((p0 + q) & 1u)) & 7u);
+                        if (((bal[q] >> lane) & 1u) && o < rcap) rb[q * rcap + o] = ent;
+                        cntc[q] += __popc(bal[q] & cmask);
                     }
                 }
             }
         }
         __syncwarp();
-        // rows: pad to 8 entries with the dummy record, copy out with 16-byte stores
+        // finish the P = 4 rows together: lane = 8 * row + class
+        {
+            static_assert(P == 4, "row finishing maps 8 lanes (bank classes) to each of 4 rows");
+            const uint32_t qr = lane >> 3;
+            const bool live = qr < np;
+            uint32_t nc = cntc[0];
+            nc = qr == 1 ? cntc[1] : nc;
+            nc = qr == 2 ? cntc[2] : nc;
+            nc = qr == 3 ? cntc[3] : nc;
+            if (!live) nc = 0;
+            const uint32_t rot = 4u * ((p0 + qr) & 1u);
+            uint32_t n = nc, mx = nc;
 #pragma unroll
-        for (int q = 0; q < P; ++q) {
-            if ((uint32_t)q < np) {
-                worst = max(worst, cnt[q]);
-                const uint32_t n = min(cnt[q], stride);
-                const uint32_t nv = (n + 7u) >> 3;
-                uint16_t *r = rb + q * stride;
-                if (lane < 8 && n + lane < 8 * nv) r[n + lane] = (uint16_t)dummy_ent;
-                __syncwarp();
+            for (int o = 1; o < 8; o <<= 1) {
+                n += __shfl_xor_sync(0xffffffffu, n, o);
+                mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+            }
+            // row length in blocks of 8; a class longer than the assembly buffer lost entries -> overflow
+            uint32_t need = (n + 7u) & ~7u;
+            if (8u * mx > rcap) need = max(need, 8u * mx - RB_EXTRA);
+            worst = max(worst, need);
+            const uint32_t nblk = min((n + 7u) >> 3, stride >> 3);
+            uint16_t *r = rb + qr * rcap;
+            // holes (class shorter than the row) take the entries of longer classes, then dummies of their class
+            const uint32_t nck = min(nc, rcap >> 3);
+            const uint32_t holes = nblk > nck ? nblk - nck : 0u, over = nck > nblk ? nck - nblk : 0u;
+            uint32_t hs = holes, os = over;
+#pragma unroll
+            for (int o = 1; o < 8; o <<= 1) {
+                const uint32_t a = __shfl_up_sync(0xffffffffu, hs, o, 8), bb = __shfl_up_sync(0xffffffffu, os, o, 8);
+                if ((int)cls >= o) { hs += a; os += bb; }
+            }
+            const uint32_t n_holes = __shfl_sync(0xffffffffu, hs, 7, 8), n_over = __shfl_sync(0xffffffffu, os, 7, 8);
+            uint32_t *sc = scr + 24 * qr;
+            sc[cls] = nck;
+            sc[8 + cls] = hs - holes;
+            sc[16 + cls] = os - over;
+            __syncwarp();
+            for (uint32_t o = cls; o < n_holes; o += 8) {
+                uint32_t c = 0;
+#pragma unroll
+                for (int k = 1; k < 8; ++k) c += o >= sc[8 + k] ? 1u : 0u;
+                // classes without holes share their successor's start: the count above lands on the last class whose
+                // first hole is <= o, which is the one that owns hole o
+                const uint32_t bk = sc[c] + (o - sc[8 + c]);
+                uint16_t v;
+                if (o < n_over) {
+                    uint32_t cs = 0;
+#pragma unroll
+                    for (int k = 1; k < 8; ++k) cs += o >= sc[16 + k] ? 1u : 0u;
+                    const uint32_t k2 = nblk + (o - sc[16 + cs]);
+                    v = r[8u * k2 + ((cs - k2 - rot) & 7u)];
+                } else {
+                    v = (uint16_t)((tc.n_staged + ((c - tc.n_staged) & 7u)) << tp.shift);
+                }
+                r[8u * bk + ((c - bk - rot) & 7u)] = v;
+            }
+            __syncwarp();
+#pragma unroll
+            for (int q = 0; q < P; ++q) {
+                const uint32_t nb = __shfl_sync(0xffffffffu, nblk, 8 * q);
                 uint4 *dst = (uint4 *)(nl16 + (size_t)(tc.g0 + p0 + q) * stride);
-                const uint4 *src = (const uint4 *)r;
-                for (uint32_t v = lane; v < nv; v += 32) dst[v] = src[v];
-                if (lane == 0) nl_cnt[tc.g0 + p0 + q] = n;
+                const uint4 *src = (const uint4 *)(rb + q * rcap);
+                for (uint32_t v = lane; v < nb; v += 32) dst[v] = src[v];
+            }
+            if (live && cls == 0) {
+                nl_cnt[tc.g0 + p0 + qr] = min(n, 8u * nblk);
                 total += n;
             }
         }
         __syncwarp();
     }
-    if (lane == 0) {
-        if (total) atomicAdd(&flags->nl_total, total);
-        if (worst > stride) atomicMax(&flags->nl_overflow, worst);
-    }
+    total += __shfl_xor_sync(0xffffffffu, total, 8);
+    total += __shfl_xor_sync(0xffffffffu, total, 16);
+    if (lane == 0 && total) atomicAdd(&flags->nl_total, total);
+    if (worst > stride) atomicMax(&flags->nl_overflow, worst);
 }
 
 // ===============================================================================================================
@@ -437,7 +500,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj(TileParams tp, Geom 
     extern __shared__ __align__(16) char smem_raw[];
     const TileSmem h = tile_carve(smem_raw, tp.B);
     R4 *rec = (R4 *)h.rest;
-    uint8_t *scell = (uint8_t *)(h.rest + sizeof(R4) * (max_staged + 1));
+    uint8_t *scell = (uint8_t *)(h.rest + sizeof(R4) * (max_staged + N_DUMMY));
 
     TileCtx tc;
     tile_setup(tp, g, blockIdx.x, h, tc);
@@ -502,6 +565,203 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj(TileParams tp, Geom 
 }
 
 // ===============================================================================================================
+// S4a, mixed precision, the bench path: k_tile_lj3
+//
+// Row layout written by k_tile_build: a row is a sequence of blocks of 8 entries; slot e of block b of the row of
+// tile-local home particle p holds a record whose staged index s has bank class  s & 7 == (e + b + 4 (p & 1)) & 7
+// (a real neighbour, or the dummy record of that class); the few entries of classes longer than the row sit in
+// holes of shorter classes.  A float4 record is 16 bytes, so the class is the 16-byte bank group of the record, and
+// an LDS.128 is served one quarter-warp (8 lanes) per wavefront when the 8 records lie in 8 different groups.
+// With W = 4 the lanes of a quarter-warp hold blocks b..b+3 of an even particle and b..b+3 of the next (odd) one,
+// with W >= 8 they hold 8 consecutive blocks of one particle: at unrolled slot e the 8 records have the 8 different
+// classes (e + b' + ...) & 7 -> the gather is conflict-free except for the relocated entries.
+//
+// Arithmetic (R1, R25, R26): coordinates are staged divided by sigma, so s2 = 1/r'^2; per pair
+// g = (s6 - 1/2) s8 and F_i = (48 eps / sigma) sum_j g d'_ij.  The r < rc decision: d = r'^2 - rc'^2 in fp32; |d| >= guard
+// decides by sign; a block of 8 entries in which some |d| < guard is re-evaluated with the exact fp64 test.
+// 8 contributions are summed in fp32, the block sum is widened and accumulated in fp64 (MD_OPT_ACC_BLOCK = 8).
+// ===============================================================================================================
+struct LJ3 {
+    double rc2_exact;     // rc^2 in box units (exact re-test)
+    double inv_sigma;     // staging scale
+    double fscale;        // 48 eps / sigma
+    float rc2s, guard;    // rc'^2 and the guard band in scaled units
+};
+
+__device__ __forceinline__ float4 lds_f4(uint32_t addr)
+{
+    float4 v;
+    asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ unsigned long long f2_pack(float a, float b)
+{
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
+    return r;
+}
+__device__ __forceinline__ void f2_unpack(unsigned long long v, float &a, float &b)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
+}
+__device__ __forceinline__ unsigned long long f2_mul(unsigned long long a, unsigned long long b)
+{
+    unsigned long long r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ unsigned long long f2_add(unsigned long long a, unsigned long long b)
+{
+    unsigned long long r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ unsigned long long f2_fma(unsigned long long a, unsigned long long b, unsigned long long c)
+{
+    unsigned long long r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+
+// slow path of one block of 8 entries: the same sum with every in-band decision taken by the exact fp64 test (R26)
+__device__ __noinline__ void lj3_block_exact(const uint4 q, uint32_t rec_addr, float mx, float my, float mz, float rc2s,
+                                            float guard, const double4 *__restrict__ pos, double Lx, double Ly, double Lz,
+                                            double rc2_exact, uint32_t gi, const uint32_t *gstart, const uint32_t *sstart,
+                                            uint32_t n_sc, float *out)
+{
+    const uint32_t qq[4] = {q.x, q.y, q.z, q.w};
+    float ax = 0.f, ay = 0.f, az = 0.f;
+#pragma unroll 1
+    for (int e = 0; e < 8; ++e) {
+        const uint32_t off = (e & 1) ? (qq[e >> 1] >> 16) : (qq[e >> 1] & 0xffffu);
+        const float4 pj = lds_f4(rec_addr + off);
+        const float dx = mx - pj.x, dy = my - pj.y, dz = mz - pj.z;
+        const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+        const float d = r2 - rc2s;
+        bool in = d < -guard;
+        if (fabsf(d) < guard) {
+            const uint32_t s = off >> 4;
+            uint32_t lo = 0, hi = n_sc;
+            while (hi - lo > 1) {
+                const uint32_t mid = (lo + hi) >> 1;
+                if (sstart[mid] <= s) lo = mid; else hi = mid;
+            }
+            in = tile_exact_r2_impl(pos, Lx, Ly, Lz, gi, gstart[lo] + (s - sstart[lo])) < rc2_exact;
+        }
+        const float rinv2 = md_rcp(r2);
+        const float s6 = rinv2 * rinv2 * rinv2;
+        float f = (s6 - 0.5f) * (s6 * rinv2);
+        f = in ? f : 0.f;
+        ax = fmaf(f, dx, ax); ay = fmaf(f, dy, ay); az = fmaf(f, dz, az);
+    }
+    out[0] = ax; out[1] = ay; out[2] = az;
+}
+
+template <int W, bool X2>
+__global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj3(TileParams tp, Geom g, const double4 *__restrict__ pos,
+                                                             const uint32_t *__restrict__ nl_cnt,
+                                                             const uint16_t *__restrict__ nl16, LJ3 lj,
+                                                             uint32_t max_staged, double4 *__restrict__ force)
+{
+    extern __shared__ __align__(16) char smem_raw[];
+    float4 *rec = (float4 *)smem_raw;  // records first: their shared-memory address is a launch constant
+    const TileSmem h = tile_carve(smem_raw + sizeof(float4) * (max_staged + N_DUMMY), tp.B);
+    uint8_t *scell = (uint8_t *)h.rest;
+
+    TileCtx tc;
+    tile_setup(tp, g, blockIdx.x, h, tc);
+    tile_stage<float4, false>(g, tc, h, pos, nullptr, rec, nullptr, scell, lj.inv_sigma);
+    // staged index of every home particle (replaces a search per particle)
+    uint16_t *hsidx = (uint16_t *)(scell + ((max_staged + 16) & ~15u));
+    for (uint32_t hc = threadIdx.x >> 5; hc < tc.n_hc; hc += blockDim.x >> 5) {
+        const uint32_t p0 = h.hc_first[hc], p1 = h.hc_first[hc + 1], s0 = h.sstart[h.hc_sc[hc]];
+        for (uint32_t p = p0 + (threadIdx.x & 31u); p < p1; p += 32) hsidx[p] = (uint16_t)(s0 + (p - p0));
+    }
+    __syncthreads();
+
+    const unsigned lane = threadIdx.x & (W - 1);
+    const unsigned seg_mask = md_seg_mask<W>();
+    const uint32_t n_groups = blockDim.x / W;
+    const uint32_t rec_addr = (uint32_t)__cvta_generic_to_shared(rec);
+    const float rc2s = lj.rc2s, guard = lj.guard, nguard = -lj.guard;
+    const uint32_t stride8 = tp.stride >> 3;
+
+    for (uint32_t p = threadIdx.x / W; p < tc.n_home; p += n_groups) {
+        const float4 me = rec[hsidx[p]];
+        const uint32_t nblk = (nl_cnt[tc.g0 + p] + 7u) >> 3;
+        const uint4 *row = (const uint4 *)nl16 + (size_t)(tc.g0 + p) * stride8;
+        double fx = 0.0, fy = 0.0, fz = 0.0;
+        uint4 q = lane < nblk ? __ldg(row + lane) : make_uint4(0, 0, 0, 0);
+        for (uint32_t b = lane; b < nblk; b += W) {
+            const uint4 qn = b + W < nblk ? __ldg(row + b + W) : q;  // prefetch the next block of 8 entries
+            const uint32_t qq[4] = {q.x, q.y, q.z, q.w};
+            float ax, ay, az, band = 3e38f;
+            if (X2) {
+                unsigned long long ax2 = 0ull, ay2 = 0ull, az2 = 0ull;  // (0.f, 0.f)
+                const unsigned long long mrc2 = f2_pack(-rc2s, -rc2s), mhalf = f2_pack(-0.5f, -0.5f);
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const float4 pa = lds_f4(rec_addr + (qq[e] & 0xffffu));
+                    const float4 pb = lds_f4(rec_addr + (qq[e] >> 16));
+                    const unsigned long long dx = f2_pack(me.x - pa.x, me.x - pb.x);
+                    const unsigned long long dy = f2_pack(me.y - pa.y, me.y - pb.y);
+                    const unsigned long long dz = f2_pack(me.z - pa.z, me.z - pb.z);
+                    const unsigned long long r2 = f2_fma(dz, dz, f2_fma(dy, dy, f2_mul(dx, dx)));
+                    const unsigned long long d = f2_add(r2, mrc2);
+                    float r2a, r2b, da, db;
+                    f2_unpack(r2, r2a, r2b);
+                    f2_unpack(d, da, db);
+                    band = fminf(band, fminf(fabsf(da), fabsf(db)));
+                    const unsigned long long ri = f2_pack(md_rcp(r2a), md_rcp(r2b));
+                    const unsigned long long s6 = f2_mul(f2_mul(ri, ri), ri);
+                    const unsigned long long ff = f2_mul(f2_add(s6, mhalf), f2_mul(s6, ri));
+                    float fa, fb;
+                    f2_unpack(ff, fa, fb);
+                    fa = da < nguard ? fa : 0.f;
+                    fb = db < nguard ? fb : 0.f;
+                    const unsigned long long f = f2_pack(fa, fb);
+                    ax2 = f2_fma(f, dx, ax2);
+                    ay2 = f2_fma(f, dy, ay2);
+                    az2 = f2_fma(f, dz, az2);
+                }
+                float t0, t1;
+                f2_unpack(ax2, t0, t1); ax = t0 + t1;
+                f2_unpack(ay2, t0, t1); ay = t0 + t1;
+                f2_unpack(az2, t0, t1); az = t0 + t1;
+            } else {
+                ax = ay = az = 0.f;
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const uint32_t off = (e & 1) ? (qq[e >> 1] >> 16) : (qq[e >> 1] & 0xffffu);
+                    const float4 pj = lds_f4(rec_addr + off);
+                    const float dx = me.x - pj.x, dy = me.y - pj.y, dz = me.z - pj.z;
+                    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                    const float d = r2 - rc2s;
+                    band = fminf(band, fabsf(d));
+                    const float rinv2 = md_rcp(r2);
+                    const float s6 = rinv2 * rinv2 * rinv2;
+                    float f = (s6 - 0.5f) * (s6 * rinv2);
+                    f = d < nguard ? f : 0.f;
+                    ax = fmaf(f, dx, ax); ay = fmaf(f, dy, ay); az = fmaf(f, dz, az);
+                }
+            }
+            if (band < guard) {  // some pair of this block is inside the guard band: exact decisions (rare)
+                float o[3];
+                lj3_block_exact(q, rec_addr, me.x, me.y, me.z, rc2s, guard, pos, g.L[0], g.L[1], g.L[2], lj.rc2_exact,
+                                tc.g0 + p, h.gstart, h.sstart, tc.n_sc, o);
+                ax = o[0]; ay = o[1]; az = o[2];
+            }
+            fx += (double)ax; fy += (double)ay; fz += (double)az;
+            q = qn;
+        }
+        fx = md_seg_sum<W>(fx, seg_mask);
+        fy = md_seg_sum<W>(fy, seg_mask);
+        fz = md_seg_sum<W>(fz, seg_mask);
+        if (lane == 0) force[tc.g0 + p] = make_double4(fx * lj.fscale, fy * lj.fscale, fz * lj.fscale, 0.0);
+    }
+}
+
+// ===============================================================================================================
 // S4b DPD forces, one CTA per tile, W threads per home particle, fp64; positions, velocities and tags staged
 // ===============================================================================================================
 struct DPDTile {
@@ -519,13 +779,13 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_dpd(TileParams tp, Geom
     extern __shared__ __align__(16) char smem_raw[];
     const TileSmem h = tile_carve(smem_raw, tp.B);
     double4 *rec = (double4 *)h.rest;
-    double4 *svel = rec + (max_staged + 1);
-    uint8_t *scell = (uint8_t *)(svel + (max_staged + 1));
+    double4 *svel = rec + (max_staged + N_DUMMY);
+    uint8_t *scell = (uint8_t *)(svel + (max_staged + N_DUMMY));
 
     TileCtx tc;
     tile_setup(tp, g, blockIdx.x, h, tc);
     tile_stage<double4, true>(g, tc, h, pos, vel, rec, svel, scell);
-    if (threadIdx.x == 0) svel[tc.n_staged] = make_double4(0, 0, 0, 1);
+    if (threadIdx.x < N_DUMMY) svel[tc.n_staged + threadIdx.x] = make_double4(0, 0, 0, 1);
     __syncthreads();
 
     const unsigned lane = threadIdx.x & (W - 1);
@@ -596,7 +856,7 @@ __global__ void k_tile_decode(TileParams tp, Geom g, const double *__restrict__ 
     const unsigned lt = md_lanemask_lt();
     for (uint32_t p = wid; p < tc.n_home; p += nw) {
         const uint32_t gi = tc.g0 + p;
-        const uint32_t cnt = nl_cnt[gi];
+        const uint32_t cnt = (nl_cnt[gi] + 7u) & ~7u;  // stored rows are whole blocks of 8, dummies interspersed
         const uint16_t *row = nl16 + (size_t)gi * tp.stride;
         const double xi = pos_ref[3ull * gi], yi = pos_ref[3ull * gi + 1], zi = pos_ref[3ull * gi + 2];
         uint32_t *out = FILL ? nl_idx + nl_off[gi] : nullptr;
@@ -676,8 +936,8 @@ static double tile_extent(md_ctx *c)
 static size_t tile_smem_common(md_ctx *c, size_t rec_bytes, bool with_vel)
 {
     size_t s = tile_header_bytes(c->tile_B);
-    s += rec_bytes * (c->tile_max_staged + 1);
-    if (with_vel) s += sizeof(double4) * (c->tile_max_staged + 1);
+    s += rec_bytes * (c->tile_max_staged + N_DUMMY);
+    if (with_vel) s += sizeof(double4) * (c->tile_max_staged + N_DUMMY);
     s += (c->tile_max_staged + 16) & ~(size_t)15;  // staged-cell table of tile_stage
     return s;
 }
@@ -700,7 +960,7 @@ static int set_smem(md_ctx *c, K kernel, size_t bytes)
 static const size_t TILE_SMEM_LIMIT = 227 * 1024 - 64;
 
 // entries are pre-shifted byte offsets when every staged index (and the dummy) fits in 12 bits
-static uint32_t tile_shift(md_ctx *c) { return c->tile_max_staged + 1 < 4096 ? 4u : 0u; }
+static uint32_t tile_shift(md_ctx *c) { return c->tile_max_staged + N_DUMMY <= 4096 ? 4u : 0u; }
 
 // returns MD_OK and sets *fits = false if the largest tile does not fit in shared memory (caller falls back)
 int launch_tile_build(md_ctx *c, bool *fits)
@@ -709,8 +969,8 @@ int launch_tile_build(md_ctx *c, bool *fits)
     const int block = std::min(c->cfg[MD_K_NLIST].block, TILE_MAX_BLOCK);
     const uint32_t nw = (uint32_t)block / 32;
     size_t smem = tile_smem_common(c, sizeof(float4), false);
-    smem += sizeof(uint16_t) * (size_t)nw * BUILD_P * c->nl_stride;  // row assembly buffers
-    *fits = smem <= TILE_SMEM_LIMIT && ms < 65535 && c->tile_B <= 4;
+    smem += sizeof(uint16_t) * (size_t)nw * BUILD_P * (c->nl_stride + RB_EXTRA) + sizeof(uint32_t) * nw * BUILD_P * 24;  // row assembly
+    *fits = smem <= TILE_SMEM_LIMIT && ms + N_DUMMY <= 65536 && c->tile_B <= 4;
     if (!*fits) return MD_OK;
     c->nl_shift = tile_shift(c);
     const double R = c->r_list * 1.001, E = tile_extent(c), rl2 = c->r_list * c->r_list;
@@ -768,6 +1028,38 @@ int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
     p.thr_out = p.rc2_exact + gd;
     const size_t smem = tile_smem_common(c, mixed ? sizeof(float4) : sizeof(double4), false);
     TileParams tp = make_tp(c);
+    static const int lj3_mode = getenv("B200MD_LJ3") ? atoi(getenv("B200MD_LJ3")) : 2;
+    if (mixed && !energy && c->nl_shift && c->acc_block == 8 && cf.w >= 4 && lj3_mode) {
+        const size_t smem = tile_smem_common(c, sizeof(float4), false) + ((2 * (size_t)c->tile_max_home + 15) & ~(size_t)15);
+        LJ3 q;
+        q.rc2_exact = p.rc2_exact;
+        q.inv_sigma = 1.0 / sigma;
+        q.fscale = 48.0 * eps / sigma;
+        const double rc2s = p.rc2_exact / p.sig2;
+        q.rc2s = (float)rc2s;
+        // guard in scaled units: the fp32 error bound of r'^2 plus the rounding of rc'^2 itself
+        q.guard = (float)(1.0001 * (gd / p.sig2 + 2.0 * 5.9604644775390625e-08 * rc2s));
+        const int w = cf.w > 8 ? 8 : cf.w;
+        if (w == 4) {
+            if (lj3_mode == 2) {
+                MD_TRY(set_smem(c, k_tile_lj3<4, true>, smem));
+                k_tile_lj3<4, true><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force);
+            } else {
+                MD_TRY(set_smem(c, k_tile_lj3<4, false>, smem));
+                k_tile_lj3<4, false><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force);
+            }
+        } else {
+            if (lj3_mode == 2) {
+                MD_TRY(set_smem(c, k_tile_lj3<8, true>, smem));
+                k_tile_lj3<8, true><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force);
+            } else {
+                MD_TRY(set_smem(c, k_tile_lj3<8, false>, smem));
+                k_tile_lj3<8, false><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force);
+            }
+        }
+        MD_LAUNCH_CHECK(c);
+        return MD_OK;
+    }
     MD_DISPATCH_W(cf.w, {
         if (mixed) {
             if (c->acc_block == 1) MD_TRY((launch_lj_energy<W_, true, 1>(c, tp, p, cf.block, smem, energy)));
