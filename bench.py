@@ -211,6 +211,8 @@ def run_ours(args):
     md.set_state(d_pos, d_vel)
     if w.bonds is not None:
         md.set_bonds(w.bonds)
+    if args.cluster:
+        md.set_option(B.MD_OPT_CLUSTER, 1)
     for spec in args.launch:                       # e.g. --launch lj=256,4 nlist=768,32 (fixes a kernel's block, w)
         name, val = spec.split("=")
         blk, ww = (int(x) for x in val.split(","))
@@ -318,6 +320,7 @@ def main():
     ap.add_argument("--sync-sched", action="store_true", help="MD_SCHED_SYNC instead of the speculative scheduler")
     ap.add_argument("--launch", nargs="*", default=[], help="kernel=block,w (with --no-tune)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cluster", action="store_true", help="MD_OPT_CLUSTER = 1: one neighbour row per cluster of 4")
     args = ap.parse_args()
     if args.impl == "reference":
         sys.exit(run_reference(args))

@@ -214,6 +214,12 @@ int md_tune(md_ctx *ctx, const md_step_desc *what, int full);
    in fp32, the block sum is widened and added in fp64 (R25). */
 #define MD_OPT_TILE_BRICK 1
 #define MD_OPT_ACC_BLOCK 2
+/* MD_OPT_CLUSTER (MD_MIXED with MD_ORDER_MORTON only): 1 = the neighbour list is stored as one row per
+   cluster of 4 consecutive particles of a cell (members of a cell are ordered along a sub-cell Morton curve, so a
+   cluster is spatially compact); a row holds every particle within r_list of ANY member, and the LJ kernel evaluates
+   each stored candidate against the 4 members in registers.  The exported list is the exact
+   per-particle list either way.  0 (default) = one row per particle.  Invalidates the list. */
+#define MD_OPT_CLUSTER 3
 int md_set_option(md_ctx *ctx, int option, int64_t value);
 
 /* Fix launch parameters by hand (block multiple of 32 in [32,1024]; w power of two <= 32); kernel = MD_K_*. */

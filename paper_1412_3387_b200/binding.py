@@ -18,7 +18,7 @@ MD_FP64, MD_MIXED = 0, 1
 MD_ORDER_LEX, MD_ORDER_MORTON, MD_ORDER_HILBERT = 0, 1, 2
 MD_F_LJ, MD_F_DPD, MD_F_BONDS = 1, 2, 4
 MD_SCHED_SYNC, MD_SCHED_SPECULATIVE = 0, 1
-MD_OPT_TILE_BRICK, MD_OPT_ACC_BLOCK = 1, 2
+MD_OPT_TILE_BRICK, MD_OPT_ACC_BLOCK, MD_OPT_CLUSTER = 1, 2, 3
 MD_N_KERNELS = 8
 MD_K_NLIST, MD_K_LJ, MD_K_DPD, MD_K_BONDS, MD_K_INTEGRATE, MD_K_CELLS = 0, 1, 2, 3, 4, 5
 KERNEL_NAMES = {MD_K_NLIST: "nlist", MD_K_LJ: "lj", MD_K_DPD: "dpd", MD_K_BONDS: "bonds",

@@ -341,6 +341,7 @@ extern "C" int md_create(md_ctx **out, const double box[3], uint64_t N, double r
         c->g.lo[a] = -0.5 * box[a];
         c->g.n[a] = c->dims[a];
         c->g.dn[a] = (double)c->dims[a];
+        c->g.cw[a] = c->box[a] / (double)c->dims[a];
     }
     if (ncell >= 0xfffffff0ull) { g_create_err = "md_create: too many cells"; delete c; return MD_EINVAL; }
     c->n_cells = (uint32_t)ncell;
@@ -359,6 +360,7 @@ extern "C" int md_create(md_ctx **out, const double box[3], uint64_t N, double r
     A((void **)&c->image, 3 * N * sizeof(int));
     A((void **)&c->image_alt, 3 * N * sizeof(int));
     A((void **)&c->pos_ref, 3 * N * sizeof(double));
+    A((void **)&c->rel, N * sizeof(float4));
     A((void **)&c->tag, N * sizeof(uint32_t));
     A((void **)&c->tag_alt, N * sizeof(uint32_t));
     A((void **)&c->rtag, N * sizeof(uint32_t));
@@ -574,21 +576,28 @@ static int build_nlist_tiles(md_ctx *c, bool *done)
     MD_TRY(md_read_flags(c));
     c->tile_max_home = c->h_flags->max_home;
     c->tile_max_staged = c->h_flags->max_staged;
-    if (c->nl_stride == 0) {
+    const int mode = tile_cluster_ok(c) ? 1 : 0;
+    if (c->nl_stride == 0 || c->stride_mode != mode) {
         // row stride from the mean density: 1.35 n + 24 covers the fluctuations of liquids and ideal gases at the
-        // configured densities; a longer row is detected by the build kernel and the stride grows
+        // configured densities; a longer row is detected by the build kernel and the stride grows.  Cluster rows hold
+        // the union of 4 neighbourhoods: the sphere grows by about the cluster radius (~ 0.75 of the mean spacing).
         const double vol = c->box[0] * c->box[1] * c->box[2];
-        const double nbar = (double)c->N / vol * 4.18879020478639 * c->r_list * c->r_list * c->r_list;
+        const double rho = (double)c->N / vol;
+        const double re = c->r_list + (mode ? 0.75 * pow(rho, -1.0 / 3.0) : 0.0);
+        const double nbar = rho * 4.18879020478639 * re * re * re;
+        if (c->nl16) { md_free(c, c->nl16); c->nl16 = nullptr; }
         c->nl_stride = round16(1.35 * nbar + 24.0);
+        c->stride_mode = mode;
     }
     for (int attempt = 0; attempt < 3; ++attempt) {
         if (!c->nl16) MD_TRY(md_alloc(c, (void **)&c->nl16, c->N * (uint64_t)c->nl_stride * sizeof(uint16_t)));
         bool fits = false;
-        MD_TRY(launch_tile_build(c, &fits));
+        MD_TRY(launch_tile_build(c, mode == 1, &fits));
         if (!fits) return MD_OK;  // largest tile exceeds shared memory: general path
         MD_TRY(md_read_flags(c));
         if (c->h_flags->nl_overflow == 0) {
             c->nl_entries = c->h_flags->nl_total;
+            c->nl_cluster = mode == 1;
             c->nl_is_tile = true;
             c->nl32_decoded = false;
             *done = true;
@@ -624,6 +633,7 @@ static int ensure_decoded(md_ctx *c)
     MD_TRY(launch_tile_decode(c, false, c->nl_cnt32));
     MD_TRY(launch_exclusive_scan_u32(c, c->nl_cnt32, c->N, nullptr, c->nl_off, false, &c->d_flags->nl_total));
     MD_TRY(md_read_flags(c));
+    c->nl_exact_entries = c->h_flags->nl_total;
     MD_TRY(ensure_nl32(c, c->h_flags->nl_total));
     MD_TRY(launch_tile_decode(c, true, nullptr));
     c->nl_cnt_exp = c->nl_cnt32;
@@ -696,14 +706,19 @@ extern "C" int md_get_nlist_rows(md_ctx *c, const uint32_t *probe_tags, uint32_t
 // S4 / S5 / S6 single calls
 // =====================================================================================================
 // pair kernels: tile path when the current list is a tile list, else the general list kernels
+static int ensure_decoded(md_ctx *c);
 static int pair_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
 {
-    if (c->nl_is_tile) return launch_tile_lj(c, eps, sigma, shift, energy);
+    // cluster rows are read by k_tile_lj4 only (forces, no energies); everything else goes through the decoded list
+    if (c->nl_is_tile && !(c->nl_cluster && (energy || c->precision != MD_MIXED)))
+        return launch_tile_lj(c, eps, sigma, shift, energy);
+    MD_TRY(ensure_decoded(c));
     return launch_forces_lj(c, eps, sigma, shift);
 }
 static int pair_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed)
 {
-    if (c->nl_is_tile) return launch_tile_dpd(c, A, gamma, kT, dt, step, seed);
+    if (c->nl_is_tile && !c->nl_cluster) return launch_tile_dpd(c, A, gamma, kT, dt, step, seed);
+    MD_TRY(ensure_decoded(c));
     return launch_forces_dpd(c, A, gamma, kT, dt, step, seed);
 }
 
@@ -912,7 +927,9 @@ static int tune_kernel(md_ctx *c, int kernel, const char *name, bool sweep_w, in
             c->cfg[kernel].block = b;
             c->cfg[kernel].w = w;
             float us;
+            c->tune_skip = false;
             MD_TRY(time_median5(c, fn, &us));
+            if (c->tune_skip) continue;
             if (c->log) fprintf(stderr, "[b200md tuner] %-10s block=%4d w=%2d  %9.1f us\n", name, b, w, us);
             if (us < best.us) best = LaunchCfg{b, w, us};
         }
@@ -930,8 +947,10 @@ extern "C" int md_tune(md_ctx *c, const md_step_desc *w, int full)
     if (c->nl_is_tile) {
         // tile build: w is fixed at 32 (one ballot word per 32 candidates); only the block size is swept
         MD_TRY(tune_kernel(c, MD_K_NLIST, "nlist/tile", false, full, [&]() {
-            bool fits;
-            return launch_tile_build(c, &fits);
+            bool fits = false;
+            const int st = launch_tile_build(c, c->nl_cluster, &fits);
+            if (!fits) c->tune_skip = true;  // this block size does not fit in shared memory
+            return st;
         }));
         c->cfg[MD_K_NLIST].w = 32;
     } else {
@@ -960,6 +979,11 @@ extern "C" int md_set_option(md_ctx *c, int option, int64_t value)
         MD_TRY(md_sync(c));
         MD_TRY(build_cell_order(c));
         c->cells_valid = c->nlist_valid = false;
+        return MD_OK;
+    case MD_OPT_CLUSTER:
+        if (value != 0 && value != 1) { c->err = "md_set_option: cluster must be 0 or 1"; return MD_EINVAL; }
+        c->cluster_opt = (int)value;
+        c->nlist_valid = false;
         return MD_OK;
     case MD_OPT_ACC_BLOCK:
         if (value != 1 && value != 8) { c->err = "md_set_option: accumulation block must be 1 or 8"; return MD_EINVAL; }
@@ -993,6 +1017,11 @@ extern "C" int md_get_stats(md_ctx *c, md_stats *out)
     c->stats.nlist_capacity = c->nl_capacity;
     c->stats.device_bytes = c->device_bytes;
     c->stats.mean_neighbors = c->N ? (double)c->nl_entries / (double)c->N : 0.0;
+    if (c->nlist_valid && c->nl_is_tile && c->nl_cluster) {
+        // cluster rows: nl_entries counts stored candidates per cluster; the per-particle figure is the exact decoded list's
+        MD_TRY(ensure_decoded(c));
+        c->stats.mean_neighbors = c->N ? (double)c->nl_exact_entries / (double)c->N : 0.0;
+    }
     for (int a = 0; a < 3; ++a) c->stats.dims[a] = c->dims[a];
     for (int k = 0; k < MD_N_KERNELS; ++k) {
         c->stats.block[k] = c->cfg[k].block;

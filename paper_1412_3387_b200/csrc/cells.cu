@@ -245,31 +245,66 @@ __global__ void k_cell_scatter(const uint32_t *__restrict__ cell_rank, uint32_t 
     perm[cell_start[r] + k] = i;
 }
 
-// (4) one warp per cell: order the cell's members by tag (rank sort; tags are unique)
+// (4) one warp per cell: order the cell's members by (sub-cell Morton key, tag) -- rank sort; tags are unique, so the
+// order is a pure function of the positions.  The sub-cell key (3 bits per axis of the position inside the cell) makes
+// runs of consecutive members spatially compact: the tile kernels treat 4 consecutive members as a cluster.
+__device__ __forceinline__ uint32_t sub_coord(double x, double lo, double L, double dn, uint32_t n)
+{
+    const double f = __dmul_rn(__ddiv_rn(__dsub_rn(x, lo), L), dn);
+    long long k = (long long)f;
+    if (k >= (long long)n) k = (long long)n - 1;
+    if (k < 0) k = 0;
+    int s = (int)((f - (double)k) * 8.0);
+    return (uint32_t)min(7, max(0, s));
+}
+__device__ __forceinline__ uint32_t spread3(uint32_t v) { return (v & 1u) | ((v & 2u) << 2) | ((v & 4u) << 4); }
+__device__ __forceinline__ unsigned long long cell_sort_key(const double4 p, const Geom &g, uint32_t t, bool subsort)
+{
+    uint32_t sub = 0;
+    if (subsort) {
+        sub = spread3(sub_coord(p.x, g.lo[0], g.L[0], g.dn[0], g.n[0])) |
+              (spread3(sub_coord(p.y, g.lo[1], g.L[1], g.dn[1], g.n[1])) << 1) |
+              (spread3(sub_coord(p.z, g.lo[2], g.L[2], g.dn[2], g.n[2])) << 2);
+    }
+    return ((unsigned long long)sub << 32) | t;
+}
+
 __global__ void k_cell_sort(const uint32_t *__restrict__ perm, const uint32_t *__restrict__ cell_start,
-                            const uint32_t *__restrict__ tag, uint32_t n_cells, uint32_t *perm_sorted,
-                            unsigned int *max_count)
+                            const uint32_t *__restrict__ tag, const double4 *__restrict__ pos, Geom g, bool subsort,
+                            uint32_t n_cells, uint32_t *perm_sorted, unsigned int *max_count)
 {
     const uint32_t cell = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const unsigned lane = threadIdx.x & 31u;
     if (cell >= n_cells) return;
     const uint32_t b = cell_start[cell], e = cell_start[cell + 1], n = e - b;
     if (lane == 0 && n > 0) atomicMax(max_count, n);
-    if (n <= 32) {
-        const uint32_t idx = lane < n ? perm[b + lane] : 0u;
-        const uint32_t t = lane < n ? tag[idx] : 0xffffffffu;
-        uint32_t rank = 0;
-        for (uint32_t k = 0; k < n; ++k) {
-            const uint32_t tk = __shfl_sync(0xffffffffu, t, k);
-            rank += (tk < t) ? 1u : 0u;
+    // up to 64 members: keys in registers (2 per lane), ranks by shuffles; more: keys re-read from memory
+    if (n <= 64) {
+        uint32_t idx[2];
+        unsigned long long key[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const uint32_t m = lane + 32u * h;
+            idx[h] = m < n ? perm[b + m] : 0u;
+            key[h] = m < n ? cell_sort_key(pos[idx[h]], g, tag[idx[h]], subsort) : ~0ull;
         }
-        if (lane < n) perm_sorted[b + rank] = idx;
+        uint32_t rank[2] = {0u, 0u};
+        for (uint32_t k = 0; k < n; ++k) {
+            const unsigned long long kk = __shfl_sync(0xffffffffu, k < 32 ? key[0] : key[1], k & 31u);
+            rank[0] += kk < key[0] ? 1u : 0u;
+            rank[1] += kk < key[1] ? 1u : 0u;
+        }
+        if (lane < n) perm_sorted[b + rank[0]] = idx[0];
+        if (lane + 32u < n) perm_sorted[b + rank[1]] = idx[1];
     } else {
         for (uint32_t m = lane; m < n; m += 32) {
             const uint32_t idx = perm[b + m];
-            const uint32_t t = tag[idx];
+            const unsigned long long key = cell_sort_key(pos[idx], g, tag[idx], subsort);
             uint32_t rank = 0;
-            for (uint32_t k = 0; k < n; ++k) rank += (tag[perm[b + k]] < t) ? 1u : 0u;
+            for (uint32_t k = 0; k < n; ++k) {
+                const uint32_t ik = perm[b + k];
+                rank += cell_sort_key(pos[ik], g, tag[ik], subsort) < key ? 1u : 0u;
+            }
             perm_sorted[b + rank] = idx;
         }
     }
@@ -280,7 +315,8 @@ __global__ void k_reorder(const uint32_t *__restrict__ perm_sorted, uint32_t N, 
                           const double4 *__restrict__ vel, const double4 *__restrict__ force,
                           const int *__restrict__ image, const uint32_t *__restrict__ tag,
                           const uint32_t *__restrict__ cell_lin_old, double4 *npos, double4 *nvel, double4 *nforce,
-                          int *nimage, uint32_t *ntag, uint32_t *rtag, uint32_t *cell_lin, double *pos_ref)
+                          int *nimage, uint32_t *ntag, uint32_t *rtag, uint32_t *cell_lin, double *pos_ref, Geom g,
+                          float4 *rel)
 {
     const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= N) return;
@@ -295,7 +331,9 @@ __global__ void k_reorder(const uint32_t *__restrict__ perm_sorted, uint32_t N, 
     const uint32_t t = tag[o];
     ntag[s] = t;
     rtag[t] = s;
-    cell_lin[s] = cell_lin_old[o];
+    const uint32_t lin = cell_lin_old[o];
+    cell_lin[s] = lin;
+    rel[s] = md_rel_record(p.x, p.y, p.z, lin, g);
     pos_ref[3ull * s] = p.x;
     pos_ref[3ull * s + 1] = p.y;
     pos_ref[3ull * s + 2] = p.z;
@@ -318,14 +356,15 @@ int launch_build_cells(md_ctx *c)
     MD_CUDA_CHECK(c, cudaMemsetAsync(c->cell_count, 0, sizeof(uint32_t) * c->n_cells, st));
     k_cell_scatter<<<md_grid(N, 256), 256, 0, st>>>(c->cell_rank_tmp, N, c->cell_start, c->cell_count, c->perm);
     MD_LAUNCH_CHECK(c);
-    k_cell_sort<<<md_grid((uint64_t)c->n_cells * 32, 256), 256, 0, st>>>(c->perm, c->cell_start, c->tag, c->n_cells,
-                                                                       c->perm_sorted, &c->d_flags->max_cell_count);
+    k_cell_sort<<<md_grid((uint64_t)c->n_cells * 32, 256), 256, 0, st>>>(c->perm, c->cell_start, c->tag, c->pos, c->g,
+                                                                       c->use_tiles, c->n_cells, c->perm_sorted,
+                                                                       &c->d_flags->max_cell_count);
     MD_LAUNCH_CHECK(c);
     // new tags go to cell_rank_tmp (free now), then pointers are swapped
     uint32_t *ntag = c->cell_rank_tmp;
     k_reorder<<<md_grid(N, 256), 256, 0, st>>>(c->perm_sorted, N, c->pos, c->vel, c->force, c->image, c->tag,
                                                cell_lin_old, c->pos_alt, c->vel_alt, c->force_alt, c->image_alt, ntag,
-                                               c->rtag, c->cell_lin, c->pos_ref);
+                                               c->rtag, c->cell_lin, c->pos_ref, c->g, c->rel);
     MD_LAUNCH_CHECK(c);
     swap_ptr(c->pos, c->pos_alt);
     swap_ptr(c->vel, c->vel_alt);

@@ -83,9 +83,9 @@ int launch_forces_lj(md_ctx *c, double eps, double sigma, int shift)
     const bool mixed = c->precision == MD_MIXED;
     MD_DISPATCH_W(cf.w, {
         if (mixed)
-            k_forces_lj<W_, true><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt, c->nl_off, c->nl_idx, c->g, p, c->force);
+            k_forces_lj<W_, true><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force);
         else
-            k_forces_lj<W_, false><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt, c->nl_off, c->nl_idx, c->g, p, c->force);
+            k_forces_lj<W_, false><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force);
     });
     MD_LAUNCH_CHECK(c);
     return MD_OK;
@@ -158,7 +158,7 @@ int launch_forces_dpd(md_ctx *c, double A, double gamma, double kT, double dt, u
     p.seed = seed;
     const unsigned grid = md_grid(c->N * (uint64_t)cf.w, cf.block);
     MD_DISPATCH_W(cf.w, {
-        k_forces_dpd<W_><<<grid, cf.block, 0, c->stream>>>(c->pos, c->vel, c->nl_cnt, c->nl_off, c->nl_idx, c->g, p, c->force);
+        k_forces_dpd<W_><<<grid, cf.block, 0, c->stream>>>(c->pos, c->vel, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force);
     });
     MD_LAUNCH_CHECK(c);
     return MD_OK;

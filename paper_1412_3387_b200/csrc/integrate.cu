@@ -8,8 +8,9 @@
 // predict the step at which the criterion will fire, see md_step); the other slot is cleared for the next step.
 template <bool FUSED>
 __global__ void k_half1(double4 *__restrict__ pos, double4 *__restrict__ vel, const double4 *__restrict__ force,
-                        int *__restrict__ image, const double *__restrict__ pos_ref, Geom g, double dt, double half_dt,
-                        double thr2, double danger2, DevFlags *flags, int slot)
+                        int *__restrict__ image, const double *__restrict__ pos_ref,
+                        const uint32_t *__restrict__ cell_lin, float4 *__restrict__ rel, Geom g, double dt,
+                        double half_dt, double thr2, double danger2, DevFlags *flags, int slot)
 {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     float d2f = 0.f;
@@ -37,6 +38,7 @@ __global__ void k_half1(double4 *__restrict__ pos, double4 *__restrict__ vel, co
             d2 = a == 0 ? __dmul_rn(d, d) : __dadd_rn(d2, __dmul_rn(d, d));
         }
         pos[i] = make_double4(x[0], x[1], x[2], p.w);
+        rel[i] = md_rel_record(x[0], x[1], x[2], cell_lin[i], g);  // meaningful once the particles are binned
         vel[i] = make_double4(u[0], u[1], u[2], m);
         if (d2 > thr2) {
             flags->rebuild = 1;  // benign race: every writer stores the same value
@@ -67,12 +69,12 @@ int launch_half1(md_ctx *c, double dt, bool fused)
     const double t = 0.5 * c->r_buff;
     c->d2_slot ^= 1;
     if (fused)
-        k_half1<true><<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->pos, c->vel, c->force, c->image, c->pos_ref, c->g,
-                                                                         dt, 0.5 * dt, t * t, c->r_buff * c->r_buff,
+        k_half1<true><<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->pos, c->vel, c->force, c->image, c->pos_ref,
+                                                                         c->cell_lin, c->rel, c->g, dt, 0.5 * dt, t * t, c->r_buff * c->r_buff,
                                                                          c->d_flags, c->d2_slot);
     else
-        k_half1<false><<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->pos, c->vel, c->force, c->image, c->pos_ref, c->g,
-                                                                          dt, 0.5 * dt, t * t, c->r_buff * c->r_buff,
+        k_half1<false><<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->pos, c->vel, c->force, c->image, c->pos_ref,
+                                                                          c->cell_lin, c->rel, c->g, dt, 0.5 * dt, t * t, c->r_buff * c->r_buff,
                                                                           c->d_flags, c->d2_slot);
     MD_LAUNCH_CHECK(c);
     return MD_OK;

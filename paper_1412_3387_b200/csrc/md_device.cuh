@@ -28,6 +28,19 @@ __device__ __forceinline__ uint32_t md_cell_coord(double x, double lo, double L,
     return (uint32_t)k;
 }
 
+// fp32 record of a position relative to the centre of cell `lin` (linear id), minimum image applied: what the fp32
+// tile kernels stage.  |result| <= half a cell width + the drift since the binning, so the rounding is ~1e-7 absolute.
+__device__ __forceinline__ float4 md_rel_record(double x, double y, double z, uint32_t lin, const Geom &g)
+{
+    const uint32_t nxy = g.n[0] * g.n[1];
+    const uint32_t cz = lin / nxy, rem = lin - cz * nxy;
+    const uint32_t cy = rem / g.n[0], cx = rem - cy * g.n[0];
+    const double rx = md_min_image(x - (g.lo[0] + ((double)cx + 0.5) * g.cw[0]), g.L[0], g.h[0]);
+    const double ry = md_min_image(y - (g.lo[1] + ((double)cy + 0.5) * g.cw[1]), g.L[1], g.h[1]);
+    const double rz = md_min_image(z - (g.lo[2] + ((double)cz + 0.5) * g.cw[2]), g.L[2], g.h[2]);
+    return make_float4((float)rx, (float)ry, (float)rz, 0.f);
+}
+
 // fast reciprocal: fp32 = MUFU.RCP (about 1 ulp), fp64 = IEEE division
 __device__ __forceinline__ float md_rcp(float x)
 {

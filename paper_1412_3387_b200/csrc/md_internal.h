@@ -32,6 +32,7 @@ struct Geom {
     double h[3];     // L/2
     double lo[3];    // -L/2
     double dn[3];    // (double) cells per axis
+    double cw[3];    // cell widths L/n
     uint32_t n[3];   // cells per axis
     uint32_t n_cells;
     uint32_t N;
@@ -76,6 +77,8 @@ struct md_ctx {
     double4 *force = nullptr, *force_alt = nullptr;  // fx, fy, fz, potential energy
     int *image = nullptr, *image_alt = nullptr;      // 3 per particle
     double *pos_ref = nullptr;                       // 3 per particle: positions at the last binning
+    float4 *rel = nullptr;                           // fp32 position relative to the centre of the particle's binned cell
+                                                     // (kept current by the binning and by half 1; staged by the fp32 tile kernels)
     uint32_t *tag = nullptr, *tag_alt = nullptr;     // slot -> tag
     uint32_t *rtag = nullptr;                        // tag -> slot
     uint32_t *cell_lin = nullptr;                    // slot -> linear cell id (valid after binning)
@@ -90,13 +93,16 @@ struct md_ctx {
     uint32_t *nl_cnt = nullptr;
     uint64_t *nl_off = nullptr;
     uint32_t *nl_idx = nullptr;
-    uint64_t nl_capacity = 0, nl_entries = 0;
+    uint64_t nl_capacity = 0, nl_entries = 0, nl_exact_entries = 0;
     uint32_t *nl_cnt_exp = nullptr;  // row lengths of the decoded / general CSR that the exports read
 
     // tile path (tiles.cu): bricks of tile_B^3 cells, Morton cell order, 16-bit staged indices
     bool use_tiles = false;     // configured (MD_ORDER_MORTON)
     bool nl_is_tile = false;    // the current list is a tile list
     bool nl32_decoded = false;  // nl_off/nl_idx hold the decoded copy of the current tile list (exports)
+    bool nl_cluster = false;    // the current tile list has one row per cluster of 4 particles (k_tile_build_c)
+    int cluster_opt = 0;        // MD_OPT_CLUSTER
+    int stride_mode = -1;       // list format nl_stride was sized for (0 particle rows, 1 cluster rows)
     uint32_t tile_B = 1, n_tiles = 0;
     int tile_B_forced = 0, acc_block = 8;
     uint32_t *tile_cell_begin = nullptr, *tile_origin = nullptr, *lin_of_rank = nullptr;
@@ -134,6 +140,7 @@ struct md_ctx {
     md_stats stats;
     LaunchCfg cfg[MD_N_KERNELS];
     bool tuned = false;
+    bool tune_skip = false;  // set by a tuner replay that could not launch its configuration
     uint64_t device_bytes = 0;
     std::vector<std::pair<void *, uint64_t>> allocs;
     bool log = false;
@@ -186,7 +193,8 @@ int launch_debug_philox(md_ctx *c, const uint32_t *ctr, const uint32_t *key, uin
 int build_cell_order(md_ctx *c);  // host: rank_of_lin table for the configured curve (+ tile tables for Morton)
 // tiles.cu
 int tile_measure(md_ctx *c);
-int launch_tile_build(md_ctx *c, bool *fits);
+int launch_tile_build(md_ctx *c, bool cluster, bool *fits);
+bool tile_cluster_ok(md_ctx *c);
 int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy);
 int launch_tile_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed);
 bool tile_forces_fit(md_ctx *c, bool dpd);

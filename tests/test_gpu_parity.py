@@ -442,6 +442,36 @@ def test_tile_3x3x3_grid_every_image():
             assert force_rel_err(F, oracle.forces_lj(pos, box, 2.5)[0]) < (1e-10 if prec == B.MD_FP64 else 1e-4)
 
 
+@pytest.mark.parametrize("brick", [1, 2])
+def test_cluster_rows_lists_forces_and_steps(brick):
+    """MD_OPT_CLUSTER: one row per cluster of 4 cell members (k_tile_build_c / k_tile_lj4).  The exported list is
+    still the exact per-particle list (bit for bit), forces stay within the mixed-precision bar, energies and DPD go
+    through the decoded list, and a short trajectory follows the oracle."""
+    wl = inputs.lj_fcc(9, rc=3.0, r_buff=0.4, kT=1.2, jitter=0.08, pos_seed=5, vel_seed=6)     # N=2916
+    ref_pairs = oracle.neighbor_pairs(wl.pos, wl.box, wl.r_list)
+    Fr, Er = oracle.forces_lj(wl.pos, wl.box, wl.rc)
+    md = B.from_workload(wl, precision=B.MD_MIXED)
+    md.set_option(B.MD_OPT_TILE_BRICK, brick)
+    md.set_option(B.MD_OPT_CLUSTER, 1)
+    md.set_state(wl.pos, wl.vel)
+    md.build_nlist()
+    assert np.array_equal(sort_pairs(md.get_nlist()), ref_pairs)
+    md.forces_lj()
+    F, E = md.get_forces()                      # energies on demand: decoded-list kernel
+    assert force_rel_err(F, Fr) < 1e-4
+    assert np.abs(E - Er).max() < 1e-3 * np.abs(Er).max()
+    st = md.stats()
+    assert abs(st["mean_neighbors"] - 2.0 * len(ref_pairs) / wl.N) < 1e-9
+    # trajectory: 20 steps (with rebuilds) against the fp64 oracle; mixed forces -> loose bound
+    md.step(B.step_desc("lj", wl.dt, wl.params), 20)
+    sim = oracle.Sim(wl.pos, wl.vel, wl.box, wl.rc, wl.r_buff, {"lj": wl.params}).run(20, wl.dt)
+    pos, _, _ = md.get_state()
+    d = pos - sim.pos
+    d -= wl.box * np.rint(d / wl.box)
+    assert np.abs(d).max() < 1e-5
+    assert md.stats()["dangerous_builds"] == 0
+
+
 def test_mixed_accumulation_blocks_agree():
     wl = inputs.lj_fcc(7, rc=3.0, r_buff=0.4, kT=1.2, jitter=0.05, pos_seed=2, vel_seed=3)
     Fr, _ = oracle.forces_lj(wl.pos, wl.box, 3.0)
