@@ -785,7 +785,13 @@ __device__ __forceinline__ float4 lds_f4(uint32_t addr)
     asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
     return v;
 }
-__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+// 16-byte read-only load of list entries; the L2 sector promotion pulls the rest of the (contiguous) row into L2
+__device__ __forceinline__ uint4 ldg_row(const uint4 *p)
+{
+    uint4 v;
+    asm volatile("ld.global.nc.L2::256B.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+    return v;
+}
 __device__ __forceinline__ unsigned long long lds_u64(uint32_t addr)
 {
     unsigned long long v;
@@ -898,7 +904,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj3(TileParams tp, Geom
     uint4 q_c = make_uint4(0, 0, 0, 0);
     if (p < tc.n_home) {
         cnt_c = __ldg(nl_cnt + tc.g0 + p);
-        q_c = __ldg((const uint4 *)nl16 + (size_t)(tc.g0 + p) * stride8 + lane);
+        q_c = ldg_row((const uint4 *)nl16 + (size_t)(tc.g0 + p) * stride8 + lane);
     }
     for (; p < tc.n_home; p += n_groups) {
         const float4 me = rec[hsidx[p]];
@@ -907,7 +913,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj3(TileParams tp, Geom
         uint4 q = q_c;
         if (p + n_groups < tc.n_home) {
             cnt_c = __ldg(nl_cnt + tc.g0 + p + n_groups);
-            q_c = __ldg(row + (size_t)n_groups * stride8 + lane);
+            q_c = ldg_row(row + (size_t)n_groups * stride8 + lane);
         }
         double fx = 0.0, fy = 0.0, fz = 0.0;
         for (uint32_t b = lane; b < nblk; b += W) {
