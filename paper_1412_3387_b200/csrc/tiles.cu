@@ -986,6 +986,177 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj3(TileParams tp, Geom
 }
 
 // ===============================================================================================================
+// S4a, fp64 (configs 1 and 5): k_tile_lj3d, the fp64 twin of k_tile_lj3.  Records are split into (x, y) pairs of 16
+// bytes -- so the bank-class row layout makes the LDS.128 gather conflict-free exactly as for float4 records -- and a
+// separate z array (LDS.64).  Coordinates are staged divided by sigma; g = (s6 - 1/2) s8, F_i = (48 eps / sigma) sum g d'.
+// The reciprocal is MUFU.RCP64H plus one Newton step (relative error ~2^-46, far inside the 1e-10 bar); the r < rc
+// decision uses the same guard band (fp64 width ~1e-14) with the exact re-test of R2.
+// ===============================================================================================================
+__device__ __forceinline__ double md_rcp_nr1(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y, 1.0);
+    return fma(y, e, y);
+}
+__device__ __forceinline__ double2 lds_d2(uint32_t addr)
+{
+    double2 v;
+    asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ double lds_d(uint32_t addr)
+{
+    double v;
+    asm("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+
+struct LJ3D {
+    double rc2_exact, inv_sigma, fscale, rc2s, guard;
+    double eps4, uc;  // energies: U = 4 eps (s12 - s6) - U(rc), half to each particle
+};
+
+template <bool PRE>
+__device__ __noinline__ void lj3d_block_corr(const uint4 q, uint32_t xy_addr, uint32_t z_addr, double mx, double my, double mz,
+                                            double rc2s, double guard, const double4 *__restrict__ pos, double Lx, double Ly,
+                                            double Lz, double rc2_exact, double eps4, double uc, uint32_t gi,
+                                            const uint32_t *gstart, const uint32_t *sstart, uint32_t n_sc, double *out)
+{
+    const uint32_t qq[4] = {q.x, q.y, q.z, q.w};
+    double ax = 0.0, ay = 0.0, az = 0.0, ae = 0.0;
+#pragma unroll 1
+    for (int e = 0; e < 8; ++e) {
+        const uint32_t ent = (e & 1) ? (qq[e >> 1] >> 16) : (qq[e >> 1] & 0xffffu);
+        const uint32_t s = PRE ? ent >> 4 : ent;
+        const double2 pxy = lds_d2(xy_addr + 16u * s);
+        const double pz = lds_d(z_addr + 8u * s);
+        const double dx = mx - pxy.x, dy = my - pxy.y, dz = mz - pz;
+        const double r2 = dx * dx + dy * dy + dz * dz;
+        if (fabs(r2 - rc2s) < guard) {
+            uint32_t lo = 0, hi = n_sc;
+            while (hi - lo > 1) {
+                const uint32_t mid = (lo + hi) >> 1;
+                if (sstart[mid] <= s) lo = mid; else hi = mid;
+            }
+            if (tile_exact_r2_impl(pos, Lx, Ly, Lz, gi, gstart[lo] + (s - sstart[lo])) < rc2_exact) {
+                const double rinv2 = md_rcp_nr1(r2);
+                const double s6 = rinv2 * rinv2 * rinv2;
+                const double f = (s6 - 0.5) * (s6 * rinv2);
+                ax += f * dx; ay += f * dy; az += f * dz;
+                ae += 0.5 * (eps4 * (s6 * s6 - s6) - uc);
+            }
+        }
+    }
+    out[0] = ax; out[1] = ay; out[2] = az; out[3] = ae;
+}
+
+template <int W, bool PRE, bool ENERGY>
+__global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj3d(TileParams tp, Geom g, const double4 *__restrict__ pos,
+                                                              const uint32_t *__restrict__ nl_cnt,
+                                                              const uint16_t *__restrict__ nl16, LJ3D lj,
+                                                              uint32_t max_staged, double4 *__restrict__ force)
+{
+    extern __shared__ __align__(16) char smem_raw[];
+    double2 *rxy = (double2 *)smem_raw;                       // records first: launch-constant shared addresses
+    double *rz = (double *)(rxy + (max_staged + N_DUMMY));
+    const TileSmem h = tile_carve((char *)(rz + ((max_staged + N_DUMMY + 1) & ~1u)), tp.B);
+    uint8_t *scell = (uint8_t *)h.rest;
+    uint16_t *hsidx = (uint16_t *)(scell + ((max_staged + 16) & ~15u));
+
+    TileCtx tc;
+    tile_setup(tp, g, blockIdx.x, h, tc);
+    {   // stage: coordinates relative to the brick centre, periodic image applied, divided by sigma (see tile_stage)
+        const uint32_t lane32 = threadIdx.x & 31u, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+        for (uint32_t sc = wid; sc < tc.n_sc; sc += nw) {
+            const uint32_t b = h.sstart[sc], e = h.sstart[sc + 1];
+            for (uint32_t s = b + lane32; s < e; s += 32) scell[s] = (uint8_t)sc;
+        }
+        for (uint32_t hc = wid; hc < tc.n_hc; hc += nw) {
+            const uint32_t p0 = h.hc_first[hc], p1 = h.hc_first[hc + 1], s0 = h.sstart[h.hc_sc[hc]];
+            for (uint32_t p = p0 + lane32; p < p1; p += 32) hsidx[p] = (uint16_t)(s0 + (p - p0));
+        }
+        __syncthreads();
+        for (uint32_t s = threadIdx.x; s < tc.n_staged; s += blockDim.x) {
+            const uint32_t sc = scell[s];
+            const double4 p = pos[h.gstart[sc] + (s - h.sstart[sc])];
+            const double *cg = h.cgeo + 6 * sc;
+            rxy[s] = make_double2((cg[3] + md_min_image(p.x - cg[0], g.L[0], g.h[0])) * lj.inv_sigma,
+                                  (cg[4] + md_min_image(p.y - cg[1], g.L[1], g.h[1])) * lj.inv_sigma);
+            rz[s] = (cg[5] + md_min_image(p.z - cg[2], g.L[2], g.h[2])) * lj.inv_sigma;
+        }
+        if (threadIdx.x < N_DUMMY) {
+            rxy[tc.n_staged + threadIdx.x] = make_double2(1e150, 1e150);
+            rz[tc.n_staged + threadIdx.x] = 1e150;
+        }
+    }
+    __syncthreads();
+
+    const unsigned lane = threadIdx.x & (W - 1);
+    const unsigned seg_mask = md_seg_mask<W>();
+    const uint32_t n_groups = blockDim.x / W;
+    const uint32_t xy_addr = (uint32_t)__cvta_generic_to_shared(rxy), z_addr = (uint32_t)__cvta_generic_to_shared(rz);
+    const double rc2s = lj.rc2s, guard = lj.guard, nguard = -lj.guard;
+    const uint32_t stride8 = tp.stride >> 3;
+
+    uint32_t p = threadIdx.x / W;
+    uint32_t cnt_c = 0;
+    uint4 q_c = make_uint4(0, 0, 0, 0);
+    if (p < tc.n_home) {  // software pipeline over the group's particles, as in k_tile_lj3
+        cnt_c = __ldg(nl_cnt + tc.g0 + p);
+        q_c = __ldg((const uint4 *)nl16 + (size_t)(tc.g0 + p) * stride8 + lane);
+    }
+    for (; p < tc.n_home; p += n_groups) {
+        const uint32_t self = hsidx[p];
+        const double2 mxy = rxy[self];
+        const double mz = rz[self];
+        const uint32_t nblk = (cnt_c + 7u) >> 3;
+        const uint4 *row = (const uint4 *)nl16 + (size_t)(tc.g0 + p) * stride8;
+        uint4 q = q_c;
+        if (p + n_groups < tc.n_home) {
+            cnt_c = __ldg(nl_cnt + tc.g0 + p + n_groups);
+            q_c = __ldg(row + (size_t)n_groups * stride8 + lane);
+        }
+        double fx = 0.0, fy = 0.0, fz = 0.0, en = 0.0;
+        for (uint32_t b = lane; b < nblk; b += W) {
+            const uint4 qn = b + W < nblk ? __ldg(row + b + W) : q;  // prefetch the next block of 8 entries
+            const uint32_t qq[4] = {q.x, q.y, q.z, q.w};
+            bool band = false;
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+                const uint32_t ent = (e & 1) ? (qq[e >> 1] >> 16) : (qq[e >> 1] & 0xffffu);
+                // PRE: ent = staged index << 4 = byte offset of the (x, y) record
+                const double2 pxy = lds_d2(xy_addr + (PRE ? ent : 16u * ent));
+                const double pz = lds_d(z_addr + (PRE ? ent >> 1 : 8u * ent));
+                const double dx = mxy.x - pxy.x, dy = mxy.y - pxy.y, dz = mz - pz;
+                const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                const double d = r2 - rc2s;
+                band |= fabs(d) < guard;
+                const double rinv2 = md_rcp_nr1(r2);
+                const double s6 = rinv2 * rinv2 * rinv2;
+                double f = (s6 - 0.5) * (s6 * rinv2);
+                f = d < nguard ? f : 0.0;
+                fx = fma(f, dx, fx); fy = fma(f, dy, fy); fz = fma(f, dz, fz);
+                if (ENERGY) en += d < nguard ? 0.5 * (lj.eps4 * (s6 * s6 - s6) - lj.uc) : 0.0;
+            }
+            if (band) {  // some pair of this block is inside the guard band: exact decisions (rare)
+                double o[4];
+                lj3d_block_corr<PRE>(q, xy_addr, z_addr, mxy.x, mxy.y, mz, rc2s, guard, pos, g.L[0], g.L[1], g.L[2],
+                                     lj.rc2_exact, lj.eps4, lj.uc, tc.g0 + p, h.gstart, h.sstart, tc.n_sc, o);
+                fx += o[0]; fy += o[1]; fz += o[2];
+                if (ENERGY) en += o[3];
+            }
+            q = qn;
+        }
+        fx = md_seg_sum<W>(fx, seg_mask);
+        fy = md_seg_sum<W>(fy, seg_mask);
+        fz = md_seg_sum<W>(fz, seg_mask);
+        if (ENERGY) en = md_seg_sum<W>(en, seg_mask);
+        if (lane == 0) force[tc.g0 + p] = make_double4(fx * lj.fscale, fy * lj.fscale, fz * lj.fscale, en);
+    }
+}
+
+// ===============================================================================================================
 // S4a, mixed precision, cluster rows (k_tile_build_c): k_tile_lj4.  W lanes share a cluster of 4 home particles
 // (i0..i3, held in registers as two packed pairs) and stride over the blocks of the cluster's row; every staged
 // candidate j is loaded once (one LDS.128) and evaluated against the 4 members with f32x2 arithmetic.  Same
@@ -1580,6 +1751,34 @@ int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
         }
         MD_LAUNCH_CHECK(c);
         return MD_OK;
+    }
+    if (!mixed && lj3_mode && !c->nl_cluster) {
+        const size_t ns = c->tile_max_staged + N_DUMMY;
+        const size_t smemd = 16 * ns + 8 * ((ns + 1) & ~(size_t)1) + tile_header_bytes(c->tile_B) +
+                             ((c->tile_max_staged + 16) & ~(size_t)15) + ((2 * (size_t)c->tile_max_home + 15) & ~(size_t)15);
+        if (smemd <= TILE_SMEM_LIMIT) {
+            LJ3D q;
+            q.rc2_exact = p.rc2_exact;
+            q.inv_sigma = 1.0 / sigma;
+            q.fscale = 48.0 * eps / sigma;
+            q.rc2s = p.rc2_exact / p.sig2;
+            q.guard = 2.0 * gd / p.sig2 + 8.0 * 1.1102230246251565e-16 * q.rc2s;
+            q.eps4 = p.eps4;
+            q.uc = p.uc;
+#define LJ3D_LAUNCH(PRE_, EN_)                                                                                              \
+    do {                                                                                                                   \
+        MD_TRY(set_smem(c, (k_tile_lj3d<W_, PRE_, EN_>), smemd));                                                         \
+        k_tile_lj3d<W_, PRE_, EN_><<<c->n_tiles, cf.block, smemd, c->stream>>>(tp, c->g, c->pos, c->nl_cnt, c->nl16, q,    \
+                                                                                c->tile_max_staged, c->force);             \
+    } while (0)
+            MD_DISPATCH_W(cf.w, {
+                if (c->nl_shift) { if (energy) LJ3D_LAUNCH(true, true); else LJ3D_LAUNCH(true, false); }
+                else { if (energy) LJ3D_LAUNCH(false, true); else LJ3D_LAUNCH(false, false); }
+            });
+#undef LJ3D_LAUNCH
+            MD_LAUNCH_CHECK(c);
+            return MD_OK;
+        }
     }
     if (mixed && !energy && c->nl_shift && c->acc_block == 8 && cf.w >= 4 && lj3_mode) {
         const size_t smem = tile_smem_common(c, sizeof(float4), false) + ((2 * (size_t)c->tile_max_home + 15) & ~(size_t)15);
