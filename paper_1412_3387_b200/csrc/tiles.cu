@@ -503,6 +503,205 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build(TileParams tp, Ge
 }
 
 // ===============================================================================================================
+// S2, the default build: k_tile_build8.  A warp task is 8 consecutive home particles of one cell; lane = 8 phase + h
+// holds home particle h and visits the candidates j = base + phase, base + 4 + phase, ... (base a multiple of 8), so
+// the 8 lanes of a quarter-warp read ONE staged record (a broadcast: one wavefront per quarter) and test it against
+// their 8 home particles.  The bank class of a candidate is j & 7 = phase or phase + 4: each (home particle, class) is
+// owned by exactly one lane, which keeps the running count of that class in a register and writes a hit straight to
+// its slot (block k, slot (class - k - rot) & 7) of the row assembled in shared memory -- Fig. 4's compaction
+// with the prefix sum replaced by per-lane counters: no ballot, no popc, no atomics, no
+// communication between lanes until the row is finished (holes, copy-out: as in k_tile_build, 4 rows at a time).
+// ===============================================================================================================
+constexpr int BUILD8_P = 8;
+
+// one x-run of 3 stencil cells [b, e) for one lane: candidates b' + ph, b' + ph + 4, ... (b' = b rounded down to 8).
+// Branch-free: the slot is computed for every candidate, the store and the count are predicated on the hit.
+// SELF: the run holds the lane's own particle (staged index b + selfd), which is not its own neighbour.
+template <bool SELF>
+__device__ __forceinline__ void b8_run(const float4 *rec, uint32_t b, uint32_t e, uint32_t ph, float ax, float ay, float az,
+                                       float th, uint32_t selfd, uint32_t c0, uint32_t c1, uint32_t rcap, uint16_t *myrow,
+                                       uint32_t sh, uint32_t &k0, uint32_t &k1)
+{
+    const uint32_t len = e - b;
+    const uint32_t base0 = b & ~7u;
+    uint32_t d0 = base0 + ph - b;  // candidate index relative to b; "negative" wraps to a huge value and fails d0 < len
+    const float4 *pr = rec + base0 + ph;  // records past the run are other cells' or the dummies: inside the staged array
+    uint32_t ent = (base0 + ph) << sh;
+    const uint32_t dent = 8u << sh, ent4 = 4u << sh;
+#pragma unroll 4
+    for (uint32_t base = base0; base < e; base += 8, d0 += 8, pr += 8, ent += dent) {
+        const float4 pa = pr[0];
+        const float4 pb = pr[4];
+        float t0 = fmaf(ax, pa.x, pa.w), t1 = fmaf(ax, pb.x, pb.w);
+        t0 = fmaf(ay, pa.y, t0); t1 = fmaf(ay, pb.y, t1);
+        t0 = fmaf(az, pa.z, t0); t1 = fmaf(az, pb.z, t1);
+        bool h0 = t0 < th && d0 < len, h1 = t1 < th && d0 + 4u < len;
+        if (SELF) { h0 = h0 && d0 != selfd; h1 = h1 && d0 + 4u != selfd; }
+        const uint32_t o0 = 8u * k0 + ((c0 - k0) & 7u), o1 = 8u * k1 + ((c1 - k1) & 7u);
+        if (h0 && o0 < rcap) myrow[o0] = (uint16_t)ent;
+        if (h1 && o1 < rcap) myrow[o1] = (uint16_t)(ent + ent4);
+        k0 += h0 ? 1u : 0u;
+        k1 += h1 ? 1u : 0u;
+    }
+}
+
+__global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build8(TileParams tp, Geom g, const float4 *__restrict__ rel,
+                                                                float thr_out /* r_list^2 + guard */,
+                                                                uint32_t max_staged, uint32_t *__restrict__ nl_cnt,
+                                                                uint16_t *__restrict__ nl16, DevFlags *flags)
+{
+    constexpr int P = BUILD8_P;
+    extern __shared__ __align__(16) char smem_raw[];
+    const TileSmem h = tile_carve(smem_raw, tp.B);
+    float4 *rec = (float4 *)h.rest;
+    const uint32_t nw = blockDim.x >> 5;
+    // rows of a task are 16 bytes further apart than their capacity: lanes that write the same slot of their 8 rows
+    // (the usual case, the counts run in step) then fall into different banks
+    const uint32_t stride = tp.stride, rcap = tp.stride + RB_EXTRA, rpitch = rcap + 8;
+    uint16_t *rowbuf = (uint16_t *)(h.rest + sizeof(float4) * (max_staged + N_DUMMY));  // [nw][P][rpitch]
+    uint32_t *scratch = (uint32_t *)(rowbuf + (size_t)nw * P * rpitch);                 // [nw][4][24]
+    uint8_t *scell = (uint8_t *)(scratch + nw * 4 * 24);                                // [max_staged]
+
+    TileCtx tc;
+    tile_setup(tp, g, blockIdx.x, h, tc);
+    tile_stage_rel<true>(tc, h, rel, rec, scell, 1.f);
+    if (threadIdx.x < 32) {  // first task of each home cell: exclusive scan of ceil(count / P), n_hc <= 64
+        uint32_t carry = 0;
+        for (uint32_t base = 0; base <= tc.n_hc; base += 32) {
+            const uint32_t hc = base + threadIdx.x;
+            const uint32_t v = hc < tc.n_hc ? (h.hc_first[hc + 1] - h.hc_first[hc] + P - 1) / P : 0u;
+            uint32_t inc = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t u = __shfl_up_sync(0xffffffffu, inc, o);
+                if ((int)threadIdx.x >= o) inc += u;
+            }
+            if (hc <= tc.n_hc) h.hc_task[hc] = carry + inc - v;
+            carry += __shfl_sync(0xffffffffu, inc, 31);
+        }
+    }
+    __syncthreads();
+
+    const unsigned lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;
+    const uint32_t hh = lane & 7u, ph = lane >> 3;  // home particle of the task, candidate phase
+    const uint32_t n_tasks = h.hc_task[tc.n_hc];
+    uint16_t *rb = rowbuf + (size_t)wid * P * rpitch;
+    uint16_t *myrow = rb + hh * rpitch;
+    uint32_t *scr = scratch + wid * 4 * 24;
+    const uint32_t sh = tp.shift;
+    unsigned long long total = 0;
+    uint32_t worst = 0;
+
+    for (uint32_t task = wid; task < n_tasks; task += nw) {
+        uint32_t hc = 0;
+        {
+            uint32_t lo = 0, hi = tc.n_hc;
+            while (hi - lo > 1) {
+                const uint32_t mid = (lo + hi) >> 1;
+                if (h.hc_task[mid] <= task) lo = mid; else hi = mid;
+            }
+            hc = lo;
+        }
+        const uint32_t p0 = h.hc_first[hc] + (task - h.hc_task[hc]) * P;
+        const uint32_t np = min((uint32_t)P, h.hc_first[hc + 1] - p0);
+        const uint32_t sch = h.hc_sc[hc];
+        const uint32_t ixh = sch % tc.sx, iyh = (sch / tc.sx) % tc.sy, izh = sch / (tc.sx * tc.sy);
+        const uint32_t self0 = h.sstart[sch] + (p0 - h.hc_first[hc]);
+        // hit <=> |b|^2 - 2 a.b < thr - |a|^2
+        const float4 m = rec[self0 + min(hh, np - 1)];
+        const float ax = -2.f * m.x, ay = -2.f * m.y, az = -2.f * m.z;
+        const float th = hh < np ? thr_out - m.w : -3e38f;  // absent particles never hit
+        const uint32_t self = self0 + hh;
+        const uint32_t rot = 4u * ((p0 + hh) & 1u);
+        // slot of the k-th entry of class c: 8 k + ((c - k - rot) & 7); c = ph (k0) or ph + 4 (k1)
+        uint32_t k0 = 0, k1 = 0;
+        const uint32_t c0 = ph - rot, c1 = ph + 4u - rot;
+#pragma unroll 1
+        for (int run = 0; run < 9; ++run) {
+            const uint32_t iy = iyh + (run % 3) - 1, iz = izh + (run / 3) - 1;
+            const uint32_t sc0 = (ixh - 1) + tc.sx * (iy + tc.sy * iz);
+            const uint32_t b = h.sstart[sc0], e = h.sstart[sc0 + 3];
+            if (run == 4) b8_run<true>(rec, b, e, ph, ax, ay, az, th, self - b, c0, c1, rcap, myrow, sh, k0, k1);
+            else b8_run<false>(rec, b, e, ph, ax, ay, az, th, 0u, c0, c1, rcap, myrow, sh, k0, k1);
+        }
+        __syncwarp();
+        // finish 4 rows at a time: lane = 8 * row + class; the count of (row, class) lives in lane 8 (class & 3) + row
+#pragma unroll 1
+        for (uint32_t r0 = 0; r0 < np; r0 += 4) {
+            const uint32_t cls = lane & 7u, qr = r0 + (lane >> 3);
+            const uint32_t owner = 8u * (cls & 3u) + (qr & 7u);
+            const uint32_t ka = __shfl_sync(0xffffffffu, k0, owner), kb = __shfl_sync(0xffffffffu, k1, owner);
+            const bool live = qr < np;
+            const uint32_t nc = live ? (cls < 4u ? ka : kb) : 0u;
+            const uint32_t rrot = 4u * ((p0 + qr) & 1u);
+            uint32_t n = nc, mx = nc;
+#pragma unroll
+            for (int o = 1; o < 8; o <<= 1) {
+                n += __shfl_xor_sync(0xffffffffu, n, o);
+                mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+            }
+            // row length in blocks of 8; a class longer than the assembly buffer lost entries -> overflow
+            uint32_t need = (n + 7u) & ~7u;
+            if (8u * mx > rcap) need = max(need, 8u * mx - RB_EXTRA);
+            worst = max(worst, need);
+            const uint32_t nblk = min((n + 7u) >> 3, stride >> 3);
+            uint16_t *r = rb + (qr & 7u) * rpitch;
+            // holes (class shorter than the row) take the entries of longer classes, then dummies of their class
+            const uint32_t nck = min(nc, rcap >> 3);
+            const uint32_t holes = nblk > nck ? nblk - nck : 0u, over = nck > nblk ? nck - nblk : 0u;
+            uint32_t hs = holes, os = over;
+#pragma unroll
+            for (int o = 1; o < 8; o <<= 1) {
+                const uint32_t a = __shfl_up_sync(0xffffffffu, hs, o, 8), bb = __shfl_up_sync(0xffffffffu, os, o, 8);
+                if ((int)cls >= o) { hs += a; os += bb; }
+            }
+            const uint32_t n_holes = __shfl_sync(0xffffffffu, hs, 7, 8), n_over = __shfl_sync(0xffffffffu, os, 7, 8);
+            uint32_t *sc = scr + 24 * (lane >> 3);
+            sc[cls] = nck;
+            sc[8 + cls] = hs - holes;
+            sc[16 + cls] = os - over;
+            __syncwarp();
+            for (uint32_t o = cls; o < n_holes; o += 8) {
+                uint32_t c = 0;
+#pragma unroll
+                for (int k = 1; k < 8; ++k) c += o >= sc[8 + k] ? 1u : 0u;
+                const uint32_t bk = sc[c] + (o - sc[8 + c]);
+                uint16_t v;
+                if (o < n_over) {
+                    uint32_t cs = 0;
+#pragma unroll
+                    for (int k = 1; k < 8; ++k) cs += o >= sc[16 + k] ? 1u : 0u;
+                    const uint32_t k2 = nblk + (o - sc[16 + cs]);
+                    v = r[8u * k2 + ((cs - k2 - rrot) & 7u)];
+                } else {
+                    v = (uint16_t)((tc.n_staged + ((c - tc.n_staged) & 7u)) << sh);
+                }
+                r[8u * bk + ((c - bk - rrot) & 7u)] = v;
+            }
+            __syncwarp();
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const uint32_t nb = __shfl_sync(0xffffffffu, nblk, 8 * q);
+                if (r0 + q < np) {
+                    uint4 *dst = (uint4 *)(nl16 + (size_t)(tc.g0 + p0 + r0 + q) * stride);
+                    const uint4 *src = (const uint4 *)(rb + (r0 + q) * rpitch);
+                    for (uint32_t v = lane; v < nb; v += 32) dst[v] = src[v];
+                }
+            }
+            if (live && cls == 0) {
+                nl_cnt[tc.g0 + p0 + qr] = min(n, 8u * nblk);
+                total += n;
+            }
+            __syncwarp();
+        }
+    }
+    total += __shfl_xor_sync(0xffffffffu, total, 8);
+    total += __shfl_xor_sync(0xffffffffu, total, 16);
+    if (lane == 0 && total) atomicAdd(&flags->nl_total, total);
+    if (worst > stride) atomicMax(&flags->nl_overflow, worst);
+}
+
+// ===============================================================================================================
 // S2, cluster rows: one row per cluster of (up to) P = 4 consecutive members of a home cell (the same warp tasks as
 // above).  A candidate is kept when it lies within r_list (+ guard) of ANY member of the cluster; the cluster's own
 // members are left out (the force kernel handles the pairs inside a cluster separately).  The row is stored in the
@@ -1653,8 +1852,10 @@ int launch_tile_build(md_ctx *c, bool cluster, bool *fits)
     const int block = std::min(c->cfg[MD_K_NLIST].block, TILE_MAX_BLOCK);
     const uint32_t nw = (uint32_t)block / 32;
     size_t smem = tile_smem_common(c, sizeof(float4), false);
-    const size_t rows = cluster ? 1 : BUILD_P;
-    smem += sizeof(uint16_t) * (size_t)nw * rows * (c->nl_stride + RB_EXTRA) + sizeof(uint32_t) * nw * rows * 24;  // row assembly
+    static const int build_mode = getenv("B200MD_BUILD") ? atoi(getenv("B200MD_BUILD")) : 8;
+    const bool b8 = !cluster && build_mode == 8;
+    const size_t rows = cluster ? 1 : (b8 ? BUILD8_P : BUILD_P);
+    smem += sizeof(uint16_t) * (size_t)nw * rows * (c->nl_stride + RB_EXTRA + (b8 ? 8 : 0)) + sizeof(uint32_t) * nw * (b8 ? 4 : rows) * 24;  // row assembly
     *fits = smem <= TILE_SMEM_LIMIT && ms + N_DUMMY <= 65536 && c->tile_B <= 4;
     if (!*fits) return MD_OK;
     c->nl_shift = tile_shift(c);
@@ -1667,6 +1868,10 @@ int launch_tile_build(md_ctx *c, bool cluster, bool *fits)
         MD_TRY(set_smem(c, k_tile_build_c<BUILD_P>, smem));
         k_tile_build_c<BUILD_P><<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->rel, (float)(rl2 + gd), ms, c->nl_cnt,
                                                                        c->nl16, c->d_flags);
+    } else if (b8) {
+        MD_TRY(set_smem(c, k_tile_build8, smem));
+        k_tile_build8<<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->rel, (float)(rl2 + gd), ms, c->nl_cnt, c->nl16,
+                                                             c->d_flags);
     } else {
         MD_TRY(set_smem(c, k_tile_build<BUILD_P>, smem));
         k_tile_build<BUILD_P><<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->rel, (float)(rl2 + gd), ms, c->nl_cnt,
