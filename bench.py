@@ -32,6 +32,11 @@ UNIT = "particle-steps/s"
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed
+# `ncu --set full` capture (profiles/r1_v4_cfg2.md); None where no capture of that workload/kernel exists
+NCU_TRAFFIC = {("cfg2-lj-1M-mixed", "k_tile_lj3"): 459.6e6}
+
+
 def measured_hbm_peak():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -270,6 +275,14 @@ def run_ours(args):
         peak, peak_src = measured_hbm_peak()
         value = world * w.N * args.steps / (ms_max * 1e-3)
         fk = "lj" if w.kind == "lj" else "dpd"
+        if args.order != "morton":
+            kernel = "k_forces_" + fk
+        elif fk == "dpd":
+            kernel = "k_tile_dpd"
+        elif precision == B.MD_MIXED:
+            kernel = "k_tile_lj4" if args.cluster else "k_tile_lj3"
+        else:
+            kernel = "k_tile_lj3d"
         f_ms = st1["stage_ms"][fk] / max(1, st1["stage_launches"][fk])
         achieved = w.N * b_force / (f_ms * 1e-3) / 1e9 if f_ms > 0 else 0.0
         stage_share = {n: round(v / ms, 4) for n, v in st1["stage_ms"].items() if v > 0}
@@ -295,8 +308,9 @@ def run_ours(args):
                     "d2h_bytes_per_step": int(2 * w.pos.nbytes / args.steps)},
             "gpu_launches": int(st1["launches"] - st0["launches"]),
             "clocks": clocks,
-            "roofline": {"bound": "hbm", "kernel": "k_forces_" + fk, "achieved": achieved, "peak": peak,
-                         "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+            "roofline": {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak,
+                         "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": NCU_TRAFFIC.get((w.name, kernel)),
                          "bytes_per_particle": b_force, "launch_ms": f_ms},
         }
         if world == 1 and not args.no_cpu_baseline:
