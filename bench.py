@@ -181,6 +181,22 @@ def run_reference(args):
 
 
 # ----------------------------------------------------------------------------------------------------------------
+def replica_max_times(times_ms, world, device):
+    """Replicas only: no collective on the data path; the only exchange of a multi-rank run is this
+    MAX over the ranks' timed regions (device-timed, max over ranks)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(times_ms), dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def aggregate_value(n_particles, steps, world, ms_max):
+    """Whole-job particle-steps/s of `world` independent replicas of n_particles each, timed by the slowest rank."""
+    return world * n_particles * steps / (ms_max * 1e-3)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -218,6 +234,11 @@ def run_ours(args):
         md.set_bonds(w.bonds)
     if args.cluster:
         md.set_option(B.MD_OPT_CLUSTER, 1)
+    if args.brick:
+        md.set_option(B.MD_OPT_TILE_BRICK, args.brick)
+        md.set_state(d_pos, d_vel)
+        if w.bonds is not None:
+            md.set_bonds(w.bonds)
     for spec in args.launch:                       # e.g. --launch lj=256,4 nlist=768,32 (fixes a kernel's block, w)
         name, val = spec.split("=")
         blk, ww = (int(x) for x in val.split(","))
@@ -261,10 +282,7 @@ def run_ours(args):
     e2e_s = time.perf_counter() - t0
     barrier()
 
-    t = torch.tensor([ms, e2e_s * 1e3], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max, e2e_ms = float(t[0]), float(t[1])
+    ms_max, e2e_ms = replica_max_times([ms, e2e_s * 1e3], world, "cuda")
 
     if rank == 0:
         steps = st1["steps"] - st0["steps"]
@@ -273,7 +291,7 @@ def run_ours(args):
         nbar = st1["mean_neighbors"]
         b_min, b_force = algorithmic_bytes(w.kind, nbar, k)
         peak, peak_src = measured_hbm_peak()
-        value = world * w.N * args.steps / (ms_max * 1e-3)
+        value = aggregate_value(w.N, args.steps, world, ms_max)
         fk = "lj" if w.kind == "lj" else "dpd"
         if args.order != "morton":
             kernel = "k_forces_" + fk
@@ -335,6 +353,7 @@ def main():
     ap.add_argument("--launch", nargs="*", default=[], help="kernel=block,w (with --no-tune)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cluster", action="store_true", help="MD_OPT_CLUSTER = 1: one neighbour row per cluster of 4")
+    ap.add_argument("--brick", type=int, default=0, help="MD_OPT_TILE_BRICK: 1, 2 or 4 cells per brick edge (0 = auto)")
     args = ap.parse_args()
     if args.impl == "reference":
         sys.exit(run_reference(args))

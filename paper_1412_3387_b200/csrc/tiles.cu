@@ -525,23 +525,33 @@ __device__ __forceinline__ void b8_run(const float4 *rec, uint32_t b, uint32_t e
     const uint32_t len = e - b;
     const uint32_t base0 = b & ~7u;
     uint32_t d0 = base0 + ph - b;  // candidate index relative to b; "negative" wraps to a huge value and fails d0 < len
-    const float4 *pr = rec + base0 + ph;  // records past the run are other cells' or the dummies: inside the staged array
+    // 4 candidates per trip and no remainder loop: candidates past the run fail d < len; what is read there are other
+    // cells' records, the dummies or (at the very end of the staged array) the row buffers -- never used
+    const float4 *pr = rec + base0 + ph;
     uint32_t ent = (base0 + ph) << sh;
-    const uint32_t dent = 8u << sh, ent4 = 4u << sh;
-#pragma unroll 4
-    for (uint32_t base = base0; base < e; base += 8, d0 += 8, pr += 8, ent += dent) {
-        const float4 pa = pr[0];
-        const float4 pb = pr[4];
-        float t0 = fmaf(ax, pa.x, pa.w), t1 = fmaf(ax, pb.x, pb.w);
-        t0 = fmaf(ay, pa.y, t0); t1 = fmaf(ay, pb.y, t1);
-        t0 = fmaf(az, pa.z, t0); t1 = fmaf(az, pb.z, t1);
-        bool h0 = t0 < th && d0 < len, h1 = t1 < th && d0 + 4u < len;
-        if (SELF) { h0 = h0 && d0 != selfd; h1 = h1 && d0 + 4u != selfd; }
-        const uint32_t o0 = 8u * k0 + ((c0 - k0) & 7u), o1 = 8u * k1 + ((c1 - k1) & 7u);
-        if (h0 && o0 < rcap) myrow[o0] = (uint16_t)ent;
-        if (h1 && o1 < rcap) myrow[o1] = (uint16_t)(ent + ent4);
-        k0 += h0 ? 1u : 0u;
-        k1 += h1 ? 1u : 0u;
+    const uint32_t dent = 16u << sh, e4 = 4u << sh;
+#pragma unroll 2
+    for (uint32_t base = base0; base < e; base += 16, d0 += 16, pr += 16, ent += dent) {
+        float t[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const float4 pc = pr[4 * u];
+            t[u] = fmaf(az, pc.z, fmaf(ay, pc.y, fmaf(ax, pc.x, pc.w)));
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            bool hit = t[u] < th && d0 + 4u * u < len;
+            if (SELF) hit = hit && d0 + 4u * u != selfd;
+            if (u & 1) {
+                const uint32_t o = 8u * k1 + ((c1 - k1) & 7u);
+                if (hit && o < rcap) myrow[o] = (uint16_t)(ent + u * e4);
+                k1 += hit ? 1u : 0u;
+            } else {
+                const uint32_t o = 8u * k0 + ((c0 - k0) & 7u);
+                if (hit && o < rcap) myrow[o] = (uint16_t)(ent + u * e4);
+                k0 += hit ? 1u : 0u;
+            }
+        }
     }
 }
 
@@ -1087,32 +1097,43 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj3(TileParams tp, Geom
         const uint32_t p0 = h.hc_first[hc], p1 = h.hc_first[hc + 1], s0 = h.sstart[h.hc_sc[hc]];
         for (uint32_t p = p0 + (threadIdx.x & 31u); p < p1; p += 32) hsidx[p] = (uint16_t)(s0 + (p - p0));
     }
+    __shared__ uint32_t next_p[2];  // next unassigned home particle of each parity, in units of 2
+    if (threadIdx.x < 2) next_p[threadIdx.x] = blockDim.x / (2 * W);
     __syncthreads();
 
     const unsigned lane = threadIdx.x & (W - 1);
     const unsigned seg_mask = md_seg_mask<W>();
-    const uint32_t n_groups = blockDim.x / W;
     const uint32_t rec_addr = (uint32_t)__cvta_generic_to_shared(rec);
     const float rc2s = lj.rc2s, guard = lj.guard, nguard = -lj.guard;
     const uint32_t stride8 = tp.stride >> 3;
 
     // software pipeline over the group's particles: the row length and the first block of the NEXT particle are
     // requested before the current one is evaluated (rows have a fixed stride, so block `lane` of a row always exists)
-    uint32_t p = threadIdx.x / W;
+    // Particles are handed out dynamically (rows differ in length): a group takes the next particle of ITS parity --
+    // the bank-class layout ties the parity of the home index to the half of the quarter-warp the group sits in --
+    // from a shared counter, one particle ahead of the one it evaluates.
+    const uint32_t grp = threadIdx.x / W, par = grp & 1u;
+    auto grab = [&]() -> uint32_t {
+        uint32_t v = 0;
+        if (lane == 0) v = atomicAdd(&next_p[par], 1u);
+        return 2u * __shfl_sync(seg_mask, v, 0, W) + par;
+    };
+    uint32_t p = grp;
     uint32_t cnt_c = 0;
     uint4 q_c = make_uint4(0, 0, 0, 0);
     if (p < tc.n_home) {
         cnt_c = __ldg(nl_cnt + tc.g0 + p);
         q_c = ldg_row((const uint4 *)nl16 + (size_t)(tc.g0 + p) * stride8 + lane);
     }
-    for (; p < tc.n_home; p += n_groups) {
+    while (p < tc.n_home) {
         const float4 me = rec[hsidx[p]];
         const uint32_t nblk = (cnt_c + 7u) >> 3;
         const uint4 *row = (const uint4 *)nl16 + (size_t)(tc.g0 + p) * stride8;
         uint4 q = q_c;
-        if (p + n_groups < tc.n_home) {
-            cnt_c = __ldg(nl_cnt + tc.g0 + p + n_groups);
-            q_c = ldg_row(row + (size_t)n_groups * stride8 + lane);
+        const uint32_t pn = grab();
+        if (pn < tc.n_home) {
+            cnt_c = __ldg(nl_cnt + tc.g0 + pn);
+            q_c = ldg_row((const uint4 *)nl16 + (size_t)(tc.g0 + pn) * stride8 + lane);
         }
         double fx = 0.0, fy = 0.0, fz = 0.0;
         for (uint32_t b = lane; b < nblk; b += W) {
@@ -1181,6 +1202,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj3(TileParams tp, Geom
         fy = md_seg_sum<W>(fy, seg_mask);
         fz = md_seg_sum<W>(fz, seg_mask);
         if (lane == 0) force[tc.g0 + p] = make_double4(fx * lj.fscale, fy * lj.fscale, fz * lj.fscale, 0.0);
+        p = pn;
     }
 }
 
