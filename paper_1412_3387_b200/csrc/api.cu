@@ -234,6 +234,7 @@ static uint32_t choose_brick(md_ctx *c)
 
 int build_cell_order(md_ctx *c)
 {
+    c->tile_desc_valid = false;
     for (uint32_t **p : {&c->rank_of_lin, &c->lin_of_rank, &c->tile_cell_begin, &c->tile_origin})
         if (*p) { md_free(c, *p); *p = nullptr; }
     c->use_tiles = false;
@@ -511,6 +512,7 @@ static int do_build_cells(md_ctx *c)
 {
     ProfScope ps(c, MD_K_CELLS);
     MD_TRY(launch_build_cells(c));
+    c->tile_desc_valid = false;  // the per-tile header tables follow cell_start
     c->cells_valid = true;
     c->nlist_valid = false;
     c->steps_since_build = 0;

@@ -107,6 +107,9 @@ struct md_ctx {
     int tile_B_forced = 0, acc_block = 8;
     uint32_t *tile_cell_begin = nullptr, *tile_origin = nullptr, *lin_of_rank = nullptr;
     uint32_t tile_max_home = 0, tile_max_staged = 0;
+    uint32_t *tile_desc = nullptr;   // per-tile header tables written by k_tile_header at every rebuild
+    uint64_t tile_desc_len = 0;      // words allocated
+    bool tile_desc_valid = false;    // tile_desc matches the current binning
     uint16_t *nl16 = nullptr;        // fixed-stride rows: row of slot i starts at nl16 + i * nl_stride
     uint32_t nl_stride = 0;          // entries per row, multiple of 16
     uint32_t nl_shift = 0;           // entry = staged index << nl_shift

@@ -48,7 +48,16 @@ struct TileParams {
     const uint32_t *rank_of_lin;      // linear id -> cell rank
     const uint32_t *cell_start;       // [n_cells+1] first particle slot of each cell rank
     double cw[3];                     // cell widths
+    const uint32_t *desc;             // per-tile header precomputed at the rebuild (k_tile_header), or nullptr
+    uint32_t desc_words;              // words per tile in desc
 };
+
+constexpr uint32_t TILE_DESC_CTX = 16;  // words reserved for the TileCtx at the start of a tile's descriptor
+__host__ __device__ inline uint32_t tile_desc_table_words(uint32_t B)
+{
+    const uint32_t nsc = (B + 2) * (B + 2) * (B + 2), nhc = B * B * B;
+    return nsc + (nsc + 1) + nhc + (nhc + 1);  // gstart, sstart, hc_sc, hc_first: contiguous in TileSmem
+}
 
 struct TileCtx {
     uint32_t x0, y0, z0, ex, ey, ez, sx, sy, sz, n_sc, n_staged, n_home, g0, cb, n_hc;
@@ -99,6 +108,32 @@ __device__ __forceinline__ TileSmem tile_carve(char *smem, uint32_t B)
 // ---------------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void tile_setup(const TileParams &tp, const Geom &g, uint32_t t, const TileSmem &h, TileCtx &tc)
 {
+    if (tp.desc) {
+        // the tables depend on the binning only: k_tile_header wrote them at the rebuild; one coalesced copy and one
+        // barrier instead of four dependent global round trips, a scan and three barriers
+        const uint32_t *d = tp.desc + (size_t)t * tp.desc_words;
+        const uint32_t words = tile_desc_table_words(tp.B);
+        for (uint32_t i = threadIdx.x; i < words; i += blockDim.x) h.gstart[i] = __ldg(d + TILE_DESC_CTX + i);
+        uint32_t *tcw = (uint32_t *)&tc;
+#pragma unroll
+        for (int i = 0; i < (int)(sizeof(TileCtx) / 4); ++i) tcw[i] = __ldg(d + i);
+        for (uint32_t sc = threadIdx.x; sc < tc.n_sc; sc += blockDim.x) {
+            const uint32_t ix = sc % tc.sx, iy = (sc / tc.sx) % tc.sy, iz = sc / (tc.sx * tc.sy);
+            const uint32_t cx = (tc.x0 + ix + g.n[0] - 1) % g.n[0];
+            const uint32_t cy = (tc.y0 + iy + g.n[1] - 1) % g.n[1];
+            const uint32_t cz = (tc.z0 + iz + g.n[2] - 1) % g.n[2];
+            double *cg = h.cgeo + 6 * sc;
+            cg[0] = g.lo[0] + ((double)cx + 0.5) * tp.cw[0];
+            cg[1] = g.lo[1] + ((double)cy + 0.5) * tp.cw[1];
+            cg[2] = g.lo[2] + ((double)cz + 0.5) * tp.cw[2];
+            cg[3] = ((double)ix - 0.5 - 0.5 * (double)tc.ex) * tp.cw[0];
+            cg[4] = ((double)iy - 0.5 - 0.5 * (double)tc.ey) * tp.cw[1];
+            cg[5] = ((double)iz - 0.5 - 0.5 * (double)tc.ez) * tp.cw[2];
+            h.coff[sc] = make_float4((float)cg[3], (float)cg[4], (float)cg[5], 0.f);
+        }
+        __syncthreads();
+        return;
+    }
     tc.x0 = tp.tile_origin[3 * t];
     tc.y0 = tp.tile_origin[3 * t + 1];
     tc.z0 = tp.tile_origin[3 * t + 2];
@@ -281,26 +316,24 @@ __device__ __forceinline__ double tile_exact_r2(const double4 *__restrict__ pos,
 }
 
 // ===============================================================================================================
-// sizes of the largest tile (for shared-memory sizing), one thread per tile
+// once per rebuild, one CTA per tile: the tile's header tables (tile_setup's slow path) go to global memory, and the
+// sizes of the largest tile (shared-memory sizing) to the flags
 // ===============================================================================================================
-__global__ void k_tile_sizes(TileParams tp, Geom g, unsigned int *max_home, unsigned int *max_staged)
+__global__ void k_tile_header(TileParams tp, Geom g, uint32_t *desc, unsigned int *max_home, unsigned int *max_staged)
 {
-    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= tp.n_tiles) return;
-    const uint32_t x0 = tp.tile_origin[3 * t], y0 = tp.tile_origin[3 * t + 1], z0 = tp.tile_origin[3 * t + 2];
-    const uint32_t sx = min(tp.B, g.n[0] - x0) + 2, sy = min(tp.B, g.n[1] - y0) + 2, sz = min(tp.B, g.n[2] - z0) + 2;
-    uint32_t staged = 0;
-    for (uint32_t iz = 0; iz < sz; ++iz)
-        for (uint32_t iy = 0; iy < sy; ++iy)
-            for (uint32_t ix = 0; ix < sx; ++ix) {
-                const uint32_t cx = (x0 + ix + g.n[0] - 1) % g.n[0], cy = (y0 + iy + g.n[1] - 1) % g.n[1],
-                               cz = (z0 + iz + g.n[2] - 1) % g.n[2];
-                const uint32_t r = tp.rank_of_lin[cx + g.n[0] * (cy + g.n[1] * cz)];
-                staged += tp.cell_start[r + 1] - tp.cell_start[r];
-            }
-    const uint32_t cb = tp.tile_cell_begin[t], ce = tp.tile_cell_begin[t + 1];
-    atomicMax(max_home, tp.cell_start[ce] - tp.cell_start[cb]);
-    atomicMax(max_staged, staged);
+    extern __shared__ __align__(16) char smem_raw[];
+    const TileSmem h = tile_carve(smem_raw, tp.B);
+    TileCtx tc;
+    tile_setup(tp, g, blockIdx.x, h, tc);  // tp.desc == nullptr here
+    uint32_t *d = desc + (size_t)blockIdx.x * tp.desc_words;
+    const uint32_t words = tile_desc_table_words(tp.B);
+    for (uint32_t i = threadIdx.x; i < words; i += blockDim.x) d[TILE_DESC_CTX + i] = h.gstart[i];
+    if (threadIdx.x == 0) {
+        const uint32_t *tcw = (const uint32_t *)&tc;
+        for (int i = 0; i < (int)(sizeof(TileCtx) / 4); ++i) d[i] = tcw[i];
+        atomicMax(max_home, tc.n_home);
+        atomicMax(max_staged, tc.n_staged);
+    }
 }
 
 // ===============================================================================================================
@@ -1077,7 +1110,7 @@ __device__ __noinline__ void lj3_block_corr(const uint4 q, uint32_t rec_addr, fl
 }
 
 template <int W, bool X2>
-__global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj3(TileParams tp, Geom g, const double4 *__restrict__ pos,
+__global__ void __launch_bounds__(256, 4) k_tile_lj3(TileParams tp, Geom g, const double4 *__restrict__ pos,
                                                              const float4 *__restrict__ rel,
                                                              const uint32_t *__restrict__ nl_cnt,
                                                              const uint16_t *__restrict__ nl16, LJ3 lj,
@@ -1800,6 +1833,8 @@ static TileParams make_tp(md_ctx *c)
     tp.rank_of_lin = c->rank_of_lin;
     tp.cell_start = c->cell_start;
     for (int a = 0; a < 3; ++a) tp.cw[a] = c->box[a] / (double)c->dims[a];
+    tp.desc_words = (TILE_DESC_CTX + tile_desc_table_words(c->tile_B) + 3u) & ~3u;
+    tp.desc = c->tile_desc_valid ? c->tile_desc : nullptr;
     return tp;
 }
 
@@ -1847,8 +1882,21 @@ static size_t tile_smem_common(md_ctx *c, size_t rec_bytes, bool with_vel)
 int tile_measure(md_ctx *c)
 {
     MD_CUDA_CHECK(c, cudaMemsetAsync(&c->d_flags->max_home, 0, 2 * sizeof(unsigned int), c->stream));
-    k_tile_sizes<<<md_grid(c->n_tiles, 128), 128, 0, c->stream>>>(make_tp(c), c->g, &c->d_flags->max_home, &c->d_flags->max_staged);
+    c->tile_desc_valid = false;
+    TileParams tp = make_tp(c);  // slow-path setup inside k_tile_header
+    const uint64_t need = (uint64_t)c->n_tiles * tp.desc_words;
+    if (need > c->tile_desc_len) {
+        if (c->tile_desc) { md_free(c, c->tile_desc); c->tile_desc = nullptr; }
+        c->tile_desc_len = 0;
+        MD_TRY(md_alloc(c, (void **)&c->tile_desc, need * sizeof(uint32_t)));
+        c->tile_desc_len = need;
+    }
+    const size_t smem = tile_header_bytes(c->tile_B);
+    if (smem > 48 * 1024)
+        MD_CUDA_CHECK(c, cudaFuncSetAttribute(k_tile_header, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_tile_header<<<c->n_tiles, 128, smem, c->stream>>>(tp, c->g, c->tile_desc, &c->d_flags->max_home, &c->d_flags->max_staged);
     MD_LAUNCH_CHECK(c);
+    c->tile_desc_valid = true;
     return MD_OK;
 }
 
@@ -2018,6 +2066,7 @@ int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
         // guard in scaled units: the fp32 error bound of r'^2 plus the rounding of rc'^2 itself
         q.guard = (float)(1.0001 * (gd / p.sig2 + 2.0 * 5.9604644775390625e-08 * rc2s));
         const int w = cf.w > 8 ? 8 : cf.w;
+        cf.block = std::min(cf.block, 256);  // k_tile_lj3 is compiled for 4 CTAs of 256 threads per SM (64 registers)
         if (w == 4) {
             if (lj3_mode == 2) {
                 MD_TRY(set_smem(c, k_tile_lj3<4, true>, smem));
