@@ -290,12 +290,28 @@ __device__ __forceinline__ void tile_stage_rel(const TileCtx &tc, const TileSmem
         for (uint32_t s = b + lane; s < e; s += 32) scell[s] = (uint8_t)sc;
     }
     __syncthreads();
-    for (uint32_t s = threadIdx.x; s < tc.n_staged; s += blockDim.x) {
-        const uint32_t sc = scell[s];
-        const float4 r = __ldg(rel + h.gstart[sc] + (s - h.sstart[sc]));
-        const float4 o = h.coff[sc];
-        const float x = (r.x + o.x) * scale, y = (r.y + o.y) * scale, z = (r.z + o.z) * scale;
-        rec[s] = make_float4(x, y, z, WITH_R2 ? x * x + y * y + z * z : 0.f);
+    // 4 records per thread and trip, all 4 global loads issued before the first is used: the loop is a chain of L2
+    // round trips otherwise (a thread stages ~9 records)
+    for (uint32_t s0 = threadIdx.x; s0 < tc.n_staged; s0 += 4 * blockDim.x) {
+        float4 r[4];
+        uint32_t scs[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const uint32_t s = s0 + u * blockDim.x;
+            if (s < tc.n_staged) {
+                scs[u] = scell[s];
+                r[u] = __ldg(rel + h.gstart[scs[u]] + (s - h.sstart[scs[u]]));
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const uint32_t s = s0 + u * blockDim.x;
+            if (s < tc.n_staged) {
+                const float4 o = h.coff[scs[u]];
+                const float x = (r[u].x + o.x) * scale, y = (r[u].y + o.y) * scale, z = (r[u].z + o.z) * scale;
+                rec[s] = make_float4(x, y, z, WITH_R2 ? x * x + y * y + z * z : 0.f);
+            }
+        }
     }
     if (threadIdx.x < N_DUMMY) rec[tc.n_staged + threadIdx.x] = RecTraits<float4>::far();
 }
@@ -1331,13 +1347,28 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj3d(TileParams tp, Geo
             for (uint32_t p = p0 + lane32; p < p1; p += 32) hsidx[p] = (uint16_t)(s0 + (p - p0));
         }
         __syncthreads();
-        for (uint32_t s = threadIdx.x; s < tc.n_staged; s += blockDim.x) {
-            const uint32_t sc = scell[s];
-            const double4 p = pos[h.gstart[sc] + (s - h.sstart[sc])];
-            const double *cg = h.cgeo + 6 * sc;
-            rxy[s] = make_double2((cg[3] + md_min_image(p.x - cg[0], g.L[0], g.h[0])) * lj.inv_sigma,
-                                  (cg[4] + md_min_image(p.y - cg[1], g.L[1], g.h[1])) * lj.inv_sigma);
-            rz[s] = (cg[5] + md_min_image(p.z - cg[2], g.L[2], g.h[2])) * lj.inv_sigma;
+        for (uint32_t s0 = threadIdx.x; s0 < tc.n_staged; s0 += 2 * blockDim.x) {  // 2 loads in flight per thread
+            double4 pp[2];
+            uint32_t scs[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const uint32_t s = s0 + u * blockDim.x;
+                if (s < tc.n_staged) {
+                    scs[u] = scell[s];
+                    pp[u] = pos[h.gstart[scs[u]] + (s - h.sstart[scs[u]])];
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const uint32_t s = s0 + u * blockDim.x;
+                if (s < tc.n_staged) {
+                    const double4 p = pp[u];
+                    const double *cg = h.cgeo + 6 * scs[u];
+                    rxy[s] = make_double2((cg[3] + md_min_image(p.x - cg[0], g.L[0], g.h[0])) * lj.inv_sigma,
+                                          (cg[4] + md_min_image(p.y - cg[1], g.L[1], g.h[1])) * lj.inv_sigma);
+                    rz[s] = (cg[5] + md_min_image(p.z - cg[2], g.L[2], g.h[2])) * lj.inv_sigma;
+                }
+            }
         }
         if (threadIdx.x < N_DUMMY) {
             rxy[tc.n_staged + threadIdx.x] = make_double2(1e150, 1e150);
