@@ -1781,6 +1781,155 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_dpd(TileParams tp, Geom
 }
 
 // ===============================================================================================================
+// S4b, two-phase variant (the default): k_tile_dpd2.  Only ~38 % of the list entries of a DPD fluid are inside rc
+// (r_list = 1.4 rc), and the pair term is heavy (fp64 rsqrt, 10 Philox rounds): evaluated in place, every lane of a
+// warp pays for it at every entry at which ANY lane is in range.  Phase 1 runs the distance test over the group's
+// row and compacts the in-range entries (W-lane prefix sum of the hit counts, the paper's Fig. 4 compaction applied
+// to the force loop) into a per-group list in shared memory; phase 2 deals that list out evenly to the W lanes.
+// Records are split into 16-byte pairs (x,y) (z,vx) (vy,vz) + a tag array, so that with the bank-class row layout the
+// gathers are conflict-free (see k_tile_lj3d).
+// ===============================================================================================================
+__device__ __forceinline__ double md_rsqrt_nr1(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double t = x * y;
+    return fma(y * 0.5, fma(-t, y, 1.0), y);  // one Newton step: relative error ~2^-45
+}
+
+template <int W>
+__global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_dpd2(TileParams tp, Geom g, const double4 *__restrict__ pos,
+                                                              const double4 *__restrict__ vel,
+                                                              const uint32_t *__restrict__ nl_cnt,
+                                                              const uint16_t *__restrict__ nl16, DPDTile dp,
+                                                              uint32_t max_staged, uint32_t max_home,
+                                                              double4 *__restrict__ force)
+{
+    extern __shared__ __align__(16) char smem_raw[];
+    const uint32_t ns = max_staged + N_DUMMY;
+    double2 *ra = (double2 *)smem_raw;  // (x, y)
+    double2 *rb = ra + ns;              // (z, vx)
+    double2 *rc = rb + ns;              // (vy, vz)
+    uint32_t *rt = (uint32_t *)(rc + ns);                                   // tag
+    const TileSmem h = tile_carve((char *)(rt + ((ns + 3u) & ~3u)), tp.B);
+    uint8_t *scell = (uint8_t *)h.rest;
+    uint16_t *hsidx = (uint16_t *)(scell + ((max_staged + 16) & ~15u));
+    uint16_t *stash = hsidx + ((max_home + 7u) & ~7u);                      // [stride][n_groups] in-range entries
+
+    TileCtx tc;
+    tile_setup(tp, g, blockIdx.x, h, tc);
+    {
+        const uint32_t lane32 = threadIdx.x & 31u, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+        for (uint32_t sc = wid; sc < tc.n_sc; sc += nw) {
+            const uint32_t b = h.sstart[sc], e = h.sstart[sc + 1];
+            for (uint32_t s = b + lane32; s < e; s += 32) scell[s] = (uint8_t)sc;
+        }
+        for (uint32_t hc = wid; hc < tc.n_hc; hc += nw) {
+            const uint32_t p0 = h.hc_first[hc], p1 = h.hc_first[hc + 1], s0 = h.sstart[h.hc_sc[hc]];
+            for (uint32_t p = p0 + lane32; p < p1; p += 32) hsidx[p] = (uint16_t)(s0 + (p - p0));
+        }
+        __syncthreads();
+        for (uint32_t s = threadIdx.x; s < tc.n_staged; s += blockDim.x) {
+            const uint32_t sc = scell[s];
+            const uint32_t gi = h.gstart[sc] + (s - h.sstart[sc]);
+            const double4 p = pos[gi];
+            const double4 v = vel[gi];
+            const double *cg = h.cgeo + 6 * sc;
+            ra[s] = make_double2(cg[3] + md_min_image(p.x - cg[0], g.L[0], g.h[0]),
+                                 cg[4] + md_min_image(p.y - cg[1], g.L[1], g.h[1]));
+            rb[s] = make_double2(cg[5] + md_min_image(p.z - cg[2], g.L[2], g.h[2]), v.x);
+            rc[s] = make_double2(v.y, v.z);
+            rt[s] = md_lane_to_tag(p.w);
+        }
+        if (threadIdx.x < N_DUMMY) {
+            ra[tc.n_staged + threadIdx.x] = make_double2(1e150, 1e150);
+            rb[tc.n_staged + threadIdx.x] = make_double2(1e150, 0.0);
+        }
+    }
+    __syncthreads();
+
+    const unsigned lane = threadIdx.x & (W - 1);
+    const unsigned seg_mask = md_seg_mask<W>();
+    const uint32_t n_groups = blockDim.x / W, grp = threadIdx.x / W;
+    const uint32_t stride8 = tp.stride >> 3;
+    const uint32_t sh = tp.shift;
+    uint16_t *my_stash = stash + grp;
+
+    for (uint32_t p = grp; p < tc.n_home; p += n_groups) {
+        const uint32_t self = hsidx[p];
+        const double2 ma = ra[self], mb = rb[self], mc = rc[self];
+        const uint32_t ti = rt[self];
+        const uint32_t nblk = (nl_cnt[tc.g0 + p] + 7u) >> 3;
+        const uint4 *row = (const uint4 *)nl16 + (size_t)(tc.g0 + p) * stride8;
+        // ---- phase 1: distance tests, in-range entries compacted into the group's list
+        uint32_t n_in = 0;  // entries in the list so far (the same in all lanes of the group)
+        for (uint32_t b0 = 0; b0 < nblk; b0 += W) {
+            const uint32_t b = b0 + lane;
+            uint32_t hits = 0;
+            uint4 q = make_uint4(0, 0, 0, 0);
+            if (b < nblk) {
+                q = __ldg(row + b);
+                const uint32_t qq[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const uint32_t j = ((qq[e >> 1] >> ((e & 1) * 16)) & 0xffffu) >> sh;
+                    const double2 pa = ra[j];
+                    const double pz = rb[j].x;
+                    const double dx = ma.x - pa.x, dy = ma.y - pa.y, dz = mb.x - pz;
+                    const double r2 = dx * dx + dy * dy + dz * dz;
+                    bool in = r2 < dp.thr_in;
+                    if (!in && r2 < dp.thr_out)
+                        in = tile_exact_r2(pos, g, tc.g0 + p, tile_global_of_staged(h, tc.n_sc, j)) < dp.rc2_exact;
+                    if (in && r2 > 0.0) hits |= 1u << e;
+                }
+            }
+            // exclusive prefix of the hit counts over the W lanes of the group
+            const uint32_t c = __popc(hits);
+            uint32_t inc = c;
+#pragma unroll
+            for (int o = 1; o < W; o <<= 1) {
+                const uint32_t u = __shfl_up_sync(seg_mask, inc, o, W);
+                if ((int)lane >= o) inc += u;
+            }
+            uint32_t k = n_in + inc - c;
+            n_in += __shfl_sync(seg_mask, inc, W - 1, W);
+            const uint32_t qq[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+                if ((hits >> e) & 1u) {
+                    my_stash[k * n_groups] = (uint16_t)(((qq[e >> 1] >> ((e & 1) * 16)) & 0xffffu) >> sh);
+                    ++k;
+                }
+            }
+        }
+        __syncwarp(seg_mask);
+        // ---- phase 2: the heavy pair term, in-range pairs dealt out evenly to the W lanes
+        const double vix = mb.y, viy = mc.x, viz = mc.y;
+        double fx = 0.0, fy = 0.0, fz = 0.0, en = 0.0;
+        for (uint32_t k = lane; k < n_in; k += W) {
+            const uint32_t j = my_stash[k * n_groups];
+            const double2 pa = ra[j], pb = rb[j], pc = rc[j];
+            const double dx = ma.x - pa.x, dy = ma.y - pa.y, dz = mb.x - pb.x;
+            const double r2 = dx * dx + dy * dy + dz * dz;
+            const double rinv = md_rsqrt_nr1(r2);
+            const double r = r2 * rinv;
+            const double w = 1.0 - r * dp.inv_rc;
+            const double rv = (dx * (vix - pb.y) + dy * (viy - pc.x) + dz * (viz - pc.y)) * rinv;
+            const double theta = md_dpd_theta(ti, rt[j], dp.step, dp.seed);
+            const double f = (dp.A * w - dp.gamma * w * w * rv + dp.sr * w * theta) * rinv;
+            fx += f * dx; fy += f * dy; fz += f * dz;
+            en += 0.25 * dp.A * dp.rc * w * w;
+        }
+        __syncwarp(seg_mask);
+        fx = md_seg_sum<W>(fx, seg_mask);
+        fy = md_seg_sum<W>(fy, seg_mask);
+        fz = md_seg_sum<W>(fz, seg_mask);
+        en = md_seg_sum<W>(en, seg_mask);
+        if (lane == 0) force[tc.g0 + p] = make_double4(fx, fy, fz, en);
+    }
+}
+
+// ===============================================================================================================
 // decode the 16-bit tile list into the general 32-bit CSR (exports / parity read-back only).  The stored list is a
 // guard-band superset; here every entry is tested with the exact fp64 expression (R2) on the positions the
 // list was built from (pos_ref, the snapshot taken at the binning), so the exported list is the plain definition.
@@ -2146,8 +2295,26 @@ int launch_tile_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uin
     const double gd = guard_fp64(tile_extent(c), c->rc * 1.001);
     p.thr_in = p.rc2_exact - gd;
     p.thr_out = p.rc2_exact + gd;
-    const size_t smem = tile_smem_common(c, sizeof(double4), true);
     TileParams tp = make_tp(c);
+    static const int dpd_mode = getenv("B200MD_DPD") ? atoi(getenv("B200MD_DPD")) : 2;
+    if (dpd_mode == 2) {
+        const size_t ns = c->tile_max_staged + N_DUMMY;
+        const int w = std::max(1, std::min(cf.w, 32));
+        const size_t n_groups = (size_t)cf.block / w;
+        const size_t smem2 = 48 * ns + 4 * ((ns + 3) & ~(size_t)3) + tile_header_bytes(c->tile_B) +
+                             ((c->tile_max_staged + 16) & ~(size_t)15) + 2 * (((size_t)c->tile_max_home + 7) & ~(size_t)7) +
+                             2 * n_groups * c->nl_stride;
+        if (smem2 <= TILE_SMEM_LIMIT) {
+            MD_DISPATCH_W(cf.w, {
+                MD_TRY(set_smem(c, k_tile_dpd2<W_>, smem2));
+                k_tile_dpd2<W_><<<c->n_tiles, cf.block, smem2, c->stream>>>(tp, c->g, c->pos, c->vel, c->nl_cnt, c->nl16, p,
+                                                                         c->tile_max_staged, c->tile_max_home, c->force);
+            });
+            MD_LAUNCH_CHECK(c);
+            return MD_OK;
+        }
+    }
+    const size_t smem = tile_smem_common(c, sizeof(double4), true);
     MD_DISPATCH_W(cf.w, {
         MD_TRY(set_smem(c, k_tile_dpd<W_>, smem));
         k_tile_dpd<W_><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->vel, c->nl_cnt, c->nl16, p,
