@@ -840,6 +840,7 @@ extern "C" int md_step(md_ctx *c, const md_step_desc *w, uint64_t n_steps)
     if (!c->have_state) { c->err = "md_step: md_set_state first"; return MD_ESTATE; }
     if (!(w->dt > 0.0)) { c->err = "md_step: dt must be positive"; return MD_EINVAL; }
     if (n_steps == 0) return MD_OK;
+    c->force_hint = w->flags;
     if (!c->nlist_valid) MD_TRY(rebuild(c));
     if (!c->force_valid) MD_TRY(eval_forces(c, w, c->step, false));  // R16: F(t0) before the first half-kick
     if (!c->ev_flags) MD_CUDA_CHECK(c, cudaEventCreateWithFlags(&c->ev_flags, cudaEventDisableTiming));
@@ -944,6 +945,7 @@ extern "C" int md_tune(md_ctx *c, const md_step_desc *w, int full)
 {
     if (!c || !w) return MD_EINVAL;
     if (!c->have_state) { c->err = "md_tune: md_set_state first"; return MD_ESTATE; }
+    c->force_hint = w->flags;
     if (!c->nlist_valid) MD_TRY(rebuild(c));
     // the kernels are pure functions of the live state, so they can be replayed without advancing the simulation
     if (c->nl_is_tile) {

@@ -100,6 +100,7 @@ struct md_ctx {
     bool use_tiles = false;     // configured (MD_ORDER_MORTON)
     bool nl_is_tile = false;    // the current list is a tile list
     bool nl32_decoded = false;  // nl_off/nl_idx hold the decoded copy of the current tile list (exports)
+    bool nl_rot2 = false;       // rows of the current tile list rotate by 2 (p & 3): laid out for W = 2 force kernels
     bool nl_cluster = false;    // the current tile list has one row per cluster of 4 particles (k_tile_build_c)
     int cluster_opt = 0;        // MD_OPT_CLUSTER
     int stride_mode = -1;       // list format nl_stride was sized for (0 particle rows, 1 cluster rows)
@@ -131,7 +132,8 @@ struct md_ctx {
     // status
     bool have_state = false, cells_valid = false, nlist_valid = false, force_valid = false;
     bool energy_valid = false;  // the energy lane of `force` belongs to the current forces (md_step skips energies)
-    md_step_desc last_desc;     // what the current forces were evaluated with (re-evaluation with energies on demand)
+    uint32_t force_hint = 0;    // MD_F_* of the latest md_step / md_tune description: which pair kernel reads the list
+    md_step_desc last_desc{};   // what the current forces were evaluated with (re-evaluation with energies on demand)
     uint64_t last_force_step = 0;
     bool last_from_step = false;
     uint64_t step = 0;

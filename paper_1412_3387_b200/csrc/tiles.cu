@@ -48,6 +48,7 @@ struct TileParams {
     const uint32_t *rank_of_lin;      // linear id -> cell rank
     const uint32_t *cell_start;       // [n_cells+1] first particle slot of each cell rank
     double cw[3];                     // cell widths
+    uint32_t rot_mul, rot_mask;       // bank-class rotation of the row of home particle p: rot_mul * (p & rot_mask)
     const uint32_t *desc;             // per-tile header precomputed at the rebuild (k_tile_header), or nullptr
     uint32_t desc_words;              // words per tile in desc
 };
@@ -465,7 +466,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build(TileParams tp, Ge
                     if (bal[q]) {
                         // k-th entry of class c goes to block k, slot (c - k - rot) & 7 (Fig. 4 steps 4-7 per class)
                         const uint32_t k = cntc[q] + __popc(bal[q] & cmask_lt);
-                        const uint32_t o = 8u * k + ((cls - k - 4u * ((p0 + q) & 1u)) & 7u);
+                        const uint32_t o = 8u * k + ((cls - k - tp.rot_mul * ((p0 + q) & tp.rot_mask)) & 7u);
                         if (((bal[q] >> lane) & 1u) && o < rcap) rb[q * rcap + o] = ent;
                         cntc[q] += __popc(bal[q] & cmask);
                     }
@@ -483,7 +484,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build(TileParams tp, Ge
             nc = qr == 2 ? cntc[2] : nc;
             nc = qr == 3 ? cntc[3] : nc;
             if (!live) nc = 0;
-            const uint32_t rot = 4u * ((p0 + qr) & 1u);
+            const uint32_t rot = tp.rot_mul * ((p0 + qr) & tp.rot_mask);
             uint32_t n = nc, mx = nc;
 #pragma unroll
             for (int o = 1; o < 8; o <<= 1) {
@@ -671,7 +672,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build8(TileParams tp, G
         const float ax = -2.f * m.x, ay = -2.f * m.y, az = -2.f * m.z;
         const float th = hh < np ? thr_out - m.w : -3e38f;  // absent particles never hit
         const uint32_t self = self0 + hh;
-        const uint32_t rot = 4u * ((p0 + hh) & 1u);
+        const uint32_t rot = tp.rot_mul * ((p0 + hh) & tp.rot_mask);
         // slot of the k-th entry of class c: 8 k + ((c - k - rot) & 7); c = ph (k0) or ph + 4 (k1)
         uint32_t k0 = 0, k1 = 0;
         const uint32_t c0 = ph - rot, c1 = ph + 4u - rot;
@@ -692,7 +693,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build8(TileParams tp, G
             const uint32_t ka = __shfl_sync(0xffffffffu, k0, owner), kb = __shfl_sync(0xffffffffu, k1, owner);
             const bool live = qr < np;
             const uint32_t nc = live ? (cls < 4u ? ka : kb) : 0u;
-            const uint32_t rrot = 4u * ((p0 + qr) & 1u);
+            const uint32_t rrot = tp.rot_mul * ((p0 + qr) & tp.rot_mask);
             uint32_t n = nc, mx = nc;
 #pragma unroll
             for (int o = 1; o < 8; o <<= 1) {
@@ -2013,6 +2014,11 @@ static TileParams make_tp(md_ctx *c)
     tp.rank_of_lin = c->rank_of_lin;
     tp.cell_start = c->cell_start;
     for (int a = 0; a < 3; ++a) tp.cw[a] = c->box[a] / (double)c->dims[a];
+    // rows rotate so that the 8 lanes of a quarter-warp of the force kernel meet 8 different bank classes: with W >= 4
+    // lanes per particle a quarter holds 2 particles x 4 blocks (rotation 0 / 4), with W = 2 it holds 4 particles x 2
+    // blocks (rotation 0 / 2 / 4 / 6).  Layout only: any rotation is a correct list.
+    tp.rot_mul = c->nl_rot2 ? 2u : 4u;
+    tp.rot_mask = c->nl_rot2 ? 3u : 1u;
     tp.desc_words = (TILE_DESC_CTX + tile_desc_table_words(c->tile_B) + 3u) & ~3u;
     tp.desc = c->tile_desc_valid ? c->tile_desc : nullptr;
     return tp;
@@ -2109,6 +2115,10 @@ int launch_tile_build(md_ctx *c, bool cluster, bool *fits)
     *fits = smem <= TILE_SMEM_LIMIT && ms + N_DUMMY <= 65536 && c->tile_B <= 4;
     if (!*fits) return MD_OK;
     c->nl_shift = tile_shift(c);
+    {   // the force kernel that will read the list: the last step description says which, else LJ
+        const bool dpd = (c->force_hint & MD_F_DPD) != 0 && !(c->force_hint & MD_F_LJ);
+        c->nl_rot2 = !cluster && c->cfg[dpd ? MD_K_DPD : MD_K_LJ].w == 2;
+    }
     const double R = c->r_list * 1.001, E = tile_extent(c), rl2 = c->r_list * c->r_list;
     MD_CUDA_CHECK(c, cudaMemsetAsync(&c->d_flags->nl_total, 0, sizeof(unsigned long long), c->stream));
     MD_CUDA_CHECK(c, cudaMemsetAsync(&c->d_flags->nl_overflow, 0, sizeof(unsigned int), c->stream));
