@@ -296,7 +296,7 @@ def run_ours(args):
         if args.order != "morton":
             kernel = "k_forces_" + fk
         elif fk == "dpd":
-            kernel = "k_tile_dpd"
+            kernel = "k_tile_dpd2"
         elif precision == B.MD_MIXED:
             kernel = "k_tile_lj4" if args.cluster else "k_tile_lj3"
         else:

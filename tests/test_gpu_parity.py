@@ -168,12 +168,14 @@ def test_nlist_invariants_and_dense_cell():
 
 
 # ---------------------------------------------------------------------------------------------------- S4a LJ
-@pytest.mark.parametrize("w,block", [(1, 64), (4, 128), (8, 128), (32, 256)])
+@pytest.mark.parametrize("w,block", [(1, 64), (2, 128), (4, 128), (8, 128), (32, 256)])
 def test_lj_forces_fp64(w, block):
     wl = _thermalised_lj(6)                                         # N=864
     md = B.from_workload(wl)
     md.set_launch(B.MD_K_LJ, block, w)
     md.build_nlist(); md.forces_lj(1.0, 1.0, 1)
+    # the row layout follows w (rotation 0/2/4/6 for w = 2): the exported list is the same list
+    assert np.array_equal(sort_pairs(md.get_nlist()), oracle.neighbor_pairs(wl.pos, wl.box, wl.r_list))
     F, E = md.get_forces()
     Fr, Er = oracle.forces_lj(wl.pos, wl.box, wl.rc, 1.0, 1.0, 1)
     assert force_rel_err(F, Fr) < 1e-10
@@ -211,7 +213,7 @@ def test_lj_perfect_fcc_energy():
 
 
 # ---------------------------------------------------------------------------------------------------- S4b DPD
-@pytest.mark.parametrize("w", [1, 4, 32])
+@pytest.mark.parametrize("w", [1, 2, 4, 32])
 def test_dpd_forces(w):
     wl = inputs.dpd_fluid(3000, pos_seed=4, vel_seed=5)             # L=10: 7^3 cells of width 1.43
     p = wl.params
