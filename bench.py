@@ -97,7 +97,13 @@ class ClockSampler:
 
 def workload_for(args):
     from paper_1412_3387_b200 import inputs
-    return inputs.config(args.config, scale=args.scale)
+    w = inputs.config(args.config, scale=args.scale)
+    if getattr(args, "r_buff", None):
+        # the paper tunes r_buff per benchmark; the configured value (0.4) stays
+        # the default of every reported run, this override is for the tuning sweep only and is named in the workload
+        import dataclasses
+        w = dataclasses.replace(w, r_buff=float(args.r_buff), name=w.name + "-rbuff%g" % args.r_buff)
+    return w
 
 
 def algorithmic_bytes(kind, nbar, k):
@@ -353,6 +359,8 @@ def main():
     ap.add_argument("--launch", nargs="*", default=[], help="kernel=block,w (with --no-tune)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cluster", action="store_true", help="MD_OPT_CLUSTER = 1: one neighbour row per cluster of 4")
+    ap.add_argument("--r-buff", type=float, default=None, dest="r_buff",
+                    help="override the configured skin r_buff = 0.4 (tuning sweep; not a reported configuration)")
     ap.add_argument("--brick", type=int, default=0, help="MD_OPT_TILE_BRICK: 1, 2 or 4 cells per brick edge (0 = auto)")
     args = ap.parse_args()
     if args.impl == "reference":
