@@ -227,6 +227,17 @@ int md_set_launch(md_ctx *ctx, int kernel, int block, int w);
 
 int md_get_stats(md_ctx *ctx, md_stats *out); /* synchronises */
 
+/* Device-side thermodynamic reductions (the paper reduces kinetic energy every NVT step,
+   PAPER.md:208, :214): kinetic = sum 1/2 m v^2, potential = sum of the per-particle potential energies of the current
+   forces (md_get_forces' energy lane; forces left by md_step are re-evaluated with energies, R16 / md_get_forces),
+   momentum = sum m v, temperature = 2 kinetic / (3 N - 3) (R18).  Two kernels, fixed summation order (per-block
+   partial sums in slot order, then one block over the partials): the result is bit-reproducible for a given state.
+   out: HOST pointer.  Synchronises.  MD_ESTATE if no force is current (potential would be undefined). */
+typedef struct md_thermo_t {
+    double kinetic, potential, momentum[3], temperature;
+} md_thermo_t;
+int md_thermo(md_ctx *ctx, md_thermo_t *out);
+
 /* on = 1: bracket every stage launched by md_step / md_build_* / md_forces_* / md_integrate_nve with CUDA events on the
    context's stream and accumulate their durations into md_stats.stage_ms (MD_K_CELLS = binning + reorder, MD_K_NLIST =
    count + scan + fill, MD_K_LJ / MD_K_DPD / MD_K_BONDS force kernels, MD_K_INTEGRATE both halves).  Resets the

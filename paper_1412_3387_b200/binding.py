@@ -28,7 +28,7 @@ EXPORTS = ["md_create", "md_configure", "md_destroy", "md_last_error", "md_set_s
            "md_get_state", "md_get_forces", "md_build_cells", "md_get_cells", "md_build_nlist", "md_get_nlist",
            "md_get_nlist_rows", "md_forces_lj", "md_forces_dpd", "md_forces_bonds", "md_integrate_nve",
            "md_needs_rebuild", "md_step", "md_tune", "md_set_option", "md_set_launch", "md_get_stats", "md_set_profiling",
-           "md_debug_philox"]
+           "md_debug_philox", "md_thermo"]
 
 
 class md_step_desc(C.Structure):
@@ -36,6 +36,11 @@ class md_step_desc(C.Structure):
                 ("lj_epsilon", C.c_double), ("lj_sigma", C.c_double),
                 ("dpd_A", C.c_double), ("dpd_gamma", C.c_double), ("dpd_kT", C.c_double),
                 ("dpd_seed", C.c_uint64), ("bond_k", C.c_double), ("bond_r0", C.c_double)]
+
+
+class md_thermo_t(C.Structure):
+    _fields_ = [("kinetic", C.c_double), ("potential", C.c_double), ("momentum", C.c_double * 3),
+                ("temperature", C.c_double)]
 
 
 class md_stats(C.Structure):
@@ -90,6 +95,7 @@ def load():
         "md_get_stats": [vp, C.POINTER(md_stats)],
         "md_set_profiling": [vp, i32],
         "md_debug_philox": [vp, vp, vp, vp, u64],
+        "md_thermo": [vp, vp],
     }
     for name, args in sig.items():
         fn = getattr(L, name)
@@ -273,6 +279,12 @@ class MD:
         d["stage_launches"] = {KERNEL_NAMES[k]: st.stage_launches[k] for k in KERNEL_NAMES}
         d["launch"] = {KERNEL_NAMES[k]: dict(block=st.block[k], w=st.w[k], us=st.tuned_us[k]) for k in KERNEL_NAMES}
         return d
+
+    def thermo(self) -> dict:
+        t = md_thermo_t()
+        self._chk(self.L.md_thermo(self.h, C.byref(t)), "md_thermo")
+        return dict(kinetic=t.kinetic, potential=t.potential, momentum=np.array(list(t.momentum)),
+                    temperature=t.temperature)
 
     def debug_philox(self, ctr, key):
         ctr = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)

@@ -1036,6 +1036,21 @@ extern "C" int md_get_stats(md_ctx *c, md_stats *out)
     return MD_OK;
 }
 
+extern "C" int md_thermo(md_ctx *c, md_thermo_t *out)
+{
+    if (!c || !out) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_thermo: md_set_state first"; return MD_ESTATE; }
+    if (!c->force_valid) { c->err = "md_thermo: no force has been computed for the current positions"; return MD_ESTATE; }
+    if (!c->energy_valid && c->last_from_step) MD_TRY(eval_forces(c, &c->last_desc, c->last_force_step, true));
+    double r[5];
+    MD_TRY(launch_thermo(c, r));
+    out->kinetic = r[0];
+    out->potential = r[1];
+    out->momentum[0] = r[2]; out->momentum[1] = r[3]; out->momentum[2] = r[4];
+    out->temperature = c->N > 1 ? 2.0 * r[0] / (3.0 * (double)c->N - 3.0) : 0.0;
+    return MD_OK;
+}
+
 extern "C" int md_debug_philox(md_ctx *c, const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint64_t n)
 {
     if (!c || !ctr || !key || !out) return MD_EINVAL;

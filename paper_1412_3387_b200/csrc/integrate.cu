@@ -87,3 +87,74 @@ int launch_half2(md_ctx *c, double dt)
     MD_LAUNCH_CHECK(c);
     return MD_OK;
 }
+
+// ------------------------------------------------------------------------------------------------------------
+// md_thermo: kinetic energy, potential energy and momentum.  Fixed summation order: block b
+// sums a contiguous range of slots (thread-strided, then a shared-memory tree), one block then sums the partials.
+// ------------------------------------------------------------------------------------------------------------
+constexpr int THERMO_BLOCK = 256;
+constexpr uint32_t THERMO_PER_BLOCK = 4096;  // slots per block of the first pass
+
+__device__ __forceinline__ void thermo_block_sum(double v[5], double *sm /* [5][THERMO_BLOCK] */)
+{
+#pragma unroll
+    for (int k = 0; k < 5; ++k) sm[k * THERMO_BLOCK + threadIdx.x] = v[k];
+    __syncthreads();
+    for (int o = THERMO_BLOCK / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+#pragma unroll
+            for (int k = 0; k < 5; ++k) sm[k * THERMO_BLOCK + threadIdx.x] += sm[k * THERMO_BLOCK + threadIdx.x + o];
+        }
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(THERMO_BLOCK) k_thermo_partial(const double4 *__restrict__ vel,
+                                                                 const double4 *__restrict__ force, uint32_t N,
+                                                                 double *__restrict__ partial /* [gridDim.x][5] */)
+{
+    __shared__ double sm[5 * THERMO_BLOCK];
+    const uint32_t b0 = blockIdx.x * THERMO_PER_BLOCK, b1 = min(N, b0 + THERMO_PER_BLOCK);
+    double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    for (uint32_t i = b0 + threadIdx.x; i < b1; i += THERMO_BLOCK) {
+        const double4 u = vel[i];
+        v[0] += 0.5 * u.w * (u.x * u.x + u.y * u.y + u.z * u.z);
+        v[1] += force[i].w;
+        v[2] += u.w * u.x; v[3] += u.w * u.y; v[4] += u.w * u.z;
+    }
+    thermo_block_sum(v, sm);
+    if (threadIdx.x < 5) partial[5ull * blockIdx.x + threadIdx.x] = sm[threadIdx.x * THERMO_BLOCK];
+}
+
+__global__ void __launch_bounds__(THERMO_BLOCK) k_thermo_final(const double *__restrict__ partial, uint32_t n_partial,
+                                                               double *__restrict__ out /* [5] */)
+{
+    __shared__ double sm[5 * THERMO_BLOCK];
+    double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    for (uint32_t b = threadIdx.x; b < n_partial; b += THERMO_BLOCK) {
+#pragma unroll
+        for (int k = 0; k < 5; ++k) v[k] += partial[5ull * b + k];
+    }
+    thermo_block_sum(v, sm);
+    if (threadIdx.x < 5) out[threadIdx.x] = sm[threadIdx.x * THERMO_BLOCK];
+}
+
+int launch_thermo(md_ctx *c, double *out5_host)
+{
+    const uint32_t N = (uint32_t)c->N;
+    const uint32_t nb = (N + THERMO_PER_BLOCK - 1) / THERMO_PER_BLOCK;
+    const uint64_t need = 5ull * nb + 8;
+    if (need > c->thermo_len) {
+        if (c->thermo_buf) { md_free(c, c->thermo_buf); c->thermo_buf = nullptr; }
+        c->thermo_len = 0;
+        MD_TRY(md_alloc(c, (void **)&c->thermo_buf, need * sizeof(double)));
+        c->thermo_len = need;
+    }
+    double *res = c->thermo_buf + 5ull * nb;
+    k_thermo_partial<<<nb, THERMO_BLOCK, 0, c->stream>>>(c->vel, c->force, N, c->thermo_buf);
+    MD_LAUNCH_CHECK(c);
+    k_thermo_final<<<1, THERMO_BLOCK, 0, c->stream>>>(c->thermo_buf, nb, res);
+    MD_LAUNCH_CHECK(c);
+    MD_CUDA_CHECK(c, cudaMemcpyAsync(out5_host, res, 5 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    return md_sync(c);
+}

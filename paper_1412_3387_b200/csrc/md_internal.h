@@ -126,6 +126,8 @@ struct md_ctx {
     uint64_t scan_tmp_len = 0;
     void *stage = nullptr;  // host<->device staging
     uint64_t stage_bytes = 0;
+    double *thermo_buf = nullptr;  // per-block partial sums of md_thermo + the 5 results
+    uint64_t thermo_len = 0;
     DevFlags *d_flags = nullptr;
     DevFlags *h_flags = nullptr;  // pinned
 
@@ -189,6 +191,7 @@ int launch_forces_dpd(md_ctx *c, double A, double gamma, double kT, double dt, u
 int launch_forces_bonds(md_ctx *c, double k, double r0);
 int launch_half1(md_ctx *c, double dt, bool fused);  // fused: preceded by the previous step's half 2
 int launch_half2(md_ctx *c, double dt);
+int launch_thermo(md_ctx *c, double *out6_host);  // kinetic, potential, px, py, pz (device reduction, then D2H + sync)
 int launch_export_pairs_count(md_ctx *c, uint32_t *cnt);
 int launch_export_pairs_fill(md_ctx *c, const uint64_t *off, uint32_t *pairs);
 int launch_export_rows(md_ctx *c, const uint32_t *probe_tags, uint32_t n_probe, uint32_t *counts, uint32_t *nbr,

@@ -384,6 +384,37 @@ def test_nve_energy_drift_gpu_config1():
     assert st["dangerous_builds"] == 0 and 1000 / 25 <= st["rebuilds"] <= 1000 / 4
 
 
+def test_thermo_reductions():
+    """md_thermo (device reductions): kinetic and potential energy, momentum, temperature against
+    plain sums over the read-back state and the oracle's per-particle energies; bit-reproducible."""
+    wl = _thermalised_lj(6, kT=1.3)
+    md = B.from_workload(wl)
+    md.step(B.step_desc("lj", wl.dt, wl.params), 12)                # forces left by md_step: energies on demand
+    t1 = md.thermo(); t2 = md.thermo()
+    assert t1["kinetic"] == t2["kinetic"] and t1["potential"] == t2["potential"]
+    pos, vel, _ = md.get_state()
+    ke = 0.5 * np.sum(vel * vel)
+    _, Er = oracle.forces_lj(pos, wl.box, wl.rc)
+    assert abs(t1["kinetic"] - ke) < 1e-12 * ke
+    assert abs(t1["potential"] - Er.sum()) < 1e-10 * abs(Er.sum())
+    assert np.abs(t1["momentum"] - vel.sum(axis=0)).max() < 1e-11 * np.abs(vel).sum()
+    assert abs(t1["temperature"] - 2.0 * ke / (3 * wl.N - 3)) < 1e-12
+    # NVE: the total energy of the thermalised state stays put over the 12 steps (R23 bound, per particle)
+    e0 = 0.5 * np.sum(wl.vel * wl.vel) + oracle.forces_lj(wl.pos, wl.box, wl.rc)[1].sum()
+    assert abs(t1["kinetic"] + t1["potential"] - e0) / wl.N < 2e-3
+    # polymer: DPD conservative energy + bond energy lanes are summed as well
+    wp = inputs.polymer_melt(20, chain_len=32)
+    mp = B.from_workload(wp)
+    q = wp.params
+    mp.build_nlist()
+    mp.forces_dpd(q["A"], q["gamma"], q["kT"], wp.dt, 3, q["seed"])
+    mp.forces_bonds(q["bond_k"], q["bond_r0"])
+    _, E = mp.get_forces()
+    tp = mp.thermo()
+    assert abs(tp["potential"] - E.sum()) < 1e-12 * abs(E.sum())
+    assert abs(tp["kinetic"] - 0.5 * np.sum(wp.vel * wp.vel)) < 1e-12 * tp["kinetic"]
+
+
 def test_tuner_runs_and_keeps_results():
     wl = _thermalised_lj(8)                                             # N=2048
     desc = B.step_desc("lj", wl.dt, wl.params)
