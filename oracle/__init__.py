@@ -204,6 +204,45 @@ def probe_forces_dpd(pos, vel, box, rc, A, gamma, kT, dt, step, seed, probes):
 
 
 # ------------------------------------------------------------------------------------------------------
+# NVT: Nose-Hoover thermostat (SURVEY.md 8(f) row 1; "NVT ... Nose-Hoover" PAPER.md:63, :208, :214; the paper prints
+# no equations -> DESIGN.md R30).  Equations of motion: dx/dt = v, dv/dt = F/m - xi v, dxi/dt = (T_inst/T0 - 1)/tau^2,
+# deta/dt = xi, T_inst = 2 K / g with g = 3N - 3 (R18).  Velocity-Verlet discretisation, step by step, plain numpy:
+#   half 1:      v <- (v + (dt/2) F/m) / (1 + (dt/2) xi) ;  x <- x + dt v ;  wrap
+#   thermostat:  K' = sum 1/2 m v^2 ;  xi_old = xi ;  xi <- xi + (dt/tau^2) (2K'/(g kT0) - 1) ;  eta <- eta + (dt/2)(xi + xi_old)
+#   forces at the new x
+#   half 2:      v <- v + (dt/2) (F/m - xi v)
+# Conserved: K + U + g kT0 (tau^2 xi^2 / 2 + eta).
+# ------------------------------------------------------------------------------------------------------
+def nvt_half1(pos, vel, image, force, box, dt, xi, mass=None):
+    """In place on pos, vel, image (C-contiguous float64 / int32)."""
+    m = 1.0 if mass is None else np.asarray(mass, dtype=np.float64)[:, None]
+    vel[:] = (vel + (0.5 * dt * force) / m) / (1.0 + 0.5 * dt * xi)
+    pos += dt * vel
+    b = np.asarray(box, dtype=np.float64)
+    hi = pos >= 0.5 * b
+    lo = pos < -0.5 * b
+    pos[hi] -= np.broadcast_to(b, pos.shape)[hi]
+    pos[lo] += np.broadcast_to(b, pos.shape)[lo]
+    image[hi] += 1
+    image[lo] -= 1
+
+
+def nvt_thermostat(vel, dt, kT, tau, xi, eta, mass=None):
+    """Returns (xi_new, eta_new, K) from the velocities left by half 1."""
+    m = 1.0 if mass is None else np.asarray(mass, dtype=np.float64)[:, None]
+    K = 0.5 * float(np.sum(m * vel * vel))
+    g = 3 * vel.shape[0] - 3
+    xi_new = xi + (dt / (tau * tau)) * (2.0 * K / (g * kT) - 1.0)
+    eta_new = eta + 0.5 * dt * (xi_new + xi)
+    return xi_new, eta_new, K
+
+
+def nvt_half2(vel, force, dt, xi, mass=None):
+    m = 1.0 if mass is None else np.asarray(mass, dtype=np.float64)[:, None]
+    vel += 0.5 * dt * (force / m - xi * vel)
+
+
+# ------------------------------------------------------------------------------------------------------
 # The step loop, in the order of DESIGN.md "The path" (S6a -> S3 -> [S1,S2] -> S4 (+S5) -> S6b).
 # ------------------------------------------------------------------------------------------------------
 class Sim:
@@ -217,7 +256,9 @@ class Sim:
     only to log WHEN the CUDA path must rebuild.
     """
 
-    def __init__(self, pos, vel, box, rc, r_buff, what, bonds=None, mass=None, step0=0):
+    def __init__(self, pos, vel, box, rc, r_buff, what, bonds=None, mass=None, step0=0, nvt=None):
+        self.nvt = nvt                       # None = NVE; dict(kT, tau) = Nose-Hoover (R30)
+        self.xi, self.eta = 0.0, 0.0
         self.box = np.ascontiguousarray(np.broadcast_to(np.asarray(box, dtype=np.float64), (3,)))
         self.pos = wrap(pos, self.box)
         self.vel = np.array(vel, dtype=np.float64, order="C")
@@ -255,14 +296,29 @@ class Sim:
         if self.force is None:
             self.compute_forces(dt, self.step)          # DESIGN.md R16: F(t0) before the first half-kick
         for _ in range(n_steps):
-            vv_half1(self.pos, self.vel, self.image, self.force, self.box, dt, self.mass)
+            if self.nvt is None:
+                vv_half1(self.pos, self.vel, self.image, self.force, self.box, dt, self.mass)
+            else:
+                nvt_half1(self.pos, self.vel, self.image, self.force, self.box, dt, self.xi, self.mass)
+                self.xi_half1 = self.xi
+                self.xi, self.eta, _ = nvt_thermostat(self.vel, dt, self.nvt["kT"], self.nvt["tau"], self.xi, self.eta,
+                                                      self.mass)
             if needs_rebuild(self.pos, self.pos_ref, self.box, self.r_buff):
                 self.pos_ref = self.pos.copy()
                 self.rebuild_steps.append(self.step + 1)
             self.compute_forces(dt, self.step + 1)      # DESIGN.md R15: hash counter = step being completed
-            vv_half2(self.vel, self.force, dt, self.mass)
+            if self.nvt is None:
+                vv_half2(self.vel, self.force, dt, self.mass)
+            else:
+                nvt_half2(self.vel, self.force, dt, self.xi, self.mass)
             self.step += 1
         return self
+
+    def nvt_conserved(self):
+        """K + U + g kT0 (tau^2 xi^2 / 2 + eta) (R30)."""
+        g = 3 * self.N - 3
+        return (self.kinetic_energy() + self.potential_energy()
+                + g * self.nvt["kT"] * (0.5 * self.nvt["tau"] ** 2 * self.xi ** 2 + self.eta))
 
     def kinetic_energy(self):
         m = 1.0 if self.mass is None else np.asarray(self.mass)[:, None]
