@@ -229,7 +229,13 @@ def run_ours(args):
     order = {"lex": B.MD_ORDER_LEX, "morton": B.MD_ORDER_MORTON, "hilbert": B.MD_ORDER_HILBERT}[args.order]
     md = B.MD(w.box, w.N, w.rc, w.r_buff, precision=precision, stream=stream.cuda_stream, order=order,
               sched=B.MD_SCHED_SYNC if args.sync_sched else B.MD_SCHED_SPECULATIVE)
-    desc = B.step_desc(w.kind, w.dt, w.params)
+    nvt = None
+    if args.nvt:
+        import dataclasses
+        kT = float(w.params.get("kT", 1.2 if args.config == 2 else 1.0))
+        nvt = dict(kT=kT, tau=0.5)
+        w = dataclasses.replace(w, name=w.name + "-nvt")
+    desc = B.step_desc(w.kind, w.dt, w.params, nvt=nvt)
 
     # inputs resident in HBM before the timed region
     d_pos = torch.from_numpy(w.pos).to("cuda")
@@ -361,6 +367,9 @@ def main():
     ap.add_argument("--cluster", action="store_true", help="MD_OPT_CLUSTER = 1: one neighbour row per cluster of 4")
     ap.add_argument("--r-buff", type=float, default=None, dest="r_buff",
                     help="override the configured skin r_buff = 0.4 (tuning sweep; not a reported configuration)")
+    ap.add_argument("--nvt", action="store_true",
+                    help="Nose-Hoover NVT (MD_F_NVT, kT = the workload's temperature, tau = 0.5) instead of NVE: "
+                         "SURVEY 8(f) row 1; named in the workload, not a BASELINE configuration")
     ap.add_argument("--brick", type=int, default=0, help="MD_OPT_TILE_BRICK: 1, 2 or 4 cells per brick edge (0 = auto)")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -61,6 +61,7 @@ typedef enum {
 #define MD_F_LJ 1u
 #define MD_F_DPD 2u
 #define MD_F_BONDS 4u
+#define MD_F_NVT 8u /* md_step integrates with the Nose-Hoover thermostat (md_integrate_nvt) instead of NVE */
 
 /* scheduling of md_step */
 #define MD_SCHED_SYNC 0        /* the host waits for the rebuild flag of half 1 before it enqueues the forces */
@@ -76,6 +77,7 @@ typedef struct {
     double dpd_A, dpd_gamma, dpd_kT;
     uint64_t dpd_seed;
     double bond_k, bond_r0;
+    double nvt_kT, nvt_tau; /* MD_F_NVT: target temperature (k_B T0) and thermostat period tau */
 } md_step_desc;
 
 #define MD_N_KERNELS 8
@@ -224,6 +226,17 @@ int md_set_option(md_ctx *ctx, int option, int64_t value);
 
 /* Fix launch parameters by hand (block multiple of 32 in [32,1024]; w power of two <= 32); kernel = MD_K_*. */
 int md_set_launch(md_ctx *ctx, int kernel, int block, int w);
+
+/* NVT, Nose-Hoover thermostat (named by the paper, which prints no
+   equations: DESIGN.md R30).  dv/dt = F/m - xi v, dxi/dt = (T_inst/T0 - 1)/tau^2, deta/dt = xi, T_inst = 2K/(3N-3).
+   half = 1: v <- (v + (dt/2) F/m) / (1 + (dt/2) xi); x <- x + dt v; wrap; displacement check (as md_integrate_nve);
+             then K' = sum 1/2 m v^2 is reduced on the device (fixed order) and xi <- xi + (dt/tau^2)(2K'/((3N-3) kT) - 1),
+             eta <- eta + (dt/2)(xi + xi_old): no host round trip.
+   half = 2: v <- v + (dt/2)(F/m - xi v).
+   The thermostat variables live in the context: md_set_state resets them to 0. */
+int md_integrate_nvt(md_ctx *ctx, double dt, int half, double kT, double tau);
+int md_set_thermostat(md_ctx *ctx, double xi, double eta);
+int md_get_thermostat(md_ctx *ctx, double *xi, double *eta); /* HOST pointers; synchronises */
 
 int md_get_stats(md_ctx *ctx, md_stats *out); /* synchronises */
 

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "csrc", "libb200md.so")
 
 MD_FP64, MD_MIXED = 0, 1
 MD_ORDER_LEX, MD_ORDER_MORTON, MD_ORDER_HILBERT = 0, 1, 2
-MD_F_LJ, MD_F_DPD, MD_F_BONDS = 1, 2, 4
+MD_F_LJ, MD_F_DPD, MD_F_BONDS, MD_F_NVT = 1, 2, 4, 8
 MD_SCHED_SYNC, MD_SCHED_SPECULATIVE = 0, 1
 MD_OPT_TILE_BRICK, MD_OPT_ACC_BLOCK, MD_OPT_CLUSTER = 1, 2, 3
 MD_N_KERNELS = 8
@@ -28,14 +28,15 @@ EXPORTS = ["md_create", "md_configure", "md_destroy", "md_last_error", "md_set_s
            "md_get_state", "md_get_forces", "md_build_cells", "md_get_cells", "md_build_nlist", "md_get_nlist",
            "md_get_nlist_rows", "md_forces_lj", "md_forces_dpd", "md_forces_bonds", "md_integrate_nve",
            "md_needs_rebuild", "md_step", "md_tune", "md_set_option", "md_set_launch", "md_get_stats", "md_set_profiling",
-           "md_debug_philox", "md_thermo"]
+           "md_debug_philox", "md_thermo", "md_integrate_nvt", "md_set_thermostat", "md_get_thermostat"]
 
 
 class md_step_desc(C.Structure):
     _fields_ = [("flags", C.c_uint32), ("lj_energy_shift", C.c_int32), ("dt", C.c_double),
                 ("lj_epsilon", C.c_double), ("lj_sigma", C.c_double),
                 ("dpd_A", C.c_double), ("dpd_gamma", C.c_double), ("dpd_kT", C.c_double),
-                ("dpd_seed", C.c_uint64), ("bond_k", C.c_double), ("bond_r0", C.c_double)]
+                ("dpd_seed", C.c_uint64), ("bond_k", C.c_double), ("bond_r0", C.c_double),
+                ("nvt_kT", C.c_double), ("nvt_tau", C.c_double)]
 
 
 class md_thermo_t(C.Structure):
@@ -96,6 +97,9 @@ def load():
         "md_set_profiling": [vp, i32],
         "md_debug_philox": [vp, vp, vp, vp, u64],
         "md_thermo": [vp, vp],
+        "md_integrate_nvt": [vp, C.c_double, i32, C.c_double, C.c_double],
+        "md_set_thermostat": [vp, C.c_double, C.c_double],
+        "md_get_thermostat": [vp, vp, vp],
     }
     for name, args in sig.items():
         fn = getattr(L, name)
@@ -120,7 +124,8 @@ def _ptr(a):
     raise TypeError(type(a))
 
 
-def step_desc(kind: str, dt: float, params: dict) -> md_step_desc:
+def step_desc(kind: str, dt: float, params: dict, nvt: dict = None) -> md_step_desc:
+    """nvt = dict(kT, tau): Nose-Hoover thermostat (MD_F_NVT) instead of NVE."""
     d = md_step_desc()
     d.dt = dt
     d.lj_epsilon, d.lj_sigma, d.lj_energy_shift = 1.0, 1.0, 1
@@ -141,6 +146,9 @@ def step_desc(kind: str, dt: float, params: dict) -> md_step_desc:
         d.flags = 0
     else:
         raise ValueError(kind)
+    if nvt is not None:
+        d.flags |= MD_F_NVT
+        d.nvt_kT, d.nvt_tau = float(nvt["kT"]), float(nvt["tau"])
     return d
 
 
@@ -246,6 +254,17 @@ class MD:
 
     def integrate_nve(self, dt, half):
         self._chk(self.L.md_integrate_nve(self.h, float(dt), int(half)), "md_integrate_nve")
+
+    def integrate_nvt(self, dt, half, kT, tau):
+        self._chk(self.L.md_integrate_nvt(self.h, float(dt), int(half), float(kT), float(tau)), "md_integrate_nvt")
+
+    def set_thermostat(self, xi, eta):
+        self._chk(self.L.md_set_thermostat(self.h, float(xi), float(eta)), "md_set_thermostat")
+
+    def get_thermostat(self):
+        xi, eta = C.c_double(), C.c_double()
+        self._chk(self.L.md_get_thermostat(self.h, C.byref(xi), C.byref(eta)), "md_get_thermostat")
+        return xi.value, eta.value
 
     def needs_rebuild(self) -> bool:
         f = C.c_int()

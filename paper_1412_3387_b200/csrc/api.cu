@@ -362,6 +362,7 @@ extern "C" int md_create(md_ctx **out, const double box[3], uint64_t N, double r
     A((void **)&c->image_alt, 3 * N * sizeof(int));
     A((void **)&c->pos_ref, 3 * N * sizeof(double));
     A((void **)&c->rel, N * sizeof(float4));
+    A((void **)&c->nvt_state, 4 * sizeof(double));
     A((void **)&c->tag, N * sizeof(uint32_t));
     A((void **)&c->tag_alt, N * sizeof(uint32_t));
     A((void **)&c->rtag, N * sizeof(uint32_t));
@@ -435,6 +436,7 @@ extern "C" int md_set_state(md_ctx *c, const double *pos, const double *vel, con
     MD_TRY(stage_in(c, st, vel, b3, &dv));
     MD_TRY(stage_in(c, st, mass, b1, &dm));
     MD_TRY(launch_pack_state(c, (const double *)dp, (const double *)dv, (const double *)dm));
+    MD_CUDA_CHECK(c, cudaMemsetAsync(c->nvt_state, 0, 4 * sizeof(double), c->stream));  // thermostat at rest (R30)
     MD_CUDA_CHECK(c, cudaMemsetAsync(c->force, 0, c->N * sizeof(double4), c->stream));
     MD_CUDA_CHECK(c, cudaMemsetAsync(c->d_flags, 0, sizeof(DevFlags), c->stream));
     c->have_state = true;
@@ -781,6 +783,46 @@ extern "C" int md_integrate_nve(md_ctx *c, double dt, int half)
     return MD_EINVAL;
 }
 
+extern "C" int md_integrate_nvt(md_ctx *c, double dt, int half, double kT, double tau)
+{
+    if (!c) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_integrate_nvt: md_set_state first"; return MD_ESTATE; }
+    if (!(kT > 0.0) || !(tau > 0.0)) { c->err = "md_integrate_nvt: kT and tau must be positive"; return MD_EINVAL; }
+    if (half == 1) {
+        if (!c->cells_valid) MD_TRY(do_build_cells(c));
+        ProfScope ps(c, MD_K_INTEGRATE);
+        MD_TRY(launch_half1(c, dt, false, true));
+        MD_TRY(launch_nvt_thermostat(c, dt, kT, tau));
+        c->steps_since_build++;
+        c->force_valid = false;
+        return MD_OK;
+    }
+    if (half == 2) { ProfScope ps(c, MD_K_INTEGRATE); return launch_half2(c, dt, true); }
+    c->err = "md_integrate_nvt: half must be 1 or 2";
+    return MD_EINVAL;
+}
+
+extern "C" int md_set_thermostat(md_ctx *c, double xi, double eta)
+{
+    if (!c) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_set_thermostat: md_set_state first"; return MD_ESTATE; }
+    const double v[2] = {xi, eta};
+    MD_CUDA_CHECK(c, cudaMemcpyAsync(c->nvt_state, v, sizeof(v), cudaMemcpyHostToDevice, c->stream));
+    return md_sync(c);
+}
+
+extern "C" int md_get_thermostat(md_ctx *c, double *xi, double *eta)
+{
+    if (!c || !xi || !eta) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_get_thermostat: md_set_state first"; return MD_ESTATE; }
+    double v[2];
+    MD_CUDA_CHECK(c, cudaMemcpyAsync(v, c->nvt_state, sizeof(v), cudaMemcpyDeviceToHost, c->stream));
+    MD_TRY(md_sync(c));
+    *xi = v[0];
+    *eta = v[1];
+    return MD_OK;
+}
+
 extern "C" int md_needs_rebuild(md_ctx *c, int *flag)
 {
     if (!c || !flag) return MD_EINVAL;
@@ -840,6 +882,8 @@ extern "C" int md_step(md_ctx *c, const md_step_desc *w, uint64_t n_steps)
     if (!c->have_state) { c->err = "md_step: md_set_state first"; return MD_ESTATE; }
     if (!(w->dt > 0.0)) { c->err = "md_step: dt must be positive"; return MD_EINVAL; }
     if (n_steps == 0) return MD_OK;
+    const bool nvt = (w->flags & MD_F_NVT) != 0;
+    if (nvt && (!(w->nvt_kT > 0.0) || !(w->nvt_tau > 0.0))) { c->err = "md_step: nvt_kT and nvt_tau must be positive"; return MD_EINVAL; }
     c->force_hint = w->flags;
     if (!c->nlist_valid) MD_TRY(rebuild(c));
     if (!c->force_valid) MD_TRY(eval_forces(c, w, c->step, false));  // R16: F(t0) before the first half-kick
@@ -848,7 +892,8 @@ extern "C" int md_step(md_ctx *c, const md_step_desc *w, uint64_t n_steps)
     for (uint64_t s = 0; s < n_steps; ++s) {
         if (s == 0) {
             ProfScope ps(c, MD_K_INTEGRATE);
-            MD_TRY(launch_half1(c, w->dt, false));
+            MD_TRY(launch_half1(c, w->dt, false, nvt));
+            if (nvt) MD_TRY(launch_nvt_thermostat(c, w->dt, w->nvt_kT, w->nvt_tau));
         }
         c->steps_since_build++;
         MD_CUDA_CHECK(c, cudaMemcpyAsync(c->h_flags, c->d_flags, sizeof(DevFlags), cudaMemcpyDeviceToHost, c->stream));
@@ -880,8 +925,12 @@ extern "C" int md_step(md_ctx *c, const md_step_desc *w, uint64_t n_steps)
         (void)thr2;
         {
             ProfScope ps(c, MD_K_INTEGRATE);
-            if (s + 1 < n_steps) MD_TRY(launch_half1(c, w->dt, true));  // half 2 of this step + half 1 of the next
-            else MD_TRY(launch_half2(c, w->dt));
+            if (s + 1 < n_steps) {
+                MD_TRY(launch_half1(c, w->dt, true, nvt));  // half 2 of this step + half 1 of the next
+                if (nvt) MD_TRY(launch_nvt_thermostat(c, w->dt, w->nvt_kT, w->nvt_tau));
+            } else {
+                MD_TRY(launch_half2(c, w->dt, nvt));
+            }
         }
         c->step++;
         c->stats.steps++;

@@ -6,14 +6,19 @@
 // as k_half2 followed by k_half1, so the result is bit-identical to the two separate launches).
 // The largest squared displacement of the step goes to flags->max_d2[slot] (float bits; the host uses it to
 // predict the step at which the criterion will fire, see md_step); the other slot is cleared for the next step.
-template <bool FUSED>
+// NVT (R30): v <- (v + kick) / (1 + (dt/2) xi) in half 1, v <- v + (dt/2)(F/m - xi v) in half 2, xi read from
+// nvt[0]; the fused launch applies half 2 and the next half 1 with the same xi (the one the thermostat update left).
+template <bool FUSED, bool NVT>
 __global__ void k_half1(double4 *__restrict__ pos, double4 *__restrict__ vel, const double4 *__restrict__ force,
                         int *__restrict__ image, const double *__restrict__ pos_ref,
                         const uint32_t *__restrict__ cell_lin, float4 *__restrict__ rel, Geom g, double dt,
-                        double half_dt, double thr2, double danger2, DevFlags *flags, int slot)
+                        double half_dt, double thr2, double danger2, DevFlags *flags, int slot,
+                        const double *__restrict__ nvt)
 {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     float d2f = 0.f;
+    const double xi = NVT ? nvt[0] : 0.0;
+    const double denom = __dadd_rn(1.0, __dmul_rn(half_dt, xi));
     if (i < g.N) {
         double4 p = pos[i];
         double4 v = vel[i];
@@ -28,8 +33,13 @@ __global__ void k_half1(double4 *__restrict__ pos, double4 *__restrict__ vel, co
             // same operation order as the definition: v + ((dt/2) F)/m ; x + dt v   (no FMA: positions parity 1e-12
             // does not need it, but it keeps single steps bit-comparable with a plain CPU evaluation)
             const double kick = __ddiv_rn(__dmul_rn(half_dt, ff[a]), m);
-            if (FUSED) u[a] = __dadd_rn(u[a], kick);
-            u[a] = __dadd_rn(u[a], kick);
+            if (NVT) {
+                if (FUSED) u[a] = __dadd_rn(u[a], __dmul_rn(half_dt, __dsub_rn(__ddiv_rn(ff[a], m), __dmul_rn(xi, u[a]))));
+                u[a] = __ddiv_rn(__dadd_rn(u[a], kick), denom);
+            } else {
+                if (FUSED) u[a] = __dadd_rn(u[a], kick);
+                u[a] = __dadd_rn(u[a], kick);
+            }
             double xn = __dadd_rn(x[a], __dmul_rn(dt, u[a]));
             if (xn >= g.h[a]) { xn = __dsub_rn(xn, g.L[a]); image[3ull * i + a] += 1; }
             else if (xn < -g.h[a]) { xn = __dadd_rn(xn, g.L[a]); image[3ull * i + a] -= 1; }
@@ -51,6 +61,20 @@ __global__ void k_half1(double4 *__restrict__ pos, double4 *__restrict__ vel, co
     if (i == 0) flags->max_d2[slot ^ 1] = 0u;
 }
 
+__global__ void k_half2_nvt(double4 *__restrict__ vel, const double4 *__restrict__ force, uint32_t N, double half_dt,
+                            const double *__restrict__ nvt)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double xi = nvt[0];
+    double4 v = vel[i];
+    const double4 f = force[i];
+    v.x = __dadd_rn(v.x, __dmul_rn(half_dt, __dsub_rn(__ddiv_rn(f.x, v.w), __dmul_rn(xi, v.x))));
+    v.y = __dadd_rn(v.y, __dmul_rn(half_dt, __dsub_rn(__ddiv_rn(f.y, v.w), __dmul_rn(xi, v.y))));
+    v.z = __dadd_rn(v.z, __dmul_rn(half_dt, __dsub_rn(__ddiv_rn(f.z, v.w), __dmul_rn(xi, v.z))));
+    vel[i] = v;
+}
+
 __global__ void k_half2(double4 *__restrict__ vel, const double4 *__restrict__ force, uint32_t N, double half_dt)
 {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -63,27 +87,33 @@ __global__ void k_half2(double4 *__restrict__ vel, const double4 *__restrict__ f
     vel[i] = v;
 }
 
-int launch_half1(md_ctx *c, double dt, bool fused)
+int launch_half1(md_ctx *c, double dt, bool fused, bool nvt)
 {
     const LaunchCfg &cf = c->cfg[MD_K_INTEGRATE];
     const double t = 0.5 * c->r_buff;
     c->d2_slot ^= 1;
-    if (fused)
-        k_half1<true><<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->pos, c->vel, c->force, c->image, c->pos_ref,
-                                                                         c->cell_lin, c->rel, c->g, dt, 0.5 * dt, t * t, c->r_buff * c->r_buff,
-                                                                         c->d_flags, c->d2_slot);
-    else
-        k_half1<false><<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->pos, c->vel, c->force, c->image, c->pos_ref,
-                                                                          c->cell_lin, c->rel, c->g, dt, 0.5 * dt, t * t, c->r_buff * c->r_buff,
-                                                                          c->d_flags, c->d2_slot);
+    const unsigned grid = md_grid(c->N, cf.block);
+#define HALF1_ARGS c->pos, c->vel, c->force, c->image, c->pos_ref, c->cell_lin, c->rel, c->g, dt, 0.5 * dt, t * t, \
+                   c->r_buff * c->r_buff, c->d_flags, c->d2_slot, c->nvt_state
+    if (nvt) {
+        if (fused) k_half1<true, true><<<grid, cf.block, 0, c->stream>>>(HALF1_ARGS);
+        else k_half1<false, true><<<grid, cf.block, 0, c->stream>>>(HALF1_ARGS);
+    } else {
+        if (fused) k_half1<true, false><<<grid, cf.block, 0, c->stream>>>(HALF1_ARGS);
+        else k_half1<false, false><<<grid, cf.block, 0, c->stream>>>(HALF1_ARGS);
+    }
+#undef HALF1_ARGS
     MD_LAUNCH_CHECK(c);
     return MD_OK;
 }
 
-int launch_half2(md_ctx *c, double dt)
+int launch_half2(md_ctx *c, double dt, bool nvt)
 {
     const LaunchCfg &cf = c->cfg[MD_K_INTEGRATE];
-    k_half2<<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->vel, c->force, (uint32_t)c->N, 0.5 * dt);
+    if (nvt)
+        k_half2_nvt<<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->vel, c->force, (uint32_t)c->N, 0.5 * dt, c->nvt_state);
+    else
+        k_half2<<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->vel, c->force, (uint32_t)c->N, 0.5 * dt);
     MD_LAUNCH_CHECK(c);
     return MD_OK;
 }
@@ -139,7 +169,28 @@ __global__ void __launch_bounds__(THERMO_BLOCK) k_thermo_final(const double *__r
     if (threadIdx.x < 5) out[threadIdx.x] = sm[threadIdx.x * THERMO_BLOCK];
 }
 
+static int thermo_reduce(md_ctx *c, double **res_out);
+
 int launch_thermo(md_ctx *c, double *out5_host)
+{
+    double *res = nullptr;
+    MD_TRY(thermo_reduce(c, &res));
+    MD_CUDA_CHECK(c, cudaMemcpyAsync(out5_host, res, 5 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    return md_sync(c);
+}
+
+// Nose-Hoover thermostat update (R30), on the device: K' from the two reduction kernels above, then one thread
+__global__ void k_nvt_update(const double *__restrict__ sums, double *__restrict__ nvt, double dt, double kT, double tau,
+                             double dof)
+{
+    const double K = sums[0];
+    const double xi_old = nvt[0];
+    const double xi = xi_old + (dt / (tau * tau)) * (2.0 * K / (dof * kT) - 1.0);
+    nvt[0] = xi;
+    nvt[1] = nvt[1] + 0.5 * dt * (xi + xi_old);
+}
+
+static int thermo_reduce(md_ctx *c, double **res_out)
 {
     const uint32_t N = (uint32_t)c->N;
     const uint32_t nb = (N + THERMO_PER_BLOCK - 1) / THERMO_PER_BLOCK;
@@ -155,6 +206,15 @@ int launch_thermo(md_ctx *c, double *out5_host)
     MD_LAUNCH_CHECK(c);
     k_thermo_final<<<1, THERMO_BLOCK, 0, c->stream>>>(c->thermo_buf, nb, res);
     MD_LAUNCH_CHECK(c);
-    MD_CUDA_CHECK(c, cudaMemcpyAsync(out5_host, res, 5 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
-    return md_sync(c);
+    *res_out = res;
+    return MD_OK;
+}
+
+int launch_nvt_thermostat(md_ctx *c, double dt, double kT, double tau)
+{
+    double *res = nullptr;
+    MD_TRY(thermo_reduce(c, &res));
+    k_nvt_update<<<1, 1, 0, c->stream>>>(res, c->nvt_state, dt, kT, tau, 3.0 * (double)c->N - 3.0);
+    MD_LAUNCH_CHECK(c);
+    return MD_OK;
 }

@@ -126,6 +126,7 @@ struct md_ctx {
     uint64_t scan_tmp_len = 0;
     void *stage = nullptr;  // host<->device staging
     uint64_t stage_bytes = 0;
+    double *nvt_state = nullptr;   // device: xi, eta (Nose-Hoover), allocated with the state
     double *thermo_buf = nullptr;  // per-block partial sums of md_thermo + the 5 results
     uint64_t thermo_len = 0;
     DevFlags *d_flags = nullptr;
@@ -189,8 +190,10 @@ int launch_nlist_fill(md_ctx *c);
 int launch_forces_lj(md_ctx *c, double eps, double sigma, int shift);
 int launch_forces_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed);
 int launch_forces_bonds(md_ctx *c, double k, double r0);
-int launch_half1(md_ctx *c, double dt, bool fused);  // fused: preceded by the previous step's half 2
-int launch_half2(md_ctx *c, double dt);
+// fused: preceded by the previous step's half 2.  nvt: Nose-Hoover friction xi read from c->nvt_state (R30)
+int launch_half1(md_ctx *c, double dt, bool fused, bool nvt = false);
+int launch_half2(md_ctx *c, double dt, bool nvt = false);
+int launch_nvt_thermostat(md_ctx *c, double dt, double kT, double tau);  // K' reduction + xi, eta update, all on the device
 int launch_thermo(md_ctx *c, double *out6_host);  // kinetic, potential, px, py, pz (device reduction, then D2H + sync)
 int launch_export_pairs_count(md_ctx *c, uint32_t *cnt);
 int launch_export_pairs_fill(md_ctx *c, const uint64_t *off, uint32_t *pairs);

@@ -29,7 +29,7 @@ def test_library_builds_and_exports_every_declared_symbol():
 
 def test_struct_layouts_match_header():
     import ctypes as C
-    assert C.sizeof(B.md_step_desc) == 80
+    assert C.sizeof(B.md_step_desc) == 96
     assert C.sizeof(B.md_stats) == 6 * 8 + 8 + 12 + 4 + 3 * 4 * B.MD_N_KERNELS + 8 + 16 * B.MD_N_KERNELS + 16
 
 

@@ -415,6 +415,53 @@ def test_thermo_reductions():
     assert abs(tp["kinetic"] - 0.5 * np.sum(wp.vel * wp.vel)) < 1e-12 * tp["kinetic"]
 
 
+def test_nvt_single_steps_and_trajectory():
+    """Nose-Hoover NVT (R30): md_integrate_nvt half by half and md_step(MD_F_NVT) against the oracle."""
+    wl = _thermalised_lj(6, kT=0.7)                                   # N = 864
+    kT0, tau, dt = 1.2, 0.4, wl.dt
+    # --- one step, half by half: positions 1e-12, thermostat variables to rounding
+    md = B.from_workload(wl)
+    md.build_nlist(); md.forces_lj()
+    md.set_thermostat(0.05, -0.01)
+    sim = oracle.Sim(wl.pos, wl.vel, wl.box, wl.rc, wl.r_buff, {"lj": wl.params}, nvt=dict(kT=kT0, tau=tau))
+    sim.xi, sim.eta = 0.05, -0.01
+    sim.compute_forces(dt, 0)
+    md.integrate_nvt(dt, 1, kT0, tau)
+    oracle.nvt_half1(sim.pos, sim.vel, sim.image, sim.force, sim.box, dt, sim.xi)
+    xi1, eta1, _ = oracle.nvt_thermostat(sim.vel, dt, kT0, tau, sim.xi, sim.eta)
+    pos, vel, img = md.get_state()
+    assert np.abs(min_image_diff(pos, sim.pos, wl.box)).max() < 1e-12
+    assert np.abs(vel - sim.vel).max() < 1e-12 and np.array_equal(img, sim.image)
+    gxi, geta = md.get_thermostat()
+    assert abs(gxi - xi1) < 1e-13 and abs(geta - eta1) < 1e-14
+    if md.needs_rebuild():
+        md.build_cells(); md.build_nlist()
+    md.forces_lj()
+    sim.xi, sim.eta = xi1, eta1
+    sim.compute_forces(dt, 1)
+    md.integrate_nvt(dt, 2, kT0, tau)
+    oracle.nvt_half2(sim.vel, sim.force, dt, sim.xi)
+    _, vel, _ = md.get_state()
+    assert np.abs(vel - sim.vel).max() < 1e-11
+    # --- md_step with the thermostat (fused half 2 + half 1, device-side K reduction), 40 steps with rebuilds
+    md2 = B.from_workload(wl)
+    md2.step(B.step_desc("lj", dt, wl.params, nvt=dict(kT=kT0, tau=tau)), 40)
+    sim2 = oracle.Sim(wl.pos, wl.vel, wl.box, wl.rc, wl.r_buff, {"lj": wl.params}, nvt=dict(kT=kT0, tau=tau)).run(40, dt)
+    pos, vel, _ = md2.get_state()
+    assert np.abs(min_image_diff(pos, sim2.pos, wl.box)).max() < 1e-9     # Lyapunov growth from 1e-16 over 40 steps
+    gxi, geta = md2.get_thermostat()
+    assert abs(gxi - sim2.xi) < 1e-10 and abs(geta - sim2.eta) < 1e-10
+    assert md2.stats()["rebuilds"] >= 2 and md2.stats()["dangerous_builds"] == 0
+    # the thermostat heats the T = 0.35 liquid (0.7 equipartitioned with the lattice) towards 1.2: xi went negative
+    assert sim2.xi < 0.0
+    # --- thermostat off (xi = 0, tau huge) is NVE, bit for bit in the positions
+    a = B.from_workload(wl); b = B.from_workload(wl)
+    a.step(B.step_desc("lj", dt, wl.params), 10)
+    b.step(B.step_desc("lj", dt, wl.params, nvt=dict(kT=kT0, tau=1e150)), 10)
+    pa, va, _ = a.get_state(); pb, vb, _ = b.get_state()
+    assert np.abs(min_image_diff(pa, pb, wl.box)).max() < 1e-13 and np.abs(va - vb).max() < 1e-13
+
+
 def test_tuner_runs_and_keeps_results():
     wl = _thermalised_lj(8)                                             # N=2048
     desc = B.step_desc("lj", wl.dt, wl.params)
