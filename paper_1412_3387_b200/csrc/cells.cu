@@ -333,7 +333,7 @@ __global__ void k_reorder(const uint32_t *__restrict__ perm_sorted, uint32_t N, 
     rtag[t] = s;
     const uint32_t lin = cell_lin_old[o];
     cell_lin[s] = lin;
-    rel[s] = md_rel_record(p.x, p.y, p.z, lin, g);
+    if (MD_STAGE_FROM_REL) rel[s] = md_rel_record(p.x, p.y, p.z, lin, g);
     pos_ref[3ull * s] = p.x;
     pos_ref[3ull * s + 1] = p.y;
     pos_ref[3ull * s + 2] = p.z;

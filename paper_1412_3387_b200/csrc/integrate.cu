@@ -48,7 +48,7 @@ __global__ void k_half1(double4 *__restrict__ pos, double4 *__restrict__ vel, co
             d2 = a == 0 ? __dmul_rn(d, d) : __dadd_rn(d2, __dmul_rn(d, d));
         }
         pos[i] = make_double4(x[0], x[1], x[2], p.w);
-        rel[i] = md_rel_record(x[0], x[1], x[2], cell_lin[i], g);  // meaningful once the particles are binned
+        if (MD_STAGE_FROM_REL) rel[i] = md_rel_record(x[0], x[1], x[2], cell_lin[i], g);  // meaningful once binned
         vel[i] = make_double4(u[0], u[1], u[2], m);
         if (d2 > thr2) {
             flags->rebuild = 1;  // benign race: every writer stores the same value

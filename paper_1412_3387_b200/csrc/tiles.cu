@@ -283,7 +283,8 @@ __device__ __forceinline__ void tile_stage(const Geom &g, const TileCtx &tc, con
 // md_rel_record): staged coordinate = fl(fl(x - C_w) + fl(c_s)), times `scale`.  No fp64, 16 bytes per particle.
 template <bool WITH_R2>
 __device__ __forceinline__ void tile_stage_rel(const TileCtx &tc, const TileSmem &h, const float4 *__restrict__ rel,
-                                               float4 *rec, uint8_t *scell, float scale)
+                                               float4 *rec, uint8_t *scell, float scale,
+                                               const double4 *__restrict__ pos, const Geom &g)
 {
     const uint32_t lane = threadIdx.x & 31u, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     for (uint32_t sc = wid; sc < tc.n_sc; sc += nw) {
@@ -291,6 +292,35 @@ __device__ __forceinline__ void tile_stage_rel(const TileCtx &tc, const TileSmem
         for (uint32_t s = b + lane; s < e; s += 32) scell[s] = (uint8_t)sc;
     }
     __syncthreads();
+    if (!MD_STAGE_FROM_REL) {
+        // fp64 staging: the coordinate relative to the brick centre is formed in fp64 and rounded ONCE (R25)
+        const double dscale = (double)scale;
+        for (uint32_t s0 = threadIdx.x; s0 < tc.n_staged; s0 += 2 * blockDim.x) {
+            double4 pp[2];
+            uint32_t scs[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const uint32_t s = s0 + u * blockDim.x;
+                if (s < tc.n_staged) {
+                    scs[u] = scell[s];
+                    pp[u] = pos[h.gstart[scs[u]] + (s - h.sstart[scs[u]])];
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const uint32_t s = s0 + u * blockDim.x;
+                if (s < tc.n_staged) {
+                    const double *cg = h.cgeo + 6 * scs[u];
+                    const float x = (float)((cg[3] + md_min_image(pp[u].x - cg[0], g.L[0], g.h[0])) * dscale);
+                    const float y = (float)((cg[4] + md_min_image(pp[u].y - cg[1], g.L[1], g.h[1])) * dscale);
+                    const float z = (float)((cg[5] + md_min_image(pp[u].z - cg[2], g.L[2], g.h[2])) * dscale);
+                    rec[s] = make_float4(x, y, z, WITH_R2 ? x * x + y * y + z * z : 0.f);
+                }
+            }
+        }
+        if (threadIdx.x < N_DUMMY) rec[tc.n_staged + threadIdx.x] = RecTraits<float4>::far();
+        return;
+    }
     // 4 records per thread and trip, all 4 global loads issued before the first is used: the loop is a chain of L2
     // round trips otherwise (a thread stages ~9 records)
     for (uint32_t s0 = threadIdx.x; s0 < tc.n_staged; s0 += 4 * blockDim.x) {
@@ -364,7 +394,7 @@ __device__ __forceinline__ unsigned md_lanemask_lt()
 }
 
 template <int P>
-__global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build(TileParams tp, Geom g, const float4 *__restrict__ rel,
+__global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build(TileParams tp, Geom g, const float4 *__restrict__ rel, const double4 *__restrict__ pos,
                                                                float thr_out /* r_list^2 + guard */,
                                                                uint32_t max_staged, uint32_t *__restrict__ nl_cnt,
                                                                uint16_t *__restrict__ nl16, DevFlags *flags)
@@ -379,7 +409,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build(TileParams tp, Ge
 
     TileCtx tc;
     tile_setup(tp, g, blockIdx.x, h, tc);
-    tile_stage_rel<true>(tc, h, rel, rec, scell, 1.f);
+    tile_stage_rel<true>(tc, h, rel, rec, scell, 1.f, pos, g);
     if (threadIdx.x < 32) {  // first task of each home cell: exclusive scan of ceil(count / P), n_hc <= 64
         uint32_t carry = 0;
         for (uint32_t base = 0; base <= tc.n_hc; base += 32) {
@@ -605,7 +635,7 @@ __device__ __forceinline__ void b8_run(const float4 *rec, uint32_t b, uint32_t e
     }
 }
 
-__global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build8(TileParams tp, Geom g, const float4 *__restrict__ rel,
+__global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build8(TileParams tp, Geom g, const float4 *__restrict__ rel, const double4 *__restrict__ pos,
                                                                 float thr_out /* r_list^2 + guard */,
                                                                 uint32_t max_staged, uint32_t *__restrict__ nl_cnt,
                                                                 uint16_t *__restrict__ nl16, DevFlags *flags)
@@ -624,7 +654,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build8(TileParams tp, G
 
     TileCtx tc;
     tile_setup(tp, g, blockIdx.x, h, tc);
-    tile_stage_rel<true>(tc, h, rel, rec, scell, 1.f);
+    tile_stage_rel<true>(tc, h, rel, rec, scell, 1.f, pos, g);
     if (threadIdx.x < 32) {  // first task of each home cell: exclusive scan of ceil(count / P), n_hc <= 64
         uint32_t carry = 0;
         for (uint32_t base = 0; base <= tc.n_hc; base += 32) {
@@ -770,7 +800,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build8(TileParams tp, G
 // registers, in the list build and again in the force kernel, which cuts the shared-memory gathers 4-fold.
 // ===============================================================================================================
 template <int P>
-__global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build_c(TileParams tp, Geom g, const float4 *__restrict__ rel,
+__global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build_c(TileParams tp, Geom g, const float4 *__restrict__ rel, const double4 *__restrict__ pos,
                                                                  float thr_out /* r_list^2 + guard */,
                                                                  uint32_t max_staged, uint32_t *__restrict__ nl_cnt,
                                                                  uint16_t *__restrict__ nl16, DevFlags *flags)
@@ -786,7 +816,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build_c(TileParams tp, 
 
     TileCtx tc;
     tile_setup(tp, g, blockIdx.x, h, tc);
-    tile_stage_rel<true>(tc, h, rel, rec, scell, 1.f);
+    tile_stage_rel<true>(tc, h, rel, rec, scell, 1.f, pos, g);
     if (threadIdx.x < 32) {  // first task of each home cell: exclusive scan of ceil(count / P), n_hc <= 64
         uint32_t carry = 0;
         for (uint32_t base = 0; base <= tc.n_hc; base += 32) {
@@ -953,7 +983,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj(TileParams tp, Geom 
 
     TileCtx tc;
     tile_setup(tp, g, blockIdx.x, h, tc);
-    if constexpr (MIXED) tile_stage_rel<false>(tc, h, rel, (float4 *)rec, scell, 1.f);
+    if constexpr (MIXED) tile_stage_rel<false>(tc, h, rel, (float4 *)rec, scell, 1.f, pos, g);
     else tile_stage<R4, false>(g, tc, h, pos, nullptr, rec, nullptr, scell);
     __syncthreads();
 
@@ -1140,7 +1170,7 @@ __global__ void __launch_bounds__(256, 4) k_tile_lj3(TileParams tp, Geom g, cons
 
     TileCtx tc;
     tile_setup(tp, g, blockIdx.x, h, tc);
-    tile_stage_rel<false>(tc, h, rel, rec, scell, (float)lj.inv_sigma);
+    tile_stage_rel<false>(tc, h, rel, rec, scell, (float)lj.inv_sigma, pos, g);
     // staged index of every home particle (replaces a search per particle)
     uint16_t *hsidx = (uint16_t *)(scell + ((max_staged + 16) & ~15u));
     for (uint32_t hc = threadIdx.x >> 5; hc < tc.n_hc; hc += blockDim.x >> 5) {
@@ -1568,7 +1598,7 @@ __global__ void __launch_bounds__(256, MINB) k_tile_lj4(TileParams tp, Geom g, c
 
     TileCtx tc;
     tile_setup(tp, g, blockIdx.x, h, tc);
-    tile_stage_rel<false>(tc, h, rel, rec, scell, (float)lj.inv_sigma);
+    tile_stage_rel<false>(tc, h, rel, rec, scell, (float)lj.inv_sigma, pos, g);
     if (threadIdx.x < 32) {  // first cluster of each home cell (n_hc <= 64), as in the build kernel
         uint32_t carry = 0;
         for (uint32_t base = 0; base <= tc.n_hc; base += 32) {
@@ -2126,15 +2156,15 @@ int launch_tile_build(md_ctx *c, bool cluster, bool *fits)
     const double gd = guard_dot_fp32(E, R);
     if (cluster) {
         MD_TRY(set_smem(c, k_tile_build_c<BUILD_P>, smem));
-        k_tile_build_c<BUILD_P><<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->rel, (float)(rl2 + gd), ms, c->nl_cnt,
+        k_tile_build_c<BUILD_P><<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->rel, c->pos, (float)(rl2 + gd), ms, c->nl_cnt,
                                                                        c->nl16, c->d_flags);
     } else if (b8) {
         MD_TRY(set_smem(c, k_tile_build8, smem));
-        k_tile_build8<<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->rel, (float)(rl2 + gd), ms, c->nl_cnt, c->nl16,
+        k_tile_build8<<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->rel, c->pos, (float)(rl2 + gd), ms, c->nl_cnt, c->nl16,
                                                              c->d_flags);
     } else {
         MD_TRY(set_smem(c, k_tile_build<BUILD_P>, smem));
-        k_tile_build<BUILD_P><<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->rel, (float)(rl2 + gd), ms, c->nl_cnt,
+        k_tile_build<BUILD_P><<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->rel, c->pos, (float)(rl2 + gd), ms, c->nl_cnt,
                                                                      c->nl16, c->d_flags);
     }
     MD_LAUNCH_CHECK(c);
