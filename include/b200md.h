@@ -47,10 +47,12 @@ typedef enum {
    option"; here a run-time mode, R25) */
 #define MD_FP64 0   /* everything fp64 */
 #define MD_MIXED 1  /* LJ pair polynomial in fp32 on fp32 separations, r<rc decision as fp64 would take it,
-                       per-pair contributions summed in fp64; positions, velocities, integration, cell ids,
-                       neighbour-list decisions, displacement check stay fp64 */
+                       contributions accumulated in fp64 (fp32 sums of 8 consecutive list entries are widened,
+                       MD_OPT_ACC_BLOCK); positions, velocities, integration, cell ids, neighbour-list decisions,
+                       displacement check stay fp64 */
 
-/* internal storage order of the cells (particles are always sorted by cell, ties by tag) */
+/* internal storage order of the cells (particles are always sorted by cell; inside a cell by tag, with
+   MD_ORDER_MORTON by (3-bit-per-axis sub-cell Morton key, tag): a pure function of the positions either way) */
 #define MD_ORDER_LEX 0     /* x fastest, then y, then z; general list kernels (32-bit indices, L1/L2 gathers) */
 #define MD_ORDER_MORTON 1  /* Z-order curve over (cx, cy, cz); enables the tile kernels: one CTA per brick of cells,
                               stencil staged in shared memory, 16-bit list entries (the fast path, default of the
