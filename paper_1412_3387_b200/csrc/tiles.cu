@@ -1177,8 +1177,10 @@ __global__ void __launch_bounds__(256, 4) k_tile_lj3(TileParams tp, Geom g, cons
         const uint32_t p0 = h.hc_first[hc], p1 = h.hc_first[hc + 1], s0 = h.sstart[h.hc_sc[hc]];
         for (uint32_t p = p0 + (threadIdx.x & 31u); p < p1; p += 32) hsidx[p] = (uint16_t)(s0 + (p - p0));
     }
-    __shared__ uint32_t next_p[2];  // next unassigned home particle of each parity, in units of 2
-    if (threadIdx.x < 2) next_p[threadIdx.x] = blockDim.x / (2 * W);
+    // next unassigned home particle of each residue class (p mod 2 for W >= 4, p mod 4 for W = 2: the row rotation)
+    constexpr uint32_t NRES = W == 2 ? 4u : 2u;
+    __shared__ uint32_t next_p[4];
+    if (threadIdx.x < NRES) next_p[threadIdx.x] = blockDim.x / (NRES * W);
     __syncthreads();
 
     const unsigned lane = threadIdx.x & (W - 1);
@@ -1192,11 +1194,11 @@ __global__ void __launch_bounds__(256, 4) k_tile_lj3(TileParams tp, Geom g, cons
     // Particles are handed out dynamically (rows differ in length): a group takes the next particle of ITS parity --
     // the bank-class layout ties the parity of the home index to the half of the quarter-warp the group sits in --
     // from a shared counter, one particle ahead of the one it evaluates.
-    const uint32_t grp = threadIdx.x / W, par = grp & 1u;
+    const uint32_t grp = threadIdx.x / W, par = grp & (NRES - 1u);
     auto grab = [&]() -> uint32_t {
         uint32_t v = 0;
         if (lane == 0) v = atomicAdd(&next_p[par], 1u);
-        return 2u * __shfl_sync(seg_mask, v, 0, W) + par;
+        return NRES * __shfl_sync(seg_mask, v, 0, W) + par;
     };
     uint32_t p = grp;
     uint32_t cnt_c = 0;
@@ -2275,7 +2277,7 @@ int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
             return MD_OK;
         }
     }
-    if (mixed && !energy && c->nl_shift && c->acc_block == 8 && cf.w >= 4 && lj3_mode) {
+    if (mixed && !energy && c->nl_shift && c->acc_block == 8 && cf.w >= 2 && lj3_mode) {
         const size_t smem = tile_smem_common(c, sizeof(float4), false) + ((2 * (size_t)c->tile_max_home + 15) & ~(size_t)15);
         LJ3 q;
         q.rc2_exact = p.rc2_exact;
@@ -2287,7 +2289,10 @@ int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
         q.guard = (float)(1.0001 * (gd / p.sig2 + 2.0 * 5.9604644775390625e-08 * rc2s));
         const int w = cf.w > 8 ? 8 : cf.w;
         cf.block = std::min(cf.block, 256);  // k_tile_lj3 is compiled for 4 CTAs of 256 threads per SM (64 registers)
-        if (w == 4) {
+        if (w == 2) {  // rows laid out with rotation 2 (p & 3) when the list was built for W = 2 (launch_tile_build)
+            MD_TRY(set_smem(c, (k_tile_lj3<2, true>), smem));
+            k_tile_lj3<2, true><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force);
+        } else if (w == 4) {
             if (lj3_mode == 2) {
                 MD_TRY(set_smem(c, k_tile_lj3<4, true>, smem));
                 k_tile_lj3<4, true><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force);
