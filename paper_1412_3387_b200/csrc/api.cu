@@ -1014,19 +1014,19 @@ extern "C" int md_tune(md_ctx *c, const md_step_desc *w, int full)
     }
     if (w->flags & MD_F_LJ)
         MD_TRY(tune_kernel(c, MD_K_LJ, c->nl_is_tile ? "lj/tile" : "lj", true, full, [&]() {
-            // the row rotation of the tile list follows W (2 lanes per particle or more): time each W on its own layout
-            if (c->nl_is_tile && !c->nl_cluster && c->nl_rot2 != (c->cfg[MD_K_LJ].w == 2)) MD_TRY(do_build_nlist(c));
+            // the row rotation of the tile list follows W (1, 2 or more lanes per particle): time each W on its own layout
+            if (c->nl_is_tile && !c->nl_cluster && c->nl_rotw != tile_rot_class(c->cfg[MD_K_LJ].w)) MD_TRY(do_build_nlist(c));
             return pair_lj(c, w->lj_epsilon, w->lj_sigma, w->lj_energy_shift, false);
         }));
     if (w->flags & MD_F_DPD)
         MD_TRY(tune_kernel(c, MD_K_DPD, c->nl_is_tile ? "dpd/tile" : "dpd", true, full, [&]() {
-            if (c->nl_is_tile && !c->nl_cluster && c->nl_rot2 != (c->cfg[MD_K_DPD].w == 2)) MD_TRY(do_build_nlist(c));
+            if (c->nl_is_tile && !c->nl_cluster && c->nl_rotw != tile_rot_class(c->cfg[MD_K_DPD].w)) MD_TRY(do_build_nlist(c));
             return pair_dpd(c, w->dpd_A, w->dpd_gamma, w->dpd_kT, w->dt, c->step, w->dpd_seed);
         }));
     // the list the run starts with has the layout of the chosen W
     if (c->nl_is_tile && !c->nl_cluster) {
         const bool dpd = (w->flags & MD_F_DPD) != 0 && !(w->flags & MD_F_LJ);
-        if (c->nl_rot2 != (c->cfg[dpd ? MD_K_DPD : MD_K_LJ].w == 2)) MD_TRY(do_build_nlist(c));
+        if (c->nl_rotw != tile_rot_class(c->cfg[dpd ? MD_K_DPD : MD_K_LJ].w)) MD_TRY(do_build_nlist(c));
     }
     c->force_valid = false;  // the replays overwrote the force array with a partial evaluation (pair term only)
     c->tuned = true;

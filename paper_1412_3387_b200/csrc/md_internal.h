@@ -100,7 +100,8 @@ struct md_ctx {
     bool use_tiles = false;     // configured (MD_ORDER_MORTON)
     bool nl_is_tile = false;    // the current list is a tile list
     bool nl32_decoded = false;  // nl_off/nl_idx hold the decoded copy of the current tile list (exports)
-    bool nl_rot2 = false;       // rows of the current tile list rotate by 2 (p & 3): laid out for W = 2 force kernels
+    int nl_rotw = 4;            // lanes per particle (1, 2 or 4 = "4 or more") the rows of the current tile list are rotated for
+
     bool nl_cluster = false;    // the current tile list has one row per cluster of 4 particles (k_tile_build_c)
     int cluster_opt = 0;        // MD_OPT_CLUSTER
     int stride_mode = -1;       // list format nl_stride was sized for (0 particle rows, 1 cluster rows)
@@ -206,6 +207,7 @@ int build_cell_order(md_ctx *c);  // host: rank_of_lin table for the configured 
 int tile_measure(md_ctx *c);
 int launch_tile_build(md_ctx *c, bool cluster, bool *fits);
 bool tile_cluster_ok(md_ctx *c);
+static inline int tile_rot_class(int w) { return w <= 1 ? 1 : (w == 2 ? 2 : 4); }
 int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy);
 int launch_tile_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed);
 bool tile_forces_fit(md_ctx *c, bool dpd);

@@ -1177,9 +1177,10 @@ __global__ void __launch_bounds__(256, 4) k_tile_lj3(TileParams tp, Geom g, cons
         const uint32_t p0 = h.hc_first[hc], p1 = h.hc_first[hc + 1], s0 = h.sstart[h.hc_sc[hc]];
         for (uint32_t p = p0 + (threadIdx.x & 31u); p < p1; p += 32) hsidx[p] = (uint16_t)(s0 + (p - p0));
     }
-    // next unassigned home particle of each residue class (p mod 2 for W >= 4, p mod 4 for W = 2: the row rotation)
-    constexpr uint32_t NRES = W == 2 ? 4u : 2u;
-    __shared__ uint32_t next_p[4];
+    // next unassigned home particle of each residue class (p mod 2 for W >= 4, mod 4 for W = 2, mod 8 for W = 1: the
+    // row rotation)
+    constexpr uint32_t NRES = W == 1 ? 8u : (W == 2 ? 4u : 2u);
+    __shared__ uint32_t next_p[8];
     if (threadIdx.x < NRES) next_p[threadIdx.x] = blockDim.x / (NRES * W);
     __syncthreads();
 
@@ -2048,9 +2049,10 @@ static TileParams make_tp(md_ctx *c)
     for (int a = 0; a < 3; ++a) tp.cw[a] = c->box[a] / (double)c->dims[a];
     // rows rotate so that the 8 lanes of a quarter-warp of the force kernel meet 8 different bank classes: with W >= 4
     // lanes per particle a quarter holds 2 particles x 4 blocks (rotation 0 / 4), with W = 2 it holds 4 particles x 2
-    // blocks (rotation 0 / 2 / 4 / 6).  Layout only: any rotation is a correct list.
-    tp.rot_mul = c->nl_rot2 ? 2u : 4u;
-    tp.rot_mask = c->nl_rot2 ? 3u : 1u;
+    // blocks (rotation 0 / 2 / 4 / 6), with W = 1 eight particles x 1 block (rotation 0 .. 7).  Layout only: any
+    // rotation is a correct list.
+    tp.rot_mul = (uint32_t)c->nl_rotw;          // W = 1: rotation p & 7;  W = 2: 2 (p & 3);  W >= 4: 4 (p & 1)
+    tp.rot_mask = 8u / (uint32_t)c->nl_rotw - 1u;
     tp.desc_words = (TILE_DESC_CTX + tile_desc_table_words(c->tile_B) + 3u) & ~3u;
     tp.desc = c->tile_desc_valid ? c->tile_desc : nullptr;
     return tp;
@@ -2149,7 +2151,7 @@ int launch_tile_build(md_ctx *c, bool cluster, bool *fits)
     c->nl_shift = tile_shift(c);
     {   // the force kernel that will read the list: the last step description says which, else LJ
         const bool dpd = (c->force_hint & MD_F_DPD) != 0 && !(c->force_hint & MD_F_LJ);
-        c->nl_rot2 = !cluster && c->cfg[dpd ? MD_K_DPD : MD_K_LJ].w == 2;
+        c->nl_rotw = cluster ? 4 : tile_rot_class(c->cfg[dpd ? MD_K_DPD : MD_K_LJ].w);
     }
     const double R = c->r_list * 1.001, E = tile_extent(c), rl2 = c->r_list * c->r_list;
     MD_CUDA_CHECK(c, cudaMemsetAsync(&c->d_flags->nl_total, 0, sizeof(unsigned long long), c->stream));
@@ -2277,7 +2279,7 @@ int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
             return MD_OK;
         }
     }
-    if (mixed && !energy && c->nl_shift && c->acc_block == 8 && cf.w >= 2 && lj3_mode) {
+    if (mixed && !energy && c->nl_shift && c->acc_block == 8 && lj3_mode) {
         const size_t smem = tile_smem_common(c, sizeof(float4), false) + ((2 * (size_t)c->tile_max_home + 15) & ~(size_t)15);
         LJ3 q;
         q.rc2_exact = p.rc2_exact;
@@ -2289,7 +2291,10 @@ int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
         q.guard = (float)(1.0001 * (gd / p.sig2 + 2.0 * 5.9604644775390625e-08 * rc2s));
         const int w = cf.w > 8 ? 8 : cf.w;
         cf.block = std::min(cf.block, 256);  // k_tile_lj3 is compiled for 4 CTAs of 256 threads per SM (64 registers)
-        if (w == 2) {  // rows laid out with rotation 2 (p & 3) when the list was built for W = 2 (launch_tile_build)
+        if (w <= 1) {
+            MD_TRY(set_smem(c, (k_tile_lj3<1, true>), smem));
+            k_tile_lj3<1, true><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force);
+        } else if (w == 2) {  // rows laid out with rotation 2 (p & 3) when the list was built for W = 2 (launch_tile_build)
             MD_TRY(set_smem(c, (k_tile_lj3<2, true>), smem));
             k_tile_lj3<2, true><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force);
         } else if (w == 4) {
