@@ -33,8 +33,8 @@ FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback when 
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/r1_v5_cfg2.md); None where no capture of that workload/kernel exists
-NCU_TRAFFIC = {("cfg2-lj-1M-mixed", "k_tile_lj3"): 463.0e6}
+# `ncu --set full` capture (profiles/r1_v7_cfg2.md); None where no capture of that workload/kernel exists
+NCU_TRAFFIC = {("cfg2-lj-1M-mixed", "k_tile_lj3"): 463.7e6}
 
 
 def measured_hbm_peak():
