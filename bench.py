@@ -266,7 +266,7 @@ def run_ours(args):
     md.get_state(h_pos, h_vel, None)
     torch.cuda.synchronize()
     st0 = md.stats()
-    md.set_profiling(True)
+    md.set_profiling(2)            # CUDA events around the pair-force stage only (the roofline kernel): 2 events per step
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
@@ -281,7 +281,18 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else None
     ms = e0.elapsed_time(e1)
     st1 = md.stats()
-    md.set_profiling(False)
+    # stage shares: a short untimed continuation with every stage bracketed by events (about 8 events per step)
+    md.set_profiling(1)
+    n_share = max(20, min(200, args.steps // 4))
+    with torch.cuda.stream(stream):
+        s0 = torch.cuda.Event(enable_timing=True); s1 = torch.cuda.Event(enable_timing=True)
+        s0.record(stream)
+        md.step(desc, n_share)
+        s1.record(stream)
+    torch.cuda.synchronize()
+    ms_share = s0.elapsed_time(s1)
+    st_share = md.stats()
+    md.set_profiling(0)
 
     # ---- end to end through the C-ABI with HOST buffers: upload state, K steps, download state ----------------
     o_pos = torch.empty_like(h_pos).pin_memory()
@@ -318,7 +329,7 @@ def run_ours(args):
             kernel = "k_tile_lj3d"
         f_ms = st1["stage_ms"][fk] / max(1, st1["stage_launches"][fk])
         achieved = w.N * b_force / (f_ms * 1e-3) / 1e9 if f_ms > 0 else 0.0
-        stage_share = {n: round(v / ms, 4) for n, v in st1["stage_ms"].items() if v > 0}
+        stage_share = {n: round(v / ms_share, 4) for n, v in st_share["stage_ms"].items() if v > 0}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": ms_max / args.steps, "higher_is_better": True,
@@ -334,6 +345,7 @@ def run_ours(args):
                        "wasted_forces": st1["wasted_forces"] - st0["wasted_forces"],
                        "launch": {n: [v["block"], v["w"]] for n, v in st1["launch"].items()},
                        "stage_share_of_step": stage_share,
+                       "stage_share_from": "%d further steps with every stage bracketed by CUDA events" % n_share,
                        "step_bmin_bytes_per_particle": b_min,
                        "step_roofline_frac": (w.N * b_min * args.steps / (ms_max * 1e-3)) / (peak * 1e9)},
             "e2e": {"value": world * w.N * args.steps / (e2e_ms * 1e-3), "unit": UNIT,

@@ -256,7 +256,8 @@ int md_thermo(md_ctx *ctx, md_thermo_t *out);
 /* on = 1: bracket every stage launched by md_step / md_build_* / md_forces_* / md_integrate_nve with CUDA events on the
    context's stream and accumulate their durations into md_stats.stage_ms (MD_K_CELLS = binning + reorder, MD_K_NLIST =
    count + scan + fill, MD_K_LJ / MD_K_DPD / MD_K_BONDS force kernels, MD_K_INTEGRATE both halves).  Resets the
-   accumulators.  on = 0 switches the events off. */
+   accumulators.  on = 2: only the pair-force stages (MD_K_LJ / MD_K_DPD) are bracketed -- two events per step instead of
+   about eight, for timing a run while measuring its dominant kernel.  on = 0 switches the events off. */
 int md_set_profiling(md_ctx *ctx, int on);
 
 /* Test hook: Philox4x32-10 of `n` (counter, key) inputs evaluated ON THE DEVICE by the same device function the

@@ -64,6 +64,7 @@ static cudaEvent_t prof_event(md_ctx *c)
 ProfScope::ProfScope(md_ctx *ctx, int kernel) : c(ctx), k(kernel)
 {
     if (!c->profiling) return;
+    if (c->profiling == 2 && kernel != MD_K_LJ && kernel != MD_K_DPD) return;
     e0 = prof_event(c);
     e1 = prof_event(c);
     cudaEventRecord(e0, c->stream);
@@ -117,7 +118,7 @@ extern "C" int md_set_profiling(md_ctx *c, int on)
     if (!c) return MD_EINVAL;
     MD_TRY(md_sync(c));
     prof_resolve(c);
-    c->profiling = on != 0;
+    c->profiling = on == 2 ? 2 : (on != 0 ? 1 : 0);
     for (int k = 0; k < MD_N_KERNELS; ++k) { c->stats.stage_ms[k] = 0.0; c->stats.stage_launches[k] = 0; }
     return MD_OK;
 }

@@ -155,7 +155,7 @@ struct md_ctx {
     bool log = false;
 
     // per-stage event timing (md_set_profiling)
-    bool profiling = false;
+    int profiling = 0;  // 0 off, 1 every stage, 2 pair-force stages only (md_set_profiling)
     std::vector<cudaEvent_t> ev_pool;
     struct Pending { int k; cudaEvent_t e0, e1; };
     std::vector<Pending> ev_pending;
