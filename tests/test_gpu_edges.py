@@ -57,3 +57,27 @@ def test_dpd_sparse_and_tiny_systems(N, L):
     F, _ = md.get_forces()
     Fr = oracle.forces_dpd(wpos, vel, box, 1.0, 25.0, 4.5, 1.0, 0.02, 9, 42)
     assert np.abs(F - Fr).max() <= 1e-10 * np.abs(Fr).max() + 1e-13
+
+
+@pytest.mark.parametrize("prec,cluster", [(B.MD_FP64, 0), (B.MD_MIXED, 0), (B.MD_MIXED, 1)])
+def test_inhomogeneous_slab_grows_the_row_stride(prec, cluster):
+    """All particles in a slab a quarter of the box wide: local density 4x the mean, so the rows are ~4x longer than the
+    density-based stride estimate -> the build reports the overflow, the stride grows and the list is built again."""
+    rng = np.random.default_rng(1)
+    box = np.array([14.0, 14.0, 14.0])
+    N = 1500
+    pos = (rng.random((N, 3)) - 0.5) * box
+    pos[:, 0] = (rng.random(N) - 0.5) * 3.5
+    wpos = oracle.wrap(pos, box)
+    ref = oracle.neighbor_pairs(wpos, box, 2.9)
+    assert 2 * len(ref) / N > 2.5 * (N / box.prod()) * 4.18879 * 2.9 ** 3        # rows far beyond the mean-density estimate
+    md = B.MD(box, N, 2.5, 0.4, precision=prec)
+    md.set_option(B.MD_OPT_CLUSTER, cluster)
+    md.set_state(pos, np.zeros((N, 3)))
+    md.build_nlist()
+    assert np.array_equal(sort_pairs(md.get_nlist()), ref)
+    assert abs(md.stats()["mean_neighbors"] - 2 * len(ref) / N) < 0.01 * 2 * len(ref) / N
+    md.forces_lj()
+    F, _ = md.get_forces()
+    Fr, _ = oracle.forces_lj(wpos, box, 2.5)
+    assert np.abs(F - Fr).max() <= (1e-10 if prec == B.MD_FP64 else 1e-4) * np.abs(Fr).max()
