@@ -206,10 +206,13 @@ int md_step(md_ctx *ctx, const md_step_desc *what, uint64_t n_steps);
 
 /* ---- S8 runtime tuner ------------------------------------------------------------------ */
 
-/* Sweeps block size (multiples of 32 up to 1024; `full` = all 32, else a pruned set) x threads per particle
-   w in {1,2,4,8,16,32} for the neighbour-list kernel and the pair-force kernel `what` selects, on the live state
-   (the kernels are pure functions of it), median of 5 timed launches each, and fixes the fastest.  Choices are
-   reported by md_get_stats and, if the environment variable B200MD_LOG is set, printed to stderr. */
+/* Sweeps, for EVERY kernel family of the step `what` describes (binning, neighbour list, pair force, bonds,
+   integrator), the block size (multiples of 32 up to the kernel's compiled limit; `full` = all of them, else a pruned
+   set) and, where the kernel has it, the threads per particle w in {1,2,4,8,16,32}, on the live state (the kernels are
+   pure functions of it; half 1 is replayed with dt = 0, the binning only while no step has been taken since the last
+   one), median of 5 timed launches each, and fixes the fastest.  md_get_stats reports the LAUNCHED (block, w) per
+   kernel; with the environment variable B200MD_LOG set every timing is printed to stderr.  MD_OPT_RETUNE_PERIOD = M
+   makes md_step repeat a local re-scan (neighbouring block sizes, w/2 .. 2w) after every M rebuilds. */
 int md_tune(md_ctx *ctx, const md_step_desc *what, int full);
 
 /* Options of the tile path (MD_ORDER_MORTON).  MD_OPT_TILE_BRICK: edge of the cell brick one CTA owns, 1, 2 or 4
@@ -224,6 +227,7 @@ int md_tune(md_ctx *ctx, const md_step_desc *what, int full);
    each stored candidate against the 4 members in registers.  The exported list is the exact
    per-particle list either way.  0 (default) = one row per particle.  Invalidates the list. */
 #define MD_OPT_CLUSTER 3
+#define MD_OPT_RETUNE_PERIOD 4 /* rebuilds between periodic local re-scans of the tuner inside md_step; 0 (default) = never */
 int md_set_option(md_ctx *ctx, int option, int64_t value);
 
 /* Fix launch parameters by hand (block multiple of 32 in [32,1024]; w power of two <= 32); kernel = MD_K_*. */
@@ -263,6 +267,15 @@ int md_set_profiling(md_ctx *ctx, int on);
 /* Test hook: Philox4x32-10 of `n` (counter, key) inputs evaluated ON THE DEVICE by the same device function the
    DPD kernel uses.  ctr: n x 4 uint32, key: n x 2 uint32, out: n x 4 uint32 (host or device pointers). */
 int md_debug_philox(md_ctx *ctx, const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint64_t n);
+
+/* Measurement hook (measured, not nominal, peaks of the non-tensor pipes; PAPER.md:300 is the paper's
+   only statement on what bounds the path): issue rate of one instruction kind on the whole GPU, every thread running 8
+   independent chains, in giga lane-instructions per second (an FMA counts once; FMA2 = packed fma.rn.f32x2, counted
+   once per instruction, i.e. two FMAs; CVT = cvt.f64.f32 / cvt.rn.f32.f64; LDS128 = conflict-free 16-byte shared loads).
+   Best of 3 timed launches on the context's stream; synchronises.  giga_per_s: HOST pointer. */
+enum { MD_PEAK_FP32_FMA = 0, MD_PEAK_FP32_FMA2 = 1, MD_PEAK_FP64_FMA = 2, MD_PEAK_INT32_MAD = 3, MD_PEAK_INT32_MULHI = 4,
+       MD_PEAK_CVT_F32_F64 = 5, MD_PEAK_RCP_F32 = 6, MD_PEAK_LDS128 = 7 };
+int md_debug_peak(md_ctx *ctx, int pipe, double *giga_per_s);
 
 #ifdef __cplusplus
 }

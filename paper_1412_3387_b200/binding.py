@@ -18,7 +18,7 @@ MD_FP64, MD_MIXED = 0, 1
 MD_ORDER_LEX, MD_ORDER_MORTON, MD_ORDER_HILBERT = 0, 1, 2
 MD_F_LJ, MD_F_DPD, MD_F_BONDS, MD_F_NVT = 1, 2, 4, 8
 MD_SCHED_SYNC, MD_SCHED_SPECULATIVE = 0, 1
-MD_OPT_TILE_BRICK, MD_OPT_ACC_BLOCK, MD_OPT_CLUSTER = 1, 2, 3
+MD_OPT_TILE_BRICK, MD_OPT_ACC_BLOCK, MD_OPT_CLUSTER, MD_OPT_RETUNE_PERIOD = 1, 2, 3, 4
 MD_N_KERNELS = 8
 MD_K_NLIST, MD_K_LJ, MD_K_DPD, MD_K_BONDS, MD_K_INTEGRATE, MD_K_CELLS = 0, 1, 2, 3, 4, 5
 KERNEL_NAMES = {MD_K_NLIST: "nlist", MD_K_LJ: "lj", MD_K_DPD: "dpd", MD_K_BONDS: "bonds",
@@ -28,7 +28,7 @@ EXPORTS = ["md_create", "md_configure", "md_destroy", "md_last_error", "md_set_s
            "md_get_state", "md_get_forces", "md_build_cells", "md_get_cells", "md_build_nlist", "md_get_nlist",
            "md_get_nlist_rows", "md_forces_lj", "md_forces_dpd", "md_forces_bonds", "md_integrate_nve",
            "md_needs_rebuild", "md_step", "md_tune", "md_set_option", "md_set_launch", "md_get_stats", "md_set_profiling",
-           "md_debug_philox", "md_thermo", "md_integrate_nvt", "md_set_thermostat", "md_get_thermostat"]
+           "md_debug_philox", "md_debug_peak", "md_thermo", "md_integrate_nvt", "md_set_thermostat", "md_get_thermostat"]
 
 
 class md_step_desc(C.Structure):
@@ -96,6 +96,7 @@ def load():
         "md_get_stats": [vp, C.POINTER(md_stats)],
         "md_set_profiling": [vp, i32],
         "md_debug_philox": [vp, vp, vp, vp, u64],
+        "md_debug_peak": [vp, i32, C.POINTER(dbl)],
         "md_thermo": [vp, vp],
         "md_integrate_nvt": [vp, C.c_double, i32, C.c_double, C.c_double],
         "md_set_thermostat": [vp, C.c_double, C.c_double],
@@ -304,6 +305,15 @@ class MD:
         self._chk(self.L.md_thermo(self.h, C.byref(t)), "md_thermo")
         return dict(kinetic=t.kinetic, potential=t.potential, momentum=np.array(list(t.momentum)),
                     temperature=t.temperature)
+
+    PEAK_PIPES = {"fp32_fma": 0, "fp32_fma2": 1, "fp64_fma": 2, "int32_mad": 3, "int32_mulhi": 4, "cvt_f32_f64": 5,
+                  "rcp_f32": 6, "lds128": 7}
+
+    def debug_peak(self, pipe) -> float:
+        """Measured issue rate of one pipe in giga lane-instructions per second (md_debug_peak)."""
+        v = C.c_double()
+        self._chk(self.L.md_debug_peak(self.h, self.PEAK_PIPES.get(pipe, pipe), C.byref(v)), "md_debug_peak")
+        return v.value
 
     def debug_philox(self, ctr, key):
         ctr = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)

@@ -223,6 +223,18 @@ static uint64_t hilbert3(uint32_t x, uint32_t y, uint32_t z, int bits)
     return h;
 }
 
+// grid of the cell-relative fp32 records (Geom::q0): every staged coordinate of a tile -- at most (B/2 + 1) cell widths +
+// r_buff from the brick centre -- must be an exact float multiple of q0, i.e. stay below 2^24 q0
+static void set_record_grid(md_ctx *c, uint32_t B)
+{
+    double E = 0.0;
+    for (int a = 0; a < 3; ++a) E = std::max(E, (0.5 * B + 1.0) * c->g.cw[a] + c->r_buff + 1e-6);
+    c->g.q0 = ldexp(1.0, ilogb(E) + 1 - 24);
+    c->g.q0i = 1.0 / c->g.q0;
+    c->g.qr = c->g.q0 / 510.0;
+    c->g.qri = 510.0 / c->g.q0;
+}
+
 static uint32_t choose_brick(md_ctx *c)
 {
     if (c->tile_B_forced) return (uint32_t)c->tile_B_forced;
@@ -240,6 +252,7 @@ int build_cell_order(md_ctx *c)
         if (*p) { md_free(c, *p); *p = nullptr; }
     c->use_tiles = false;
     c->n_tiles = 0;
+    set_record_grid(c, c->order == MD_ORDER_MORTON ? choose_brick(c) : 1u);
     if (c->order == MD_ORDER_LEX) return MD_OK;
     const uint32_t nx = c->dims[0], ny = c->dims[1], nz = c->dims[2];
     int bits = 1;
@@ -349,6 +362,7 @@ extern "C" int md_create(md_ctx **out, const double box[3], uint64_t N, double r
     c->n_cells = (uint32_t)ncell;
     c->g.n_cells = c->n_cells;
     c->g.N = (uint32_t)N;
+    set_record_grid(c, 1);
     set_default_cfg(c);
 
     int s = MD_OK;
@@ -490,13 +504,27 @@ extern "C" int md_get_state(md_ctx *c, double *pos, double *vel, int32_t *image)
 
 static int eval_forces(md_ctx *c, const md_step_desc *w, uint64_t step, bool energy);
 
+// md_step evaluates LJ forces without the per-particle energies.  When they are asked for, the same evaluation is
+// repeated with the energy lane switched on INTO THE SCRATCH TWIN of the force array and only the energy lane is copied
+// over: the forces that the next half-kick uses stay those of the step's own kernel, whether or not energies were read.
+static int energies_on_demand(md_ctx *c)
+{
+    std::swap(c->force, c->force_alt);
+    const int s = eval_forces(c, &c->last_desc, c->last_force_step, true);
+    std::swap(c->force, c->force_alt);
+    MD_TRY(s);
+    MD_TRY(launch_copy_energy(c, c->force_alt));
+    c->energy_valid = true;
+    return MD_OK;
+}
+
 extern "C" int md_get_forces(md_ctx *c, double *force, double *energy)
 {
     if (!c) return MD_EINVAL;
     if (!c->force_valid) { c->err = "md_get_forces: no force has been computed for the current positions"; return MD_ESTATE; }
     // md_step evaluates LJ forces without the per-particle energies; the forces are a pure function of the current
     // state, so the same evaluation is repeated with the energy lane switched on when it is asked for
-    if (energy && !c->energy_valid && c->last_from_step) MD_TRY(eval_forces(c, &c->last_desc, c->last_force_step, true));
+    if (energy && !c->energy_valid && c->last_from_step) MD_TRY(energies_on_demand(c));
     const uint64_t b3 = 3 * c->N * sizeof(double), b1 = c->N * sizeof(double);
     Stage st(c);
     MD_TRY(st.reserve(stage_need(force, b3) + stage_need(energy, b1)));
@@ -595,7 +623,8 @@ static int build_nlist_tiles(md_ctx *c, bool *done)
         c->stride_mode = mode;
     }
     for (int attempt = 0; attempt < 3; ++attempt) {
-        if (!c->nl16) MD_TRY(md_alloc(c, (void **)&c->nl16, c->N * (uint64_t)c->nl_stride * sizeof(uint16_t)));
+        if (!c->nl16) MD_TRY(md_alloc(c, (void **)&c->nl16, (c->N + 1) * (uint64_t)c->nl_stride * sizeof(uint16_t)));  // + one row: the force kernels
+                                                                                      // request block `lane` of a row before they know its length
         bool fits = false;
         MD_TRY(launch_tile_build(c, mode == 1, &fits));
         if (!fits) return MD_OK;  // largest tile exceeds shared memory: general path
@@ -650,7 +679,9 @@ extern "C" int md_build_nlist(md_ctx *c)
 {
     if (!c) return MD_EINVAL;
     if (!c->have_state) { c->err = "md_build_nlist: md_set_state first"; return MD_ESTATE; }
-    if (!c->cells_valid) MD_TRY(do_build_cells(c));
+    // bins taken before an integration step are stale: the list kernels assume positions as binned (image shifts per
+    // cell, cell-relative records), so the binning is repeated whenever half 1 has run since
+    if (!c->cells_valid || c->steps_since_build > 0) MD_TRY(do_build_cells(c));
     return do_build_nlist(c);
 }
 
@@ -715,14 +746,15 @@ static int ensure_decoded(md_ctx *c);
 static int pair_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
 {
     // cluster rows are read by k_tile_lj4 only (forces, no energies); everything else goes through the decoded list
-    if (c->nl_is_tile && !(c->nl_cluster && (energy || c->precision != MD_MIXED)))
+    // a tile list whose largest tile fits the build kernel but not this force kernel's records goes through the decoded list
+    if (c->nl_is_tile && !(c->nl_cluster && (energy || c->precision != MD_MIXED)) && tile_forces_fit(c, false))
         return launch_tile_lj(c, eps, sigma, shift, energy);
     MD_TRY(ensure_decoded(c));
     return launch_forces_lj(c, eps, sigma, shift);
 }
 static int pair_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed)
 {
-    if (c->nl_is_tile && !c->nl_cluster) return launch_tile_dpd(c, A, gamma, kT, dt, step, seed);
+    if (c->nl_is_tile && !c->nl_cluster && tile_forces_fit(c, true)) return launch_tile_dpd(c, A, gamma, kT, dt, step, seed);
     MD_TRY(ensure_decoded(c));
     return launch_forces_dpd(c, A, gamma, kT, dt, step, seed);
 }
@@ -737,6 +769,7 @@ extern "C" int md_forces_lj(md_ctx *c, double eps, double sigma, int shift)
 {
     if (!c) return MD_EINVAL;
     MD_TRY(need_nlist(c, "md_forces_lj"));
+    c->lj_sigma_hint = sigma;
     ProfScope ps(c, MD_K_LJ);
     MD_TRY(pair_lj(c, eps, sigma, shift, true));
     c->force_valid = c->energy_valid = true;
@@ -863,6 +896,8 @@ static int eval_forces(md_ctx *c, const md_step_desc *w, uint64_t step, bool ene
     return MD_OK;
 }
 
+static int tune_all(md_ctx *c, const md_step_desc *w, int mode);
+
 static int rebuild(md_ctx *c)
 {
     MD_TRY(do_build_cells(c));
@@ -886,10 +921,16 @@ extern "C" int md_step(md_ctx *c, const md_step_desc *w, uint64_t n_steps)
     const bool nvt = (w->flags & MD_F_NVT) != 0;
     if (nvt && (!(w->nvt_kT > 0.0) || !(w->nvt_tau > 0.0))) { c->err = "md_step: nvt_kT and nvt_tau must be positive"; return MD_EINVAL; }
     c->force_hint = w->flags;
+    if (w->flags & MD_F_LJ) {
+        // the near sections of a mixed-precision tile list are sized for sigma (R25): a list built for a smaller one is rebuilt
+        if (c->nlist_valid && c->nl_is_tile && c->precision == MD_MIXED && c->nl_near_r < MD_NEAR_SIGMAS * w->lj_sigma * (1.0 - 1e-12) &&
+            c->steps_since_build == 0)
+            c->nlist_valid = false;
+        c->lj_sigma_hint = w->lj_sigma;
+    }
     if (!c->nlist_valid) MD_TRY(rebuild(c));
     if (!c->force_valid) MD_TRY(eval_forces(c, w, c->step, false));  // R16: F(t0) before the first half-kick
     if (!c->ev_flags) MD_CUDA_CHECK(c, cudaEventCreateWithFlags(&c->ev_flags, cudaEventDisableTiming));
-    const double thr2 = 0.25 * c->r_buff * c->r_buff;
     for (uint64_t s = 0; s < n_steps; ++s) {
         if (s == 0) {
             ProfScope ps(c, MD_K_INTEGRATE);
@@ -919,11 +960,12 @@ extern "C" int md_step(md_ctx *c, const md_step_desc *w, uint64_t n_steps)
             if (c->h_flags->dangerous) c->stats.dangerous_builds++;
             if (speculate) c->stats.wasted_forces++;
             MD_TRY(rebuild(c));
+            // periodic re-scan: density and temperature drift move the optimum
+            if (c->retune_period && c->stats.rebuilds - c->rebuilds_at_tune >= c->retune_period) MD_TRY(tune_all(c, w, 2));
             MD_TRY(eval_forces(c, w, c->step + 1, false));
         } else if (!speculate) {
             MD_TRY(eval_forces(c, w, c->step + 1, false));
         }
-        (void)thr2;
         {
             ProfScope ps(c, MD_K_INTEGRATE);
             if (s + 1 < n_steps) {
@@ -966,16 +1008,42 @@ static int time_median5(md_ctx *c, F &&fn, float *us)
     return MD_OK;
 }
 
+// largest block size the kernel behind MD_K_* can be launched with in the current configuration (the __launch_bounds__
+// of the variant the launcher picks): the tuner sweeps launchable sizes only and md_get_stats reports the launched one
+int md_block_limit(const md_ctx *c, int kernel)
+{
+    const bool tile = c->nlist_valid ? c->nl_is_tile : c->use_tiles;
+    switch (kernel) {
+    case MD_K_NLIST: return tile ? MD_TILE_MAX_BLOCK : 1024;
+    case MD_K_LJ: return !tile ? 1024 : (c->precision == MD_MIXED ? MD_LJ3_MAX_BLOCK : MD_TILE_MAX_BLOCK);
+    case MD_K_DPD: return tile ? MD_TILE_MAX_BLOCK : 1024;
+    case MD_K_INTEGRATE: return MD_HALF1_MAX_BLOCK;
+    default: return 1024;
+    }
+}
+
+// mode 0: pruned grid, 1: every multiple of 32, 2: local re-scan around the current setting (periodic re-tune)
 template <typename F>
-static int tune_kernel(md_ctx *c, int kernel, const char *name, bool sweep_w, int full, F &&fn)
+static int tune_kernel(md_ctx *c, int kernel, const char *name, bool sweep_w, int w_max, int mode, F &&fn)
 {
     static const int pruned[] = {32, 64, 96, 128, 192, 256, 384, 512, 768, 1024};
-    std::vector<int> blocks;
-    if (full) for (int b = 32; b <= 1024; b += 32) blocks.push_back(b);
-    else blocks.assign(pruned, pruned + sizeof(pruned) / sizeof(int));
-    LaunchCfg best = c->cfg[kernel];
+    const int n_pruned = (int)(sizeof(pruned) / sizeof(int));
+    const int limit = md_block_limit(c, kernel);
+    const LaunchCfg cur = c->cfg[kernel];
+    std::vector<int> blocks, ws;
+    if (mode == 1) { for (int b = 32; b <= limit; b += 32) blocks.push_back(b); }
+    else if (mode == 2) {
+        int at = 0;
+        for (int i = 0; i < n_pruned; ++i) if (pruned[i] <= std::min(cur.block, limit)) at = i;
+        for (int i = std::max(0, at - 1); i <= std::min(n_pruned - 1, at + 1); ++i) if (pruned[i] <= limit) blocks.push_back(pruned[i]);
+    } else { for (int i = 0; i < n_pruned; ++i) if (pruned[i] <= limit) blocks.push_back(pruned[i]); }
+    if (!sweep_w) ws.push_back(cur.w);
+    else if (mode == 2) { for (int w = std::max(1, cur.w / 2); w <= std::min(w_max, cur.w * 2); w *= 2) ws.push_back(w); }
+    else { for (int w = 1; w <= w_max; w *= 2) ws.push_back(w); }
+    LaunchCfg best = cur;
+    best.block = std::min(best.block, limit);
     best.us = 1e30f;
-    for (int w = 1; w <= (sweep_w ? 32 : 1); w *= 2)
+    for (int w : ws)
         for (int b : blocks) {
             c->cfg[kernel].block = b;
             c->cfg[kernel].w = w;
@@ -986,8 +1054,68 @@ static int tune_kernel(md_ctx *c, int kernel, const char *name, bool sweep_w, in
             if (c->log) fprintf(stderr, "[b200md tuner] %-10s block=%4d w=%2d  %9.1f us\n", name, b, w, us);
             if (us < best.us) best = LaunchCfg{b, w, us};
         }
+    if (best.us > 1e29f) best.us = 0.f;  // nothing launchable was timed: keep the setting
     c->cfg[kernel] = best;
     if (c->log) fprintf(stderr, "[b200md tuner] %-10s -> block=%d w=%d (%.1f us)\n", name, best.block, best.w, best.us);
+    return MD_OK;
+}
+
+static int tune_all(md_ctx *c, const md_step_desc *w, int mode)
+{
+    c->force_hint = w->flags;
+    if (w->flags & MD_F_LJ) c->lj_sigma_hint = w->lj_sigma;
+    const uint64_t rebuilds0 = c->stats.rebuilds + (c->nlist_valid ? 0 : 1);  // the replays are not rebuilds of the run
+    // the kernels are pure functions of the live state, so they can be replayed without advancing the simulation
+    // (every kernel is tuned).  Binning: only when no step has been taken since the last one (a replay
+    // re-takes the reference snapshot of the displacement check, which must not move in time).
+    if (c->cells_valid && c->steps_since_build == 0) {
+        MD_TRY(tune_kernel(c, MD_K_CELLS, "cells", false, 1, mode, [&]() { return launch_build_cells(c); }));
+        c->tile_desc_valid = false;
+        c->nlist_valid = false;
+        MD_CUDA_CHECK(c, cudaMemsetAsync(&c->d_flags->rebuild, 0, 2 * sizeof(int), c->stream));
+    }
+    if (!c->nlist_valid) MD_TRY(rebuild(c));
+    if (c->nl_is_tile) {
+        // tile build: the lanes per particle are fixed by the kernel (4 candidate phases, or a full warp with the ballot
+        // variant); only the block size is swept
+        MD_TRY(tune_kernel(c, MD_K_NLIST, "nlist/tile", false, 1, mode, [&]() {
+            bool fits = false;
+            const int st = launch_tile_build(c, c->nl_cluster, &fits);
+            if (!fits) c->tune_skip = true;  // this block size does not fit in shared memory
+            return st;
+        }));
+        c->cfg[MD_K_NLIST].w = tile_build_lanes(c);
+    } else {
+        MD_TRY(tune_kernel(c, MD_K_NLIST, "nlist", true, 32, mode, [&]() {
+            MD_TRY(launch_nlist_count(c));
+            return launch_nlist_fill(c);
+        }));
+    }
+    if (w->flags & MD_F_LJ)
+        MD_TRY(tune_kernel(c, MD_K_LJ, c->nl_is_tile ? "lj/tile" : "lj", true, c->nl_is_tile && c->precision == MD_MIXED ? 8 : 32, mode, [&]() {
+            // the row rotation of the tile list follows W (1, 2 or more lanes per particle): time each W on its own layout
+            if (c->nl_is_tile && !c->nl_cluster && c->nl_rotw != tile_rot_class(c->cfg[MD_K_LJ].w)) MD_TRY(do_build_nlist(c));
+            return pair_lj(c, w->lj_epsilon, w->lj_sigma, w->lj_energy_shift, false);
+        }));
+    if (w->flags & MD_F_DPD)
+        MD_TRY(tune_kernel(c, MD_K_DPD, c->nl_is_tile ? "dpd/tile" : "dpd", true, 32, mode, [&]() {
+            if (c->nl_is_tile && !c->nl_cluster && c->nl_rotw != tile_rot_class(c->cfg[MD_K_DPD].w)) MD_TRY(do_build_nlist(c));
+            return pair_dpd(c, w->dpd_A, w->dpd_gamma, w->dpd_kT, w->dt, c->step, w->dpd_seed);
+        }));
+    if ((w->flags & MD_F_BONDS) && c->n_bonds)
+        MD_TRY(tune_kernel(c, MD_K_BONDS, "bonds", false, 1, mode, [&]() { return launch_forces_bonds(c, w->bond_k, w->bond_r0); }));
+    // half 1 with dt = 0 is the identity on positions and velocities (x + 0 v, v + 0 F/m) with the full memory traffic
+    MD_TRY(tune_kernel(c, MD_K_INTEGRATE, "integrate", false, 1, mode, [&]() { return launch_half1(c, 0.0, false, false); }));
+    // the list the run starts with has the layout of the chosen W
+    if (c->nl_is_tile && !c->nl_cluster) {
+        const bool dpd = (w->flags & MD_F_DPD) != 0 && !(w->flags & MD_F_LJ);
+        if (c->nl_rotw != tile_rot_class(c->cfg[dpd ? MD_K_DPD : MD_K_LJ].w)) MD_TRY(do_build_nlist(c));
+    }
+    c->force_valid = false;  // the replays overwrote the force array with a partial evaluation
+    c->tuned = true;
+    c->stats.tuner_runs++;
+    c->stats.rebuilds = rebuilds0;
+    c->rebuilds_at_tune = c->stats.rebuilds;
     return MD_OK;
 }
 
@@ -995,44 +1123,8 @@ extern "C" int md_tune(md_ctx *c, const md_step_desc *w, int full)
 {
     if (!c || !w) return MD_EINVAL;
     if (!c->have_state) { c->err = "md_tune: md_set_state first"; return MD_ESTATE; }
-    c->force_hint = w->flags;
-    if (!c->nlist_valid) MD_TRY(rebuild(c));
-    // the kernels are pure functions of the live state, so they can be replayed without advancing the simulation
-    if (c->nl_is_tile) {
-        // tile build: w is fixed at 32 (one ballot word per 32 candidates); only the block size is swept
-        MD_TRY(tune_kernel(c, MD_K_NLIST, "nlist/tile", false, full, [&]() {
-            bool fits = false;
-            const int st = launch_tile_build(c, c->nl_cluster, &fits);
-            if (!fits) c->tune_skip = true;  // this block size does not fit in shared memory
-            return st;
-        }));
-        c->cfg[MD_K_NLIST].w = 32;
-    } else {
-        MD_TRY(tune_kernel(c, MD_K_NLIST, "nlist", true, full, [&]() {
-            MD_TRY(launch_nlist_count(c));
-            return launch_nlist_fill(c);
-        }));
-    }
-    if (w->flags & MD_F_LJ)
-        MD_TRY(tune_kernel(c, MD_K_LJ, c->nl_is_tile ? "lj/tile" : "lj", true, full, [&]() {
-            // the row rotation of the tile list follows W (1, 2 or more lanes per particle): time each W on its own layout
-            if (c->nl_is_tile && !c->nl_cluster && c->nl_rotw != tile_rot_class(c->cfg[MD_K_LJ].w)) MD_TRY(do_build_nlist(c));
-            return pair_lj(c, w->lj_epsilon, w->lj_sigma, w->lj_energy_shift, false);
-        }));
-    if (w->flags & MD_F_DPD)
-        MD_TRY(tune_kernel(c, MD_K_DPD, c->nl_is_tile ? "dpd/tile" : "dpd", true, full, [&]() {
-            if (c->nl_is_tile && !c->nl_cluster && c->nl_rotw != tile_rot_class(c->cfg[MD_K_DPD].w)) MD_TRY(do_build_nlist(c));
-            return pair_dpd(c, w->dpd_A, w->dpd_gamma, w->dpd_kT, w->dt, c->step, w->dpd_seed);
-        }));
-    // the list the run starts with has the layout of the chosen W
-    if (c->nl_is_tile && !c->nl_cluster) {
-        const bool dpd = (w->flags & MD_F_DPD) != 0 && !(w->flags & MD_F_LJ);
-        if (c->nl_rotw != tile_rot_class(c->cfg[dpd ? MD_K_DPD : MD_K_LJ].w)) MD_TRY(do_build_nlist(c));
-    }
-    c->force_valid = false;  // the replays overwrote the force array with a partial evaluation (pair term only)
-    c->tuned = true;
-    c->stats.tuner_runs++;
-    return MD_OK;
+    if (!c->cells_valid) MD_TRY(do_build_cells(c));
+    return tune_all(c, w, full ? 1 : 0);
 }
 
 extern "C" int md_set_option(md_ctx *c, int option, int64_t value)
@@ -1054,6 +1146,10 @@ extern "C" int md_set_option(md_ctx *c, int option, int64_t value)
     case MD_OPT_ACC_BLOCK:
         if (value != 1 && value != 8) { c->err = "md_set_option: accumulation block must be 1 or 8"; return MD_EINVAL; }
         c->acc_block = (int)value;
+        return MD_OK;
+    case MD_OPT_RETUNE_PERIOD:
+        if (value < 0) { c->err = "md_set_option: re-tune period must be >= 0"; return MD_EINVAL; }
+        c->retune_period = (uint64_t)value;
         return MD_OK;
     default:
         c->err = "md_set_option: unknown option";
@@ -1090,7 +1186,7 @@ extern "C" int md_get_stats(md_ctx *c, md_stats *out)
     }
     for (int a = 0; a < 3; ++a) c->stats.dims[a] = c->dims[a];
     for (int k = 0; k < MD_N_KERNELS; ++k) {
-        c->stats.block[k] = c->cfg[k].block;
+        c->stats.block[k] = std::min(c->cfg[k].block, md_block_limit(c, k));  // the launched size
         c->stats.w[k] = c->cfg[k].w;
         c->stats.tuned_us[k] = c->cfg[k].us;
     }
@@ -1103,7 +1199,7 @@ extern "C" int md_thermo(md_ctx *c, md_thermo_t *out)
     if (!c || !out) return MD_EINVAL;
     if (!c->have_state) { c->err = "md_thermo: md_set_state first"; return MD_ESTATE; }
     if (!c->force_valid) { c->err = "md_thermo: no force has been computed for the current positions"; return MD_ESTATE; }
-    if (!c->energy_valid && c->last_from_step) MD_TRY(eval_forces(c, &c->last_desc, c->last_force_step, true));
+    if (!c->energy_valid && c->last_from_step) MD_TRY(energies_on_demand(c));
     double r[5];
     MD_TRY(launch_thermo(c, r));
     out->kinetic = r[0];

@@ -350,11 +350,12 @@ int launch_build_cells(md_ctx *c)
     MD_CUDA_CHECK(c, cudaMemsetAsync(&c->d_flags->max_cell_count, 0, sizeof(unsigned int), st));
     // cell_lin_old lives in perm_sorted's sibling scratch: use tag_alt as temporary for old linear ids
     uint32_t *cell_lin_old = c->tag_alt;
-    k_cell_id<<<md_grid(N, 256), 256, 0, st>>>(c->pos, c->g, c->rank_of_lin, cell_lin_old, c->cell_rank_tmp, c->cell_count);
+    const int blk = c->cfg[MD_K_CELLS].block;  // the streaming kernels of the binning follow the tuner
+    k_cell_id<<<md_grid(N, blk), blk, 0, st>>>(c->pos, c->g, c->rank_of_lin, cell_lin_old, c->cell_rank_tmp, c->cell_count);
     MD_LAUNCH_CHECK(c);
     MD_TRY(launch_exclusive_scan_u32(c, c->cell_count, c->n_cells, c->cell_start, nullptr, false, nullptr));
     MD_CUDA_CHECK(c, cudaMemsetAsync(c->cell_count, 0, sizeof(uint32_t) * c->n_cells, st));
-    k_cell_scatter<<<md_grid(N, 256), 256, 0, st>>>(c->cell_rank_tmp, N, c->cell_start, c->cell_count, c->perm);
+    k_cell_scatter<<<md_grid(N, blk), blk, 0, st>>>(c->cell_rank_tmp, N, c->cell_start, c->cell_count, c->perm);
     MD_LAUNCH_CHECK(c);
     k_cell_sort<<<md_grid((uint64_t)c->n_cells * 32, 256), 256, 0, st>>>(c->perm, c->cell_start, c->tag, c->pos, c->g,
                                                                        c->use_tiles, c->n_cells, c->perm_sorted,
@@ -362,7 +363,7 @@ int launch_build_cells(md_ctx *c)
     MD_LAUNCH_CHECK(c);
     // new tags go to cell_rank_tmp (free now), then pointers are swapped
     uint32_t *ntag = c->cell_rank_tmp;
-    k_reorder<<<md_grid(N, 256), 256, 0, st>>>(c->perm_sorted, N, c->pos, c->vel, c->force, c->image, c->tag,
+    k_reorder<<<md_grid(N, blk), blk, 0, st>>>(c->perm_sorted, N, c->pos, c->vel, c->force, c->image, c->tag,
                                                cell_lin_old, c->pos_alt, c->vel_alt, c->force_alt, c->image_alt, ntag,
                                                c->rtag, c->cell_lin, c->pos_ref, c->g, c->rel);
     MD_LAUNCH_CHECK(c);

@@ -208,6 +208,20 @@ int launch_forces_bonds(md_ctx *c, double k, double r0)
     return MD_OK;
 }
 
+// energies on demand (md_get_forces / md_thermo after md_step): only the energy lane of a re-evaluation is kept
+__global__ void k_copy_energy(double4 *__restrict__ force, const double4 *__restrict__ src, uint32_t N)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) force[i].w = src[i].w;
+}
+
+int launch_copy_energy(md_ctx *c, const double4 *src)
+{
+    k_copy_energy<<<md_grid(c->N, 256), 256, 0, c->stream>>>(c->force, src, (uint32_t)c->N);
+    MD_LAUNCH_CHECK(c);
+    return MD_OK;
+}
+
 // ------------------------------------------------------------------------------------------------------------
 // test hook: the device hash, as the DPD kernel calls it
 // ------------------------------------------------------------------------------------------------------------

@@ -11,7 +11,7 @@
 // NVT (R30): v <- (v + kick) / (1 + (dt/2) xi) in half 1, v <- v + (dt/2)(F/m - xi v) in half 2, xi read from
 // nvt[0]; the fused launch applies half 2 and the next half 1 with the same xi (the one the thermostat update left).
 template <bool FUSED, bool NVT>
-__global__ void __launch_bounds__(256, 6) k_half1(double4 *__restrict__ pos, double4 *__restrict__ vel, const double4 *__restrict__ force,
+__global__ void __launch_bounds__(MD_HALF1_MAX_BLOCK, 6) k_half1(double4 *__restrict__ pos, double4 *__restrict__ vel, const double4 *__restrict__ force,
                         int *__restrict__ image, const double *__restrict__ pos_ref,
                         const uint32_t *__restrict__ cell_lin, float4 *__restrict__ rel, Geom g, double dt,
                         double half_dt, double thr2, double danger2, DevFlags *flags, int slot,
@@ -92,7 +92,7 @@ __global__ void k_half2(double4 *__restrict__ vel, const double4 *__restrict__ f
 int launch_half1(md_ctx *c, double dt, bool fused, bool nvt)
 {
     LaunchCfg cf = c->cfg[MD_K_INTEGRATE];
-    cf.block = std::min(cf.block, 256);  // k_half1 is compiled for 6 blocks of 256 threads per SM (latency bound: occupancy)
+    cf.block = std::min(cf.block, MD_HALF1_MAX_BLOCK);  // k_half1 is compiled for 6 blocks of 256 threads per SM (latency bound: occupancy)
     const double t = 0.5 * c->r_buff;
     c->d2_slot ^= 1;
     const unsigned grid = md_grid(c->N, cf.block);

@@ -34,8 +34,40 @@ __device__ __forceinline__ uint32_t md_cell_coord(double x, double lo, double L,
 // mixed-precision force error over all 2^20 particles from 4.4e-4 to 3.2e-4 (R11 norm) -- neither reaches 1e-4 there.
 constexpr bool MD_STAGE_FROM_REL = true;
 
+// Three signed 10-bit integers in one word: residuals of fp32 coordinates in units of a quantum, clamped to +-511 and
+// stored biased by 512.  Conversions between integers and doubles go through the 2^52 trick (an integer n in the low
+// word of a double with exponent 2^52 IS the double 2^52 + n): the conversion unit runs at 1/8 of the FP32 rate on B200
+// (md_debug_peak) and was the bottleneck of the mixed-precision force kernel when these used cvt instructions.
+#define MD_TWO52 4503599627370496.0
+__device__ __forceinline__ double md_small_int_to_double(int n)  // |n| < 2^31
+{
+    return __hiloint2double(0x43300000, (int)((unsigned)n ^ 0x80000000u)) - (MD_TWO52 + 2147483648.0);
+}
+__device__ __forceinline__ int md_round_to_int(double x)  // |x| < 2^31, round to nearest even
+{
+    return __double2loint(x + (MD_TWO52 + 2147483648.0)) ^ (int)0x80000000;
+}
+// fields of a packed residual word: 10 bits each, value + 255 (value in [-255, 255]); the sum of two such words is a
+// word of fields value_a + value_b + 510 in [0, 1020] (no carry between fields), and differences of equally biased
+// fields need no un-biasing
+__device__ __forceinline__ int md_res_x(uint32_t w) { return (int)(w & 0x3ffu); }
+__device__ __forceinline__ int md_res_y(uint32_t w) { return (int)((w >> 10) & 0x3ffu); }
+__device__ __forceinline__ int md_res_z(uint32_t w) { return (int)((w >> 20) & 0x3ffu); }
+
+// one coordinate on the grid: n q0 as a float (exact: |n| < 2^24) and the residual (v - n q0) / qr in [-255, 255] + 255
+__device__ __forceinline__ float md_grid_coord(double v, double q0, double q0i, double qri, uint32_t &field)
+{
+    const double n = (double)md_round_to_int(v * q0i);
+    const double vq = n * q0;
+    field = (uint32_t)(max(-255, min(255, md_round_to_int((v - vq) * qri))) + 255);
+    return (float)vq;
+}
+
 // fp32 record of a position relative to the centre of cell `lin` (linear id), minimum image applied: what the fp32
-// tile kernels stage.  |result| <= half a cell width + the drift since the binning, so the rounding is ~1e-7 absolute.
+// tile kernels stage.  x, y, z are rounded to the grid q0 (a multiple of q0 below 2^24 q0 is an exact float, and so is
+// its sum with a cell offset on the same grid: the tile kernels stage WITHOUT a rounding); what the grid drops is kept in
+// .w as three 10-bit residuals in units of qr = q0 / 510, so that the mixed-precision force kernel can rebuild
+// separations to ~1e-9 for the pairs of the first shell (R25).
 __device__ __forceinline__ float4 md_rel_record(double x, double y, double z, uint32_t lin, const Geom &g)
 {
     const uint32_t nxy = g.n[0] * g.n[1];
@@ -44,7 +76,11 @@ __device__ __forceinline__ float4 md_rel_record(double x, double y, double z, ui
     const double rx = md_min_image(x - (g.lo[0] + ((double)cx + 0.5) * g.cw[0]), g.L[0], g.h[0]);
     const double ry = md_min_image(y - (g.lo[1] + ((double)cy + 0.5) * g.cw[1]), g.L[1], g.h[1]);
     const double rz = md_min_image(z - (g.lo[2] + ((double)cz + 0.5) * g.cw[2]), g.L[2], g.h[2]);
-    return make_float4((float)rx, (float)ry, (float)rz, 0.f);
+    uint32_t fx, fy, fz;
+    const float vx = md_grid_coord(rx, g.q0, g.q0i, g.qri, fx);
+    const float vy = md_grid_coord(ry, g.q0, g.q0i, g.qri, fy);
+    const float vz = md_grid_coord(rz, g.q0, g.q0i, g.qri, fz);
+    return make_float4(vx, vy, vz, __uint_as_float(fx | (fy << 10) | (fz << 20)));
 }
 
 // fast reciprocal: fp32 = MUFU.RCP (about 1 ulp), fp64 = IEEE division

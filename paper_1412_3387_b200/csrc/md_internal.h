@@ -20,6 +20,18 @@
         }                                                                                          \
     } while (0)
 
+// compiled block-size limits (__launch_bounds__) of the kernel families; the tuner sweeps launchable sizes only
+#define MD_TILE_MAX_BLOCK 512   // tile kernels (up to 128 registers per thread)
+#define MD_LJ3_MAX_BLOCK 256    // k_tile_lj3: 4 CTAs of 256 threads per SM at 64 registers
+#define MD_HALF1_MAX_BLOCK 256  // k_half1: 6 CTAs of 256 threads per SM
+
+// nl_cnt word of a tile row: entries in the low 24 bits, blocks of the near section (the LAST K blocks of the row,
+// evaluated in fp64 by the mixed-precision force kernel; R25) in the high 8
+// pairs closer than MD_NEAR_SIGMAS sigma are evaluated in fp64 in MD_MIXED mode (first neighbour shell of a liquid)
+#define MD_NEAR_SIGMAS 1.5
+#define MD_NL_NEAR_SHIFT 24
+#define MD_NL_CNT_MASK 0xffffffu
+
 #define MD_TRY(expr)                  \
     do {                              \
         int _s = (expr);              \
@@ -33,6 +45,9 @@ struct Geom {
     double lo[3];    // -L/2
     double dn[3];    // (double) cells per axis
     double cw[3];    // cell widths L/n
+    double q0, q0i;  // grid of the cell-relative fp32 records (md_rel_record): multiples of q0 = 2^-24 x the binade above
+                     // the staged extent, so that record + cell offset is an EXACT fp32 sum in the tile kernels
+    double qr, qri;  // quantum of the residuals carried in rel.w: q0 / 510
     uint32_t n[3];   // cells per axis
     uint32_t n_cells;
     uint32_t N;
@@ -100,6 +115,8 @@ struct md_ctx {
     bool use_tiles = false;     // configured (MD_ORDER_MORTON)
     bool nl_is_tile = false;    // the current list is a tile list
     bool nl32_decoded = false;  // nl_off/nl_idx hold the decoded copy of the current tile list (exports)
+    double nl_near_r = 0.0;     // force-time radius the near sections of the current tile list cover (0: none)
+    double lj_sigma_hint = 1.0; // sigma of the latest LJ call / step description: sizes the near section at the build
     int nl_rotw = 4;            // lanes per particle (1, 2 or 4 = "4 or more") the rows of the current tile list are rotated for
 
     bool nl_cluster = false;    // the current tile list has one row per cluster of 4 particles (k_tile_build_c)
@@ -149,6 +166,8 @@ struct md_ctx {
     md_stats stats;
     LaunchCfg cfg[MD_N_KERNELS];
     bool tuned = false;
+    uint64_t rebuilds_at_tune = 0;   // stats.rebuilds when the tuner last ran
+    uint64_t retune_period = 0;      // MD_OPT_RETUNE_PERIOD: local re-scan after this many rebuilds inside md_step (0 = off)
     bool tune_skip = false;  // set by a tuner replay that could not launch its configuration
     uint64_t device_bytes = 0;
     std::vector<std::pair<void *, uint64_t>> allocs;
@@ -184,6 +203,8 @@ int launch_exclusive_scan_u32(md_ctx *c, const uint32_t *in, uint64_t n, uint32_
 int launch_pack_state(md_ctx *c, const double *pos, const double *vel, const double *mass);
 int launch_unpack_state(md_ctx *c, double *pos, double *vel, int32_t *image);
 int launch_unpack_forces(md_ctx *c, double *force, double *energy);
+int launch_copy_energy(md_ctx *c, const double4 *src);  // force[i].w = src[i].w
+int md_block_limit(const md_ctx *c, int kernel);      // largest block size the kernel behind MD_K_* can be launched with
 int launch_unpack_cells(md_ctx *c, uint32_t *cell_of);
 int launch_build_cells(md_ctx *c);
 int launch_nlist_count(md_ctx *c);
@@ -207,6 +228,7 @@ int build_cell_order(md_ctx *c);  // host: rank_of_lin table for the configured 
 int tile_measure(md_ctx *c);
 int launch_tile_build(md_ctx *c, bool cluster, bool *fits);
 bool tile_cluster_ok(md_ctx *c);
+int tile_build_lanes(md_ctx *c);  // lanes that cooperate on one particle in the tile build kernel in use
 static inline int tile_rot_class(int w) { return w <= 1 ? 1 : (w == 2 ? 2 : 4); }
 int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy);
 int launch_tile_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed);

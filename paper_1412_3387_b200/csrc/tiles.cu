@@ -31,7 +31,7 @@
 
 #include "md_device.cuh"
 
-constexpr int TILE_MAX_BLOCK = 512;  // __launch_bounds__ of the tile kernels (up to 128 registers per thread)
+constexpr int TILE_MAX_BLOCK = MD_TILE_MAX_BLOCK;  // __launch_bounds__ of the tile kernels (up to 128 registers per thread)
 constexpr int BUILD_P = 4;           // home particles per warp task in the build kernel
 constexpr uint32_t N_DUMMY = 8;      // far-away dummy records after the staged ones, one per bank class (row padding)
 constexpr uint32_t RB_EXTRA = 96;    // build kernel: row assembly buffers hold this many entries more than a stored row
@@ -106,6 +106,17 @@ __device__ __forceinline__ TileSmem tile_carve(char *smem, uint32_t B)
     return t;
 }
 
+// offset of a staged cell (centre of its image relative to the brick centre, cg[3..5]) on the grid q0 of the cell-relative
+// records, with what the grid drops as residual fields in .w (see md_rel_record): record + offset is an exact fp32 sum
+__device__ __forceinline__ float4 tile_grid_offset(const double *cg, const Geom &g)
+{
+    uint32_t fx, fy, fz;
+    const float ox = md_grid_coord(cg[3], g.q0, g.q0i, g.qri, fx);
+    const float oy = md_grid_coord(cg[4], g.q0, g.q0i, g.qri, fy);
+    const float oz = md_grid_coord(cg[5], g.q0, g.q0i, g.qri, fz);
+    return make_float4(ox, oy, oz, __uint_as_float(fx | (fy << 10) | (fz << 20)));
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void tile_setup(const TileParams &tp, const Geom &g, uint32_t t, const TileSmem &h, TileCtx &tc)
 {
@@ -130,7 +141,7 @@ __device__ __forceinline__ void tile_setup(const TileParams &tp, const Geom &g, 
             cg[3] = ((double)ix - 0.5 - 0.5 * (double)tc.ex) * tp.cw[0];
             cg[4] = ((double)iy - 0.5 - 0.5 * (double)tc.ey) * tp.cw[1];
             cg[5] = ((double)iz - 0.5 - 0.5 * (double)tc.ez) * tp.cw[2];
-            h.coff[sc] = make_float4((float)cg[3], (float)cg[4], (float)cg[5], 0.f);
+            h.coff[sc] = tile_grid_offset(cg, g);
         }
         __syncthreads();
         return;
@@ -165,7 +176,7 @@ __device__ __forceinline__ void tile_setup(const TileParams &tp, const Geom &g, 
         cg[3] = ((double)ix - 0.5 - 0.5 * (double)tc.ex) * tp.cw[0];
         cg[4] = ((double)iy - 0.5 - 0.5 * (double)tc.ey) * tp.cw[1];
         cg[5] = ((double)iz - 0.5 - 0.5 * (double)tc.ez) * tp.cw[2];
-        h.coff[sc] = make_float4((float)cg[3], (float)cg[4], (float)cg[5], 0.f);
+        h.coff[sc] = tile_grid_offset(cg, g);
     }
     // home cells (consecutive ranks): their staged-cell index and first tile-local particle
     for (uint32_t hc = threadIdx.x; hc <= tc.n_hc; hc += blockDim.x) {
@@ -341,6 +352,46 @@ __device__ __forceinline__ void tile_stage_rel(const TileCtx &tc, const TileSmem
                 const float4 o = h.coff[scs[u]];
                 const float x = (r[u].x + o.x) * scale, y = (r[u].y + o.y) * scale, z = (r[u].z + o.z) * scale;
                 rec[s] = make_float4(x, y, z, WITH_R2 ? x * x + y * y + z * z : 0.f);
+            }
+        }
+    }
+    if (threadIdx.x < N_DUMMY) rec[tc.n_staged + threadIdx.x] = RecTraits<float4>::far();
+}
+
+// k_tile_lj3's staging.  The cell-relative records lie on the grid q0 (md_rel_record) and so do the cell offsets
+// (tile_grid_offset: the offset of every staged cell rounded to the grid; what that drops joins the residuals), hence
+//     staged coordinate = record + offset     is an EXACT fp32 sum (every staged coordinate is below 2^24 q0),
+//     staged residual   = record residual + offset residual   (one integer add on the packed 10-bit fields),
+// and coordinate + qr * residual is the true brick-relative coordinate to ~ qr = q0 / 510 (~1e-9 at config 2).  The far
+// loop reads x, y, z; the near section rebuilds separations from both in fp64 without leaving shared memory (R25).
+// 16 bytes per staged particle from L2 and 6 instructions per record, no fp64 and no conversion.
+__device__ __forceinline__ void tile_stage_exact(const TileCtx &tc, const TileSmem &h, const float4 *__restrict__ rel,
+                                                 float4 *rec, uint8_t *scell, const Geom &g)
+{
+    const uint32_t lane = threadIdx.x & 31u, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (uint32_t sc = wid; sc < tc.n_sc; sc += nw) {
+        const uint32_t b = h.sstart[sc], e = h.sstart[sc + 1];
+        for (uint32_t s = b + lane; s < e; s += 32) scell[s] = (uint8_t)sc;
+    }
+    __syncthreads();
+    for (uint32_t s0 = threadIdx.x; s0 < tc.n_staged; s0 += 4 * blockDim.x) {
+        float4 r[4];
+        uint32_t scs[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const uint32_t s = s0 + u * blockDim.x;
+            if (s < tc.n_staged) {
+                scs[u] = scell[s];
+                r[u] = __ldg(rel + h.gstart[scs[u]] + (s - h.sstart[scs[u]]));
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const uint32_t s = s0 + u * blockDim.x;
+            if (s < tc.n_staged) {
+                const float4 o = h.coff[scs[u]];
+                rec[s] = make_float4(r[u].x + o.x, r[u].y + o.y, r[u].z + o.z,
+                                     __uint_as_float(__float_as_uint(r[u].w) + __float_as_uint(o.w)));
             }
         }
     }
@@ -592,6 +643,84 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build(TileParams tp, Ge
 // with the prefix sum replaced by per-lane counters: no ballot, no popc, no atomics, no
 // communication between lanes until the row is finished (holes, copy-out: as in k_tile_build, 4 rows at a time).
 // ===============================================================================================================
+// Near section of a row assembled in shared memory (k_tile_build8, MD_MIXED; R25): every neighbour closer than
+// r_near + r_buff now -- i.e. every pair that can come within r_near before the next rebuild -- is moved into the LAST
+// K = ceil(n_near / 8) blocks of the row, which the mixed-precision force kernel evaluates in fp64.  Called by the 8 lanes
+// of a row together (lane = class): the lane owns the column of its class, slot (cls - b - rot) & 7 of every block b.  A
+// near entry above the section first changes places with a far entry (or dummy) of the SAME column inside the section,
+// so the bank-class layout of the far blocks survives; what is left over (columns with more than K near entries) goes
+// to the free section slots of other columns (the near section is read entry by entry: its layout is free).
+// M: one bit per block (uint32_t for rows of up to 32 blocks, else 64; longer rows get no near section).  Returns K.
+template <typename M>
+__device__ __forceinline__ uint32_t near_partition(uint16_t *r, const float4 *rec, const float4 mh, float thr_near,
+                                                   uint32_t nblk, uint32_t cls, uint32_t rrot, uint32_t sh, uint16_t *hp)
+{
+    constexpr uint32_t BITS = 8u * (uint32_t)sizeof(M);
+    const M one = (M)1;
+    const float nax = -2.f * mh.x, nay = -2.f * mh.y, naz = -2.f * mh.z, nth = thr_near - mh.w;
+    const uint32_t nb = nblk <= BITS ? nblk : 0u;
+    M nearbits = 0;
+#pragma unroll 2
+    for (uint32_t b = 0; b < nb; ++b) {
+        const uint32_t s = (uint32_t)r[8u * b + ((cls - b - rrot) & 7u)] >> sh;
+        const float4 pc = rec[s];
+        const float t = fmaf(naz, pc.z, fmaf(nay, pc.y, fmaf(nax, pc.x, pc.w)));
+        nearbits |= (M)(t < nth ? 1u : 0u) << b;
+    }
+    uint32_t n_near = sizeof(M) == 8 ? (uint32_t)__popcll((unsigned long long)nearbits) : (uint32_t)__popc((uint32_t)nearbits);
+#pragma unroll
+    for (int o = 1; o < 8; o <<= 1) n_near += __shfl_xor_sync(0xffffffffu, n_near, o);
+    const uint32_t K = min((n_near + 7u) >> 3, nb);
+    const uint32_t b0 = nb - K;  // first block of the near section
+    const M all = nb >= BITS ? ~(M)0 : (one << nb) - one;
+    const M sect = all & ~(b0 >= BITS ? ~(M)0 : (one << b0) - one);
+    M hole = ~nearbits & sect;        // section slots of my column that hold no near entry
+    M over = nearbits & ~sect & all;  // near entries of my column outside the section
+    auto low = [](M m) -> uint32_t {
+        return sizeof(M) == 8 ? (uint32_t)__ffsll((long long)m) - 1u : (uint32_t)__ffs((int)m) - 1u;
+    };
+    auto cnt = [](M m) -> uint32_t {
+        return sizeof(M) == 8 ? (uint32_t)__popcll((unsigned long long)m) : (uint32_t)__popc((uint32_t)m);
+    };
+    while (hole && over) {
+        const uint32_t i = low(hole), j = low(over);
+        uint16_t *pa = r + 8u * i + ((cls - i - rrot) & 7u), *pb = r + 8u * j + ((cls - j - rrot) & 7u);
+        const uint16_t t = *pa; *pa = *pb; *pb = t;
+        hole &= hole - one;
+        over &= over - one;
+    }
+    // left-overs across the 8 columns of the row: the o-th stranded near entry takes the o-th free section slot
+    const uint32_t nh = cnt(hole), no = cnt(over);
+    uint32_t hsum = nh, osum = no;
+#pragma unroll
+    for (int o = 1; o < 8; o <<= 1) {
+        const uint32_t a = __shfl_up_sync(0xffffffffu, hsum, o, 8), bb = __shfl_up_sync(0xffffffffu, osum, o, 8);
+        if ((int)cls >= o) { hsum += a; osum += bb; }
+    }
+    const uint32_t n_over = __shfl_sync(0xffffffffu, osum, 7, 8);
+    if (__any_sync(0xffffffffu, n_over != 0u)) {
+        __syncwarp();
+        {
+            uint32_t o = hsum - nh;
+            for (M m = hole; m && o < 48u && o < n_over; m &= m - one, ++o) {
+                const uint32_t i = low(m);
+                hp[o] = (uint16_t)(8u * i + ((cls - i - rrot) & 7u));
+            }
+        }
+        __syncwarp();
+        {
+            uint32_t o = osum - no;
+            for (M m = over; m && o < 48u; m &= m - one, ++o) {
+                const uint32_t j = low(m);
+                uint16_t *pa = r + hp[o], *pb = r + 8u * j + ((cls - j - rrot) & 7u);
+                const uint16_t t = *pa; *pa = *pb; *pb = t;
+            }
+        }
+    }
+    __syncwarp();
+    return K;
+}
+
 constexpr int BUILD8_P = 8;
 
 // one x-run of 3 stencil cells [b, e) for one lane: candidates b' + ph, b' + ph + 4, ... (b' = b rounded down to 8).
@@ -637,6 +766,7 @@ __device__ __forceinline__ void b8_run(const float4 *rec, uint32_t b, uint32_t e
 
 __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build8(TileParams tp, Geom g, const float4 *__restrict__ rel, const double4 *__restrict__ pos,
                                                                 float thr_out /* r_list^2 + guard */,
+                                                                float thr_near /* (r_near + r_buff)^2 + guard, or 0: no near section */,
                                                                 uint32_t max_staged, uint32_t *__restrict__ nl_cnt,
                                                                 uint16_t *__restrict__ nl16, DevFlags *flags)
 {
@@ -769,6 +899,20 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build8(TileParams tp, G
                 r[8u * bk + ((c - bk - rrot) & 7u)] = v;
             }
             __syncwarp();
+            // ---- near section (MD_MIXED, R25): every neighbour closer than r_near + r_buff now -- i.e. every
+            // pair that can come within r_near before the next rebuild -- is moved into the LAST K = ceil(n_near / 8)
+            // blocks of the row, which the mixed-precision force kernel evaluates in fp64 on the global positions.  The
+            // lane owns the column of its class: slot (cls - b - rot) & 7 of every block b.  A near entry above the
+            // section first changes places with a far entry (or dummy) of the SAME column inside the section, so the
+            // bank-class layout of the far blocks survives; what is left over (columns with more than K near entries)
+            // goes to the free slots of other columns (the near section is read entry by entry, its layout is free).
+            uint32_t K = 0;
+            if (thr_near > 0.f) {
+                const float4 mh = rec[self0 + min(qr, np - 1)];
+                uint16_t *hp = (uint16_t *)(scr + 24 * (lane >> 3));  // 48 slot positions per row in flight
+                K = stride <= 256u ? near_partition<uint32_t>(r, rec, mh, thr_near, nblk, cls, rrot, sh, hp)
+                                   : near_partition<unsigned long long>(r, rec, mh, thr_near, nblk, cls, rrot, sh, hp);
+            }
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const uint32_t nb = __shfl_sync(0xffffffffu, nblk, 8 * q);
@@ -779,7 +923,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build8(TileParams tp, G
                 }
             }
             if (live && cls == 0) {
-                nl_cnt[tc.g0 + p0 + qr] = min(n, 8u * nblk);
+                nl_cnt[tc.g0 + p0 + qr] = min(n, 8u * nblk) | (K << MD_NL_NEAR_SHIFT);
                 total += n;
             }
             __syncwarp();
@@ -957,7 +1101,27 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build_c(TileParams tp, 
 struct LJTile {
     double rc2_exact, sig2, eps24, eps4, uc;
     double thr_in, thr_out;  // rc^2 -+ guard
+    double near2;            // MD_MIXED: pairs with r^2 below this are evaluated in fp64 on the global positions (R25)
 };
+
+// one pair by the plain fp64 definition on the global positions (MD_MIXED, pairs of the first shell: DESIGN.md R25)
+__device__ __noinline__ void lj_near_pair(const double4 *__restrict__ pos, double Lx, double Ly, double Lz, uint32_t gi,
+                                          uint32_t gj, double rc2_exact, double sig2, double eps24, double eps4, double uc,
+                                          double *acc /* fx, fy, fz, energy: accumulated */)
+{
+    const double4 a = pos[gi], b = pos[gj];
+    const double dx = md_min_image(__dsub_rn(a.x, b.x), Lx, 0.5 * Lx);
+    const double dy = md_min_image(__dsub_rn(a.y, b.y), Ly, 0.5 * Ly);
+    const double dz = md_min_image(__dsub_rn(a.z, b.z), Lz, 0.5 * Lz);
+    const double r2 = md_r2_exact(dx, dy, dz);
+    if (r2 < rc2_exact) {
+        const double rinv2 = 1.0 / r2;
+        const double s2 = sig2 * rinv2, s6 = s2 * s2 * s2;
+        const double f = eps24 * s6 * (2.0 * s6 - 1.0) * rinv2;
+        acc[0] += f * dx; acc[1] += f * dy; acc[2] += f * dz;
+        acc[3] += 0.5 * (eps4 * s6 * (s6 - 1.0) - uc);
+    }
+}
 
 // record referenced by a list entry: PRE = the entry is (staged index << 4), i.e. the byte offset of a float4 record
 template <typename R4, bool PRE>
@@ -997,7 +1161,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj(TileParams tp, Geom 
     for (uint32_t p = threadIdx.x / W; p < tc.n_home; p += n_groups) {
         const uint32_t hc = tile_home_cell(h, tc.n_hc, p);
         const R4 me = rec[tile_staged_of_home(h, hc, p)];
-        const uint32_t cnt = nl_cnt[tc.g0 + p];
+        const uint32_t cnt = nl_cnt[tc.g0 + p] & MD_NL_CNT_MASK;
         const uint32_t nblk = (cnt + 7u) >> 3;
         const uint4 *row = (const uint4 *)nl16 + (size_t)(tc.g0 + p) * stride8;
         double fx = 0.0, fy = 0.0, fz = 0.0, en = 0.0;
@@ -1016,6 +1180,14 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj(TileParams tp, Geom 
                 if (!in && r2 < thr_out) {  // guard band around rc^2: the plain fp64 definition decides (R26)
                     const uint32_t j = PRE ? ent >> 4 : ent;
                     in = tile_exact_r2(pos, g, tc.g0 + p, tile_global_of_staged(h, tc.n_sc, j)) < lj.rc2_exact;
+                }
+                if (MIXED && r2 < (real)lj.near2) {  // first shell: fp64 on the global positions
+                    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+                    lj_near_pair(pos, g.L[0], g.L[1], g.L[2], tc.g0 + p, tile_global_of_staged(h, tc.n_sc, PRE ? ent >> 4 : ent),
+                                 lj.rc2_exact, lj.sig2, lj.eps24, lj.eps4, lj.uc, acc);
+                    fx += acc[0]; fy += acc[1]; fz += acc[2];
+                    if (ENERGY) en += acc[3];
+                    in = false;
                 }
                 const real rinv2 = md_rcp(r2);
                 const real s2 = sig2 * rinv2;
@@ -1061,6 +1233,17 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj(TileParams tp, Geom 
 // decides by sign; a block of 8 entries in which some |d| < guard is re-evaluated with the exact fp64 test.
 // 8 contributions are summed in fp32, the block sum is widened and accumulated in fp64 (MD_OPT_ACC_BLOCK = 8).
 // ===============================================================================================================
+// k_tile_lj3: coordinates stay in box units (the staging is exact, see tile_stage_exact); sigma enters as s2 = sigma^2 / r^2,
+// g = (s6 - 1/2) s6 s2 and F_i = (48 eps / sigma^2) sum_j g d_ij
+struct LJ3U {
+    double rc2_exact;     // rc^2 (exact re-test)
+    double sig2;          // sigma^2
+    double guard64;       // decision band of the near section around rc^2 (rebuilt fp64 separations)
+    double fscale;        // 48 eps / sigma^2
+    float rc2s, guard;    // rc^2 and the guard band of the fp32 far loop
+    float sig2f;
+};
+
 struct LJ3 {
     double rc2_exact;     // rc^2 in box units (exact re-test)
     double inv_sigma;     // staging scale
@@ -1126,7 +1309,7 @@ __device__ __forceinline__ unsigned long long f2_fma(unsigned long long a, unsig
 // slow path of one block of 8 entries.  The fast path treats a pair inside the guard band as out of range, so what is
 // left to do is ADD the pairs of the band that the exact fp64 test puts inside rc (R26).
 __device__ __noinline__ void lj3_block_corr(const uint4 q, uint32_t rec_addr, float mx, float my, float mz, float rc2s,
-                                           float guard, const double4 *__restrict__ pos, double Lx, double Ly, double Lz,
+                                           float guard, float sig2, const double4 *__restrict__ pos, double Lx, double Ly, double Lz,
                                            double rc2_exact, uint32_t gi, const uint32_t *gstart, const uint32_t *sstart,
                                            uint32_t n_sc, float *out)
 {
@@ -1146,7 +1329,7 @@ __device__ __noinline__ void lj3_block_corr(const uint4 q, uint32_t rec_addr, fl
                 if (sstart[mid] <= s) lo = mid; else hi = mid;
             }
             if (tile_exact_r2_impl(pos, Lx, Ly, Lz, gi, gstart[lo] + (s - sstart[lo])) < rc2_exact) {
-                const float rinv2 = md_rcp(r2);
+                const float rinv2 = md_rcp(r2) * sig2;
                 const float s6 = rinv2 * rinv2 * rinv2;
                 const float f = (s6 - 0.5f) * (s6 * rinv2);
                 ax = fmaf(f, dx, ax); ay = fmaf(f, dy, ay); az = fmaf(f, dz, az);
@@ -1156,12 +1339,65 @@ __device__ __noinline__ void lj3_block_corr(const uint4 q, uint32_t rec_addr, fl
     out[0] = ax; out[1] = ay; out[2] = az;
 }
 
+__device__ __forceinline__ double md_rcp_nr1(double x);
+
+// Near section of a row (its first K blocks, see near_partition): fp32 separations cannot hold the 1e-4 bar on the steep
+// part of the potential (|dF/dr| ~ 450 at r ~ sigma: a coordinate error of 5e-7 is 2e-4 in the force; R25), so
+// these blocks are evaluated in fp64 on separations rebuilt from the staged records and their residuals
+// (tile_stage_exact): d = (x_i - x_j) + qr (res_i - res_j), the first term an exact fp32 difference of grid values, good
+// to ~1e-9, with the same shared-memory gather as the far loop and inside the same loop over the row's blocks.
+// r < rc: decided by the rebuilt r^2 outside a band of width `guard`, by the exact expression on the global positions
+// inside it (R26).  Returns sum g d of one block of 8 entries.
+__device__ __noinline__ void lj3_near(const uint2 *__restrict__ halves, uint32_t n_halves, uint32_t lane, uint32_t W,
+                                      uint32_t rec_addr, float4 me, double qr, double sig2, double rc2, double guard,
+                                      const double4 *__restrict__ pos, double Lx, double Ly, double Lz, uint32_t gi,
+                                      const uint32_t *gstart, const uint32_t *sstart, uint32_t n_sc, double *out)
+{
+    const uint32_t mw = __float_as_uint(me.w);
+    const int mrx = md_res_x(mw), mry = md_res_y(mw), mrz = md_res_z(mw);
+    double ax = 0.0, ay = 0.0, az = 0.0;
+    uint2 q = lane < n_halves ? __ldg(halves + lane) : make_uint2(0u, 0u);  // (prefetched into L1 by the caller)
+    for (uint32_t u = lane; u < n_halves; u += W) {
+        const uint2 qn = u + W < n_halves ? __ldg(halves + u + W) : q;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const uint32_t ww = e < 2 ? q.x : q.y;
+            const uint32_t off = (e & 1) ? (ww >> 16) : (ww & 0xffffu);
+            const float4 pj = lds_f4(rec_addr + off);
+            const uint32_t pw = __float_as_uint(pj.w);
+            const double dx = fma(qr, md_small_int_to_double(mrx - md_res_x(pw)), (double)(me.x - pj.x));
+            const double dy = fma(qr, md_small_int_to_double(mry - md_res_y(pw)), (double)(me.y - pj.y));
+            const double dz = fma(qr, md_small_int_to_double(mrz - md_res_z(pw)), (double)(me.z - pj.z));
+            const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+            const double d = r2 - rc2;
+            bool in = d < -guard;
+            if (!in && d < guard) {  // (the dummy records of the padding are far outside)
+                const uint32_t s = off >> 4;
+                uint32_t lo = 0, hi = n_sc;
+                while (hi - lo > 1) {
+                    const uint32_t mid = (lo + hi) >> 1;
+                    if (sstart[mid] <= s) lo = mid; else hi = mid;
+                }
+                in = tile_exact_r2_impl(pos, Lx, Ly, Lz, gi, gstart[lo] + (s - sstart[lo])) < rc2;
+            }
+            const double ri = sig2 * md_rcp_nr1(r2);
+            const double s6 = ri * ri * ri;
+            double f = (s6 - 0.5) * (s6 * ri);
+            f = in ? f : 0.0;
+            ax = fma(f, dx, ax); ay = fma(f, dy, ay); az = fma(f, dz, az);
+        }
+        q = qn;
+    }
+    out[0] = ax; out[1] = ay; out[2] = az;
+}
+
 template <int W, bool X2>
-__global__ void __launch_bounds__(256, 4) k_tile_lj3(TileParams tp, Geom g, const double4 *__restrict__ pos,
+__global__ void __launch_bounds__(MD_LJ3_MAX_BLOCK, 4) k_tile_lj3(TileParams tp, Geom g, const double4 *__restrict__ pos,
                                                              const float4 *__restrict__ rel,
                                                              const uint32_t *__restrict__ nl_cnt,
-                                                             const uint16_t *__restrict__ nl16, LJ3 lj,
-                                                             uint32_t max_staged, double4 *__restrict__ force)
+                                                             const uint16_t *__restrict__ nl16, LJ3U lj,
+                                                             uint32_t max_staged,
+                                                             double4 *__restrict__ force)
 {
     extern __shared__ __align__(16) char smem_raw[];
     float4 *rec = (float4 *)smem_raw;  // records first: their shared-memory address is a launch constant
@@ -1170,7 +1406,7 @@ __global__ void __launch_bounds__(256, 4) k_tile_lj3(TileParams tp, Geom g, cons
 
     TileCtx tc;
     tile_setup(tp, g, blockIdx.x, h, tc);
-    tile_stage_rel<false>(tc, h, rel, rec, scell, (float)lj.inv_sigma, pos, g);
+    tile_stage_exact(tc, h, rel, rec, scell, g);
     // staged index of every home particle (replaces a search per particle)
     uint16_t *hsidx = (uint16_t *)(scell + ((max_staged + 16) & ~15u));
     for (uint32_t hc = threadIdx.x >> 5; hc < tc.n_hc; hc += blockDim.x >> 5) {
@@ -1210,7 +1446,8 @@ __global__ void __launch_bounds__(256, 4) k_tile_lj3(TileParams tp, Geom g, cons
     }
     while (p < tc.n_home) {
         const float4 me = rec[hsidx[p]];
-        const uint32_t nblk = (cnt_c + 7u) >> 3;
+        const uint32_t n_near_blk = cnt_c >> MD_NL_NEAR_SHIFT;                          // the last K blocks: fp64 (lj3_near)
+        const uint32_t nblk = (((cnt_c & MD_NL_CNT_MASK) + 7u) >> 3) - n_near_blk;      // far blocks: fp32 below
         const uint4 *row = (const uint4 *)nl16 + (size_t)(tc.g0 + p) * stride8;
         uint4 q = q_c;
         const uint32_t pn = grab();
@@ -1219,6 +1456,9 @@ __global__ void __launch_bounds__(256, 4) k_tile_lj3(TileParams tp, Geom g, cons
             q_c = ldg_row((const uint4 *)nl16 + (size_t)(tc.g0 + pn) * stride8 + lane);
         }
         double fx = 0.0, fy = 0.0, fz = 0.0;
+        // the lane's first half-block of the near section is requested now (into L1, no register) and used after the far loop
+        const uint2 *halves = (const uint2 *)(row + nblk);
+        if (lane < 2u * n_near_blk) asm volatile("prefetch.global.L1 [%0];" ::"l"(halves + lane));
         for (uint32_t b = lane; b < nblk; b += W) {
             const uint4 qn = b + W < nblk ? __ldg(row + b + W) : q;  // prefetch the next block of 8 entries
             const uint32_t qq[4] = {q.x, q.y, q.z, q.w};
@@ -1226,6 +1466,7 @@ __global__ void __launch_bounds__(256, 4) k_tile_lj3(TileParams tp, Geom g, cons
             if (X2) {
                 unsigned long long ax2 = 0ull, ay2 = 0ull, az2 = 0ull;  // (0.f, 0.f)
                 const unsigned long long mrc2 = f2_pack(-rc2s, -rc2s), mhalf = f2_pack(-0.5f, -0.5f);
+                const unsigned long long sg2 = f2_pack(lj.sig2f, lj.sig2f);
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
                     const float4 pa = lds_f4(rec_addr + (qq[e] & 0xffffu));
@@ -1239,7 +1480,7 @@ __global__ void __launch_bounds__(256, 4) k_tile_lj3(TileParams tp, Geom g, cons
                     f2_unpack(r2, r2a, r2b);
                     f2_unpack(d, da, db);
                     band = fminf(band, fminf(fabsf(da), fabsf(db)));
-                    const unsigned long long ri = f2_pack(md_rcp(r2a), md_rcp(r2b));
+                    const unsigned long long ri = f2_mul(f2_pack(md_rcp(r2a), md_rcp(r2b)), sg2);
                     const unsigned long long s6 = f2_mul(f2_mul(ri, ri), ri);
                     const unsigned long long ff = f2_mul(f2_add(s6, mhalf), f2_mul(s6, ri));
                     float fa, fb;
@@ -1265,7 +1506,7 @@ __global__ void __launch_bounds__(256, 4) k_tile_lj3(TileParams tp, Geom g, cons
                     const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
                     const float d = r2 - rc2s;
                     band = fminf(band, fabsf(d));
-                    const float rinv2 = md_rcp(r2);
+                    const float rinv2 = md_rcp(r2) * lj.sig2f;
                     const float s6 = rinv2 * rinv2 * rinv2;
                     float f = (s6 - 0.5f) * (s6 * rinv2);
                     f = d < nguard ? f : 0.f;
@@ -1274,12 +1515,18 @@ __global__ void __launch_bounds__(256, 4) k_tile_lj3(TileParams tp, Geom g, cons
             }
             if (band < guard) {  // some pair of this block is inside the guard band: exact decisions (rare)
                 float o[3];
-                lj3_block_corr(q, rec_addr, me.x, me.y, me.z, rc2s, guard, pos, g.L[0], g.L[1], g.L[2], lj.rc2_exact,
+                lj3_block_corr(q, rec_addr, me.x, me.y, me.z, rc2s, guard, lj.sig2f, pos, g.L[0], g.L[1], g.L[2], lj.rc2_exact,
                                tc.g0 + p, h.gstart, h.sstart, tc.n_sc, o);
                 ax += o[0]; ay += o[1]; az += o[2];
             }
             fx += (double)ax; fy += (double)ay; fz += (double)az;
             q = qn;
+        }
+        if (n_near_blk) {  // the fp64 near section
+            double o[3];
+            lj3_near(halves, 2u * n_near_blk, lane, W, rec_addr, me, g.qr, lj.sig2, lj.rc2_exact, lj.guard64, pos, g.L[0],
+                     g.L[1], g.L[2], tc.g0 + p, h.gstart, h.sstart, tc.n_sc, o);
+            fx += o[0]; fy += o[1]; fz += o[2];
         }
         fx = md_seg_sum<W>(fx, seg_mask);
         fy = md_seg_sum<W>(fy, seg_mask);
@@ -1422,7 +1669,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj3d(TileParams tp, Geo
     uint32_t cnt_c = 0;
     uint4 q_c = make_uint4(0, 0, 0, 0);
     if (p < tc.n_home) {  // software pipeline over the group's particles, as in k_tile_lj3
-        cnt_c = __ldg(nl_cnt + tc.g0 + p);
+        cnt_c = __ldg(nl_cnt + tc.g0 + p) & MD_NL_CNT_MASK;
         q_c = __ldg((const uint4 *)nl16 + (size_t)(tc.g0 + p) * stride8 + lane);
     }
     for (; p < tc.n_home; p += n_groups) {
@@ -1433,7 +1680,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj3d(TileParams tp, Geo
         const uint4 *row = (const uint4 *)nl16 + (size_t)(tc.g0 + p) * stride8;
         uint4 q = q_c;
         if (p + n_groups < tc.n_home) {
-            cnt_c = __ldg(nl_cnt + tc.g0 + p + n_groups);
+            cnt_c = __ldg(nl_cnt + tc.g0 + p + n_groups) & MD_NL_CNT_MASK;
             q_c = __ldg(row + (size_t)n_groups * stride8 + lane);
         }
         double fx = 0.0, fy = 0.0, fz = 0.0, en = 0.0;
@@ -1654,7 +1901,7 @@ __global__ void __launch_bounds__(256, MINB) k_tile_lj4(TileParams tp, Geom g, c
     uint4 q_c = make_uint4(0, 0, 0, 0);
     if (cl < ncl) {  // software pipeline over the group's clusters, as in k_tile_lj3
         const uint32_t gp = tc.g0 + (ctab[2 * cl] & 0xffffffu);
-        cnt_c = __ldg(nl_cnt + gp);
+        cnt_c = __ldg(nl_cnt + gp) & MD_NL_CNT_MASK;
         q_c = __ldg((const uint4 *)nl16 + (size_t)gp * stride8 + lane);
     }
     for (; cl < ncl; cl += n_groups) {
@@ -1688,7 +1935,7 @@ __global__ void __launch_bounds__(256, MINB) k_tile_lj4(TileParams tp, Geom g, c
         uint4 q = q_c;
         if (cl + n_groups < ncl) {
             const uint32_t gp = tc.g0 + (ctab[2 * (cl + n_groups)] & 0xffffffu);
-            cnt_c = __ldg(nl_cnt + gp);
+            cnt_c = __ldg(nl_cnt + gp) & MD_NL_CNT_MASK;
             q_c = __ldg((const uint4 *)nl16 + (size_t)gp * stride8 + lane);
         }
         for (uint32_t b = lane; b < nblk; b += W) {
@@ -1777,7 +2024,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_dpd(TileParams tp, Geom
         const double4 me = rec[self];
         const double4 vi = svel[self];
         const uint32_t ti = md_lane_to_tag(me.w);
-        const uint32_t cnt = nl_cnt[tc.g0 + p];
+        const uint32_t cnt = nl_cnt[tc.g0 + p] & MD_NL_CNT_MASK;
         const uint32_t nblk = (cnt + 7u) >> 3;
         const uint4 *row = (const uint4 *)nl16 + (size_t)(tc.g0 + p) * stride8;
         double fx = 0.0, fy = 0.0, fz = 0.0, en = 0.0;
@@ -1893,7 +2140,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_dpd2(TileParams tp, Geo
         const uint32_t self = hsidx[p];
         const double2 ma = ra[self], mb = rb[self], mc = rc[self];
         const uint32_t ti = rt[self];
-        const uint32_t nblk = (nl_cnt[tc.g0 + p] + 7u) >> 3;
+        const uint32_t nblk = ((nl_cnt[tc.g0 + p] & MD_NL_CNT_MASK) + 7u) >> 3;
         const uint4 *row = (const uint4 *)nl16 + (size_t)(tc.g0 + p) * stride8;
         // ---- phase 1: distance tests, in-range entries compacted into the group's list
         uint32_t n_in = 0;  // entries in the list so far (the same in all lanes of the group)
@@ -1990,7 +2237,7 @@ __global__ void k_tile_decode(TileParams tp, Geom g, const double *__restrict__ 
             np = min(4u, h.hc_first[hc + 1] - p0);
             rowg = tc.g0 + p0;
         }
-        const uint32_t cnt = (nl_cnt[rowg] + 7u) & ~7u;  // stored rows are whole blocks of 8, dummies interspersed
+        const uint32_t cnt = ((nl_cnt[rowg] & MD_NL_CNT_MASK) + 7u) & ~7u;  // stored rows are whole blocks of 8, dummies interspersed
         const uint16_t *row = nl16 + (size_t)rowg * tp.stride;
         const double xi = pos_ref[3ull * gi], yi = pos_ref[3ull * gi + 1], zi = pos_ref[3ull * gi + 2];
         uint32_t *out = FILL ? nl_idx + nl_off[gi] : nullptr;
@@ -2136,14 +2383,21 @@ static uint32_t tile_shift(md_ctx *c) { return c->tile_max_staged + N_DUMMY <= 4
 // cluster rows need pre-shifted 16-bit entries (byte offsets of float4 records)
 bool tile_cluster_ok(md_ctx *c) { return c->precision == MD_MIXED && c->cluster_opt && tile_shift(c) == 4u; }
 
+static int tile_build_mode()
+{
+    static const int build_mode = getenv("B200MD_BUILD") ? atoi(getenv("B200MD_BUILD")) : 8;
+    return build_mode;
+}
+// k_tile_build8: 4 candidate phases per home particle; ballot variants: a full warp
+int tile_build_lanes(md_ctx *c) { return (!c->nl_cluster && tile_build_mode() == 8) ? 4 : 32; }
+
 int launch_tile_build(md_ctx *c, bool cluster, bool *fits)
 {
     const uint32_t ms = c->tile_max_staged;
     const int block = std::min(c->cfg[MD_K_NLIST].block, TILE_MAX_BLOCK);
     const uint32_t nw = (uint32_t)block / 32;
     size_t smem = tile_smem_common(c, sizeof(float4), false);
-    static const int build_mode = getenv("B200MD_BUILD") ? atoi(getenv("B200MD_BUILD")) : 8;
-    const bool b8 = !cluster && build_mode == 8;
+    const bool b8 = !cluster && tile_build_mode() == 8;
     const size_t rows = cluster ? 1 : (b8 ? BUILD8_P : BUILD_P);
     smem += sizeof(uint16_t) * (size_t)nw * rows * (c->nl_stride + RB_EXTRA + (b8 ? 8 : 0)) + sizeof(uint32_t) * nw * (b8 ? 4 : rows) * 24;  // row assembly
     *fits = smem <= TILE_SMEM_LIMIT && ms + N_DUMMY <= 65536 && c->tile_B <= 4;
@@ -2158,14 +2412,24 @@ int launch_tile_build(md_ctx *c, bool cluster, bool *fits)
     MD_CUDA_CHECK(c, cudaMemsetAsync(&c->d_flags->nl_overflow, 0, sizeof(unsigned int), c->stream));
     TileParams tp = make_tp(c);
     const double gd = guard_dot_fp32(E, R);
+    // near section (MD_MIXED, particle rows): neighbours within r_near + r_buff at the build, r_near = MD_NEAR_SIGMAS sigma
+    // of the LJ parameters last seen (R25); the force kernel checks that the section covers its own sigma
+    float thr_near = 0.f;
+    c->nl_near_r = 0.0;
+    static const double near_sig = getenv("B200MD_NEAR") ? atof(getenv("B200MD_NEAR")) : MD_NEAR_SIGMAS;  // diagnostic
+    if (!cluster && b8 && c->precision == MD_MIXED && near_sig > 0.0) {
+        c->nl_near_r = near_sig * c->lj_sigma_hint;
+        const double rn = c->nl_near_r + c->r_buff;
+        thr_near = (float)(rn * rn + gd);
+    }
     if (cluster) {
         MD_TRY(set_smem(c, k_tile_build_c<BUILD_P>, smem));
         k_tile_build_c<BUILD_P><<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->rel, c->pos, (float)(rl2 + gd), ms, c->nl_cnt,
                                                                        c->nl16, c->d_flags);
     } else if (b8) {
         MD_TRY(set_smem(c, k_tile_build8, smem));
-        k_tile_build8<<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->rel, c->pos, (float)(rl2 + gd), ms, c->nl_cnt, c->nl16,
-                                                             c->d_flags);
+        k_tile_build8<<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->rel, c->pos, (float)(rl2 + gd), thr_near, ms, c->nl_cnt,
+                                                             c->nl16, c->d_flags);
     } else {
         MD_TRY(set_smem(c, k_tile_build<BUILD_P>, smem));
         k_tile_build<BUILD_P><<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->rel, c->pos, (float)(rl2 + gd), ms, c->nl_cnt,
@@ -2216,6 +2480,7 @@ int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
     const double gd = mixed ? guard_fp32(E, R) : guard_fp64(E, R);
     p.thr_in = p.rc2_exact - gd;
     p.thr_out = p.rc2_exact + gd;
+    p.near2 = MD_NEAR_SIGMAS * MD_NEAR_SIGMAS * p.sig2;
     const size_t smem = tile_smem_common(c, mixed ? sizeof(float4) : sizeof(double4), false);
     TileParams tp = make_tp(c);
     static const int lj3_mode = getenv("B200MD_LJ3") ? atoi(getenv("B200MD_LJ3")) : 2;
@@ -2279,18 +2544,22 @@ int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
             return MD_OK;
         }
     }
-    if (mixed && !energy && c->nl_shift && c->acc_block == 8 && lj3_mode) {
+    if (mixed && !energy && c->nl_shift && c->acc_block == 8 && lj3_mode && (c->nl_near_r >= MD_NEAR_SIGMAS * sigma * (1.0 - 1e-12) || getenv("B200MD_NEAR"))) {
         const size_t smem = tile_smem_common(c, sizeof(float4), false) + ((2 * (size_t)c->tile_max_home + 15) & ~(size_t)15);
-        LJ3 q;
+        LJ3U q;
         q.rc2_exact = p.rc2_exact;
-        q.inv_sigma = 1.0 / sigma;
-        q.fscale = 48.0 * eps / sigma;
-        const double rc2s = p.rc2_exact / p.sig2;
-        q.rc2s = (float)rc2s;
-        // guard in scaled units: the fp32 error bound of r'^2 plus the rounding of rc'^2 itself
-        q.guard = (float)(1.0001 * (gd / p.sig2 + 2.0 * 5.9604644775390625e-08 * rc2s));
+        q.sig2 = p.sig2;
+        q.sig2f = (float)p.sig2;
+        q.fscale = 48.0 * eps / p.sig2;
+        q.rc2s = (float)p.rc2_exact;
+        // guard of the far loop: the fp32 error bound of r^2 plus the rounding of rc^2 itself
+        q.guard = (float)(1.0001 * (gd + 2.0 * 5.9604644775390625e-08 * p.rc2_exact));
+        {   // near section: a rebuilt separation component is good to ~2.5 qr (two residuals and two offsets of half a quantum)
+            const double dsep = 2.5 * c->g.qr + 1e-15 * E;
+            q.guard64 = 4.0 * (2.0 * 1.7320508075688772 * R * dsep + 3.0 * dsep * dsep);
+        }
         const int w = cf.w > 8 ? 8 : cf.w;
-        cf.block = std::min(cf.block, 256);  // k_tile_lj3 is compiled for 4 CTAs of 256 threads per SM (64 registers)
+        cf.block = std::min(cf.block, MD_LJ3_MAX_BLOCK);  // k_tile_lj3 is compiled for 4 CTAs of 256 threads per SM (64 registers)
         if (w <= 1) {
             MD_TRY(set_smem(c, (k_tile_lj3<1, true>), smem));
             k_tile_lj3<1, true><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force);
