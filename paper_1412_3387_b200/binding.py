@@ -234,6 +234,12 @@ class MD:
         self._chk(self.L.md_get_nlist(self.h, C.byref(n), _ptr(pairs), n.value), "md_get_nlist")
         return pairs
 
+    def count_nlist(self) -> int:
+        """Number of unordered pairs of the exported list (md_get_nlist with pairs = NULL)."""
+        n = C.c_uint64()
+        self._chk(self.L.md_get_nlist(self.h, C.byref(n), None, 0), "md_get_nlist")
+        return int(n.value)
+
     def get_nlist_rows(self, probe_tags, row_stride=512):
         pr = np.ascontiguousarray(probe_tags, dtype=np.uint32)
         counts = np.empty(pr.shape[0], dtype=np.uint32)

@@ -1545,10 +1545,14 @@ __global__ void __launch_bounds__(MD_LJ3_MAX_BLOCK, 4) k_tile_lj3(TileParams tp,
 // ===============================================================================================================
 __device__ __forceinline__ double md_rcp_nr1(double x)
 {
+    // MUFU.RCP64H (relative error e ~ 2^-23) and one third-order step y (1 + e + e^2): relative error e^3 ~ 2^-69, i.e. a
+    // correctly rounded reciprocal up to the last bit.  (A plain Newton step leaves 2^-46; times the r^-14 sensitivity
+    // of the pair term that is 2e-11 absolute on a first-shell pair -- above the 1e-10 bar for the few particles of a
+    // million whose net force nearly cancels.)
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
     const double e = fma(-x, y, 1.0);
-    return fma(y, e, y);
+    return fma(y, fma(e, e, e), y);
 }
 __device__ __forceinline__ double2 lds_d2(uint32_t addr)
 {
@@ -2072,10 +2076,11 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_dpd(TileParams tp, Geom
 // ===============================================================================================================
 __device__ __forceinline__ double md_rsqrt_nr1(double x)
 {
+    // MUFU.RSQ64H and one third-order step: with e = 1 - x y^2, 1/sqrt(x) = y (1 + e/2 + 3 e^2/8 + ...): error ~ e^3
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    const double t = x * y;
-    return fma(y * 0.5, fma(-t, y, 1.0), y);  // one Newton step: relative error ~2^-45
+    const double e = fma(-x * y, y, 1.0);
+    return fma(y, e * fma(0.375, e, 0.5), y);
 }
 
 template <int W>

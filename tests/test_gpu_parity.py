@@ -565,8 +565,10 @@ def test_mixed_accumulation_blocks_agree():
 
 
 def test_tile_guard_band_pairs_at_the_cutoff():
-    """Pairs placed within 1e-7 of r_list and of rc (inside the fp32 guard band) take the exact fp64 decision."""
-    wl = inputs.lj_fcc(8, rc=2.5, r_buff=0.4)                                # perfect FCC, N=2048, L=13.4
+    """Pairs placed within 1e-7 of r_list and of rc (inside the fp32 guard band) take the exact fp64 decision.  The
+    base configuration is a jittered lattice (a liquid-like force distribution), so the R11 norm applies as it stands:
+    1e-10 in fp64, 1e-4 in mixed precision, for md_forces_lj and for the kernels md_step launches."""
+    wl = inputs.lj_fcc(8, rc=2.5, r_buff=0.4, kT=1.0, jitter=0.05, pos_seed=11, vel_seed=12)     # N=2048, L=13.4
     pos, box = wl.pos.copy(), wl.box
     rng = np.random.default_rng(3)
     used = np.zeros(wl.N, dtype=bool)
@@ -592,11 +594,115 @@ def test_tile_guard_band_pairs_at_the_cutoff():
     pos = oracle.wrap(pos, box)
     ref_pairs = oracle.neighbor_pairs(pos, box, 2.9)
     Fr = oracle.forces_lj(pos, box, 2.5)[0]
-    for prec in (B.MD_FP64, B.MD_MIXED):
+    desc = B.step_desc("lj", 1e-300, wl.params)          # a step that moves nothing: the forces are those of `pos`
+    for prec, bar in ((B.MD_FP64, 1e-10), (B.MD_MIXED, 1e-4)):
         md = B.MD(box, len(pos), 2.5, 0.4, precision=prec)
         md.set_state(pos, np.zeros_like(pos)); md.build_nlist()
         assert np.array_equal(sort_pairs(md.get_nlist()), ref_pairs)
         md.forces_lj()
         F, _ = md.get_forces()
-        # a wrongly included / excluded pair at rc changes a force by |F(rc)| = 0.039: far above either tolerance
-        assert np.abs(F - Fr).max() < 2e-3
+        # a wrongly included / excluded pair at rc changes a force by |F(rc)| = 0.039: far above either bar
+        assert force_rel_err(F, Fr) < bar
+        # the kernels md_step launches (k_tile_lj3 / k_tile_lj3d, no energies): forces read back WITHOUT an energy buffer
+        ms = B.MD(box, len(pos), 2.5, 0.4, precision=prec)
+        ms.set_state(pos, np.zeros_like(pos))
+        ms.step(desc, 1)
+        Fs = np.empty_like(F); ms.get_forces(Fs, None)
+        assert force_rel_err(Fs, Fr) < bar
+
+
+def _step_forces(md, desc, n=1):
+    """Forces left by md_step, read back without an energy buffer (so nothing is re-evaluated), and the state."""
+    md.step(desc, n)
+    F = np.empty((md.N, 3)); md.get_forces(F, None)
+    pos, vel, _ = md.get_state()
+    return F, pos, vel
+
+
+@pytest.mark.parametrize("cluster", [0, 1])
+def test_step_kernels_forces_against_oracle(cluster):
+    """The kernels bench.py times (md_step: k_tile_lj3 with its near section and guard band, k_tile_lj4 with cluster
+    rows, k_tile_lj3d) compared DIRECTLY with the oracle at the positions md_step left: no energy
+    buffer is passed, so md_get_forces returns what the step's own kernel wrote."""
+    wl = inputs.lj_fcc(9, rc=3.0, r_buff=0.4, kT=1.2, jitter=0.05, pos_seed=2, vel_seed=3)       # config-2 recipe, N=2916
+    desc = B.step_desc("lj", wl.dt, wl.params)
+    for prec, bar in ((B.MD_MIXED, 1e-4), (B.MD_FP64, 1e-10)):
+        if cluster and prec != B.MD_MIXED:
+            continue
+        for w in (1, 2, 4, 8):
+            md = B.from_workload(wl, precision=prec)
+            md.set_option(B.MD_OPT_CLUSTER, cluster)
+            md.set_state(wl.pos, wl.vel)
+            md.set_launch(B.MD_K_LJ, 256, w)
+            F, pos, _ = _step_forces(md, desc, 25)          # 25 steps: at least one displacement-triggered rebuild
+            assert md.stats()["rebuilds"] >= 2
+            Fr, _ = oracle.forces_lj(pos, wl.box, wl.rc)
+            assert force_rel_err(F, Fr) < bar, (prec, w)
+            # reading energies afterwards must not change the forces the next half-kick uses
+            F2, E2 = md.get_forces()
+            assert np.array_equal(F2, F)
+            assert np.abs(E2 - oracle.forces_lj(pos, wl.box, wl.rc)[1]).max() < 10 * bar * np.abs(E2).max()
+
+
+def test_mixed_precision_other_sigma_and_near_section():
+    """sigma != 1: the near section of the rows is sized for the sigma md_step is called with (list rebuilt if it was
+    built for a smaller one); md_forces_lj with yet another sigma goes through the generic kernel; both within 1e-4."""
+    wl = inputs.lj_fcc(8, rc=2.5, r_buff=0.4, kT=1.0, jitter=0.05, pos_seed=5, vel_seed=6)
+    box, pos = wl.box * 1.15, oracle.wrap(wl.pos * 1.15, wl.box * 1.15)
+    for sigma in (1.15, 0.9):
+        md = B.MD(box, wl.N, 2.5 * 1.15, 0.4, precision=B.MD_MIXED)
+        md.set_state(pos, np.zeros_like(pos))
+        md.build_nlist()                                    # built before any sigma is known (hint = 1)
+        desc = B.step_desc("lj", 1e-300, dict(epsilon=0.8, sigma=sigma, energy_shift=1))
+        F, p2, _ = _step_forces(md, desc)
+        Fr, _ = oracle.forces_lj(p2, box, 2.5 * 1.15, 0.8, sigma, 1)
+        assert force_rel_err(F, Fr) < 1e-4
+        md.forces_lj(0.8, 1.3 * sigma, 1)
+        Fg, _ = md.get_forces()
+        assert force_rel_err(Fg, oracle.forces_lj(p2, box, 2.5 * 1.15, 0.8, 1.3 * sigma, 1)[0]) < 1e-4
+
+
+def test_build_nlist_after_integration_rebins():
+    """md_build_nlist alone after md_integrate_nve: the stale binning is redone, list bit-exact."""
+    for prec in (B.MD_FP64, B.MD_MIXED):
+        wl = _thermalised_lj(6, kT=3.0)
+        md = B.from_workload(wl, precision=prec)
+        md.build_nlist(); md.forces_lj()
+        for _ in range(40):
+            md.integrate_nve(wl.dt, 1)
+            if md.needs_rebuild():
+                break
+            md.forces_lj()
+            md.integrate_nve(wl.dt, 2)
+        assert md.needs_rebuild()
+        md.build_nlist()                                    # no md_build_cells before it
+        pos, _, _ = md.get_state()
+        assert np.array_equal(sort_pairs(md.get_nlist()), oracle.neighbor_pairs(pos, wl.box, wl.r_list))
+        assert np.array_equal(md.get_cells()[0], oracle.cell_assign(pos, wl.box, wl.r_list)[0])
+        assert not md.needs_rebuild()
+        md.forces_lj()
+        assert force_rel_err(md.get_forces()[0], oracle.forces_lj(pos, wl.box, wl.rc)[0]) < (1e-10 if prec == B.MD_FP64 else 1e-4)
+
+
+def test_tuner_reports_launched_sizes_and_retunes():
+    """md_tune sweeps every kernel family over launchable block sizes only; md_get_stats reports the launched (block, w);
+    MD_OPT_RETUNE_PERIOD makes md_step re-scan after that many rebuilds; results unchanged."""
+    wl = inputs.lj_fcc(10, rc=3.0, r_buff=0.4, kT=1.5, jitter=0.05, pos_seed=2, vel_seed=3)      # N=4000
+    desc = B.step_desc("lj", wl.dt, wl.params)
+    md = B.from_workload(wl, precision=B.MD_MIXED)
+    md.tune(desc, False)
+    st = md.stats()
+    assert st["launch"]["lj"]["block"] <= 256 and st["launch"]["nlist"]["block"] <= 512      # compiled limits
+    assert st["launch"]["integrate"]["block"] <= 256 and st["launch"]["lj"]["w"] <= 8
+    for k in ("cells", "nlist", "lj", "integrate"):
+        assert st["launch"][k]["us"] > 0, k
+    assert st["rebuilds"] == 1                              # the tuner's replays are not rebuilds of the run
+    md.set_launch(B.MD_K_LJ, 1024, 2)                       # a hand-set size above the limit is reported as launched
+    assert md.stats()["launch"]["lj"]["block"] == 256
+    md.set_option(B.MD_OPT_RETUNE_PERIOD, 2)
+    ref = B.from_workload(wl, precision=B.MD_MIXED)
+    ref.set_launch(B.MD_K_LJ, 256, 2)
+    md.step(desc, 60); ref.step(desc, 60)
+    assert md.stats()["tuner_runs"] >= 2 and md.stats()["rebuilds"] == ref.stats()["rebuilds"] >= 4
+    pa, _, _ = md.get_state(); pb, _, _ = ref.get_state()
+    assert np.abs(min_image_diff(pa, pb, wl.box)).max() < 1e-6   # same trajectory up to the summation order of other W
