@@ -32,9 +32,22 @@ UNIT = "particle-steps/s"
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/r1_v7_cfg2.md); None where no capture of that workload/kernel exists
-NCU_TRAFFIC = {("cfg2-lj-1M-mixed", "k_tile_lj3"): 463.7e6}
+def ncu_traffic(workload, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed
+    `ncu --set full` captures (profiles/ncu_traffic.json: one entry per workload and kernel, stamped with the hash of
+    the kernel source it was taken from).  None if there is no capture, or if the source has changed since (stale)."""
+    import hashlib
+    try:
+        tab = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))
+        src = open(os.path.join(ROOT, "paper_1412_3387_b200", "csrc", "tiles.cu"), "rb").read()
+        sha = hashlib.sha256(src).hexdigest()[:16]
+        for e in tab["entries"]:
+            if e["workload"] == workload and e["kernel"] == kernel:
+                return (float(e["dram_bytes_per_launch"]), None) if e["tiles_cu_sha16"] == sha else (
+                    None, "capture %s is of tiles.cu %s, now %s" % (e.get("file", "?"), e["tiles_cu_sha16"], sha))
+    except Exception as ex:  # noqa: BLE001
+        return None, "profiles/ncu_traffic.json: %s" % ex
+    return None, "no capture of this workload/kernel"
 
 
 def measured_hbm_peak():
@@ -58,7 +71,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -104,6 +117,17 @@ def workload_for(args):
         import dataclasses
         w = dataclasses.replace(w, r_buff=float(args.r_buff), name=w.name + "-rbuff%g" % args.r_buff)
     return w
+
+
+def algorithmic_ops(kind, nbar, rc, r_list):
+    """SURVEY.md 8(d) "arithmetic work for context", per particle and force evaluation, as lane-instructions (an FMA
+    counts once): n_bar distance tests of ~9 instructions (3 subtractions, 3 multiply-adds, compare, minimum image
+    amortised) and n_c = n_bar (rc / r_list)^3 in-range pair terms -- LJ 7 instructions + 1 reciprocal; DPD 12 fp64
+    instructions + rsqrt and ~70 integer instructions of Philox4x32-10."""
+    n_c = nbar * (rc / r_list) ** 3
+    if kind == "lj":
+        return {"fp": 9.0 * nbar + 8.0 * n_c, "int": 0.0}
+    return {"fp": 9.0 * nbar + 13.0 * n_c, "int": 70.0 * n_c}
 
 
 def algorithmic_bytes(kind, nbar, k):
@@ -227,8 +251,12 @@ def run_ours(args):
     precision = B.MD_MIXED if w.precision == "mixed" else B.MD_FP64
     stream = torch.cuda.Stream()
     order = {"lex": B.MD_ORDER_LEX, "morton": B.MD_ORDER_MORTON, "hilbert": B.MD_ORDER_HILBERT}[args.order]
+    # device memory comes from torch (md_workspace_bytes -> torch.empty -> md_set_workspace); streams too
     md = B.MD(w.box, w.N, w.rc, w.r_buff, precision=precision, stream=stream.cuda_stream, order=order,
-              sched=B.MD_SCHED_SYNC if args.sync_sched else B.MD_SCHED_SPECULATIVE)
+              sched=B.MD_SCHED_SYNC if args.sync_sched else B.MD_SCHED_SPECULATIVE,
+              workspace=None if args.own_alloc else "torch")
+    # measured issue rates of the pipes the pair-force kernel runs on (md_debug_peak), before the timed region
+    peaks = {k: md.debug_peak(k) for k in ("fp32_fma", "fp64_fma", "int32_mad")} if rank == 0 else {}
     nvt = None
     if args.nvt:
         import dataclasses
@@ -265,22 +293,25 @@ def run_ours(args):
     h_vel = torch.empty((w.N, 3), dtype=torch.float64).pin_memory()
     md.get_state(h_pos, h_vel, None)
     torch.cuda.synchronize()
-    st0 = md.stats()
-    md.set_profiling(2)            # CUDA events around the pair-force stage only (the roofline kernel): 2 events per step
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    e0 = torch.cuda.Event(enable_timing=True)
-    e1 = torch.cuda.Event(enable_timing=True)
-    barrier()
-    with torch.cuda.stream(stream):
-        e0.record(stream)
-        md.step(desc, args.steps)
-        e1.record(stream)
-    barrier()
+    # three repetitions of exactly `steps` steps each (the trajectory continues); the median one is reported
+    reps = []
+    for rep in range(1 if args.reps < 2 else args.reps):
+        ra = md.stats()
+        md.set_profiling(2)        # CUDA events around the pair-force stage only (the roofline kernel): 2 events per step
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        barrier()
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            md.step(desc, args.steps)
+            e1.record(stream)
+        barrier()
+        reps.append((e0.elapsed_time(e1), ra, md.stats()))
     clocks = sampler.stop() if rank == 0 else None
-    ms = e0.elapsed_time(e1)
-    st1 = md.stats()
+    rep_ms = [r[0] for r in reps]
     # stage shares: a short untimed continuation with every stage bracketed by events (about 8 events per step)
     md.set_profiling(1)
     n_share = max(20, min(200, args.steps // 4))
@@ -308,7 +339,10 @@ def run_ours(args):
     e2e_s = time.perf_counter() - t0
     barrier()
 
-    ms_max, e2e_ms = replica_max_times([ms, e2e_s * 1e3], world, "cuda")
+    (e2e_ms,) = replica_max_times([e2e_s * 1e3], world, "cuda")
+    rep_ms = replica_max_times(rep_ms, world, "cuda")                      # per repetition: the slowest rank
+    mi = sorted(range(len(rep_ms)), key=lambda i: rep_ms[i])[len(rep_ms) // 2]
+    ms_max, (_, st0, st1) = rep_ms[mi], reps[mi]
 
     if rank == 0:
         steps = st1["steps"] - st0["steps"]
@@ -330,6 +364,12 @@ def run_ours(args):
         f_ms = st1["stage_ms"][fk] / max(1, st1["stage_launches"][fk])
         achieved = w.N * b_force / (f_ms * 1e-3) / 1e9 if f_ms > 0 else 0.0
         stage_share = {n: round(v / ms_share, 4) for n, v in st_share["stage_ms"].items() if v > 0}
+        traffic, traffic_note = ncu_traffic(w.name, kernel)
+        ops = algorithmic_ops(w.kind, nbar, w.rc, w.rc + w.r_buff)
+        fp_pipe = "fp32_fma" if precision == B.MD_MIXED else "fp64_fma"
+        t_min = ops["fp"] / peaks[fp_pipe] + ops["int"] / peaks["int32_mad"]          # ns per particle at the pipe peaks
+        alu_ach = w.N * (ops["fp"] + ops["int"]) / (f_ms * 1e-3) / 1e9 if f_ms > 0 else 0.0
+        alu_peak = (ops["fp"] + ops["int"]) / t_min
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": ms_max / args.steps, "higher_is_better": True,
@@ -344,6 +384,9 @@ def run_ours(args):
                        "speculative_forces": st1["speculative_forces"] - st0["speculative_forces"],
                        "wasted_forces": st1["wasted_forces"] - st0["wasted_forces"],
                        "launch": {n: [v["block"], v["w"]] for n, v in st1["launch"].items()},
+                       "reps_ms_per_step": [r / args.steps for r in rep_ms], "reported": "median of %d repetitions" % len(rep_ms),
+                       "best_ms_per_step": min(rep_ms) / args.steps,
+                       "device_memory": "own cudaMalloc" if args.own_alloc else "torch tensor (md_workspace_bytes, md_set_workspace)",
                        "stage_share_of_step": stage_share,
                        "stage_share_from": "%d further steps with every stage bracketed by CUDA events" % n_share,
                        "step_bmin_bytes_per_particle": b_min,
@@ -355,8 +398,14 @@ def run_ours(args):
             "clocks": clocks,
             "roofline": {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak,
                          "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": NCU_TRAFFIC.get((w.name, kernel)),
+                         "traffic": traffic, "traffic_note": traffic_note,
                          "bytes_per_particle": b_force, "launch_ms": f_ms},
+            # second roofline: the same kernel's ALGORITHMIC instruction rate against the measured issue
+            # rate of the pipe(s) it runs on (md_debug_peak, giga lane-instructions per second, an FMA counts once)
+            "roofline_alu": {"pipe": fp_pipe + ("+int32_mad" if ops["int"] else ""), "kernel": kernel,
+                             "achieved": alu_ach, "peak": alu_peak, "unit": "G lane-instr/s",
+                             "frac": alu_ach / alu_peak if alu_peak else None,
+                             "instr_per_particle": ops, "measured_pipe_peaks": peaks},
         }
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(w)
@@ -385,6 +434,8 @@ def main():
     ap.add_argument("--nvt", action="store_true",
                     help="Nose-Hoover NVT (MD_F_NVT, kT = the workload's temperature, tau = 0.5) instead of NVE: "
                          "SURVEY 8(f) row 1; named in the workload, not a BASELINE configuration")
+    ap.add_argument("--reps", type=int, default=3, help="timed repetitions of --steps steps; the median is reported")
+    ap.add_argument("--own-alloc", action="store_true", help="let the library cudaMalloc instead of a torch workspace")
     ap.add_argument("--brick", type=int, default=0, help="MD_OPT_TILE_BRICK: 1, 2 or 4 cells per brick edge (0 = auto)")
     args = ap.parse_args()
     if args.impl == "reference":

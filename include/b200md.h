@@ -19,8 +19,9 @@
  *    on the context's stream; calls with a host OUTPUT pointer synchronise that stream before
  *    returning.  No torch types appear here; the Python binding passes tensor.data_ptr().
  *  - All device work runs on the stream given to md_configure (default: the legacy default stream).
- *  - The context owns all internal device memory (allocated with cudaMalloc at create/configure time,
- *    the neighbour list grows on demand at a rebuild).  One context per host thread; no global state.
+ *  - Internal device memory: carved from a caller-provided workspace (md_workspace_bytes, md_set_workspace) or, without
+ *    one, allocated with cudaMalloc at configure time (the neighbour list grows on demand at a rebuild).  One context
+ *    per host thread; no global state.
  *  - There is NO CPU fallback: every entry point needs a CUDA device and fails with MD_ECUDA otherwise.
  */
 #ifndef B200MD_H
@@ -113,6 +114,18 @@ typedef struct {
    and buffer ("skin") r_buff; the list radius is r_list = rc + r_buff.  box: HOST pointer to 3 doubles.
    Fails with MD_EINVAL unless floor(box[a]/r_list) >= 3 on every axis. */
 int md_create(md_ctx **out, const double box[3], uint64_t N, double rc, double r_buff);
+
+/* Device memory from the caller (north_star: "PyTorch used only for device memory and streams").
+   md_workspace_bytes: an upper estimate of everything a context of this problem allocates -- state and its reorder twins,
+   cell and tile tables, the neighbour list at 1.5x the stride its density suggests, the exact 32-bit copy that the list
+   exports build, staging for host-pointer arguments, a bond table of up to 2 bonds per particle.  box, bytes: HOST.
+   md_set_workspace: right after md_create (MD_ESTATE once anything is allocated); `workspace` is a DEVICE pointer the caller
+   owns and keeps alive until md_destroy.  Every internal buffer is then carved from it (first fit, 256-byte blocks;
+   buffers that grow -- a longer row stride at a rebuild, a larger export -- are re-carved); a request that does not fit
+   returns MD_ENOMEM with the missing bytes in md_last_error, nothing is allocated behind the caller's back.  Without
+   this call the context allocates with cudaMalloc.  Results are bit-identical either way. */
+int md_workspace_bytes(const double box[3], uint64_t N, double rc, double r_buff, int precision, uint64_t *bytes);
+int md_set_workspace(md_ctx *ctx, void *workspace, uint64_t bytes);
 
 /* precision: MD_FP64 | MD_MIXED.  stream: a cudaStream_t (as void*), NULL = default stream.
    order: MD_ORDER_*.  sched: MD_SCHED_*.  May be called again before md_set_state. */

@@ -24,7 +24,7 @@ MD_K_NLIST, MD_K_LJ, MD_K_DPD, MD_K_BONDS, MD_K_INTEGRATE, MD_K_CELLS = 0, 1, 2,
 KERNEL_NAMES = {MD_K_NLIST: "nlist", MD_K_LJ: "lj", MD_K_DPD: "dpd", MD_K_BONDS: "bonds",
                 MD_K_INTEGRATE: "integrate", MD_K_CELLS: "cells"}
 
-EXPORTS = ["md_create", "md_configure", "md_destroy", "md_last_error", "md_set_state", "md_set_bonds",
+EXPORTS = ["md_create", "md_workspace_bytes", "md_set_workspace", "md_configure", "md_destroy", "md_last_error", "md_set_state", "md_set_bonds",
            "md_get_state", "md_get_forces", "md_build_cells", "md_get_cells", "md_build_nlist", "md_get_nlist",
            "md_get_nlist_rows", "md_forces_lj", "md_forces_dpd", "md_forces_bonds", "md_integrate_nve",
            "md_needs_rebuild", "md_step", "md_tune", "md_set_option", "md_set_launch", "md_get_stats", "md_set_profiling",
@@ -74,6 +74,8 @@ def load():
     sig = {
         "md_create": [C.POINTER(vp), C.POINTER(dbl), u64, dbl, dbl],
         "md_configure": [vp, i32, vp, i32, i32],
+        "md_workspace_bytes": [C.POINTER(dbl), u64, dbl, dbl, i32, C.POINTER(u64)],
+        "md_set_workspace": [vp, vp, u64],
         "md_destroy": [vp],
         "md_set_state": [vp, vp, vp, vp, u64],
         "md_set_bonds": [vp, vp, vp, u64],
@@ -125,6 +127,16 @@ def _ptr(a):
     raise TypeError(type(a))
 
 
+def workspace_bytes(box, N, rc, r_buff, precision=MD_FP64) -> int:
+    """md_workspace_bytes: device bytes a context of this problem needs (upper estimate)."""
+    b = (C.c_double * 3)(*[float(x) for x in np.broadcast_to(np.asarray(box, dtype=np.float64), (3,))])
+    n = C.c_uint64()
+    s = load().md_workspace_bytes(b, int(N), float(rc), float(r_buff), int(precision), C.byref(n))
+    if s != 0:
+        raise MDError(f"md_workspace_bytes -> {s}")
+    return int(n.value)
+
+
 def step_desc(kind: str, dt: float, params: dict, nvt: dict = None) -> md_step_desc:
     """nvt = dict(kT, tau): Nose-Hoover thermostat (MD_F_NVT) instead of NVE."""
     d = md_step_desc()
@@ -156,7 +168,10 @@ def step_desc(kind: str, dt: float, params: dict, nvt: dict = None) -> md_step_d
 class MD:
     """One simulation context (md_ctx).  Methods are 1:1 with the C entry points (md_ prefix dropped)."""
 
-    def __init__(self, box, N, rc, r_buff, precision=MD_FP64, stream=None, order=MD_ORDER_MORTON, sched=MD_SCHED_SPECULATIVE):
+    def __init__(self, box, N, rc, r_buff, precision=MD_FP64, stream=None, order=MD_ORDER_MORTON, sched=MD_SCHED_SPECULATIVE,
+                 workspace=None):
+        """workspace: None (the library allocates), a CUDA uint8 tensor (md_set_workspace), or "torch": a tensor of
+        md_workspace_bytes bytes is taken from torch's allocator and kept alive with this object."""
         self.L = load()
         self.N = int(N)
         b = (C.c_double * 3)(*[float(x) for x in np.broadcast_to(np.asarray(box, dtype=np.float64), (3,))])
@@ -165,6 +180,14 @@ class MD:
         if s != 0:
             raise MDError(f"md_create -> {s}: {self.L.md_last_error(None).decode()}")
         self.h = h
+        self.workspace = None
+        if isinstance(workspace, str) and workspace == "torch":
+            import torch
+            workspace = torch.empty(workspace_bytes(box, N, rc, r_buff, precision), dtype=torch.uint8, device="cuda")
+        if workspace is not None:
+            self.workspace = workspace          # kept alive until close()
+            self._chk(self.L.md_set_workspace(self.h, workspace.data_ptr(), workspace.numel() * workspace.element_size()),
+                      "md_set_workspace")
         self._chk(self.L.md_configure(self.h, precision, stream, order, sched), "md_configure")
 
     def _chk(self, s, who):
@@ -175,6 +198,7 @@ class MD:
         if getattr(self, "h", None):
             self.L.md_destroy(self.h)
             self.h = None
+            self.workspace = None
 
     def __del__(self):
         try:

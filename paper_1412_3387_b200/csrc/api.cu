@@ -16,6 +16,26 @@ int md_alloc(md_ctx *c, void **p, uint64_t bytes)
 {
     *p = nullptr;
     if (bytes == 0) bytes = 16;
+    if (c->ws_base) {  // first fit in the caller's workspace
+        const uint64_t need = (bytes + 255) & ~255ull;
+        for (size_t i = 0; i < c->ws_blocks.size(); ++i) {
+            md_ctx::WsBlock &b = c->ws_blocks[i];
+            if (b.used || b.size < need) continue;
+            if (b.size > need) {
+                const md_ctx::WsBlock rest{b.off + need, b.size - need, false};
+                b.size = need;
+                c->ws_blocks.insert(c->ws_blocks.begin() + i + 1, rest);
+            }
+            c->ws_blocks[i].used = true;
+            *p = c->ws_base + c->ws_blocks[i].off;
+            c->device_bytes += need;
+            c->ws_peak = std::max(c->ws_peak, c->ws_blocks[i].off + need);
+            return MD_OK;
+        }
+        c->err = "workspace too small: " + std::to_string(bytes) + " more bytes needed, " + std::to_string(c->device_bytes) +
+                 " of " + std::to_string(c->ws_bytes) + " in use (size it with md_workspace_bytes)";
+        return MD_ENOMEM;
+    }
     cudaError_t e = cudaMalloc(p, bytes);
     if (e != cudaSuccess) {
         c->err = std::string("cudaMalloc(") + std::to_string(bytes) + "): " + cudaGetErrorString(e);
@@ -30,6 +50,24 @@ int md_alloc(md_ctx *c, void **p, uint64_t bytes)
 void md_free(md_ctx *c, void *p)
 {
     if (!p) return;
+    if (c->ws_base) {  // work already enqueued on the context's stream still owns the block in stream order
+        const uint64_t off = (uint64_t)((char *)p - c->ws_base);
+        for (size_t i = 0; i < c->ws_blocks.size(); ++i) {
+            if (c->ws_blocks[i].off != off || !c->ws_blocks[i].used) continue;
+            c->ws_blocks[i].used = false;
+            c->device_bytes -= c->ws_blocks[i].size;
+            if (i + 1 < c->ws_blocks.size() && !c->ws_blocks[i + 1].used) {
+                c->ws_blocks[i].size += c->ws_blocks[i + 1].size;
+                c->ws_blocks.erase(c->ws_blocks.begin() + i + 1);
+            }
+            if (i > 0 && !c->ws_blocks[i - 1].used) {
+                c->ws_blocks[i - 1].size += c->ws_blocks[i].size;
+                c->ws_blocks.erase(c->ws_blocks.begin() + i);
+            }
+            return;
+        }
+        return;
+    }
     for (auto it = c->allocs.begin(); it != c->allocs.end(); ++it)
         if (it->first == p) {
             c->device_bytes -= it->second;
@@ -318,6 +356,46 @@ static void set_default_cfg(md_ctx *c)
 
 static thread_local std::string g_create_err;
 
+// the per-particle and per-cell arrays: allocated at the first md_configure / md_set_state, so that md_set_workspace can
+// come between md_create and them
+static int alloc_state(md_ctx *c)
+{
+    if (c->state_allocated) return MD_OK;
+    const uint64_t N = c->N;
+    int s = MD_OK;
+    auto A = [&](void **p, uint64_t bytes) { if (s == MD_OK) s = md_alloc(c, p, bytes); };
+    A((void **)&c->pos, N * sizeof(double4));
+    A((void **)&c->pos_alt, N * sizeof(double4));
+    A((void **)&c->vel, N * sizeof(double4));
+    A((void **)&c->vel_alt, N * sizeof(double4));
+    A((void **)&c->force, N * sizeof(double4));
+    A((void **)&c->force_alt, N * sizeof(double4));
+    A((void **)&c->image, 3 * N * sizeof(int));
+    A((void **)&c->image_alt, 3 * N * sizeof(int));
+    A((void **)&c->pos_ref, 3 * N * sizeof(double));
+    A((void **)&c->rel, N * sizeof(float4));
+    A((void **)&c->nvt_state, 4 * sizeof(double));
+    A((void **)&c->tag, N * sizeof(uint32_t));
+    A((void **)&c->tag_alt, N * sizeof(uint32_t));
+    A((void **)&c->rtag, N * sizeof(uint32_t));
+    A((void **)&c->cell_lin, N * sizeof(uint32_t));
+    A((void **)&c->cell_rank_tmp, N * sizeof(uint32_t));
+    A((void **)&c->perm, N * sizeof(uint32_t));
+    A((void **)&c->perm_sorted, N * sizeof(uint32_t));
+    A((void **)&c->cell_count, (uint64_t)c->n_cells * sizeof(uint32_t));
+    A((void **)&c->cell_start, ((uint64_t)c->n_cells + 1) * sizeof(uint32_t));
+    A((void **)&c->nl_cnt, N * sizeof(uint32_t));
+    A((void **)&c->nl_off, (N + 1) * sizeof(uint64_t));
+    A((void **)&c->d_flags, sizeof(DevFlags));
+    if (s == MD_OK && cudaMallocHost((void **)&c->h_flags, sizeof(DevFlags)) != cudaSuccess) { c->err = "cudaMallocHost failed"; s = MD_ENOMEM; }
+    if (s == MD_OK && cudaMemset(c->d_flags, 0, sizeof(DevFlags)) != cudaSuccess) s = MD_ECUDA;
+    if (s == MD_OK && cudaMemset(c->force, 0, N * sizeof(double4)) != cudaSuccess) s = MD_ECUDA;
+    if (s != MD_OK) return s;
+    c->state_allocated = true;
+    return MD_OK;
+}
+
+
 extern "C" int md_create(md_ctx **out, const double box[3], uint64_t N, double rc, double r_buff)
 {
     if (!out) return MD_EINVAL;
@@ -365,39 +443,6 @@ extern "C" int md_create(md_ctx **out, const double box[3], uint64_t N, double r
     set_record_grid(c, 1);
     set_default_cfg(c);
 
-    int s = MD_OK;
-    auto A = [&](void **p, uint64_t bytes) { if (s == MD_OK) s = md_alloc(c, p, bytes); };
-    A((void **)&c->pos, N * sizeof(double4));
-    A((void **)&c->pos_alt, N * sizeof(double4));
-    A((void **)&c->vel, N * sizeof(double4));
-    A((void **)&c->vel_alt, N * sizeof(double4));
-    A((void **)&c->force, N * sizeof(double4));
-    A((void **)&c->force_alt, N * sizeof(double4));
-    A((void **)&c->image, 3 * N * sizeof(int));
-    A((void **)&c->image_alt, 3 * N * sizeof(int));
-    A((void **)&c->pos_ref, 3 * N * sizeof(double));
-    A((void **)&c->rel, N * sizeof(float4));
-    A((void **)&c->nvt_state, 4 * sizeof(double));
-    A((void **)&c->tag, N * sizeof(uint32_t));
-    A((void **)&c->tag_alt, N * sizeof(uint32_t));
-    A((void **)&c->rtag, N * sizeof(uint32_t));
-    A((void **)&c->cell_lin, N * sizeof(uint32_t));
-    A((void **)&c->cell_rank_tmp, N * sizeof(uint32_t));
-    A((void **)&c->perm, N * sizeof(uint32_t));
-    A((void **)&c->perm_sorted, N * sizeof(uint32_t));
-    A((void **)&c->cell_count, (uint64_t)c->n_cells * sizeof(uint32_t));
-    A((void **)&c->cell_start, ((uint64_t)c->n_cells + 1) * sizeof(uint32_t));
-    A((void **)&c->nl_cnt, N * sizeof(uint32_t));
-    A((void **)&c->nl_off, (N + 1) * sizeof(uint64_t));
-    A((void **)&c->d_flags, sizeof(DevFlags));
-    if (s == MD_OK && cudaMallocHost((void **)&c->h_flags, sizeof(DevFlags)) != cudaSuccess) { c->err = "cudaMallocHost failed"; s = MD_ENOMEM; }
-    if (s == MD_OK && cudaMemset(c->d_flags, 0, sizeof(DevFlags)) != cudaSuccess) s = MD_ECUDA;
-    if (s == MD_OK && cudaMemset(c->force, 0, N * sizeof(double4)) != cudaSuccess) s = MD_ECUDA;
-    if (s != MD_OK) {
-        g_create_err = c->err;
-        md_destroy(c);
-        return s;
-    }
     *out = c;
     return MD_OK;
 }
@@ -410,6 +455,7 @@ extern "C" int md_configure(md_ctx *c, int precision, void *stream, int order, i
         c->err = "md_configure: bad argument";
         return MD_EINVAL;
     }
+    MD_TRY(alloc_state(c));
     c->precision = precision;
     c->stream = (cudaStream_t)stream;
     c->sched = sched;
@@ -418,6 +464,48 @@ extern "C" int md_configure(md_ctx *c, int precision, void *stream, int order, i
         MD_TRY(build_cell_order(c));
         c->cells_valid = c->nlist_valid = false;
     }
+    return MD_OK;
+}
+
+// ---- caller-provided device memory ("PyTorch used only for device memory and streams") ---------------
+extern "C" int md_set_workspace(md_ctx *c, void *workspace, uint64_t bytes)
+{
+    if (!c) return MD_EINVAL;
+    if (c->state_allocated || c->device_bytes) { c->err = "md_set_workspace: call it right after md_create (device memory is already allocated)"; return MD_ESTATE; }
+    if (!workspace || bytes < 4096 || !is_device_ptr(workspace)) { c->err = "md_set_workspace: a device pointer and its size are required"; return MD_EINVAL; }
+    const uint64_t skew = (256 - ((uintptr_t)workspace & 255)) & 255;  // blocks are 256-byte aligned
+    c->ws_base = (char *)workspace + skew;
+    c->ws_bytes = (bytes - skew) & ~255ull;
+    c->ws_blocks.assign(1, md_ctx::WsBlock{0, c->ws_bytes, false});
+    c->ws_peak = 0;
+    return MD_OK;
+}
+
+extern "C" int md_workspace_bytes(const double box[3], uint64_t N, double rc, double r_buff, int precision, uint64_t *bytes)
+{
+    if (!box || !bytes || N == 0 || !(rc > 0.0) || !(r_buff >= 0.0)) return MD_EINVAL;
+    (void)precision;  // both modes keep the same arrays (the fp32 records exist in fp64 mode too)
+    const double r_list = rc + r_buff;
+    double ncell = 1.0, vol = 1.0;
+    for (int a = 0; a < 3; ++a) {
+        const double n = floor(box[a] / r_list);
+        if (!(box[a] > 0.0) || n < 3.0) return MD_EINVAL;
+        ncell *= n;
+        vol *= box[a];
+    }
+    const double n = (double)N;
+    const double nbar = n / vol * 4.18879020478639 * r_list * r_list * r_list;  // mean neighbours per particle
+    double b = 0.0;
+    b += n * (6 * 32 + 2 * 12 + 24 + 16 + 7 * 4 + 4 + 8);           // state, twins, records, tags, permutations, row lengths, offsets
+    b += ncell * (4 * 4 + 320.0) + 65536.0;                          // cell tables, curve tables, per-tile headers
+    b += (n + 1.0) * (1.5 * (1.35 * nbar + 24.0) + 32.0) * 2.0;      // 16-bit rows at the density-based stride, grown once by 1.5
+    b += n * 4.0 + n * (nbar + 4.0) * 4.0 * 1.125 + 4096.0;          // the exact 32-bit list (general path; exports of a tile list)
+    b += n * (4.0 + 8.0) + n * 20.0;                                 // export scratch; bond table for up to 2 bonds per particle
+    b += 2.0 * 3.0 * 8.0 * n * 1.125 + 65536.0;                      // staging of host-pointer state arguments ...
+    b += n * (nbar + 4.0) * 4.0 * 1.125;                             // ... or of an exported pair list (8 bytes per pair)
+    b += 64.0 * 256.0 + 1048576.0;                                   // block rounding, small tables
+    b *= 1.10;                                                       // first-fit fragmentation
+    *bytes = (uint64_t)b;
     return MD_OK;
 }
 
@@ -443,6 +531,7 @@ extern "C" const char *md_last_error(md_ctx *c) { return c ? c->err.c_str() : g_
 extern "C" int md_set_state(md_ctx *c, const double *pos, const double *vel, const double *mass, uint64_t step0)
 {
     if (!c || !pos || !vel) { if (c) c->err = "md_set_state: pos and vel are required"; return MD_EINVAL; }
+    MD_TRY(alloc_state(c));
     const uint64_t b3 = 3 * c->N * sizeof(double), b1 = c->N * sizeof(double);
     Stage st(c);
     MD_TRY(st.reserve(stage_need(pos, b3) + stage_need(vel, b3) + stage_need(mass, b1)));
@@ -465,6 +554,7 @@ extern "C" int md_set_bonds(md_ctx *c, const uint32_t *ta, const uint32_t *tb, u
     if (!c) return MD_EINVAL;
     if (nb > 0 && (!ta || !tb)) { c->err = "md_set_bonds: null tag array"; return MD_EINVAL; }
     if (nb >= 0x7fffffffull) { c->err = "md_set_bonds: too many bonds"; return MD_EINVAL; }
+    MD_TRY(alloc_state(c));
     MD_TRY(md_sync(c));
     if (c->bond_off) { md_free(c, c->bond_off); c->bond_off = nullptr; }
     if (c->bond_partner) { md_free(c, c->bond_partner); c->bond_partner = nullptr; }

@@ -171,6 +171,13 @@ struct md_ctx {
     bool tune_skip = false;  // set by a tuner replay that could not launch its configuration
     uint64_t device_bytes = 0;
     std::vector<std::pair<void *, uint64_t>> allocs;
+    // caller-provided workspace (md_set_workspace): every internal buffer is carved from it (first fit, 256-byte units);
+    // without one the context allocates with cudaMalloc
+    char *ws_base = nullptr;
+    uint64_t ws_bytes = 0, ws_peak = 0;
+    struct WsBlock { uint64_t off, size; bool used; };
+    std::vector<WsBlock> ws_blocks;
+    bool state_allocated = false;  // the per-particle arrays exist (allocated at the first md_configure / md_set_state)
     bool log = false;
 
     // per-stage event timing (md_set_profiling)

@@ -706,3 +706,34 @@ def test_tuner_reports_launched_sizes_and_retunes():
     assert md.stats()["tuner_runs"] >= 2 and md.stats()["rebuilds"] == ref.stats()["rebuilds"] >= 4
     pa, _, _ = md.get_state(); pb, _, _ = ref.get_state()
     assert np.abs(min_image_diff(pa, pb, wl.box)).max() < 1e-6   # same trajectory up to the summation order of other W
+
+
+def test_caller_workspace_bit_identical_and_enomem():
+    """md_workspace_bytes + md_set_workspace: every internal buffer carved from a torch tensor; results
+    bit-identical to the cudaMalloc path for LJ mixed (tile list, exports) and the polymer melt; a workspace that is too
+    small fails with MD_ENOMEM and names the missing bytes."""
+    import torch
+    for wl, prec in ((inputs.lj_fcc(9, rc=3.0, r_buff=0.4, kT=1.2, jitter=0.05, pos_seed=2, vel_seed=3), B.MD_MIXED),
+                     (inputs.polymer_melt(40, chain_len=32), B.MD_FP64)):
+        desc = B.step_desc(wl.kind, wl.dt, wl.params)
+        a = B.from_workload(wl, precision=prec)
+        need = B.workspace_bytes(wl.box, wl.N, wl.rc, wl.r_buff, prec)
+        ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+        b = B.from_workload(wl, precision=prec, workspace=ws)
+        c = B.from_workload(wl, precision=prec, workspace="torch")
+        for md in (a, b, c):
+            md.step(desc, 30)
+        pa, va, _ = a.get_state()
+        for md in (b, c):
+            p, v, _ = md.get_state()
+            assert np.array_equal(p, pa) and np.array_equal(v, va)
+            assert np.array_equal(sort_pairs(md.get_nlist()), sort_pairs(a.get_nlist()))
+            assert np.array_equal(md.get_forces()[0], a.get_forces()[0])
+        st = b.stats()
+        assert 0 < st["device_bytes"] <= need
+        b.close(); c.close()
+    small = torch.empty(1 << 16, dtype=torch.uint8, device="cuda")
+    with pytest.raises(B.MDError, match="workspace too small"):
+        B.from_workload(wl, workspace=small)
+    md = B.MD(wl.box, wl.N, wl.rc, wl.r_buff)               # after md_configure the workspace can no longer be set
+    assert md.L.md_set_workspace(md.h, small.data_ptr(), small.numel()) == -2
