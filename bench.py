@@ -285,6 +285,14 @@ def run_ours(args):
         md.set_launch({v: k for k, v in B.KERNEL_NAMES.items()}[name], blk, ww)
     if not args.no_tune:
         md.tune(desc, False)
+    if args.auto_rbuff:
+        # the library picks the skin with the most steps per second (md_tune_rbuff); named in the
+        # workload -- the reported BASELINE configuration keeps r_buff = 0.4
+        import dataclasses
+        rb = md.tune_rbuff(desc, None, 200)
+        w = dataclasses.replace(w, r_buff=rb, name=w.name + "-autorbuff%g" % rb)
+        if not args.no_tune:
+            md.tune(desc, False)
 
     # ---- device-resident timing ---------------------------------------------------------------------------
     md.step(desc, max(3, args.warmup))
@@ -431,6 +439,8 @@ def main():
     ap.add_argument("--cluster", action="store_true", help="MD_OPT_CLUSTER = 1: one neighbour row per cluster of 4")
     ap.add_argument("--r-buff", type=float, default=None, dest="r_buff",
                     help="override the configured skin r_buff = 0.4 (tuning sweep; not a reported configuration)")
+    ap.add_argument("--auto-rbuff", action="store_true", dest="auto_rbuff",
+                    help="md_tune_rbuff: let the library choose the skin (tuning run; not a reported configuration)")
     ap.add_argument("--nvt", action="store_true",
                     help="Nose-Hoover NVT (MD_F_NVT, kT = the workload's temperature, tau = 0.5) instead of NVE: "
                          "SURVEY 8(f) row 1; named in the workload, not a BASELINE configuration")

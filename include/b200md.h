@@ -106,6 +106,8 @@ typedef struct {
     uint64_t stage_launches[MD_N_KERNELS];  /* the context's stream), accumulated since profiling was switched on  */
     uint64_t speculative_forces;            /* force evaluations enqueued before the rebuild flag was known ...     */
     uint64_t wasted_forces;                 /* ... and how many of them were discarded because a rebuild was due    */
+    double r_buff;                          /* the skin in use (md_create's, or the one md_tune_rbuff chose)         */
+    double rbuff_tuned_tps;                 /* time steps per second of that skin in md_tune_rbuff's burst (0: never tuned) */
 } md_stats;
 
 /* ---- lifetime ------------------------------------------------------------------------------------------ */
@@ -227,6 +229,17 @@ int md_step(md_ctx *ctx, const md_step_desc *what, uint64_t n_steps);
    kernel; with the environment variable B200MD_LOG set every timing is printed to stderr.  MD_OPT_RETUNE_PERIOD = M
    makes md_step repeat a local re-scan (neighbouring block sizes, w/2 .. 2w) after every M rebuilds. */
 int md_tune(md_ctx *ctx, const md_step_desc *what, int full);
+
+/* SURVEY.md 8(f) row 2.  The paper determines r_buff per benchmark "as the value that yields the highest number of time
+   steps per second".  For each candidate skin (candidates[n_candidates], HOST; NULL = 0.5 ... 2 times the
+   current one in steps of 0.25; values the box cannot hold -- fewer than 3 cells per axis -- are skipped) the context is
+   re-gridded, `what` is run for burst_steps / 10 untimed and burst_steps (0 = 200) timed steps from the SAME saved state, and
+   the fastest skin is kept: the state, the step counter and the statistics are those from before the call, the cell grid
+   and the neighbour list are those of the chosen skin (rebuilt at the next call).  *chosen (HOST, may be NULL) and
+   md_get_stats().r_buff report it; B200MD_LOG prints every burst.  Trajectories do not depend on the skin beyond
+   floating-point summation order; bench.py reports the configured r_buff = 0.4 unless asked (--auto-rbuff). */
+int md_tune_rbuff(md_ctx *ctx, const md_step_desc *what, const double *candidates, uint32_t n_candidates,
+                  uint64_t burst_steps, double *chosen);
 
 /* Options of the tile path (MD_ORDER_MORTON).  MD_OPT_TILE_BRICK: edge of the cell brick one CTA owns, 1, 2 or 4
    (0 = choose from the density); invalidates cells and list.  MD_OPT_ACC_BLOCK (MD_MIXED only): 1 = every pair's

@@ -27,7 +27,7 @@ KERNEL_NAMES = {MD_K_NLIST: "nlist", MD_K_LJ: "lj", MD_K_DPD: "dpd", MD_K_BONDS:
 EXPORTS = ["md_create", "md_workspace_bytes", "md_set_workspace", "md_configure", "md_destroy", "md_last_error", "md_set_state", "md_set_bonds",
            "md_get_state", "md_get_forces", "md_build_cells", "md_get_cells", "md_build_nlist", "md_get_nlist",
            "md_get_nlist_rows", "md_forces_lj", "md_forces_dpd", "md_forces_bonds", "md_integrate_nve",
-           "md_needs_rebuild", "md_step", "md_tune", "md_set_option", "md_set_launch", "md_get_stats", "md_set_profiling",
+           "md_needs_rebuild", "md_step", "md_tune", "md_tune_rbuff", "md_set_option", "md_set_launch", "md_get_stats", "md_set_profiling",
            "md_debug_philox", "md_debug_peak", "md_thermo", "md_integrate_nvt", "md_set_thermostat", "md_get_thermostat"]
 
 
@@ -51,7 +51,8 @@ class md_stats(C.Structure):
                 ("block", C.c_int32 * MD_N_KERNELS), ("w", C.c_int32 * MD_N_KERNELS),
                 ("tuned_us", C.c_float * MD_N_KERNELS), ("tuner_runs", C.c_uint32), ("launches", C.c_uint32),
                 ("stage_ms", C.c_double * MD_N_KERNELS), ("stage_launches", C.c_uint64 * MD_N_KERNELS),
-                ("speculative_forces", C.c_uint64), ("wasted_forces", C.c_uint64)]
+                ("speculative_forces", C.c_uint64), ("wasted_forces", C.c_uint64),
+                ("r_buff", C.c_double), ("rbuff_tuned_tps", C.c_double)]
 
 
 class MDError(RuntimeError):
@@ -93,6 +94,7 @@ def load():
         "md_needs_rebuild": [vp, C.POINTER(i32)],
         "md_step": [vp, C.POINTER(md_step_desc), u64],
         "md_tune": [vp, C.POINTER(md_step_desc), i32],
+        "md_tune_rbuff": [vp, C.POINTER(md_step_desc), C.POINTER(dbl), u32, u64, C.POINTER(dbl)],
         "md_set_launch": [vp, i32, i32, i32],
         "md_set_option": [vp, i32, C.c_int64],
         "md_get_stats": [vp, C.POINTER(md_stats)],
@@ -309,6 +311,17 @@ class MD:
     def tune(self, desc: md_step_desc, full: bool = False):
         self._chk(self.L.md_tune(self.h, C.byref(desc), int(full)), "md_tune")
 
+    def tune_rbuff(self, desc: md_step_desc, candidates=None, burst_steps=0) -> float:
+        """md_tune_rbuff: the skin with the most steps per second among `candidates` (None = 0.5 .. 2 x the current one)."""
+        out = C.c_double()
+        if candidates is None:
+            arr, n = None, 0
+        else:
+            n = len(candidates)
+            arr = (C.c_double * n)(*[float(x) for x in candidates])
+        self._chk(self.L.md_tune_rbuff(self.h, C.byref(desc), arr, n, int(burst_steps), C.byref(out)), "md_tune_rbuff")
+        return out.value
+
     def set_profiling(self, on: bool):
         self._chk(self.L.md_set_profiling(self.h, int(on)), "md_set_profiling")
 
@@ -323,7 +336,7 @@ class MD:
         self._chk(self.L.md_get_stats(self.h, C.byref(st)), "md_get_stats")
         d = {k: getattr(st, k) for k in ("steps", "rebuilds", "dangerous_builds", "nlist_entries", "nlist_capacity",
                                          "device_bytes", "mean_neighbors", "max_cell_count", "tuner_runs", "launches",
-                                         "speculative_forces", "wasted_forces")}
+                                         "speculative_forces", "wasted_forces", "r_buff", "rbuff_tuned_tps")}
         d["dims"] = list(st.dims)
         d["stage_ms"] = {KERNEL_NAMES[k]: st.stage_ms[k] for k in KERNEL_NAMES}
         d["stage_launches"] = {KERNEL_NAMES[k]: st.stage_launches[k] for k in KERNEL_NAMES}

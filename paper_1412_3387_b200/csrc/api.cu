@@ -16,20 +16,31 @@ int md_alloc(md_ctx *c, void **p, uint64_t bytes)
 {
     *p = nullptr;
     if (bytes == 0) bytes = 16;
-    if (c->ws_base) {  // first fit in the caller's workspace
+    if (c->ws_base) {
+        // first fit in the caller's workspace; buffers above 1/32 of it (neighbour lists, exports, staging: the ones that
+        // are re-carved when they grow) are taken from the TOP so that they do not fragment the long-lived small ones
         const uint64_t need = (bytes + 255) & ~255ull;
-        for (size_t i = 0; i < c->ws_blocks.size(); ++i) {
-            md_ctx::WsBlock &b = c->ws_blocks[i];
-            if (b.used || b.size < need) continue;
-            if (b.size > need) {
-                const md_ctx::WsBlock rest{b.off + need, b.size - need, false};
-                b.size = need;
-                c->ws_blocks.insert(c->ws_blocks.begin() + i + 1, rest);
+        const bool big = need > c->ws_bytes / 32;
+        const size_t nb = c->ws_blocks.size();
+        for (size_t k = 0; k < nb; ++k) {
+            const size_t i = big ? nb - 1 - k : k;
+            if (c->ws_blocks[i].used || c->ws_blocks[i].size < need) continue;
+            size_t at = i;
+            if (c->ws_blocks[i].size > need) {
+                const uint64_t off = c->ws_blocks[i].off, size = c->ws_blocks[i].size;
+                if (big) {  // [free rest][this allocation]
+                    c->ws_blocks[i].size = size - need;
+                    c->ws_blocks.insert(c->ws_blocks.begin() + i + 1, md_ctx::WsBlock{off + size - need, need, false});
+                    at = i + 1;
+                } else {    // [this allocation][free rest]
+                    c->ws_blocks[i].size = need;
+                    c->ws_blocks.insert(c->ws_blocks.begin() + i + 1, md_ctx::WsBlock{off + need, size - need, false});
+                }
             }
-            c->ws_blocks[i].used = true;
-            *p = c->ws_base + c->ws_blocks[i].off;
+            c->ws_blocks[at].used = true;
+            *p = c->ws_base + c->ws_blocks[at].off;
             c->device_bytes += need;
-            c->ws_peak = std::max(c->ws_peak, c->ws_blocks[i].off + need);
+            c->ws_peak = std::max(c->ws_peak, c->ws_blocks[at].off + need);
             return MD_OK;
         }
         c->err = "workspace too small: " + std::to_string(bytes) + " more bytes needed, " + std::to_string(c->device_bytes) +
@@ -343,6 +354,40 @@ int build_cell_order(md_ctx *c)
 // =====================================================================================================
 // lifetime
 // =====================================================================================================
+// cell grid and geometry record of a skin r_buff (md_create; md_tune_rbuff changes it on a live context)
+static int set_geometry(md_ctx *c, double r_buff)
+{
+    const double r_list = c->rc + r_buff;
+    uint64_t ncell = 1;
+    uint32_t dims[3];
+    for (int a = 0; a < 3; ++a) {
+        const double n = floor(c->box[a] / r_list);
+        if (!(c->box[a] > 0.0) || n < 3.0 || n > 2097151.0) {
+            c->err = "box too small for the 27-cell stencil (need floor(L/(rc+r_buff)) >= 3 per axis)";
+            return MD_EINVAL;
+        }
+        dims[a] = (uint32_t)n;
+        ncell *= dims[a];
+    }
+    if (ncell >= 0xfffffff0ull) { c->err = "too many cells"; return MD_EINVAL; }
+    c->r_buff = r_buff;
+    c->r_list = r_list;
+    for (int a = 0; a < 3; ++a) {
+        c->dims[a] = dims[a];
+        c->g.L[a] = c->box[a];
+        c->g.h[a] = 0.5 * c->box[a];
+        c->g.lo[a] = -0.5 * c->box[a];
+        c->g.n[a] = dims[a];
+        c->g.dn[a] = (double)dims[a];
+        c->g.cw[a] = c->box[a] / (double)dims[a];
+    }
+    c->n_cells = (uint32_t)ncell;
+    c->g.n_cells = c->n_cells;
+    c->g.N = (uint32_t)c->N;
+    set_record_grid(c, 1);
+    return MD_OK;
+}
+
 static void set_default_cfg(md_ctx *c)
 {
     for (int k = 0; k < MD_N_KERNELS; ++k) c->cfg[k] = LaunchCfg{128, 1, 0.f};
@@ -411,36 +456,13 @@ extern "C" int md_create(md_ctx **out, const double box[3], uint64_t N, double r
     memset(&c->stats, 0, sizeof(c->stats));
     c->N = N;
     c->rc = rc;
-    c->r_buff = r_buff;
-    c->r_list = rc + r_buff;
     c->precision = MD_FP64;
     c->order = MD_ORDER_LEX;
     c->sched = MD_SCHED_SPECULATIVE;
     c->stream = 0;
     c->log = getenv("B200MD_LOG") != nullptr;
-    uint64_t ncell = 1;
-    for (int a = 0; a < 3; ++a) {
-        c->box[a] = box[a];
-        double n = floor(box[a] / c->r_list);
-        if (!(box[a] > 0.0) || n < 3.0 || n > 2097151.0) {
-            g_create_err = "md_create: box too small for the 27-cell stencil (need floor(L/(rc+r_buff)) >= 3 per axis)";
-            delete c;
-            return MD_EINVAL;
-        }
-        c->dims[a] = (uint32_t)n;
-        ncell *= c->dims[a];
-        c->g.L[a] = box[a];
-        c->g.h[a] = 0.5 * box[a];
-        c->g.lo[a] = -0.5 * box[a];
-        c->g.n[a] = c->dims[a];
-        c->g.dn[a] = (double)c->dims[a];
-        c->g.cw[a] = c->box[a] / (double)c->dims[a];
-    }
-    if (ncell >= 0xfffffff0ull) { g_create_err = "md_create: too many cells"; delete c; return MD_EINVAL; }
-    c->n_cells = (uint32_t)ncell;
-    c->g.n_cells = c->n_cells;
-    c->g.N = (uint32_t)N;
-    set_record_grid(c, 1);
+    for (int a = 0; a < 3; ++a) c->box[a] = box[a];
+    if (set_geometry(c, r_buff) != MD_OK) { g_create_err = c->err; delete c; return MD_EINVAL; }
     set_default_cfg(c);
 
     *out = c;
@@ -1217,6 +1239,103 @@ extern "C" int md_tune(md_ctx *c, const md_step_desc *w, int full)
     return tune_all(c, w, full ? 1 : 0);
 }
 
+// ---- the skin that gives the most time steps per second -------------------
+static int set_rbuff(md_ctx *c, double r_buff)
+{
+    MD_TRY(md_sync(c));
+    MD_TRY(set_geometry(c, r_buff));
+    md_free(c, c->cell_count);
+    md_free(c, c->cell_start);
+    c->cell_count = c->cell_start = nullptr;
+    MD_TRY(md_alloc(c, (void **)&c->cell_count, (uint64_t)c->n_cells * sizeof(uint32_t)));
+    MD_TRY(md_alloc(c, (void **)&c->cell_start, ((uint64_t)c->n_cells + 1) * sizeof(uint32_t)));
+    MD_TRY(build_cell_order(c));
+    if (c->nl16) { md_free(c, c->nl16); c->nl16 = nullptr; }
+    c->nl_stride = 0;
+    c->cells_valid = c->nlist_valid = false;
+    return MD_OK;
+}
+
+extern "C" int md_tune_rbuff(md_ctx *c, const md_step_desc *w, const double *candidates, uint32_t n_candidates,
+                             uint64_t burst_steps, double *chosen)
+{
+    if (!c || !w) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_tune_rbuff: md_set_state first"; return MD_ESTATE; }
+    if (burst_steps == 0) burst_steps = 200;
+    std::vector<double> cand;
+    if (candidates && n_candidates) cand.assign(candidates, candidates + n_candidates);
+    else for (double f : {0.5, 0.75, 1.0, 1.25, 1.5, 1.75, 2.0}) cand.push_back(f * (c->r_buff > 0.0 ? c->r_buff : 0.1 * c->rc));
+    // the live state, saved in slot order (a consistent set of arrays) and restored after every burst
+    const uint64_t N = c->N;
+    struct Save { void *src; uint64_t bytes; void *copy; };
+    std::vector<Save> sv = {{c->pos, N * sizeof(double4), nullptr},   {c->vel, N * sizeof(double4), nullptr},
+                            {c->force, N * sizeof(double4), nullptr}, {c->image, 3 * N * sizeof(int), nullptr},
+                            {c->tag, N * sizeof(uint32_t), nullptr},  {c->rtag, N * sizeof(uint32_t), nullptr},
+                            {c->nvt_state, 4 * sizeof(double), nullptr}};
+    int s = MD_OK;
+    for (auto &v : sv) {
+        if (s == MD_OK) s = md_alloc(c, &v.copy, v.bytes);
+        if (s == MD_OK && cudaMemcpyAsync(v.copy, v.src, v.bytes, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess) s = MD_ECUDA;
+    }
+    const uint64_t step0 = c->step;
+    const bool fvalid = c->force_valid, evalid = c->energy_valid;
+    const md_stats stats0 = c->stats;
+    const double r0 = c->r_buff;
+    auto restore = [&]() -> int {
+        // the binning swaps the array twins: copy into whatever the context points at now
+        void *dst[7] = {c->pos, c->vel, c->force, c->image, c->tag, c->rtag, c->nvt_state};
+        for (size_t i = 0; i < sv.size(); ++i)
+            MD_CUDA_CHECK(c, cudaMemcpyAsync(dst[i], sv[i].copy, sv[i].bytes, cudaMemcpyDeviceToDevice, c->stream));
+        c->step = step0;
+        c->force_valid = fvalid;
+        c->energy_valid = evalid;
+        c->cells_valid = c->nlist_valid = false;
+        c->last_d2 = 0.f;
+        c->d2_rate = 0.0;
+        return MD_OK;
+    };
+    double best_r = r0, best_tps = 0.0;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (s == MD_OK && (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess)) s = MD_ECUDA;
+    for (size_t k = 0; k < cand.size() && s == MD_OK; ++k) {
+        if (!(cand[k] >= 0.0) || set_rbuff(c, cand[k]) != MD_OK) continue;  // skins the box cannot hold are skipped
+        s = md_step(c, w, std::max<uint64_t>(10, burst_steps / 10));        // first list build + a few rebuilds, untimed
+        if (s == MD_OK) {
+            cudaEventRecord(e0, c->stream);
+            s = md_step(c, w, burst_steps);
+            cudaEventRecord(e1, c->stream);
+        }
+        if (s == MD_ENOMEM) {  // a skin whose list does not fit the caller's workspace is not a candidate
+            if (c->log) fprintf(stderr, "[b200md tuner] r_buff=%.4f  skipped: %s\n", cand[k], c->err.c_str());
+            cudaStreamSynchronize(c->stream);
+            s = restore();
+            continue;
+        }
+        if (s != MD_OK) break;
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double tps = 1e3 * (double)burst_steps / ms;
+        if (c->log) fprintf(stderr, "[b200md tuner] r_buff=%.4f  %10.1f steps/s\n", cand[k], tps);
+        if (tps > best_tps) { best_tps = tps; best_r = cand[k]; }
+        s = restore();
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    int s2 = set_rbuff(c, best_r);   // (also when a burst failed: back to a valid configuration and the saved state)
+    if (s2 == MD_OK) s2 = restore();
+    if (s2 == MD_OK) s2 = md_sync(c);
+    for (auto &v : sv) if (v.copy) md_free(c, v.copy);
+    const uint64_t launches = c->stats.launches;
+    c->stats = stats0;               // the bursts are not steps or rebuilds of the run
+    c->stats.launches = launches;
+    c->stats.r_buff = c->r_buff;
+    c->stats.rbuff_tuned_tps = best_tps;
+    if (c->log) fprintf(stderr, "[b200md tuner] r_buff -> %.4f (%.1f steps/s)\n", best_r, best_tps);
+    if (chosen) *chosen = best_r;
+    return s != MD_OK ? s : s2;
+}
+
 extern "C" int md_set_option(md_ctx *c, int option, int64_t value)
 {
     if (!c) return MD_EINVAL;
@@ -1275,6 +1394,7 @@ extern "C" int md_get_stats(md_ctx *c, md_stats *out)
         c->stats.mean_neighbors = c->N ? (double)c->nl_exact_entries / (double)c->N : 0.0;
     }
     for (int a = 0; a < 3; ++a) c->stats.dims[a] = c->dims[a];
+    c->stats.r_buff = c->r_buff;
     for (int k = 0; k < MD_N_KERNELS; ++k) {
         c->stats.block[k] = std::min(c->cfg[k].block, md_block_limit(c, k));  // the launched size
         c->stats.w[k] = c->cfg[k].w;

@@ -737,3 +737,42 @@ def test_caller_workspace_bit_identical_and_enomem():
         B.from_workload(wl, workspace=small)
     md = B.MD(wl.box, wl.N, wl.rc, wl.r_buff)               # after md_configure the workspace can no longer be set
     assert md.L.md_set_workspace(md.h, small.data_ptr(), small.numel()) == -2
+
+
+def test_tune_rbuff_keeps_the_state_and_the_trajectory():
+    """md_tune_rbuff: bursts over candidate skins start from the same saved state; afterwards state,
+    step counter and statistics are untouched, the chosen skin is one of the candidates and is reported, skins the box
+    cannot hold are skipped, and the run that follows matches the oracle (forces never depend on the skin)."""
+    wl = inputs.dpd_fluid(3000, pos_seed=4, vel_seed=5)                  # L = 10: at most r_list = 3.33
+    desc = B.step_desc("dpd", wl.dt, wl.params)
+    md = B.from_workload(wl)
+    md.step(desc, 5)
+    p0, v0, i0 = md.get_state()
+    st0 = md.stats()
+    cands = [0.2, 0.4, 0.6, 0.8, 5.0]                                    # 5.0: floor(10 / 6) = 1 cell -> skipped
+    rb = md.tune_rbuff(desc, cands, 40)
+    assert rb in cands[:4]
+    p1, v1, i1 = md.get_state()
+    assert np.array_equal(p0, p1) and np.array_equal(v0, v1) and np.array_equal(i0, i1)
+    st1 = md.stats()
+    assert st1["steps"] == st0["steps"] == 5 and st1["rebuilds"] == st0["rebuilds"] and st1["r_buff"] == rb
+    assert st1["rbuff_tuned_tps"] > 0
+    md.step(desc, 10)
+    q = wl.params
+    sim = oracle.Sim(wl.pos, wl.vel, wl.box, wl.rc, wl.r_buff,
+                     {"dpd": dict(A=q["A"], gamma=q["gamma"], kT=q["kT"], seed=q["seed"])}).run(15, wl.dt)
+    p2, _, _ = md.get_state()
+    assert np.abs(min_image_diff(p2, sim.pos, wl.box)).max() < 1e-9
+    # the list is the one of the chosen skin
+    md.build_nlist()
+    assert np.array_equal(sort_pairs(md.get_nlist()), oracle.neighbor_pairs(p2, wl.box, wl.rc + rb))
+    # LJ mixed with the tile path and a torch workspace
+    wj = inputs.lj_fcc(9, rc=3.0, r_buff=0.4, kT=1.2, jitter=0.05, pos_seed=2, vel_seed=3)
+    mj = B.from_workload(wj, precision=B.MD_MIXED, workspace="torch")
+    dj = B.step_desc("lj", wj.dt, wj.params)
+    mj.step(dj, 3)
+    a = mj.get_state()[0]
+    rj = mj.tune_rbuff(dj, None, 30)
+    assert 0.2 <= rj <= 0.8 and np.array_equal(a, mj.get_state()[0])
+    F, pos, _ = _step_forces(mj, dj, 10)
+    assert force_rel_err(F, oracle.forces_lj(pos, wj.box, wj.rc)[0]) < 1e-4
