@@ -142,6 +142,88 @@ def forces_bonds(pos, box, bonds, k, r0, force=None, energy=None):
     return F, E
 
 
+# ---- virial / pressure and further force fields (md_oracle_ext.c) ------------------------------------
+PAIR_KINDS = {"lj": 0, "yukawa": 1, "gaussian": 2, "morse": 3}
+
+
+def _p4(params):
+    p = np.zeros(4)
+    p[:len(params)] = params
+    return p, p.ctypes.data_as(_dp)
+
+
+def pair_forces(pos, box, rc, kind, params, energy_shift=1):
+    """kind: "lj" (eps, sigma) | "yukawa" (eps, kappa) | "gaussian" (eps, sigma) | "morse" (D0, alpha, r0)."""
+    pos, pp = _d(pos)
+    b, bp = _box(box)
+    p, ppar = _p4(params)
+    N = pos.shape[0]
+    F = np.zeros((N, 3)); E = np.zeros(N)
+    lib().orc_pair_forces(pp, C.c_uint64(N), bp, C.c_double(rc), C.c_int(PAIR_KINDS[kind]), ppar, C.c_int(energy_shift),
+                          F.ctypes.data_as(_dp), E.ctypes.data_as(_dp))
+    return F, E
+
+
+def virial_pair(pos, box, rc, kind, params):
+    """W (xx, yy, zz, xy, xz, yz) = sum over pairs of d (x) F."""
+    pos, pp = _d(pos)
+    b, bp = _box(box)
+    p, ppar = _p4(params)
+    W = np.zeros(6)
+    lib().orc_virial_pair(pp, C.c_uint64(pos.shape[0]), bp, C.c_double(rc), C.c_int(PAIR_KINDS[kind]), ppar,
+                          W.ctypes.data_as(_dp))
+    return W
+
+
+def virial_dpd(pos, vel, box, rc, A, gamma, kT, dt, step, seed):
+    pos, pp = _d(pos)
+    vel, vp = _d(vel)
+    b, bp = _box(box)
+    W = np.zeros(6)
+    lib().orc_virial_dpd(pp, vp, C.c_uint64(pos.shape[0]), bp, C.c_double(rc), C.c_double(A), C.c_double(gamma),
+                         C.c_double(kT), C.c_double(dt), C.c_uint64(step), C.c_uint64(seed), W.ctypes.data_as(_dp))
+    return W
+
+
+def forces_bonds_kind(pos, box, bonds, kind, k, r0, force=None, energy=None, virial=None):
+    """kind: "harmonic" | "fene".  Accumulates into force / energy / virial (fresh zero arrays if None)."""
+    pos, pp = _d(pos)
+    b, bp = _box(box)
+    N = pos.shape[0]
+    bonds = np.ascontiguousarray(bonds, dtype=np.uint32).reshape(-1, 2)
+    ta, tap = _u(bonds[:, 0])
+    tb, tbp = _u(bonds[:, 1])
+    F = np.zeros((N, 3)) if force is None else force
+    E = np.zeros(N) if energy is None else energy
+    W = np.zeros(6) if virial is None else virial
+    lib().orc_forces_bonds_kind(pp, C.c_uint64(N), bp, tap, tbp, C.c_uint64(bonds.shape[0]),
+                                C.c_int({"harmonic": 0, "fene": 1}[kind]), C.c_double(k), C.c_double(r0),
+                                F.ctypes.data_as(_dp), E.ctypes.data_as(_dp), W.ctypes.data_as(_dp))
+    return F, E, W
+
+
+def forces_angles(pos, box, angles, k, theta0, force=None, energy=None, virial=None):
+    """angles: (n, 3) tags (a, b, c), b the vertex.  Accumulates; returns (force, energy, virial)."""
+    pos, pp = _d(pos)
+    b, bp = _box(box)
+    N = pos.shape[0]
+    ang = np.ascontiguousarray(angles, dtype=np.uint32).reshape(-1, 3)
+    ta, tap = _u(ang[:, 0]); tb, tbp = _u(ang[:, 1]); tc, tcp = _u(ang[:, 2])
+    F = np.zeros((N, 3)) if force is None else force
+    E = np.zeros(N) if energy is None else energy
+    W = np.zeros(6) if virial is None else virial
+    lib().orc_forces_angles(pp, C.c_uint64(N), bp, tap, tbp, tcp, C.c_uint64(ang.shape[0]), C.c_double(k),
+                            C.c_double(theta0), F.ctypes.data_as(_dp), E.ctypes.data_as(_dp), W.ctypes.data_as(_dp))
+    return F, E, W
+
+
+def pressure(vel, box, W, mass=None):
+    """P = (2 K + tr W) / (3 V)  (virial theorem, R32)."""
+    m = 1.0 if mass is None else np.asarray(mass)[:, None]
+    K = 0.5 * float(np.sum(m * np.asarray(vel) ** 2))
+    return (2.0 * K + W[0] + W[1] + W[2]) / (3.0 * float(np.prod(np.broadcast_to(box, (3,)))))
+
+
 def vv_half1(pos, vel, image, force, box, dt, mass=None):
     """In place on pos, vel, image (C-contiguous float64 / int32 arrays)."""
     b, bp = _box(box)

@@ -1,0 +1,219 @@
+/*
+ * md_oracle_ext.c -- ORACLE (test infrastructure), second file: the rows of SURVEY.md 8(f) that go beyond the five
+ * configurations -- virial / pressure (row 1) and further short-range force fields (row 3).  Same rules as
+ * md_oracle.c: plain C, single thread, fp64, O(N^2) over all pairs or a plain loop over the bonded terms, no cells, no
+ * lists, no blocking; shares no code with the CUDA path (paper_1412_3387_b200/csrc); only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline may call it.  Built with -ffp-contract=off.
+ *
+ * The paper names these features and prints no formula (pair potentials "Lennard-Jones, Gaussian, Morse,
+ * Yukawa", bonds "harmonic, FENE", "angle, dihedral"; NPT/NPH integrators need the pressure),
+ * so each function states the textbook form it takes (R31-R36).
+ *
+ * Pins (tests/test_oracle_ext.py; no function here is "parity unpinned"):
+ *   orc_pair_forces    Yukawa/Gaussian/Morse: closed-form values, F = -dU/dr by central differences, strict cut-off,
+ *                      Newton's third law, kind 0 (LJ) equal to orc_forces_lj
+ *   orc_virial_pair    two-body closed form r F(r); ideal gas (no forces) P = rho kT; tr W = -3 V dU/dV by a
+ *                      finite-difference box rescale; symmetric tensor; DPD equation of state (weak, statistical)
+ *   orc_forces_fene    closed form, gradient, divergence at r -> r0, Newton
+ *   orc_virial_bonds   two-body closed form, -3 V dU/dV
+ *   orc_forces_angles  zero force at theta0, closed form for a right angle, gradient, zero net force and torque
+ */
+#include <math.h>
+#include <stdint.h>
+#include <string.h>
+
+/* minimum image and squared distance: restated here (R8), the two oracle files share no helper */
+static double minimg(double d, double L)
+{
+    double h = 0.5 * L;
+    if (d >= h) d -= L;
+    else if (d < -h) d += L;
+    return d;
+}
+
+static double sep(const double *xa, const double *xb, const double box[3], double d[3])
+{
+    d[0] = minimg(xa[0] - xb[0], box[0]);
+    d[1] = minimg(xa[1] - xb[1], box[1]);
+    d[2] = minimg(xa[2] - xb[2], box[2]);
+    return (d[0] * d[0] + d[1] * d[1]) + d[2] * d[2];
+}
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * R31 pair potentials, pairs with r^2 < rc^2 (strict), f = -(dU/dr)/r so that F_a = f d, d = minimg(x_a - x_b):
+ *   kind 0  Lennard-Jones  U = 4 p0 ((p1/r)^12 - (p1/r)^6)                      (R1; p0 = epsilon, p1 = sigma)
+ *   kind 1  Yukawa         U = p0 exp(-p1 r) / r                                (p0 = epsilon, p1 = kappa)
+ *   kind 2  Gaussian       U = p0 exp(-r^2 / (2 p1^2))                          (p0 = epsilon, p1 = sigma)
+ *   kind 3  Morse          U = p0 (exp(-2 p1 (r - p2)) - 2 exp(-p1 (r - p2)))   (p0 = D0, p1 = alpha, p2 = r0)
+ * energy_shift: U - U(rc).  Returns f and writes U (unshifted) to *u.
+ * ---------------------------------------------------------------------------------------------------------------- */
+static double pair_term(int kind, double r2, const double p[4], double *u)
+{
+    double r = sqrt(r2);
+    if (kind == 0) {
+        double s2 = p[1] * p[1] / r2, s6 = s2 * s2 * s2, s12 = s6 * s6;
+        *u = 4.0 * p[0] * (s12 - s6);
+        return 24.0 * p[0] * (2.0 * s12 - s6) / r2;
+    }
+    if (kind == 1) {
+        double e = p[0] * exp(-p[1] * r);
+        *u = e / r;
+        return e * (p[1] * r + 1.0) / (r2 * r);
+    }
+    if (kind == 2) {
+        double e = p[0] * exp(-r2 / (2.0 * p[1] * p[1]));
+        *u = e;
+        return e / (p[1] * p[1]);
+    }
+    {
+        double e1 = exp(-p[1] * (r - p[2])), e2 = e1 * e1;
+        *u = p[0] * (e2 - 2.0 * e1);
+        return 2.0 * p[1] * p[0] * (e2 - e1) / r;
+    }
+}
+
+/* force (N*3) and energy (N, may be NULL; half of each pair energy to each particle) are OVERWRITTEN */
+void orc_pair_forces(const double *pos, uint64_t N, const double box[3], double rc, int kind, const double p[4],
+                     int energy_shift, double *force, double *energy)
+{
+    double rc2 = rc * rc, uc = 0.0, d[3], u;
+    if (energy_shift) (void)pair_term(kind, rc2, p, &uc);
+    memset(force, 0, sizeof(double) * 3 * N);
+    if (energy) memset(energy, 0, sizeof(double) * N);
+    for (uint64_t a = 0; a < N; ++a)
+        for (uint64_t b = a + 1; b < N; ++b) {
+            double r2 = sep(pos + 3 * a, pos + 3 * b, box, d);
+            if (r2 < rc2 && r2 > 0.0) {
+                double f = pair_term(kind, r2, p, &u);
+                for (int k = 0; k < 3; ++k) { force[3 * a + k] += f * d[k]; force[3 * b + k] -= f * d[k]; }
+                if (energy) { energy[a] += 0.5 * (u - uc); energy[b] += 0.5 * (u - uc); }
+            }
+        }
+}
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * R32 virial of the pair forces: W_ab = sum over pairs of d_a F_b (F = force on the first particle of the pair, d its
+ * separation from the second), order xx, yy, zz, xy, xz, yz.  The pressure follows as
+ *   P = (2 K + W_xx + W_yy + W_zz) / (3 V),  K = sum 1/2 m v^2     (virial theorem; NPT/NPH of PAPER.md:63 need it).
+ * ---------------------------------------------------------------------------------------------------------------- */
+static void add_virial(double W[6], const double d[3], const double F[3])
+{
+    W[0] += d[0] * F[0]; W[1] += d[1] * F[1]; W[2] += d[2] * F[2];
+    W[3] += d[0] * F[1]; W[4] += d[0] * F[2]; W[5] += d[1] * F[2];
+}
+
+void orc_virial_pair(const double *pos, uint64_t N, const double box[3], double rc, int kind, const double p[4],
+                     double W[6])
+{
+    double rc2 = rc * rc, d[3], u, F[3];
+    memset(W, 0, sizeof(double) * 6);
+    for (uint64_t a = 0; a < N; ++a)
+        for (uint64_t b = a + 1; b < N; ++b) {
+            double r2 = sep(pos + 3 * a, pos + 3 * b, box, d);
+            if (r2 < rc2 && r2 > 0.0) {
+                double f = pair_term(kind, r2, p, &u);
+                F[0] = f * d[0]; F[1] = f * d[1]; F[2] = f * d[2];
+                add_virial(W, d, F);
+            }
+        }
+}
+
+/* DPD (R9): the virial of all three terms of the pair force, as orc_forces_dpd evaluates them:
+ * F = fs rhat, fs = A w - gamma w^2 (rhat . v_ab) + sqrt(2 gamma kT) w theta_ab / sqrt(dt); theta_ab is orc_dpd_theta of
+ * md_oracle.c (the two files are linked into one library). */
+double orc_dpd_theta(uint32_t tag_a, uint32_t tag_b, uint64_t step, uint64_t seed);
+void orc_virial_dpd(const double *pos, const double *vel, uint64_t N, const double box[3], double rc, double A,
+                    double gamma, double kT, double dt, uint64_t step, uint64_t seed, double W[6])
+{
+    double rc2 = rc * rc, d[3], F[3];
+    memset(W, 0, sizeof(double) * 6);
+    for (uint64_t a = 0; a < N; ++a)
+        for (uint64_t b = a + 1; b < N; ++b) {
+            double r2 = sep(pos + 3 * a, pos + 3 * b, box, d);
+            if (r2 < rc2 && r2 > 0.0) {
+                double r = sqrt(r2), w = 1.0 - r / rc;
+                double rh[3] = {d[0] / r, d[1] / r, d[2] / r};
+                double rv = rh[0] * (vel[3 * a] - vel[3 * b]) + rh[1] * (vel[3 * a + 1] - vel[3 * b + 1]) +
+                            rh[2] * (vel[3 * a + 2] - vel[3 * b + 2]);
+                double fs = A * w - gamma * w * w * rv +
+                            sqrt(2.0 * gamma * kT) * w * orc_dpd_theta((uint32_t)a, (uint32_t)b, step, seed) / sqrt(dt);
+                F[0] = fs * rh[0]; F[1] = fs * rh[1]; F[2] = fs * rh[2];
+                add_virial(W, d, F);
+            }
+        }
+}
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * R33 bonds: kind 0 harmonic U = k/2 (r - r0)^2 (R19);  kind 1 FENE U = -1/2 k r0^2 ln(1 - (r/r0)^2), r < r0
+ * (Kremer-Grest form without the WCA part, which is a pair potential here): F_a = -k d / (1 - r^2/r0^2).  r >= r0 gives
+ * NaN (the bond is broken: the caller's time step was too long).  force / energy are ACCUMULATED, W (may be NULL) too.
+ * ---------------------------------------------------------------------------------------------------------------- */
+void orc_forces_bonds_kind(const double *pos, uint64_t N, const double box[3], const uint32_t *tag_a,
+                           const uint32_t *tag_b, uint64_t n_bonds, int kind, double k, double r0, double *force,
+                           double *energy, double *W)
+{
+    (void)N;
+    double d[3], F[3];
+    for (uint64_t m = 0; m < n_bonds; ++m) {
+        uint64_t a = tag_a[m], b = tag_b[m];
+        double r2 = sep(pos + 3 * a, pos + 3 * b, box, d);
+        if (!(r2 > 0.0)) continue;
+        double f, u;
+        if (kind == 0) {
+            double r = sqrt(r2);
+            f = -k * (r - r0) / r;
+            u = 0.5 * k * (r - r0) * (r - r0);
+        } else {
+            double x = r2 / (r0 * r0);
+            f = x < 1.0 ? -k / (1.0 - x) : NAN;
+            u = x < 1.0 ? -0.5 * k * r0 * r0 * log(1.0 - x) : NAN;
+        }
+        F[0] = f * d[0]; F[1] = f * d[1]; F[2] = f * d[2];
+        if (force)
+            for (int c = 0; c < 3; ++c) { force[3 * a + c] += F[c]; force[3 * b + c] -= F[c]; }
+        if (energy) { energy[a] += 0.5 * u; energy[b] += 0.5 * u; }
+        if (W) add_virial(W, d, F);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * R34 harmonic angles: triplet (a, b, c) with b the vertex, r1 = minimg(x_a - x_b), r2 = minimg(x_c - x_b),
+ * cos(theta) = r1.r2 / (|r1| |r2|), U = k/2 (theta - theta0)^2,
+ *   F_a = (k (theta - theta0) / sin(theta)) (r2 / (|r1||r2|) - cos(theta) r1 / |r1|^2),  F_c likewise with 1 <-> 2,
+ *   F_b = -F_a - F_c.  sin(theta) < 1e-12 (collinear): the term is skipped.  One third of U to each particle.
+ * force / energy ACCUMULATED; W (may be NULL) += r1 (x) F_a + r2 (x) F_c.
+ * ---------------------------------------------------------------------------------------------------------------- */
+void orc_forces_angles(const double *pos, uint64_t N, const double box[3], const uint32_t *tag_a, const uint32_t *tag_b,
+                       const uint32_t *tag_c, uint64_t n_angles, double k, double theta0, double *force,
+                       double *energy, double *W)
+{
+    (void)N;
+    double r1[3], r2[3], Fa[3], Fc[3];
+    for (uint64_t m = 0; m < n_angles; ++m) {
+        uint64_t a = tag_a[m], b = tag_b[m], c = tag_c[m];
+        double l1s = sep(pos + 3 * a, pos + 3 * b, box, r1), l2s = sep(pos + 3 * c, pos + 3 * b, box, r2);
+        if (!(l1s > 0.0) || !(l2s > 0.0)) continue;
+        double l1 = sqrt(l1s), l2 = sqrt(l2s);
+        double cs = (r1[0] * r2[0] + r1[1] * r2[1] + r1[2] * r2[2]) / (l1 * l2);
+        if (cs > 1.0) cs = 1.0;
+        if (cs < -1.0) cs = -1.0;
+        double sn = sqrt(1.0 - cs * cs);
+        if (sn < 1e-12) continue;
+        double th = acos(cs), g = k * (th - theta0) / sn;
+        for (int x = 0; x < 3; ++x) {
+            Fa[x] = g * (r2[x] / (l1 * l2) - cs * r1[x] / l1s);
+            Fc[x] = g * (r1[x] / (l1 * l2) - cs * r2[x] / l2s);
+        }
+        if (force)
+            for (int x = 0; x < 3; ++x) {
+                force[3 * a + x] += Fa[x];
+                force[3 * c + x] += Fc[x];
+                force[3 * b + x] -= Fa[x] + Fc[x];
+            }
+        if (energy) {
+            double u = 0.5 * k * (th - theta0) * (th - theta0) / 3.0;
+            energy[a] += u; energy[b] += u; energy[c] += u;
+        }
+        if (W) { add_virial(W, r1, Fa); add_virial(W, r2, Fc); }
+    }
+}

@@ -1,0 +1,196 @@
+"""Pins of oracle/md_oracle_ext.c: virial / pressure, Yukawa / Gaussian / Morse pairs, FENE
+bonds, harmonic angles -- against closed forms, numerical gradients, invariants and the routines of md_oracle.c they
+must reduce to.  No GPU."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1412_3387_b200 import inputs
+
+BOX = np.array([12.0, 13.0, 14.0])
+
+
+def _two(r, axis=(1.0, 0.0, 0.0), at=(5.5, -6.0, 6.5)):
+    """Two particles a distance r apart along `axis`, straddling the periodic boundary."""
+    a = np.array(at)
+    b = a - r * np.array(axis) / np.linalg.norm(axis)
+    return oracle.wrap(np.stack([a, b]), BOX)
+
+
+# ------------------------------------------------------------------------------------------------- pair potentials
+CLOSED = [  # kind, params, r, U(r), F(r) = -dU/dr  (written out by hand from the textbook forms, R31)
+    ("yukawa", (2.0, 1.5), 1.2, 2.0 * math.exp(-1.8) / 1.2, 2.0 * math.exp(-1.8) * (1.5 * 1.2 + 1.0) / 1.2 ** 2),
+    ("gaussian", (3.0, 0.8), 1.1, 3.0 * math.exp(-1.21 / 1.28), 3.0 * math.exp(-1.21 / 1.28) * 1.1 / 0.64),
+    ("morse", (1.7, 2.0, 1.0), 1.3, 1.7 * (math.exp(-1.2) - 2.0 * math.exp(-0.6)),
+     2.0 * 2.0 * 1.7 * (math.exp(-1.2) - math.exp(-0.6))),
+    ("morse", (1.7, 2.0, 1.0), 1.0, -1.7, 0.0),                      # the minimum: depth D0, zero force
+]
+
+
+@pytest.mark.parametrize("kind,p,r,U,F", CLOSED)
+def test_pair_closed_forms(kind, p, r, U, F):
+    pos = _two(r, axis=(1.0, 2.0, -0.5))
+    Fo, Eo = oracle.pair_forces(pos, BOX, 3.0, kind, p, energy_shift=0)
+    assert abs(Eo.sum() - U) < 1e-14 * max(1.0, abs(U))
+    d = pos[0] - pos[1]
+    d -= BOX * np.rint(d / BOX)
+    assert np.abs(Fo[0] - F * d / r).max() < 1e-13 * max(1.0, abs(F))   # along the separation, repulsive if F > 0
+    assert np.abs(Fo[0] + Fo[1]).max() == 0.0                             # Newton's third law, exactly
+
+
+@pytest.mark.parametrize("kind,p", [("yukawa", (2.0, 1.5)), ("gaussian", (3.0, 0.8)), ("morse", (1.7, 2.0, 1.0)),
+                                     ("lj", (0.9, 1.05))])
+def test_pair_force_is_minus_gradient_and_cutoff_is_strict(kind, p):
+    for r in (0.95, 1.4, 2.2):
+        h = 1e-6
+        U = [oracle.pair_forces(_two(x), BOX, 3.0, kind, p, 0)[1].sum() for x in (r - h, r + h)]
+        F = oracle.pair_forces(_two(r), BOX, 3.0, kind, p, 0)[0][0, 0]
+        assert abs(F + (U[1] - U[0]) / (2 * h)) < 1e-7 * max(1.0, abs(F))
+    rc = 2.0
+    inside, outside = np.nextafter(rc, 0.0), rc
+    assert np.abs(oracle.pair_forces(_two(inside, at=(0.5, 0.0, 0.0)), BOX, rc, kind, p, 0)[0]).max() > 0.0
+    assert np.abs(oracle.pair_forces(_two(outside, at=(0.5, 0.0, 0.0)), BOX, rc, kind, p, 0)[0]).max() == 0.0
+    # the shift removes U(rc): a pair just inside the cut-off has (almost) no energy left
+    assert abs(oracle.pair_forces(_two(inside, at=(0.5, 0.0, 0.0)), BOX, rc, kind, p, 1)[1].sum()) < 1e-12
+
+
+def test_pair_kind0_is_the_lj_routine_and_many_body_sums():
+    w = inputs.lj_fcc(4, rc=2.5, r_buff=0.4, kT=1.0, jitter=0.08, pos_seed=3, vel_seed=4)
+    F0, E0 = oracle.pair_forces(w.pos, w.box, 2.5, "lj", (0.9, 1.05), 1)
+    F1, E1 = oracle.forces_lj(w.pos, w.box, 2.5, 0.9, 1.05, 1)
+    assert np.array_equal(F0, F1) and np.array_equal(E0, E1)
+    for kind, p in (("yukawa", (2.0, 1.5)), ("gaussian", (3.0, 0.8)), ("morse", (1.7, 2.0, 1.0))):
+        F, E = oracle.pair_forces(w.pos, w.box, 2.5, kind, p, 1)
+        assert np.abs(F.sum(axis=0)).max() < 1e-11 * np.abs(F).sum()
+
+
+# ------------------------------------------------------------------------------------------------- virial, pressure
+def test_virial_two_body_and_symmetry():
+    pos = _two(1.2, axis=(1.0, 2.0, -0.5))
+    d = pos[0] - pos[1]
+    d -= BOX * np.rint(d / BOX)
+    F = oracle.pair_forces(pos, BOX, 3.0, "yukawa", (2.0, 1.5), 0)[0][0]
+    W = oracle.virial_pair(pos, BOX, 3.0, "yukawa", (2.0, 1.5))
+    assert np.allclose(W[:3], d * F, rtol=0, atol=1e-15) and np.allclose(W[3:], [d[0] * F[1], d[0] * F[2], d[1] * F[2]], atol=1e-15)
+    assert abs(W[:3].sum() - 1.2 * CLOSED[0][4]) < 1e-13                      # tr W = r F(r)
+    assert abs(d[0] * F[1] - d[1] * F[0]) < 1e-15                             # central force: the tensor is symmetric
+
+
+def test_ideal_gas_pressure_and_virial_theorem_by_box_rescale():
+    w = inputs.lj_fcc(4, rc=2.5, r_buff=0.4, kT=1.3, jitter=0.08, pos_seed=3, vel_seed=4)     # N = 256
+    V = float(np.prod(w.box))
+    assert abs(oracle.pressure(w.vel, w.box, np.zeros(6)) - (w.N - 1) * 1.3 / V) < 1e-12      # P = rho kT ((3N-3) dof, R18)
+    for kind, p in (("lj", (1.0, 1.0)), ("yukawa", (2.0, 1.5)), ("morse", (1.7, 2.0, 1.0))):
+        # tr W = -3 V dU/dV for the UNSHIFTED, smoothly truncated energy: scale box and positions by (1 +- h); pairs
+        # must not cross the cut-off during the rescale, so the cut-off scales along (rc is a length of the system here)
+        W = oracle.virial_pair(w.pos, w.box, 2.5, kind, p)
+        h = 1e-6
+        U = [oracle.pair_forces(w.pos * s, w.box * s, 2.5 * s, kind, p, 0)[1].sum() for s in (1 - h, 1 + h)]
+        dU_dlnV = (U[1] - U[0]) / (2 * h) / 3.0
+        if kind == "lj":                                                       # (sigma does not scale: U really changes)
+            assert abs(W[:3].sum() + 3.0 * dU_dlnV) < 2e-6 * abs(W[:3].sum())
+        else:
+            assert abs(W[:3].sum() + 3.0 * dU_dlnV) < 2e-6 * max(1.0, abs(W[:3].sum()))
+    # perfect FCC: the virial tensor is isotropic and its off-diagonal part vanishes by symmetry
+    f = inputs.lj_fcc(4, rc=2.5, r_buff=0.4)
+    W = oracle.virial_pair(f.pos, f.box, 2.5, "lj", (1.0, 1.0))
+    assert np.abs(W[3:]).max() < 1e-9 * abs(W[0]) and abs(W[0] - W[1]) < 1e-9 * abs(W[0]) and abs(W[1] - W[2]) < 1e-9 * abs(W[0])
+
+
+def test_dpd_virial_reduces_to_the_conservative_pair_form_and_equation_of_state():
+    w = inputs.dpd_fluid(3000, pos_seed=4, vel_seed=5)
+    p = w.params
+    # gamma = 0 switches drag and noise off: F = A (1 - r/rc) rhat, whose virial is sum A (1 - r) r over pairs
+    W = oracle.virial_dpd(w.pos, w.vel, w.box, 1.0, p["A"], 0.0, p["kT"], w.dt, 3, p["seed"])
+    pairs = oracle.neighbor_pairs(w.pos, w.box, 1.0)
+    d = w.pos[pairs[:, 0]] - w.pos[pairs[:, 1]]
+    d -= w.box * np.rint(d / w.box)
+    r = np.sqrt((d * d).sum(1))
+    assert abs(W[:3].sum() - (p["A"] * (1.0 - r) * r).sum()) < 1e-10 * W[:3].sum()
+    # tr W of the full force = sum over pairs of d . F_pair, F from the force routine on a two-particle system
+    Wf = oracle.virial_dpd(w.pos[:2] * 0 + np.array([[0.0, 0, 0], [0.6, 0.1, -0.2]]), w.vel[:2], w.box, 1.0, p["A"], p["gamma"],
+                           p["kT"], w.dt, 7, p["seed"])
+    F2 = oracle.forces_dpd(np.array([[0.0, 0, 0], [0.6, 0.1, -0.2]]), w.vel[:2], w.box, 1.0, p["A"], p["gamma"], p["kT"],
+                           w.dt, 7, p["seed"])
+    assert abs(Wf[:3].sum() - np.dot(np.array([-0.6, -0.1, 0.2]), F2[0])) < 1e-13
+    # Groot-Warren equation of state p = rho kT + 0.101 A rho^2 at rho = 3, A = 25 (= 25.7): weak, statistical pin on the
+    # UNEQUILIBRATED uniform random start (ideal-gas structure: the mean-field value A rho^2 pi/30 = 23.6 + 3)
+    P = oracle.pressure(w.vel, w.box, W)
+    assert abs(P - (3.0 + math.pi / 30.0 * 25.0 * 9.0)) < 0.05 * P
+
+
+# ------------------------------------------------------------------------------------------------- bonds
+def test_fene_closed_form_gradient_and_harmonic_equivalence():
+    k, r0 = 30.0, 1.5
+    for r in (0.4, 0.97, 1.45):
+        pos = _two(r, axis=(0.3, -1.0, 2.0))
+        F, E, W = oracle.forces_bonds_kind(pos, BOX, [[0, 1]], "fene", k, r0)
+        assert abs(E.sum() + 0.5 * k * r0 * r0 * math.log(1.0 - (r / r0) ** 2)) < 1e-12 * max(1.0, abs(E.sum()))
+        Fr = -k * r / (1.0 - (r / r0) ** 2)                                    # attractive: pulls a towards b
+        d = pos[0] - pos[1]
+        d -= BOX * np.rint(d / BOX)
+        assert np.abs(F[0] - Fr * d / r).max() < 1e-12 * abs(Fr) and np.abs(F[0] + F[1]).max() == 0.0
+        assert abs(W[:3].sum() - r * Fr) < 1e-12 * abs(r * Fr)
+        h = 1e-6
+        U = [oracle.forces_bonds_kind(_two(x, axis=(0.3, -1.0, 2.0)), BOX, [[0, 1]], "fene", k, r0)[1].sum() for x in (r - h, r + h)]
+        assert abs(Fr + (U[1] - U[0]) / (2 * h)) < 1e-6 * abs(Fr)
+    assert abs(oracle.forces_bonds_kind(_two(1.4999999), BOX, [[0, 1]], "fene", k, r0)[0][0, 0]) > 1e7   # diverges at r0
+    assert np.isnan(oracle.forces_bonds_kind(_two(1.6), BOX, [[0, 1]], "fene", k, r0)[0]).any()           # broken bond
+    w = inputs.polymer_melt(8, chain_len=16)
+    q = w.params
+    Fh, Eh, Wh = oracle.forces_bonds_kind(w.pos, w.box, w.bonds, "harmonic", q["bond_k"], q["bond_r0"])
+    F1, E1 = oracle.forces_bonds(w.pos, w.box, w.bonds, q["bond_k"], q["bond_r0"])
+    assert np.array_equal(Fh, F1) and np.array_equal(Eh, E1)
+    # bond virial by the box rescale (bond lengths scale with the box)
+    h = 1e-6
+    U = [oracle.forces_bonds(w.pos * s, w.box * s, w.bonds, q["bond_k"], q["bond_r0"])[1].sum() for s in (1 - h, 1 + h)]
+    assert abs(Wh[:3].sum() + (U[1] - U[0]) / (2 * h)) < 1e-6 * abs(Wh[:3].sum())
+
+
+# ------------------------------------------------------------------------------------------------- angles
+def _tri(theta, l1=1.1, l2=0.8):
+    b = np.array([5.8, 6.2, -6.9])                      # vertex next to the periodic boundary
+    a = b + l1 * np.array([1.0, 0.0, 0.0])
+    c = b + l2 * np.array([math.cos(theta), math.sin(theta), 0.0])
+    return oracle.wrap(np.stack([a, b, c]), BOX)
+
+
+def test_angle_zero_at_theta0_right_angle_closed_form_and_energy():
+    k = 12.0
+    F, E, W = oracle.forces_angles(_tri(2.0), BOX, [[0, 1, 2]], k, 2.0)
+    assert np.abs(F).max() < 1e-13 and abs(E.sum()) < 1e-26
+    th, th0 = math.pi / 2, 2.0
+    F, E, W = oracle.forces_angles(_tri(th), BOX, [[0, 1, 2]], k, th0)
+    assert abs(E.sum() - 0.5 * k * (th - th0) ** 2) < 1e-14 and abs(E[0] - E[1]) < 1e-16
+    # at a right angle: |F_a| = k |theta - theta0| / l1, perpendicular to r1, opening the angle (theta < theta0)
+    assert np.abs(F[0] - np.array([0.0, -k * (th0 - th) / 1.1, 0.0])).max() < 1e-13
+    assert np.abs(F[2] - np.array([-k * (th0 - th) / 0.8, 0.0, 0.0])).max() < 1e-13
+    assert np.abs(F.sum(axis=0)).max() < 1e-14
+
+
+def test_angle_gradient_net_force_and_torque():
+    rng = np.random.default_rng(5)
+    w = inputs.polymer_melt(6, chain_len=12)
+    ang = np.array([[12 * c + i, 12 * c + i + 1, 12 * c + i + 2] for c in range(6) for i in range(10)], dtype=np.uint32)
+    k, th0 = 7.0, 1.9
+    F, E, W = oracle.forces_angles(w.pos, w.box, ang, k, th0)
+    assert np.abs(F.sum(axis=0)).max() < 1e-11 * np.abs(F).sum()
+    # torque about the chain's own frame: unwrap each chain, sum r x F per chain = 0
+    for c in range(6):
+        x = w.pos[12 * c:12 * c + 12].copy()
+        for i in range(1, 12):
+            d = x[i] - x[i - 1]
+            x[i] = x[i - 1] + d - w.box * np.rint(d / w.box)
+        assert np.abs(np.cross(x, F[12 * c:12 * c + 12]).sum(axis=0)).max() < 1e-10 * np.abs(F).sum()
+    for _ in range(6):                                   # F = -grad U by central differences on random coordinates
+        i, a = int(rng.integers(0, w.N)), int(rng.integers(0, 3))
+        h = 1e-6
+        U = []
+        for s in (-h, h):
+            p = w.pos.copy(); p[i, a] += s
+            U.append(oracle.forces_angles(p, w.box, ang, k, th0)[1].sum())
+        assert abs(F[i, a] + (U[1] - U[0]) / (2 * h)) < 1e-6 * max(1.0, abs(F[i, a]))
+    h = 1e-6                                             # angles do not change under a uniform rescale: zero virial trace
+    assert abs(W[:3].sum()) < 1e-10 * np.abs(F).sum()
