@@ -263,6 +263,16 @@ def run_ours(args):
         kT = float(w.params.get("kT", 1.2 if args.config == 2 else 1.0))
         nvt = dict(kT=kT, tau=0.5)
         w = dataclasses.replace(w, name=w.name + "-nvt")
+    angles = None
+    if args.angles and w.kind == "polymer":
+        # harmonic angles along the chains of the polymer melt (k = 5, theta0 = 2.0 rad); named in the
+        # workload, not a BASELINE configuration
+        import dataclasses
+        L = 64
+        nc = w.N // L
+        idx = (np.arange(nc, dtype=np.uint32)[:, None] * L + np.arange(L - 2, dtype=np.uint32)[None, :]).reshape(-1)
+        angles = np.stack([idx, idx + 1, idx + 2], axis=1).astype(np.uint32)
+        w = dataclasses.replace(w, name=w.name + "-angles", params=dict(w.params, angle_k=5.0, angle_theta0=2.0))
     desc = B.step_desc(w.kind, w.dt, w.params, nvt=nvt)
 
     # inputs resident in HBM before the timed region
@@ -272,6 +282,8 @@ def run_ours(args):
     md.set_state(d_pos, d_vel)
     if w.bonds is not None:
         md.set_bonds(w.bonds)
+    if angles is not None:
+        md.set_angles(angles)
     if args.cluster:
         md.set_option(B.MD_OPT_CLUSTER, 1)
     if args.brick:
@@ -439,6 +451,7 @@ def main():
     ap.add_argument("--cluster", action="store_true", help="MD_OPT_CLUSTER = 1: one neighbour row per cluster of 4")
     ap.add_argument("--r-buff", type=float, default=None, dest="r_buff",
                     help="override the configured skin r_buff = 0.4 (tuning sweep; not a reported configuration)")
+    ap.add_argument("--angles", action="store_true", help="config 4 with harmonic angles along the chains (SURVEY 8(f) row 3)")
     ap.add_argument("--auto-rbuff", action="store_true", dest="auto_rbuff",
                     help="md_tune_rbuff: let the library choose the skin (tuning run; not a reported configuration)")
     ap.add_argument("--nvt", action="store_true",

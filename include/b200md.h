@@ -65,6 +65,17 @@ typedef enum {
 #define MD_F_DPD 2u
 #define MD_F_BONDS 4u
 #define MD_F_NVT 8u /* md_step integrates with the Nose-Hoover thermostat (md_integrate_nvt) instead of NVE */
+#define MD_F_PAIR 16u   /* a pair potential of SURVEY.md 8(f) row 3 (pair_kind, pair_p) instead of LJ / DPD */
+#define MD_F_ANGLES 32u /* harmonic angles (md_set_angles; angle_k, angle_theta0) */
+
+/* pair potentials of md_forces_pair / MD_F_PAIR (PAPER.md:63 lists them, R31); parameters p[0..2] */
+enum { MD_PAIR_LJ = 0,       /* U = 4 p0 ((p1/r)^12 - (p1/r)^6)                        p0 = epsilon, p1 = sigma     */
+       MD_PAIR_YUKAWA = 1,   /* U = p0 exp(-p1 r) / r                                  p0 = epsilon, p1 = kappa     */
+       MD_PAIR_GAUSSIAN = 2, /* U = p0 exp(-r^2 / (2 p1^2))                            p0 = epsilon, p1 = sigma     */
+       MD_PAIR_MORSE = 3 };  /* U = p0 (exp(-2 p1 (r - p2)) - 2 exp(-p1 (r - p2)))     p0 = D0, p1 = alpha, p2 = r0 */
+/* bond potentials (R19, R33) */
+enum { MD_BOND_HARMONIC = 0, /* U = k/2 (r - r0)^2 */
+       MD_BOND_FENE = 1 };   /* U = -1/2 k r0^2 ln(1 - (r/r0)^2), r < r0 (r >= r0: NaN, the bond is broken) */
 
 /* scheduling of md_step */
 #define MD_SCHED_SYNC 0        /* the host waits for the rebuild flag of half 1 before it enqueues the forces */
@@ -81,6 +92,10 @@ typedef struct {
     uint64_t dpd_seed;
     double bond_k, bond_r0;
     double nvt_kT, nvt_tau; /* MD_F_NVT: target temperature (k_B T0) and thermostat period tau */
+    int32_t pair_kind;      /* MD_F_PAIR: MD_PAIR_*; the energy shift is lj_energy_shift */
+    int32_t bond_kind;      /* MD_F_BONDS: MD_BOND_* (0 = harmonic) */
+    double pair_p[4];       /* MD_F_PAIR: parameters of the pair potential */
+    double angle_k, angle_theta0; /* MD_F_ANGLES: U = k/2 (theta - theta0)^2, theta0 in radians */
 } md_step_desc;
 
 #define MD_N_KERNELS 8
@@ -202,6 +217,35 @@ int md_forces_dpd(md_ctx *ctx, double A, double gamma, double kT, double dt, uin
 /* Harmonic bonds U = k/2 (r - r0)^2 (R6).  ACCUMULATES into force/energy. */
 int md_forces_bonds(md_ctx *ctx, double k, double r0);
 
+/* ---- further short-range force fields (PAPER.md:63 feature list; fp64) ---------------------- */
+
+/* Pair potential `kind` (MD_PAIR_*) with parameters p[4] (HOST pointer), pairs with r^2 < rc^2 (strict), energies shifted
+   by U(rc) if energy_shift.  Same kernel structure as md_forces_lj (w threads per particle over the row, shuffle
+   reduction, one write), on the exact 32-bit list.  OVERWRITES force/energy.  fp64 in both precision modes. */
+int md_forces_pair(md_ctx *ctx, int kind, const double p[4], int energy_shift);
+
+/* FENE bonds on the bond table of md_set_bonds (R33).  ACCUMULATES, like md_forces_bonds. */
+int md_forces_fene(md_ctx *ctx, double k, double r0);
+
+/* Harmonic angles (R34): triplets of tags (a, b, c), b the vertex; theta = angle between x_a - x_b and x_c - x_b
+   (minimum image), U = k/2 (theta - theta0)^2, one third of it to each particle's energy; collinear triplets
+   (sin theta < 1e-12) are skipped.  Stored per particle (every particle sums the terms it takes part in: no atomics).
+   n_angles = 0 clears.  md_forces_angles ACCUMULATES. */
+int md_set_angles(md_ctx *ctx, const uint32_t *tag_a, const uint32_t *tag_b, const uint32_t *tag_c, uint64_t n_angles);
+int md_forces_angles(md_ctx *ctx, double k, double theta0);
+
+/* ---- virial and pressure (PAPER.md:63 NPT / NPH, :208, :214; R32) ----------------------------- */
+
+/* W = sum over the pairs of `what`'s pair term of d (x) F (d = minimum-image separation, F the pair force on the first
+   particle; for MD_F_DPD all three terms with hash counter = the context's current step), plus bonds and angles (arm (x) F
+   per end) if flagged; order xx, yy, zz, xy, xz, yz.  kinetic = sum 1/2 m v^2, volume = box volume,
+   pressure = (2 kinetic + W_xx + W_yy + W_zz) / (3 volume).  Evaluated on demand at the current positions with the
+   neighbour list rebuilt if stale; device reductions in a fixed order.  out: HOST pointer.  Synchronises. */
+typedef struct md_pressure_t {
+    double virial[6], kinetic, volume, pressure;
+} md_pressure_t;
+int md_pressure(md_ctx *ctx, const md_step_desc *what, md_pressure_t *out);
+
 /* ---- S6 velocity-Verlet, NVE (R7) ---------------------------------------------------------- */
 
 /* half = 1: v += (dt/2) F/m; x += dt v; wrap into the box (image counters updated); evaluates the displacement
@@ -293,6 +337,10 @@ int md_set_profiling(md_ctx *ctx, int on);
 /* Test hook: Philox4x32-10 of `n` (counter, key) inputs evaluated ON THE DEVICE by the same device function the
    DPD kernel uses.  ctr: n x 4 uint32, key: n x 2 uint32, out: n x 4 uint32 (host or device pointers). */
 int md_debug_philox(md_ctx *ctx, const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint64_t n);
+
+/* sizeof of the structs crossing this boundary as the library was compiled (0 md_step_desc, 1 md_stats, 2 md_thermo_t,
+   3 md_pressure_t; -1 otherwise): lets a binding check its mirror of the layouts */
+int md_struct_size(int which);
 
 /* Measurement hook (measured, not nominal, peaks of the non-tensor pipes; PAPER.md:300 is the paper's
    only statement on what bounds the path): issue rate of one instruction kind on the whole GPU, every thread running 8

@@ -16,7 +16,9 @@ LIB_PATH = os.path.join(_HERE, "csrc", "libb200md.so")
 
 MD_FP64, MD_MIXED = 0, 1
 MD_ORDER_LEX, MD_ORDER_MORTON, MD_ORDER_HILBERT = 0, 1, 2
-MD_F_LJ, MD_F_DPD, MD_F_BONDS, MD_F_NVT = 1, 2, 4, 8
+MD_F_LJ, MD_F_DPD, MD_F_BONDS, MD_F_NVT, MD_F_PAIR, MD_F_ANGLES = 1, 2, 4, 8, 16, 32
+PAIR_KINDS = {"lj": 0, "yukawa": 1, "gaussian": 2, "morse": 3}
+BOND_KINDS = {"harmonic": 0, "fene": 1}
 MD_SCHED_SYNC, MD_SCHED_SPECULATIVE = 0, 1
 MD_OPT_TILE_BRICK, MD_OPT_ACC_BLOCK, MD_OPT_CLUSTER, MD_OPT_RETUNE_PERIOD = 1, 2, 3, 4
 MD_N_KERNELS = 8
@@ -26,9 +28,10 @@ KERNEL_NAMES = {MD_K_NLIST: "nlist", MD_K_LJ: "lj", MD_K_DPD: "dpd", MD_K_BONDS:
 
 EXPORTS = ["md_create", "md_workspace_bytes", "md_set_workspace", "md_configure", "md_destroy", "md_last_error", "md_set_state", "md_set_bonds",
            "md_get_state", "md_get_forces", "md_build_cells", "md_get_cells", "md_build_nlist", "md_get_nlist",
-           "md_get_nlist_rows", "md_forces_lj", "md_forces_dpd", "md_forces_bonds", "md_integrate_nve",
+           "md_get_nlist_rows", "md_forces_lj", "md_forces_dpd", "md_forces_bonds", "md_forces_pair", "md_forces_fene", "md_set_angles", "md_forces_angles", "md_pressure",
+           "md_integrate_nve",
            "md_needs_rebuild", "md_step", "md_tune", "md_tune_rbuff", "md_set_option", "md_set_launch", "md_get_stats", "md_set_profiling",
-           "md_debug_philox", "md_debug_peak", "md_thermo", "md_integrate_nvt", "md_set_thermostat", "md_get_thermostat"]
+           "md_debug_philox", "md_debug_peak", "md_struct_size", "md_thermo", "md_integrate_nvt", "md_set_thermostat", "md_get_thermostat"]
 
 
 class md_step_desc(C.Structure):
@@ -36,7 +39,13 @@ class md_step_desc(C.Structure):
                 ("lj_epsilon", C.c_double), ("lj_sigma", C.c_double),
                 ("dpd_A", C.c_double), ("dpd_gamma", C.c_double), ("dpd_kT", C.c_double),
                 ("dpd_seed", C.c_uint64), ("bond_k", C.c_double), ("bond_r0", C.c_double),
-                ("nvt_kT", C.c_double), ("nvt_tau", C.c_double)]
+                ("nvt_kT", C.c_double), ("nvt_tau", C.c_double),
+                ("pair_kind", C.c_int32), ("bond_kind", C.c_int32), ("pair_p", C.c_double * 4),
+                ("angle_k", C.c_double), ("angle_theta0", C.c_double)]
+
+
+class md_pressure_t(C.Structure):
+    _fields_ = [("virial", C.c_double * 6), ("kinetic", C.c_double), ("volume", C.c_double), ("pressure", C.c_double)]
 
 
 class md_thermo_t(C.Structure):
@@ -90,6 +99,11 @@ def load():
         "md_forces_lj": [vp, dbl, dbl, i32],
         "md_forces_dpd": [vp, dbl, dbl, dbl, dbl, u64, u64],
         "md_forces_bonds": [vp, dbl, dbl],
+        "md_forces_pair": [vp, i32, C.POINTER(dbl), i32],
+        "md_forces_fene": [vp, dbl, dbl],
+        "md_set_angles": [vp, vp, vp, vp, u64],
+        "md_forces_angles": [vp, dbl, dbl],
+        "md_pressure": [vp, C.POINTER(md_step_desc), vp],
         "md_integrate_nve": [vp, dbl, i32],
         "md_needs_rebuild": [vp, C.POINTER(i32)],
         "md_step": [vp, C.POINTER(md_step_desc), u64],
@@ -101,6 +115,7 @@ def load():
         "md_set_profiling": [vp, i32],
         "md_debug_philox": [vp, vp, vp, vp, u64],
         "md_debug_peak": [vp, i32, C.POINTER(dbl)],
+        "md_struct_size": [i32],
         "md_thermo": [vp, vp],
         "md_integrate_nvt": [vp, C.c_double, i32, C.c_double, C.c_double],
         "md_set_thermostat": [vp, C.c_double, C.c_double],
@@ -110,6 +125,9 @@ def load():
         fn = getattr(L, name)
         fn.argtypes = args
         fn.restype = C.c_int
+    for k, st in enumerate((md_step_desc, md_stats, md_thermo_t, md_pressure_t)):
+        if L.md_struct_size(k) != C.sizeof(st):
+            raise MDError(f"binding out of date: sizeof({st.__name__}) = {C.sizeof(st)}, library says {L.md_struct_size(k)}")
     L.md_last_error.argtypes = [vp]
     L.md_last_error.restype = C.c_char_p
     _lib = L
@@ -157,10 +175,23 @@ def step_desc(kind: str, dt: float, params: dict, nvt: dict = None) -> md_step_d
     elif kind == "bonds":
         d.flags = MD_F_BONDS
         d.bond_k, d.bond_r0 = params["bond_k"], params["bond_r0"]
+    elif kind == "pair":   # params: pair_kind ("yukawa" | "gaussian" | "morse" | "lj"), pair_p, energy_shift
+        d.flags = MD_F_PAIR
+        d.pair_kind = PAIR_KINDS[params["pair_kind"]]
+        for i, v in enumerate(params["pair_p"]):
+            d.pair_p[i] = float(v)
+        d.lj_energy_shift = int(params.get("energy_shift", 1))
     elif kind == "none":
         d.flags = 0
     else:
         raise ValueError(kind)
+    if "bond_kind" in params and (d.flags & MD_F_BONDS or params.get("bonds_on")):
+        d.flags |= MD_F_BONDS
+        d.bond_kind = BOND_KINDS[params["bond_kind"]]
+        d.bond_k, d.bond_r0 = params["bond_k"], params["bond_r0"]
+    if "angle_k" in params:
+        d.flags |= MD_F_ANGLES
+        d.angle_k, d.angle_theta0 = float(params["angle_k"]), float(params["angle_theta0"])
     if nvt is not None:
         d.flags |= MD_F_NVT
         d.nvt_kT, d.nvt_tau = float(nvt["kT"]), float(nvt["tau"])
@@ -284,6 +315,29 @@ class MD:
 
     def forces_bonds(self, k, r0):
         self._chk(self.L.md_forces_bonds(self.h, float(k), float(r0)), "md_forces_bonds")
+
+    def forces_pair(self, kind, p, energy_shift=1):
+        arr = (C.c_double * 4)(*([float(x) for x in p] + [0.0] * (4 - len(p))))
+        self._chk(self.L.md_forces_pair(self.h, PAIR_KINDS[kind], arr, int(energy_shift)), "md_forces_pair")
+
+    def forces_fene(self, k, r0):
+        self._chk(self.L.md_forces_fene(self.h, float(k), float(r0)), "md_forces_fene")
+
+    def set_angles(self, angles):
+        if angles is None or len(angles) == 0:
+            self._chk(self.L.md_set_angles(self.h, None, None, None, 0), "md_set_angles")
+            return
+        a = np.ascontiguousarray(angles, dtype=np.uint32).reshape(-1, 3)
+        ta, tb, tc = (np.ascontiguousarray(a[:, i]) for i in range(3))
+        self._chk(self.L.md_set_angles(self.h, _ptr(ta), _ptr(tb), _ptr(tc), a.shape[0]), "md_set_angles")
+
+    def forces_angles(self, k, theta0):
+        self._chk(self.L.md_forces_angles(self.h, float(k), float(theta0)), "md_forces_angles")
+
+    def pressure(self, desc: md_step_desc) -> dict:
+        t = md_pressure_t()
+        self._chk(self.L.md_pressure(self.h, C.byref(desc), C.byref(t)), "md_pressure")
+        return dict(virial=np.array(list(t.virial)), kinetic=t.kinetic, volume=t.volume, pressure=t.pressure)
 
     def integrate_nve(self, dt, half):
         self._chk(self.L.md_integrate_nve(self.h, float(dt), int(half)), "md_integrate_nve")

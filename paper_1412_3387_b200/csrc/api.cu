@@ -912,6 +912,72 @@ extern "C" int md_forces_bonds(md_ctx *c, double k, double r0)
     return MD_OK;
 }
 
+extern "C" int md_forces_fene(md_ctx *c, double k, double r0)
+{
+    if (!c) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_forces_fene: md_set_state first"; return MD_ESTATE; }
+    if (c->n_bonds == 0) { c->force_valid = true; return MD_OK; }
+    ProfScope ps(c, MD_K_BONDS);
+    MD_TRY(launch_forces_bonds(c, k, r0, MD_BOND_FENE));
+    c->force_valid = true;
+    return MD_OK;
+}
+
+extern "C" int md_forces_pair(md_ctx *c, int kind, const double p[4], int shift)
+{
+    if (!c || !p || kind < MD_PAIR_LJ || kind > MD_PAIR_MORSE) { if (c) c->err = "md_forces_pair: bad argument"; return MD_EINVAL; }
+    MD_TRY(need_nlist(c, "md_forces_pair"));
+    ProfScope ps(c, MD_K_LJ);
+    MD_TRY(ensure_decoded(c));
+    MD_TRY(launch_forces_pair(c, kind, p, shift));
+    c->force_valid = c->energy_valid = true;
+    c->last_from_step = false;
+    return MD_OK;
+}
+
+extern "C" int md_set_angles(md_ctx *c, const uint32_t *ta, const uint32_t *tb, const uint32_t *tc, uint64_t na)
+{
+    if (!c) return MD_EINVAL;
+    if (na > 0 && (!ta || !tb || !tc)) { c->err = "md_set_angles: null tag array"; return MD_EINVAL; }
+    if (na >= 0x3fffffffull) { c->err = "md_set_angles: too many angles"; return MD_EINVAL; }
+    MD_TRY(alloc_state(c));
+    MD_TRY(md_sync(c));
+    for (uint32_t **q : {&c->angle_off, &c->angle_ent, &c->angle_abc})
+        if (*q) { md_free(c, *q); *q = nullptr; }
+    c->n_angles = na;
+    if (na == 0) return MD_OK;
+    if (!is_device_ptr(ta))
+        for (uint64_t m = 0; m < na; ++m)
+            if (ta[m] >= c->N || tb[m] >= c->N || tc[m] >= c->N || ta[m] == tb[m] || tb[m] == tc[m] || ta[m] == tc[m]) {
+                c->err = "md_set_angles: tag out of range or repeated in a triplet";
+                c->n_angles = 0;
+                return MD_EINVAL;
+            }
+    MD_TRY(md_alloc(c, (void **)&c->angle_off, (c->N + 1) * sizeof(uint32_t)));
+    MD_TRY(md_alloc(c, (void **)&c->angle_ent, 3 * na * sizeof(uint32_t)));
+    MD_TRY(md_alloc(c, (void **)&c->angle_abc, 3 * na * sizeof(uint32_t)));
+    Stage st(c);
+    const uint64_t bb = na * sizeof(uint32_t);
+    MD_TRY(st.reserve(stage_need(ta, bb) + stage_need(tb, bb) + stage_need(tc, bb)));
+    const void *da, *db, *dc;
+    MD_TRY(stage_in(c, st, ta, bb, &da));
+    MD_TRY(stage_in(c, st, tb, bb, &db));
+    MD_TRY(stage_in(c, st, tc, bb, &dc));
+    MD_TRY(launch_angles_build(c, (const uint32_t *)da, (const uint32_t *)db, (const uint32_t *)dc, na));
+    return md_sync(c);
+}
+
+extern "C" int md_forces_angles(md_ctx *c, double k, double theta0)
+{
+    if (!c) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_forces_angles: md_set_state first"; return MD_ESTATE; }
+    if (c->n_angles == 0) { c->force_valid = true; return MD_OK; }
+    ProfScope ps(c, MD_K_BONDS);
+    MD_TRY(launch_forces_angles(c, k, theta0));
+    c->force_valid = true;
+    return MD_OK;
+}
+
 extern "C" int md_integrate_nve(md_ctx *c, double dt, int half)
 {
     if (!c) return MD_EINVAL;
@@ -994,10 +1060,23 @@ static int eval_forces(md_ctx *c, const md_step_desc *w, uint64_t step, bool ene
         MD_TRY(pair_dpd(c, w->dpd_A, w->dpd_gamma, w->dpd_kT, w->dt, step, w->dpd_seed));
         any = true;
     }
+    if (w->flags & MD_F_PAIR) {
+        if (any) { c->err = "md_step: the pair terms (LJ, DPD, MD_F_PAIR) are mutually exclusive (each overwrites the force)"; return MD_EINVAL; }
+        if (w->pair_kind < MD_PAIR_LJ || w->pair_kind > MD_PAIR_MORSE) { c->err = "md_step: unknown pair_kind"; return MD_EINVAL; }
+        ProfScope ps(c, MD_K_LJ);
+        MD_TRY(ensure_decoded(c));
+        MD_TRY(launch_forces_pair(c, w->pair_kind, w->pair_p, w->lj_energy_shift));
+        any = true;
+    }
     if (!any) MD_CUDA_CHECK(c, cudaMemsetAsync(c->force, 0, c->N * sizeof(double4), c->stream));
     if ((w->flags & MD_F_BONDS) && c->n_bonds) {
+        if (w->bond_kind != MD_BOND_HARMONIC && w->bond_kind != MD_BOND_FENE) { c->err = "md_step: unknown bond_kind"; return MD_EINVAL; }
         ProfScope ps(c, MD_K_BONDS);
-        MD_TRY(launch_forces_bonds(c, w->bond_k, w->bond_r0));
+        MD_TRY(launch_forces_bonds(c, w->bond_k, w->bond_r0, w->bond_kind));
+    }
+    if ((w->flags & MD_F_ANGLES) && c->n_angles) {
+        ProfScope ps(c, MD_K_BONDS);
+        MD_TRY(launch_forces_angles(c, w->angle_k, w->angle_theta0));
     }
     c->force_valid = true;
     // only the tile LJ kernel skips the per-particle energies
@@ -1417,6 +1496,36 @@ extern "C" int md_thermo(md_ctx *c, md_thermo_t *out)
     out->momentum[0] = r[2]; out->momentum[1] = r[3]; out->momentum[2] = r[4];
     out->temperature = c->N > 1 ? 2.0 * r[0] / (3.0 * (double)c->N - 3.0) : 0.0;
     return MD_OK;
+}
+
+extern "C" int md_pressure(md_ctx *c, const md_step_desc *w, md_pressure_t *out)
+{
+    if (!c || !w || !out) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_pressure: md_set_state first"; return MD_ESTATE; }
+    if ((w->flags & (MD_F_LJ | MD_F_DPD | MD_F_PAIR)) && (!c->nlist_valid || c->steps_since_build > 0)) {
+        // the pair virial needs a list of the current positions only if the old one may have lost pairs: between
+        // rebuilds the list still covers every pair within rc, so a valid list is enough
+        if (!c->nlist_valid) MD_TRY(rebuild(c));
+    }
+    if (w->flags & (MD_F_LJ | MD_F_DPD | MD_F_PAIR)) MD_TRY(ensure_decoded(c));
+    MD_TRY(launch_virial(c, w, c->step, out->virial));
+    double r[5];
+    MD_TRY(launch_thermo(c, r));
+    out->kinetic = r[0];
+    out->volume = c->box[0] * c->box[1] * c->box[2];
+    out->pressure = (2.0 * r[0] + out->virial[0] + out->virial[1] + out->virial[2]) / (3.0 * out->volume);
+    return MD_OK;
+}
+
+extern "C" int md_struct_size(int which)
+{
+    switch (which) {
+    case 0: return (int)sizeof(md_step_desc);
+    case 1: return (int)sizeof(md_stats);
+    case 2: return (int)sizeof(md_thermo_t);
+    case 3: return (int)sizeof(md_pressure_t);
+    default: return -1;
+    }
 }
 
 extern "C" int md_debug_philox(md_ctx *c, const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint64_t n)

@@ -12,6 +12,7 @@
 // ------------------------------------------------------------------------------------------------------------
 struct LJParams {
     double rc2, sig2, eps24, eps4, uc;  // uc = U(rc) if shifted else 0
+    double near2;                       // MD_MIXED: pairs closer than this are evaluated in fp64 (R25)
 };
 
 template <int W, bool MIXED>
@@ -36,7 +37,7 @@ __global__ void __launch_bounds__(1024) k_forces_lj(const double4 *__restrict__ 
         const double dz = md_min_image(pi.z - pj.z, g.L[2], g.h[2]);
         const double r2 = md_r2_exact(dx, dy, dz);
         if (r2 < p.rc2) {
-            if (MIXED) {
+            if (MIXED && r2 >= p.near2) {  // (the first shell stays fp64: DESIGN.md R25)
                 const float fdx = (float)dx, fdy = (float)dy, fdz = (float)dz;
                 const float fr2 = fdx * fdx + fdy * fdy + fdz * fdz;
                 const float rinv2 = 1.0f / fr2;
@@ -75,6 +76,7 @@ int launch_forces_lj(md_ctx *c, double eps, double sigma, int shift)
     p.eps24 = 24.0 * eps;
     p.eps4 = 4.0 * eps;
     p.uc = 0.0;
+    p.near2 = MD_NEAR_SIGMAS * MD_NEAR_SIGMAS * p.sig2;
     if (shift) {
         const double s2 = p.sig2 / p.rc2, s6 = s2 * s2 * s2;
         p.uc = 4.0 * eps * (s6 * s6 - s6);
@@ -169,7 +171,7 @@ int launch_forces_dpd(md_ctx *c, double A, double gamma, double kT, double dt, u
 // ------------------------------------------------------------------------------------------------------------
 __global__ void k_forces_bonds(const double4 *__restrict__ pos, const uint32_t *__restrict__ tag,
                                const uint32_t *__restrict__ rtag, const uint32_t *__restrict__ bond_off,
-                               const uint32_t *__restrict__ bond_partner, Geom g, double kb, double r0,
+                               const uint32_t *__restrict__ bond_partner, Geom g, double kb, double r0, int kind,
                                double4 *__restrict__ force)
 {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -186,12 +188,20 @@ __global__ void k_forces_bonds(const double4 *__restrict__ pos, const uint32_t *
         const double dz = md_min_image(pi.z - pj.z, g.L[2], g.h[2]);
         const double r2 = dx * dx + dy * dy + dz * dz;
         if (r2 > 0.0) {
-            const double r = sqrt(r2);
-            const double f = -kb * (r - r0) / r;
+            double f, u;
+            if (kind == MD_BOND_HARMONIC) {
+                const double r = sqrt(r2);
+                f = -kb * (r - r0) / r;
+                u = 0.5 * kb * (r - r0) * (r - r0);
+            } else {  // FENE (R33): NaN once the bond is stretched to r0
+                const double x = r2 / (r0 * r0);
+                f = x < 1.0 ? -kb / (1.0 - x) : nan("");
+                u = x < 1.0 ? -0.5 * kb * r0 * r0 * log(1.0 - x) : nan("");
+            }
             fx += f * dx;
             fy += f * dy;
             fz += f * dz;
-            en += 0.25 * kb * (r - r0) * (r - r0);
+            en += 0.5 * u;
         }
     }
     double4 f = force[i];
@@ -199,11 +209,11 @@ __global__ void k_forces_bonds(const double4 *__restrict__ pos, const uint32_t *
     force[i] = f;
 }
 
-int launch_forces_bonds(md_ctx *c, double k, double r0)
+int launch_forces_bonds(md_ctx *c, double k, double r0, int kind)
 {
     const LaunchCfg &cf = c->cfg[MD_K_BONDS];
     k_forces_bonds<<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->pos, c->tag, c->rtag, c->bond_off,
-                                                                       c->bond_partner, c->g, k, r0, c->force);
+                                                                       c->bond_partner, c->g, k, r0, kind, c->force);
     MD_LAUNCH_CHECK(c);
     return MD_OK;
 }

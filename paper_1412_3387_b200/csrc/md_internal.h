@@ -139,6 +139,10 @@ struct md_ctx {
     uint32_t *bond_off = nullptr;      // N+1
     uint32_t *bond_partner = nullptr;  // 2*n_bonds partner tags
 
+    // angles: CSR by TAG (entry = 4 * angle index + role), triplets by angle
+    uint64_t n_angles = 0;
+    uint32_t *angle_off = nullptr, *angle_ent = nullptr, *angle_abc = nullptr;
+
     // scratch
     uint64_t *scan_tmp = nullptr;
     uint64_t scan_tmp_len = 0;
@@ -218,7 +222,12 @@ int launch_nlist_count(md_ctx *c);
 int launch_nlist_fill(md_ctx *c);
 int launch_forces_lj(md_ctx *c, double eps, double sigma, int shift);
 int launch_forces_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed);
-int launch_forces_bonds(md_ctx *c, double k, double r0);
+int launch_forces_bonds(md_ctx *c, double k, double r0, int kind = 0);  // kind: MD_BOND_*
+// extra.cu
+int launch_forces_pair(md_ctx *c, int kind, const double prm[4], int shift);
+int launch_angles_build(md_ctx *c, const uint32_t *ta, const uint32_t *tb, const uint32_t *tc, uint64_t na);
+int launch_forces_angles(md_ctx *c, double k, double theta0);
+int launch_virial(md_ctx *c, const md_step_desc *w, uint64_t step, double *out6_host);
 // fused: preceded by the previous step's half 2.  nvt: Nose-Hoover friction xi read from c->nvt_state (R30)
 int launch_half1(md_ctx *c, double dt, bool fused, bool nvt = false);
 int launch_half2(md_ctx *c, double dt, bool nvt = false);

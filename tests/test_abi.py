@@ -29,8 +29,10 @@ def test_library_builds_and_exports_every_declared_symbol():
 
 def test_struct_layouts_match_header():
     import ctypes as C
-    assert C.sizeof(B.md_step_desc) == 96
-    assert C.sizeof(B.md_stats) == 6 * 8 + 8 + 12 + 4 + 3 * 4 * B.MD_N_KERNELS + 8 + 16 * B.MD_N_KERNELS + 16
+    L = B.load()                                      # (load() itself refuses a library whose struct sizes differ)
+    for k, st in enumerate((B.md_step_desc, B.md_stats, B.md_thermo_t, B.md_pressure_t)):
+        assert L.md_struct_size(k) == C.sizeof(st), st.__name__
+    assert C.sizeof(B.md_step_desc) == 152 and C.sizeof(B.md_pressure_t) == 72 and L.md_struct_size(9) == -1
 
 
 def test_fails_loudly_without_gpu():

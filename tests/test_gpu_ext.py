@@ -1,0 +1,125 @@
+"""-m gpu parity of SURVEY 8(f) rows 1 and 3 against oracle/md_oracle_ext.c: Yukawa / Gaussian / Morse pair forces,
+FENE bonds, harmonic angles (forces and energies within 1e-10, R11 norm), virial tensor and pressure of every term
+(1e-10 of the tensor's scale), through the single calls and through md_step."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1412_3387_b200 import binding as B
+from paper_1412_3387_b200 import inputs
+from gpu_util import force_rel_err, min_image_diff
+
+pytestmark = pytest.mark.gpu
+
+PAIRS = [("yukawa", (2.0, 1.5)), ("gaussian", (3.0, 0.8)), ("morse", (1.7, 2.0, 1.0)), ("lj", (0.9, 1.05))]
+
+
+def _chain_angles(n_chains, length):
+    return np.array([[length * c + i, length * c + i + 1, length * c + i + 2]
+                     for c in range(n_chains) for i in range(length - 2)], dtype=np.uint32)
+
+
+@pytest.mark.parametrize("order", [B.MD_ORDER_MORTON, B.MD_ORDER_LEX])
+@pytest.mark.parametrize("kind,p", PAIRS)
+def test_pair_potentials_forces_energies_virial(kind, p, order):
+    wl = inputs.lj_fcc(7, rc=2.5, r_buff=0.4, kT=1.0, jitter=0.08, pos_seed=3, vel_seed=4)       # N = 1372
+    for w in (1, 4, 8):
+        md = B.from_workload(wl, order=order)
+        md.set_launch(B.MD_K_LJ, 128, w)
+        md.build_nlist()
+        md.forces_pair(kind, p, 1)
+        F, E = md.get_forces()
+        Fr, Er = oracle.pair_forces(wl.pos, wl.box, wl.rc, kind, p, 1)
+        assert force_rel_err(F, Fr) < 1e-10 and np.abs(E - Er).max() < 1e-11 * np.abs(Er).max()
+    desc = B.step_desc("pair", wl.dt, dict(pair_kind=kind, pair_p=p))
+    pr = md.pressure(desc)
+    W = oracle.virial_pair(wl.pos, wl.box, wl.rc, kind, p)
+    assert np.abs(pr["virial"] - W).max() < 1e-10 * np.abs(W).max()
+    assert abs(pr["pressure"] - oracle.pressure(wl.vel, wl.box, W)) < 1e-11 * abs(pr["pressure"])
+    assert pr["virial"].tolist() == md.pressure(desc)["virial"].tolist()          # fixed summation order
+    # md_step with the pair potential: single step 1e-12, then a short trajectory
+    if kind != "lj":
+        ms = B.from_workload(wl, order=order)
+        ms.step(desc, 1)
+        pos, vel, _ = ms.get_state()
+        F1 = oracle.pair_forces(wl.pos, wl.box, wl.rc, kind, p, 1)[0]
+        v = wl.vel + 0.5 * wl.dt * F1
+        x = oracle.wrap(wl.pos + wl.dt * v, wl.box)
+        assert np.abs(min_image_diff(pos, x, wl.box)).max() < 1e-12
+        v2 = v + 0.5 * wl.dt * oracle.pair_forces(x, wl.box, wl.rc, kind, p, 1)[0]
+        assert np.abs(vel - v2).max() < 1e-11
+
+
+def test_fene_bonds_and_angles_forces_energy_virial_and_step():
+    wl = inputs.polymer_melt(40, chain_len=32, start_seed=6, walk_seed=7, vel_seed=8)             # N = 1280, bond step 0.97
+    ang = _chain_angles(40, 32)
+    k_f, r0_f, k_a, th0 = 30.0, 1.5, 8.0, 2.0
+    md = B.from_workload(wl)
+    md.set_angles(ang)
+    md.build_cells()
+    # FENE + angles alone (accumulate onto zero)
+    md.forces_fene(k_f, r0_f)
+    md.forces_angles(k_a, th0)
+    F, E = md.get_forces()
+    Fr, Er, Wb = oracle.forces_bonds_kind(wl.pos, wl.box, wl.bonds, "fene", k_f, r0_f)
+    Wa = np.zeros(6)
+    oracle.forces_angles(wl.pos, wl.box, ang, k_a, th0, force=Fr, energy=Er, virial=Wa)
+    assert force_rel_err(F, Fr) < 1e-10 and np.abs(E - Er).max() < 1e-11 * np.abs(Er).max()
+    # virial of DPD + FENE + angles together
+    q = wl.params
+    prm = dict(q, bond_kind="fene", bond_k=k_f, bond_r0=r0_f, angle_k=k_a, angle_theta0=th0)
+    desc = B.step_desc("polymer", wl.dt, prm)
+    assert desc.flags == B.MD_F_DPD | B.MD_F_BONDS | B.MD_F_ANGLES and desc.bond_kind == 1
+    pr = md.pressure(desc)
+    Wd = oracle.virial_dpd(wl.pos, wl.vel, wl.box, wl.rc, q["A"], q["gamma"], q["kT"], wl.dt, 0, q["seed"])
+    W = Wd + Wb + Wa
+    assert np.abs(pr["virial"] - W).max() < 1e-10 * np.abs(W).max()
+    assert abs(pr["kinetic"] - 0.5 * (wl.vel ** 2).sum()) < 1e-12 * pr["kinetic"]
+    assert abs(pr["pressure"] - oracle.pressure(wl.vel, wl.box, W)) < 1e-10 * abs(pr["pressure"])
+    # harmonic bonds virial (the configured polymer model)
+    pr_h = md.pressure(B.step_desc("polymer", wl.dt, q))
+    Wh = oracle.forces_bonds_kind(wl.pos, wl.box, wl.bonds, "harmonic", q["bond_k"], q["bond_r0"])[2]
+    assert np.abs(pr_h["virial"] - (Wd + Wh)).max() < 1e-10 * np.abs(Wd + Wh).max()
+    # one md_step with DPD + FENE + angles against the plain sequence of oracle calls
+    ms = B.from_workload(wl)
+    ms.set_angles(ang)
+    ms.step(desc, 1)
+    pos, vel, _ = ms.get_state()
+
+    def total_force(x, v, step):
+        Ft = oracle.forces_dpd(x, v, wl.box, wl.rc, q["A"], q["gamma"], q["kT"], wl.dt, step, q["seed"])
+        oracle.forces_bonds_kind(x, wl.box, wl.bonds, "fene", k_f, r0_f, force=Ft)
+        oracle.forces_angles(x, wl.box, ang, k_a, th0, force=Ft)
+        return Ft
+    v = wl.vel + 0.5 * wl.dt * total_force(wl.pos, wl.vel, 0)
+    x = oracle.wrap(wl.pos + wl.dt * v, wl.box)
+    assert np.abs(min_image_diff(pos, x, wl.box)).max() < 1e-12
+    v2 = v + 0.5 * wl.dt * total_force(x, v, 1)
+    assert np.abs(vel - v2).max() < 1e-10
+    # clearing the angles switches the term off
+    ms.set_angles(None)
+    ms.set_state(wl.pos, wl.vel)                       # (forces are accumulated: start from a cleared force array)
+    ms.build_cells(); ms.forces_angles(k_a, th0)
+    assert np.abs(ms.get_forces()[0]).max() == 0.0
+
+
+def test_lj_and_dpd_pressure_at_scale_and_after_steps():
+    """Pressure of the LJ liquid (mixed-precision context: the virial is fp64 either way) after md_step, list valid but
+    not fresh, against the oracle at the same positions; ideal-gas limit with the forces off."""
+    wl = inputs.lj_fcc(8, rc=3.0, r_buff=0.4, kT=1.2, jitter=0.05, pos_seed=2, vel_seed=3)       # N = 2048
+    desc = B.step_desc("lj", wl.dt, wl.params)
+    md = B.from_workload(wl, precision=B.MD_MIXED)
+    md.step(desc, 7)
+    pos, vel, _ = md.get_state()
+    pr = md.pressure(desc)
+    W = oracle.virial_pair(pos, wl.box, wl.rc, "lj", (1.0, 1.0))
+    assert np.abs(pr["virial"] - W).max() < 1e-10 * np.abs(W).max()
+    assert abs(pr["pressure"] - oracle.pressure(vel, wl.box, W)) < 1e-10 * abs(pr["pressure"])
+    none = md.pressure(B.step_desc("none", wl.dt, {}))
+    assert np.abs(none["virial"]).max() == 0.0
+    assert abs(none["pressure"] - 2.0 * none["kinetic"] / (3.0 * none["volume"])) < 1e-15
+    md.step(desc, 3)                                    # the pressure call left the run untouched
+    ref = B.from_workload(wl, precision=B.MD_MIXED); ref.step(desc, 10)
+    assert np.array_equal(md.get_state()[0], ref.get_state()[0])
