@@ -253,7 +253,7 @@ def run_ours(args):
     order = {"lex": B.MD_ORDER_LEX, "morton": B.MD_ORDER_MORTON, "hilbert": B.MD_ORDER_HILBERT}[args.order]
     # device memory comes from torch (md_workspace_bytes -> torch.empty -> md_set_workspace); streams too
     md = B.MD(w.box, w.N, w.rc, w.r_buff, precision=precision, stream=stream.cuda_stream, order=order,
-              sched=B.MD_SCHED_SYNC if args.sync_sched else B.MD_SCHED_SPECULATIVE,
+              sched={"sync": B.MD_SCHED_SYNC, "speculative": B.MD_SCHED_SPECULATIVE, "batch": B.MD_SCHED_BATCH}[args.sched],
               workspace=None if args.own_alloc else "torch")
     # measured issue rates of the pipes the pair-force kernel runs on (md_debug_peak), before the timed region
     peaks = {k: md.debug_peak(k) for k in ("fp32_fma", "fp64_fma", "int32_mad")} if rank == 0 else {}
@@ -400,7 +400,7 @@ def run_ours(args):
                        "l2": "inputs larger than L2 (neighbour list %.0f MB + state)" % (4e-6 * st1["nlist_entries"]),
                        "tps": world * args.steps / (ms_max * 1e-3) / world, "rebuild_period_k": k,
                        "mean_neighbors": nbar, "rebuilds": rebuilds, "dangerous_builds": st1["dangerous_builds"],
-                       "order": args.order, "sched": "sync" if args.sync_sched else "speculative",
+                       "order": args.order, "sched": args.sched,
                        "speculative_forces": st1["speculative_forces"] - st0["speculative_forces"],
                        "wasted_forces": st1["wasted_forces"] - st0["wasted_forces"],
                        "launch": {n: [v["block"], v["w"]] for n, v in st1["launch"].items()},
@@ -445,7 +445,8 @@ def main():
     ap.add_argument("--scale", type=float, default=1.0)
     ap.add_argument("--order", default="morton", choices=["lex", "morton", "hilbert"])
     ap.add_argument("--no-tune", action="store_true")
-    ap.add_argument("--sync-sched", action="store_true", help="MD_SCHED_SYNC instead of the speculative scheduler")
+    ap.add_argument("--sched", default="batch", choices=["sync", "speculative", "batch"],
+                    help="md_step scheduler (MD_SCHED_*): batch = kernels of several steps enqueued ahead, gated on the device")
     ap.add_argument("--launch", nargs="*", default=[], help="kernel=block,w (with --no-tune)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cluster", action="store_true", help="MD_OPT_CLUSTER = 1: one neighbour row per cluster of 4")

@@ -82,6 +82,11 @@ enum { MD_BOND_HARMONIC = 0, /* U = k/2 (r - r0)^2 */
 #define MD_SCHED_SPECULATIVE 1 /* default: forces are enqueued before the flag arrives whenever no rebuild is predicted
                                   (PAPER.md:122); if the flag says "rebuild" they are discarded and evaluated again on
                                   the new list.  Results are identical in both modes */
+#define MD_SCHED_BATCH 2       /* no host round trip per step (launch overhead at small N): the kernels of
+                                  a batch of steps are enqueued ahead, each gated on a device-side flag; when half 1 of a
+                                  step fires the criterion, everything enqueued after it returns at once and the host,
+                                  which reads the flag once per batch, rebuilds and resumes from that step.  Same kernels
+                                  on the same data: results identical to the other two modes */
 
 typedef struct {
     uint32_t flags;      /* MD_F_* */

@@ -19,7 +19,7 @@ MD_ORDER_LEX, MD_ORDER_MORTON, MD_ORDER_HILBERT = 0, 1, 2
 MD_F_LJ, MD_F_DPD, MD_F_BONDS, MD_F_NVT, MD_F_PAIR, MD_F_ANGLES = 1, 2, 4, 8, 16, 32
 PAIR_KINDS = {"lj": 0, "yukawa": 1, "gaussian": 2, "morse": 3}
 BOND_KINDS = {"harmonic": 0, "fene": 1}
-MD_SCHED_SYNC, MD_SCHED_SPECULATIVE = 0, 1
+MD_SCHED_SYNC, MD_SCHED_SPECULATIVE, MD_SCHED_BATCH = 0, 1, 2
 MD_OPT_TILE_BRICK, MD_OPT_ACC_BLOCK, MD_OPT_CLUSTER, MD_OPT_RETUNE_PERIOD = 1, 2, 3, 4
 MD_N_KERNELS = 8
 MD_K_NLIST, MD_K_LJ, MD_K_DPD, MD_K_BONDS, MD_K_INTEGRATE, MD_K_CELLS = 0, 1, 2, 3, 4, 5
@@ -201,7 +201,7 @@ def step_desc(kind: str, dt: float, params: dict, nvt: dict = None) -> md_step_d
 class MD:
     """One simulation context (md_ctx).  Methods are 1:1 with the C entry points (md_ prefix dropped)."""
 
-    def __init__(self, box, N, rc, r_buff, precision=MD_FP64, stream=None, order=MD_ORDER_MORTON, sched=MD_SCHED_SPECULATIVE,
+    def __init__(self, box, N, rc, r_buff, precision=MD_FP64, stream=None, order=MD_ORDER_MORTON, sched=MD_SCHED_BATCH,
                  workspace=None):
         """workspace: None (the library allocates), a CUDA uint8 tensor (md_set_workspace), or "torch": a tensor of
         md_workspace_bytes bytes is taken from torch's allocator and kept alive with this object."""

@@ -458,7 +458,7 @@ extern "C" int md_create(md_ctx **out, const double box[3], uint64_t N, double r
     c->rc = rc;
     c->precision = MD_FP64;
     c->order = MD_ORDER_LEX;
-    c->sched = MD_SCHED_SPECULATIVE;
+    c->sched = MD_SCHED_BATCH;
     c->stream = 0;
     c->log = getenv("B200MD_LOG") != nullptr;
     for (int a = 0; a < 3; ++a) c->box[a] = box[a];
@@ -473,7 +473,7 @@ extern "C" int md_configure(md_ctx *c, int precision, void *stream, int order, i
 {
     if (!c) return MD_EINVAL;
     if ((precision != MD_FP64 && precision != MD_MIXED) || order < 0 || order > MD_ORDER_HILBERT ||
-        (sched != MD_SCHED_SYNC && sched != MD_SCHED_SPECULATIVE)) {
+        (sched != MD_SCHED_SYNC && sched != MD_SCHED_SPECULATIVE && sched != MD_SCHED_BATCH)) {
         c->err = "md_configure: bad argument";
         return MD_EINVAL;
     }
@@ -1068,7 +1068,7 @@ static int eval_forces(md_ctx *c, const md_step_desc *w, uint64_t step, bool ene
         MD_TRY(launch_forces_pair(c, w->pair_kind, w->pair_p, w->lj_energy_shift));
         any = true;
     }
-    if (!any) MD_CUDA_CHECK(c, cudaMemsetAsync(c->force, 0, c->N * sizeof(double4), c->stream));
+    if (!any) MD_TRY(launch_zero_force(c));
     if ((w->flags & MD_F_BONDS) && c->n_bonds) {
         if (w->bond_kind != MD_BOND_HARMONIC && w->bond_kind != MD_BOND_FENE) { c->err = "md_step: unknown bond_kind"; return MD_EINVAL; }
         ProfScope ps(c, MD_K_BONDS);
@@ -1093,6 +1093,76 @@ static int rebuild(md_ctx *c)
 {
     MD_TRY(do_build_cells(c));
     return do_build_nlist(c);
+}
+
+// MD_SCHED_BATCH: no host round trip per step.  The kernels of a whole batch of steps are enqueued before the host looks at
+// the rebuild flag; each is gated on DevFlags::rebuild_at (md_internal.h: Gate).  When half 1 of the batch's step m fires
+// the displacement criterion it writes m; the force kernel of step m and everything enqueued after it find their gate
+// closed and return at once, so the state stays exactly as that half 1 left it.  The host reads the flag once per batch,
+// rebuilds, and resumes with the forces of step m: the same sequence of kernels on the same data as the other schedulers
+// (bit-identical results).  The batch length follows the predicted distance to the next rebuild (largest displacement seen
+// and its growth per step): a wrong prediction costs empty launches, never correctness.  PAPER.md:122 overlaps the check
+// with a speculative force evaluation; PAPER.md:120, :163 are the launch overheads this removes at small N.
+static int md_step_batch(md_ctx *c, const md_step_desc *w, uint64_t n_steps, bool nvt)
+{
+    // half 1 of the first step, not gated; its flag is read before anything else is enqueued
+    {
+        ProfScope ps(c, MD_K_INTEGRATE);
+        c->gate_s = c->gate_set = c->gate_nvt = 0;
+        MD_TRY(launch_half1(c, w->dt, false, nvt));
+        if (nvt) MD_TRY(launch_nvt_thermostat(c, w->dt, w->nvt_kT, w->nvt_tau));
+    }
+    c->steps_since_build++;
+    MD_TRY(md_read_flags(c));
+    bool flagged = c->h_flags->rebuild != 0;
+    uint64_t done = 0;
+    while (done < n_steps) {
+        if (flagged) {
+            if (c->h_flags->dangerous) c->stats.dangerous_builds++;
+            MD_TRY(rebuild(c));
+            if (c->retune_period && c->stats.rebuilds - c->rebuilds_at_tune >= c->retune_period) MD_TRY(tune_all(c, w, 2));
+        } else {
+            float d2;
+            memcpy(&d2, &c->h_flags->max_d2[c->d2_slot], sizeof(float));
+            c->last_d2 = d2;
+            if (c->steps_since_build > 0) c->d2_rate = sqrt((double)d2) / (double)c->steps_since_build;
+        }
+        // batch length: the steps the largest displacement still has to the threshold at its observed growth
+        uint64_t K = n_steps - done;
+        {
+            const double room = 0.5 * c->r_buff - sqrt((double)c->last_d2);
+            const double rate = c->d2_rate > 0.0 ? c->d2_rate : 0.0;
+            uint64_t pred = rate > 0.0 ? (uint64_t)std::max(1.0, floor(room / rate)) : (c->steps_since_build == 0 ? 2 : 4);
+            K = std::min<uint64_t>(K, std::min<uint64_t>(std::max<uint64_t>(pred, 1), 64));
+        }
+        MD_CUDA_CHECK(c, cudaMemsetAsync(&c->d_flags->rebuild_at, 0, sizeof(unsigned int), c->stream));
+        for (uint64_t j = 1; j <= K; ++j) {
+            c->gate_s = (unsigned int)j;
+            MD_TRY(eval_forces(c, w, c->step + j, false));  // R15: hash counter = index of the step being completed
+            ProfScope ps(c, MD_K_INTEGRATE);
+            if (done + j < n_steps) {
+                c->gate_set = c->gate_nvt = (unsigned int)(j + 1);
+                MD_TRY(launch_half1(c, w->dt, true, nvt));   // half 2 of step j + half 1 of step j + 1
+                if (nvt) { c->gate_nvt = (unsigned int)j; MD_TRY(launch_nvt_thermostat(c, w->dt, w->nvt_kT, w->nvt_tau)); }
+            } else {
+                MD_TRY(launch_half2(c, w->dt, nvt));
+            }
+        }
+        c->gate_s = c->gate_set = c->gate_nvt = 0;
+        MD_TRY(md_read_flags(c));
+        const uint64_t m = c->h_flags->rebuild_at;        // 0: every enqueued step ran; else steps 1 .. m-1 ran, half 1 of m fired
+        const uint64_t ran = m == 0 ? K : m - 1;
+        flagged = m != 0;
+        done += ran;
+        c->step += ran;
+        c->stats.steps += ran;
+        // half-1 steps since the binning: `ran` full steps' worth, plus the trailing half 1 of the next step if it ran
+        c->steps_since_build += m == 0 ? (done < n_steps ? K : K - 1) : ran;
+        if (m != 0) c->force_valid = false;
+        if (c->profiling) prof_resolve_ready(c);
+    }
+    c->force_valid = true;
+    return MD_OK;
 }
 
 // Step loop.  The displacement criterion is decided on the device by half 1; the host needs the flag to
@@ -1121,6 +1191,7 @@ extern "C" int md_step(md_ctx *c, const md_step_desc *w, uint64_t n_steps)
     }
     if (!c->nlist_valid) MD_TRY(rebuild(c));
     if (!c->force_valid) MD_TRY(eval_forces(c, w, c->step, false));  // R16: F(t0) before the first half-kick
+    if (c->sched == MD_SCHED_BATCH) return md_step_batch(c, w, n_steps, nvt);
     if (!c->ev_flags) MD_CUDA_CHECK(c, cudaEventCreateWithFlags(&c->ev_flags, cudaEventDisableTiming));
     for (uint64_t s = 0; s < n_steps; ++s) {
         if (s == 0) {

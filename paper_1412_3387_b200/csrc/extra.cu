@@ -49,8 +49,9 @@ template <int W, int POT>
 __global__ void __launch_bounds__(1024) k_forces_pair(const double4 *__restrict__ pos, const uint32_t *__restrict__ nl_cnt,
                                                       const uint64_t *__restrict__ nl_off,
                                                       const uint32_t *__restrict__ nl_idx, Geom g, PairParams p,
-                                                      double4 *__restrict__ force)
+                                                      double4 *__restrict__ force, Gate gate)
 {
+    if (md_gate_closed(gate)) return;
     const uint32_t i = (uint32_t)(((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) / W);
     const unsigned lane = threadIdx.x & (W - 1);
     const unsigned seg_mask = md_seg_mask<W>();
@@ -96,10 +97,10 @@ int launch_forces_pair(md_ctx *c, int kind, const double prm[4], int shift)
     const unsigned grid = md_grid(c->N * (uint64_t)w, cf.block);
 #define PAIR_LAUNCH(W_)                                                                                                          \
     switch (kind) {                                                                                                              \
-    case MD_PAIR_LJ: k_forces_pair<W_, MD_PAIR_LJ><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force); break; \
-    case MD_PAIR_YUKAWA: k_forces_pair<W_, MD_PAIR_YUKAWA><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force); break; \
-    case MD_PAIR_GAUSSIAN: k_forces_pair<W_, MD_PAIR_GAUSSIAN><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force); break; \
-    default: k_forces_pair<W_, MD_PAIR_MORSE><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force); break; \
+    case MD_PAIR_LJ: k_forces_pair<W_, MD_PAIR_LJ><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force, md_gate(c)); break; \
+    case MD_PAIR_YUKAWA: k_forces_pair<W_, MD_PAIR_YUKAWA><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force, md_gate(c)); break; \
+    case MD_PAIR_GAUSSIAN: k_forces_pair<W_, MD_PAIR_GAUSSIAN><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force, md_gate(c)); break; \
+    default: k_forces_pair<W_, MD_PAIR_MORSE><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force, md_gate(c)); break; \
     }
     switch (w) {
     case 1: PAIR_LAUNCH(1); break;
@@ -205,8 +206,9 @@ __device__ __forceinline__ bool angle_term(const double4 *__restrict__ pos, cons
 __global__ void k_forces_angles(const double4 *__restrict__ pos, const uint32_t *__restrict__ tag,
                                 const uint32_t *__restrict__ rtag, const uint32_t *__restrict__ off,
                                 const uint32_t *__restrict__ ent, const uint32_t *__restrict__ abc, Geom g, double k,
-                                double theta0, double4 *__restrict__ force)
+                                double theta0, double4 *__restrict__ force, Gate gate)
 {
+    if (md_gate_closed(gate)) return;
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.N) return;
     const uint32_t t = tag[i];
@@ -228,7 +230,7 @@ int launch_forces_angles(md_ctx *c, double k, double theta0)
 {
     const LaunchCfg &cf = c->cfg[MD_K_BONDS];
     k_forces_angles<<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->pos, c->tag, c->rtag, c->angle_off, c->angle_ent,
-                                                                        c->angle_abc, c->g, k, theta0, c->force);
+                                                                        c->angle_abc, c->g, k, theta0, c->force, md_gate(c));
     MD_LAUNCH_CHECK(c);
     return MD_OK;
 }

@@ -19,8 +19,9 @@ template <int W, bool MIXED>
 __global__ void __launch_bounds__(1024) k_forces_lj(const double4 *__restrict__ pos, const uint32_t *__restrict__ nl_cnt,
                                                     const uint64_t *__restrict__ nl_off,
                                                     const uint32_t *__restrict__ nl_idx, Geom g, LJParams p,
-                                                    double4 *__restrict__ force)
+                                                    double4 *__restrict__ force, Gate gate)
 {
+    if (md_gate_closed(gate)) return;
     const uint32_t i = (uint32_t)(((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) / W);
     const unsigned lane = threadIdx.x & (W - 1);
     const unsigned seg_mask = md_seg_mask<W>();
@@ -85,9 +86,9 @@ int launch_forces_lj(md_ctx *c, double eps, double sigma, int shift)
     const bool mixed = c->precision == MD_MIXED;
     MD_DISPATCH_W(cf.w, {
         if (mixed)
-            k_forces_lj<W_, true><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force);
+            k_forces_lj<W_, true><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force, md_gate(c));
         else
-            k_forces_lj<W_, false><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force);
+            k_forces_lj<W_, false><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force, md_gate(c));
     });
     MD_LAUNCH_CHECK(c);
     return MD_OK;
@@ -107,8 +108,9 @@ __global__ void __launch_bounds__(1024) k_forces_dpd(const double4 *__restrict__
                                                      const uint32_t *__restrict__ nl_cnt,
                                                      const uint64_t *__restrict__ nl_off,
                                                      const uint32_t *__restrict__ nl_idx, Geom g, DPDParams p,
-                                                     double4 *__restrict__ force)
+                                                     double4 *__restrict__ force, Gate gate)
 {
+    if (md_gate_closed(gate)) return;
     const uint32_t i = (uint32_t)(((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) / W);
     const unsigned lane = threadIdx.x & (W - 1);
     const unsigned seg_mask = md_seg_mask<W>();
@@ -160,7 +162,7 @@ int launch_forces_dpd(md_ctx *c, double A, double gamma, double kT, double dt, u
     p.seed = seed;
     const unsigned grid = md_grid(c->N * (uint64_t)cf.w, cf.block);
     MD_DISPATCH_W(cf.w, {
-        k_forces_dpd<W_><<<grid, cf.block, 0, c->stream>>>(c->pos, c->vel, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force);
+        k_forces_dpd<W_><<<grid, cf.block, 0, c->stream>>>(c->pos, c->vel, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force, md_gate(c));
     });
     MD_LAUNCH_CHECK(c);
     return MD_OK;
@@ -172,8 +174,9 @@ int launch_forces_dpd(md_ctx *c, double A, double gamma, double kT, double dt, u
 __global__ void k_forces_bonds(const double4 *__restrict__ pos, const uint32_t *__restrict__ tag,
                                const uint32_t *__restrict__ rtag, const uint32_t *__restrict__ bond_off,
                                const uint32_t *__restrict__ bond_partner, Geom g, double kb, double r0, int kind,
-                               double4 *__restrict__ force)
+                               double4 *__restrict__ force, Gate gate)
 {
+    if (md_gate_closed(gate)) return;
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.N) return;
     const uint32_t t = tag[i];
@@ -213,7 +216,22 @@ int launch_forces_bonds(md_ctx *c, double k, double r0, int kind)
 {
     const LaunchCfg &cf = c->cfg[MD_K_BONDS];
     k_forces_bonds<<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->pos, c->tag, c->rtag, c->bond_off,
-                                                                       c->bond_partner, c->g, k, r0, kind, c->force);
+                                                                       c->bond_partner, c->g, k, r0, kind, c->force, md_gate(c));
+    MD_LAUNCH_CHECK(c);
+    return MD_OK;
+}
+
+// forces of a step without a pair term start from zero (gated like a force kernel: MD_SCHED_BATCH)
+__global__ void k_zero_force(double4 *__restrict__ force, uint32_t N, Gate gate)
+{
+    if (md_gate_closed(gate)) return;
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) force[i] = make_double4(0.0, 0.0, 0.0, 0.0);
+}
+
+int launch_zero_force(md_ctx *c)
+{
+    k_zero_force<<<md_grid(c->N, 256), 256, 0, c->stream>>>(c->force, (uint32_t)c->N, md_gate(c));
     MD_LAUNCH_CHECK(c);
     return MD_OK;
 }

@@ -15,8 +15,9 @@ __global__ void __launch_bounds__(MD_HALF1_MAX_BLOCK, 6) k_half1(double4 *__rest
                         int *__restrict__ image, const double *__restrict__ pos_ref,
                         const uint32_t *__restrict__ cell_lin, float4 *__restrict__ rel, Geom g, double dt,
                         double half_dt, double thr2, double danger2, DevFlags *flags, int slot,
-                        const double *__restrict__ nvt)
+                        const double *__restrict__ nvt, Gate gate, unsigned int at_val)
 {
+    if (md_gate_closed(gate)) return;
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     float d2f = 0.f;
     const double xi = NVT ? nvt[0] : 0.0;
@@ -54,6 +55,7 @@ __global__ void __launch_bounds__(MD_HALF1_MAX_BLOCK, 6) k_half1(double4 *__rest
         vel[i] = make_double4(u[0], u[1], u[2], m);
         if (d2 > thr2) {
             flags->rebuild = 1;  // benign race: every writer stores the same value
+            if (at_val) flags->rebuild_at = at_val;
             if (d2 > danger2) flags->dangerous = 1;
         }
         d2f = __double2float_ru(d2);
@@ -64,8 +66,9 @@ __global__ void __launch_bounds__(MD_HALF1_MAX_BLOCK, 6) k_half1(double4 *__rest
 }
 
 __global__ void k_half2_nvt(double4 *__restrict__ vel, const double4 *__restrict__ force, uint32_t N, double half_dt,
-                            const double *__restrict__ nvt)
+                            const double *__restrict__ nvt, Gate gate)
 {
+    if (md_gate_closed(gate)) return;
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const double xi = nvt[0];
@@ -77,8 +80,9 @@ __global__ void k_half2_nvt(double4 *__restrict__ vel, const double4 *__restrict
     vel[i] = v;
 }
 
-__global__ void k_half2(double4 *__restrict__ vel, const double4 *__restrict__ force, uint32_t N, double half_dt)
+__global__ void k_half2(double4 *__restrict__ vel, const double4 *__restrict__ force, uint32_t N, double half_dt, Gate gate)
 {
+    if (md_gate_closed(gate)) return;
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     double4 v = vel[i];
@@ -96,8 +100,11 @@ int launch_half1(md_ctx *c, double dt, bool fused, bool nvt)
     const double t = 0.5 * c->r_buff;
     c->d2_slot ^= 1;
     const unsigned grid = md_grid(c->N, cf.block);
+    // gate of a plain half 1 of index s: closed by an EARLIER firing only (index < s); of the fused launch (half 2 of s +
+    // half 1 of s + 1): closed by a firing at <= s
+    const Gate hg = fused ? md_gate(c) : Gate{c->gate_s > 1 ? &c->d_flags->rebuild_at : nullptr, c->gate_s - 1};
 #define HALF1_ARGS c->pos, c->vel, c->force, c->image, c->pos_ref, c->cell_lin, c->rel, c->g, dt, 0.5 * dt, t * t, \
-                   c->r_buff * c->r_buff, c->d_flags, c->d2_slot, c->nvt_state
+                   c->r_buff * c->r_buff, c->d_flags, c->d2_slot, c->nvt_state, hg, c->gate_set
     if (nvt) {
         if (fused) k_half1<true, true><<<grid, cf.block, 0, c->stream>>>(HALF1_ARGS);
         else k_half1<false, true><<<grid, cf.block, 0, c->stream>>>(HALF1_ARGS);
@@ -114,9 +121,9 @@ int launch_half2(md_ctx *c, double dt, bool nvt)
 {
     const LaunchCfg &cf = c->cfg[MD_K_INTEGRATE];
     if (nvt)
-        k_half2_nvt<<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->vel, c->force, (uint32_t)c->N, 0.5 * dt, c->nvt_state);
+        k_half2_nvt<<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->vel, c->force, (uint32_t)c->N, 0.5 * dt, c->nvt_state, md_gate(c));
     else
-        k_half2<<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->vel, c->force, (uint32_t)c->N, 0.5 * dt);
+        k_half2<<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->vel, c->force, (uint32_t)c->N, 0.5 * dt, md_gate(c));
     MD_LAUNCH_CHECK(c);
     return MD_OK;
 }
@@ -144,8 +151,9 @@ __device__ __forceinline__ void thermo_block_sum(double v[5], double *sm /* [5][
 
 __global__ void __launch_bounds__(THERMO_BLOCK) k_thermo_partial(const double4 *__restrict__ vel,
                                                                  const double4 *__restrict__ force, uint32_t N,
-                                                                 double *__restrict__ partial /* [gridDim.x][5] */)
+                                                                 double *__restrict__ partial /* [gridDim.x][5] */, Gate gate)
 {
+    if (md_gate_closed(gate)) return;
     __shared__ double sm[5 * THERMO_BLOCK];
     const uint32_t b0 = blockIdx.x * THERMO_PER_BLOCK, b1 = min(N, b0 + THERMO_PER_BLOCK);
     double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
@@ -160,8 +168,9 @@ __global__ void __launch_bounds__(THERMO_BLOCK) k_thermo_partial(const double4 *
 }
 
 __global__ void __launch_bounds__(THERMO_BLOCK) k_thermo_final(const double *__restrict__ partial, uint32_t n_partial,
-                                                               double *__restrict__ out /* [5] */)
+                                                               double *__restrict__ out /* [5] */, Gate gate)
 {
+    if (md_gate_closed(gate)) return;
     __shared__ double sm[5 * THERMO_BLOCK];
     double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
     for (uint32_t b = threadIdx.x; b < n_partial; b += THERMO_BLOCK) {
@@ -172,7 +181,7 @@ __global__ void __launch_bounds__(THERMO_BLOCK) k_thermo_final(const double *__r
     if (threadIdx.x < 5) out[threadIdx.x] = sm[threadIdx.x * THERMO_BLOCK];
 }
 
-static int thermo_reduce(md_ctx *c, double **res_out);
+static int thermo_reduce(md_ctx *c, double **res_out, Gate gate = Gate{nullptr, 0});
 
 int launch_thermo(md_ctx *c, double *out5_host)
 {
@@ -184,8 +193,9 @@ int launch_thermo(md_ctx *c, double *out5_host)
 
 // Nose-Hoover thermostat update (R30), on the device: K' from the two reduction kernels above, then one thread
 __global__ void k_nvt_update(const double *__restrict__ sums, double *__restrict__ nvt, double dt, double kT, double tau,
-                             double dof)
+                             double dof, Gate gate)
 {
+    if (md_gate_closed(gate)) return;
     const double K = sums[0];
     const double xi_old = nvt[0];
     const double xi = xi_old + (dt / (tau * tau)) * (2.0 * K / (dof * kT) - 1.0);
@@ -193,7 +203,7 @@ __global__ void k_nvt_update(const double *__restrict__ sums, double *__restrict
     nvt[1] = nvt[1] + 0.5 * dt * (xi + xi_old);
 }
 
-static int thermo_reduce(md_ctx *c, double **res_out)
+static int thermo_reduce(md_ctx *c, double **res_out, Gate gate)
 {
     const uint32_t N = (uint32_t)c->N;
     const uint32_t nb = (N + THERMO_PER_BLOCK - 1) / THERMO_PER_BLOCK;
@@ -205,9 +215,9 @@ static int thermo_reduce(md_ctx *c, double **res_out)
         c->thermo_len = need;
     }
     double *res = c->thermo_buf + 5ull * nb;
-    k_thermo_partial<<<nb, THERMO_BLOCK, 0, c->stream>>>(c->vel, c->force, N, c->thermo_buf);
+    k_thermo_partial<<<nb, THERMO_BLOCK, 0, c->stream>>>(c->vel, c->force, N, c->thermo_buf, gate);
     MD_LAUNCH_CHECK(c);
-    k_thermo_final<<<1, THERMO_BLOCK, 0, c->stream>>>(c->thermo_buf, nb, res);
+    k_thermo_final<<<1, THERMO_BLOCK, 0, c->stream>>>(c->thermo_buf, nb, res, gate);
     MD_LAUNCH_CHECK(c);
     *res_out = res;
     return MD_OK;
@@ -215,9 +225,11 @@ static int thermo_reduce(md_ctx *c, double **res_out)
 
 int launch_nvt_thermostat(md_ctx *c, double dt, double kT, double tau)
 {
+    // part of the half 1 it follows: same gate as that launch (c->gate_nvt is set by the caller)
+    const Gate tg = Gate{c->gate_nvt ? &c->d_flags->rebuild_at : nullptr, c->gate_nvt};
     double *res = nullptr;
-    MD_TRY(thermo_reduce(c, &res));
-    k_nvt_update<<<1, 1, 0, c->stream>>>(res, c->nvt_state, dt, kT, tau, 3.0 * (double)c->N - 3.0);
+    MD_TRY(thermo_reduce(c, &res, tg));
+    k_nvt_update<<<1, 1, 0, c->stream>>>(res, c->nvt_state, dt, kT, tau, 3.0 * (double)c->N - 3.0, tg);
     MD_LAUNCH_CHECK(c);
     return MD_OK;
 }

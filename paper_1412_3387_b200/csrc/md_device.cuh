@@ -92,6 +92,15 @@ __device__ __forceinline__ float md_rcp(float x)
 }
 __device__ __forceinline__ double md_rcp(double x) { return 1.0 / x; }
 
+// closed <=> a half 1 of enqueue index <= g.s has fired the criterion (uniform over the grid: read once per thread)
+__device__ __forceinline__ bool md_gate_closed(const Gate g)
+{
+    if (!g.at) return false;
+    const unsigned int at = *(const volatile unsigned int *)g.at;
+    return at != 0u && at <= g.s;
+}
+static inline Gate md_gate(md_ctx *c) { return Gate{c->gate_s ? &c->d_flags->rebuild_at : nullptr, c->gate_s}; }
+
 // ---- tag lane: pos.w carries the particle tag as raw bits --------------------------------------------------
 __device__ __forceinline__ double md_tag_to_lane(uint32_t tag) { return __longlong_as_double((long long)tag); }
 __device__ __forceinline__ uint32_t md_lane_to_tag(double w) { return (uint32_t)__double_as_longlong(w); }

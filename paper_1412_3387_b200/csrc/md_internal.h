@@ -38,6 +38,15 @@
         if (_s != MD_OK) return _s;   \
     } while (0)
 
+// MD_SCHED_BATCH: the kernels of several steps are enqueued before the host looks at the rebuild
+// flag.  Each carries a gate; once half 1 of enqueue index m has fired the displacement criterion (rebuild_at = m), the
+// kernels with gate index >= m find the gate closed and return at once, so the state stays as that half 1 left it until
+// the host has rebuilt the list.  at == nullptr: not gated.
+struct Gate {
+    const unsigned int *at;
+    unsigned int s;
+};
+
 // geometry handed to kernels by value
 struct Geom {
     double L[3];     // box edges
@@ -60,7 +69,8 @@ struct DevFlags {
     unsigned int max_cell_count;  // most populated cell at the last binning
     unsigned int max_home;        // largest tile: home particles
     unsigned int max_staged;      // largest tile: staged (stencil) particles
-    int pad;
+    unsigned int rebuild_at;      // MD_SCHED_BATCH: enqueue index of the step whose half 1 fired the criterion (0: none); kernels
+                                  // enqueued for that step's forces and everything after it return at once (md_gate_closed)
     unsigned long long nl_total;  // entries of the list being built (general path: padded rows; tile path: sum of row lengths)
     unsigned int nl_overflow;     // tile build: longest row if it exceeds the row stride (host grows the stride, rebuilds)
     unsigned int pad2;
@@ -166,6 +176,9 @@ struct md_ctx {
     float last_d2 = 0.f;             // largest squared displacement seen at the last flag read-back
     double d2_rate = 0.0;            // observed growth of the largest displacement per step (rebuild predictor)
     uint64_t steps_since_build = 0;  // half-1 steps since the last binning
+    unsigned int gate_s = 0;         // MD_SCHED_BATCH: gate index of the kernels being enqueued (0: not gated), see Gate
+    unsigned int gate_nvt = 0;       // ... gate index of a thermostat update being enqueued (the half 1 it belongs to)
+    unsigned int gate_set = 0;       // ... and the index a half 1 being enqueued writes to DevFlags::rebuild_at when it fires
     cudaEvent_t ev_flags = nullptr;  // recorded after the asynchronous flag read-back of md_step
     md_stats stats;
     LaunchCfg cfg[MD_N_KERNELS];
@@ -214,6 +227,7 @@ int launch_exclusive_scan_u32(md_ctx *c, const uint32_t *in, uint64_t n, uint32_
 int launch_pack_state(md_ctx *c, const double *pos, const double *vel, const double *mass);
 int launch_unpack_state(md_ctx *c, double *pos, double *vel, int32_t *image);
 int launch_unpack_forces(md_ctx *c, double *force, double *energy);
+int launch_zero_force(md_ctx *c);
 int launch_copy_energy(md_ctx *c, const double4 *src);  // force[i].w = src[i].w
 int md_block_limit(const md_ctx *c, int kernel);      // largest block size the kernel behind MD_K_* can be launched with
 int launch_unpack_cells(md_ctx *c, uint32_t *cell_of);

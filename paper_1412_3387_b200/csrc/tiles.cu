@@ -1136,8 +1136,9 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj(TileParams tp, Geom 
                                                             const float4 *__restrict__ rel,
                                                             const uint32_t *__restrict__ nl_cnt,
                                                             const uint16_t *__restrict__ nl16, LJTile lj,
-                                                            uint32_t max_staged, double4 *__restrict__ force)
+                                                            uint32_t max_staged, double4 *__restrict__ force, Gate gate)
 {
+    if (md_gate_closed(gate)) return;
     typedef typename std::conditional<MIXED, float4, double4>::type R4;
     typedef typename RecTraits<R4>::real real;
     extern __shared__ __align__(16) char smem_raw[];
@@ -1397,8 +1398,9 @@ __global__ void __launch_bounds__(MD_LJ3_MAX_BLOCK, 4) k_tile_lj3(TileParams tp,
                                                              const uint32_t *__restrict__ nl_cnt,
                                                              const uint16_t *__restrict__ nl16, LJ3U lj,
                                                              uint32_t max_staged,
-                                                             double4 *__restrict__ force)
+                                                             double4 *__restrict__ force, Gate gate)
 {
+    if (md_gate_closed(gate)) return;
     extern __shared__ __align__(16) char smem_raw[];
     float4 *rec = (float4 *)smem_raw;  // records first: their shared-memory address is a launch constant
     const TileSmem h = tile_carve(smem_raw + sizeof(float4) * (max_staged + N_DUMMY), tp.B);
@@ -1610,8 +1612,9 @@ template <int W, bool PRE, bool ENERGY>
 __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj3d(TileParams tp, Geom g, const double4 *__restrict__ pos,
                                                               const uint32_t *__restrict__ nl_cnt,
                                                               const uint16_t *__restrict__ nl16, LJ3D lj,
-                                                              uint32_t max_staged, double4 *__restrict__ force)
+                                                              uint32_t max_staged, double4 *__restrict__ force, Gate gate)
 {
+    if (md_gate_closed(gate)) return;
     extern __shared__ __align__(16) char smem_raw[];
     double2 *rxy = (double2 *)smem_raw;                       // records first: launch-constant shared addresses
     double *rz = (double *)(rxy + (max_staged + N_DUMMY));
@@ -1840,8 +1843,9 @@ __global__ void __launch_bounds__(256, MINB) k_tile_lj4(TileParams tp, Geom g, c
                                                         const float4 *__restrict__ rel,
                                                         const uint32_t *__restrict__ nl_cnt,
                                                         const uint16_t *__restrict__ nl16, LJ3 lj, uint32_t max_staged,
-                                                        uint32_t max_clusters, double4 *__restrict__ force)
+                                                        uint32_t max_clusters, double4 *__restrict__ force, Gate gate)
 {
+    if (md_gate_closed(gate)) return;
     extern __shared__ __align__(16) char smem_raw[];
     float4 *rec = (float4 *)smem_raw;  // records first: their shared-memory address is a launch constant
     const TileSmem h = tile_carve(smem_raw + sizeof(float4) * (max_staged + N_DUMMY), tp.B);
@@ -2002,8 +2006,9 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_dpd(TileParams tp, Geom
                                                              const double4 *__restrict__ vel,
                                                              const uint32_t *__restrict__ nl_cnt,
                                                              const uint16_t *__restrict__ nl16, DPDTile dp,
-                                                             uint32_t max_staged, double4 *__restrict__ force)
+                                                             uint32_t max_staged, double4 *__restrict__ force, Gate gate)
 {
+    if (md_gate_closed(gate)) return;
     extern __shared__ __align__(16) char smem_raw[];
     const TileSmem h = tile_carve(smem_raw, tp.B);
     double4 *rec = (double4 *)h.rest;
@@ -2089,8 +2094,9 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_dpd2(TileParams tp, Geo
                                                               const uint32_t *__restrict__ nl_cnt,
                                                               const uint16_t *__restrict__ nl16, DPDTile dp,
                                                               uint32_t max_staged, uint32_t max_home,
-                                                              double4 *__restrict__ force)
+                                                              double4 *__restrict__ force, Gate gate)
 {
+    if (md_gate_closed(gate)) return;
     extern __shared__ __align__(16) char smem_raw[];
     const uint32_t ns = max_staged + N_DUMMY;
     double2 *ra = (double2 *)smem_raw;  // (x, y)
@@ -2450,11 +2456,11 @@ static int launch_lj_pre(md_ctx *c, const TileParams &tp, const LJTile &p, int b
     if (c->nl_shift) {
         MD_TRY(set_smem(c, k_tile_lj<W, MIXED, ACC, ENERGY, true>, smem));
         k_tile_lj<W, MIXED, ACC, ENERGY, true><<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, p,
-                                                                                     c->tile_max_staged, c->force);
+                                                                                     c->tile_max_staged, c->force, md_gate(c));
     } else {
         MD_TRY(set_smem(c, k_tile_lj<W, MIXED, ACC, ENERGY, false>, smem));
         k_tile_lj<W, MIXED, ACC, ENERGY, false><<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, p,
-                                                                                      c->tile_max_staged, c->force);
+                                                                                      c->tile_max_staged, c->force, md_gate(c));
     }
     return MD_OK;
 }
@@ -2504,18 +2510,18 @@ int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
         const int block = std::min(cf.block, 256);
         if (cf.w >= 8) {
             MD_TRY(set_smem(c, (k_tile_lj4<8, 3>), smem4));
-            k_tile_lj4<8, 3><<<c->n_tiles, block, smem4, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, (uint32_t)ncl_max, c->force);
+            k_tile_lj4<8, 3><<<c->n_tiles, block, smem4, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, (uint32_t)ncl_max, c->force, md_gate(c));
         } else {
             static const int minb = getenv("B200MD_LJ4_MINB") ? atoi(getenv("B200MD_LJ4_MINB")) : 3;
             if (minb == 4) {
                 MD_TRY(set_smem(c, (k_tile_lj4<4, 4>), smem4));
-                k_tile_lj4<4, 4><<<c->n_tiles, block, smem4, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, (uint32_t)ncl_max, c->force);
+                k_tile_lj4<4, 4><<<c->n_tiles, block, smem4, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, (uint32_t)ncl_max, c->force, md_gate(c));
             } else if (minb == 2) {
                 MD_TRY(set_smem(c, (k_tile_lj4<4, 2>), smem4));
-                k_tile_lj4<4, 2><<<c->n_tiles, block, smem4, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, (uint32_t)ncl_max, c->force);
+                k_tile_lj4<4, 2><<<c->n_tiles, block, smem4, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, (uint32_t)ncl_max, c->force, md_gate(c));
             } else {
                 MD_TRY(set_smem(c, (k_tile_lj4<4, 3>), smem4));
-                k_tile_lj4<4, 3><<<c->n_tiles, block, smem4, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, (uint32_t)ncl_max, c->force);
+                k_tile_lj4<4, 3><<<c->n_tiles, block, smem4, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, (uint32_t)ncl_max, c->force, md_gate(c));
             }
         }
         MD_LAUNCH_CHECK(c);
@@ -2538,7 +2544,7 @@ int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
     do {                                                                                                                   \
         MD_TRY(set_smem(c, (k_tile_lj3d<W_, PRE_, EN_>), smemd));                                                         \
         k_tile_lj3d<W_, PRE_, EN_><<<c->n_tiles, cf.block, smemd, c->stream>>>(tp, c->g, c->pos, c->nl_cnt, c->nl16, q,    \
-                                                                                c->tile_max_staged, c->force);             \
+                                                                                c->tile_max_staged, c->force, md_gate(c));             \
     } while (0)
             MD_DISPATCH_W(cf.w, {
                 if (c->nl_shift) { if (energy) LJ3D_LAUNCH(true, true); else LJ3D_LAUNCH(true, false); }
@@ -2567,25 +2573,25 @@ int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
         cf.block = std::min(cf.block, MD_LJ3_MAX_BLOCK);  // k_tile_lj3 is compiled for 4 CTAs of 256 threads per SM (64 registers)
         if (w <= 1) {
             MD_TRY(set_smem(c, (k_tile_lj3<1, true>), smem));
-            k_tile_lj3<1, true><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force);
+            k_tile_lj3<1, true><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force, md_gate(c));
         } else if (w == 2) {  // rows laid out with rotation 2 (p & 3) when the list was built for W = 2 (launch_tile_build)
             MD_TRY(set_smem(c, (k_tile_lj3<2, true>), smem));
-            k_tile_lj3<2, true><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force);
+            k_tile_lj3<2, true><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force, md_gate(c));
         } else if (w == 4) {
             if (lj3_mode == 2) {
                 MD_TRY(set_smem(c, k_tile_lj3<4, true>, smem));
-                k_tile_lj3<4, true><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force);
+                k_tile_lj3<4, true><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force, md_gate(c));
             } else {
                 MD_TRY(set_smem(c, k_tile_lj3<4, false>, smem));
-                k_tile_lj3<4, false><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force);
+                k_tile_lj3<4, false><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force, md_gate(c));
             }
         } else {
             if (lj3_mode == 2) {
                 MD_TRY(set_smem(c, k_tile_lj3<8, true>, smem));
-                k_tile_lj3<8, true><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force);
+                k_tile_lj3<8, true><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force, md_gate(c));
             } else {
                 MD_TRY(set_smem(c, k_tile_lj3<8, false>, smem));
-                k_tile_lj3<8, false><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force);
+                k_tile_lj3<8, false><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, c->force, md_gate(c));
             }
         }
         MD_LAUNCH_CHECK(c);
@@ -2632,7 +2638,7 @@ int launch_tile_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uin
             MD_DISPATCH_W(cf.w, {
                 MD_TRY(set_smem(c, k_tile_dpd2<W_>, smem2));
                 k_tile_dpd2<W_><<<c->n_tiles, cf.block, smem2, c->stream>>>(tp, c->g, c->pos, c->vel, c->nl_cnt, c->nl16, p,
-                                                                         c->tile_max_staged, c->tile_max_home, c->force);
+                                                                         c->tile_max_staged, c->tile_max_home, c->force, md_gate(c));
             });
             MD_LAUNCH_CHECK(c);
             return MD_OK;
@@ -2642,7 +2648,7 @@ int launch_tile_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uin
     MD_DISPATCH_W(cf.w, {
         MD_TRY(set_smem(c, k_tile_dpd<W_>, smem));
         k_tile_dpd<W_><<<c->n_tiles, cf.block, smem, c->stream>>>(tp, c->g, c->pos, c->vel, c->nl_cnt, c->nl16, p,
-                                                               c->tile_max_staged, c->force);
+                                                               c->tile_max_staged, c->force, md_gate(c));
     });
     MD_LAUNCH_CHECK(c);
     return MD_OK;

@@ -314,6 +314,18 @@ def test_speculative_scheduler_equals_synchronous(kind):
     assert sb["speculative_forces"] > 0 and sb["wasted_forces"] <= sb["rebuilds"]
     fa, _ = a.get_forces(); fb, _ = b.get_forces()
     assert np.array_equal(fa, fb)
+    # MD_SCHED_BATCH: kernels of whole batches enqueued ahead, gated on the device-side flag; no host round trip per step
+    d = B.from_workload(wl, sched=B.MD_SCHED_BATCH)
+    e = B.from_workload(wl, sched=B.MD_SCHED_BATCH)
+    d.step(desc, 40)
+    for n in (1, 7, 2, 30):
+        e.step(desc, n)
+    for md in (d, e):
+        p, v, i = md.get_state()
+        assert np.array_equal(pa, p) and np.array_equal(va, v) and np.array_equal(ia, i)
+        assert np.array_equal(md.get_forces()[0], fa)
+        st = md.stats()
+        assert st["rebuilds"] == sa["rebuilds"] and st["steps"] == 40 and st["dangerous_builds"] == 0
 
 
 def test_free_flight_images_and_rebuild_step():
@@ -454,6 +466,11 @@ def test_nvt_single_steps_and_trajectory():
     assert md2.stats()["rebuilds"] >= 2 and md2.stats()["dangerous_builds"] == 0
     # the thermostat heats the T = 0.35 liquid (0.7 equipartitioned with the lattice) towards 1.2: xi went negative
     assert sim2.xi < 0.0
+    # --- the batch scheduler with the thermostat: bit-identical to the speculative one
+    md3 = B.from_workload(wl, sched=B.MD_SCHED_BATCH)
+    md3.step(B.step_desc("lj", dt, wl.params, nvt=dict(kT=kT0, tau=tau)), 40)
+    p3, v3, _ = md3.get_state()
+    assert np.array_equal(p3, pos) and np.array_equal(v3, vel) and md3.get_thermostat() == (gxi, geta)
     # --- thermostat off (xi = 0, tau huge) is NVE, bit for bit in the positions
     a = B.from_workload(wl); b = B.from_workload(wl)
     a.step(B.step_desc("lj", dt, wl.params), 10)
