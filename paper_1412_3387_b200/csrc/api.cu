@@ -280,8 +280,8 @@ static void set_record_grid(md_ctx *c, uint32_t B)
     for (int a = 0; a < 3; ++a) E = std::max(E, (0.5 * B + 1.0) * c->g.cw[a] + c->r_buff + 1e-6);
     c->g.q0 = ldexp(1.0, ilogb(E) + 1 - 24);
     c->g.q0i = 1.0 / c->g.q0;
-    c->g.qr = c->g.q0 / 510.0;
-    c->g.qri = 510.0 / c->g.q0;
+    c->g.qr = c->g.q0 / 512.0;  // a power of two: residual arithmetic in the near section is exact (lj3_near)
+    c->g.qri = 512.0 / c->g.q0;
 }
 
 static uint32_t choose_brick(md_ctx *c)

@@ -66,7 +66,7 @@ __device__ __forceinline__ float md_grid_coord(double v, double q0, double q0i, 
 // fp32 record of a position relative to the centre of cell `lin` (linear id), minimum image applied: what the fp32
 // tile kernels stage.  x, y, z are rounded to the grid q0 (a multiple of q0 below 2^24 q0 is an exact float, and so is
 // its sum with a cell offset on the same grid: the tile kernels stage WITHOUT a rounding); what the grid drops is kept in
-// .w as three 10-bit residuals in units of qr = q0 / 510, so that the mixed-precision force kernel can rebuild
+// .w as three 10-bit residuals in units of qr = q0 / 512 (clamped to +-255), so that the mixed-precision force kernel can rebuild
 // separations to ~1e-9 for the pairs of the first shell (R25).
 __device__ __forceinline__ float4 md_rel_record(double x, double y, double z, uint32_t lin, const Geom &g)
 {

@@ -56,7 +56,7 @@ struct Geom {
     double cw[3];    // cell widths L/n
     double q0, q0i;  // grid of the cell-relative fp32 records (md_rel_record): multiples of q0 = 2^-24 x the binade above
                      // the staged extent, so that record + cell offset is an EXACT fp32 sum in the tile kernels
-    double qr, qri;  // quantum of the residuals carried in rel.w: q0 / 510
+    double qr, qri;  // quantum of the residuals carried in rel.w: q0 / 512 (fields hold -255 .. 255)
     uint32_t n[3];   // cells per axis
     uint32_t n_cells;
     uint32_t N;

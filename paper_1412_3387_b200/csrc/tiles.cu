@@ -364,7 +364,7 @@ __device__ __forceinline__ void tile_stage_rel(const TileCtx &tc, const TileSmem
 //     staged residual   = record residual + offset residual   (one integer add on the packed 10-bit fields),
 // and coordinate + qr * residual is the true brick-relative coordinate to ~ qr = q0 / 510 (~1e-9 at config 2).  The far
 // loop reads x, y, z; the near section rebuilds separations from both in fp64 without leaving shared memory (R25).
-// 16 bytes per staged particle from L2 and 6 instructions per record, no fp64 and no conversion.
+// 16 bytes per staged particle from L2, a handful of instructions per record, no fp64 and no conversion.
 __device__ __forceinline__ void tile_stage_exact(const TileCtx &tc, const TileSmem &h, const float4 *__restrict__ rel,
                                                  float4 *rec, uint8_t *scell, const Geom &g)
 {
@@ -1355,7 +1355,13 @@ __device__ __noinline__ void lj3_near(const uint2 *__restrict__ halves, uint32_t
                                       const uint32_t *gstart, const uint32_t *sstart, uint32_t n_sc, double *out)
 {
     const uint32_t mw = __float_as_uint(me.w);
-    const int mrx = md_res_x(mw), mry = md_res_y(mw), mrz = md_res_z(mw);
+    // d = (x_i - x_j) + qr (f_i - f_j), f the biased residual fields (0 .. 1020), without an int -> double conversion: the
+    // double with high word 0x43300000 and low word n IS 2^52 + n, so with n = f_i + 1024 - f_j (positive) and
+    // Cq = qr (2^52 + 1024):  d = fma(qr, 2^52 + n, (x_i - Cq) - x_j), every step exact (qr is a power of two, the coordinates
+    // are multiples of 512 qr below 2^33 qr), one rounding at the end
+    const int mrx = md_res_x(mw) + 1024, mry = md_res_y(mw) + 1024, mrz = md_res_z(mw) + 1024;
+    const double Cq = qr * (MD_TWO52 + 1024.0);
+    const double mx = (double)me.x - Cq, my = (double)me.y - Cq, mz = (double)me.z - Cq;
     double ax = 0.0, ay = 0.0, az = 0.0;
     uint2 q = lane < n_halves ? __ldg(halves + lane) : make_uint2(0u, 0u);  // (prefetched into L1 by the caller)
     for (uint32_t u = lane; u < n_halves; u += W) {
@@ -1366,9 +1372,9 @@ __device__ __noinline__ void lj3_near(const uint2 *__restrict__ halves, uint32_t
             const uint32_t off = (e & 1) ? (ww >> 16) : (ww & 0xffffu);
             const float4 pj = lds_f4(rec_addr + off);
             const uint32_t pw = __float_as_uint(pj.w);
-            const double dx = fma(qr, md_small_int_to_double(mrx - md_res_x(pw)), (double)(me.x - pj.x));
-            const double dy = fma(qr, md_small_int_to_double(mry - md_res_y(pw)), (double)(me.y - pj.y));
-            const double dz = fma(qr, md_small_int_to_double(mrz - md_res_z(pw)), (double)(me.z - pj.z));
+            const double dx = fma(qr, __hiloint2double(0x43300000, mrx - md_res_x(pw)), mx - (double)pj.x);
+            const double dy = fma(qr, __hiloint2double(0x43300000, mry - md_res_y(pw)), my - (double)pj.y);
+            const double dz = fma(qr, __hiloint2double(0x43300000, mrz - md_res_z(pw)), mz - (double)pj.z);
             const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
             const double d = r2 - rc2;
             bool in = d < -guard;
