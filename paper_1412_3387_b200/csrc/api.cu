@@ -1278,7 +1278,7 @@ int md_block_limit(const md_ctx *c, int kernel)
     switch (kernel) {
     case MD_K_NLIST: return tile ? MD_TILE_MAX_BLOCK : 1024;
     case MD_K_LJ: return !tile ? 1024 : (c->precision == MD_MIXED ? MD_LJ3_MAX_BLOCK : MD_TILE_MAX_BLOCK);
-    case MD_K_DPD: return tile ? MD_TILE_MAX_BLOCK : 1024;
+    case MD_K_DPD: return tile ? MD_DPD2_MAX_BLOCK : 1024;
     case MD_K_INTEGRATE: return MD_HALF1_MAX_BLOCK;
     default: return 1024;
     }

@@ -23,6 +23,7 @@
 // compiled block-size limits (__launch_bounds__) of the kernel families; the tuner sweeps launchable sizes only
 #define MD_TILE_MAX_BLOCK 512   // tile kernels (up to 128 registers per thread)
 #define MD_LJ3_MAX_BLOCK 256    // k_tile_lj3: 4 CTAs of 256 threads per SM at 64 registers
+#define MD_DPD2_MAX_BLOCK 256   // k_tile_dpd2: 4 CTAs of 256 threads per SM at 64 registers
 #define MD_HALF1_MAX_BLOCK 256  // k_half1: 6 CTAs of 256 threads per SM
 
 // nl_cnt word of a tile row: entries in the low 24 bits, blocks of the near section (the LAST K blocks of the row,

@@ -2095,7 +2095,7 @@ __device__ __forceinline__ double md_rsqrt_nr1(double x)
 }
 
 template <int W>
-__global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_dpd2(TileParams tp, Geom g, const double4 *__restrict__ pos,
+__global__ void __launch_bounds__(MD_DPD2_MAX_BLOCK, 4) k_tile_dpd2(TileParams tp, Geom g, const double4 *__restrict__ pos,
                                                               const double4 *__restrict__ vel,
                                                               const uint32_t *__restrict__ nl_cnt,
                                                               const uint16_t *__restrict__ nl16, DPDTile dp,
@@ -2634,6 +2634,7 @@ int launch_tile_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uin
     TileParams tp = make_tp(c);
     static const int dpd_mode = getenv("B200MD_DPD") ? atoi(getenv("B200MD_DPD")) : 2;
     if (dpd_mode == 2) {
+        cf.block = std::min(cf.block, MD_DPD2_MAX_BLOCK);  // k_tile_dpd2 is compiled for 4 CTAs of 256 threads per SM (64 registers)
         const size_t ns = c->tile_max_staged + N_DUMMY;
         const int w = std::max(1, std::min(cf.w, 32));
         const size_t n_groups = (size_t)cf.block / w;
