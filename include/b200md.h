@@ -49,8 +49,10 @@ typedef enum {
 #define MD_FP64 0   /* everything fp64 */
 #define MD_MIXED 1  /* LJ pair polynomial in fp32 on fp32 separations, r<rc decision as fp64 would take it,
                        contributions accumulated in fp64 (fp32 sums of 8 consecutive list entries are widened,
-                       MD_OPT_ACC_BLOCK); positions, velocities, integration, cell ids, neighbour-list decisions,
-                       displacement check stay fp64 */
+                       MD_OPT_ACC_BLOCK); pairs of the first neighbour shell (every pair that can be closer than 1.5 sigma
+                       before the next rebuild) are evaluated in fp64 -- fp32 cannot hold the 1e-4 force bar there (DESIGN.md
+                       R25); positions, velocities, integration, cell ids, neighbour-list decisions, displacement check
+                       stay fp64.  The other pair potentials, bonds and angles are fp64 in both modes */
 
 /* internal storage order of the cells (particles are always sorted by cell; inside a cell by tag, with
    MD_ORDER_MORTON by (3-bit-per-axis sub-cell Morton key, tag): a pure function of the positions either way) */

@@ -391,7 +391,7 @@ static int set_geometry(md_ctx *c, double r_buff)
 static void set_default_cfg(md_ctx *c)
 {
     for (int k = 0; k < MD_N_KERNELS; ++k) c->cfg[k] = LaunchCfg{128, 1, 0.f};
-    c->cfg[MD_K_NLIST] = LaunchCfg{256, 8, 0.f};
+    c->cfg[MD_K_NLIST] = LaunchCfg{256, 4, 0.f};
     c->cfg[MD_K_LJ] = LaunchCfg{256, 2, 0.f};
     c->cfg[MD_K_DPD] = LaunchCfg{128, 4, 0.f};
     c->cfg[MD_K_BONDS] = LaunchCfg{128, 1, 0.f};

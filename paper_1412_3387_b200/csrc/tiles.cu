@@ -11,7 +11,8 @@
 //   * the staged coordinates are small (|x| < ~2.5 cell widths), so fp32 separations keep ~1e-6 absolute accuracy
 //     although absolute fp32 coordinates would not (hard part 3).
 //
-// Neighbour list (Fig. 4), w = 32: a warp strides over the 9 x-runs of the 27 stencil cells, one
+// Neighbour list (Fig. 4), ballot variant k_tile_build, w = 32 (the default is k_tile_build8 further
+// down: 4 candidate phases x 8 home particles per warp, no ballot): a warp strides over the 9 x-runs of the 27 stencil cells, one
 // ballot per 32 candidates (Fig. 4 steps 2-3) for BUILD_P home particles of one cell at a time (a candidate is loaded
 // once and tested against BUILD_P particles held in registers).  The distance test is the fp32 dot-product form
 // |b|^2 - 2 a.b < R^2 - |a|^2 (three FFMA per candidate, |b|^2 staged with the record) against R^2 = r_list^2 + guard,
@@ -298,12 +299,12 @@ __device__ __forceinline__ void tile_stage_rel(const TileCtx &tc, const TileSmem
                                                const double4 *__restrict__ pos, const Geom &g)
 {
     const uint32_t lane = threadIdx.x & 31u, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    for (uint32_t sc = wid; sc < tc.n_sc; sc += nw) {
-        const uint32_t b = h.sstart[sc], e = h.sstart[sc + 1];
-        for (uint32_t s = b + lane; s < e; s += 32) scell[s] = (uint8_t)sc;
-    }
-    __syncthreads();
     if (!MD_STAGE_FROM_REL) {
+        for (uint32_t sc = wid; sc < tc.n_sc; sc += nw) {
+            const uint32_t b = h.sstart[sc], e = h.sstart[sc + 1];
+            for (uint32_t s = b + lane; s < e; s += 32) scell[s] = (uint8_t)sc;
+        }
+        __syncthreads();
         // fp64 staging: the coordinate relative to the brick centre is formed in fp64 and rounded ONCE (R25)
         const double dscale = (double)scale;
         for (uint32_t s0 = threadIdx.x; s0 < tc.n_staged; s0 += 2 * blockDim.x) {
@@ -332,26 +333,40 @@ __device__ __forceinline__ void tile_stage_rel(const TileCtx &tc, const TileSmem
         if (threadIdx.x < N_DUMMY) rec[tc.n_staged + threadIdx.x] = RecTraits<float4>::far();
         return;
     }
-    // 4 records per thread and trip, all 4 global loads issued before the first is used: the loop is a chain of L2
-    // round trips otherwise (a thread stages ~9 records)
-    for (uint32_t s0 = threadIdx.x; s0 < tc.n_staged; s0 += 4 * blockDim.x) {
+    // a warp takes two staged cells at a time; the (up to) four loads of a lane -- members 0..31 and 32..63 of each --
+    // are issued before the first is used (the loop is a chain of L2 round trips otherwise); longer cells loop on.
+    // (No per-record cell table: `scell` is not filled on this path.)
+    for (uint32_t sc0 = 2u * wid; sc0 < tc.n_sc; sc0 += 2u * nw) {
         float4 r[4];
-        uint32_t scs[4];
+        uint32_t sb[2], sn[2], gs[2];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const uint32_t s = s0 + u * blockDim.x;
-            if (s < tc.n_staged) {
-                scs[u] = scell[s];
-                r[u] = __ldg(rel + h.gstart[scs[u]] + (s - h.sstart[scs[u]]));
-            }
+        for (int u = 0; u < 2; ++u) {
+            const uint32_t sc = min(sc0 + u, tc.n_sc - 1u);
+            sb[u] = h.sstart[sc];
+            sn[u] = sc0 + u < tc.n_sc ? h.sstart[sc + 1] - sb[u] : 0u;
+            gs[u] = h.gstart[sc];
         }
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-            const uint32_t s = s0 + u * blockDim.x;
-            if (s < tc.n_staged) {
-                const float4 o = h.coff[scs[u]];
+            const uint32_t k = lane + 32u * (u >> 1);
+            if (k < sn[u & 1]) r[u] = __ldg(rel + gs[u & 1] + k);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const uint32_t k = lane + 32u * (u >> 1);
+            if (k < sn[u & 1]) {
+                const float4 o = h.coff[min(sc0 + (u & 1), tc.n_sc - 1u)];
                 const float x = (r[u].x + o.x) * scale, y = (r[u].y + o.y) * scale, z = (r[u].z + o.z) * scale;
-                rec[s] = make_float4(x, y, z, WITH_R2 ? x * x + y * y + z * z : 0.f);
+                rec[sb[u & 1] + k] = make_float4(x, y, z, WITH_R2 ? x * x + y * y + z * z : 0.f);
+            }
+        }
+#pragma unroll 1
+        for (int u = 0; u < 2; ++u) {  // cells of more than 64 members
+            const float4 o = h.coff[min(sc0 + u, tc.n_sc - 1u)];
+            for (uint32_t k = 64u + lane; k < sn[u]; k += 32) {
+                const float4 q = __ldg(rel + gs[u] + k);
+                const float x = (q.x + o.x) * scale, y = (q.y + o.y) * scale, z = (q.z + o.z) * scale;
+                rec[sb[u] + k] = make_float4(x, y, z, WITH_R2 ? x * x + y * y + z * z : 0.f);
             }
         }
     }
@@ -366,32 +381,42 @@ __device__ __forceinline__ void tile_stage_rel(const TileCtx &tc, const TileSmem
 // loop reads x, y, z; the near section rebuilds separations from both in fp64 without leaving shared memory (R25).
 // 16 bytes per staged particle from L2, a handful of instructions per record, no fp64 and no conversion.
 __device__ __forceinline__ void tile_stage_exact(const TileCtx &tc, const TileSmem &h, const float4 *__restrict__ rel,
-                                                 float4 *rec, uint8_t *scell, const Geom &g)
+                                                 float4 *rec)
 {
+    // a warp takes two staged cells at a time; the (up to) four loads of a lane -- members 0..31 and 32..63 of each --
+    // are issued before the first is used (the loop is a chain of L2 round trips otherwise); longer cells loop on
     const uint32_t lane = threadIdx.x & 31u, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    for (uint32_t sc = wid; sc < tc.n_sc; sc += nw) {
-        const uint32_t b = h.sstart[sc], e = h.sstart[sc + 1];
-        for (uint32_t s = b + lane; s < e; s += 32) scell[s] = (uint8_t)sc;
-    }
-    __syncthreads();
-    for (uint32_t s0 = threadIdx.x; s0 < tc.n_staged; s0 += 4 * blockDim.x) {
+    for (uint32_t sc0 = 2u * wid; sc0 < tc.n_sc; sc0 += 2u * nw) {
         float4 r[4];
-        uint32_t scs[4];
+        uint32_t sb[2], sn[2], gs[2];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const uint32_t s = s0 + u * blockDim.x;
-            if (s < tc.n_staged) {
-                scs[u] = scell[s];
-                r[u] = __ldg(rel + h.gstart[scs[u]] + (s - h.sstart[scs[u]]));
-            }
+        for (int u = 0; u < 2; ++u) {
+            const uint32_t sc = min(sc0 + u, tc.n_sc - 1u);
+            sb[u] = h.sstart[sc];
+            sn[u] = sc0 + u < tc.n_sc ? h.sstart[sc + 1] - sb[u] : 0u;
+            gs[u] = h.gstart[sc];
         }
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-            const uint32_t s = s0 + u * blockDim.x;
-            if (s < tc.n_staged) {
-                const float4 o = h.coff[scs[u]];
-                rec[s] = make_float4(r[u].x + o.x, r[u].y + o.y, r[u].z + o.z,
-                                     __uint_as_float(__float_as_uint(r[u].w) + __float_as_uint(o.w)));
+            const uint32_t k = lane + 32u * (u >> 1);
+            if (k < sn[u & 1]) r[u] = __ldg(rel + gs[u & 1] + k);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const uint32_t k = lane + 32u * (u >> 1);
+            if (k < sn[u & 1]) {
+                const float4 o = h.coff[min(sc0 + (u & 1), tc.n_sc - 1u)];
+                rec[sb[u & 1] + k] = make_float4(r[u].x + o.x, r[u].y + o.y, r[u].z + o.z,
+                                                 __uint_as_float(__float_as_uint(r[u].w) + __float_as_uint(o.w)));
+            }
+        }
+#pragma unroll 1
+        for (int u = 0; u < 2; ++u) {  // cells of more than 64 members
+            const float4 o = h.coff[min(sc0 + u, tc.n_sc - 1u)];
+            for (uint32_t k = 64u + lane; k < sn[u]; k += 32) {
+                const float4 q = __ldg(rel + gs[u] + k);
+                rec[sb[u] + k] = make_float4(q.x + o.x, q.y + o.y, q.z + o.z,
+                                             __uint_as_float(__float_as_uint(q.w) + __float_as_uint(o.w)));
             }
         }
     }
@@ -1229,13 +1254,14 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj(TileParams tp, Geom 
 // with W >= 8 they hold 8 consecutive blocks of one particle: at unrolled slot e the 8 records have the 8 different
 // classes (e + b' + ...) & 7 -> the gather is conflict-free except for the relocated entries.
 //
-// Arithmetic (R1, R25, R26): coordinates are staged divided by sigma, so s2 = 1/r'^2; per pair
-// g = (s6 - 1/2) s8 and F_i = (48 eps / sigma) sum_j g d'_ij.  The r < rc decision: d = r'^2 - rc'^2 in fp32; |d| >= guard
-// decides by sign; a block of 8 entries in which some |d| < guard is re-evaluated with the exact fp64 test.
-// 8 contributions are summed in fp32, the block sum is widened and accumulated in fp64 (MD_OPT_ACC_BLOCK = 8).
+// Arithmetic (R1, R25, R26).  Far blocks (all but the last K of a row): packed fp32.  Coordinates stay in box
+// units (the staging is exact, tile_stage_exact); s2 = sigma^2 / r^2, per pair g = (s6 - 1/2) s6 s2 and
+// F_i = (48 eps / sigma^2) sum_j g d_ij.  The r < rc decision: d = r^2 - rc^2 in fp32; |d| >= guard decides by sign; a block of
+// 8 entries in which some |d| < guard is re-evaluated with the exact fp64 test.  8 contributions are summed in fp32, the
+// block sum is widened and accumulated in fp64 (MD_OPT_ACC_BLOCK = 8).  Near section (the last K blocks: every neighbour
+// that can be closer than MD_NEAR_SIGMAS sigma before the next rebuild, see near_partition): fp64 on separations rebuilt
+// from the staged records and their residuals (lj3_near) -- fp32 cannot hold the 1e-4 bar on the first shell.
 // ===============================================================================================================
-// k_tile_lj3: coordinates stay in box units (the staging is exact, see tile_stage_exact); sigma enters as s2 = sigma^2 / r^2,
-// g = (s6 - 1/2) s6 s2 and F_i = (48 eps / sigma^2) sum_j g d_ij
 struct LJ3U {
     double rc2_exact;     // rc^2 (exact re-test)
     double sig2;          // sigma^2
@@ -1414,7 +1440,7 @@ __global__ void __launch_bounds__(MD_LJ3_MAX_BLOCK, 4) k_tile_lj3(TileParams tp,
 
     TileCtx tc;
     tile_setup(tp, g, blockIdx.x, h, tc);
-    tile_stage_exact(tc, h, rel, rec, scell, g);
+    tile_stage_exact(tc, h, rel, rec);
     // staged index of every home particle (replaces a search per particle)
     uint16_t *hsidx = (uint16_t *)(scell + ((max_staged + 16) & ~15u));
     for (uint32_t hc = threadIdx.x >> 5; hc < tc.n_hc; hc += blockDim.x >> 5) {
