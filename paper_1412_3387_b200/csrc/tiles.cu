@@ -245,6 +245,30 @@ __device__ __forceinline__ uint32_t tile_global_of_staged(const TileSmem &h, uin
     return h.gstart[sc] + (s - h.sstart[sc]);
 }
 
+// Walks every staged record cell by cell: a group of LPC lanes (8, 16 or 32, from the mean cell population) takes a
+// staged cell, two members per lane in flight: load(global slot) for both, then store(staged index, staged cell, value).
+// Replaces a per-record cell table (one pass less, no search per record).
+template <typename T, typename Load, typename Store>
+__device__ __forceinline__ void tile_for_each_staged(const TileCtx &tc, const TileSmem &h, Load load, Store store)
+{
+    const uint32_t mean = tc.n_staged / max(tc.n_sc, 1u);
+    const uint32_t lpc = mean <= 12u ? 8u : (mean <= 26u ? 16u : 32u);  // two members per lane cover a typical cell
+    const uint32_t lane = threadIdx.x & 31u, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const uint32_t cpw = 32u / lpc, sub = lane / lpc, m = lane % lpc;
+    for (uint32_t sc = wid * cpw + sub; sc < tc.n_sc; sc += nw * cpw) {
+        const uint32_t b = h.sstart[sc], n = h.sstart[sc + 1] - b, gs = h.gstart[sc];
+        for (uint32_t k = m; k < n; k += 2u * lpc) {
+            T v[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u)
+                if (k + u * lpc < n) v[u] = load(gs + k + u * lpc);
+#pragma unroll
+            for (int u = 0; u < 2; ++u)
+                if (k + u * lpc < n) store(b + k + u * lpc, sc, v[u]);
+        }
+    }
+}
+
 template <typename R4> struct RecTraits;
 template <> struct RecTraits<float4> {
     typedef float real;
@@ -1658,38 +1682,18 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj3d(TileParams tp, Geo
     tile_setup(tp, g, blockIdx.x, h, tc);
     {   // stage: coordinates relative to the brick centre, periodic image applied, divided by sigma (see tile_stage)
         const uint32_t lane32 = threadIdx.x & 31u, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-        for (uint32_t sc = wid; sc < tc.n_sc; sc += nw) {
-            const uint32_t b = h.sstart[sc], e = h.sstart[sc + 1];
-            for (uint32_t s = b + lane32; s < e; s += 32) scell[s] = (uint8_t)sc;
-        }
         for (uint32_t hc = wid; hc < tc.n_hc; hc += nw) {
             const uint32_t p0 = h.hc_first[hc], p1 = h.hc_first[hc + 1], s0 = h.sstart[h.hc_sc[hc]];
             for (uint32_t p = p0 + lane32; p < p1; p += 32) hsidx[p] = (uint16_t)(s0 + (p - p0));
         }
-        __syncthreads();
-        for (uint32_t s0 = threadIdx.x; s0 < tc.n_staged; s0 += 2 * blockDim.x) {  // 2 loads in flight per thread
-            double4 pp[2];
-            uint32_t scs[2];
-#pragma unroll
-            for (int u = 0; u < 2; ++u) {
-                const uint32_t s = s0 + u * blockDim.x;
-                if (s < tc.n_staged) {
-                    scs[u] = scell[s];
-                    pp[u] = pos[h.gstart[scs[u]] + (s - h.sstart[scs[u]])];
-                }
-            }
-#pragma unroll
-            for (int u = 0; u < 2; ++u) {
-                const uint32_t s = s0 + u * blockDim.x;
-                if (s < tc.n_staged) {
-                    const double4 p = pp[u];
-                    const double *cg = h.cgeo + 6 * scs[u];
-                    rxy[s] = make_double2((cg[3] + md_min_image(p.x - cg[0], g.L[0], g.h[0])) * lj.inv_sigma,
-                                          (cg[4] + md_min_image(p.y - cg[1], g.L[1], g.h[1])) * lj.inv_sigma);
-                    rz[s] = (cg[5] + md_min_image(p.z - cg[2], g.L[2], g.h[2])) * lj.inv_sigma;
-                }
-            }
-        }
+        tile_for_each_staged<double4>(
+            tc, h, [&](uint32_t gi) { return pos[gi]; },
+            [&](uint32_t s, uint32_t sc, const double4 &p) {
+                const double *cg = h.cgeo + 6 * sc;
+                rxy[s] = make_double2((cg[3] + md_min_image(p.x - cg[0], g.L[0], g.h[0])) * lj.inv_sigma,
+                                      (cg[4] + md_min_image(p.y - cg[1], g.L[1], g.h[1])) * lj.inv_sigma);
+                rz[s] = (cg[5] + md_min_image(p.z - cg[2], g.L[2], g.h[2])) * lj.inv_sigma;
+            });
         if (threadIdx.x < N_DUMMY) {
             rxy[tc.n_staged + threadIdx.x] = make_double2(1e150, 1e150);
             rz[tc.n_staged + threadIdx.x] = 1e150;
@@ -2144,27 +2148,21 @@ __global__ void __launch_bounds__(MD_DPD2_MAX_BLOCK, 4) k_tile_dpd2(TileParams t
     tile_setup(tp, g, blockIdx.x, h, tc);
     {
         const uint32_t lane32 = threadIdx.x & 31u, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-        for (uint32_t sc = wid; sc < tc.n_sc; sc += nw) {
-            const uint32_t b = h.sstart[sc], e = h.sstart[sc + 1];
-            for (uint32_t s = b + lane32; s < e; s += 32) scell[s] = (uint8_t)sc;
-        }
         for (uint32_t hc = wid; hc < tc.n_hc; hc += nw) {
             const uint32_t p0 = h.hc_first[hc], p1 = h.hc_first[hc + 1], s0 = h.sstart[h.hc_sc[hc]];
             for (uint32_t p = p0 + lane32; p < p1; p += 32) hsidx[p] = (uint16_t)(s0 + (p - p0));
         }
-        __syncthreads();
-        for (uint32_t s = threadIdx.x; s < tc.n_staged; s += blockDim.x) {
-            const uint32_t sc = scell[s];
-            const uint32_t gi = h.gstart[sc] + (s - h.sstart[sc]);
-            const double4 p = pos[gi];
-            const double4 v = vel[gi];
-            const double *cg = h.cgeo + 6 * sc;
-            ra[s] = make_double2(cg[3] + md_min_image(p.x - cg[0], g.L[0], g.h[0]),
-                                 cg[4] + md_min_image(p.y - cg[1], g.L[1], g.h[1]));
-            rb[s] = make_double2(cg[5] + md_min_image(p.z - cg[2], g.L[2], g.h[2]), v.x);
-            rc[s] = make_double2(v.y, v.z);
-            rt[s] = md_lane_to_tag(p.w);
-        }
+        struct PV { double4 p, v; };
+        tile_for_each_staged<PV>(
+            tc, h, [&](uint32_t gi) { PV x; x.p = pos[gi]; x.v = vel[gi]; return x; },
+            [&](uint32_t s, uint32_t sc, const PV &x) {
+                const double *cg = h.cgeo + 6 * sc;
+                ra[s] = make_double2(cg[3] + md_min_image(x.p.x - cg[0], g.L[0], g.h[0]),
+                                     cg[4] + md_min_image(x.p.y - cg[1], g.L[1], g.h[1]));
+                rb[s] = make_double2(cg[5] + md_min_image(x.p.z - cg[2], g.L[2], g.h[2]), x.v.x);
+                rc[s] = make_double2(x.v.y, x.v.z);
+                rt[s] = md_lane_to_tag(x.p.w);
+            });
         if (threadIdx.x < N_DUMMY) {
             ra[tc.n_staged + threadIdx.x] = make_double2(1e150, 1e150);
             rb[tc.n_staged + threadIdx.x] = make_double2(1e150, 0.0);
