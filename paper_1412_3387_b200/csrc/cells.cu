@@ -271,33 +271,36 @@ __device__ __forceinline__ unsigned long long cell_sort_key(const double4 p, con
 
 __global__ void k_cell_sort(const uint32_t *__restrict__ perm, const uint32_t *__restrict__ cell_start,
                             const uint32_t *__restrict__ tag, const double4 *__restrict__ pos, Geom g, bool subsort,
-                            uint32_t n_cells, uint32_t *perm_sorted, unsigned int *max_count)
+                            uint32_t n_cells, uint32_t lpc /* lanes per cell: 8, 16 or 32 */, uint32_t *perm_sorted,
+                            unsigned int *max_count)
 {
-    const uint32_t cell = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const unsigned lane = threadIdx.x & 31u;
-    if (cell >= n_cells) return;
+    // a group of lpc lanes per cell (from the mean population: a sparse DPD cell of 8 members does not need a warp)
+    const uint32_t cell = (blockIdx.x * blockDim.x + threadIdx.x) / lpc;
+    const unsigned lane = threadIdx.x & (lpc - 1u);
+    const unsigned gmask = lpc == 32u ? 0xffffffffu : (((1u << lpc) - 1u) << ((threadIdx.x & 31u) & ~(lpc - 1u)));
+    if (cell >= n_cells) return;  // (whole groups leave: n_cells * lpc threads are a multiple of lpc)
     const uint32_t b = cell_start[cell], e = cell_start[cell + 1], n = e - b;
     if (lane == 0 && n > 0) atomicMax(max_count, n);
-    // up to 64 members: keys in registers (2 per lane), ranks by shuffles; more: keys re-read from memory
-    if (n <= 64) {
+    // up to 2 lpc members: keys in registers (2 per lane), ranks by shuffles inside the group; more: keys re-read from memory
+    if (n <= 2u * lpc) {
         uint32_t idx[2];
         unsigned long long key[2];
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
-            const uint32_t m = lane + 32u * h;
+            const uint32_t m = lane + lpc * h;
             idx[h] = m < n ? perm[b + m] : 0u;
             key[h] = m < n ? cell_sort_key(pos[idx[h]], g, tag[idx[h]], subsort) : ~0ull;
         }
         uint32_t rank[2] = {0u, 0u};
         for (uint32_t k = 0; k < n; ++k) {
-            const unsigned long long kk = __shfl_sync(0xffffffffu, k < 32 ? key[0] : key[1], k & 31u);
+            const unsigned long long kk = __shfl_sync(gmask, k < lpc ? key[0] : key[1], k & (lpc - 1u), lpc);
             rank[0] += kk < key[0] ? 1u : 0u;
             rank[1] += kk < key[1] ? 1u : 0u;
         }
         if (lane < n) perm_sorted[b + rank[0]] = idx[0];
-        if (lane + 32u < n) perm_sorted[b + rank[1]] = idx[1];
+        if (lane + lpc < n) perm_sorted[b + rank[1]] = idx[1];
     } else {
-        for (uint32_t m = lane; m < n; m += 32) {
+        for (uint32_t m = lane; m < n; m += lpc) {
             const uint32_t idx = perm[b + m];
             const unsigned long long key = cell_sort_key(pos[idx], g, tag[idx], subsort);
             uint32_t rank = 0;
@@ -357,9 +360,11 @@ int launch_build_cells(md_ctx *c)
     MD_CUDA_CHECK(c, cudaMemsetAsync(c->cell_count, 0, sizeof(uint32_t) * c->n_cells, st));
     k_cell_scatter<<<md_grid(N, blk), blk, 0, st>>>(c->cell_rank_tmp, N, c->cell_start, c->cell_count, c->perm);
     MD_LAUNCH_CHECK(c);
-    k_cell_sort<<<md_grid((uint64_t)c->n_cells * 32, 256), 256, 0, st>>>(c->perm, c->cell_start, c->tag, c->pos, c->g,
-                                                                       c->use_tiles, c->n_cells, c->perm_sorted,
-                                                                       &c->d_flags->max_cell_count);
+    const double ppc = (double)c->N / (double)c->n_cells;
+    const uint32_t lpc = ppc <= 6.0 ? 8u : (ppc <= 13.0 ? 16u : 32u);  // 2 lpc members fit in registers; beyond: slow path
+    k_cell_sort<<<md_grid((uint64_t)c->n_cells * lpc, 256), 256, 0, st>>>(c->perm, c->cell_start, c->tag, c->pos, c->g,
+                                                                        c->use_tiles, c->n_cells, lpc, c->perm_sorted,
+                                                                        &c->d_flags->max_cell_count);
     MD_LAUNCH_CHECK(c);
     // new tags go to cell_rank_tmp (free now), then pointers are swapped
     uint32_t *ntag = c->cell_rank_tmp;
