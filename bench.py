@@ -284,8 +284,6 @@ def run_ours(args):
         md.set_bonds(w.bonds)
     if angles is not None:
         md.set_angles(angles)
-    if args.cluster:
-        md.set_option(B.MD_OPT_CLUSTER, 1)
     if args.brick:
         md.set_option(B.MD_OPT_TILE_BRICK, args.brick)
         md.set_state(d_pos, d_vel)
@@ -378,7 +376,7 @@ def run_ours(args):
         elif fk == "dpd":
             kernel = "k_tile_dpd2"
         elif precision == B.MD_MIXED:
-            kernel = "k_tile_lj4" if args.cluster else "k_tile_lj3"
+            kernel = "k_tile_lj3"
         else:
             kernel = "k_tile_lj3d"
         f_ms = st1["stage_ms"][fk] / max(1, st1["stage_launches"][fk])
@@ -449,7 +447,6 @@ def main():
                     help="md_step scheduler (MD_SCHED_*): batch = kernels of several steps enqueued ahead, gated on the device")
     ap.add_argument("--launch", nargs="*", default=[], help="kernel=block,w (with --no-tune)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cluster", action="store_true", help="MD_OPT_CLUSTER = 1: one neighbour row per cluster of 4")
     ap.add_argument("--r-buff", type=float, default=None, dest="r_buff",
                     help="override the configured skin r_buff = 0.4 (tuning sweep; not a reported configuration)")
     ap.add_argument("--angles", action="store_true", help="config 4 with harmonic angles along the chains (SURVEY 8(f) row 3)")

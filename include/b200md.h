@@ -221,7 +221,7 @@ int md_forces_lj(md_ctx *ctx, double epsilon, double sigma, int energy_shift);
    Uses the velocities as stored at the time of the call.  OVERWRITES force (energy lane = conservative energy). */
 int md_forces_dpd(md_ctx *ctx, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed);
 
-/* Harmonic bonds U = k/2 (r - r0)^2 (R6).  ACCUMULATES into force/energy. */
+/* Harmonic bonds U = k/2 (r - r0)^2 (R19).  ACCUMULATES into force/energy. */
 int md_forces_bonds(md_ctx *ctx, double k, double r0);
 
 /* ---- further short-range force fields (PAPER.md:63 feature list; fp64) ---------------------- */
@@ -298,12 +298,6 @@ int md_tune_rbuff(md_ctx *ctx, const md_step_desc *what, const double *candidate
    in fp32, the block sum is widened and added in fp64 (R25). */
 #define MD_OPT_TILE_BRICK 1
 #define MD_OPT_ACC_BLOCK 2
-/* MD_OPT_CLUSTER (MD_MIXED with MD_ORDER_MORTON only): 1 = the neighbour list is stored as one row per
-   cluster of 4 consecutive particles of a cell (members of a cell are ordered along a sub-cell Morton curve, so a
-   cluster is spatially compact); a row holds every particle within r_list of ANY member, and the LJ kernel evaluates
-   each stored candidate against the 4 members in registers.  The exported list is the exact
-   per-particle list either way.  0 (default) = one row per particle.  Invalidates the list. */
-#define MD_OPT_CLUSTER 3
 #define MD_OPT_RETUNE_PERIOD 4 /* rebuilds between periodic local re-scans of the tuner inside md_step; 0 (default) = never */
 int md_set_option(md_ctx *ctx, int option, int64_t value);
 

@@ -248,7 +248,7 @@ void orc_forces_dpd(const double *pos, const double *vel, uint64_t N, const doub
 
 /* ------------------------------------------------------------------------------------------------
  * O6 harmonic bonds (named PAPER.md:63; a bond is an unordered pair of particle IDs, PAPER.md:147;
- * U = k/2 (r - r0)^2, R6):  F_a += -k (r - r0) d/r, F_b -= same, d = minimg(x_a - x_b);
+ * U = k/2 (r - r0)^2, R19):  F_a += -k (r - r0) d/r, F_b -= same, d = minimg(x_a - x_b);
  * r == 0 gives zero force.  force (and energy if not NULL, half to each end) are ACCUMULATED.
  * ---------------------------------------------------------------------------------------------- */
 void orc_forces_bonds(const double *pos, uint64_t N, const double box[3], const uint32_t *tag_a,

@@ -721,29 +721,24 @@ static int build_nlist_tiles(md_ctx *c, bool *done)
     MD_TRY(md_read_flags(c));
     c->tile_max_home = c->h_flags->max_home;
     c->tile_max_staged = c->h_flags->max_staged;
-    const int mode = tile_cluster_ok(c) ? 1 : 0;
-    if (c->nl_stride == 0 || c->stride_mode != mode) {
+    if (c->nl_stride == 0) {
         // row stride from the mean density: 1.35 n + 24 covers the fluctuations of liquids and ideal gases at the
-        // configured densities; a longer row is detected by the build kernel and the stride grows.  Cluster rows hold
-        // the union of 4 neighbourhoods: the sphere grows by about the cluster radius (~ 0.75 of the mean spacing).
+        // configured densities; a longer row is detected by the build kernel and the stride grows
         const double vol = c->box[0] * c->box[1] * c->box[2];
         const double rho = (double)c->N / vol;
-        const double re = c->r_list + (mode ? 0.75 * pow(rho, -1.0 / 3.0) : 0.0);
-        const double nbar = rho * 4.18879020478639 * re * re * re;
+        const double nbar = rho * 4.18879020478639 * c->r_list * c->r_list * c->r_list;
         if (c->nl16) { md_free(c, c->nl16); c->nl16 = nullptr; }
         c->nl_stride = round16(1.35 * nbar + 24.0);
-        c->stride_mode = mode;
     }
     for (int attempt = 0; attempt < 3; ++attempt) {
         if (!c->nl16) MD_TRY(md_alloc(c, (void **)&c->nl16, (c->N + 1) * (uint64_t)c->nl_stride * sizeof(uint16_t)));  // + one row: the force kernels
                                                                                       // request block `lane` of a row before they know its length
         bool fits = false;
-        MD_TRY(launch_tile_build(c, mode == 1, &fits));
+        MD_TRY(launch_tile_build(c, &fits));
         if (!fits) return MD_OK;  // largest tile exceeds shared memory: general path
         MD_TRY(md_read_flags(c));
         if (c->h_flags->nl_overflow == 0) {
             c->nl_entries = c->h_flags->nl_total;
-            c->nl_cluster = mode == 1;
             c->nl_is_tile = true;
             c->nl32_decoded = false;
             *done = true;
@@ -857,16 +852,15 @@ extern "C" int md_get_nlist_rows(md_ctx *c, const uint32_t *probe_tags, uint32_t
 static int ensure_decoded(md_ctx *c);
 static int pair_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
 {
-    // cluster rows are read by k_tile_lj4 only (forces, no energies); everything else goes through the decoded list
     // a tile list whose largest tile fits the build kernel but not this force kernel's records goes through the decoded list
-    if (c->nl_is_tile && !(c->nl_cluster && (energy || c->precision != MD_MIXED)) && tile_forces_fit(c, false))
+    if (c->nl_is_tile && tile_forces_fit(c, false))
         return launch_tile_lj(c, eps, sigma, shift, energy);
     MD_TRY(ensure_decoded(c));
     return launch_forces_lj(c, eps, sigma, shift);
 }
 static int pair_dpd(md_ctx *c, double A, double gamma, double kT, double dt, uint64_t step, uint64_t seed)
 {
-    if (c->nl_is_tile && !c->nl_cluster && tile_forces_fit(c, true)) return launch_tile_dpd(c, A, gamma, kT, dt, step, seed);
+    if (c->nl_is_tile && tile_forces_fit(c, true)) return launch_tile_dpd(c, A, gamma, kT, dt, step, seed);
     MD_TRY(ensure_decoded(c));
     return launch_forces_dpd(c, A, gamma, kT, dt, step, seed);
 }
@@ -1342,7 +1336,7 @@ static int tune_all(md_ctx *c, const md_step_desc *w, int mode)
         // variant); only the block size is swept
         MD_TRY(tune_kernel(c, MD_K_NLIST, "nlist/tile", false, 1, mode, [&]() {
             bool fits = false;
-            const int st = launch_tile_build(c, c->nl_cluster, &fits);
+            const int st = launch_tile_build(c, &fits);
             if (!fits) c->tune_skip = true;  // this block size does not fit in shared memory
             return st;
         }));
@@ -1356,12 +1350,12 @@ static int tune_all(md_ctx *c, const md_step_desc *w, int mode)
     if (w->flags & MD_F_LJ)
         MD_TRY(tune_kernel(c, MD_K_LJ, c->nl_is_tile ? "lj/tile" : "lj", true, c->nl_is_tile && c->precision == MD_MIXED ? 8 : 32, mode, [&]() {
             // the row rotation of the tile list follows W (1, 2 or more lanes per particle): time each W on its own layout
-            if (c->nl_is_tile && !c->nl_cluster && c->nl_rotw != tile_rot_class(c->cfg[MD_K_LJ].w)) MD_TRY(do_build_nlist(c));
+            if (c->nl_is_tile && c->nl_rotw != tile_rot_class(c->cfg[MD_K_LJ].w)) MD_TRY(do_build_nlist(c));
             return pair_lj(c, w->lj_epsilon, w->lj_sigma, w->lj_energy_shift, false);
         }));
     if (w->flags & MD_F_DPD)
         MD_TRY(tune_kernel(c, MD_K_DPD, c->nl_is_tile ? "dpd/tile" : "dpd", true, 32, mode, [&]() {
-            if (c->nl_is_tile && !c->nl_cluster && c->nl_rotw != tile_rot_class(c->cfg[MD_K_DPD].w)) MD_TRY(do_build_nlist(c));
+            if (c->nl_is_tile && c->nl_rotw != tile_rot_class(c->cfg[MD_K_DPD].w)) MD_TRY(do_build_nlist(c));
             return pair_dpd(c, w->dpd_A, w->dpd_gamma, w->dpd_kT, w->dt, c->step, w->dpd_seed);
         }));
     if ((w->flags & MD_F_BONDS) && c->n_bonds)
@@ -1369,7 +1363,7 @@ static int tune_all(md_ctx *c, const md_step_desc *w, int mode)
     // half 1 with dt = 0 is the identity on positions and velocities (x + 0 v, v + 0 F/m) with the full memory traffic
     MD_TRY(tune_kernel(c, MD_K_INTEGRATE, "integrate", false, 1, mode, [&]() { return launch_half1(c, 0.0, false, false); }));
     // the list the run starts with has the layout of the chosen W
-    if (c->nl_is_tile && !c->nl_cluster) {
+    if (c->nl_is_tile) {
         const bool dpd = (w->flags & MD_F_DPD) != 0 && !(w->flags & MD_F_LJ);
         if (c->nl_rotw != tile_rot_class(c->cfg[dpd ? MD_K_DPD : MD_K_LJ].w)) MD_TRY(do_build_nlist(c));
     }
@@ -1497,11 +1491,6 @@ extern "C" int md_set_option(md_ctx *c, int option, int64_t value)
         MD_TRY(build_cell_order(c));
         c->cells_valid = c->nlist_valid = false;
         return MD_OK;
-    case MD_OPT_CLUSTER:
-        if (value != 0 && value != 1) { c->err = "md_set_option: cluster must be 0 or 1"; return MD_EINVAL; }
-        c->cluster_opt = (int)value;
-        c->nlist_valid = false;
-        return MD_OK;
     case MD_OPT_ACC_BLOCK:
         if (value != 1 && value != 8) { c->err = "md_set_option: accumulation block must be 1 or 8"; return MD_EINVAL; }
         c->acc_block = (int)value;
@@ -1538,11 +1527,6 @@ extern "C" int md_get_stats(md_ctx *c, md_stats *out)
     c->stats.nlist_capacity = c->nl_capacity;
     c->stats.device_bytes = c->device_bytes;
     c->stats.mean_neighbors = c->N ? (double)c->nl_entries / (double)c->N : 0.0;
-    if (c->nlist_valid && c->nl_is_tile && c->nl_cluster) {
-        // cluster rows: nl_entries counts stored candidates per cluster; the per-particle figure is the exact decoded list's
-        MD_TRY(ensure_decoded(c));
-        c->stats.mean_neighbors = c->N ? (double)c->nl_exact_entries / (double)c->N : 0.0;
-    }
     for (int a = 0; a < 3; ++a) c->stats.dims[a] = c->dims[a];
     c->stats.r_buff = c->r_buff;
     for (int k = 0; k < MD_N_KERNELS; ++k) {

@@ -247,7 +247,7 @@ __global__ void k_cell_scatter(const uint32_t *__restrict__ cell_rank, uint32_t 
 
 // (4) one warp per cell: order the cell's members by (sub-cell Morton key, tag) -- rank sort; tags are unique, so the
 // order is a pure function of the positions.  The sub-cell key (3 bits per axis of the position inside the cell) makes
-// runs of consecutive members spatially compact: the tile kernels treat 4 consecutive members as a cluster.
+// runs of consecutive members spatially compact: a build task of 8 consecutive members has a small extent.
 __device__ __forceinline__ uint32_t sub_coord(double x, double lo, double L, double dn, uint32_t n)
 {
     const double f = __dmul_rn(__ddiv_rn(__dsub_rn(x, lo), L), dn);

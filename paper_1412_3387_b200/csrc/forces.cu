@@ -169,7 +169,7 @@ int launch_forces_dpd(md_ctx *c, double A, double gamma, double kT, double dt, u
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// harmonic bonds (R6): every particle sums its own bonds (CSR by tag, partners ascending), no atomics.
+// harmonic (R19) and FENE (R33) bonds: every particle sums its own bonds (CSR by tag, partners ascending), no atomics.
 // ------------------------------------------------------------------------------------------------------------
 __global__ void k_forces_bonds(const double4 *__restrict__ pos, const uint32_t *__restrict__ tag,
                                const uint32_t *__restrict__ rtag, const uint32_t *__restrict__ bond_off,

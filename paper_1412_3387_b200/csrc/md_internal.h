@@ -130,9 +130,6 @@ struct md_ctx {
     double lj_sigma_hint = 1.0; // sigma of the latest LJ call / step description: sizes the near section at the build
     int nl_rotw = 4;            // lanes per particle (1, 2 or 4 = "4 or more") the rows of the current tile list are rotated for
 
-    bool nl_cluster = false;    // the current tile list has one row per cluster of 4 particles (k_tile_build_c)
-    int cluster_opt = 0;        // MD_OPT_CLUSTER
-    int stride_mode = -1;       // list format nl_stride was sized for (0 particle rows, 1 cluster rows)
     uint32_t tile_B = 1, n_tiles = 0;
     int tile_B_forced = 0, acc_block = 8;
     uint32_t *tile_cell_begin = nullptr, *tile_origin = nullptr, *lin_of_rank = nullptr;
@@ -257,8 +254,7 @@ int launch_debug_philox(md_ctx *c, const uint32_t *ctr, const uint32_t *key, uin
 int build_cell_order(md_ctx *c);  // host: rank_of_lin table for the configured curve (+ tile tables for Morton)
 // tiles.cu
 int tile_measure(md_ctx *c);
-int launch_tile_build(md_ctx *c, bool cluster, bool *fits);
-bool tile_cluster_ok(md_ctx *c);
+int launch_tile_build(md_ctx *c, bool *fits);
 int tile_build_lanes(md_ctx *c);  // lanes that cooperate on one particle in the tile build kernel in use
 static inline int tile_rot_class(int w) { return w <= 1 ? 1 : (w == 2 ? 2 : 4); }
 int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy);

@@ -985,166 +985,6 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build8(TileParams tp, G
 }
 
 // ===============================================================================================================
-// S2, cluster rows: one row per cluster of (up to) P = 4 consecutive members of a home cell (the same warp tasks as
-// above).  A candidate is kept when it lies within r_list (+ guard) of ANY member of the cluster; the cluster's own
-// members are left out (the force kernel handles the pairs inside a cluster separately).  The row is stored in the
-// row of the cluster's first particle, bank-class layout with rot = 0.  This is the w-threads-per-particle idea of
-// Fig. 4 with the roles turned: a staged candidate is loaded once and evaluated against 4 home particles held in
-// registers, in the list build and again in the force kernel, which cuts the shared-memory gathers 4-fold.
-// ===============================================================================================================
-template <int P>
-__global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_build_c(TileParams tp, Geom g, const float4 *__restrict__ rel, const double4 *__restrict__ pos,
-                                                                 float thr_out /* r_list^2 + guard */,
-                                                                 uint32_t max_staged, uint32_t *__restrict__ nl_cnt,
-                                                                 uint16_t *__restrict__ nl16, DevFlags *flags)
-{
-    extern __shared__ __align__(16) char smem_raw[];
-    const TileSmem h = tile_carve(smem_raw, tp.B);
-    float4 *rec = (float4 *)h.rest;
-    const uint32_t nw = blockDim.x >> 5;
-    const uint32_t stride = tp.stride, rcap = tp.stride + RB_EXTRA;
-    uint16_t *rowbuf = (uint16_t *)(h.rest + sizeof(float4) * (max_staged + N_DUMMY));  // [nw][stride + RB_EXTRA]
-    uint32_t *scratch = (uint32_t *)(rowbuf + (size_t)nw * rcap);                       // [nw][24]
-    uint8_t *scell = (uint8_t *)(scratch + nw * 24);                                    // [max_staged]
-
-    TileCtx tc;
-    tile_setup(tp, g, blockIdx.x, h, tc);
-    tile_stage_rel<true>(tc, h, rel, rec, scell, 1.f, pos, g);
-    if (threadIdx.x < 32) {  // first task of each home cell: exclusive scan of ceil(count / P), n_hc <= 64
-        uint32_t carry = 0;
-        for (uint32_t base = 0; base <= tc.n_hc; base += 32) {
-            const uint32_t hc = base + threadIdx.x;
-            const uint32_t v = hc < tc.n_hc ? (h.hc_first[hc + 1] - h.hc_first[hc] + P - 1) / P : 0u;
-            uint32_t inc = v;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t u = __shfl_up_sync(0xffffffffu, inc, o);
-                if ((int)threadIdx.x >= o) inc += u;
-            }
-            if (hc <= tc.n_hc) h.hc_task[hc] = carry + inc - v;
-            carry += __shfl_sync(0xffffffffu, inc, 31);
-        }
-    }
-    __syncthreads();
-
-    const unsigned lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;
-    const unsigned lt = md_lanemask_lt();
-    const uint32_t n_tasks = h.hc_task[tc.n_hc];
-    const uint32_t cls = lane & 7u;
-    const unsigned cmask_lt = (0x01010101u << cls) & lt, cmask = 0x01010101u << cls;
-    uint16_t *r = rowbuf + (size_t)wid * rcap;
-    uint32_t *sc = scratch + wid * 24;
-    unsigned long long total = 0;
-    uint32_t worst = 0;
-
-    for (uint32_t task = wid; task < n_tasks; task += nw) {
-        uint32_t hc = 0;
-        {
-            uint32_t lo = 0, hi = tc.n_hc;
-            while (hi - lo > 1) {
-                const uint32_t mid = (lo + hi) >> 1;
-                if (h.hc_task[mid] <= task) lo = mid; else hi = mid;
-            }
-            hc = lo;
-        }
-        const uint32_t p0 = h.hc_first[hc] + (task - h.hc_task[hc]) * P;
-        const uint32_t np = min((uint32_t)P, h.hc_first[hc + 1] - p0);
-        const uint32_t sch = h.hc_sc[hc];
-        const uint32_t ixh = sch % tc.sx, iyh = (sch / tc.sx) % tc.sy, izh = sch / (tc.sx * tc.sy);
-        const uint32_t self0 = h.sstart[sch] + (p0 - h.hc_first[hc]);
-        float ax[P], ay[P], az[P], th[P];
-#pragma unroll
-        for (int q = 0; q < P; ++q) {
-            const float4 m = rec[self0 + min((uint32_t)q, np - 1)];
-            ax[q] = -2.f * m.x; ay[q] = -2.f * m.y; az[q] = -2.f * m.z;
-            th[q] = thr_out - m.w;  // an absent member repeats the last one
-        }
-        uint32_t cntc = 0;
-#pragma unroll 1
-        for (int run = 0; run < 9; ++run) {
-            const uint32_t iy = iyh + (run % 3) - 1, iz = izh + (run / 3) - 1;
-            const uint32_t sc0 = (ixh - 1) + tc.sx * (iy + tc.sy * iz);
-            const uint32_t b = h.sstart[sc0], e = h.sstart[sc0 + 3];
-#pragma unroll 1
-            for (uint32_t base = b & ~7u; base < e; base += 32) {
-                const uint32_t j = base + lane;
-                const float4 pj = rec[(j >= b && j < e) ? j : tc.n_staged];
-                bool hit = false;
-#pragma unroll
-                for (int q = 0; q < P; ++q) {
-                    float t = fmaf(ax[q], pj.x, pj.w);
-                    t = fmaf(ay[q], pj.y, t);
-                    t = fmaf(az[q], pj.z, t);
-                    hit |= t < th[q];
-                }
-                hit &= j - self0 >= np;  // not a member of this cluster
-                const unsigned bal = __ballot_sync(0xffffffffu, hit);
-                if (bal) {
-                    const uint32_t k = cntc + __popc(bal & cmask_lt);
-                    const uint32_t o = 8u * k + ((cls - k) & 7u);
-                    if (hit && o < rcap) r[o] = (uint16_t)(j << tp.shift);
-                    cntc += __popc(bal & cmask);
-                }
-            }
-        }
-        __syncwarp();
-        {
-            uint32_t n = cntc, mx = cntc;
-#pragma unroll
-            for (int o = 1; o < 8; o <<= 1) {
-                n += __shfl_xor_sync(0xffffffffu, n, o);
-                mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-            }
-            uint32_t need = (n + 7u) & ~7u;
-            if (8u * mx > rcap) need = max(need, 8u * mx - RB_EXTRA);
-            worst = max(worst, need);
-            const uint32_t nblk = min((n + 7u) >> 3, stride >> 3);
-            const uint32_t nck = min(cntc, rcap >> 3);
-            const uint32_t holes = nblk > nck ? nblk - nck : 0u, over = nck > nblk ? nck - nblk : 0u;
-            uint32_t hs = holes, os = over;
-#pragma unroll
-            for (int o = 1; o < 8; o <<= 1) {
-                const uint32_t a = __shfl_up_sync(0xffffffffu, hs, o, 8), bb = __shfl_up_sync(0xffffffffu, os, o, 8);
-                if ((int)cls >= o) { hs += a; os += bb; }
-            }
-            const uint32_t n_holes = __shfl_sync(0xffffffffu, hs, 7), n_over = __shfl_sync(0xffffffffu, os, 7);
-            if (lane < 8) {
-                sc[lane] = nck;
-                sc[8 + lane] = hs - holes;
-                sc[16 + lane] = os - over;
-            }
-            __syncwarp();
-            for (uint32_t o = lane; o < n_holes; o += 32) {
-                uint32_t c = 0;
-#pragma unroll
-                for (int k = 1; k < 8; ++k) c += o >= sc[8 + k] ? 1u : 0u;
-                const uint32_t bk = sc[c] + (o - sc[8 + c]);
-                uint16_t v;
-                if (o < n_over) {
-                    uint32_t cs = 0;
-#pragma unroll
-                    for (int k = 1; k < 8; ++k) cs += o >= sc[16 + k] ? 1u : 0u;
-                    const uint32_t k2 = nblk + (o - sc[16 + cs]);
-                    v = r[8u * k2 + ((cs - k2) & 7u)];
-                } else {
-                    v = (uint16_t)((tc.n_staged + ((c - tc.n_staged) & 7u)) << tp.shift);
-                }
-                r[8u * bk + ((c - bk) & 7u)] = v;
-            }
-            __syncwarp();
-            uint4 *dst = (uint4 *)(nl16 + (size_t)(tc.g0 + p0) * stride);
-            const uint4 *src = (const uint4 *)r;
-            for (uint32_t v = lane; v < nblk; v += 32) dst[v] = src[v];
-            if (lane < np) nl_cnt[tc.g0 + p0 + lane] = lane == 0 ? min(n, 8u * nblk) : 0u;
-            total += n;
-        }
-        __syncwarp();
-    }
-    if (lane == 0 && total) atomicAdd(&flags->nl_total, total);
-    if (worst > stride) atomicMax(&flags->nl_overflow, worst);
-}
-
-// ===============================================================================================================
 // S4a LJ forces, one CTA per tile, W threads per home particle
 // ===============================================================================================================
 struct LJTile {
@@ -1295,12 +1135,6 @@ struct LJ3U {
     float sig2f;
 };
 
-struct LJ3 {
-    double rc2_exact;     // rc^2 in box units (exact re-test)
-    double inv_sigma;     // staging scale
-    double fscale;        // 48 eps / sigma
-    float rc2s, guard;    // rc'^2 and the guard band in scaled units
-};
 
 __device__ __forceinline__ float4 lds_f4(uint32_t addr)
 {
@@ -1766,270 +1600,6 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj3d(TileParams tp, Geo
 }
 
 // ===============================================================================================================
-// S4a, mixed precision, cluster rows (k_tile_build_c): k_tile_lj4.  W lanes share a cluster of 4 home particles
-// (i0..i3, held in registers as two packed pairs) and stride over the blocks of the cluster's row; every staged
-// candidate j is loaded once (one LDS.128) and evaluated against the 4 members with f32x2 arithmetic.  Same
-// arithmetic and guard-band rule as k_tile_lj3; a lane sums its share of the row in fp32, the lanes' sums are widened
-// and reduced in fp64.  The pairs inside a cluster are not in the row: lane m < 4 of the group evaluates member m as
-// a candidate with its own pair masked.
-// ===============================================================================================================
-struct LJ4Acc {
-    unsigned long long xa, ya, za, xb, yb, zb;  // packed fp32 sums for members (0,1) and (2,3)
-};
-
-template <bool MASK>
-__device__ __forceinline__ void lj4_pair2(unsigned long long nx, unsigned long long ny, unsigned long long nz,
-                                          unsigned long long xj, unsigned long long yj, unsigned long long zj,
-                                          unsigned long long mrc2, unsigned long long mhalf, float nguard, float &band,
-                                          bool m0, bool m1, unsigned long long &ax, unsigned long long &ay,
-                                          unsigned long long &az)
-{
-    // d' = x_j - x_i (the sign is undone when the sums are written out)
-    const unsigned long long dx = f2_add(xj, nx), dy = f2_add(yj, ny), dz = f2_add(zj, nz);
-    const unsigned long long r2 = f2_fma(dz, dz, f2_fma(dy, dy, f2_mul(dx, dx)));
-    const unsigned long long d = f2_add(r2, mrc2);
-    float r2a, r2b, da, db;
-    f2_unpack(r2, r2a, r2b);
-    f2_unpack(d, da, db);
-    band = fminf(band, fminf(fabsf(da), fabsf(db)));
-    const unsigned long long ri = f2_pack(md_rcp(r2a), md_rcp(r2b));
-    const unsigned long long s6 = f2_mul(f2_mul(ri, ri), ri);
-    const unsigned long long ff = f2_mul(f2_add(s6, mhalf), f2_mul(s6, ri));
-    float fa, fb;
-    f2_unpack(ff, fa, fb);
-    fa = (da < nguard && (!MASK || m0)) ? fa : 0.f;
-    fb = (db < nguard && (!MASK || m1)) ? fb : 0.f;
-    const unsigned long long f = f2_pack(fa, fb);
-    ax = f2_fma(f, dx, ax);
-    ay = f2_fma(f, dy, ay);
-    az = f2_fma(f, dz, az);
-}
-
-// slow path of one block of 8 entries for the 4 members.  The fast path treats a pair inside the guard band as out of
-// range, so all that is left to do is ADD the pairs of the band that the exact fp64 test puts inside rc (R26).
-__device__ __noinline__ void lj4_block_corr(const uint4 q, uint32_t rec_addr, uint32_t self_addr, uint32_t np, float rc2s,
-                                           float guard, const double4 *__restrict__ pos, double Lx, double Ly, double Lz,
-                                           double rc2_exact, uint32_t gi0, const uint32_t *gstart, const uint32_t *sstart,
-                                           uint32_t n_sc, float *out /* [12]: sums of f d', member-major */)
-{
-    const uint32_t qq[4] = {q.x, q.y, q.z, q.w};
-#pragma unroll 1
-    for (uint32_t m = 0; m < 4; ++m) {
-        float ax = 0.f, ay = 0.f, az = 0.f;
-        if (m < np) {
-            const float4 me = lds_f4(self_addr + 16u * m);
-#pragma unroll 1
-            for (int e = 0; e < 8; ++e) {
-                const uint32_t off = (e & 1) ? (qq[e >> 1] >> 16) : (qq[e >> 1] & 0xffffu);
-                const float4 pj = lds_f4(rec_addr + off);
-                const float dx = pj.x - me.x, dy = pj.y - me.y, dz = pj.z - me.z;
-                const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                if (fabsf(r2 - rc2s) < guard) {
-                    const uint32_t s = off >> 4;
-                    uint32_t lo = 0, hi = n_sc;
-                    while (hi - lo > 1) {
-                        const uint32_t mid = (lo + hi) >> 1;
-                        if (sstart[mid] <= s) lo = mid; else hi = mid;
-                    }
-                    if (tile_exact_r2_impl(pos, Lx, Ly, Lz, gi0 + m, gstart[lo] + (s - sstart[lo])) < rc2_exact) {
-                        const float rinv2 = md_rcp(r2);
-                        const float s6 = rinv2 * rinv2 * rinv2;
-                        const float f = (s6 - 0.5f) * (s6 * rinv2);
-                        ax = fmaf(f, dx, ax); ay = fmaf(f, dy, ay); az = fmaf(f, dz, az);
-                    }
-                }
-            }
-        }
-        out[3 * m] = ax; out[3 * m + 1] = ay; out[3 * m + 2] = az;
-    }
-}
-
-// the same for the pairs inside a cluster, seen from candidate = member `cand`
-__device__ __noinline__ void lj4_intra_corr(uint32_t self_addr, uint32_t np, uint32_t cand, float rc2s, float guard,
-                                           const double4 *__restrict__ pos, double Lx, double Ly, double Lz,
-                                           double rc2_exact, uint32_t gi0, float *out)
-{
-    const float4 pj = lds_f4(self_addr + 16u * cand);
-#pragma unroll 1
-    for (uint32_t m = 0; m < 4; ++m) {
-        float ax = 0.f, ay = 0.f, az = 0.f;
-        if (m < np && m != cand) {
-            const float4 me = lds_f4(self_addr + 16u * m);
-            const float dx = pj.x - me.x, dy = pj.y - me.y, dz = pj.z - me.z;
-            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            if (fabsf(r2 - rc2s) < guard && tile_exact_r2_impl(pos, Lx, Ly, Lz, gi0 + m, gi0 + cand) < rc2_exact) {
-                const float rinv2 = md_rcp(r2);
-                const float s6 = rinv2 * rinv2 * rinv2;
-                const float f = (s6 - 0.5f) * (s6 * rinv2);
-                ax = f * dx; ay = f * dy; az = f * dz;
-            }
-        }
-        out[3 * m] = ax; out[3 * m + 1] = ay; out[3 * m + 2] = az;
-    }
-}
-
-__device__ __forceinline__ void lj4_add(LJ4Acc &a, const float *o)
-{
-    a.xa = f2_add(a.xa, f2_pack(o[0], o[3])); a.ya = f2_add(a.ya, f2_pack(o[1], o[4])); a.za = f2_add(a.za, f2_pack(o[2], o[5]));
-    a.xb = f2_add(a.xb, f2_pack(o[6], o[9])); a.yb = f2_add(a.yb, f2_pack(o[7], o[10])); a.zb = f2_add(a.zb, f2_pack(o[8], o[11]));
-}
-
-template <int W, int MINB>
-__global__ void __launch_bounds__(256, MINB) k_tile_lj4(TileParams tp, Geom g, const double4 *__restrict__ pos,
-                                                        const float4 *__restrict__ rel,
-                                                        const uint32_t *__restrict__ nl_cnt,
-                                                        const uint16_t *__restrict__ nl16, LJ3 lj, uint32_t max_staged,
-                                                        uint32_t max_clusters, double4 *__restrict__ force, Gate gate)
-{
-    if (md_gate_closed(gate)) return;
-    extern __shared__ __align__(16) char smem_raw[];
-    float4 *rec = (float4 *)smem_raw;  // records first: their shared-memory address is a launch constant
-    const TileSmem h = tile_carve(smem_raw + sizeof(float4) * (max_staged + N_DUMMY), tp.B);
-    uint8_t *scell = (uint8_t *)h.rest;
-    uint32_t *ctab = (uint32_t *)(scell + ((max_staged + 16) & ~15u));  // per cluster: (first member p0 | members << 24,
-                                                                        // staged index of the first member)
-    __shared__ uint32_t n_clusters;
-
-    TileCtx tc;
-    tile_setup(tp, g, blockIdx.x, h, tc);
-    tile_stage_rel<false>(tc, h, rel, rec, scell, (float)lj.inv_sigma, pos, g);
-    if (threadIdx.x < 32) {  // first cluster of each home cell (n_hc <= 64), as in the build kernel
-        uint32_t carry = 0;
-        for (uint32_t base = 0; base <= tc.n_hc; base += 32) {
-            const uint32_t hc = base + threadIdx.x;
-            const uint32_t v = hc < tc.n_hc ? (h.hc_first[hc + 1] - h.hc_first[hc] + 3u) / 4u : 0u;
-            uint32_t inc = v;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t u = __shfl_up_sync(0xffffffffu, inc, o);
-                if ((int)threadIdx.x >= o) inc += u;
-            }
-            if (hc <= tc.n_hc) h.hc_task[hc] = carry + inc - v;
-            carry += __shfl_sync(0xffffffffu, inc, 31);
-        }
-        if (threadIdx.x == 0) n_clusters = carry;
-    }
-    __syncthreads();
-    // per cluster also the negated member coordinates as packed pairs (-x0,-x1) (-y0,-y1) (-z0,-z1) (-x2,-x3) ...:
-    // the force loop loads them with 64-bit loads straight into aligned register pairs.  An absent member is the
-    // far-away dummy record (all its pairs are out of range).
-    float2 *mtab = (float2 *)(ctab + 2 * max_clusters);
-    for (uint32_t hc = threadIdx.x >> 5; hc < tc.n_hc; hc += blockDim.x >> 5) {
-        const uint32_t p0 = h.hc_first[hc], p1 = h.hc_first[hc + 1], t0 = h.hc_task[hc];
-        const uint32_t s0 = h.sstart[h.hc_sc[hc]];
-        for (uint32_t k = threadIdx.x & 31u; 4u * k < p1 - p0; k += 32) {
-            const uint32_t np = min(4u, p1 - p0 - 4u * k), s = s0 + 4u * k;
-            ctab[2 * (t0 + k)] = (p0 + 4u * k) | (np << 24);
-            ctab[2 * (t0 + k) + 1] = s;
-            const float4 m0 = rec[s], m1 = rec[np > 1 ? s + 1 : tc.n_staged], m2 = rec[np > 2 ? s + 2 : tc.n_staged],
-                         m3 = rec[np > 3 ? s + 3 : tc.n_staged];
-            float2 *mt = mtab + 6 * (t0 + k);
-            mt[0] = make_float2(-m0.x, -m1.x); mt[1] = make_float2(-m0.y, -m1.y); mt[2] = make_float2(-m0.z, -m1.z);
-            mt[3] = make_float2(-m2.x, -m3.x); mt[4] = make_float2(-m2.y, -m3.y); mt[5] = make_float2(-m2.z, -m3.z);
-        }
-    }
-    __syncthreads();
-
-    const unsigned lane = threadIdx.x & (W - 1);
-    const unsigned seg_mask = md_seg_mask<W>();
-    const uint32_t n_groups = blockDim.x / W;
-    const uint32_t rec_addr = (uint32_t)__cvta_generic_to_shared(rec);
-    const float rc2s = lj.rc2s, guard = lj.guard, nguard = -lj.guard;
-    const uint32_t stride8 = tp.stride >> 3;
-    const unsigned long long mrc2 = f2_pack_fixed(-rc2s, -rc2s), mhalf = f2_pack(-0.5f, -0.5f);
-    const uint32_t ncl = n_clusters;
-    const uint32_t mtab_addr = (uint32_t)__cvta_generic_to_shared(mtab);
-
-    uint32_t cl = threadIdx.x / W;
-    uint32_t cnt_c = 0;
-    uint4 q_c = make_uint4(0, 0, 0, 0);
-    if (cl < ncl) {  // software pipeline over the group's clusters, as in k_tile_lj3
-        const uint32_t gp = tc.g0 + (ctab[2 * cl] & 0xffffffu);
-        cnt_c = __ldg(nl_cnt + gp) & MD_NL_CNT_MASK;
-        q_c = __ldg((const uint4 *)nl16 + (size_t)gp * stride8 + lane);
-    }
-    for (; cl < ncl; cl += n_groups) {
-        const uint2 ce = *(const uint2 *)(ctab + 2 * cl);
-        const uint32_t p0 = ce.x & 0xffffffu, np = ce.x >> 24;
-        const uint32_t self_addr = rec_addr + 16u * ce.y;  // members of a cell are consecutive staged records
-        // negated member coordinates, packed (0,1) and (2,3)
-        const uint32_t mt_addr = mtab_addr + 48u * cl;
-        const unsigned long long nxa = lds_u64(mt_addr), nya = lds_u64(mt_addr + 8), nza = lds_u64(mt_addr + 16),
-                                 nxb = lds_u64(mt_addr + 24), nyb = lds_u64(mt_addr + 32), nzb = lds_u64(mt_addr + 40);
-        // this lane's share of the cluster's pairs is summed in fp32 (R25); lanes are widened and reduced in fp64
-        LJ4Acc a = {0ull, 0ull, 0ull, 0ull, 0ull, 0ull};
-
-        // pairs inside the cluster: lane m evaluates member m as the candidate, its own pair (and absent members) masked
-        {
-            float band = 3e38f;
-            const bool act = lane < np;
-            const float4 pj = lds_f4(act ? self_addr + 16u * lane : rec_addr + 16u * tc.n_staged);
-            const unsigned long long xj = f2_pack(pj.x, pj.x), yj = f2_pack(pj.y, pj.y), zj = f2_pack(pj.z, pj.z);
-            lj4_pair2<true>(nxa, nya, nza, xj, yj, zj, mrc2, mhalf, nguard, band, lane != 0, lane != 1, a.xa, a.ya, a.za);
-            lj4_pair2<true>(nxb, nyb, nzb, xj, yj, zj, mrc2, mhalf, nguard, band, lane != 2, lane != 3, a.xb, a.yb, a.zb);
-            if (band < guard && act) {  // the own pair has |d| = rc'^2: never in the band
-                float o[12];
-                lj4_intra_corr(self_addr, np, lane, rc2s, guard, pos, g.L[0], g.L[1], g.L[2], lj.rc2_exact, tc.g0 + p0, o);
-                lj4_add(a, o);
-            }
-        }
-
-        const uint32_t nblk = (cnt_c + 7u) >> 3;
-        const uint4 *row = (const uint4 *)nl16 + (size_t)(tc.g0 + p0) * stride8;
-        uint4 q = q_c;
-        if (cl + n_groups < ncl) {
-            const uint32_t gp = tc.g0 + (ctab[2 * (cl + n_groups)] & 0xffffffu);
-            cnt_c = __ldg(nl_cnt + gp) & MD_NL_CNT_MASK;
-            q_c = __ldg((const uint4 *)nl16 + (size_t)gp * stride8 + lane);
-        }
-        for (uint32_t b = lane; b < nblk; b += W) {
-            const uint4 qn = b + W < nblk ? __ldg(row + b + W) : q;  // prefetch the next block of 8 entries
-            float band = 3e38f;
-#pragma unroll 1
-            for (int k = 0; k < 4; ++k) {  // 2 entries per trip: more unrolling only buys register spills
-                const uint32_t w = k == 0 ? q.x : (k == 1 ? q.y : (k == 2 ? q.z : q.w));
-                const float4 pa = lds_f4(rec_addr + (w & 0xffffu));
-                const float4 pb = lds_f4(rec_addr + (w >> 16));
-                {
-                    const unsigned long long xj = f2_pack(pa.x, pa.x), yj = f2_pack(pa.y, pa.y), zj = f2_pack(pa.z, pa.z);
-                    lj4_pair2<false>(nxa, nya, nza, xj, yj, zj, mrc2, mhalf, nguard, band, true, true, a.xa, a.ya, a.za);
-                    lj4_pair2<false>(nxb, nyb, nzb, xj, yj, zj, mrc2, mhalf, nguard, band, true, true, a.xb, a.yb, a.zb);
-                }
-                {
-                    const unsigned long long xj = f2_pack(pb.x, pb.x), yj = f2_pack(pb.y, pb.y), zj = f2_pack(pb.z, pb.z);
-                    lj4_pair2<false>(nxa, nya, nza, xj, yj, zj, mrc2, mhalf, nguard, band, true, true, a.xa, a.ya, a.za);
-                    lj4_pair2<false>(nxb, nyb, nzb, xj, yj, zj, mrc2, mhalf, nguard, band, true, true, a.xb, a.yb, a.zb);
-                }
-            }
-            if (band < guard) {  // some pair of this block is inside the guard band: exact decisions (rare)
-                float o[12];
-                lj4_block_corr(q, rec_addr, self_addr, np, rc2s, guard, pos, g.L[0], g.L[1], g.L[2], lj.rc2_exact,
-                               tc.g0 + p0, h.gstart, h.sstart, tc.n_sc, o);
-                lj4_add(a, o);
-            }
-            q = qn;
-        }
-        // member `lane & 3` of the sums: sum over the W lanes in fp64, lane m < np writes member m.
-        float t[12];
-        f2_unpack(a.xa, t[0], t[3]); f2_unpack(a.ya, t[1], t[4]); f2_unpack(a.za, t[2], t[5]);
-        f2_unpack(a.xb, t[6], t[9]); f2_unpack(a.yb, t[7], t[10]); f2_unpack(a.zb, t[8], t[11]);
-        double fx = 0.0, fy = 0.0, fz = 0.0;
-#pragma unroll
-        for (int m = 0; m < 4; ++m) {
-            const double sx = md_seg_sum<W>((double)t[3 * m], seg_mask);
-            const double sy = md_seg_sum<W>((double)t[3 * m + 1], seg_mask);
-            const double sz = md_seg_sum<W>((double)t[3 * m + 2], seg_mask);
-            if (lane == (unsigned)m) { fx = sx; fy = sy; fz = sz; }
-        }
-        // the sums hold f (x_j - x_i): F_i = -(48 eps / sigma) sum
-        if (lane < np) {
-            const double sc = -lj.fscale;
-            force[tc.g0 + p0 + lane] = make_double4(fx * sc, fy * sc, fz * sc, 0.0);
-        }
-    }
-}
-
-// ===============================================================================================================
 // S4b DPD forces, one CTA per tile, W threads per home particle, fp64; positions, velocities and tags staged
 // ===============================================================================================================
 struct DPDTile {
@@ -2260,7 +1830,7 @@ __global__ void __launch_bounds__(MD_DPD2_MAX_BLOCK, 4) k_tile_dpd2(TileParams t
 template <bool FILL>
 __global__ void k_tile_decode(TileParams tp, Geom g, const double *__restrict__ pos_ref,
                               const uint32_t *__restrict__ nl_cnt, const uint16_t *__restrict__ nl16, double rl2,
-                              bool cluster, uint32_t *__restrict__ cnt32, const uint64_t *__restrict__ nl_off,
+                              uint32_t *__restrict__ cnt32, const uint64_t *__restrict__ nl_off,
                               uint32_t *nl_idx)
 {
     extern __shared__ __align__(16) char smem_raw[];
@@ -2271,13 +1841,7 @@ __global__ void k_tile_decode(TileParams tp, Geom g, const double *__restrict__ 
     const unsigned lt = md_lanemask_lt();
     for (uint32_t p = wid; p < tc.n_home; p += nw) {
         const uint32_t gi = tc.g0 + p;
-        uint32_t rowg = gi, p0 = p, np = 1;
-        if (cluster) {  // the row of p's cluster is stored with the cluster's first member
-            const uint32_t hc = tile_home_cell(h, tc.n_hc, p);
-            p0 = h.hc_first[hc] + ((p - h.hc_first[hc]) & ~3u);
-            np = min(4u, h.hc_first[hc + 1] - p0);
-            rowg = tc.g0 + p0;
-        }
+        const uint32_t rowg = gi;
         const uint32_t cnt = ((nl_cnt[rowg] & MD_NL_CNT_MASK) + 7u) & ~7u;  // stored rows are whole blocks of 8, dummies interspersed
         const uint16_t *row = nl16 + (size_t)rowg * tp.stride;
         const double xi = pos_ref[3ull * gi], yi = pos_ref[3ull * gi + 1], zi = pos_ref[3ull * gi + 2];
@@ -2296,19 +1860,6 @@ __global__ void k_tile_decode(TileParams tp, Geom g, const double *__restrict__ 
                     const double dz = md_min_image(__dsub_rn(zi, pos_ref[3ull * gj + 2]), g.L[2], g.h[2]);
                     keep = md_r2_exact(dx, dy, dz) < rl2;
                 }
-            }
-            const unsigned bal = __ballot_sync(0xffffffffu, keep);
-            if (FILL && keep) out[n + __popc(bal & lt)] = gj;
-            n += __popc(bal);
-        }
-        if (cluster) {  // the other members of the cluster are not in the row
-            bool keep = false;
-            const uint32_t gj = tc.g0 + p0 + lane;
-            if (lane < np && gj != gi) {
-                const double dx = md_min_image(__dsub_rn(xi, pos_ref[3ull * gj]), g.L[0], g.h[0]);
-                const double dy = md_min_image(__dsub_rn(yi, pos_ref[3ull * gj + 1]), g.L[1], g.h[1]);
-                const double dz = md_min_image(__dsub_rn(zi, pos_ref[3ull * gj + 2]), g.L[2], g.h[2]);
-                keep = md_r2_exact(dx, dy, dz) < rl2;
             }
             const unsigned bal = __ballot_sync(0xffffffffu, keep);
             if (FILL && keep) out[n + __popc(bal & lt)] = gj;
@@ -2421,8 +1972,6 @@ static const size_t TILE_SMEM_LIMIT = 227 * 1024 - 64;
 static uint32_t tile_shift(md_ctx *c) { return c->tile_max_staged + N_DUMMY <= 4096 ? 4u : 0u; }
 
 // returns MD_OK and sets *fits = false if the largest tile does not fit in shared memory (caller falls back)
-// cluster rows need pre-shifted 16-bit entries (byte offsets of float4 records)
-bool tile_cluster_ok(md_ctx *c) { return c->precision == MD_MIXED && c->cluster_opt && tile_shift(c) == 4u; }
 
 static int tile_build_mode()
 {
@@ -2430,23 +1979,23 @@ static int tile_build_mode()
     return build_mode;
 }
 // k_tile_build8: 4 candidate phases per home particle; ballot variants: a full warp
-int tile_build_lanes(md_ctx *c) { return (!c->nl_cluster && tile_build_mode() == 8) ? 4 : 32; }
+int tile_build_lanes(md_ctx *) { return tile_build_mode() == 8 ? 4 : 32; }
 
-int launch_tile_build(md_ctx *c, bool cluster, bool *fits)
+int launch_tile_build(md_ctx *c, bool *fits)
 {
     const uint32_t ms = c->tile_max_staged;
     const int block = std::min(c->cfg[MD_K_NLIST].block, TILE_MAX_BLOCK);
     const uint32_t nw = (uint32_t)block / 32;
     size_t smem = tile_smem_common(c, sizeof(float4), false);
-    const bool b8 = !cluster && tile_build_mode() == 8;
-    const size_t rows = cluster ? 1 : (b8 ? BUILD8_P : BUILD_P);
+    const bool b8 = tile_build_mode() == 8;
+    const size_t rows = b8 ? BUILD8_P : BUILD_P;
     smem += sizeof(uint16_t) * (size_t)nw * rows * (c->nl_stride + RB_EXTRA + (b8 ? 8 : 0)) + sizeof(uint32_t) * nw * (b8 ? 4 : rows) * 24;  // row assembly
     *fits = smem <= TILE_SMEM_LIMIT && ms + N_DUMMY <= 65536 && c->tile_B <= 4;
     if (!*fits) return MD_OK;
     c->nl_shift = tile_shift(c);
     {   // the force kernel that will read the list: the last step description says which, else LJ
         const bool dpd = (c->force_hint & MD_F_DPD) != 0 && !(c->force_hint & MD_F_LJ);
-        c->nl_rotw = cluster ? 4 : tile_rot_class(c->cfg[dpd ? MD_K_DPD : MD_K_LJ].w);
+        c->nl_rotw = tile_rot_class(c->cfg[dpd ? MD_K_DPD : MD_K_LJ].w);
     }
     const double R = c->r_list * 1.001, E = tile_extent(c), rl2 = c->r_list * c->r_list;
     MD_CUDA_CHECK(c, cudaMemsetAsync(&c->d_flags->nl_total, 0, sizeof(unsigned long long), c->stream));
@@ -2458,16 +2007,12 @@ int launch_tile_build(md_ctx *c, bool cluster, bool *fits)
     float thr_near = 0.f;
     c->nl_near_r = 0.0;
     static const double near_sig = getenv("B200MD_NEAR") ? atof(getenv("B200MD_NEAR")) : MD_NEAR_SIGMAS;  // diagnostic
-    if (!cluster && b8 && c->precision == MD_MIXED && near_sig > 0.0) {
+    if (b8 && c->precision == MD_MIXED && near_sig > 0.0) {
         c->nl_near_r = near_sig * c->lj_sigma_hint;
         const double rn = c->nl_near_r + c->r_buff;
         thr_near = (float)(rn * rn + gd);
     }
-    if (cluster) {
-        MD_TRY(set_smem(c, k_tile_build_c<BUILD_P>, smem));
-        k_tile_build_c<BUILD_P><<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->rel, c->pos, (float)(rl2 + gd), ms, c->nl_cnt,
-                                                                       c->nl16, c->d_flags);
-    } else if (b8) {
+    if (b8) {
         MD_TRY(set_smem(c, k_tile_build8, smem));
         k_tile_build8<<<c->n_tiles, block, smem, c->stream>>>(tp, c->g, c->rel, c->pos, (float)(rl2 + gd), thr_near, ms, c->nl_cnt,
                                                              c->nl16, c->d_flags);
@@ -2525,39 +2070,7 @@ int launch_tile_lj(md_ctx *c, double eps, double sigma, int shift, bool energy)
     const size_t smem = tile_smem_common(c, mixed ? sizeof(float4) : sizeof(double4), false);
     TileParams tp = make_tp(c);
     static const int lj3_mode = getenv("B200MD_LJ3") ? atoi(getenv("B200MD_LJ3")) : 2;
-    if (c->nl_cluster) {
-        if (!mixed || energy || !c->nl_shift) { c->err = "launch_tile_lj: cluster rows serve mixed-precision forces only"; return MD_ESTATE; }
-        // records, header, staged-cell table, cluster table (2 words per cluster; at most n_home / 4 + one per home cell)
-        const size_t ncl_max = c->tile_max_home / 4 + (size_t)c->tile_B * c->tile_B * c->tile_B + 1;
-        const size_t smem4 = tile_smem_common(c, sizeof(float4), false) + (8 + 48) * ncl_max;
-        LJ3 q;
-        q.rc2_exact = p.rc2_exact;
-        q.inv_sigma = 1.0 / sigma;
-        q.fscale = 48.0 * eps / sigma;
-        const double rc2s = p.rc2_exact / p.sig2;
-        q.rc2s = (float)rc2s;
-        q.guard = (float)(1.0001 * (gd / p.sig2 + 2.0 * 5.9604644775390625e-08 * rc2s));
-        const int block = std::min(cf.block, 256);
-        if (cf.w >= 8) {
-            MD_TRY(set_smem(c, (k_tile_lj4<8, 3>), smem4));
-            k_tile_lj4<8, 3><<<c->n_tiles, block, smem4, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, (uint32_t)ncl_max, c->force, md_gate(c));
-        } else {
-            static const int minb = getenv("B200MD_LJ4_MINB") ? atoi(getenv("B200MD_LJ4_MINB")) : 3;
-            if (minb == 4) {
-                MD_TRY(set_smem(c, (k_tile_lj4<4, 4>), smem4));
-                k_tile_lj4<4, 4><<<c->n_tiles, block, smem4, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, (uint32_t)ncl_max, c->force, md_gate(c));
-            } else if (minb == 2) {
-                MD_TRY(set_smem(c, (k_tile_lj4<4, 2>), smem4));
-                k_tile_lj4<4, 2><<<c->n_tiles, block, smem4, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, (uint32_t)ncl_max, c->force, md_gate(c));
-            } else {
-                MD_TRY(set_smem(c, (k_tile_lj4<4, 3>), smem4));
-                k_tile_lj4<4, 3><<<c->n_tiles, block, smem4, c->stream>>>(tp, c->g, c->pos, c->rel, c->nl_cnt, c->nl16, q, c->tile_max_staged, (uint32_t)ncl_max, c->force, md_gate(c));
-            }
-        }
-        MD_LAUNCH_CHECK(c);
-        return MD_OK;
-    }
-    if (!mixed && lj3_mode && !c->nl_cluster) {
+    if (!mixed && lj3_mode) {
         const size_t ns = c->tile_max_staged + N_DUMMY;
         const size_t smemd = 16 * ns + 8 * ((ns + 1) & ~(size_t)1) + tile_header_bytes(c->tile_B) +
                              ((c->tile_max_staged + 16) & ~(size_t)15) + ((2 * (size_t)c->tile_max_home + 15) & ~(size_t)15);
@@ -2698,10 +2211,10 @@ int launch_tile_decode(md_ctx *c, bool fill, uint32_t *cnt32)
     const double rl2 = c->r_list * c->r_list;
     if (fill)
         k_tile_decode<true><<<c->n_tiles, 256, smem, c->stream>>>(make_tp(c), c->g, c->pos_ref, c->nl_cnt, c->nl16, rl2,
-                                                                 c->nl_cluster, nullptr, c->nl_off, c->nl_idx);
+                                                                 nullptr, c->nl_off, c->nl_idx);
     else
         k_tile_decode<false><<<c->n_tiles, 256, smem, c->stream>>>(make_tp(c), c->g, c->pos_ref, c->nl_cnt, c->nl16, rl2,
-                                                                  c->nl_cluster, cnt32, nullptr, nullptr);
+                                                                  cnt32, nullptr, nullptr);
     MD_LAUNCH_CHECK(c);
     return MD_OK;
 }

@@ -1,6 +1,5 @@
 """-m gpu edge cases of the hot path: one and two particles, boxes that are almost empty (most cells and whole tiles hold
-no particle), a box at the smallest legal size with overlapping particles; every kernel variant (fp64, mixed, cluster
-rows, DPD) against the O(N^2) oracle.  Neighbour lists bit-exact, forces within the bars of test_gpu_parity.py."""
+no particle), a box at the smallest legal size with overlapping particles; every kernel variant (fp64, mixed, DPD) against the O(N^2) oracle.  Neighbour lists bit-exact, forces within the bars of test_gpu_parity.py."""
 import numpy as np
 import pytest
 
@@ -26,9 +25,8 @@ def test_lj_sparse_and_tiny_systems(prec, N, L):
     ref = oracle.neighbor_pairs(wpos, box, 2.9)
     Fr, _ = oracle.forces_lj(wpos, box, 2.5)
     tol = 1e-10 if prec == B.MD_FP64 else 1e-4
-    for cluster in ((0, 1) if prec == B.MD_MIXED else (0,)):
+    for _ in (0,):
         md = B.MD(box, N, 2.5, 0.4, precision=prec)
-        md.set_option(B.MD_OPT_CLUSTER, cluster)
         md.set_state(pos, vel)
         md.build_nlist()
         assert np.array_equal(sort_pairs(md.get_nlist()), ref)
@@ -59,8 +57,8 @@ def test_dpd_sparse_and_tiny_systems(N, L):
     assert force_rel_err(F, Fr) <= 1e-10 or np.abs(F - Fr).max() <= 1e-13
 
 
-@pytest.mark.parametrize("prec,cluster", [(B.MD_FP64, 0), (B.MD_MIXED, 0), (B.MD_MIXED, 1)])
-def test_inhomogeneous_slab_grows_the_row_stride(prec, cluster):
+@pytest.mark.parametrize("prec", [B.MD_FP64, B.MD_MIXED])
+def test_inhomogeneous_slab_grows_the_row_stride(prec):
     """All particles in a slab a quarter of the box wide: local density 4x the mean, so the rows are ~4x longer than the
     density-based stride estimate -> the build reports the overflow, the stride grows and the list is built again."""
     rng = np.random.default_rng(1)
@@ -72,7 +70,6 @@ def test_inhomogeneous_slab_grows_the_row_stride(prec, cluster):
     ref = oracle.neighbor_pairs(wpos, box, 2.9)
     assert 2 * len(ref) / N > 2.5 * (N / box.prod()) * 4.18879 * 2.9 ** 3        # rows far beyond the mean-density estimate
     md = B.MD(box, N, 2.5, 0.4, precision=prec)
-    md.set_option(B.MD_OPT_CLUSTER, cluster)
     md.set_state(pos, np.zeros((N, 3)))
     md.build_nlist()
     assert np.array_equal(sort_pairs(md.get_nlist()), ref)

@@ -539,36 +539,6 @@ def test_tile_3x3x3_grid_every_image():
             assert force_rel_err(F, oracle.forces_lj(pos, box, 2.5)[0]) < (1e-10 if prec == B.MD_FP64 else 1e-4)
 
 
-@pytest.mark.parametrize("brick", [1, 2])
-def test_cluster_rows_lists_forces_and_steps(brick):
-    """MD_OPT_CLUSTER: one row per cluster of 4 cell members (k_tile_build_c / k_tile_lj4).  The exported list is
-    still the exact per-particle list (bit for bit), forces stay within the mixed-precision bar, energies and DPD go
-    through the decoded list, and a short trajectory follows the oracle."""
-    wl = inputs.lj_fcc(9, rc=3.0, r_buff=0.4, kT=1.2, jitter=0.08, pos_seed=5, vel_seed=6)     # N=2916
-    ref_pairs = oracle.neighbor_pairs(wl.pos, wl.box, wl.r_list)
-    Fr, Er = oracle.forces_lj(wl.pos, wl.box, wl.rc)
-    md = B.from_workload(wl, precision=B.MD_MIXED)
-    md.set_option(B.MD_OPT_TILE_BRICK, brick)
-    md.set_option(B.MD_OPT_CLUSTER, 1)
-    md.set_state(wl.pos, wl.vel)
-    md.build_nlist()
-    assert np.array_equal(sort_pairs(md.get_nlist()), ref_pairs)
-    md.forces_lj()
-    F, E = md.get_forces()                      # energies on demand: decoded-list kernel
-    assert force_rel_err(F, Fr) < 1e-4
-    assert np.abs(E - Er).max() < 1e-3 * np.abs(Er).max()
-    st = md.stats()
-    assert abs(st["mean_neighbors"] - 2.0 * len(ref_pairs) / wl.N) < 1e-9
-    # trajectory: 20 steps (with rebuilds) against the fp64 oracle; mixed forces -> loose bound
-    md.step(B.step_desc("lj", wl.dt, wl.params), 20)
-    sim = oracle.Sim(wl.pos, wl.vel, wl.box, wl.rc, wl.r_buff, {"lj": wl.params}).run(20, wl.dt)
-    pos, _, _ = md.get_state()
-    d = pos - sim.pos
-    d -= wl.box * np.rint(d / wl.box)
-    assert np.abs(d).max() < 1e-5
-    assert md.stats()["dangerous_builds"] == 0
-
-
 def test_mixed_accumulation_blocks_agree():
     wl = inputs.lj_fcc(7, rc=3.0, r_buff=0.4, kT=1.2, jitter=0.05, pos_seed=2, vel_seed=3)
     Fr, _ = oracle.forces_lj(wl.pos, wl.box, 3.0)
@@ -636,19 +606,14 @@ def _step_forces(md, desc, n=1):
     return F, pos, vel
 
 
-@pytest.mark.parametrize("cluster", [0, 1])
-def test_step_kernels_forces_against_oracle(cluster):
-    """The kernels bench.py times (md_step: k_tile_lj3 with its near section and guard band, k_tile_lj4 with cluster
-    rows, k_tile_lj3d) compared DIRECTLY with the oracle at the positions md_step left: no energy
+def test_step_kernels_forces_against_oracle():
+    """The kernels bench.py times (md_step: k_tile_lj3 with its near section and guard band, k_tile_lj3d) compared DIRECTLY with the oracle at the positions md_step left: no energy
     buffer is passed, so md_get_forces returns what the step's own kernel wrote."""
     wl = inputs.lj_fcc(9, rc=3.0, r_buff=0.4, kT=1.2, jitter=0.05, pos_seed=2, vel_seed=3)       # config-2 recipe, N=2916
     desc = B.step_desc("lj", wl.dt, wl.params)
     for prec, bar in ((B.MD_MIXED, 1e-4), (B.MD_FP64, 1e-10)):
-        if cluster and prec != B.MD_MIXED:
-            continue
         for w in (1, 2, 4, 8):
             md = B.from_workload(wl, precision=prec)
-            md.set_option(B.MD_OPT_CLUSTER, cluster)
             md.set_state(wl.pos, wl.vel)
             md.set_launch(B.MD_K_LJ, 256, w)
             F, pos, _ = _step_forces(md, desc, 25)          # 25 steps: at least one displacement-triggered rebuild
