@@ -395,7 +395,8 @@ def run_ours(args):
             "data": "synthetic",
             "config": {"workload": w.name, "N": w.N, "precision": w.precision, "rc": w.rc, "r_buff": w.r_buff,
                        "dt": w.dt, "parallelism": "replicas only" if world > 1 else "single GPU",
-                       "l2": "inputs larger than L2 (neighbour list %.0f MB + state)" % (4e-6 * st1["nlist_entries"]),
+                       "l2": "inputs larger than L2 (neighbour list %.0f MB of 16-bit entries + %.0f MB of state per step)"
+                             % (2e-6 * st1["nlist_entries"], 216e-6 * w.N),
                        "tps": world * args.steps / (ms_max * 1e-3) / world, "rebuild_period_k": k,
                        "mean_neighbors": nbar, "rebuilds": rebuilds, "dangerous_builds": st1["dangerous_builds"],
                        "order": args.order, "sched": args.sched,
@@ -417,6 +418,11 @@ def run_ours(args):
             "roofline": {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak,
                          "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": traffic, "traffic_note": traffic_note,
+                         # achieved/frac use the ALGORITHMIC bytes of SURVEY 8(d) (4-byte indices: 4 n + 56, DPD 4 n + 84 per
+                         # particle); the list is stored as 16-bit entries, so the measured DRAM traffic is lower:
+                         "bytes_model": "SURVEY 8(d) staged minimum of the pair-force kernel, 4-byte indices",
+                         "traffic_gbs": (traffic / (f_ms * 1e-3) / 1e9) if (traffic and f_ms > 0) else None,
+                         "traffic_frac": (traffic / (f_ms * 1e-3) / 1e9 / peak) if (traffic and f_ms > 0) else None,
                          "bytes_per_particle": b_force, "launch_ms": f_ms},
             # second roofline: the same kernel's ALGORITHMIC instruction rate against the measured issue
             # rate of the pipe(s) it runs on (md_debug_peak, giga lane-instructions per second, an FMA counts once)

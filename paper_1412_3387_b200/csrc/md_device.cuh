@@ -63,7 +63,17 @@ __device__ __forceinline__ float md_grid_coord(double v, double q0, double q0i, 
     return (float)vq;
 }
 
-// fp32 record of a position relative to the centre of cell `lin` (linear id), minimum image applied: what the fp32
+// Centre of cell c along axis a, SNAPPED to the grid q0 (explicitly rounded operations: the binning, half 1 and the tile
+// kernels must all get the same value).  The fp32 records are relative to these snapped centres, so the offset between
+// two cells is an exact multiple of q0 -- the same in every tile: x_i - x_j is the same real number in the tile of i and
+// in the tile of j, pair forces are exactly antisymmetric and the total momentum is conserved to fp64 rounding.
+__device__ __forceinline__ double md_cell_centre_q(uint32_t c, int a, const Geom &g)
+{
+    const double cc = __dadd_rn(g.lo[a], __dmul_rn(__dadd_rn((double)c, 0.5), g.cw[a]));
+    return __dmul_rn(rint(__dmul_rn(cc, g.q0i)), g.q0);
+}
+
+// fp32 record of a position relative to the (snapped) centre of cell `lin` (linear id), minimum image applied: what the fp32
 // tile kernels stage.  x, y, z are rounded to the grid q0 (a multiple of q0 below 2^24 q0 is an exact float, and so is
 // its sum with a cell offset on the same grid: the tile kernels stage WITHOUT a rounding); what the grid drops is kept in
 // .w as three 10-bit residuals in units of qr = q0 / 512 (clamped to +-255), so that the mixed-precision force kernel can rebuild
@@ -73,9 +83,9 @@ __device__ __forceinline__ float4 md_rel_record(double x, double y, double z, ui
     const uint32_t nxy = g.n[0] * g.n[1];
     const uint32_t cz = lin / nxy, rem = lin - cz * nxy;
     const uint32_t cy = rem / g.n[0], cx = rem - cy * g.n[0];
-    const double rx = md_min_image(x - (g.lo[0] + ((double)cx + 0.5) * g.cw[0]), g.L[0], g.h[0]);
-    const double ry = md_min_image(y - (g.lo[1] + ((double)cy + 0.5) * g.cw[1]), g.L[1], g.h[1]);
-    const double rz = md_min_image(z - (g.lo[2] + ((double)cz + 0.5) * g.cw[2]), g.L[2], g.h[2]);
+    const double rx = md_min_image(x - md_cell_centre_q(cx, 0, g), g.L[0], g.h[0]);
+    const double ry = md_min_image(y - md_cell_centre_q(cy, 1, g), g.L[1], g.h[1]);
+    const double rz = md_min_image(z - md_cell_centre_q(cz, 2, g), g.L[2], g.h[2]);
     uint32_t fx, fy, fz;
     const float vx = md_grid_coord(rx, g.q0, g.q0i, g.qri, fx);
     const float vy = md_grid_coord(ry, g.q0, g.q0i, g.qri, fy);

@@ -107,15 +107,33 @@ __device__ __forceinline__ TileSmem tile_carve(char *smem, uint32_t B)
     return t;
 }
 
-// offset of a staged cell (centre of its image relative to the brick centre, cg[3..5]) on the grid q0 of the cell-relative
-// records, with what the grid drops as residual fields in .w (see md_rel_record): record + offset is an exact fp32 sum
-__device__ __forceinline__ float4 tile_grid_offset(const double *cg, const Geom &g)
+// Offset of a staged cell for the fp32 records (md_rel_record): snapped centre of the cell (wrapped index cw_) plus its
+// periodic image shift minus the snapped brick reference -- every term a multiple of the grid q0, so the offset is exact
+// in fp32, record + offset is an exact fp32 sum, and the difference of two cells' offsets is the same in every tile.  The
+// only thing the grid drops is L - round(L) of an image shift: it goes into the residual fields of .w (value + 255).
+__device__ __forceinline__ float4 tile_grid_offset(const Geom &g, const uint32_t cw_[3], const int shift[3], const double ref[3])
 {
-    uint32_t fx, fy, fz;
-    const float ox = md_grid_coord(cg[3], g.q0, g.q0i, g.qri, fx);
-    const float oy = md_grid_coord(cg[4], g.q0, g.q0i, g.qri, fy);
-    const float oz = md_grid_coord(cg[5], g.q0, g.q0i, g.qri, fz);
-    return make_float4(ox, oy, oz, __uint_as_float(fx | (fy << 10) | (fz << 20)));
+    float o[3];
+    uint32_t f[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double Lq = __dmul_rn(rint(__dmul_rn(g.L[a], g.q0i)), g.q0);
+        const double off = (md_cell_centre_q(cw_[a], a, g) - ref[a]) + (double)shift[a] * Lq;  // multiples of q0: exact
+        o[a] = (float)off;
+        f[a] = (uint32_t)(max(-255, min(255, md_round_to_int((double)shift[a] * (g.L[a] - Lq) * g.qri))) + 255);
+    }
+    return make_float4(o[0], o[1], o[2], __uint_as_float(f[0] | (f[1] << 10) | (f[2] << 20)));
+}
+
+// snapped reference point of a brick (near its centre): staged fp32 coordinates are relative to it
+__device__ __forceinline__ void tile_ref_q(const Geom &g, const TileCtx &tc, double ref[3])
+{
+    const uint32_t o[3] = {tc.x0, tc.y0, tc.z0}, e[3] = {tc.ex, tc.ey, tc.ez};
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double cc = __dadd_rn(g.lo[a], __dmul_rn(__dadd_rn((double)o[a], 0.5 * (double)e[a]), g.cw[a]));
+        ref[a] = __dmul_rn(rint(__dmul_rn(cc, g.q0i)), g.q0);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -142,7 +160,15 @@ __device__ __forceinline__ void tile_setup(const TileParams &tp, const Geom &g, 
             cg[3] = ((double)ix - 0.5 - 0.5 * (double)tc.ex) * tp.cw[0];
             cg[4] = ((double)iy - 0.5 - 0.5 * (double)tc.ey) * tp.cw[1];
             cg[5] = ((double)iz - 0.5 - 0.5 * (double)tc.ez) * tp.cw[2];
-            h.coff[sc] = tile_grid_offset(cg, g);
+            {
+                const uint32_t cwi[3] = {cx, cy, cz};
+                // image shift of the staged cell: its unwrapped index (origin + i - 1) against the wrapped one
+                const int sh3[3] = {((int)(tc.x0 + ix) - 1 - (int)cx) / (int)g.n[0], ((int)(tc.y0 + iy) - 1 - (int)cy) / (int)g.n[1],
+                                    ((int)(tc.z0 + iz) - 1 - (int)cz) / (int)g.n[2]};
+                double ref[3];
+                tile_ref_q(g, tc, ref);
+                h.coff[sc] = tile_grid_offset(g, cwi, sh3, ref);
+            }
         }
         __syncthreads();
         return;
@@ -177,7 +203,15 @@ __device__ __forceinline__ void tile_setup(const TileParams &tp, const Geom &g, 
         cg[3] = ((double)ix - 0.5 - 0.5 * (double)tc.ex) * tp.cw[0];
         cg[4] = ((double)iy - 0.5 - 0.5 * (double)tc.ey) * tp.cw[1];
         cg[5] = ((double)iz - 0.5 - 0.5 * (double)tc.ez) * tp.cw[2];
-        h.coff[sc] = tile_grid_offset(cg, g);
+        {
+            const uint32_t cwi[3] = {cx, cy, cz};
+            // image shift of the staged cell: its unwrapped index (origin + i - 1) against the wrapped one
+            const int sh3[3] = {((int)(tc.x0 + ix) - 1 - (int)cx) / (int)g.n[0], ((int)(tc.y0 + iy) - 1 - (int)cy) / (int)g.n[1],
+                                ((int)(tc.z0 + iz) - 1 - (int)cz) / (int)g.n[2]};
+            double ref[3];
+            tile_ref_q(g, tc, ref);
+            h.coff[sc] = tile_grid_offset(g, cwi, sh3, ref);
+        }
     }
     // home cells (consecutive ranks): their staged-cell index and first tile-local particle
     for (uint32_t hc = threadIdx.x; hc <= tc.n_hc; hc += blockDim.x) {
