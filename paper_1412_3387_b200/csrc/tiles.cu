@@ -107,36 +107,36 @@ __device__ __forceinline__ TileSmem tile_carve(char *smem, uint32_t B)
     return t;
 }
 
-// Offset of a staged cell for the fp32 records (md_rel_record): snapped centre of the cell (wrapped index cw_) plus its
-// periodic image shift minus the snapped brick reference -- every term a multiple of the grid q0, so the offset is exact
-// in fp32, record + offset is an exact fp32 sum, and the difference of two cells' offsets is the same in every tile.  The
-// only thing the grid drops is L - round(L) of an image shift: it goes into the residual fields of .w (value + 255).
-__device__ __forceinline__ float4 tile_grid_offset(const Geom &g, const uint32_t cw_[3], const int shift[3], const double ref[3])
+// Offsets of the staged cells for the fp32 records (md_rel_record), per axis: snapped centre of the cell with (wrapped)
+// index along that axis, plus its periodic image shift, minus the snapped brick reference -- every term a multiple of the
+// grid q0, so the offset is exact in fp32, record + offset is an exact fp32 sum, and the difference of two cells' offsets
+// is the same in every tile.  The only thing the grid drops is L - round(L) of an image shift: it goes into the residual
+// field of that axis (value + 255).  24 threads fill axo[8 a + i], axf[8 a + i] (a staged block is at most 6 cells wide);
+// a staged cell (ix, iy, iz) then takes (axo[ix], axo[8 + iy], axo[16 + iz]) and the three fields.
+__device__ __forceinline__ void tile_axis_offsets(const Geom &g, const TileCtx &tc, float *axo, uint32_t *axf)
 {
-    float o[3];
-    uint32_t f[3];
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        const double Lq = __dmul_rn(rint(__dmul_rn(g.L[a], g.q0i)), g.q0);
-        const double off = (md_cell_centre_q(cw_[a], a, g) - ref[a]) + (double)shift[a] * Lq;  // multiples of q0: exact
-        o[a] = (float)off;
-        f[a] = (uint32_t)(max(-255, min(255, md_round_to_int((double)shift[a] * (g.L[a] - Lq) * g.qri))) + 255);
+    if (threadIdx.x < 24u) {
+        const int a = (int)(threadIdx.x >> 3);
+        const uint32_t i = threadIdx.x & 7u;
+        const uint32_t o = a == 0 ? tc.x0 : (a == 1 ? tc.y0 : tc.z0), e = a == 0 ? tc.ex : (a == 1 ? tc.ey : tc.ez);
+        if (i < e + 2u) {
+            const uint32_t n = g.n[a], u1 = o + i;  // unwrapped index + 1
+            const uint32_t cwrap = (u1 + n - 1u) % n;
+            const int shift = u1 == 0u ? -1 : (u1 > n ? 1 : 0);
+            // snapped reference point of the brick (near its centre): staged coordinates are relative to it
+            const double rc_ = __dadd_rn(g.lo[a], __dmul_rn(__dadd_rn((double)o, 0.5 * (double)e), g.cw[a]));
+            const double ref = __dmul_rn(rint(__dmul_rn(rc_, g.q0i)), g.q0);
+            const double Lq = __dmul_rn(rint(__dmul_rn(g.L[a], g.q0i)), g.q0);
+            const double off = (md_cell_centre_q(cwrap, a, g) - ref) + (double)shift * Lq;  // multiples of q0: exact
+            axo[8 * a + i] = (float)off;
+            axf[8 * a + i] = (uint32_t)(max(-255, min(255, md_round_to_int((double)shift * (g.L[a] - Lq) * g.qri))) + 255);
+        }
     }
-    return make_float4(o[0], o[1], o[2], __uint_as_float(f[0] | (f[1] << 10) | (f[2] << 20)));
+    __syncthreads();
 }
 
-// snapped reference point of a brick (near its centre): staged fp32 coordinates are relative to it
-__device__ __forceinline__ void tile_ref_q(const Geom &g, const TileCtx &tc, double ref[3])
-{
-    const uint32_t o[3] = {tc.x0, tc.y0, tc.z0}, e[3] = {tc.ex, tc.ey, tc.ez};
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        const double cc = __dadd_rn(g.lo[a], __dmul_rn(__dadd_rn((double)o[a], 0.5 * (double)e[a]), g.cw[a]));
-        ref[a] = __dmul_rn(rint(__dmul_rn(cc, g.q0i)), g.q0);
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------------------
+// COFF: also the fp32 cell offsets (h.coff) that the kernels staging from the fp32 records add; the fp64 kernels skip them
+template <bool COFF = true>
 __device__ __forceinline__ void tile_setup(const TileParams &tp, const Geom &g, uint32_t t, const TileSmem &h, TileCtx &tc)
 {
     if (tp.desc) {
@@ -148,26 +148,25 @@ __device__ __forceinline__ void tile_setup(const TileParams &tp, const Geom &g, 
         uint32_t *tcw = (uint32_t *)&tc;
 #pragma unroll
         for (int i = 0; i < (int)(sizeof(TileCtx) / 4); ++i) tcw[i] = __ldg(d + i);
+        __shared__ float s_axo[24];
+        __shared__ uint32_t s_axf[24];
+        if (COFF) tile_axis_offsets(g, tc, s_axo, s_axf);
         for (uint32_t sc = threadIdx.x; sc < tc.n_sc; sc += blockDim.x) {
             const uint32_t ix = sc % tc.sx, iy = (sc / tc.sx) % tc.sy, iz = sc / (tc.sx * tc.sy);
-            const uint32_t cx = (tc.x0 + ix + g.n[0] - 1) % g.n[0];
-            const uint32_t cy = (tc.y0 + iy + g.n[1] - 1) % g.n[1];
-            const uint32_t cz = (tc.z0 + iz + g.n[2] - 1) % g.n[2];
-            double *cg = h.cgeo + 6 * sc;
-            cg[0] = g.lo[0] + ((double)cx + 0.5) * tp.cw[0];
-            cg[1] = g.lo[1] + ((double)cy + 0.5) * tp.cw[1];
-            cg[2] = g.lo[2] + ((double)cz + 0.5) * tp.cw[2];
-            cg[3] = ((double)ix - 0.5 - 0.5 * (double)tc.ex) * tp.cw[0];
-            cg[4] = ((double)iy - 0.5 - 0.5 * (double)tc.ey) * tp.cw[1];
-            cg[5] = ((double)iz - 0.5 - 0.5 * (double)tc.ez) * tp.cw[2];
-            {
-                const uint32_t cwi[3] = {cx, cy, cz};
-                // image shift of the staged cell: its unwrapped index (origin + i - 1) against the wrapped one
-                const int sh3[3] = {((int)(tc.x0 + ix) - 1 - (int)cx) / (int)g.n[0], ((int)(tc.y0 + iy) - 1 - (int)cy) / (int)g.n[1],
-                                    ((int)(tc.z0 + iz) - 1 - (int)cz) / (int)g.n[2]};
-                double ref[3];
-                tile_ref_q(g, tc, ref);
-                h.coff[sc] = tile_grid_offset(g, cwi, sh3, ref);
+            if (COFF) {  // kernels that stage the fp32 records
+                h.coff[sc] = make_float4(s_axo[ix], s_axo[8 + iy], s_axo[16 + iz],
+                                         __uint_as_float(s_axf[ix] | (s_axf[8 + iy] << 10) | (s_axf[16 + iz] << 20)));
+            } else {     // fp64 kernels: centre of the cell inside the box, centre of its image relative to the brick centre
+                const uint32_t cx = (tc.x0 + ix + g.n[0] - 1) % g.n[0];
+                const uint32_t cy = (tc.y0 + iy + g.n[1] - 1) % g.n[1];
+                const uint32_t cz = (tc.z0 + iz + g.n[2] - 1) % g.n[2];
+                double *cg = h.cgeo + 6 * sc;
+                cg[0] = g.lo[0] + ((double)cx + 0.5) * tp.cw[0];
+                cg[1] = g.lo[1] + ((double)cy + 0.5) * tp.cw[1];
+                cg[2] = g.lo[2] + ((double)cz + 0.5) * tp.cw[2];
+                cg[3] = ((double)ix - 0.5 - 0.5 * (double)tc.ex) * tp.cw[0];
+                cg[4] = ((double)iy - 0.5 - 0.5 * (double)tc.ey) * tp.cw[1];
+                cg[5] = ((double)iz - 0.5 - 0.5 * (double)tc.ez) * tp.cw[2];
             }
         }
         __syncthreads();
@@ -187,6 +186,9 @@ __device__ __forceinline__ void tile_setup(const TileParams &tp, const Geom &g, 
     tc.n_hc = tp.tile_cell_begin[t + 1] - tc.cb;
     tc.g0 = tp.cell_start[tc.cb];
     tc.n_home = tp.cell_start[tc.cb + tc.n_hc] - tc.g0;
+    __shared__ float s_axo2[24];
+    __shared__ uint32_t s_axf2[24];
+    if (COFF) tile_axis_offsets(g, tc, s_axo2, s_axf2);
     for (uint32_t sc = threadIdx.x; sc < tc.n_sc; sc += blockDim.x) {
         const uint32_t ix = sc % tc.sx, iy = (sc / tc.sx) % tc.sy, iz = sc / (tc.sx * tc.sy);
         const uint32_t cx = (tc.x0 + ix + g.n[0] - 1) % g.n[0];
@@ -203,15 +205,9 @@ __device__ __forceinline__ void tile_setup(const TileParams &tp, const Geom &g, 
         cg[3] = ((double)ix - 0.5 - 0.5 * (double)tc.ex) * tp.cw[0];
         cg[4] = ((double)iy - 0.5 - 0.5 * (double)tc.ey) * tp.cw[1];
         cg[5] = ((double)iz - 0.5 - 0.5 * (double)tc.ez) * tp.cw[2];
-        {
-            const uint32_t cwi[3] = {cx, cy, cz};
-            // image shift of the staged cell: its unwrapped index (origin + i - 1) against the wrapped one
-            const int sh3[3] = {((int)(tc.x0 + ix) - 1 - (int)cx) / (int)g.n[0], ((int)(tc.y0 + iy) - 1 - (int)cy) / (int)g.n[1],
-                                ((int)(tc.z0 + iz) - 1 - (int)cz) / (int)g.n[2]};
-            double ref[3];
-            tile_ref_q(g, tc, ref);
-            h.coff[sc] = tile_grid_offset(g, cwi, sh3, ref);
-        }
+        if (COFF)
+            h.coff[sc] = make_float4(s_axo2[ix], s_axo2[8 + iy], s_axo2[16 + iz],
+                                     __uint_as_float(s_axf2[ix] | (s_axf2[8 + iy] << 10) | (s_axf2[16 + iz] << 20)));
     }
     // home cells (consecutive ranks): their staged-cell index and first tile-local particle
     for (uint32_t hc = threadIdx.x; hc <= tc.n_hc; hc += blockDim.x) {
@@ -505,7 +501,7 @@ __global__ void k_tile_header(TileParams tp, Geom g, uint32_t *desc, unsigned in
     extern __shared__ __align__(16) char smem_raw[];
     const TileSmem h = tile_carve(smem_raw, tp.B);
     TileCtx tc;
-    tile_setup(tp, g, blockIdx.x, h, tc);  // tp.desc == nullptr here
+    tile_setup<false>(tp, g, blockIdx.x, h, tc);  // tp.desc == nullptr here
     uint32_t *d = desc + (size_t)blockIdx.x * tp.desc_words;
     const uint32_t words = tile_desc_table_words(tp.B);
     for (uint32_t i = threadIdx.x; i < words; i += blockDim.x) d[TILE_DESC_CTX + i] = h.gstart[i];
@@ -1070,7 +1066,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj(TileParams tp, Geom 
     uint8_t *scell = (uint8_t *)(h.rest + sizeof(R4) * (max_staged + N_DUMMY));
 
     TileCtx tc;
-    tile_setup(tp, g, blockIdx.x, h, tc);
+    tile_setup<MIXED>(tp, g, blockIdx.x, h, tc);
     if constexpr (MIXED) tile_stage_rel<false>(tc, h, rel, (float4 *)rec, scell, 1.f, pos, g);
     else tile_stage<R4, false>(g, tc, h, pos, nullptr, rec, nullptr, scell);
     __syncthreads();
@@ -1547,7 +1543,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_lj3d(TileParams tp, Geo
     uint16_t *hsidx = (uint16_t *)(scell + ((max_staged + 16) & ~15u));
 
     TileCtx tc;
-    tile_setup(tp, g, blockIdx.x, h, tc);
+    tile_setup<false>(tp, g, blockIdx.x, h, tc);
     {   // stage: coordinates relative to the brick centre, periodic image applied, divided by sigma (see tile_stage)
         const uint32_t lane32 = threadIdx.x & 31u, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
         for (uint32_t hc = wid; hc < tc.n_hc; hc += nw) {
@@ -1656,7 +1652,7 @@ __global__ void __launch_bounds__(TILE_MAX_BLOCK) k_tile_dpd(TileParams tp, Geom
     uint8_t *scell = (uint8_t *)(svel + (max_staged + N_DUMMY));
 
     TileCtx tc;
-    tile_setup(tp, g, blockIdx.x, h, tc);
+    tile_setup<false>(tp, g, blockIdx.x, h, tc);
     tile_stage<double4, true>(g, tc, h, pos, vel, rec, svel, scell);
     if (threadIdx.x < N_DUMMY) svel[tc.n_staged + threadIdx.x] = make_double4(0, 0, 0, 1);
     __syncthreads();
@@ -1749,7 +1745,7 @@ __global__ void __launch_bounds__(MD_DPD2_MAX_BLOCK, 4) k_tile_dpd2(TileParams t
     uint16_t *stash = hsidx + ((max_home + 7u) & ~7u);                      // [stride][n_groups] in-range entries
 
     TileCtx tc;
-    tile_setup(tp, g, blockIdx.x, h, tc);
+    tile_setup<false>(tp, g, blockIdx.x, h, tc);
     {
         const uint32_t lane32 = threadIdx.x & 31u, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
         for (uint32_t hc = wid; hc < tc.n_hc; hc += nw) {
@@ -1870,7 +1866,7 @@ __global__ void k_tile_decode(TileParams tp, Geom g, const double *__restrict__ 
     extern __shared__ __align__(16) char smem_raw[];
     const TileSmem h = tile_carve(smem_raw, tp.B);
     TileCtx tc;
-    tile_setup(tp, g, blockIdx.x, h, tc);
+    tile_setup<false>(tp, g, blockIdx.x, h, tc);
     const unsigned lane = threadIdx.x & 31u, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const unsigned lt = md_lanemask_lt();
     for (uint32_t p = wid; p < tc.n_home; p += nw) {
@@ -1985,7 +1981,7 @@ int tile_measure(md_ctx *c)
         c->tile_desc_len = need;
     }
     const size_t smem = tile_header_bytes(c->tile_B);
-    if (smem > 48 * 1024)
+    if (smem > 40 * 1024)
         MD_CUDA_CHECK(c, cudaFuncSetAttribute(k_tile_header, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k_tile_header<<<c->n_tiles, 128, smem, c->stream>>>(tp, c->g, c->tile_desc, &c->d_flags->max_home, &c->d_flags->max_staged);
     MD_LAUNCH_CHECK(c);
@@ -1996,11 +1992,12 @@ int tile_measure(md_ctx *c)
 template <typename K>
 static int set_smem(md_ctx *c, K kernel, size_t bytes)
 {
-    if (bytes > 48 * 1024) MD_CUDA_CHECK(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    // (opt in well below the 48 KB default limit: it counts static + dynamic shared memory)
+    if (bytes > 40 * 1024) MD_CUDA_CHECK(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     return MD_OK;
 }
 
-static const size_t TILE_SMEM_LIMIT = 227 * 1024 - 64;
+static const size_t TILE_SMEM_LIMIT = 227 * 1024 - 1024;  // dynamic part: the kernels also hold a few hundred bytes of static shared memory
 
 // entries are pre-shifted byte offsets when every staged index (and the dummy) fits in 12 bits
 static uint32_t tile_shift(md_ctx *c) { return c->tile_max_staged + N_DUMMY <= 4096 ? 4u : 0u; }

@@ -28,7 +28,7 @@ def _probe_err(F, Fo, probes, frms):
     return float((np.abs(F[probes] - Fo).max(axis=1) / den).max())
 
 
-@pytest.mark.parametrize("cfg,M,steps", [(2, 256, 40), (3, 256, 6), (4, 256, 8), (5, 128, 12)])
+@pytest.mark.parametrize("cfg,M,steps", [(2, 256, 40), (3, 256, 6), (4, 256, 8), (5, 256, 12)])
 def test_full_size_probe_rows_and_forces(cfg, M, steps):
     w = inputs.config(cfg)
     md = B.from_workload(w)
