@@ -217,6 +217,30 @@ def forces_angles(pos, box, angles, k, theta0, force=None, energy=None, virial=N
     return F, E, W
 
 
+def dihedral_angle(xa, xb, xc, xd, box) -> float:
+    b, bp = _box(box)
+    L = lib()
+    L.orc_dihedral_angle.restype = C.c_double
+    arrs = [np.ascontiguousarray(x, dtype=np.float64) for x in (xa, xb, xc, xd)]
+    return float(L.orc_dihedral_angle(*[x.ctypes.data_as(_dp) for x in arrs], bp))
+
+
+def forces_dihedrals(pos, box, dihedrals, k, s, n, force=None, energy=None, virial=None):
+    """dihedrals: (m, 4) tags (a, b, c, d); U = k/2 (1 + s cos(n phi)).  Accumulates; returns (force, energy, virial)."""
+    pos, pp = _d(pos)
+    b, bp = _box(box)
+    N = pos.shape[0]
+    q = np.ascontiguousarray(dihedrals, dtype=np.uint32).reshape(-1, 4)
+    t = [_u(q[:, i]) for i in range(4)]
+    F = np.zeros((N, 3)) if force is None else force
+    E = np.zeros(N) if energy is None else energy
+    W = np.zeros(6) if virial is None else virial
+    lib().orc_forces_dihedrals(pp, C.c_uint64(N), bp, t[0][1], t[1][1], t[2][1], t[3][1], C.c_uint64(q.shape[0]),
+                               C.c_double(k), C.c_int(int(s)), C.c_int(int(n)), F.ctypes.data_as(_dp),
+                               E.ctypes.data_as(_dp), W.ctypes.data_as(_dp))
+    return F, E, W
+
+
 def pressure(vel, box, W, mass=None):
     """P = (2 K + tr W) / (3 V)  (virial theorem, R32)."""
     m = 1.0 if mass is None else np.asarray(mass)[:, None]

@@ -7,7 +7,7 @@
  *
  * The paper names these features and prints no formula (pair potentials "Lennard-Jones, Gaussian, Morse,
  * Yukawa", bonds "harmonic, FENE", "angle, dihedral"; NPT/NPH integrators need the pressure),
- * so each function states the textbook form it takes (R31-R36).
+ * so each function states the textbook form it takes (R31-R35).
  *
  * Pins (tests/test_oracle_ext.py; no function here is "parity unpinned"):
  *   orc_pair_forces    Yukawa/Gaussian/Morse: closed-form values, F = -dU/dr by central differences, strict cut-off,
@@ -17,6 +17,12 @@
  *   orc_forces_fene    closed form, gradient, divergence at r -> r0, Newton
  *   orc_virial_bonds   two-body closed form, -3 V dU/dV
  *   orc_forces_angles  zero force at theta0, closed form for a right angle, gradient, zero net force and torque
+ *   orc_dihedral_angle hand-made quadruplets (cis 0, trans pi, +-pi/2 with the sign convention), quadruplets built from
+ *                      internal coordinates (the angle put in comes back), invariance under rigid motion and the
+ *                      periodic wrap
+ *   orc_forces_dihedrals  energy k/2 (1 + s cos(n phi)) on built quadruplets for s = +-1, n = 1, 2, 3; F = -dU/dx by
+ *                      central differences on all 12 coordinates; zero net force and torque; virial against
+ *                      sum x_p (x) F_p; quarter-energy bookkeeping
  */
 #include <math.h>
 #include <stdint.h>
@@ -215,5 +221,84 @@ void orc_forces_angles(const double *pos, uint64_t N, const double box[3], const
             energy[a] += u; energy[b] += u; energy[c] += u;
         }
         if (W) { add_virial(W, r1, Fa); add_virial(W, r2, Fc); }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * R35 dihedrals ("dihedral" named only; the brush of PAPER.md:254 needs them): quadruplet (a, b, c, d),
+ * F = minimg(x_a - x_b), G = minimg(x_b - x_c), H = minimg(x_d - x_c), A = F x G, B = H x G,
+ * phi = atan2(((B x A).G)/|G|, A.B) in (-pi, pi] (0 = cis, pi = trans), U = k/2 (1 + s cos(n phi)), s = +-1, n = 1, 2, 3, ...
+ * (the periodic "harmonic" dihedral of HOOMD-blue).  Gradient of phi (Blondel & Karplus 1996):
+ *   dphi/dx_a = -|G|/|A|^2 A,   dphi/dx_d = +|G|/|B|^2 B,
+ *   dphi/dx_b = +|G|/|A|^2 A + (F.G)/(|A|^2 |G|) A - (H.G)/(|B|^2 |G|) B,
+ *   dphi/dx_c = -|G|/|B|^2 B - (F.G)/(|A|^2 |G|) A + (H.G)/(|B|^2 |G|) B,
+ * force on particle p = -dU/dphi dphi/dx_p, dU/dphi = -k/2 s n sin(n phi).  Collinear triplets (|A|^2 or |B|^2 < 1e-24
+ * |G|^4) are skipped.  One quarter of U to each particle.  force / energy ACCUMULATED; W (may be NULL) += sum over a, c, d
+ * of (x_p - x_b) (x) F_p (minimum-image arms).
+ * ---------------------------------------------------------------------------------------------------------------- */
+static void cross3(const double u[3], const double v[3], double w[3])
+{
+    w[0] = u[1] * v[2] - u[2] * v[1];
+    w[1] = u[2] * v[0] - u[0] * v[2];
+    w[2] = u[0] * v[1] - u[1] * v[0];
+}
+
+static double dot3(const double u[3], const double v[3]) { return u[0] * v[0] + u[1] * v[1] + u[2] * v[2]; }
+
+/* the angle itself (also exported for the pins): radians in (-pi, pi] */
+double orc_dihedral_angle(const double *xa, const double *xb, const double *xc, const double *xd, const double box[3])
+{
+    double F[3], G[3], H[3], A[3], B[3], C[3];
+    (void)sep(xa, xb, box, F);
+    (void)sep(xb, xc, box, G);
+    (void)sep(xd, xc, box, H);
+    cross3(F, G, A);
+    cross3(H, G, B);
+    cross3(B, A, C);
+    return atan2(dot3(C, G) / sqrt(dot3(G, G)), dot3(A, B));
+}
+
+void orc_forces_dihedrals(const double *pos, uint64_t N, const double box[3], const uint32_t *tag_a, const uint32_t *tag_b,
+                          const uint32_t *tag_c, const uint32_t *tag_d, uint64_t n_dih, double k, int s, int n,
+                          double *force, double *energy, double *W)
+{
+    (void)N;
+    double F[3], G[3], H[3], A[3], B[3], C[3];
+    for (uint64_t m = 0; m < n_dih; ++m) {
+        uint64_t a = tag_a[m], b = tag_b[m], c = tag_c[m], d = tag_d[m];
+        (void)sep(pos + 3 * a, pos + 3 * b, box, F);
+        double g2 = sep(pos + 3 * b, pos + 3 * c, box, G);
+        (void)sep(pos + 3 * d, pos + 3 * c, box, H);
+        cross3(F, G, A);
+        cross3(H, G, B);
+        double a2 = dot3(A, A), b2 = dot3(B, B);
+        if (!(g2 > 0.0) || a2 < 1e-24 * g2 * g2 || b2 < 1e-24 * g2 * g2) continue;
+        double gl = sqrt(g2);
+        cross3(B, A, C);
+        double phi = atan2(dot3(C, G) / gl, dot3(A, B));
+        double dU = -0.5 * k * (double)s * (double)n * sin((double)n * phi);
+        double fg = dot3(F, G), hg = dot3(H, G);
+        double Fa[3], Fb[3], Fc[3], Fd[3];
+        for (int x = 0; x < 3; ++x) {
+            double ga = -gl / a2 * A[x], gd = gl / b2 * B[x];
+            double gb = gl / a2 * A[x] + fg / (a2 * gl) * A[x] - hg / (b2 * gl) * B[x];
+            double gc = -gl / b2 * B[x] - fg / (a2 * gl) * A[x] + hg / (b2 * gl) * B[x];
+            Fa[x] = -dU * ga; Fb[x] = -dU * gb; Fc[x] = -dU * gc; Fd[x] = -dU * gd;
+        }
+        if (force)
+            for (int x = 0; x < 3; ++x) {
+                force[3 * a + x] += Fa[x]; force[3 * b + x] += Fb[x];
+                force[3 * c + x] += Fc[x]; force[3 * d + x] += Fd[x];
+            }
+        if (energy) {
+            double u = 0.25 * 0.5 * k * (1.0 + (double)s * cos((double)n * phi));
+            energy[a] += u; energy[b] += u; energy[c] += u; energy[d] += u;
+        }
+        if (W) {
+            double rc_[3] = {-G[0], -G[1], -G[2]}, rd[3] = {H[0] - G[0], H[1] - G[1], H[2] - G[2]};
+            add_virial(W, F, Fa);
+            add_virial(W, rc_, Fc);
+            add_virial(W, rd, Fd);
+        }
     }
 }

@@ -194,3 +194,64 @@ def test_angle_gradient_net_force_and_torque():
         assert abs(F[i, a] + (U[1] - U[0]) / (2 * h)) < 1e-6 * max(1.0, abs(F[i, a]))
     h = 1e-6                                             # angles do not change under a uniform rescale: zero virial trace
     assert abs(W[:3].sum()) < 1e-10 * np.abs(F).sum()
+
+
+# ------------------------------------------------------------------------------------------------- dihedrals (R35)
+def _quad(phi, l=(1.1, 0.9, 1.2), th=(1.9, 2.1)):
+    """a-b-c-d with bond lengths l, bond angles th and dihedral angle phi, built by hand next to the periodic boundary."""
+    b = np.array([5.7, -6.3, 6.6])
+    c = b + l[1] * np.array([1.0, 0.0, 0.0])
+    a = b + l[0] * np.array([math.cos(th[0]), math.sin(th[0]), 0.0])        # angle a-b-c = th[0], a in the xy plane (+y)
+    d = c + l[2] * np.array([-math.cos(th[1]), math.sin(th[1]) * math.cos(phi), math.sin(th[1]) * math.sin(phi)])
+    return oracle.wrap(np.stack([a, b, c, d]), BOX)
+
+
+def test_dihedral_angle_special_values_and_invariance():
+    for phi in (0.0, 0.4, math.pi / 2, 2.5, math.pi, -1.3):
+        x = _quad(phi)
+        got = oracle.dihedral_angle(x[0], x[1], x[2], x[3], BOX)
+        assert abs(math.cos(got) - math.cos(phi)) < 1e-13 and abs(math.sin(got) - math.sin(phi)) < 1e-13
+    # the sign convention is fixed by one hand-made case: d out of the abc plane towards +z of a right-handed frame
+    assert abs(oracle.dihedral_angle([1, 1, 0], [0, 0, 0], [1, 0, 0], [1, 0, 1], [20, 20, 20]) - math.pi / 2) < 1e-15
+    assert abs(oracle.dihedral_angle([1, 1, 0], [0, 0, 0], [1, 0, 0], [1, 0, -1], [20, 20, 20]) + math.pi / 2) < 1e-15
+    # reversal of the chain (d, c, b, a) keeps phi; a rigid rotation keeps it too
+    x = _quad(0.9)
+    p0 = oracle.dihedral_angle(x[0], x[1], x[2], x[3], BOX)
+    assert abs(oracle.dihedral_angle(x[3], x[2], x[1], x[0], BOX) - p0) < 1e-13
+    rng = np.random.default_rng(2)
+    Q, _ = np.linalg.qr(rng.standard_normal((3, 3)))
+    if np.linalg.det(Q) < 0:
+        Q[:, 0] *= -1
+    y = (x - x[1]) - BOX * np.rint((x - x[1]) / BOX)
+    y = y @ Q.T
+    assert abs(oracle.dihedral_angle(y[0], y[1], y[2], y[3], [50, 50, 50]) - p0) < 1e-13
+
+
+@pytest.mark.parametrize("s,n", [(1, 1), (-1, 1), (1, 2), (-1, 3)])
+def test_dihedral_energy_gradient_net_force_torque_virial(s, n):
+    k = 6.0
+    for phi in (0.3, 1.1, 2.6, -0.8):
+        x = _quad(phi)
+        F, E, W = oracle.forces_dihedrals(x, BOX, [[0, 1, 2, 3]], k, s, n)
+        p = oracle.dihedral_angle(x[0], x[1], x[2], x[3], BOX)
+        assert abs(E.sum() - 0.5 * k * (1.0 + s * math.cos(n * p))) < 1e-14 and abs(E[0] - E[3]) < 1e-16
+        assert np.abs(F.sum(axis=0)).max() < 1e-13
+        y = (x - x[1]) - BOX * np.rint((x - x[1]) / BOX)
+        assert np.abs(np.cross(y, F).sum(axis=0)).max() < 1e-12                      # no net torque
+        assert abs(W[:3].sum()) < 1e-12                                               # angles do not feel a uniform rescale
+        for i in range(4):
+            for a in range(3):
+                h = 1e-6
+                U = []
+                for sg in (-h, h):
+                    z = x.copy(); z[i, a] += sg
+                    U.append(oracle.forces_dihedrals(z, BOX, [[0, 1, 2, 3]], k, s, n)[1].sum())
+                assert abs(F[i, a] + (U[1] - U[0]) / (2 * h)) < 2e-8 * max(1.0, np.abs(F).max())
+    # extrema of the potential: no force at phi = 0 and pi
+    for phi in (0.0, math.pi):
+        assert np.abs(oracle.forces_dihedrals(_quad(phi), BOX, [[0, 1, 2, 3]], k, s, n)[0]).max() < 1e-12
+    # many terms along chains: Newton's third law over the whole system
+    w = inputs.polymer_melt(5, chain_len=12)
+    dih = np.array([[12 * c + i, 12 * c + i + 1, 12 * c + i + 2, 12 * c + i + 3] for c in range(5) for i in range(9)], dtype=np.uint32)
+    F, E, W = oracle.forces_dihedrals(w.pos, w.box, dih, k, s, n)
+    assert np.abs(F.sum(axis=0)).max() < 1e-11 * max(1.0, np.abs(F).sum())
