@@ -69,6 +69,7 @@ typedef enum {
 #define MD_F_NVT 8u /* md_step integrates with the Nose-Hoover thermostat (md_integrate_nvt) instead of NVE */
 #define MD_F_PAIR 16u   /* a pair potential of SURVEY.md 8(f) row 3 (pair_kind, pair_p) instead of LJ / DPD */
 #define MD_F_ANGLES 32u /* harmonic angles (md_set_angles; angle_k, angle_theta0) */
+#define MD_F_DIHEDRALS 64u /* periodic dihedrals (md_set_dihedrals; dihedral_k, dihedral_sign, dihedral_n) */
 
 /* pair potentials of md_forces_pair / MD_F_PAIR (PAPER.md:63 lists them, R31); parameters p[0..2] */
 enum { MD_PAIR_LJ = 0,       /* U = 4 p0 ((p1/r)^12 - (p1/r)^6)                        p0 = epsilon, p1 = sigma     */
@@ -103,6 +104,8 @@ typedef struct {
     int32_t bond_kind;      /* MD_F_BONDS: MD_BOND_* (0 = harmonic) */
     double pair_p[4];       /* MD_F_PAIR: parameters of the pair potential */
     double angle_k, angle_theta0; /* MD_F_ANGLES: U = k/2 (theta - theta0)^2, theta0 in radians */
+    double dihedral_k;            /* MD_F_DIHEDRALS: U = k/2 (1 + sign cos(n phi)) */
+    int32_t dihedral_sign, dihedral_n; /* sign = +1 or -1, n = 1, 2, 3, ... */
 } md_step_desc;
 
 #define MD_N_KERNELS 8
@@ -241,10 +244,21 @@ int md_forces_fene(md_ctx *ctx, double k, double r0);
 int md_set_angles(md_ctx *ctx, const uint32_t *tag_a, const uint32_t *tag_b, const uint32_t *tag_c, uint64_t n_angles);
 int md_forces_angles(md_ctx *ctx, double k, double theta0);
 
+/* Periodic dihedrals (R35; PAPER.md:63 names "dihedral"): quadruplets of tags (a, b, c, d) around the bond b-c.
+   F = x_a - x_b, G = x_b - x_c, H = x_d - x_c (minimum image), A = F x G, B = H x G,
+   phi = atan2((B x A).G / |G|, A.B) in (-pi, pi] (0 = cis, pi = trans); U = k/2 (1 + sign cos(n phi)), sign = +-1,
+   n >= 1; one quarter of U to each particle's energy; degenerate quadruplets (|A|^2 or |B|^2 < 1e-24 |G|^4: three
+   collinear particles) are skipped.  tag arrays: HOST or DEVICE, n_dihedrals entries each, copied; a tag out of range or
+   repeated within a quadruplet is MD_EINVAL (host arrays only).  Stored per particle like the angles (no atomics).
+   n_dihedrals = 0 clears.  md_forces_dihedrals ACCUMULATES into force/energy; MD_EINVAL for sign not +-1 or n < 1. */
+int md_set_dihedrals(md_ctx *ctx, const uint32_t *tag_a, const uint32_t *tag_b, const uint32_t *tag_c, const uint32_t *tag_d,
+                     uint64_t n_dihedrals);
+int md_forces_dihedrals(md_ctx *ctx, double k, int sign, int n);
+
 /* ---- virial and pressure (PAPER.md:63 NPT / NPH, :208, :214; R32) ----------------------------- */
 
 /* W = sum over the pairs of `what`'s pair term of d (x) F (d = minimum-image separation, F the pair force on the first
-   particle; for MD_F_DPD all three terms with hash counter = the context's current step), plus bonds and angles (arm (x) F
+   particle; for MD_F_DPD all three terms with hash counter = the context's current step), plus bonds, angles and dihedrals (arm (x) F
    per end) if flagged; order xx, yy, zz, xy, xz, yz.  kinetic = sum 1/2 m v^2, volume = box volume,
    pressure = (2 kinetic + W_xx + W_yy + W_zz) / (3 volume).  Evaluated on demand at the current positions with the
    neighbour list rebuilt if stale; device reductions in a fixed order.  out: HOST pointer.  Synchronises. */

@@ -972,6 +972,59 @@ extern "C" int md_forces_angles(md_ctx *c, double k, double theta0)
     return MD_OK;
 }
 
+extern "C" int md_set_dihedrals(md_ctx *c, const uint32_t *ta, const uint32_t *tb, const uint32_t *tc, const uint32_t *td,
+                                uint64_t nd)
+{
+    if (!c) return MD_EINVAL;
+    if (nd > 0 && (!ta || !tb || !tc || !td)) { c->err = "md_set_dihedrals: null tag array"; return MD_EINVAL; }
+    if (nd >= 0x3fffffffull) { c->err = "md_set_dihedrals: too many dihedrals"; return MD_EINVAL; }
+    MD_TRY(alloc_state(c));
+    MD_TRY(md_sync(c));
+    for (uint32_t **q : {&c->dih_off, &c->dih_ent, &c->dih_abcd})
+        if (*q) { md_free(c, *q); *q = nullptr; }
+    c->n_dihedrals = nd;
+    if (nd == 0) return MD_OK;
+    if (!is_device_ptr(ta))
+        for (uint64_t m = 0; m < nd; ++m) {
+            const uint32_t q[4] = {ta[m], tb[m], tc[m], td[m]};
+            bool bad = false;
+            for (int x = 0; x < 4; ++x) {
+                bad |= q[x] >= c->N;
+                for (int y = x + 1; y < 4; ++y) bad |= q[x] == q[y];
+            }
+            if (bad) {
+                c->err = "md_set_dihedrals: tag out of range or repeated in a quadruplet";
+                c->n_dihedrals = 0;
+                return MD_EINVAL;
+            }
+        }
+    MD_TRY(md_alloc(c, (void **)&c->dih_off, (c->N + 1) * sizeof(uint32_t)));
+    MD_TRY(md_alloc(c, (void **)&c->dih_ent, 4 * nd * sizeof(uint32_t)));
+    MD_TRY(md_alloc(c, (void **)&c->dih_abcd, 4 * nd * sizeof(uint32_t)));
+    Stage st(c);
+    const uint64_t bb = nd * sizeof(uint32_t);
+    MD_TRY(st.reserve(stage_need(ta, bb) + stage_need(tb, bb) + stage_need(tc, bb) + stage_need(td, bb)));
+    const void *da, *db, *dc, *dd;
+    MD_TRY(stage_in(c, st, ta, bb, &da));
+    MD_TRY(stage_in(c, st, tb, bb, &db));
+    MD_TRY(stage_in(c, st, tc, bb, &dc));
+    MD_TRY(stage_in(c, st, td, bb, &dd));
+    MD_TRY(launch_dihedrals_build(c, (const uint32_t *)da, (const uint32_t *)db, (const uint32_t *)dc, (const uint32_t *)dd, nd));
+    return md_sync(c);
+}
+
+extern "C" int md_forces_dihedrals(md_ctx *c, double k, int sign, int n)
+{
+    if (!c) return MD_EINVAL;
+    if ((sign != 1 && sign != -1) || n < 1) { c->err = "md_forces_dihedrals: sign must be +1 or -1 and n >= 1"; return MD_EINVAL; }
+    if (!c->have_state) { c->err = "md_forces_dihedrals: md_set_state first"; return MD_ESTATE; }
+    if (c->n_dihedrals == 0) { c->force_valid = true; return MD_OK; }
+    ProfScope ps(c, MD_K_BONDS);
+    MD_TRY(launch_forces_dihedrals(c, k, sign, n));
+    c->force_valid = true;
+    return MD_OK;
+}
+
 extern "C" int md_integrate_nve(md_ctx *c, double dt, int half)
 {
     if (!c) return MD_EINVAL;
@@ -1071,6 +1124,14 @@ static int eval_forces(md_ctx *c, const md_step_desc *w, uint64_t step, bool ene
     if ((w->flags & MD_F_ANGLES) && c->n_angles) {
         ProfScope ps(c, MD_K_BONDS);
         MD_TRY(launch_forces_angles(c, w->angle_k, w->angle_theta0));
+    }
+    if ((w->flags & MD_F_DIHEDRALS) && c->n_dihedrals) {
+        if ((w->dihedral_sign != 1 && w->dihedral_sign != -1) || w->dihedral_n < 1) {
+            c->err = "md_step: dihedral_sign must be +1 or -1 and dihedral_n >= 1";
+            return MD_EINVAL;
+        }
+        ProfScope ps(c, MD_K_BONDS);
+        MD_TRY(launch_forces_dihedrals(c, w->dihedral_k, w->dihedral_sign, w->dihedral_n));
     }
     c->force_valid = true;
     // only the tile LJ kernel skips the per-particle energies

@@ -236,7 +236,150 @@ int launch_forces_angles(md_ctx *c, double k, double theta0)
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// R32 virial W = sum over pairs of d (x) F (+ bonds, + angles: arm (x) F per end), order xx yy zz xy xz yz.  Every
+// R35 periodic dihedrals U = k/2 (1 + s cos(n phi)).  Same storage as the angles: CSR by TAG, entry = 4 * dihedral
+// index + role (0 = a, 1 = b, 2 = c, 3 = d), rows sorted; every particle sums the terms it takes part in.
+// ------------------------------------------------------------------------------------------------------------
+__global__ void k_dih_count(const uint32_t *__restrict__ ta, const uint32_t *__restrict__ tb, const uint32_t *__restrict__ tc,
+                            const uint32_t *__restrict__ td, uint64_t nd, uint32_t *cnt)
+{
+    const uint64_t m = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= nd) return;
+    atomicAdd(&cnt[ta[m]], 1u);
+    atomicAdd(&cnt[tb[m]], 1u);
+    atomicAdd(&cnt[tc[m]], 1u);
+    atomicAdd(&cnt[td[m]], 1u);
+}
+
+__global__ void k_dih_fill(const uint32_t *__restrict__ ta, const uint32_t *__restrict__ tb, const uint32_t *__restrict__ tc,
+                           const uint32_t *__restrict__ td, uint64_t nd, const uint32_t *__restrict__ off, uint32_t *fill,
+                           uint32_t *ent, uint4 *abcd)
+{
+    const uint64_t m = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= nd) return;
+    const uint4 q = make_uint4(ta[m], tb[m], tc[m], td[m]);
+    abcd[m] = q;
+    ent[off[q.x] + atomicAdd(&fill[q.x], 1u)] = 4u * (uint32_t)m;
+    ent[off[q.y] + atomicAdd(&fill[q.y], 1u)] = 4u * (uint32_t)m + 1u;
+    ent[off[q.z] + atomicAdd(&fill[q.z], 1u)] = 4u * (uint32_t)m + 2u;
+    ent[off[q.w] + atomicAdd(&fill[q.w], 1u)] = 4u * (uint32_t)m + 3u;
+}
+
+int launch_dihedrals_build(md_ctx *c, const uint32_t *ta, const uint32_t *tb, const uint32_t *tc, const uint32_t *td, uint64_t nd)
+{
+    cudaStream_t st = c->stream;
+    const uint32_t N = (uint32_t)c->N;
+    uint32_t *cnt = c->perm;  // scratch (N uint32), only valid to borrow outside a binning
+    MD_CUDA_CHECK(c, cudaMemsetAsync(cnt, 0, sizeof(uint32_t) * N, st));
+    k_dih_count<<<md_grid(nd, 256), 256, 0, st>>>(ta, tb, tc, td, nd, cnt);
+    MD_LAUNCH_CHECK(c);
+    MD_TRY(launch_exclusive_scan_u32(c, cnt, N, c->dih_off, nullptr, false, nullptr));
+    MD_CUDA_CHECK(c, cudaMemsetAsync(cnt, 0, sizeof(uint32_t) * N, st));
+    k_dih_fill<<<md_grid(nd, 256), 256, 0, st>>>(ta, tb, tc, td, nd, c->dih_off, cnt, c->dih_ent, (uint4 *)c->dih_abcd);
+    MD_LAUNCH_CHECK(c);
+    k_sort_rows_u32<<<md_grid(N, 256), 256, 0, st>>>(c->dih_off, N, c->dih_ent);
+    MD_LAUNCH_CHECK(c);
+    return MD_OK;
+}
+
+__device__ __forceinline__ void md_cross(const double u[3], const double v[3], double w[3])
+{
+    w[0] = u[1] * v[2] - u[2] * v[1];
+    w[1] = u[2] * v[0] - u[0] * v[2];
+    w[2] = u[0] * v[1] - u[1] * v[0];
+}
+
+__device__ __forceinline__ double md_dot(const double u[3], const double v[3]) { return u[0] * v[0] + u[1] * v[1] + u[2] * v[2]; }
+
+struct DihParams {
+    double k, s;  // U = k/2 (1 + s cos(n phi))
+    int n;
+};
+
+// force on the particle with role `role` of the dihedral (a, b, c, d) and (for the virial) its arm relative to b.
+// F = x_a - x_b, G = x_b - x_c, H = x_d - x_c, A = F x G, B = H x G, phi = atan2((B x A).G / |G|, A.B)
+// (only cos(n phi) and sin(n phi) are needed); gradients of phi after Blondel & Karplus; force = -dU/dphi grad phi, dU/dphi = -k/2 s n sin(n phi).
+__device__ __forceinline__ bool dihedral_term(const double4 *__restrict__ pos, const uint32_t *__restrict__ rtag,
+                                              const uint4 *__restrict__ abcd, uint32_t m, uint32_t role, const Geom &g,
+                                              const DihParams &dp, double Fo[3], double arm[3], double &u)
+{
+    const uint4 q = abcd[m];
+    const double4 xa = pos[rtag[q.x]], xb = pos[rtag[q.y]], xc = pos[rtag[q.z]], xd = pos[rtag[q.w]];
+    const double F[3] = {md_min_image(xa.x - xb.x, g.L[0], g.h[0]), md_min_image(xa.y - xb.y, g.L[1], g.h[1]),
+                         md_min_image(xa.z - xb.z, g.L[2], g.h[2])};
+    const double G[3] = {md_min_image(xb.x - xc.x, g.L[0], g.h[0]), md_min_image(xb.y - xc.y, g.L[1], g.h[1]),
+                         md_min_image(xb.z - xc.z, g.L[2], g.h[2])};
+    const double H[3] = {md_min_image(xd.x - xc.x, g.L[0], g.h[0]), md_min_image(xd.y - xc.y, g.L[1], g.h[1]),
+                         md_min_image(xd.z - xc.z, g.L[2], g.h[2])};
+    double A[3], B[3], C[3];
+    md_cross(F, G, A);
+    md_cross(H, G, B);
+    const double g2 = md_dot(G, G), a2 = md_dot(A, A), b2 = md_dot(B, B);
+    if (!(g2 > 0.0) || a2 < 1e-24 * g2 * g2 || b2 < 1e-24 * g2 * g2) return false;
+    const double gl = sqrt(g2);
+    md_cross(B, A, C);
+    // cos(n phi), sin(n phi) from cos phi = A.B / (|A| |B|), sin phi = (B x A).G / (|G| |A| |B|) by the angle-addition
+    // recurrence (n is a small integer): no atan2 / sincos in the kernel
+    const double iab = rsqrt(a2 * b2);
+    const double c1 = md_dot(A, B) * iab, s1 = md_dot(C, G) / gl * iab;
+    double cs = c1, sn = s1;
+    for (int m = 1; m < dp.n; ++m) {
+        const double t = cs * c1 - sn * s1;
+        sn = sn * c1 + cs * s1;
+        cs = t;
+    }
+    const double dU = -0.5 * dp.k * dp.s * (double)dp.n * sn;
+    u = 0.125 * dp.k * (1.0 + dp.s * cs);
+    const double fg = md_dot(F, G), hg = md_dot(H, G);
+    const double ca = gl / a2, cb = gl / b2, ea = fg / (a2 * gl), eb = hg / (b2 * gl);
+#pragma unroll
+    for (int x = 0; x < 3; ++x) {
+        double gr;  // d phi / d x_role
+        if (role == 0) gr = -ca * A[x];
+        else if (role == 1) gr = ca * A[x] + ea * A[x] - eb * B[x];
+        else if (role == 2) gr = -cb * B[x] - ea * A[x] + eb * B[x];
+        else gr = cb * B[x];
+        Fo[x] = -dU * gr;
+        arm[x] = role == 0 ? F[x] : (role == 2 ? -G[x] : (role == 3 ? H[x] - G[x] : 0.0));
+    }
+    return true;
+}
+
+__global__ void k_forces_dihedrals(const double4 *__restrict__ pos, const uint32_t *__restrict__ tag,
+                                   const uint32_t *__restrict__ rtag, const uint32_t *__restrict__ off,
+                                   const uint32_t *__restrict__ ent, const uint4 *__restrict__ abcd, Geom g, DihParams dp,
+                                   double4 *__restrict__ force, Gate gate)
+{
+    if (md_gate_closed(gate)) return;
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.N) return;
+    const uint32_t t = tag[i];
+    const uint32_t b = off[t], e = off[t + 1];
+    if (b == e) return;
+    double fx = 0.0, fy = 0.0, fz = 0.0, en = 0.0;
+    for (uint32_t q = b; q < e; ++q) {
+        double F[3], arm[3], u;
+        if (dihedral_term(pos, rtag, abcd, ent[q] >> 2, ent[q] & 3u, g, dp, F, arm, u)) {
+            fx += F[0]; fy += F[1]; fz += F[2]; en += u;
+        }
+    }
+    double4 f = force[i];
+    f.x += fx; f.y += fy; f.z += fz; f.w += en;
+    force[i] = f;
+}
+
+int launch_forces_dihedrals(md_ctx *c, double k, int sign, int n)
+{
+    const LaunchCfg &cf = c->cfg[MD_K_BONDS];
+    const DihParams dp = {k, (double)sign, n};
+    k_forces_dihedrals<<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->pos, c->tag, c->rtag, c->dih_off, c->dih_ent,
+                                                                           (const uint4 *)c->dih_abcd, c->g, dp, c->force,
+                                                                           md_gate(c));
+    MD_LAUNCH_CHECK(c);
+    return MD_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// R32 virial W = sum over pairs of d (x) F (+ bonds, + angles and dihedrals: arm (x) F per end), order xx yy zz xy xz yz.  Every
 // particle sums HALF of each of its pair and bond terms (the list is double-sided) and its own arm of each angle; a
 // block sums a contiguous range of slots (shared-memory tree), one block sums the partials: fixed order, bit-reproducible.
 // ------------------------------------------------------------------------------------------------------------
@@ -252,6 +395,8 @@ struct VirialTerms {
     double bond_k, bond_r0;
     int angles;
     double angle_k, angle_theta0;
+    int dihedrals;
+    DihParams dih;
 };
 
 __device__ __forceinline__ void vir_add(double w[6], double s, const double d[3], const double F[3])
@@ -267,7 +412,9 @@ __global__ void __launch_bounds__(VIR_BLOCK) k_virial(const double4 *__restrict_
                                                       const uint32_t *__restrict__ nl_idx,
                                                       const uint32_t *__restrict__ bond_off, const uint32_t *__restrict__ bond_partner,
                                                       const uint32_t *__restrict__ angle_off, const uint32_t *__restrict__ angle_ent,
-                                                      const uint32_t *__restrict__ angle_abc, Geom g, VirialTerms vt,
+                                                      const uint32_t *__restrict__ angle_abc, const uint32_t *__restrict__ dih_off,
+                                                      const uint32_t *__restrict__ dih_ent, const uint4 *__restrict__ dih_abcd,
+                                                      Geom g, VirialTerms vt,
                                                       double *__restrict__ partial /* [gridDim.x][6] */)
 {
     __shared__ double sm[6 * VIR_BLOCK];
@@ -325,6 +472,13 @@ __global__ void __launch_bounds__(VIR_BLOCK) k_virial(const double4 *__restrict_
                     vir_add(w, 1.0, arm, F);
             }
         }
+        if (vt.dihedrals) {
+            for (uint32_t q = dih_off[t]; q < dih_off[t + 1]; ++q) {
+                double F[3], arm[3], u;
+                if (dihedral_term(pos, rtag, dih_abcd, dih_ent[q] >> 2, dih_ent[q] & 3u, g, vt.dih, F, arm, u))
+                    vir_add(w, 1.0, arm, F);
+            }
+        }
     }
 #pragma unroll
     for (int k = 0; k < 6; ++k) sm[k * VIR_BLOCK + threadIdx.x] = w[k];
@@ -361,7 +515,7 @@ __global__ void __launch_bounds__(VIR_BLOCK) k_virial_final(const double *__rest
     if (threadIdx.x < 6) out[threadIdx.x] = sm[threadIdx.x * VIR_BLOCK];
 }
 
-// what: the interaction set (MD_F_LJ | MD_F_PAIR | MD_F_DPD, MD_F_BONDS, MD_F_ANGLES); the pair part reads the exact
+// what: the interaction set (MD_F_LJ | MD_F_PAIR | MD_F_DPD, MD_F_BONDS, MD_F_ANGLES, MD_F_DIHEDRALS); the pair part reads the exact
 // 32-bit list (the caller has decoded a tile list).  out6_host: 6 doubles on the host; synchronises.
 int launch_virial(md_ctx *c, const md_step_desc *w, uint64_t step, double *out6_host)
 {
@@ -395,10 +549,12 @@ int launch_virial(md_ctx *c, const md_step_desc *w, uint64_t step, double *out6_
     vt.angles = ((w->flags & MD_F_ANGLES) && c->n_angles) ? 1 : 0;
     vt.angle_k = w->angle_k;
     vt.angle_theta0 = w->angle_theta0;
+    vt.dihedrals = ((w->flags & MD_F_DIHEDRALS) && c->n_dihedrals) ? 1 : 0;
+    vt.dih = DihParams{w->dihedral_k, (double)w->dihedral_sign, w->dihedral_n};
 #define VIR_LAUNCH(P_)                                                                                                    \
     k_virial<P_><<<nb, VIR_BLOCK, 0, c->stream>>>(c->pos, c->vel, c->tag, c->rtag, c->nl_cnt_exp, c->nl_off, c->nl_idx,  \
                                                   c->bond_off, c->bond_partner, c->angle_off, c->angle_ent, c->angle_abc, \
-                                                  c->g, vt, buf)
+                                                  c->dih_off, c->dih_ent, (const uint4 *)c->dih_abcd, c->g, vt, buf)
     switch (pot) {
     case MD_PAIR_LJ: VIR_LAUNCH(MD_PAIR_LJ); break;
     case MD_PAIR_YUKAWA: VIR_LAUNCH(MD_PAIR_YUKAWA); break;

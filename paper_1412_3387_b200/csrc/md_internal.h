@@ -150,6 +150,9 @@ struct md_ctx {
     // angles: CSR by TAG (entry = 4 * angle index + role), triplets by angle
     uint64_t n_angles = 0;
     uint32_t *angle_off = nullptr, *angle_ent = nullptr, *angle_abc = nullptr;
+    // dihedrals: same layout, quadruplets as uint4
+    uint64_t n_dihedrals = 0;
+    uint32_t *dih_off = nullptr, *dih_ent = nullptr, *dih_abcd = nullptr;
 
     // scratch
     uint64_t *scan_tmp = nullptr;
@@ -239,6 +242,8 @@ int launch_forces_bonds(md_ctx *c, double k, double r0, int kind = 0);  // kind:
 int launch_forces_pair(md_ctx *c, int kind, const double prm[4], int shift);
 int launch_angles_build(md_ctx *c, const uint32_t *ta, const uint32_t *tb, const uint32_t *tc, uint64_t na);
 int launch_forces_angles(md_ctx *c, double k, double theta0);
+int launch_dihedrals_build(md_ctx *c, const uint32_t *ta, const uint32_t *tb, const uint32_t *tc, const uint32_t *td, uint64_t nd);
+int launch_forces_dihedrals(md_ctx *c, double k, int sign, int n);
 int launch_virial(md_ctx *c, const md_step_desc *w, uint64_t step, double *out6_host);
 // fused: preceded by the previous step's half 2.  nvt: Nose-Hoover friction xi read from c->nvt_state (R30)
 int launch_half1(md_ctx *c, double dt, bool fused, bool nvt = false);

@@ -1,5 +1,5 @@
 """-m gpu parity of SURVEY 8(f) rows 1 and 3 against oracle/md_oracle_ext.c: Yukawa / Gaussian / Morse pair forces,
-FENE bonds, harmonic angles (forces and energies within 1e-10, R11 norm), virial tensor and pressure of every term
+FENE bonds, harmonic angles, periodic dihedrals (forces and energies within 1e-10, R11 norm), virial tensor and pressure of every term
 (1e-10 of the tensor's scale), through the single calls and through md_step."""
 import math
 
@@ -19,6 +19,11 @@ PAIRS = [("yukawa", (2.0, 1.5)), ("gaussian", (3.0, 0.8)), ("morse", (1.7, 2.0, 
 def _chain_angles(n_chains, length):
     return np.array([[length * c + i, length * c + i + 1, length * c + i + 2]
                      for c in range(n_chains) for i in range(length - 2)], dtype=np.uint32)
+
+
+def _chain_dihedrals(n_chains, length):
+    return np.array([[length * c + i, length * c + i + 1, length * c + i + 2, length * c + i + 3]
+                     for c in range(n_chains) for i in range(length - 3)], dtype=np.uint32)
 
 
 @pytest.mark.parametrize("order", [B.MD_ORDER_MORTON, B.MD_ORDER_LEX])
@@ -123,3 +128,81 @@ def test_lj_and_dpd_pressure_at_scale_and_after_steps():
     md.step(desc, 3)                                    # the pressure call left the run untouched
     ref = B.from_workload(wl, precision=B.MD_MIXED); ref.step(desc, 10)
     assert np.array_equal(md.get_state()[0], ref.get_state()[0])
+
+
+@pytest.mark.parametrize("sign,n", [(1, 1), (-1, 2), (1, 3)])
+def test_dihedrals_forces_energy_virial_and_step(sign, n):
+    """R35 through the C-ABI: md_forces_dihedrals alone, its virial inside md_pressure, and one md_step of the polymer model
+    with bonds + angles + dihedrals against the plain sequence of oracle calls."""
+    wl = inputs.polymer_melt(40, chain_len=32, start_seed=16, walk_seed=17, vel_seed=18)          # N = 1280
+    dih = _chain_dihedrals(40, 32)
+    ang = _chain_angles(40, 32)
+    k_d, k_a, th0 = 6.0, 8.0, 2.0
+    md = B.from_workload(wl)
+    md.set_dihedrals(dih)
+    md.build_cells()
+    md.forces_dihedrals(k_d, sign, n)
+    F, E = md.get_forces()
+    Fr, Er, Wr = oracle.forces_dihedrals(wl.pos, wl.box, dih, k_d, sign, n)
+    assert np.abs(Fr).max() > 1.0                          # the term is really there
+    assert force_rel_err(F, Fr) < 1e-10 and np.abs(E - Er).max() < 1e-11 * np.abs(Er).max()
+    assert abs(F.sum(axis=0)).max() < 1e-10                # every quadruplet's four forces cancel
+    # the dihedral virial alone, then together with DPD + harmonic bonds + angles
+    d_only = B.step_desc("none", wl.dt, dict(dihedral_k=k_d, dihedral_sign=sign, dihedral_n=n))
+    assert d_only.flags == B.MD_F_DIHEDRALS
+    pr = md.pressure(d_only)
+    assert np.abs(pr["virial"] - Wr).max() < 1e-10 * np.abs(Wr).max()
+    q = wl.params
+    prm = dict(q, angle_k=k_a, angle_theta0=th0, dihedral_k=k_d, dihedral_sign=sign, dihedral_n=n)
+    desc = B.step_desc("polymer", wl.dt, prm)
+    assert desc.flags == B.MD_F_DPD | B.MD_F_BONDS | B.MD_F_ANGLES | B.MD_F_DIHEDRALS
+    md.set_angles(ang)
+    pr = md.pressure(desc)
+    Wd = oracle.virial_dpd(wl.pos, wl.vel, wl.box, wl.rc, q["A"], q["gamma"], q["kT"], wl.dt, 0, q["seed"])
+    Wb = oracle.forces_bonds_kind(wl.pos, wl.box, wl.bonds, "harmonic", q["bond_k"], q["bond_r0"])[2]
+    Wa = oracle.forces_angles(wl.pos, wl.box, ang, k_a, th0)[2]
+    W = Wd + Wb + Wa + Wr
+    assert np.abs(pr["virial"] - W).max() < 1e-10 * np.abs(W).max()
+    # one md_step (batch scheduler, the default) and the same step with the synchronous scheduler
+    outs = []
+    for sched in (B.MD_SCHED_BATCH, B.MD_SCHED_SYNC):
+        ms = B.from_workload(wl, sched=sched)
+        ms.set_angles(ang)
+        ms.set_dihedrals(dih)
+        ms.step(desc, 1)
+        outs.append(ms.get_state())
+    pos, vel, _ = outs[0]
+    assert np.array_equal(pos, outs[1][0]) and np.array_equal(vel, outs[1][1])
+
+    def total_force(x, v, step):
+        Ft = oracle.forces_dpd(x, v, wl.box, wl.rc, q["A"], q["gamma"], q["kT"], wl.dt, step, q["seed"])
+        oracle.forces_bonds_kind(x, wl.box, wl.bonds, "harmonic", q["bond_k"], q["bond_r0"], force=Ft)
+        oracle.forces_angles(x, wl.box, ang, k_a, th0, force=Ft)
+        oracle.forces_dihedrals(x, wl.box, dih, k_d, sign, n, force=Ft)
+        return Ft
+    v = wl.vel + 0.5 * wl.dt * total_force(wl.pos, wl.vel, 0)
+    x = oracle.wrap(wl.pos + wl.dt * v, wl.box)
+    assert np.abs(min_image_diff(pos, x, wl.box)).max() < 1e-12
+    v2 = v + 0.5 * wl.dt * total_force(x, v, 1)
+    assert np.abs(vel - v2).max() < 1e-10
+
+
+def test_dihedrals_argument_checks_and_clear():
+    wl = inputs.polymer_melt(40, chain_len=8, start_seed=1, walk_seed=2, vel_seed=3)          # N = 320
+    md = B.from_workload(wl)
+    with pytest.raises(B.MDError):
+        md.set_dihedrals(np.array([[0, 1, 2, wl.N]], dtype=np.uint32))         # tag out of range
+    with pytest.raises(B.MDError):
+        md.set_dihedrals(np.array([[0, 1, 2, 1]], dtype=np.uint32))            # repeated tag
+    md.set_dihedrals(_chain_dihedrals(40, 8))
+    md.build_cells()
+    with pytest.raises(B.MDError):
+        md.forces_dihedrals(1.0, 0, 1)                                         # sign must be +-1
+    with pytest.raises(B.MDError):
+        md.forces_dihedrals(1.0, 1, 0)                                         # n >= 1
+    md.forces_dihedrals(2.0, 1, 1)
+    assert np.abs(md.get_forces()[0]).max() > 0.0
+    md.set_dihedrals(None)
+    md.set_state(wl.pos, wl.vel)
+    md.build_cells(); md.forces_dihedrals(2.0, 1, 1)
+    assert np.abs(md.get_forces()[0]).max() == 0.0
