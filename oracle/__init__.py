@@ -241,6 +241,23 @@ def forces_dihedrals(pos, box, dihedrals, k, s, n, force=None, energy=None, viri
     return F, E, W
 
 
+def langevin_u(tag, step, seed):
+    """(u_x, u_y, u_z), uniform on (-1, 1), of particle `tag` at `step` (R36)."""
+    u = np.zeros(3)
+    lib().orc_langevin_u(C.c_uint32(int(tag)), C.c_uint64(int(step)), C.c_uint64(int(seed)), u.ctypes.data_as(_dp))
+    return u
+
+
+def forces_langevin(vel, gamma, kT, dt, step, seed, force=None):
+    """F_a += -gamma v_a + sqrt(6 gamma kT / dt) u_a(step)  (R36).  Accumulates; returns force."""
+    vel, vp = _d(vel)
+    N = vel.shape[0]
+    F = np.zeros((N, 3)) if force is None else force
+    lib().orc_forces_langevin(vp, C.c_uint64(N), C.c_double(gamma), C.c_double(kT), C.c_double(dt), C.c_uint64(int(step)),
+                              C.c_uint64(int(seed)), F.ctypes.data_as(_dp))
+    return F
+
+
 def pressure(vel, box, W, mass=None):
     """P = (2 K + tr W) / (3 V)  (virial theorem, R32)."""
     m = 1.0 if mass is None else np.asarray(mass)[:, None]
@@ -358,6 +375,7 @@ class Sim:
        lj    = dict(epsilon, sigma, energy_shift)
        dpd   = dict(A, gamma, kT, seed)
        bonds = dict(k, r0)  (+ self.bonds array)
+       langevin = dict(gamma, kT, seed)   (R36)
     Forces never depend on a neighbour list here (all pairs); the rebuild trigger (O3) is evaluated
     only to log WHEN the CUDA path must rebuild.
     """
@@ -395,6 +413,10 @@ class Sim:
             p = self.what["bonds"]
             F = np.ascontiguousarray(F)
             forces_bonds(self.pos, self.box, self.bonds, p["k"], p["r0"], F, E)
+        if "langevin" in self.what:
+            p = self.what["langevin"]
+            F = np.ascontiguousarray(F)
+            forces_langevin(self.vel, p["gamma"], p["kT"], dt, step, p["seed"], F)
         self.force, self.energy = np.ascontiguousarray(F), E
         return self.force
 

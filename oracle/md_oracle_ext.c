@@ -7,7 +7,7 @@
  *
  * The paper names these features and prints no formula (pair potentials "Lennard-Jones, Gaussian, Morse,
  * Yukawa", bonds "harmonic, FENE", "angle, dihedral"; NPT/NPH integrators need the pressure),
- * so each function states the textbook form it takes (R31-R35).
+ * so each function states the textbook form it takes (R31-R36).
  *
  * Pins (tests/test_oracle_ext.py; no function here is "parity unpinned"):
  *   orc_pair_forces    Yukawa/Gaussian/Morse: closed-form values, F = -dU/dr by central differences, strict cut-off,
@@ -23,6 +23,11 @@
  *   orc_forces_dihedrals  energy k/2 (1 + s cos(n phi)) on built quadruplets for s = +-1, n = 1, 2, 3; F = -dU/dx by
  *                      central differences on all 12 coordinates; zero net force and torque; virial against
  *                      sum x_p (x) F_p; quarter-energy bookkeeping
+ *   orc_langevin_u     the words of the KAT-pinned Philox for three (tag, step, seed) triples mapped by hand; range, mean,
+ *                      variance 1/3, independence of components, steps and tags; not DPD's stream
+ *   orc_forces_langevin  kT = 0 (pure drag), v = 0 (pure noise), gamma = 0 (off), component variance 2 gamma kT / dt;
+ *                      through Sim: exact per-step decay (1 - gamma dt / m) of free particles at kT = 0 and the
+ *                      closed-form stationary variance of the discrete scheme at kT > 0
  */
 #include <math.h>
 #include <stdint.h>
@@ -300,5 +305,41 @@ void orc_forces_dihedrals(const double *pos, uint64_t N, const double box[3], co
             add_virial(W, rc_, Fc);
             add_virial(W, rd, Fd);
         }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * R36 Langevin thermostat ("Brownian (or Langevin) dynamics"; "from the same
+ * counter-based hash").  A one-body force evaluated with the other forces of the step, i.e. at the velocities after
+ * half 1 like the DPD drag (R15), and integrated by the velocity-Verlet halves:
+ *   F_a += -gamma v_a + sqrt(6 gamma kT / dt) (u_x, u_y, u_z),
+ *   u uniform on (-1, 1) (variance 1/3, so each component of the random force has variance 2 gamma kT / dt),
+ *   (X0, X1, X2, .) = Philox4x32-10(counter = (tag, 0xffffffff, step lo, step hi), key = (seed lo, seed hi)),
+ *   u_k = 2 (X_k + 0.5) 2^-32 - 1.
+ * The second counter word 0xffffffff keeps the stream apart from the DPD pair stream (min tag, max tag, ...), whose
+ * second word is a tag < N <= 2^32 - 1.  No energy, no virial (a one-body force).  force ACCUMULATED.
+ * ---------------------------------------------------------------------------------------------------------------- */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+
+void orc_langevin_u(uint32_t tag, uint64_t step, uint64_t seed, double u[3])
+{
+    uint32_t ctr[4], key[2], out[4];
+    ctr[0] = tag;
+    ctr[1] = 0xffffffffu;
+    ctr[2] = (uint32_t)(step & 0xffffffffu);
+    ctr[3] = (uint32_t)(step >> 32);
+    key[0] = (uint32_t)(seed & 0xffffffffu);
+    key[1] = (uint32_t)(seed >> 32);
+    orc_philox4x32_10(ctr, key, out);
+    for (int k = 0; k < 3; ++k) u[k] = 2.0 * (((double)out[k] + 0.5) * (1.0 / 4294967296.0)) - 1.0;
+}
+
+void orc_forces_langevin(const double *vel, uint64_t N, double gamma, double kT, double dt, uint64_t step, uint64_t seed,
+                         double *force)
+{
+    double amp = sqrt(6.0 * gamma * kT / dt), u[3];
+    for (uint64_t a = 0; a < N; ++a) {
+        orc_langevin_u((uint32_t)a, step, seed, u);
+        for (int k = 0; k < 3; ++k) force[3 * a + k] += -gamma * vel[3 * a + k] + amp * u[k];
     }
 }

@@ -255,3 +255,73 @@ def test_dihedral_energy_gradient_net_force_torque_virial(s, n):
     dih = np.array([[12 * c + i, 12 * c + i + 1, 12 * c + i + 2, 12 * c + i + 3] for c in range(5) for i in range(9)], dtype=np.uint32)
     F, E, W = oracle.forces_dihedrals(w.pos, w.box, dih, k, s, n)
     assert np.abs(F.sum(axis=0)).max() < 1e-11 * max(1.0, np.abs(F).sum())
+
+
+# ---- R36 Langevin thermostat ------------------------------------------------------------------------------------------
+def test_langevin_uniforms_stream_and_moments():
+    """u_k = 2 (X_k + 0.5) 2^-32 - 1 from the KAT-pinned Philox with counter (tag, 0xffffffff, step lo, step hi); range,
+    mean 0, variance 1/3, the three components and successive steps / tags uncorrelated; stream apart from DPD's."""
+    for tag, step, seed in [(0, 0, 0), (5, 7, 0x1234), (123456, (1 << 33) + 5, (0xdeadbeef << 32) | 77)]:
+        X = oracle.philox4x32_10([tag, 0xFFFFFFFF, step & 0xFFFFFFFF, step >> 32], [seed & 0xFFFFFFFF, seed >> 32])
+        u = oracle.langevin_u(tag, step, seed)
+        want = [(int(x) * 2 + 1) / 2.0 ** 32 - 1.0 for x in X[:3]]      # = 2 (X + 0.5) 2^-32 - 1, exact in fp64
+        assert u.tolist() == want
+    n = 40000
+    U = np.array([oracle.langevin_u(t, 11, 99) for t in range(n)])
+    assert U.min() > -1.0 and U.max() < 1.0
+    assert np.abs(U.mean(axis=0)).max() < 4.0 / math.sqrt(3 * n)
+    assert np.abs(U.var(axis=0) - 1.0 / 3.0).max() < 4.0 * math.sqrt(4.0 / 45.0 / n)      # Var(u^2) = 1/5 - 1/9
+    c = np.corrcoef(U.T)
+    assert np.abs(c - np.eye(3)).max() < 4.0 / math.sqrt(n)
+    U2 = np.array([oracle.langevin_u(t, 12, 99) for t in range(n)])
+    assert abs(np.corrcoef(U[:, 0], U2[:, 0])[0, 1]) < 4.0 / math.sqrt(n)          # next step
+    assert abs(np.corrcoef(U[:-1, 0], U[1:, 0])[0, 1]) < 4.0 / math.sqrt(n)        # next tag
+    # not the DPD stream: theta of the pair (tag, anything) never reuses these words' counter (second word 0xffffffff)
+    th = oracle.dpd_theta(3, 4, 11, 99) / math.sqrt(3.0)
+    assert all(abs(th - x) > 1e-12 for x in oracle.langevin_u(3, 11, 99))
+
+
+def test_langevin_force_limits_and_accumulation():
+    rng = np.random.default_rng(5)
+    v = rng.normal(size=(50, 3))
+    F0 = rng.normal(size=(50, 3))
+    # kT = 0: pure drag, added to what is there
+    F = oracle.forces_langevin(v, 2.5, 0.0, 0.01, 3, 8, force=F0.copy())
+    assert np.abs(F - (F0 - 2.5 * v)).max() < 1e-15
+    # v = 0: pure noise of amplitude sqrt(6 gamma kT / dt) u
+    F = oracle.forces_langevin(np.zeros((50, 3)), 2.5, 1.7, 0.01, 3, 8)
+    U = np.array([oracle.langevin_u(t, 3, 8) for t in range(50)])
+    assert np.abs(F - math.sqrt(6 * 2.5 * 1.7 / 0.01) * U).max() < 1e-12
+    # gamma = 0 switches the thermostat off
+    assert np.abs(oracle.forces_langevin(v, 0.0, 1.7, 0.01, 3, 8)).max() == 0.0
+    # variance of a component 2 gamma kT / dt
+    n = 30000
+    F = oracle.forces_langevin(np.zeros((n, 3)), 0.8, 1.3, 0.02, 21, 4)
+    assert abs(F.var() / (2 * 0.8 * 1.3 / 0.02) - 1.0) < 4.0 * math.sqrt(0.8 / (3 * n))  # kurtosis of a uniform: Var(u^2)/Var(u)^2 = 0.8
+
+
+def test_langevin_free_particles_decay_and_equilibrium():
+    """Free particles (no other force) through Sim's velocity-Verlet: the half-step velocity obeys
+    v_h' = (1 - gamma dt / m) v_h + (dt / m) R, so (a) at kT = 0 it decays by exactly (1 - gamma dt / m) per step and
+    (b) its stationary variance is (kT / m) / (1 - gamma dt / (2 m)) -- both closed forms of the discrete scheme."""
+    box, N, dt, g = 50.0, 4000, 0.01, 3.0
+    rng = np.random.default_rng(2)
+    pos = rng.uniform(0, box, size=(N, 3))
+    v0 = rng.normal(size=(N, 3))
+    s = oracle.Sim(pos, v0, box, 1.0, 0.4, {"langevin": dict(gamma=g, kT=0.0, seed=1)})
+    s.run(1, dt)
+    # after step 1: v = v_h1 (1 - a/2) with v_h1 = v0 (1 - a/2) (F(t0) = -gamma v0), a = gamma dt
+    a = g * dt
+    assert np.abs(s.vel - v0 * (1 - a / 2) ** 2).max() < 1e-14
+    s.run(9, dt)
+    # v after n steps = v_h,n (1 - a/2), v_h,n = v_h,1 (1 - a)^(n-1)
+    assert np.abs(s.vel - v0 * (1 - a / 2) ** 2 * (1 - a) ** 9).max() < 1e-13
+    # (b) equilibrium: long run from cold, many particles; full-step velocity v = v_h (1 - a/2) + (dt/2m) R'
+    kT, g, dt = 1.5, 5.0, 0.02
+    a = g * dt
+    s = oracle.Sim(pos, np.zeros((N, 3)), box, 1.0, 0.4, {"langevin": dict(gamma=g, kT=kT, seed=7)})
+    s.run(300, dt)                                  # 300 dt = 30 relaxation times 1/gamma
+    var_h = kT / (1 - a / 2)                        # stationary variance of the half-step velocity
+    var_full = var_h * (1 - a / 2) ** 2 + (dt / 2) ** 2 * (2 * g * kT / dt)
+    got = (s.vel ** 2).mean()
+    assert abs(got / var_full - 1.0) < 4.0 * math.sqrt(2.0 / (3 * N))
