@@ -70,6 +70,7 @@ typedef enum {
 #define MD_F_PAIR 16u   /* a pair potential of SURVEY.md 8(f) row 3 (pair_kind, pair_p) instead of LJ / DPD */
 #define MD_F_ANGLES 32u /* harmonic angles (md_set_angles; angle_k, angle_theta0) */
 #define MD_F_DIHEDRALS 64u /* periodic dihedrals (md_set_dihedrals; dihedral_k, dihedral_sign, dihedral_n) */
+#define MD_F_LANGEVIN 128u /* Langevin thermostat as a one-body force (langevin_gamma, langevin_kT, langevin_seed; R36) */
 
 /* pair potentials of md_forces_pair / MD_F_PAIR (PAPER.md:63 lists them, R31); parameters p[0..2] */
 enum { MD_PAIR_LJ = 0,       /* U = 4 p0 ((p1/r)^12 - (p1/r)^6)                        p0 = epsilon, p1 = sigma     */
@@ -106,6 +107,8 @@ typedef struct {
     double angle_k, angle_theta0; /* MD_F_ANGLES: U = k/2 (theta - theta0)^2, theta0 in radians */
     double dihedral_k;            /* MD_F_DIHEDRALS: U = k/2 (1 + sign cos(n phi)) */
     int32_t dihedral_sign, dihedral_n; /* sign = +1 or -1, n = 1, 2, 3, ... */
+    double langevin_gamma, langevin_kT; /* MD_F_LANGEVIN: friction coefficient and k_B T of the bath */
+    uint64_t langevin_seed;
 } md_step_desc;
 
 #define MD_N_KERNELS 8
@@ -254,6 +257,14 @@ int md_forces_angles(md_ctx *ctx, double k, double theta0);
 int md_set_dihedrals(md_ctx *ctx, const uint32_t *tag_a, const uint32_t *tag_b, const uint32_t *tag_c, const uint32_t *tag_d,
                      uint64_t n_dihedrals);
 int md_forces_dihedrals(md_ctx *ctx, double k, int sign, int n);
+
+/* Langevin thermostat (R36; "Brownian (or Langevin) dynamics"; SURVEY.md 8(f) row 3 "from the same
+   counter-based hash"): the one-body force F_i += -gamma v_i + sqrt(6 gamma kT / dt) (u_x, u_y, u_z) at the CURRENT
+   velocities, u uniform on (-1, 1): u_k = 2 (X_k + 0.5) 2^-32 - 1, X = Philox4x32-10(counter = (tag, 0xffffffff, step lo,
+   step hi), key = (seed lo, seed hi)).  ACCUMULATES into the force; no energy, no virial.  Inside md_step (MD_F_LANGEVIN)
+   it is evaluated with the other forces, after half 1, with step = the step being completed (like the DPD terms), and the
+   velocity-Verlet halves integrate it; mutually exclusive with MD_F_NVT.  gamma < 0, kT < 0 or dt <= 0: MD_EINVAL. */
+int md_forces_langevin(md_ctx *ctx, double gamma, double kT, double dt, uint64_t step, uint64_t seed);
 
 /* ---- virial and pressure (PAPER.md:63 NPT / NPH, :208, :214; R32) ----------------------------- */
 

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "csrc", "libb200md.so")
 
 MD_FP64, MD_MIXED = 0, 1
 MD_ORDER_LEX, MD_ORDER_MORTON, MD_ORDER_HILBERT = 0, 1, 2
-MD_F_LJ, MD_F_DPD, MD_F_BONDS, MD_F_NVT, MD_F_PAIR, MD_F_ANGLES, MD_F_DIHEDRALS = 1, 2, 4, 8, 16, 32, 64
+MD_F_LJ, MD_F_DPD, MD_F_BONDS, MD_F_NVT, MD_F_PAIR, MD_F_ANGLES, MD_F_DIHEDRALS, MD_F_LANGEVIN = 1, 2, 4, 8, 16, 32, 64, 128
 PAIR_KINDS = {"lj": 0, "yukawa": 1, "gaussian": 2, "morse": 3}
 BOND_KINDS = {"harmonic": 0, "fene": 1}
 MD_SCHED_SYNC, MD_SCHED_SPECULATIVE, MD_SCHED_BATCH = 0, 1, 2
@@ -29,7 +29,7 @@ KERNEL_NAMES = {MD_K_NLIST: "nlist", MD_K_LJ: "lj", MD_K_DPD: "dpd", MD_K_BONDS:
 EXPORTS = ["md_create", "md_workspace_bytes", "md_set_workspace", "md_configure", "md_destroy", "md_last_error", "md_set_state", "md_set_bonds",
            "md_get_state", "md_get_forces", "md_build_cells", "md_get_cells", "md_build_nlist", "md_get_nlist",
            "md_get_nlist_rows", "md_forces_lj", "md_forces_dpd", "md_forces_bonds", "md_forces_pair", "md_forces_fene", "md_set_angles", "md_forces_angles",
-           "md_set_dihedrals", "md_forces_dihedrals", "md_pressure",
+           "md_set_dihedrals", "md_forces_dihedrals", "md_forces_langevin", "md_pressure",
            "md_integrate_nve",
            "md_needs_rebuild", "md_step", "md_tune", "md_tune_rbuff", "md_set_option", "md_set_launch", "md_get_stats", "md_set_profiling",
            "md_debug_philox", "md_debug_peak", "md_struct_size", "md_thermo", "md_integrate_nvt", "md_set_thermostat", "md_get_thermostat"]
@@ -43,7 +43,8 @@ class md_step_desc(C.Structure):
                 ("nvt_kT", C.c_double), ("nvt_tau", C.c_double),
                 ("pair_kind", C.c_int32), ("bond_kind", C.c_int32), ("pair_p", C.c_double * 4),
                 ("angle_k", C.c_double), ("angle_theta0", C.c_double),
-                ("dihedral_k", C.c_double), ("dihedral_sign", C.c_int32), ("dihedral_n", C.c_int32)]
+                ("dihedral_k", C.c_double), ("dihedral_sign", C.c_int32), ("dihedral_n", C.c_int32),
+                ("langevin_gamma", C.c_double), ("langevin_kT", C.c_double), ("langevin_seed", C.c_uint64)]
 
 
 class md_pressure_t(C.Structure):
@@ -107,6 +108,7 @@ def load():
         "md_forces_angles": [vp, dbl, dbl],
         "md_set_dihedrals": [vp, vp, vp, vp, vp, u64],
         "md_forces_dihedrals": [vp, dbl, i32, i32],
+        "md_forces_langevin": [vp, dbl, dbl, dbl, u64, u64],
         "md_pressure": [vp, C.POINTER(md_step_desc), vp],
         "md_integrate_nve": [vp, dbl, i32],
         "md_needs_rebuild": [vp, C.POINTER(i32)],
@@ -200,6 +202,10 @@ def step_desc(kind: str, dt: float, params: dict, nvt: dict = None) -> md_step_d
         d.flags |= MD_F_DIHEDRALS
         d.dihedral_k = float(params["dihedral_k"])
         d.dihedral_sign, d.dihedral_n = int(params.get("dihedral_sign", 1)), int(params.get("dihedral_n", 1))
+    if "langevin" in params:       # dict(gamma, kT, seed): Langevin thermostat (R36)
+        q = params["langevin"]
+        d.flags |= MD_F_LANGEVIN
+        d.langevin_gamma, d.langevin_kT, d.langevin_seed = float(q["gamma"]), float(q["kT"]), int(q["seed"])
     if nvt is not None:
         d.flags |= MD_F_NVT
         d.nvt_kT, d.nvt_tau = float(nvt["kT"]), float(nvt["tau"])
@@ -352,6 +358,9 @@ class MD:
 
     def forces_dihedrals(self, k, sign=1, n=1):
         self._chk(self.L.md_forces_dihedrals(self.h, float(k), int(sign), int(n)), "md_forces_dihedrals")
+
+    def forces_langevin(self, gamma, kT, dt, step, seed):
+        self._chk(self.L.md_forces_langevin(self.h, float(gamma), float(kT), float(dt), int(step), int(seed)), "md_forces_langevin")
 
     def pressure(self, desc: md_step_desc) -> dict:
         t = md_pressure_t()

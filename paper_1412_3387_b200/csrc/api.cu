@@ -1025,6 +1025,17 @@ extern "C" int md_forces_dihedrals(md_ctx *c, double k, int sign, int n)
     return MD_OK;
 }
 
+extern "C" int md_forces_langevin(md_ctx *c, double gamma, double kT, double dt, uint64_t step, uint64_t seed)
+{
+    if (!c) return MD_EINVAL;
+    if (!(gamma >= 0.0) || !(kT >= 0.0) || !(dt > 0.0)) { c->err = "md_forces_langevin: gamma >= 0, kT >= 0, dt > 0 required"; return MD_EINVAL; }
+    if (!c->have_state) { c->err = "md_forces_langevin: md_set_state first"; return MD_ESTATE; }
+    ProfScope ps(c, MD_K_BONDS);
+    MD_TRY(launch_forces_langevin(c, gamma, kT, dt, step, seed));
+    c->force_valid = true;
+    return MD_OK;
+}
+
 extern "C" int md_integrate_nve(md_ctx *c, double dt, int half)
 {
     if (!c) return MD_EINVAL;
@@ -1132,6 +1143,12 @@ static int eval_forces(md_ctx *c, const md_step_desc *w, uint64_t step, bool ene
         }
         ProfScope ps(c, MD_K_BONDS);
         MD_TRY(launch_forces_dihedrals(c, w->dihedral_k, w->dihedral_sign, w->dihedral_n));
+    }
+    if (w->flags & MD_F_LANGEVIN) {
+        if (!(w->langevin_gamma >= 0.0) || !(w->langevin_kT >= 0.0)) { c->err = "md_step: langevin_gamma >= 0 and langevin_kT >= 0 required"; return MD_EINVAL; }
+        if (w->flags & MD_F_NVT) { c->err = "md_step: MD_F_LANGEVIN and MD_F_NVT are mutually exclusive"; return MD_EINVAL; }
+        ProfScope ps(c, MD_K_BONDS);
+        MD_TRY(launch_forces_langevin(c, w->langevin_gamma, w->langevin_kT, w->dt, step, w->langevin_seed));
     }
     c->force_valid = true;
     // only the tile LJ kernel skips the per-particle energies

@@ -379,6 +379,41 @@ int launch_forces_dihedrals(md_ctx *c, double k, int sign, int n)
 }
 
 // ------------------------------------------------------------------------------------------------------------
+// R36 Langevin thermostat: F_i += -gamma v_i + sqrt(6 gamma kT / dt) (u_x, u_y, u_z), u_k = 2 (X_k + 0.5) 2^-32 - 1 from
+// Philox4x32-10 with counter (tag, 0xffffffff, step lo, step hi), key (seed lo, seed hi).  One thread per particle, one
+// Philox block per particle and step; the operations are written in the oracle's order (no contraction): fp64 results
+// identical up to the order of the additions into the force that is already there.
+// ------------------------------------------------------------------------------------------------------------
+__global__ void k_forces_langevin(const double4 *__restrict__ vel, const uint32_t *__restrict__ tag, uint32_t N, double gamma,
+                                  double amp, uint64_t step, uint64_t seed, double4 *__restrict__ force, Gate gate)
+{
+    if (md_gate_closed(gate)) return;
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const uint4 x = md_philox4x32_10(make_uint4(tag[i], 0xffffffffu, (uint32_t)step, (uint32_t)(step >> 32)),
+                                     make_uint2((uint32_t)seed, (uint32_t)(seed >> 32)));
+    const double4 v = vel[i];
+    double4 f = force[i];
+    const double ux = __dsub_rn(__dmul_rn(2.0, __dmul_rn(__dadd_rn((double)x.x, 0.5), 1.0 / 4294967296.0)), 1.0);
+    const double uy = __dsub_rn(__dmul_rn(2.0, __dmul_rn(__dadd_rn((double)x.y, 0.5), 1.0 / 4294967296.0)), 1.0);
+    const double uz = __dsub_rn(__dmul_rn(2.0, __dmul_rn(__dadd_rn((double)x.z, 0.5), 1.0 / 4294967296.0)), 1.0);
+    f.x = __dadd_rn(f.x, __dadd_rn(__dmul_rn(-gamma, v.x), __dmul_rn(amp, ux)));
+    f.y = __dadd_rn(f.y, __dadd_rn(__dmul_rn(-gamma, v.y), __dmul_rn(amp, uy)));
+    f.z = __dadd_rn(f.z, __dadd_rn(__dmul_rn(-gamma, v.z), __dmul_rn(amp, uz)));
+    force[i] = f;
+}
+
+int launch_forces_langevin(md_ctx *c, double gamma, double kT, double dt, uint64_t step, uint64_t seed)
+{
+    const LaunchCfg &cf = c->cfg[MD_K_BONDS];
+    k_forces_langevin<<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->vel, c->tag, (uint32_t)c->N, gamma,
+                                                                          sqrt(6.0 * gamma * kT / dt), step, seed, c->force,
+                                                                          md_gate(c));
+    MD_LAUNCH_CHECK(c);
+    return MD_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
 // R32 virial W = sum over pairs of d (x) F (+ bonds, + angles and dihedrals: arm (x) F per end), order xx yy zz xy xz yz.  Every
 // particle sums HALF of each of its pair and bond terms (the list is double-sided) and its own arm of each angle; a
 // block sums a contiguous range of slots (shared-memory tree), one block sums the partials: fixed order, bit-reproducible.

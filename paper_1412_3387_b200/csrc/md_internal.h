@@ -244,6 +244,7 @@ int launch_angles_build(md_ctx *c, const uint32_t *ta, const uint32_t *tb, const
 int launch_forces_angles(md_ctx *c, double k, double theta0);
 int launch_dihedrals_build(md_ctx *c, const uint32_t *ta, const uint32_t *tb, const uint32_t *tc, const uint32_t *td, uint64_t nd);
 int launch_forces_dihedrals(md_ctx *c, double k, int sign, int n);
+int launch_forces_langevin(md_ctx *c, double gamma, double kT, double dt, uint64_t step, uint64_t seed);
 int launch_virial(md_ctx *c, const md_step_desc *w, uint64_t step, double *out6_host);
 // fused: preceded by the previous step's half 2.  nvt: Nose-Hoover friction xi read from c->nvt_state (R30)
 int launch_half1(md_ctx *c, double dt, bool fused, bool nvt = false);

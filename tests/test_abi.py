@@ -32,7 +32,7 @@ def test_struct_layouts_match_header():
     L = B.load()                                      # (load() itself refuses a library whose struct sizes differ)
     for k, st in enumerate((B.md_step_desc, B.md_stats, B.md_thermo_t, B.md_pressure_t)):
         assert L.md_struct_size(k) == C.sizeof(st), st.__name__
-    assert C.sizeof(B.md_step_desc) == 168 and C.sizeof(B.md_pressure_t) == 72 and L.md_struct_size(9) == -1
+    assert C.sizeof(B.md_step_desc) == 192 and C.sizeof(B.md_pressure_t) == 72 and L.md_struct_size(9) == -1
 
 
 def test_fails_loudly_without_gpu():

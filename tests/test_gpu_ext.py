@@ -206,3 +206,69 @@ def test_dihedrals_argument_checks_and_clear():
     md.set_state(wl.pos, wl.vel)
     md.build_cells(); md.forces_dihedrals(2.0, 1, 1)
     assert np.abs(md.get_forces()[0]).max() == 0.0
+
+
+def test_langevin_force_and_steps_against_the_oracle():
+    """R36: md_forces_langevin on top of an LJ evaluation (same Philox words as the oracle: 1e-13), md_step with LJ +
+    Langevin for 6 steps against oracle.Sim, every scheduler bit-identical, argument checks."""
+    wl = inputs.lj_fcc(6, rc=2.5, r_buff=0.4, kT=1.0, jitter=0.06, pos_seed=9, vel_seed=10)      # N = 864
+    g, kT, seed = 1.5, 1.3, (0xabcdef << 32) | 1234
+    md = B.from_workload(wl)
+    md.build_nlist()
+    md.forces_lj(1.0, 1.0, 1)
+    md.forces_langevin(g, kT, wl.dt, (1 << 33) + 7, seed)
+    F, _ = md.get_forces()
+    Fr = oracle.forces_lj(wl.pos, wl.box, wl.rc, 1.0, 1.0, 1)[0]
+    FL = oracle.forces_langevin(wl.vel, g, kT, wl.dt, (1 << 33) + 7, seed)
+    assert np.abs(FL).max() > 10.0
+    assert force_rel_err(F, Fr + FL) < 1e-10
+    # the thermostat term alone: identical words, identical operations
+    md.set_state(wl.pos, wl.vel)
+    md.build_cells()
+    md.forces_langevin(g, kT, wl.dt, 3, seed)
+    assert np.abs(md.get_forces()[0] - oracle.forces_langevin(wl.vel, g, kT, wl.dt, 3, seed)).max() < 1e-13
+    prm = dict(wl.params, langevin=dict(gamma=g, kT=kT, seed=seed))
+    desc = B.step_desc("lj", wl.dt, prm)
+    assert desc.flags == B.MD_F_LJ | B.MD_F_LANGEVIN
+    outs = []
+    for sched in (B.MD_SCHED_BATCH, B.MD_SCHED_SPECULATIVE, B.MD_SCHED_SYNC):
+        ms = B.from_workload(wl, sched=sched)
+        ms.step(desc, 6)
+        outs.append(ms.get_state())
+    for o in outs[1:]:
+        assert np.array_equal(o[0], outs[0][0]) and np.array_equal(o[1], outs[0][1])
+    sim = oracle.Sim(wl.pos, wl.vel, wl.box, wl.rc, wl.r_buff,
+                     {"lj": dict(epsilon=1.0, sigma=1.0, energy_shift=1), "langevin": dict(gamma=g, kT=kT, seed=seed)})
+    sim.run(6, wl.dt)
+    assert np.abs(min_image_diff(outs[0][0], sim.pos, wl.box)).max() < 1e-11
+    assert np.abs(outs[0][1] - sim.vel).max() < 1e-10
+    with pytest.raises(B.MDError):
+        md.forces_langevin(-1.0, kT, wl.dt, 0, 0)
+    with pytest.raises(B.MDError):
+        md.forces_langevin(g, kT, 0.0, 0, 0)
+    with pytest.raises(B.MDError):
+        B.from_workload(wl).step(B.step_desc("lj", wl.dt, prm, nvt=dict(kT=1.0, tau=0.5)), 1)
+
+
+def test_langevin_free_particles_closed_forms_on_the_device():
+    """No other force: exact per-step decay of the velocities at kT = 0 and the stationary variance of the discrete scheme
+    at kT > 0 (the closed forms the oracle is pinned with), over 4e5 particles."""
+    N, box = 400000, 120.0
+    rng = np.random.default_rng(11)
+    pos = rng.uniform(0, box, size=(N, 3))
+    v0 = rng.normal(size=(N, 3))
+    dt, g = 0.01, 3.0
+    a = g * dt
+    md = B.MD(box, N, 1.0, 0.4)
+    md.set_state(pos, v0)
+    md.step(B.step_desc("none", dt, dict(langevin=dict(gamma=g, kT=0.0, seed=1))), 10)
+    assert np.abs(md.get_state()[1] - v0 * (1 - a / 2) ** 2 * (1 - a) ** 9).max() < 1e-12
+    kT, g, dt = 1.5, 5.0, 0.02
+    a = g * dt
+    md = B.MD(box, N, 1.0, 0.4)
+    md.set_state(pos, np.zeros((N, 3)))
+    md.step(B.step_desc("none", dt, dict(langevin=dict(gamma=g, kT=kT, seed=7))), 300)
+    var_full = kT / (1 - a / 2) * (1 - a / 2) ** 2 + (dt / 2) ** 2 * (2 * g * kT / dt)
+    v = md.get_state()[1]
+    assert abs((v ** 2).mean() / var_full - 1.0) < 4.0 * math.sqrt(2.0 / (3 * N))
+    assert np.abs(v.mean(axis=0)).max() < 4.0 * math.sqrt(var_full / N)
