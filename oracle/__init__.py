@@ -164,6 +164,21 @@ def pair_forces(pos, box, rc, kind, params, energy_shift=1):
     return F, E
 
 
+def pair_table(pos, box, r_min, r_max, U, F):
+    """Tabulated pair potential (R37): U, F = -dU/dr at M evenly spaced radii in [r_min, r_max], linear interpolation.
+    Returns (force, energy, virial)."""
+    pos, pp = _d(pos)
+    b, bp = _box(box)
+    U, Up = _d(U)
+    F, Fp = _d(F)
+    assert U.shape == F.shape and U.ndim == 1 and U.shape[0] >= 2
+    N = pos.shape[0]
+    Fo = np.zeros((N, 3)); E = np.zeros(N); W = np.zeros(6)
+    lib().orc_pair_table(pp, C.c_uint64(N), bp, C.c_double(r_min), C.c_double(r_max), C.c_uint64(U.shape[0]), Up, Fp,
+                         Fo.ctypes.data_as(_dp), E.ctypes.data_as(_dp), W.ctypes.data_as(_dp))
+    return Fo, E, W
+
+
 def virial_pair(pos, box, rc, kind, params):
     """W (xx, yy, zz, xy, xz, yz) = sum over pairs of d (x) F."""
     pos, pp = _d(pos)

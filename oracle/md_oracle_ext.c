@@ -7,7 +7,7 @@
  *
  * The paper names these features and prints no formula (pair potentials "Lennard-Jones, Gaussian, Morse,
  * Yukawa", bonds "harmonic, FENE", "angle, dihedral"; NPT/NPH integrators need the pressure),
- * so each function states the textbook form it takes (R31-R36).
+ * so each function states the textbook form it takes (R31-R37).
  *
  * Pins (tests/test_oracle_ext.py; no function here is "parity unpinned"):
  *   orc_pair_forces    Yukawa/Gaussian/Morse: closed-form values, F = -dU/dr by central differences, strict cut-off,
@@ -28,6 +28,9 @@
  *   orc_forces_langevin  kT = 0 (pure drag), v = 0 (pure noise), gamma = 0 (off), component variance 2 gamma kT / dt;
  *                      through Sim: exact per-step decay (1 - gamma dt / m) of free particles at kT = 0 and the
  *                      closed-form stationary variance of the discrete scheme at kT > 0
+ *   orc_pair_table     table values at the nodes and the straight line between two nodes; tables linear in r reproduced
+ *                      at any r; nothing outside [r_min, r_max), strict at r_max; tr W = r F(r); periodic wrap; a table
+ *                      of the LJ closed forms against orc_forces_lj with second-order convergence in h
  */
 #include <math.h>
 #include <stdint.h>
@@ -342,4 +345,40 @@ void orc_forces_langevin(const double *vel, uint64_t N, double gamma, double kT,
         orc_langevin_u((uint32_t)a, step, seed, u);
         for (int k = 0; k < 3; ++k) force[3 * a + k] += -gamma * vel[3 * a + k] + amp * u[k];
     }
+}
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * R37 tabulated pair potential ("tabulated potentials"; no formula).  The caller gives U_k and F_k = -dU/dr
+ * at r_k = r_min + k h, k = 0 .. M-1, h = (r_max - r_min) / (M - 1); both are interpolated LINEARLY:
+ *   s = (r - r_min) / h,  k = floor(s) (clamped to M-2),  t = s - k,
+ *   U(r) = U_k + t (U_{k+1} - U_k),   F(r) = F_k + t (F_{k+1} - F_k),   force on a = F(r) d / r, d = minimg(x_a - x_b).
+ * Pairs with r_min <= r < r_max contribute (r^2 < r_max^2 strict, like every cut-off here; a pair closer than r_min is
+ * outside the table and contributes nothing).  No energy shift: the table is what the caller wants.
+ * force / energy (may be NULL) OVERWRITTEN; W (may be NULL) = sum over pairs of d (x) F, overwritten.
+ * ---------------------------------------------------------------------------------------------------------------- */
+void orc_pair_table(const double *pos, uint64_t N, const double box[3], double r_min, double r_max, uint64_t M,
+                    const double *U, const double *F, double *force, double *energy, double *W)
+{
+    double h = (r_max - r_min) / (double)(M - 1), d[3], Fv[3];
+    if (force) memset(force, 0, sizeof(double) * 3 * N);
+    if (energy) memset(energy, 0, sizeof(double) * N);
+    if (W) memset(W, 0, sizeof(double) * 6);
+    for (uint64_t a = 0; a < N; ++a)
+        for (uint64_t b = a + 1; b < N; ++b) {
+            double r2 = sep(pos + 3 * a, pos + 3 * b, box, d);
+            if (!(r2 < r_max * r_max)) continue;
+            double r = sqrt(r2);
+            if (r < r_min) continue;
+            double s = (r - r_min) / h;
+            uint64_t k = (uint64_t)floor(s);
+            if (k > M - 2) k = M - 2;
+            double t = s - (double)k;
+            double u = U[k] + t * (U[k + 1] - U[k]);
+            double f = (F[k] + t * (F[k + 1] - F[k])) / r;
+            for (int x = 0; x < 3; ++x) Fv[x] = f * d[x];
+            if (force)
+                for (int x = 0; x < 3; ++x) { force[3 * a + x] += Fv[x]; force[3 * b + x] -= Fv[x]; }
+            if (energy) { energy[a] += 0.5 * u; energy[b] += 0.5 * u; }
+            if (W) add_virial(W, d, Fv);
+        }
 }

@@ -325,3 +325,65 @@ def test_langevin_free_particles_decay_and_equilibrium():
     var_full = var_h * (1 - a / 2) ** 2 + (dt / 2) ** 2 * (2 * g * kT / dt)
     got = (s.vel ** 2).mean()
     assert abs(got / var_full - 1.0) < 4.0 * math.sqrt(2.0 / (3 * N))
+
+
+# ---- R37 tabulated pair potential -------------------------------------------------------------------------------------
+def _two(r, box=20.0, direction=(0.36, -0.48, 0.8)):
+    d = np.array(direction) / np.linalg.norm(direction)
+    return np.array([[1.0, 2.0, 3.0], np.array([1.0, 2.0, 3.0]) - r * d]), box, d      # d = unit vector from b to a
+
+
+def test_pair_table_nodes_linear_tables_and_range():
+    r_min, r_max, M = 0.5, 2.5, 41                       # h = 0.05
+    rk = np.linspace(r_min, r_max, M)
+    rng = np.random.default_rng(3)
+    U, F = rng.normal(size=M), rng.normal(size=M)
+    # at a node the table values come back; between two nodes the straight line between them
+    for k, t in [(0, 0.0), (7, 0.0), (7, 0.25), (39, 0.5), (39, 0.999)]:
+        r = rk[k] + t * (rk[1] - rk[0])
+        pos, box, d = _two(r)
+        Fo, E, W = oracle.pair_table(pos, box, r_min, r_max, U, F)
+        f = F[k] + t * (F[k + 1] - F[k])
+        u = U[k] + t * (U[k + 1] - U[k])
+        assert np.abs(Fo[0] - f * d).max() < 1e-12 and np.abs(Fo[0] + Fo[1]).max() == 0.0
+        assert abs(E[0] - 0.5 * u) < 1e-12 and abs(E[1] - 0.5 * u) < 1e-12
+        assert abs(W[0] + W[1] + W[2] - r * f) < 1e-12                     # tr W = r F(r) for one pair
+    # a table that is linear in r is reproduced at any r
+    a0, a1, b0, b1 = 1.5, -0.7, 0.3, 2.0
+    for r in (0.5, 0.777, 1.93, 2.4999):
+        pos, box, d = _two(r)
+        Fo, E, _ = oracle.pair_table(pos, box, r_min, r_max, a0 + a1 * rk, b0 + b1 * rk)
+        assert np.abs(Fo[0] - (b0 + b1 * r) * d).max() < 1e-12 and abs(2 * E[0] - (a0 + a1 * r)) < 1e-12
+    # outside [r_min, r_max): nothing; strict at r_max
+    for r in (0.49, 0.4999999, 2.5, 2.6):
+        pos, box, d = _two(r)
+        Fo, E, W = oracle.pair_table(pos, box, r_min, r_max, U, F)
+        assert np.abs(Fo).max() == 0.0 and np.abs(E).max() == 0.0 and np.abs(W).max() == 0.0
+    # through the periodic wrap
+    pos, box, d = _two(1.2, box=6.0)
+    pos2 = pos.copy(); pos2[1] += [6.0, -6.0, 0.0]
+    A, B_ = oracle.pair_table(pos, box, r_min, r_max, U, F), oracle.pair_table(oracle.wrap(pos2, box), box, r_min, r_max, U, F)
+    assert np.abs(A[0] - B_[0]).max() < 1e-12
+
+
+def test_pair_table_of_lj_converges_to_lj_at_second_order():
+    """A table filled from the LJ closed forms reproduces orc_forces_lj on a liquid-like configuration with the error of
+    linear interpolation, h^2/8 max|f''|: quartering h gives 1/16 of the error."""
+    rng = np.random.default_rng(8)
+    n = 5
+    g = (np.stack(np.meshgrid(*[np.arange(n)] * 3, indexing="ij"), -1).reshape(-1, 3) + 0.5) * 1.2
+    pos = g + rng.uniform(-0.08, 0.08, size=g.shape)
+    box, rc, r_min = n * 1.2, 2.5, 0.8
+    Fr, Er = oracle.forces_lj(pos, box, rc, 1.0, 1.0, 0)
+    errs = []
+    for M in (1701, 6801):
+        rk = np.linspace(r_min, rc, M)
+        U = 4 * (rk ** -12 - rk ** -6)
+        F = 24 * (2 * rk ** -13 - rk ** -7)
+        Fo, E, W = oracle.pair_table(pos, box, r_min, rc, U, F)
+        errs.append(np.abs(Fo - Fr).max())
+        assert np.abs(E - Er).max() < 30 * (rk[1] - rk[0]) ** 2
+        Wr = oracle.virial_pair(pos, box, rc, "lj", (1.0, 1.0))
+        assert np.abs(W - Wr).max() < 1e-3 * np.abs(Wr).max()
+    assert errs[0] < 2e-3 and 12.0 < errs[0] / errs[1] < 20.0
+    assert np.abs(Fo.sum(axis=0)).max() < 1e-11                      # Newton's third law
