@@ -76,7 +76,8 @@ typedef enum {
 enum { MD_PAIR_LJ = 0,       /* U = 4 p0 ((p1/r)^12 - (p1/r)^6)                        p0 = epsilon, p1 = sigma     */
        MD_PAIR_YUKAWA = 1,   /* U = p0 exp(-p1 r) / r                                  p0 = epsilon, p1 = kappa     */
        MD_PAIR_GAUSSIAN = 2, /* U = p0 exp(-r^2 / (2 p1^2))                            p0 = epsilon, p1 = sigma     */
-       MD_PAIR_MORSE = 3 };  /* U = p0 (exp(-2 p1 (r - p2)) - 2 exp(-p1 (r - p2)))     p0 = D0, p1 = alpha, p2 = r0 */
+       MD_PAIR_MORSE = 3,    /* U = p0 (exp(-2 p1 (r - p2)) - 2 exp(-p1 (r - p2)))     p0 = D0, p1 = alpha, p2 = r0 */
+       MD_PAIR_TABLE = 4 };  /* the table of md_set_pair_table, linear interpolation (R37); p unused, no energy shift */
 /* bond potentials (R19, R33) */
 enum { MD_BOND_HARMONIC = 0, /* U = k/2 (r - r0)^2 */
        MD_BOND_FENE = 1 };   /* U = -1/2 k r0^2 ln(1 - (r/r0)^2), r < r0 (r >= r0: NaN, the bond is broken) */
@@ -236,6 +237,14 @@ int md_forces_bonds(md_ctx *ctx, double k, double r0);
    by U(rc) if energy_shift.  Same kernel structure as md_forces_lj (w threads per particle over the row, shuffle
    reduction, one write), on the exact 32-bit list.  OVERWRITES force/energy.  fp64 in both precision modes. */
 int md_forces_pair(md_ctx *ctx, int kind, const double p[4], int energy_shift);
+
+/* Tabulated pair potential (R37; "tabulated potentials"): U[k] and F[k] = -dU/dr at r_k = r_min + k h,
+   k = 0 .. m-1, h = (r_max - r_min) / (m - 1); 0 <= r_min < r_max <= r_cut, 2 <= m < 2^31.  U and F are interpolated
+   linearly in r (k = floor((r - r_min) / h), clamped to m - 2); a pair contributes if r_min <= r and r^2 < r_max^2
+   (strict), F(r) d / r to the first particle and half of U(r) to each energy.  U, F: HOST or DEVICE arrays of m
+   doubles, copied.  m = 0 clears.  Used by md_forces_pair(kind = MD_PAIR_TABLE) and MD_F_PAIR with pair_kind =
+   MD_PAIR_TABLE (MD_ESTATE if no table is set); the virial of md_pressure follows the same interpolation. */
+int md_set_pair_table(md_ctx *ctx, double r_min, double r_max, const double *U, const double *F, uint64_t m);
 
 /* FENE bonds on the bond table of md_set_bonds (R33).  ACCUMULATES, like md_forces_bonds. */
 int md_forces_fene(md_ctx *ctx, double k, double r0);

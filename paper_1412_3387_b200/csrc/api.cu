@@ -917,9 +917,36 @@ extern "C" int md_forces_fene(md_ctx *c, double k, double r0)
     return MD_OK;
 }
 
+extern "C" int md_set_pair_table(md_ctx *c, double r_min, double r_max, const double *U, const double *F, uint64_t m)
+{
+    if (!c) return MD_EINVAL;
+    MD_TRY(alloc_state(c));
+    MD_TRY(md_sync(c));
+    if (c->tab_uf) { md_free(c, c->tab_uf); c->tab_uf = nullptr; }
+    c->tab_m = 0;
+    if (m == 0) return MD_OK;
+    if (!U || !F || m < 2 || m >= 0x7fffffffull || !(r_min >= 0.0) || !(r_min < r_max) || !(r_max <= c->rc)) {
+        c->err = "md_set_pair_table: need U, F, 2 <= m < 2^31 and 0 <= r_min < r_max <= r_cut";
+        return MD_EINVAL;
+    }
+    MD_TRY(md_alloc(c, (void **)&c->tab_uf, 2 * m * sizeof(double)));
+    Stage st(c);
+    const uint64_t bb = m * sizeof(double);
+    MD_TRY(st.reserve(stage_need(U, bb) + stage_need(F, bb)));
+    const void *du, *df;
+    MD_TRY(stage_in(c, st, U, bb, &du));
+    MD_TRY(stage_in(c, st, F, bb, &df));
+    MD_TRY(launch_table_pack(c, (const double *)du, (const double *)df, (uint32_t)m));
+    c->tab_m = (uint32_t)m;
+    c->tab_rmin = r_min;
+    c->tab_rmax = r_max;
+    return md_sync(c);
+}
+
 extern "C" int md_forces_pair(md_ctx *c, int kind, const double p[4], int shift)
 {
-    if (!c || !p || kind < MD_PAIR_LJ || kind > MD_PAIR_MORSE) { if (c) c->err = "md_forces_pair: bad argument"; return MD_EINVAL; }
+    if (!c || (!p && kind != MD_PAIR_TABLE) || kind < MD_PAIR_LJ || kind > MD_PAIR_TABLE) { if (c) c->err = "md_forces_pair: bad argument"; return MD_EINVAL; }
+    if (kind == MD_PAIR_TABLE && c->tab_m == 0) { c->err = "md_forces_pair: md_set_pair_table first"; return MD_ESTATE; }
     MD_TRY(need_nlist(c, "md_forces_pair"));
     ProfScope ps(c, MD_K_LJ);
     MD_TRY(ensure_decoded(c));
@@ -1120,7 +1147,8 @@ static int eval_forces(md_ctx *c, const md_step_desc *w, uint64_t step, bool ene
     }
     if (w->flags & MD_F_PAIR) {
         if (any) { c->err = "md_step: the pair terms (LJ, DPD, MD_F_PAIR) are mutually exclusive (each overwrites the force)"; return MD_EINVAL; }
-        if (w->pair_kind < MD_PAIR_LJ || w->pair_kind > MD_PAIR_MORSE) { c->err = "md_step: unknown pair_kind"; return MD_EINVAL; }
+        if (w->pair_kind < MD_PAIR_LJ || w->pair_kind > MD_PAIR_TABLE) { c->err = "md_step: unknown pair_kind"; return MD_EINVAL; }
+        if (w->pair_kind == MD_PAIR_TABLE && c->tab_m == 0) { c->err = "md_step: md_set_pair_table first"; return MD_ESTATE; }
         ProfScope ps(c, MD_K_LJ);
         MD_TRY(ensure_decoded(c));
         MD_TRY(launch_forces_pair(c, w->pair_kind, w->pair_p, w->lj_energy_shift));
@@ -1635,6 +1663,10 @@ extern "C" int md_pressure(md_ctx *c, const md_step_desc *w, md_pressure_t *out)
 {
     if (!c || !w || !out) return MD_EINVAL;
     if (!c->have_state) { c->err = "md_pressure: md_set_state first"; return MD_ESTATE; }
+    if (w->flags & MD_F_PAIR) {
+        if (w->pair_kind < MD_PAIR_LJ || w->pair_kind > MD_PAIR_TABLE) { c->err = "md_pressure: unknown pair_kind"; return MD_EINVAL; }
+        if (w->pair_kind == MD_PAIR_TABLE && c->tab_m == 0) { c->err = "md_pressure: md_set_pair_table first"; return MD_ESTATE; }
+    }
     if ((w->flags & (MD_F_LJ | MD_F_DPD | MD_F_PAIR)) && (!c->nlist_valid || c->steps_since_build > 0)) {
         // the pair virial needs a list of the current positions only if the old one may have lost pairs: between
         // rebuilds the list still covers every pair within rc, so a valid list is enough

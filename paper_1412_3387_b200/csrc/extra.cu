@@ -1,14 +1,17 @@
-// extra.cu -- SURVEY.md 8(f) rows 1 and 3 on the device: further short-range pair potentials (Yukawa, Gaussian, Morse) on
-// the W-threads-per-particle force kernel, harmonic angles (per-particle CSR, no atomics), and the virial of every force
-// term for the pressure (NPT / NPH of PAPER.md:63 need it).  The paper names these and prints no formula: DESIGN.md
-// R31-R34.  fp64 throughout; the pair kernels read the exact 32-bit neighbour list (a tile list is decoded first).
+// extra.cu -- SURVEY.md 8(f) rows 1 and 3 on the device: further short-range pair potentials (Yukawa, Gaussian, Morse,
+// tabulated) on the W-threads-per-particle force kernel, harmonic angles and periodic dihedrals (per-particle CSR, no
+// atomics), the Langevin thermostat as a one-body force, and the virial of every force term for the pressure (NPT / NPH
+// of PAPER.md:63 need it).  The paper names these and prints no formula: DESIGN.md R31-R37.  fp64 throughout; the pair kernels read the exact 32-bit neighbour list (a tile list is decoded first).
 #include "md_device.cuh"
 
 // ------------------------------------------------------------------------------------------------------------
-// R31: f = -(dU/dr)/r and U of one pair; POT: MD_PAIR_LJ / YUKAWA / GAUSSIAN / MORSE
+// R31, R37: f = -(dU/dr)/r and U of one pair; POT: MD_PAIR_LJ / YUKAWA / GAUSSIAN / MORSE / TABLE
 // ------------------------------------------------------------------------------------------------------------
 struct PairParams {
     double rc2, p0, p1, p2, uc;  // uc = U(rc) if the energy is shifted, else 0
+    // MD_PAIR_TABLE (R37): (U_k, F_k) at r_min + k h; rc2 = r_max^2, p0 = r_min, p1 = h
+    const double2 *tab;
+    uint32_t tab_m;
 };
 
 template <int POT>
@@ -26,10 +29,21 @@ __device__ __forceinline__ double pair_eval(double r2, const PairParams &p, doub
         const double e = p.p0 * exp(-r2 / (2.0 * p.p1 * p.p1));
         u = e;
         return e / (p.p1 * p.p1);
-    } else {
+    } else if (POT == MD_PAIR_MORSE) {
         const double r = sqrt(r2), e1 = exp(-p.p1 * (r - p.p2)), e2 = e1 * e1;
         u = p.p0 * (e2 - 2.0 * e1);
         return 2.0 * p.p1 * p.p0 * (e2 - e1) / r;
+    } else {  // MD_PAIR_TABLE: linear interpolation of U and F between the two nodes around r; nothing below r_min
+        const double r = sqrt(r2);
+        u = 0.0;
+        if (r < p.p0) return 0.0;
+        const double s = __ddiv_rn(__dsub_rn(r, p.p0), p.p1);
+        uint32_t k = (uint32_t)floor(s);
+        k = min(k, p.tab_m - 2u);
+        const double t = __dsub_rn(s, (double)k);
+        const double2 a = __ldg(p.tab + k), b = __ldg(p.tab + k + 1);
+        u = a.x + t * (b.x - a.x);
+        return (a.y + t * (b.y - a.y)) / r;
     }
 }
 
@@ -83,10 +97,35 @@ __global__ void __launch_bounds__(1024) k_forces_pair(const double4 *__restrict_
 static PairParams make_pair_params(md_ctx *c, int kind, const double prm[4], int shift)
 {
     PairParams p;
+    p.tab = nullptr;
+    p.tab_m = 0;
+    if (kind == MD_PAIR_TABLE) {
+        p.rc2 = c->tab_rmax * c->tab_rmax;
+        p.p0 = c->tab_rmin;
+        p.p1 = (c->tab_rmax - c->tab_rmin) / (double)(c->tab_m - 1);
+        p.p2 = 0.0;
+        p.uc = 0.0;
+        p.tab = (const double2 *)c->tab_uf;
+        p.tab_m = c->tab_m;
+        return p;
+    }
     p.rc2 = c->rc * c->rc;
     p.p0 = prm[0]; p.p1 = prm[1]; p.p2 = prm[2];
     p.uc = shift ? pair_host_u(kind, p.rc2, p.p0, p.p1, p.p2) : 0.0;
     return p;
+}
+
+__global__ void k_table_pack(const double *__restrict__ U, const double *__restrict__ F, uint32_t m, double2 *__restrict__ tab)
+{
+    const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < m) tab[k] = make_double2(U[k], F[k]);
+}
+
+int launch_table_pack(md_ctx *c, const double *U, const double *F, uint32_t m)
+{
+    k_table_pack<<<md_grid(m, 256), 256, 0, c->stream>>>(U, F, m, (double2 *)c->tab_uf);
+    MD_LAUNCH_CHECK(c);
+    return MD_OK;
 }
 
 int launch_forces_pair(md_ctx *c, int kind, const double prm[4], int shift)
@@ -100,6 +139,7 @@ int launch_forces_pair(md_ctx *c, int kind, const double prm[4], int shift)
     case MD_PAIR_LJ: k_forces_pair<W_, MD_PAIR_LJ><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force, md_gate(c)); break; \
     case MD_PAIR_YUKAWA: k_forces_pair<W_, MD_PAIR_YUKAWA><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force, md_gate(c)); break; \
     case MD_PAIR_GAUSSIAN: k_forces_pair<W_, MD_PAIR_GAUSSIAN><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force, md_gate(c)); break; \
+    case MD_PAIR_TABLE: k_forces_pair<W_, MD_PAIR_TABLE><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force, md_gate(c)); break; \
     default: k_forces_pair<W_, MD_PAIR_MORSE><<<grid, cf.block, 0, c->stream>>>(c->pos, c->nl_cnt_exp, c->nl_off, c->nl_idx, c->g, p, c->force, md_gate(c)); break; \
     }
     switch (w) {
@@ -595,6 +635,7 @@ int launch_virial(md_ctx *c, const md_step_desc *w, uint64_t step, double *out6_
     case MD_PAIR_YUKAWA: VIR_LAUNCH(MD_PAIR_YUKAWA); break;
     case MD_PAIR_GAUSSIAN: VIR_LAUNCH(MD_PAIR_GAUSSIAN); break;
     case MD_PAIR_MORSE: VIR_LAUNCH(MD_PAIR_MORSE); break;
+    case MD_PAIR_TABLE: VIR_LAUNCH(MD_PAIR_TABLE); break;
     case VIR_DPD: VIR_LAUNCH(VIR_DPD); break;
     default: VIR_LAUNCH(VIR_NONE); break;
     }

@@ -272,3 +272,52 @@ def test_langevin_free_particles_closed_forms_on_the_device():
     v = md.get_state()[1]
     assert abs((v ** 2).mean() / var_full - 1.0) < 4.0 * math.sqrt(2.0 / (3 * N))
     assert np.abs(v.mean(axis=0)).max() < 4.0 * math.sqrt(var_full / N)
+
+
+@pytest.mark.parametrize("order", [B.MD_ORDER_MORTON, B.MD_ORDER_LEX])
+def test_tabulated_pair_potential_forces_energies_virial_and_step(order):
+    """R37 through the C-ABI: a random table (forces and energies 1e-10 of the oracle's, same interpolation), a table of the
+    LJ closed forms against the analytic LJ kernel at the interpolation error, virial, md_step, argument checks."""
+    wl = inputs.lj_fcc(7, rc=2.5, r_buff=0.4, kT=1.0, jitter=0.08, pos_seed=13, vel_seed=14)      # N = 1372
+    r_min, r_max, M = 0.7, 2.3, 257
+    rng = np.random.default_rng(4)
+    U, F = rng.normal(size=M), 5.0 * rng.normal(size=M)
+    Fr, Er, Wr = oracle.pair_table(wl.pos, wl.box, r_min, r_max, U, F)
+    for w in (1, 4, 8):
+        md = B.from_workload(wl, order=order)
+        md.set_launch(B.MD_K_LJ, 128, w)
+        md.set_pair_table(r_min, r_max, U, F)
+        md.build_nlist()
+        md.forces_pair("table")
+        Fo, E = md.get_forces()
+        assert force_rel_err(Fo, Fr) < 1e-10 and np.abs(E - Er).max() < 1e-11 * np.abs(Er).max()
+    desc = B.step_desc("pair", wl.dt, dict(pair_kind="table"))
+    pr = md.pressure(desc)
+    assert np.abs(pr["virial"] - Wr).max() < 1e-10 * np.abs(Wr).max()
+    # LJ closed forms in a fine table: the analytic kernel within the interpolation error
+    rk = np.linspace(0.8, wl.rc, 6801)
+    md.set_pair_table(0.8, wl.rc, 4 * (rk ** -12 - rk ** -6), 24 * (2 * rk ** -13 - rk ** -7))
+    md.forces_pair("table")
+    Ft = md.get_forces()[0]
+    md.forces_pair("lj", (1.0, 1.0), 0)
+    assert np.abs(Ft - md.get_forces()[0]).max() < 2e-4
+    # one md_step with the random table against the oracle sequence
+    ms = B.from_workload(wl, order=order)
+    ms.set_pair_table(r_min, r_max, U, F)
+    ms.step(desc, 1)
+    pos, vel, _ = ms.get_state()
+    v = wl.vel + 0.5 * wl.dt * Fr
+    x = oracle.wrap(wl.pos + wl.dt * v, wl.box)
+    assert np.abs(min_image_diff(pos, x, wl.box)).max() < 1e-12
+    v2 = v + 0.5 * wl.dt * oracle.pair_table(x, wl.box, r_min, r_max, U, F)[0]
+    assert np.abs(vel - v2).max() < 1e-11
+    # argument checks: r_max beyond the cut-off, one-point table, no table set
+    with pytest.raises(B.MDError):
+        ms.set_pair_table(0.5, wl.rc + 0.1, U, F)
+    with pytest.raises(B.MDError):
+        ms.set_pair_table(0.5, 2.0, U[:1], F[:1])
+    ms.set_pair_table(0, 0, None, None)
+    with pytest.raises(B.MDError):
+        ms.forces_pair("table")
+    with pytest.raises(B.MDError):
+        ms.step(desc, 1)
