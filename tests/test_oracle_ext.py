@@ -328,7 +328,7 @@ def test_langevin_free_particles_decay_and_equilibrium():
 
 
 # ---- R37 tabulated pair potential -------------------------------------------------------------------------------------
-def _two(r, box=20.0, direction=(0.36, -0.48, 0.8)):
+def _two_at(r, box=20.0, direction=(0.36, -0.48, 0.8)):
     d = np.array(direction) / np.linalg.norm(direction)
     return np.array([[1.0, 2.0, 3.0], np.array([1.0, 2.0, 3.0]) - r * d]), box, d      # d = unit vector from b to a
 
@@ -341,7 +341,7 @@ def test_pair_table_nodes_linear_tables_and_range():
     # at a node the table values come back; between two nodes the straight line between them
     for k, t in [(0, 0.0), (7, 0.0), (7, 0.25), (39, 0.5), (39, 0.999)]:
         r = rk[k] + t * (rk[1] - rk[0])
-        pos, box, d = _two(r)
+        pos, box, d = _two_at(r)
         Fo, E, W = oracle.pair_table(pos, box, r_min, r_max, U, F)
         f = F[k] + t * (F[k + 1] - F[k])
         u = U[k] + t * (U[k + 1] - U[k])
@@ -351,16 +351,16 @@ def test_pair_table_nodes_linear_tables_and_range():
     # a table that is linear in r is reproduced at any r
     a0, a1, b0, b1 = 1.5, -0.7, 0.3, 2.0
     for r in (0.5, 0.777, 1.93, 2.4999):
-        pos, box, d = _two(r)
+        pos, box, d = _two_at(r)
         Fo, E, _ = oracle.pair_table(pos, box, r_min, r_max, a0 + a1 * rk, b0 + b1 * rk)
         assert np.abs(Fo[0] - (b0 + b1 * r) * d).max() < 1e-12 and abs(2 * E[0] - (a0 + a1 * r)) < 1e-12
     # outside [r_min, r_max): nothing; strict at r_max
     for r in (0.49, 0.4999999, 2.5, 2.6):
-        pos, box, d = _two(r)
+        pos, box, d = _two_at(r)
         Fo, E, W = oracle.pair_table(pos, box, r_min, r_max, U, F)
         assert np.abs(Fo).max() == 0.0 and np.abs(E).max() == 0.0 and np.abs(W).max() == 0.0
     # through the periodic wrap
-    pos, box, d = _two(1.2, box=6.0)
+    pos, box, d = _two_at(1.2, box=6.0)
     pos2 = pos.copy(); pos2[1] += [6.0, -6.0, 0.0]
     A, B_ = oracle.pair_table(pos, box, r_min, r_max, U, F), oracle.pair_table(oracle.wrap(pos2, box), box, r_min, r_max, U, F)
     assert np.abs(A[0] - B_[0]).max() < 1e-12
