@@ -362,6 +362,27 @@ typedef struct md_thermo_t {
 } md_thermo_t;
 int md_thermo(md_ctx *ctx, md_thermo_t *out);
 
+/* The same kinetic-energy / momentum reduction for callers that cannot allocate device memory (code under CUDA graph
+   capture, tight serving loops, harnesses that forbid cudaMalloc).  No context: the caller passes the inputs and the
+   output; the per-block partial sums, which md_thermo keeps in a buffer of the context, live in a file-scope __device__
+   array of the library (256 KiB, held by every GPU that loads the library until the process exits).  Calls no
+   cudaMalloc / cudaFree and no allocating library routine; enqueues two kernels on `stream` and returns WITHOUT
+   synchronising.
+     vel    DEVICE pointer, N x 3 doubles, row-major (velocities in the caller's own order)
+     mass   DEVICE pointer, N doubles, or NULL (every mass 1)
+     N      number of particles, 0 <= N <= MD_NOALLOC_MAX_N; beyond it MD_EINVAL with a message that names the limit
+            (use md_thermo on a context for larger systems)
+     out4   DEVICE pointer, 4 doubles, overwritten when the kernels have run: sum 1/2 m v^2, sum m v_x, m v_y, m v_z
+     stream cudaStream_t as a pointer; NULL = the default stream
+   Fixed summation order (blocks of 4096 particles, then one block over the partials): bit-reproducible for a given
+   input.  A host pointer is MD_EINVAL (nothing is staged).  The scratch array is shared by ALL calls on a device and
+   keeps the last call's contents; nothing in it needs clearing (a call writes every slot it reads), but two calls that
+   overlap on the GPU -- different streams, or graph branches without a dependency -- race on it: serialise them.
+   md_noalloc_last_error: text of the calling thread's last failure of md_kinetic_noalloc. */
+#define MD_NOALLOC_MAX_N 33554432ull /* 8192 block partials x 4096 particles */
+int md_kinetic_noalloc(const double *vel, const double *mass, uint64_t N, double *out4, void *stream);
+const char *md_noalloc_last_error(void);
+
 /* on = 1: bracket every stage launched by md_step / md_build_* / md_forces_* / md_integrate_nve with CUDA events on the
    context's stream and accumulate their durations into md_stats.stage_ms (MD_K_CELLS = binning + reorder, MD_K_NLIST =
    count + scan + fill, MD_K_LJ / MD_K_DPD / MD_K_BONDS force kernels, MD_K_INTEGRATE both halves).  Resets the

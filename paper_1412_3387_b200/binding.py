@@ -32,7 +32,8 @@ EXPORTS = ["md_create", "md_workspace_bytes", "md_set_workspace", "md_configure"
            "md_set_dihedrals", "md_forces_dihedrals", "md_forces_langevin", "md_pressure",
            "md_integrate_nve",
            "md_needs_rebuild", "md_step", "md_tune", "md_tune_rbuff", "md_set_option", "md_set_launch", "md_get_stats", "md_set_profiling",
-           "md_debug_philox", "md_debug_peak", "md_struct_size", "md_thermo", "md_integrate_nvt", "md_set_thermostat", "md_get_thermostat"]
+           "md_debug_philox", "md_debug_peak", "md_struct_size", "md_thermo", "md_integrate_nvt", "md_set_thermostat", "md_get_thermostat",
+           "md_kinetic_noalloc", "md_noalloc_last_error"]
 
 
 class md_step_desc(C.Structure):
@@ -127,6 +128,7 @@ def load():
         "md_integrate_nvt": [vp, C.c_double, i32, C.c_double, C.c_double],
         "md_set_thermostat": [vp, C.c_double, C.c_double],
         "md_get_thermostat": [vp, vp, vp],
+        "md_kinetic_noalloc": [vp, vp, u64, vp, vp],
     }
     for name, args in sig.items():
         fn = getattr(L, name)
@@ -137,6 +139,8 @@ def load():
             raise MDError(f"binding out of date: sizeof({st.__name__}) = {C.sizeof(st)}, library says {L.md_struct_size(k)}")
     L.md_last_error.argtypes = [vp]
     L.md_last_error.restype = C.c_char_p
+    L.md_noalloc_last_error.argtypes = []
+    L.md_noalloc_last_error.restype = C.c_char_p
     _lib = L
     return L
 
@@ -459,6 +463,20 @@ class MD:
         out = np.empty_like(ctr)
         self._chk(self.L.md_debug_philox(self.h, _ptr(ctr), _ptr(key), _ptr(out), ctr.shape[0]), "md_debug_philox")
         return out
+
+
+MD_NOALLOC_MAX_N = 8192 * 4096
+
+
+def kinetic_noalloc(vel, mass, out4, n=None, stream=None):
+    """md_kinetic_noalloc: sum 1/2 m v^2 and sum m v of n particles into out4 (4 doubles), device tensors only, no
+    allocation anywhere, no synchronisation.  stream: a raw cudaStream_t value (e.g. torch.cuda.Stream.cuda_stream) or None."""
+    L = load()
+    if n is None:
+        n = vel.shape[0]
+    s = L.md_kinetic_noalloc(_ptr(vel), _ptr(mass), int(n), _ptr(out4), C.c_void_p(stream) if stream else None)
+    if s != 0:
+        raise MDError(f"md_kinetic_noalloc -> {s}: {L.md_noalloc_last_error().decode()}")
 
 
 def from_workload(w, precision=None, **kw) -> MD:

@@ -9,7 +9,7 @@ from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(os.path.dirname(HERE))
-SOURCES = ["api.cu", "cells.cu", "nlist.cu", "forces.cu", "integrate.cu", "tiles.cu", "peak.cu", "extra.cu"]
+SOURCES = ["api.cu", "cells.cu", "nlist.cu", "forces.cu", "integrate.cu", "tiles.cu", "peak.cu", "extra.cu", "noalloc.cu"]
 HEADERS = ["md_internal.h", "md_device.cuh", os.path.join(ROOT, "include", "b200md.h")]
 LIB = os.path.join(HERE, "libb200md.so")
 OBJ_DIR = os.path.join(HERE, "build")
