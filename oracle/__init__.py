@@ -217,6 +217,26 @@ def forces_bonds_kind(pos, box, bonds, kind, k, r0, force=None, energy=None, vir
     return F, E, W
 
 
+def bond_table(pos, box, bonds, r_min, r_max, U, F, force=None, energy=None, virial=None):
+    """Tabulated bonds (R38): U, F = -dU/dr at len(U) evenly spaced lengths in [r_min, r_max], linear interpolation; a bond
+    outside [r_min, r_max) gives NaN.  Accumulates; returns (force, energy, virial)."""
+    pos, pp = _d(pos)
+    b, bp = _box(box)
+    N = pos.shape[0]
+    bonds = np.ascontiguousarray(bonds, dtype=np.uint32).reshape(-1, 2)
+    ta, tap = _u(bonds[:, 0])
+    tb, tbp = _u(bonds[:, 1])
+    U, Up = _d(U)
+    F, Fp = _d(F)
+    assert U.shape == F.shape and U.ndim == 1 and U.shape[0] >= 2
+    Fo = np.zeros((N, 3)) if force is None else force
+    E = np.zeros(N) if energy is None else energy
+    W = np.zeros(6) if virial is None else virial
+    lib().orc_bond_table(pp, C.c_uint64(N), bp, tap, tbp, C.c_uint64(bonds.shape[0]), C.c_double(r_min), C.c_double(r_max),
+                         C.c_uint64(U.shape[0]), Up, Fp, Fo.ctypes.data_as(_dp), E.ctypes.data_as(_dp), W.ctypes.data_as(_dp))
+    return Fo, E, W
+
+
 def forces_angles(pos, box, angles, k, theta0, force=None, energy=None, virial=None):
     """angles: (n, 3) tags (a, b, c), b the vertex.  Accumulates; returns (force, energy, virial)."""
     pos, pp = _d(pos)

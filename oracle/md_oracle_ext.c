@@ -7,7 +7,7 @@
  *
  * The paper names these features and prints no formula (pair potentials "Lennard-Jones, Gaussian, Morse,
  * Yukawa", bonds "harmonic, FENE", "angle, dihedral"; NPT/NPH integrators need the pressure),
- * so each function states the textbook form it takes (R31-R37).
+ * so each function states the textbook form it takes (R31-R38).
  *
  * Pins (tests/test_oracle_ext.py; no function here is "parity unpinned"):
  *   orc_pair_forces    Yukawa/Gaussian/Morse: closed-form values, F = -dU/dr by central differences, strict cut-off,
@@ -31,6 +31,9 @@
  *   orc_pair_table     table values at the nodes and the straight line between two nodes; tables linear in r reproduced
  *                      at any r; nothing outside [r_min, r_max), strict at r_max; tr W = r F(r); periodic wrap; a table
  *                      of the LJ closed forms against orc_forces_lj with second-order convergence in h
+ *   orc_bond_table     nodes and the straight line between them, NaN outside [r_min, r_max), accumulation, bond
+ *                      direction, periodic wrap, tr W = r F(r); the table of a harmonic bond against
+ *                      orc_forces_bonds_kind (forces exact, energies within k h^2 / 8 per bond, from above)
  */
 #include <math.h>
 #include <stdint.h>
@@ -381,4 +384,42 @@ void orc_pair_table(const double *pos, uint64_t N, const double box[3], double r
             if (energy) { energy[a] += 0.5 * u; energy[b] += 0.5 * u; }
             if (W) add_virial(W, d, Fv);
         }
+}
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * R38 tabulated bonds ("harmonic, FENE and tabulated bonds"; no formula).  Same table and the same linear
+ * interpolation as the tabulated pair potential (R37), evaluated on the bond list:
+ *   U_k, F_k = -dU/dr at r_k = r_min + k h, h = (r_max - r_min) / (M - 1);  s = (r - r_min) / h, k = floor(s) clamped to
+ *   M - 2, t = s - k;  U(r) = U_k + t (U_{k+1} - U_k), F(r) = F_k + t (F_{k+1} - F_k);  F_a += F(r) d / r, F_b -= same,
+ *   d = minimg(x_a - x_b); half of U(r) to each particle.
+ * A bond with r < r_min or r >= r_max has left its table: NaN (like the FENE bond beyond r0, R33).
+ * force / energy / W (each may be NULL) are ACCUMULATED.
+ * ---------------------------------------------------------------------------------------------------------------- */
+void orc_bond_table(const double *pos, uint64_t N, const double box[3], const uint32_t *tag_a, const uint32_t *tag_b,
+                    uint64_t n_bonds, double r_min, double r_max, uint64_t M, const double *U, const double *F,
+                    double *force, double *energy, double *W)
+{
+    (void)N;
+    double h = (r_max - r_min) / (double)(M - 1), d[3], Fv[3];
+    for (uint64_t m = 0; m < n_bonds; ++m) {
+        uint64_t a = tag_a[m], b = tag_b[m];
+        double r2 = sep(pos + 3 * a, pos + 3 * b, box, d);
+        if (!(r2 > 0.0)) continue;
+        double r = sqrt(r2), f, u;
+        if (r < r_min || !(r < r_max)) {
+            f = NAN; u = NAN;
+        } else {
+            double s = (r - r_min) / h;
+            uint64_t k = (uint64_t)floor(s);
+            if (k > M - 2) k = M - 2;
+            double t = s - (double)k;
+            u = U[k] + t * (U[k + 1] - U[k]);
+            f = (F[k] + t * (F[k + 1] - F[k])) / r;
+        }
+        for (int x = 0; x < 3; ++x) Fv[x] = f * d[x];
+        if (force)
+            for (int x = 0; x < 3; ++x) { force[3 * a + x] += Fv[x]; force[3 * b + x] -= Fv[x]; }
+        if (energy) { energy[a] += 0.5 * u; energy[b] += 0.5 * u; }
+        if (W) add_virial(W, d, Fv);
+    }
 }

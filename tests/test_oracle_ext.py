@@ -387,3 +387,54 @@ def test_pair_table_of_lj_converges_to_lj_at_second_order():
         assert np.abs(W - Wr).max() < 1e-3 * np.abs(Wr).max()
     assert errs[0] < 2e-3 and 12.0 < errs[0] / errs[1] < 20.0
     assert np.abs(Fo.sum(axis=0)).max() < 1e-11                      # Newton's third law
+
+
+# ---- R38 tabulated bonds ----------------------------------------------------------------------------------------------
+def test_bond_table_nodes_lines_range_and_accumulation():
+    r_min, r_max, M = 0.4, 1.6, 25                       # h = 0.05
+    rk = np.linspace(r_min, r_max, M)
+    rng = np.random.default_rng(31)
+    U, F = rng.normal(size=M), rng.normal(size=M)
+    bond = np.array([[0, 1]], dtype=np.uint32)
+    for k, t in [(0, 0.0), (5, 0.0), (5, 0.4), (23, 0.5), (23, 0.999)]:
+        r = rk[k] + t * (rk[1] - rk[0])
+        pos, box, d = _two_at(r)
+        Fo, E, W = oracle.bond_table(pos, box, bond, r_min, r_max, U, F)
+        f = F[k] + t * (F[k + 1] - F[k])
+        u = U[k] + t * (U[k + 1] - U[k])
+        assert np.abs(Fo[0] - f * d).max() < 1e-12 and np.abs(Fo[0] + Fo[1]).max() == 0.0
+        assert abs(E[0] - 0.5 * u) < 1e-12 and abs(E[1] - 0.5 * u) < 1e-12
+        assert abs(W[0] + W[1] + W[2] - r * f) < 1e-12
+    # a bond that has left its table is broken: NaN on both ends (like FENE beyond r0)
+    for r in (0.39, 1.6, 1.7):
+        pos, box, d = _two_at(r)
+        Fo, E, _ = oracle.bond_table(pos, box, bond, r_min, r_max, U, F)
+        assert np.isnan(Fo).all() and np.isnan(E).all()
+    # accumulates onto what is there; the reversed bond gives the same forces; through the wrap
+    pos, box, d = _two_at(1.1, box=5.0)
+    F0 = rng.normal(size=(2, 3)); E0 = rng.normal(size=2); W0 = rng.normal(size=6)
+    A = oracle.bond_table(pos, box, bond, r_min, r_max, U, F)
+    Bc = oracle.bond_table(pos, box, bond, r_min, r_max, U, F, force=F0.copy(), energy=E0.copy(), virial=W0.copy())
+    assert np.abs(Bc[0] - (F0 + A[0])).max() < 1e-15 and np.abs(Bc[1] - (E0 + A[1])).max() < 1e-15
+    assert np.abs(Bc[2] - (W0 + A[2])).max() < 1e-15
+    R = oracle.bond_table(pos, box, bond[:, ::-1], r_min, r_max, U, F)
+    assert np.abs(R[0] - A[0]).max() < 1e-15 and np.abs(R[2] - A[2]).max() < 1e-15
+    pos2 = pos.copy(); pos2[1] += [-5.0, 5.0, 5.0]
+    assert np.abs(oracle.bond_table(oracle.wrap(pos2, box), box, bond, r_min, r_max, U, F)[0] - A[0]).max() < 1e-12
+
+
+def test_bond_table_of_the_harmonic_bond_is_the_harmonic_bond():
+    """F of a harmonic bond is linear in r, so its table reproduces orc_forces_bonds exactly (to rounding) on a chain;
+    U is quadratic: the interpolation error is at most k h^2 / 8 per bond."""
+    rng = np.random.default_rng(32)
+    n = 40
+    steps = rng.normal(size=(n - 1, 3)); steps *= (rng.uniform(0.7, 1.3, size=n - 1) / np.linalg.norm(steps, axis=1))[:, None]
+    pos = oracle.wrap(np.vstack([[3.0, 3.0, 3.0], 3.0 + np.cumsum(steps, axis=0)]), 9.0)
+    bonds = np.stack([np.arange(n - 1), np.arange(1, n)], axis=1).astype(np.uint32)
+    k, r0, r_min, r_max, M = 30.0, 0.9, 0.5, 1.5, 201
+    rk = np.linspace(r_min, r_max, M)
+    Ft, Et, Wt = oracle.bond_table(pos, 9.0, bonds, r_min, r_max, 0.5 * k * (rk - r0) ** 2, -k * (rk - r0))
+    Fh, Eh, Wh = oracle.forces_bonds_kind(pos, 9.0, bonds, "harmonic", k, r0)
+    assert np.abs(Ft - Fh).max() < 1e-11 and np.abs(Wt - Wh).max() < 1e-11
+    h = rk[1] - rk[0]
+    assert 0.0 <= (Et - Eh).min() and (Et - Eh).max() <= 2 * 0.5 * k * h * h / 8 + 1e-12   # chord above a convex U; 2 bonds per bead
