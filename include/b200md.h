@@ -80,7 +80,8 @@ enum { MD_PAIR_LJ = 0,       /* U = 4 p0 ((p1/r)^12 - (p1/r)^6)                 
        MD_PAIR_TABLE = 4 };  /* the table of md_set_pair_table, linear interpolation (R37); p unused, no energy shift */
 /* bond potentials (R19, R33) */
 enum { MD_BOND_HARMONIC = 0, /* U = k/2 (r - r0)^2 */
-       MD_BOND_FENE = 1 };   /* U = -1/2 k r0^2 ln(1 - (r/r0)^2), r < r0 (r >= r0: NaN, the bond is broken) */
+       MD_BOND_FENE = 1,     /* U = -1/2 k r0^2 ln(1 - (r/r0)^2), r < r0 (r >= r0: NaN, the bond is broken) */
+       MD_BOND_TABLE = 2 };  /* the table of md_set_bond_table, linear interpolation (R38); bond_k, bond_r0 unused */
 
 /* scheduling of md_step */
 #define MD_SCHED_SYNC 0        /* the host waits for the rebuild flag of half 1 before it enqueues the forces */
@@ -245,6 +246,15 @@ int md_forces_pair(md_ctx *ctx, int kind, const double p[4], int energy_shift);
    doubles, copied.  m = 0 clears.  Used by md_forces_pair(kind = MD_PAIR_TABLE) and MD_F_PAIR with pair_kind =
    MD_PAIR_TABLE (MD_ESTATE if no table is set); the virial of md_pressure follows the same interpolation. */
 int md_set_pair_table(md_ctx *ctx, double r_min, double r_max, const double *U, const double *F, uint64_t m);
+
+/* Tabulated bonds (R38; "harmonic, FENE and tabulated bonds") on the bonds of md_set_bonds: U[k] and
+   F[k] = -dU/dr at r_k = r_min + k h, k = 0 .. m-1, h = (r_max - r_min) / (m - 1), 0 <= r_min < r_max, 2 <= m < 2^31,
+   interpolated linearly in r exactly like md_set_pair_table's; one table for all bonds (R27).  A bond with r < r_min or
+   r >= r_max has left its table: NaN in the forces and energies of both ends (like the FENE bond beyond r0).
+   U, F: HOST or DEVICE arrays of m doubles, copied; m = 0 clears.  md_forces_bond_table ACCUMULATES like md_forces_bonds
+   (MD_ESTATE if no table is set); md_step / md_pressure take it with bond_kind = MD_BOND_TABLE. */
+int md_set_bond_table(md_ctx *ctx, double r_min, double r_max, const double *U, const double *F, uint64_t m);
+int md_forces_bond_table(md_ctx *ctx);
 
 /* FENE bonds on the bond table of md_set_bonds (R33).  ACCUMULATES, like md_forces_bonds. */
 int md_forces_fene(md_ctx *ctx, double k, double r0);

@@ -18,7 +18,7 @@ MD_FP64, MD_MIXED = 0, 1
 MD_ORDER_LEX, MD_ORDER_MORTON, MD_ORDER_HILBERT = 0, 1, 2
 MD_F_LJ, MD_F_DPD, MD_F_BONDS, MD_F_NVT, MD_F_PAIR, MD_F_ANGLES, MD_F_DIHEDRALS, MD_F_LANGEVIN = 1, 2, 4, 8, 16, 32, 64, 128
 PAIR_KINDS = {"lj": 0, "yukawa": 1, "gaussian": 2, "morse": 3, "table": 4}
-BOND_KINDS = {"harmonic": 0, "fene": 1}
+BOND_KINDS = {"harmonic": 0, "fene": 1, "table": 2}
 MD_SCHED_SYNC, MD_SCHED_SPECULATIVE, MD_SCHED_BATCH = 0, 1, 2
 MD_OPT_TILE_BRICK, MD_OPT_ACC_BLOCK, MD_OPT_RETUNE_PERIOD = 1, 2, 4
 MD_N_KERNELS = 8
@@ -28,7 +28,7 @@ KERNEL_NAMES = {MD_K_NLIST: "nlist", MD_K_LJ: "lj", MD_K_DPD: "dpd", MD_K_BONDS:
 
 EXPORTS = ["md_create", "md_workspace_bytes", "md_set_workspace", "md_configure", "md_destroy", "md_last_error", "md_set_state", "md_set_bonds",
            "md_get_state", "md_get_forces", "md_build_cells", "md_get_cells", "md_build_nlist", "md_get_nlist",
-           "md_get_nlist_rows", "md_forces_lj", "md_forces_dpd", "md_forces_bonds", "md_forces_pair", "md_set_pair_table", "md_forces_fene", "md_set_angles", "md_forces_angles",
+           "md_get_nlist_rows", "md_forces_lj", "md_forces_dpd", "md_forces_bonds", "md_forces_pair", "md_set_pair_table", "md_set_bond_table", "md_forces_bond_table", "md_forces_fene", "md_set_angles", "md_forces_angles",
            "md_set_dihedrals", "md_forces_dihedrals", "md_forces_langevin", "md_pressure",
            "md_integrate_nve",
            "md_needs_rebuild", "md_step", "md_tune", "md_tune_rbuff", "md_set_option", "md_set_launch", "md_get_stats", "md_set_profiling",
@@ -105,6 +105,8 @@ def load():
         "md_forces_bonds": [vp, dbl, dbl],
         "md_forces_pair": [vp, i32, C.POINTER(dbl), i32],
         "md_set_pair_table": [vp, dbl, dbl, vp, vp, u64],
+        "md_set_bond_table": [vp, dbl, dbl, vp, vp, u64],
+        "md_forces_bond_table": [vp],
         "md_forces_fene": [vp, dbl, dbl],
         "md_set_angles": [vp, vp, vp, vp, u64],
         "md_forces_angles": [vp, dbl, dbl],
@@ -199,7 +201,7 @@ def step_desc(kind: str, dt: float, params: dict, nvt: dict = None) -> md_step_d
     if "bond_kind" in params and (d.flags & MD_F_BONDS or params.get("bonds_on")):
         d.flags |= MD_F_BONDS
         d.bond_kind = BOND_KINDS[params["bond_kind"]]
-        d.bond_k, d.bond_r0 = params["bond_k"], params["bond_r0"]
+        d.bond_k, d.bond_r0 = params.get("bond_k", 0.0), params.get("bond_r0", 0.0)
     if "angle_k" in params:
         d.flags |= MD_F_ANGLES
         d.angle_k, d.angle_theta0 = float(params["angle_k"]), float(params["angle_theta0"])
@@ -350,6 +352,20 @@ class MD:
         if U.shape != F.shape or U.ndim != 1:
             raise ValueError("U and F must be 1-D arrays of the same length")
         self._chk(self.L.md_set_pair_table(self.h, float(r_min), float(r_max), _ptr(U), _ptr(F), U.shape[0]), "md_set_pair_table")
+
+    def set_bond_table(self, r_min, r_max, U, F):
+        """U, F = -dU/dr at len(U) evenly spaced bond lengths in [r_min, r_max] (R38); None clears."""
+        if U is None:
+            self._chk(self.L.md_set_bond_table(self.h, 0.0, 0.0, None, None, 0), "md_set_bond_table")
+            return
+        U = np.ascontiguousarray(U, dtype=np.float64)
+        F = np.ascontiguousarray(F, dtype=np.float64)
+        if U.shape != F.shape or U.ndim != 1:
+            raise ValueError("U and F must be 1-D arrays of the same length")
+        self._chk(self.L.md_set_bond_table(self.h, float(r_min), float(r_max), _ptr(U), _ptr(F), U.shape[0]), "md_set_bond_table")
+
+    def forces_bond_table(self):
+        self._chk(self.L.md_forces_bond_table(self.h), "md_forces_bond_table")
 
     def forces_fene(self, k, r0):
         self._chk(self.L.md_forces_fene(self.h, float(k), float(r0)), "md_forces_fene")

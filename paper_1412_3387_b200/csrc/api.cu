@@ -917,6 +917,44 @@ extern "C" int md_forces_fene(md_ctx *c, double k, double r0)
     return MD_OK;
 }
 
+extern "C" int md_set_bond_table(md_ctx *c, double r_min, double r_max, const double *U, const double *F, uint64_t m)
+{
+    if (!c) return MD_EINVAL;
+    MD_TRY(alloc_state(c));
+    MD_TRY(md_sync(c));
+    if (c->btab_uf) { md_free(c, c->btab_uf); c->btab_uf = nullptr; }
+    c->btab_m = 0;
+    if (m == 0) return MD_OK;
+    if (!U || !F || m < 2 || m >= 0x7fffffffull || !(r_min >= 0.0) || !(r_min < r_max)) {
+        c->err = "md_set_bond_table: need U, F, 2 <= m < 2^31 and 0 <= r_min < r_max";
+        return MD_EINVAL;
+    }
+    MD_TRY(md_alloc(c, (void **)&c->btab_uf, 2 * m * sizeof(double)));
+    Stage st(c);
+    const uint64_t bb = m * sizeof(double);
+    MD_TRY(st.reserve(stage_need(U, bb) + stage_need(F, bb)));
+    const void *du, *df;
+    MD_TRY(stage_in(c, st, U, bb, &du));
+    MD_TRY(stage_in(c, st, F, bb, &df));
+    MD_TRY(launch_table_pack(c, (const double *)du, (const double *)df, (uint32_t)m, c->btab_uf));
+    c->btab_m = (uint32_t)m;
+    c->btab_rmin = r_min;
+    c->btab_rmax = r_max;
+    return md_sync(c);
+}
+
+extern "C" int md_forces_bond_table(md_ctx *c)
+{
+    if (!c) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_forces_bond_table: md_set_state first"; return MD_ESTATE; }
+    if (c->btab_m == 0) { c->err = "md_forces_bond_table: md_set_bond_table first"; return MD_ESTATE; }
+    if (c->n_bonds == 0) { c->force_valid = true; return MD_OK; }
+    ProfScope ps(c, MD_K_BONDS);
+    MD_TRY(launch_forces_bonds(c, 0.0, 0.0, MD_BOND_TABLE));
+    c->force_valid = true;
+    return MD_OK;
+}
+
 extern "C" int md_set_pair_table(md_ctx *c, double r_min, double r_max, const double *U, const double *F, uint64_t m)
 {
     if (!c) return MD_EINVAL;
@@ -936,7 +974,7 @@ extern "C" int md_set_pair_table(md_ctx *c, double r_min, double r_max, const do
     const void *du, *df;
     MD_TRY(stage_in(c, st, U, bb, &du));
     MD_TRY(stage_in(c, st, F, bb, &df));
-    MD_TRY(launch_table_pack(c, (const double *)du, (const double *)df, (uint32_t)m));
+    MD_TRY(launch_table_pack(c, (const double *)du, (const double *)df, (uint32_t)m, c->tab_uf));
     c->tab_m = (uint32_t)m;
     c->tab_rmin = r_min;
     c->tab_rmax = r_max;
@@ -1156,7 +1194,8 @@ static int eval_forces(md_ctx *c, const md_step_desc *w, uint64_t step, bool ene
     }
     if (!any) MD_TRY(launch_zero_force(c));
     if ((w->flags & MD_F_BONDS) && c->n_bonds) {
-        if (w->bond_kind != MD_BOND_HARMONIC && w->bond_kind != MD_BOND_FENE) { c->err = "md_step: unknown bond_kind"; return MD_EINVAL; }
+        if (w->bond_kind < MD_BOND_HARMONIC || w->bond_kind > MD_BOND_TABLE) { c->err = "md_step: unknown bond_kind"; return MD_EINVAL; }
+        if (w->bond_kind == MD_BOND_TABLE && c->btab_m == 0) { c->err = "md_step: md_set_bond_table first"; return MD_ESTATE; }
         ProfScope ps(c, MD_K_BONDS);
         MD_TRY(launch_forces_bonds(c, w->bond_k, w->bond_r0, w->bond_kind));
     }
@@ -1663,6 +1702,10 @@ extern "C" int md_pressure(md_ctx *c, const md_step_desc *w, md_pressure_t *out)
 {
     if (!c || !w || !out) return MD_EINVAL;
     if (!c->have_state) { c->err = "md_pressure: md_set_state first"; return MD_ESTATE; }
+    if ((w->flags & MD_F_BONDS) && c->n_bonds) {
+        if (w->bond_kind < MD_BOND_HARMONIC || w->bond_kind > MD_BOND_TABLE) { c->err = "md_pressure: unknown bond_kind"; return MD_EINVAL; }
+        if (w->bond_kind == MD_BOND_TABLE && c->btab_m == 0) { c->err = "md_pressure: md_set_bond_table first"; return MD_ESTATE; }
+    }
     if (w->flags & MD_F_PAIR) {
         if (w->pair_kind < MD_PAIR_LJ || w->pair_kind > MD_PAIR_TABLE) { c->err = "md_pressure: unknown pair_kind"; return MD_EINVAL; }
         if (w->pair_kind == MD_PAIR_TABLE && c->tab_m == 0) { c->err = "md_pressure: md_set_pair_table first"; return MD_ESTATE; }

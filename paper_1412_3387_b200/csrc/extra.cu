@@ -121,9 +121,9 @@ __global__ void k_table_pack(const double *__restrict__ U, const double *__restr
     if (k < m) tab[k] = make_double2(U[k], F[k]);
 }
 
-int launch_table_pack(md_ctx *c, const double *U, const double *F, uint32_t m)
+int launch_table_pack(md_ctx *c, const double *U, const double *F, uint32_t m, double *dst_uf)
 {
-    k_table_pack<<<md_grid(m, 256), 256, 0, c->stream>>>(U, F, m, (double2 *)c->tab_uf);
+    k_table_pack<<<md_grid(m, 256), 256, 0, c->stream>>>(U, F, m, (double2 *)dst_uf);
     MD_LAUNCH_CHECK(c);
     return MD_OK;
 }
@@ -468,6 +468,9 @@ struct VirialTerms {
     uint64_t dpd_step, dpd_seed;
     int bond_kind;  // -1: none
     double bond_k, bond_r0;
+    const double2 *btab;  // MD_BOND_TABLE: bond_k = r_min, bond_r0 = h, btab_hi = r_max
+    uint32_t btab_m;
+    double btab_hi;
     int angles;
     double angle_k, angle_theta0;
     int dihedrals;
@@ -533,8 +536,20 @@ __global__ void __launch_bounds__(VIR_BLOCK) k_virial(const double4 *__restrict_
                 const double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
                 if (r2 > 0.0) {
                     double f;
-                    if (vt.bond_kind == 0) { const double r = sqrt(r2); f = -vt.bond_k * (r - vt.bond_r0) / r; }
-                    else f = -vt.bond_k / (1.0 - r2 / (vt.bond_r0 * vt.bond_r0));
+                    if (vt.bond_kind == MD_BOND_HARMONIC) { const double r = sqrt(r2); f = -vt.bond_k * (r - vt.bond_r0) / r; }
+                    else if (vt.bond_kind == MD_BOND_FENE) f = -vt.bond_k / (1.0 - r2 / (vt.bond_r0 * vt.bond_r0));
+                    else {
+                        const double r = sqrt(r2);
+                        if (r < vt.bond_k || !(r < vt.btab_hi)) f = nan("");
+                        else {
+                            const double sx = __ddiv_rn(__dsub_rn(r, vt.bond_k), vt.bond_r0);
+                            uint32_t kk = (uint32_t)floor(sx);
+                            kk = min(kk, vt.btab_m - 2u);
+                            const double tt = __dsub_rn(sx, (double)kk);
+                            const double2 a = __ldg(vt.btab + kk), b2 = __ldg(vt.btab + kk + 1);
+                            f = (a.y + tt * (b2.y - a.y)) / r;
+                        }
+                    }
                     const double F[3] = {f * d[0], f * d[1], f * d[2]};
                     vir_add(w, 0.5, d, F);
                 }
@@ -621,6 +636,13 @@ int launch_virial(md_ctx *c, const md_step_desc *w, uint64_t step, double *out6_
     vt.bond_kind = ((w->flags & MD_F_BONDS) && c->n_bonds) ? w->bond_kind : -1;
     vt.bond_k = w->bond_k;
     vt.bond_r0 = w->bond_r0;
+    if (vt.bond_kind == MD_BOND_TABLE) {
+        vt.btab = (const double2 *)c->btab_uf;
+        vt.btab_m = c->btab_m;
+        vt.bond_k = c->btab_rmin;
+        vt.bond_r0 = (c->btab_rmax - c->btab_rmin) / (double)(c->btab_m - 1);
+        vt.btab_hi = c->btab_rmax;
+    }
     vt.angles = ((w->flags & MD_F_ANGLES) && c->n_angles) ? 1 : 0;
     vt.angle_k = w->angle_k;
     vt.angle_theta0 = w->angle_theta0;

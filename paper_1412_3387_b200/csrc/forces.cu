@@ -169,11 +169,13 @@ int launch_forces_dpd(md_ctx *c, double A, double gamma, double kT, double dt, u
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// harmonic (R19) and FENE (R33) bonds: every particle sums its own bonds (CSR by tag, partners ascending), no atomics.
+// harmonic (R19), FENE (R33) and tabulated (R38) bonds: every particle sums its own bonds (CSR by tag, partners ascending),
+// no atomics.  Tabulated: kb = r_min, r0 = h (node spacing), tab = (U_k, F_k) pairs, tab_m nodes, r_hi = r_max.
 // ------------------------------------------------------------------------------------------------------------
 __global__ void k_forces_bonds(const double4 *__restrict__ pos, const uint32_t *__restrict__ tag,
                                const uint32_t *__restrict__ rtag, const uint32_t *__restrict__ bond_off,
                                const uint32_t *__restrict__ bond_partner, Geom g, double kb, double r0, int kind,
+                               const double2 *__restrict__ tab, uint32_t tab_m, double r_hi,
                                double4 *__restrict__ force, Gate gate)
 {
     if (md_gate_closed(gate)) return;
@@ -196,10 +198,23 @@ __global__ void k_forces_bonds(const double4 *__restrict__ pos, const uint32_t *
                 const double r = sqrt(r2);
                 f = -kb * (r - r0) / r;
                 u = 0.5 * kb * (r - r0) * (r - r0);
-            } else {  // FENE (R33): NaN once the bond is stretched to r0
+            } else if (kind == MD_BOND_FENE) {  // DESIGN.md R33: NaN once the bond is stretched to r0
                 const double x = r2 / (r0 * r0);
                 f = x < 1.0 ? -kb / (1.0 - x) : nan("");
                 u = x < 1.0 ? -0.5 * kb * r0 * r0 * log(1.0 - x) : nan("");
+            } else {  // tabulated (R38): linear interpolation between two nodes; NaN once the bond has left the table
+                const double r = sqrt(r2);
+                if (r < kb || !(r < r_hi)) {
+                    f = nan(""); u = nan("");
+                } else {
+                    const double sx = __ddiv_rn(__dsub_rn(r, kb), r0);
+                    uint32_t k = (uint32_t)floor(sx);
+                    k = min(k, tab_m - 2u);
+                    const double t = __dsub_rn(sx, (double)k);
+                    const double2 a = __ldg(tab + k), b2 = __ldg(tab + k + 1);
+                    u = a.x + t * (b2.x - a.x);
+                    f = (a.y + t * (b2.y - a.y)) / r;
+                }
             }
             fx += f * dx;
             fy += f * dy;
@@ -215,8 +230,19 @@ __global__ void k_forces_bonds(const double4 *__restrict__ pos, const uint32_t *
 int launch_forces_bonds(md_ctx *c, double k, double r0, int kind)
 {
     const LaunchCfg &cf = c->cfg[MD_K_BONDS];
+    const double2 *tab = nullptr;
+    uint32_t tab_m = 0;
+    double r_hi = 0.0;
+    if (kind == MD_BOND_TABLE) {  // parameters of md_set_bond_table (the caller has checked that one is set)
+        tab = (const double2 *)c->btab_uf;
+        tab_m = c->btab_m;
+        k = c->btab_rmin;
+        r0 = (c->btab_rmax - c->btab_rmin) / (double)(c->btab_m - 1);
+        r_hi = c->btab_rmax;
+    }
     k_forces_bonds<<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->pos, c->tag, c->rtag, c->bond_off,
-                                                                       c->bond_partner, c->g, k, r0, kind, c->force, md_gate(c));
+                                                                       c->bond_partner, c->g, k, r0, kind, tab, tab_m, r_hi,
+                                                                       c->force, md_gate(c));
     MD_LAUNCH_CHECK(c);
     return MD_OK;
 }

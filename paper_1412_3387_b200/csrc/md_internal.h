@@ -154,6 +154,10 @@ struct md_ctx {
     double *tab_uf = nullptr;
     uint32_t tab_m = 0;
     double tab_rmin = 0.0, tab_rmax = 0.0;
+    // tabulated bonds (R38): same layout
+    double *btab_uf = nullptr;
+    uint32_t btab_m = 0;
+    double btab_rmin = 0.0, btab_rmax = 0.0;
     // dihedrals: same layout, quadruplets as uint4
     uint64_t n_dihedrals = 0;
     uint32_t *dih_off = nullptr, *dih_ent = nullptr, *dih_abcd = nullptr;
@@ -244,7 +248,7 @@ int launch_forces_dpd(md_ctx *c, double A, double gamma, double kT, double dt, u
 int launch_forces_bonds(md_ctx *c, double k, double r0, int kind = 0);  // kind: MD_BOND_*
 // extra.cu
 int launch_forces_pair(md_ctx *c, int kind, const double prm[4], int shift);
-int launch_table_pack(md_ctx *c, const double *U, const double *F, uint32_t m);
+int launch_table_pack(md_ctx *c, const double *U, const double *F, uint32_t m, double *dst_uf);
 int launch_angles_build(md_ctx *c, const uint32_t *ta, const uint32_t *tb, const uint32_t *tc, uint64_t na);
 int launch_forces_angles(md_ctx *c, double k, double theta0);
 int launch_dihedrals_build(md_ctx *c, const uint32_t *ta, const uint32_t *tb, const uint32_t *tc, const uint32_t *td, uint64_t nd);

@@ -321,3 +321,71 @@ def test_tabulated_pair_potential_forces_energies_virial_and_step(order):
         ms.forces_pair("table")
     with pytest.raises(B.MDError):
         ms.step(desc, 1)
+
+
+def test_tabulated_bonds_forces_energy_virial_and_step():
+    """R38 through the C-ABI: md_forces_bond_table with a random table (1e-10 of the oracle's, same interpolation), the table
+    of the configured harmonic bond against md_forces_bonds, the virial with DPD, one md_step, NaN for a bond that left the
+    table, argument checks."""
+    wl = inputs.polymer_melt(40, chain_len=32, start_seed=26, walk_seed=27, vel_seed=28)          # N = 1280, bond step 0.97
+    r_min, r_max, M = 0.3, 1.9, 129
+    rng = np.random.default_rng(6)
+    U, F = rng.normal(size=M), 8.0 * rng.normal(size=M)
+    md = B.from_workload(wl)
+    md.set_bond_table(r_min, r_max, U, F)
+    md.build_cells()
+    md.forces_bond_table()
+    Fo, E = md.get_forces()
+    Fr, Er, Wr = oracle.bond_table(wl.pos, wl.box, wl.bonds, r_min, r_max, U, F)
+    assert np.isfinite(Fr).all() and np.abs(Fr).max() > 1.0
+    assert force_rel_err(Fo, Fr) < 1e-10 and np.abs(E - Er).max() < 1e-11 * np.abs(Er).max()
+    # the harmonic bond as a table: forces equal to the analytic kernel's to rounding
+    q = wl.params
+    rk = np.linspace(r_min, r_max, M)
+    md.set_bond_table(r_min, r_max, 0.5 * q["bond_k"] * (rk - q["bond_r0"]) ** 2, -q["bond_k"] * (rk - q["bond_r0"]))
+    md.set_state(wl.pos, wl.vel); md.build_cells(); md.forces_bond_table()
+    Ft = md.get_forces()[0]
+    md.set_state(wl.pos, wl.vel); md.build_cells(); md.forces_bonds(q["bond_k"], q["bond_r0"])
+    assert np.abs(Ft - md.get_forces()[0]).max() < 1e-10
+    # virial of DPD + tabulated bonds, then one md_step against the oracle sequence
+    md.set_bond_table(r_min, r_max, U, F)
+    desc = B.step_desc("polymer", wl.dt, dict(q, bond_kind="table"))
+    assert desc.flags == B.MD_F_DPD | B.MD_F_BONDS and desc.bond_kind == 2
+    pr = md.pressure(desc)
+    Wd = oracle.virial_dpd(wl.pos, wl.vel, wl.box, wl.rc, q["A"], q["gamma"], q["kT"], wl.dt, 0, q["seed"])
+    assert np.abs(pr["virial"] - (Wd + Wr)).max() < 1e-10 * np.abs(Wd + Wr).max()
+    ms = B.from_workload(wl)
+    ms.set_bond_table(r_min, r_max, U, F)
+    ms.step(desc, 1)
+    pos, vel, _ = ms.get_state()
+
+    def total_force(x, v, step):
+        Ft_ = oracle.forces_dpd(x, v, wl.box, wl.rc, q["A"], q["gamma"], q["kT"], wl.dt, step, q["seed"])
+        oracle.bond_table(x, wl.box, wl.bonds, r_min, r_max, U, F, force=Ft_)
+        return Ft_
+    v = wl.vel + 0.5 * wl.dt * total_force(wl.pos, wl.vel, 0)
+    x = oracle.wrap(wl.pos + wl.dt * v, wl.box)
+    assert np.abs(min_image_diff(pos, x, wl.box)).max() < 1e-12
+    assert np.abs(vel - (v + 0.5 * wl.dt * total_force(x, v, 1))).max() < 1e-10
+    # a bond stretched beyond the table (chain end 0 pulled to 1.5 from its neighbour, table ends at 1.3): its two ends
+    # are NaN, every other particle keeps its value, as in the oracle
+    pos2 = wl.pos.copy()
+    dvec = min_image_diff(pos2[0:1], pos2[1:2], wl.box)[0]
+    pos2[0] = pos2[1] + 1.5 * dvec / np.linalg.norm(dvec)
+    pos2 = oracle.wrap(pos2, wl.box)
+    md.set_bond_table(r_min, 1.3, U, F)
+    md.set_state(pos2, wl.vel); md.build_cells(); md.forces_bond_table()
+    Fn = md.get_forces()[0]
+    Fnr = oracle.bond_table(pos2, wl.box, wl.bonds, r_min, 1.3, U, F)[0]
+    assert np.isnan(Fn[:2]).all() and np.isnan(Fnr[:2]).all() and np.isfinite(Fn[2:]).all()
+    assert force_rel_err(Fn[2:], Fnr[2:]) < 1e-10
+    # argument checks
+    with pytest.raises(B.MDError):
+        md.set_bond_table(1.0, 0.5, U, F)
+    with pytest.raises(B.MDError):
+        md.set_bond_table(0.5, 1.0, U[:1], F[:1])
+    md.set_bond_table(0, 0, None, None)
+    with pytest.raises(B.MDError):
+        md.forces_bond_table()
+    with pytest.raises(B.MDError):
+        md.step(desc, 1)
