@@ -401,6 +401,32 @@ def nvt_half2(vel, force, dt, xi, mass=None):
 
 
 # ------------------------------------------------------------------------------------------------------
+# NVT, second scheme: the explicit reversible Martyna-Tobias-Klein update ("NVT (Nose-Hoover, then
+# MTK)"; ensembles "implement the Velocity-Verlet or the symplectic Martyna-Tobias-Klein update equations";
+# no equations printed -> DESIGN.md R39).  Same equations of motion as above with one thermostat (chain length 1),
+# Q = g kT0 tau^2, integrated by the symmetric Trotter factorisation of Martyna, Tuckerman, Tobias & Klein (1996):
+#   step = T(dt/2)  kick(dt/2)  drift(dt)  [forces]  kick(dt/2)  T(dt/2),
+#   T(dt/2):  G = (2K - g kT0)/Q ; xi += (dt/4) G ; s = exp(-xi dt/2) ; v <- s v ; K <- s^2 K ; eta += xi dt/2 ;
+#             G = (2K - g kT0)/Q ; xi += (dt/4) G
+# (each factor is the exact flow of its part, so the step is time-reversible and second order).  Conserved quantity as
+# above.  kick and drift are vv_half1 / vv_half2.
+# ------------------------------------------------------------------------------------------------------
+def mtk_thermostat_half(vel, dt, kT, tau, xi, eta, mass=None):
+    """T(dt/2) in place on vel; returns (xi, eta)."""
+    m = 1.0 if mass is None else np.asarray(mass, dtype=np.float64)[:, None]
+    g = 3 * vel.shape[0] - 3
+    Q = g * kT * tau * tau
+    K = 0.5 * float(np.sum(m * vel * vel))
+    xi = xi + 0.25 * dt * (2.0 * K - g * kT) / Q
+    s = float(np.exp(-0.5 * dt * xi))
+    vel *= s
+    K = K * s * s
+    eta = eta + 0.5 * dt * xi
+    xi = xi + 0.25 * dt * (2.0 * K - g * kT) / Q
+    return xi, eta
+
+
+# ------------------------------------------------------------------------------------------------------
 # The step loop, in the order of DESIGN.md "The path" (S6a -> S3 -> [S1,S2] -> S4 (+S5) -> S6b).
 # ------------------------------------------------------------------------------------------------------
 class Sim:
@@ -416,7 +442,7 @@ class Sim:
     """
 
     def __init__(self, pos, vel, box, rc, r_buff, what, bonds=None, mass=None, step0=0, nvt=None):
-        self.nvt = nvt                       # None = NVE; dict(kT, tau) = Nose-Hoover (R30)
+        self.nvt = nvt                       # None = NVE; dict(kT, tau) = Nose-Hoover (R30); + scheme="mtk": R39
         self.xi, self.eta = 0.0, 0.0
         self.box = np.ascontiguousarray(np.broadcast_to(np.asarray(box, dtype=np.float64), (3,)))
         self.pos = wrap(pos, self.box)
@@ -459,7 +485,11 @@ class Sim:
         if self.force is None:
             self.compute_forces(dt, self.step)          # DESIGN.md R16: F(t0) before the first half-kick
         for _ in range(n_steps):
-            if self.nvt is None:
+            mtk = self.nvt is not None and self.nvt.get("scheme") == "mtk"
+            if mtk:
+                self.xi, self.eta = mtk_thermostat_half(self.vel, dt, self.nvt["kT"], self.nvt["tau"], self.xi, self.eta,
+                                                        self.mass)
+            if self.nvt is None or mtk:
                 vv_half1(self.pos, self.vel, self.image, self.force, self.box, dt, self.mass)
             else:
                 nvt_half1(self.pos, self.vel, self.image, self.force, self.box, dt, self.xi, self.mass)
@@ -470,10 +500,13 @@ class Sim:
                 self.pos_ref = self.pos.copy()
                 self.rebuild_steps.append(self.step + 1)
             self.compute_forces(dt, self.step + 1)      # DESIGN.md R15: hash counter = step being completed
-            if self.nvt is None:
+            if self.nvt is None or mtk:
                 vv_half2(self.vel, self.force, dt, self.mass)
             else:
                 nvt_half2(self.vel, self.force, dt, self.xi, self.mass)
+            if mtk:
+                self.xi, self.eta = mtk_thermostat_half(self.vel, dt, self.nvt["kT"], self.nvt["tau"], self.xi, self.eta,
+                                                        self.mass)
             self.step += 1
         return self
 
