@@ -266,11 +266,13 @@ def run_ours(args):
     # measured issue rates of the pipes the pair-force kernel runs on (md_debug_peak), before the timed region
     peaks = {k: md.debug_peak(k) for k in ("fp32_fma", "fp64_fma", "int32_mad")} if rank == 0 else {}
     nvt = None
-    if args.nvt:
+    if args.nvt or args.mtk:
         import dataclasses
         kT = float(w.params.get("kT", 1.2 if args.config == 2 else 1.0))
         nvt = dict(kT=kT, tau=0.5)
-        w = dataclasses.replace(w, name=w.name + "-nvt")
+        if args.mtk:                     # the Martyna-Tobias-Klein update (R39) instead of the R30 scheme
+            nvt["scheme"] = "mtk"
+        w = dataclasses.replace(w, name=w.name + ("-nvt-mtk" if args.mtk else "-nvt"))
     angles = None
     if args.angles and w.kind == "polymer":
         # harmonic angles along the chains of the polymer melt (k = 5, theta0 = 2.0 rad); named in the
@@ -488,6 +490,7 @@ def main():
     ap.add_argument("--angles", action="store_true", help="config 4 with harmonic angles along the chains (SURVEY 8(f) row 3)")
     ap.add_argument("--auto-rbuff", action="store_true", dest="auto_rbuff",
                     help="md_tune_rbuff: let the library choose the skin (tuning run; not a reported configuration)")
+    ap.add_argument("--mtk", action="store_true", help="NVT with the Martyna-Tobias-Klein update (SURVEY 8(f) row 1, R39)")
     ap.add_argument("--nvt", action="store_true",
                     help="Nose-Hoover NVT (MD_F_NVT, kT = the workload's temperature, tau = 0.5) instead of NVE: "
                          "SURVEY 8(f) row 1; named in the workload, not a BASELINE configuration")

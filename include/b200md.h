@@ -71,6 +71,7 @@ typedef enum {
 #define MD_F_ANGLES 32u /* harmonic angles (md_set_angles; angle_k, angle_theta0) */
 #define MD_F_DIHEDRALS 64u /* periodic dihedrals (md_set_dihedrals; dihedral_k, dihedral_sign, dihedral_n) */
 #define MD_F_LANGEVIN 128u /* Langevin thermostat as a one-body force (langevin_gamma, langevin_kT, langevin_seed; R36) */
+#define MD_F_MTK 256u /* md_step integrates NVT with the Martyna-Tobias-Klein update (nvt_kT, nvt_tau; R39) instead of NVE */
 
 /* pair potentials of md_forces_pair / MD_F_PAIR (PAPER.md:63 lists them, R31); parameters p[0..2] */
 enum { MD_PAIR_LJ = 0,       /* U = 4 p0 ((p1/r)^12 - (p1/r)^6)                        p0 = epsilon, p1 = sigma     */
@@ -356,6 +357,15 @@ int md_set_launch(md_ctx *ctx, int kernel, int block, int w);
    half = 2: v <- v + (dt/2)(F/m - xi v).
    The thermostat variables live in the context: md_set_state resets them to 0. */
 int md_integrate_nvt(md_ctx *ctx, double dt, int half, double kT, double tau);
+/* Martyna-Tobias-Klein update for NVT (R39; "the symplectic Martyna-Tobias-Klein update equations"; SURVEY.md
+   8(f) row 1): the equations of motion of md_integrate_nvt with one thermostat, Q = (3N - 3) kT tau^2, as the symmetric
+   factorisation  step = T(dt/2) half1 [forces] half2 T(dt/2)  with the NVE halves of md_integrate_nve and
+     T(dt/2): xi += (dt/4)(2K - (3N-3) kT)/Q; s = exp(-xi dt/2); v <- s v; K <- s^2 K; eta += xi dt/2; xi += (dt/4)(2K - (3N-3) kT)/Q.
+   md_mtk_thermostat_half applies one T(dt/2) on the device (K reduction in md_thermo's fixed order, one-thread update of
+   xi and eta, one scaling pass); xi and eta are the ones of md_set_thermostat / md_get_thermostat.  md_step with MD_F_MTK
+   (excludes MD_F_NVT and MD_F_LANGEVIN) runs the whole step and merges the trailing factor of a step with the leading one
+   of the next into one reduction and one scaling pass; every scheduler gives identical results.  Time-reversible. */
+int md_mtk_thermostat_half(md_ctx *ctx, double dt, double kT, double tau);
 int md_set_thermostat(md_ctx *ctx, double xi, double eta);
 int md_get_thermostat(md_ctx *ctx, double *xi, double *eta); /* HOST pointers; synchronises */
 

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "csrc", "libb200md.so")
 
 MD_FP64, MD_MIXED = 0, 1
 MD_ORDER_LEX, MD_ORDER_MORTON, MD_ORDER_HILBERT = 0, 1, 2
-MD_F_LJ, MD_F_DPD, MD_F_BONDS, MD_F_NVT, MD_F_PAIR, MD_F_ANGLES, MD_F_DIHEDRALS, MD_F_LANGEVIN = 1, 2, 4, 8, 16, 32, 64, 128
+MD_F_LJ, MD_F_DPD, MD_F_BONDS, MD_F_NVT, MD_F_PAIR, MD_F_ANGLES, MD_F_DIHEDRALS, MD_F_LANGEVIN, MD_F_MTK = 1, 2, 4, 8, 16, 32, 64, 128, 256
 PAIR_KINDS = {"lj": 0, "yukawa": 1, "gaussian": 2, "morse": 3, "table": 4}
 BOND_KINDS = {"harmonic": 0, "fene": 1, "table": 2}
 MD_SCHED_SYNC, MD_SCHED_SPECULATIVE, MD_SCHED_BATCH = 0, 1, 2
@@ -32,7 +32,7 @@ EXPORTS = ["md_create", "md_workspace_bytes", "md_set_workspace", "md_configure"
            "md_set_dihedrals", "md_forces_dihedrals", "md_forces_langevin", "md_pressure",
            "md_integrate_nve",
            "md_needs_rebuild", "md_step", "md_tune", "md_tune_rbuff", "md_set_option", "md_set_launch", "md_get_stats", "md_set_profiling",
-           "md_debug_philox", "md_debug_peak", "md_struct_size", "md_thermo", "md_integrate_nvt", "md_set_thermostat", "md_get_thermostat",
+           "md_debug_philox", "md_debug_peak", "md_struct_size", "md_thermo", "md_integrate_nvt", "md_set_thermostat", "md_get_thermostat", "md_mtk_thermostat_half",
            "md_kinetic_noalloc", "md_noalloc_last_error"]
 
 
@@ -130,6 +130,7 @@ def load():
         "md_integrate_nvt": [vp, C.c_double, i32, C.c_double, C.c_double],
         "md_set_thermostat": [vp, C.c_double, C.c_double],
         "md_get_thermostat": [vp, vp, vp],
+        "md_mtk_thermostat_half": [vp, dbl, dbl, dbl],
         "md_kinetic_noalloc": [vp, vp, u64, vp, vp],
     }
     for name, args in sig.items():
@@ -214,7 +215,7 @@ def step_desc(kind: str, dt: float, params: dict, nvt: dict = None) -> md_step_d
         d.flags |= MD_F_LANGEVIN
         d.langevin_gamma, d.langevin_kT, d.langevin_seed = float(q["gamma"]), float(q["kT"]), int(q["seed"])
     if nvt is not None:
-        d.flags |= MD_F_NVT
+        d.flags |= MD_F_MTK if nvt.get("scheme") == "mtk" else MD_F_NVT
         d.nvt_kT, d.nvt_tau = float(nvt["kT"]), float(nvt["tau"])
     return d
 
@@ -402,6 +403,9 @@ class MD:
 
     def integrate_nve(self, dt, half):
         self._chk(self.L.md_integrate_nve(self.h, float(dt), int(half)), "md_integrate_nve")
+
+    def mtk_thermostat_half(self, dt, kT, tau):
+        self._chk(self.L.md_mtk_thermostat_half(self.h, float(dt), float(kT), float(tau)), "md_mtk_thermostat_half")
 
     def integrate_nvt(self, dt, half, kT, tau):
         self._chk(self.L.md_integrate_nvt(self.h, float(dt), int(half), float(kT), float(tau)), "md_integrate_nvt")

@@ -1137,6 +1137,15 @@ extern "C" int md_integrate_nvt(md_ctx *c, double dt, int half, double kT, doubl
     return MD_EINVAL;
 }
 
+extern "C" int md_mtk_thermostat_half(md_ctx *c, double dt, double kT, double tau)
+{
+    if (!c) return MD_EINVAL;
+    if (!c->have_state) { c->err = "md_mtk_thermostat_half: md_set_state first"; return MD_ESTATE; }
+    if (!(dt > 0.0) || !(kT > 0.0) || !(tau > 0.0)) { c->err = "md_mtk_thermostat_half: dt, kT and tau must be positive"; return MD_EINVAL; }
+    ProfScope ps(c, MD_K_INTEGRATE);
+    return launch_mtk_thermostat(c, dt, kT, tau, 1);
+}
+
 extern "C" int md_set_thermostat(md_ctx *c, double xi, double eta)
 {
     if (!c) return MD_EINVAL;
@@ -1242,12 +1251,13 @@ static int rebuild(md_ctx *c)
 // (bit-identical results).  The batch length follows the predicted distance to the next rebuild (largest displacement seen
 // and its growth per step): a wrong prediction costs empty launches, never correctness.  PAPER.md:122 overlaps the check
 // with a speculative force evaluation; PAPER.md:120, :163 are the launch overheads this removes at small N.
-static int md_step_batch(md_ctx *c, const md_step_desc *w, uint64_t n_steps, bool nvt)
+static int md_step_batch(md_ctx *c, const md_step_desc *w, uint64_t n_steps, bool nvt, bool mtk)
 {
     // half 1 of the first step, not gated; its flag is read before anything else is enqueued
     {
         ProfScope ps(c, MD_K_INTEGRATE);
         c->gate_s = c->gate_set = c->gate_nvt = 0;
+        if (mtk) MD_TRY(launch_mtk_thermostat(c, w->dt, w->nvt_kT, w->nvt_tau, 1));  // R39: leading T(dt/2) of the first step
         MD_TRY(launch_half1(c, w->dt, false, nvt));
         if (nvt) MD_TRY(launch_nvt_thermostat(c, w->dt, w->nvt_kT, w->nvt_tau));
     }
@@ -1279,12 +1289,21 @@ static int md_step_batch(md_ctx *c, const md_step_desc *w, uint64_t n_steps, boo
             c->gate_s = (unsigned int)j;
             MD_TRY(eval_forces(c, w, c->step + j, false));  // R15: hash counter = index of the step being completed
             ProfScope ps(c, MD_K_INTEGRATE);
-            if (done + j < n_steps) {
+            if (done + j < n_steps && mtk) {
+                // R39: half 2 of step j, its trailing T(dt/2) and the leading one of step j + 1 (one reduction: the second
+                // factor's K is s^2 K), all part of step j; then the plain half 1 of step j + 1
+                MD_TRY(launch_half2(c, w->dt, false));
+                MD_TRY(launch_mtk_thermostat(c, w->dt, w->nvt_kT, w->nvt_tau, 2));
+                c->gate_s = c->gate_set = (unsigned int)(j + 1);
+                MD_TRY(launch_half1(c, w->dt, false, false));
+                c->gate_s = (unsigned int)j;
+            } else if (done + j < n_steps) {
                 c->gate_set = c->gate_nvt = (unsigned int)(j + 1);
                 MD_TRY(launch_half1(c, w->dt, true, nvt));   // half 2 of step j + half 1 of step j + 1
                 if (nvt) { c->gate_nvt = (unsigned int)j; MD_TRY(launch_nvt_thermostat(c, w->dt, w->nvt_kT, w->nvt_tau)); }
             } else {
                 MD_TRY(launch_half2(c, w->dt, nvt));
+                if (mtk) MD_TRY(launch_mtk_thermostat(c, w->dt, w->nvt_kT, w->nvt_tau, 1));
             }
         }
         c->gate_s = c->gate_set = c->gate_nvt = 0;
@@ -1318,8 +1337,9 @@ extern "C" int md_step(md_ctx *c, const md_step_desc *w, uint64_t n_steps)
     if (!c->have_state) { c->err = "md_step: md_set_state first"; return MD_ESTATE; }
     if (!(w->dt > 0.0)) { c->err = "md_step: dt must be positive"; return MD_EINVAL; }
     if (n_steps == 0) return MD_OK;
-    const bool nvt = (w->flags & MD_F_NVT) != 0;
-    if (nvt && (!(w->nvt_kT > 0.0) || !(w->nvt_tau > 0.0))) { c->err = "md_step: nvt_kT and nvt_tau must be positive"; return MD_EINVAL; }
+    const bool nvt = (w->flags & MD_F_NVT) != 0, mtk = (w->flags & MD_F_MTK) != 0;
+    if ((nvt || mtk) && (!(w->nvt_kT > 0.0) || !(w->nvt_tau > 0.0))) { c->err = "md_step: nvt_kT and nvt_tau must be positive"; return MD_EINVAL; }
+    if (mtk && (w->flags & (MD_F_NVT | MD_F_LANGEVIN))) { c->err = "md_step: MD_F_MTK excludes MD_F_NVT and MD_F_LANGEVIN"; return MD_EINVAL; }
     c->force_hint = w->flags;
     if (w->flags & MD_F_LJ) {
         // the near sections of a mixed-precision tile list are sized for sigma (R25): a list built for a smaller one is rebuilt
@@ -1330,11 +1350,12 @@ extern "C" int md_step(md_ctx *c, const md_step_desc *w, uint64_t n_steps)
     }
     if (!c->nlist_valid) MD_TRY(rebuild(c));
     if (!c->force_valid) MD_TRY(eval_forces(c, w, c->step, false));  // R16: F(t0) before the first half-kick
-    if (c->sched == MD_SCHED_BATCH) return md_step_batch(c, w, n_steps, nvt);
+    if (c->sched == MD_SCHED_BATCH) return md_step_batch(c, w, n_steps, nvt, mtk);
     if (!c->ev_flags) MD_CUDA_CHECK(c, cudaEventCreateWithFlags(&c->ev_flags, cudaEventDisableTiming));
     for (uint64_t s = 0; s < n_steps; ++s) {
         if (s == 0) {
             ProfScope ps(c, MD_K_INTEGRATE);
+            if (mtk) MD_TRY(launch_mtk_thermostat(c, w->dt, w->nvt_kT, w->nvt_tau, 1));
             MD_TRY(launch_half1(c, w->dt, false, nvt));
             if (nvt) MD_TRY(launch_nvt_thermostat(c, w->dt, w->nvt_kT, w->nvt_tau));
         }
@@ -1369,11 +1390,16 @@ extern "C" int md_step(md_ctx *c, const md_step_desc *w, uint64_t n_steps)
         }
         {
             ProfScope ps(c, MD_K_INTEGRATE);
-            if (s + 1 < n_steps) {
+            if (s + 1 < n_steps && mtk) {
+                MD_TRY(launch_half2(c, w->dt, false));
+                MD_TRY(launch_mtk_thermostat(c, w->dt, w->nvt_kT, w->nvt_tau, 2));  // trailing T of this step + leading T of the next
+                MD_TRY(launch_half1(c, w->dt, false, false));
+            } else if (s + 1 < n_steps) {
                 MD_TRY(launch_half1(c, w->dt, true, nvt));  // half 2 of this step + half 1 of the next
                 if (nvt) MD_TRY(launch_nvt_thermostat(c, w->dt, w->nvt_kT, w->nvt_tau));
             } else {
                 MD_TRY(launch_half2(c, w->dt, nvt));
+                if (mtk) MD_TRY(launch_mtk_thermostat(c, w->dt, w->nvt_kT, w->nvt_tau, 1));
             }
         }
         c->step++;

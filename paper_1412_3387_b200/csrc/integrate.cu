@@ -223,6 +223,53 @@ static int thermo_reduce(md_ctx *c, double **res_out, Gate gate)
     return MD_OK;
 }
 
+// Martyna-Tobias-Klein thermostat factor T(dt/2) (R39), `halves` of them in a row (2: the trailing factor of one step and
+// the leading factor of the next): xi += (dt/4) G; s = exp(-xi dt/2); K <- s^2 K; eta += xi dt/2; xi += (dt/4) G', with
+// G = (2K - g kT)/Q, Q = g kT tau^2.  K comes from the reduction kernels above; the product of the scale factors goes to
+// nvt[2] and k_mtk_scale applies it to every velocity.
+__global__ void k_mtk_update(const double *__restrict__ sums, double *__restrict__ nvt, double dt, double kT, double tau,
+                             double dof, int halves, Gate gate)
+{
+    if (md_gate_closed(gate)) return;
+    double K = sums[0], xi = nvt[0], eta = nvt[1], s_tot = 1.0;
+    const double Q = dof * kT * tau * tau;
+    for (int h = 0; h < halves; ++h) {
+        xi = xi + 0.25 * dt * (2.0 * K - dof * kT) / Q;
+        const double s = exp(-0.5 * dt * xi);
+        K = K * s * s;
+        eta = eta + 0.5 * dt * xi;
+        xi = xi + 0.25 * dt * (2.0 * K - dof * kT) / Q;
+        s_tot *= s;
+    }
+    nvt[0] = xi;
+    nvt[1] = eta;
+    nvt[2] = s_tot;
+}
+
+__global__ void k_mtk_scale(double4 *__restrict__ vel, uint32_t N, const double *__restrict__ nvt, Gate gate)
+{
+    if (md_gate_closed(gate)) return;
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double s = nvt[2];
+    double4 v = vel[i];
+    v.x *= s; v.y *= s; v.z *= s;
+    vel[i] = v;
+}
+
+int launch_mtk_thermostat(md_ctx *c, double dt, double kT, double tau, int halves)
+{
+    const Gate tg = md_gate(c);  // part of the step whose index is c->gate_s (MD_SCHED_BATCH), open otherwise
+    double *res = nullptr;
+    MD_TRY(thermo_reduce(c, &res, tg));
+    k_mtk_update<<<1, 1, 0, c->stream>>>(res, c->nvt_state, dt, kT, tau, 3.0 * (double)c->N - 3.0, halves, tg);
+    MD_LAUNCH_CHECK(c);
+    const LaunchCfg &cf = c->cfg[MD_K_INTEGRATE];
+    k_mtk_scale<<<md_grid(c->N, cf.block), cf.block, 0, c->stream>>>(c->vel, (uint32_t)c->N, c->nvt_state, tg);
+    MD_LAUNCH_CHECK(c);
+    return MD_OK;
+}
+
 int launch_nvt_thermostat(md_ctx *c, double dt, double kT, double tau)
 {
     // part of the half 1 it follows: same gate as that launch (c->gate_nvt is set by the caller)

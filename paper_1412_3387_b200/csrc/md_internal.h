@@ -259,6 +259,7 @@ int launch_virial(md_ctx *c, const md_step_desc *w, uint64_t step, double *out6_
 int launch_half1(md_ctx *c, double dt, bool fused, bool nvt = false);
 int launch_half2(md_ctx *c, double dt, bool nvt = false);
 int launch_nvt_thermostat(md_ctx *c, double dt, double kT, double tau);  // K' reduction + xi, eta update, all on the device
+int launch_mtk_thermostat(md_ctx *c, double dt, double kT, double tau, int halves);  // R39: `halves` x T(dt/2): K reduction, xi / eta update, velocity scaling
 int launch_thermo(md_ctx *c, double *out6_host);  // kinetic, potential, px, py, pz (device reduction, then D2H + sync)
 int launch_export_pairs_count(md_ctx *c, uint32_t *cnt);
 int launch_export_pairs_fill(md_ctx *c, const uint64_t *off, uint32_t *pairs);

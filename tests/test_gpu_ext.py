@@ -389,3 +389,81 @@ def test_tabulated_bonds_forces_energy_virial_and_step():
         md.forces_bond_table()
     with pytest.raises(B.MDError):
         md.step(desc, 1)
+
+
+def test_mtk_nvt_single_factors_steps_and_reversal():
+    """Martyna-Tobias-Klein NVT (R39): md_mtk_thermostat_half + the NVE halves against the oracle's factors, md_step with
+    MD_F_MTK against oracle.Sim over 40 steps with rebuilds, every scheduler bit-identical, the NVE limit, and the time
+    reversal the factorisation guarantees, on the device."""
+    wl = inputs.lj_fcc(6, rc=2.5, r_buff=0.4, kT=0.7, jitter=0.08, pos_seed=3, vel_seed=4)       # N = 864
+    kT0, tau, dt = 1.2, 0.4, wl.dt
+    nvt = dict(kT=kT0, tau=tau, scheme="mtk")
+    # --- one step, factor by factor
+    md = B.from_workload(wl)
+    md.build_nlist(); md.forces_lj()
+    md.set_thermostat(0.05, -0.01)
+    sim = oracle.Sim(wl.pos, wl.vel, wl.box, wl.rc, wl.r_buff, {"lj": wl.params}, nvt=nvt)
+    sim.xi, sim.eta = 0.05, -0.01
+    sim.compute_forces(dt, 0)
+    md.mtk_thermostat_half(dt, kT0, tau)
+    sim.xi, sim.eta = oracle.mtk_thermostat_half(sim.vel, dt, kT0, tau, sim.xi, sim.eta)
+    _, vel, _ = md.get_state()
+    gxi, geta = md.get_thermostat()
+    assert np.abs(vel - sim.vel).max() < 1e-13 and abs(gxi - sim.xi) < 1e-13 and abs(geta - sim.eta) < 1e-14
+    assert abs(sim.xi - 0.05) > 1e-4                                  # the factor did something
+    md.integrate_nve(dt, 1)
+    oracle.vv_half1(sim.pos, sim.vel, sim.image, sim.force, sim.box, dt)
+    if md.needs_rebuild():
+        md.build_cells()
+    md.build_nlist(); md.forces_lj()
+    sim.compute_forces(dt, 1)
+    md.integrate_nve(dt, 2)
+    oracle.vv_half2(sim.vel, sim.force, dt)
+    md.mtk_thermostat_half(dt, kT0, tau)
+    sim.xi, sim.eta = oracle.mtk_thermostat_half(sim.vel, dt, kT0, tau, sim.xi, sim.eta)
+    pos, vel, img = md.get_state()
+    assert np.abs(min_image_diff(pos, sim.pos, wl.box)).max() < 1e-12 and np.array_equal(img, sim.image)
+    assert np.abs(vel - sim.vel).max() < 1e-11
+    gxi, geta = md.get_thermostat()
+    assert abs(gxi - sim.xi) < 1e-12 and abs(geta - sim.eta) < 1e-13
+    # --- md_step over 40 steps with rebuilds, the three schedulers
+    desc = B.step_desc("lj", dt, wl.params, nvt=nvt)
+    assert desc.flags == B.MD_F_LJ | B.MD_F_MTK
+    sim2 = oracle.Sim(wl.pos, wl.vel, wl.box, wl.rc, wl.r_buff, {"lj": wl.params}, nvt=nvt).run(40, dt)
+    outs = []
+    for sched in (B.MD_SCHED_BATCH, B.MD_SCHED_SPECULATIVE, B.MD_SCHED_SYNC):
+        m = B.from_workload(wl, sched=sched)
+        m.step(desc, 17); m.step(desc, 23)                            # two calls: no merged factor across the boundary
+        outs.append((m.get_state(), m.get_thermostat(), m.stats()))
+    (pos, vel, _), (gxi, geta), st = outs[0]
+    assert np.abs(min_image_diff(pos, sim2.pos, wl.box)).max() < 1e-9      # Lyapunov growth from 1e-16 over 40 steps
+    assert np.abs(vel - sim2.vel).max() < 1e-8
+    assert abs(gxi - sim2.xi) < 1e-10 and abs(geta - sim2.eta) < 1e-10 and sim2.xi < 0.0
+    assert st["rebuilds"] >= 2 and st["dangerous_builds"] == 0
+    for o in outs[1:]:
+        assert np.array_equal(o[0][0], pos) and np.array_equal(o[0][1], vel) and o[1] == (gxi, geta)
+    # --- thermostat off (tau huge): NVE
+    a = B.from_workload(wl); b = B.from_workload(wl)
+    a.step(B.step_desc("lj", dt, wl.params), 10)
+    b.step(B.step_desc("lj", dt, wl.params, nvt=dict(kT=kT0, tau=1e150, scheme="mtk")), 10)
+    pa, va, _ = a.get_state(); pb, vb, _ = b.get_state()
+    assert np.abs(min_image_diff(pa, pb, wl.box)).max() < 1e-13 and np.abs(va - vb).max() < 1e-13
+    # --- time reversal on the device: 30 steps forward, v and xi negated, 30 steps: back at the start
+    r = B.from_workload(wl)
+    r.step(desc, 30)
+    p1, v1, _ = r.get_state()
+    xi1, eta1 = r.get_thermostat()
+    assert np.abs(min_image_diff(p1, wl.pos, wl.box)).max() > 0.05
+    r.set_state(p1, -v1, None, 30)
+    r.set_thermostat(-xi1, eta1)
+    r.step(desc, 30)
+    p2, v2, _ = r.get_state()
+    xi2, eta2 = r.get_thermostat()
+    assert np.abs(min_image_diff(p2, wl.pos, wl.box)).max() < 1e-10 and np.abs(v2 + wl.vel).max() < 1e-10
+    assert abs(xi2) < 1e-11 and abs(eta2) < 1e-11
+    # --- argument checks
+    with pytest.raises(B.MDError):
+        r.mtk_thermostat_half(dt, -1.0, tau)
+    bad = B.step_desc("lj", dt, dict(wl.params, langevin=dict(gamma=1.0, kT=1.0, seed=1)), nvt=nvt)
+    with pytest.raises(B.MDError):
+        r.step(bad, 1)
