@@ -20,6 +20,7 @@ __global__ void __launch_bounds__(MD_HALF1_MAX_BLOCK, 6) k_half1(double4 *__rest
     if (md_gate_closed(gate)) return;
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     float d2f = 0.f;
+    unsigned fire = 0u;  // bit 0: moved more than r_buff / 2 since the binning; bit 1: more than r_buff (a pair may have been missed)
     const double xi = NVT ? nvt[0] : 0.0;
     const double denom = __dadd_rn(1.0, __dmul_rn(half_dt, xi));
     if (i < g.N) {
@@ -53,12 +54,18 @@ __global__ void __launch_bounds__(MD_HALF1_MAX_BLOCK, 6) k_half1(double4 *__rest
         pos[i] = make_double4(x[0], x[1], x[2], p.w);
         if (MD_STAGE_FROM_REL) rel[i] = md_rel_record(x[0], x[1], x[2], cell_lin[i], g);  // meaningful once binned
         vel[i] = make_double4(u[0], u[1], u[2], m);
-        if (d2 > thr2) {
-            flags->rebuild = 1;  // benign race: every writer stores the same value
-            if (at_val) flags->rebuild_at = at_val;
-            if (d2 > danger2) flags->dangerous = 1;
-        }
+        fire = d2 > thr2 ? (d2 > danger2 ? 3u : 1u) : 0u;
         d2f = __double2float_ru(d2);
+    }
+    // the criterion of PAPER.md:79 into the device flags.  In a DPD fluid thousands of particles cross the threshold in the
+    // same step; one store per crossing particle to the same address serialises in L2 (measured: 38 -> 120 us for this
+    // kernel at 10^6 particles), so a warp stores once, and only while the flag is not yet up (benign race: every writer
+    // stores the same value, and nobody reads the flags before the kernel has finished)
+    const unsigned wfire = __reduce_or_sync(0xffffffffu, fire);
+    if ((threadIdx.x & 31u) == 0 && wfire) {
+        if (*(volatile int *)&flags->rebuild == 0) flags->rebuild = 1;
+        if (at_val && *(volatile unsigned int *)&flags->rebuild_at == 0u) flags->rebuild_at = at_val;
+        if ((wfire & 2u) && *(volatile int *)&flags->dangerous == 0) flags->dangerous = 1;
     }
     const unsigned wmax = __reduce_max_sync(0xffffffffu, __float_as_uint(d2f));  // non-negative floats order as uints
     if ((threadIdx.x & 31u) == 0 && wmax > flags->max_d2[slot]) atomicMax(&flags->max_d2[slot], wmax);
