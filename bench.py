@@ -333,6 +333,9 @@ def run_ours(args):
     h_vel = torch.empty((w.N, 3), dtype=torch.float64).pin_memory()
     md.get_state(h_pos, h_vel, None)
     torch.cuda.synchronize()
+    # ... of every `ev_stride`-th launch: two events per launch cost a 30 us step (config 1) a third of its time
+    ev_stride = 16 if args.steps >= 64 else 1
+    md.set_option(B.MD_OPT_PROFILE_STRIDE, ev_stride)
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
@@ -340,7 +343,7 @@ def run_ours(args):
     reps = []
     for rep in range(1 if args.reps < 2 else args.reps):
         ra = md.stats()
-        md.set_profiling(2)        # CUDA events around the pair-force stage only (the roofline kernel): 2 events per step
+        md.set_profiling(2)        # CUDA events around the pair-force stage only (the roofline kernel) ...
         e0 = torch.cuda.Event(enable_timing=True)
         e1 = torch.cuda.Event(enable_timing=True)
         barrier()
@@ -362,6 +365,7 @@ def run_ours(args):
         clocks["note"] = "timed region shorter than 3 sample periods: sampling continued over %d more steps of the same run" % extra_steps
     rep_ms = [r[0] for r in reps]
     # stage shares: a short untimed continuation with every stage bracketed by events (about 8 events per step)
+    md.set_option(B.MD_OPT_PROFILE_STRIDE, 1)
     md.set_profiling(1)
     n_share = max(20, min(200, args.steps // 4))
     with torch.cuda.stream(stream):
@@ -451,6 +455,8 @@ def run_ours(args):
                          "traffic": traffic, "traffic_note": traffic_note,
                          # achieved/frac use the ALGORITHMIC bytes of SURVEY 8(d) (4-byte indices: 4 n + 56, DPD 4 n + 84 per
                          # particle); the list is stored as 16-bit entries, so the measured DRAM traffic is lower:
+                         "kernel_timing": "CUDA events on the library's stream around every %s pair-force launch of the timed region (%d launches)"
+                                          % ("one" if ev_stride == 1 else "%dth" % ev_stride, st1["stage_launches"][fk]),
                          "bytes_model": "SURVEY 8(d) staged minimum of the pair-force kernel, 4-byte indices",
                          "traffic_gbs": (traffic / (f_ms * 1e-3) / 1e9) if (traffic and f_ms > 0) else None,
                          "traffic_frac": (traffic / (f_ms * 1e-3) / 1e9 / peak) if (traffic and f_ms > 0) else None,

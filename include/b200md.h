@@ -344,6 +344,8 @@ int md_tune_rbuff(md_ctx *ctx, const md_step_desc *what, const double *candidate
 #define MD_OPT_TILE_BRICK 1
 #define MD_OPT_ACC_BLOCK 2
 #define MD_OPT_RETUNE_PERIOD 4 /* rebuilds between periodic local re-scans of the tuner inside md_step; 0 (default) = never */
+#define MD_OPT_PROFILE_STRIDE 8 /* md_set_profiling(ctx, 2) brackets every S-th pair-force launch with events (default 1 = every one);
+                                  stage_ms / stage_launches then hold the sampled launches only */
 int md_set_option(md_ctx *ctx, int option, int64_t value);
 
 /* Fix launch parameters by hand (block multiple of 32 in [32,1024]; w power of two <= 32); kernel = MD_K_*. */

@@ -20,7 +20,7 @@ MD_F_LJ, MD_F_DPD, MD_F_BONDS, MD_F_NVT, MD_F_PAIR, MD_F_ANGLES, MD_F_DIHEDRALS,
 PAIR_KINDS = {"lj": 0, "yukawa": 1, "gaussian": 2, "morse": 3, "table": 4}
 BOND_KINDS = {"harmonic": 0, "fene": 1, "table": 2}
 MD_SCHED_SYNC, MD_SCHED_SPECULATIVE, MD_SCHED_BATCH = 0, 1, 2
-MD_OPT_TILE_BRICK, MD_OPT_ACC_BLOCK, MD_OPT_RETUNE_PERIOD = 1, 2, 4
+MD_OPT_TILE_BRICK, MD_OPT_ACC_BLOCK, MD_OPT_RETUNE_PERIOD, MD_OPT_PROFILE_STRIDE = 1, 2, 4, 8
 MD_N_KERNELS = 8
 MD_K_NLIST, MD_K_LJ, MD_K_DPD, MD_K_BONDS, MD_K_INTEGRATE, MD_K_CELLS = 0, 1, 2, 3, 4, 5
 KERNEL_NAMES = {MD_K_NLIST: "nlist", MD_K_LJ: "lj", MD_K_DPD: "dpd", MD_K_BONDS: "bonds",

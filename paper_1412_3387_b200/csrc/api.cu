@@ -113,7 +113,12 @@ static cudaEvent_t prof_event(md_ctx *c)
 ProfScope::ProfScope(md_ctx *ctx, int kernel) : c(ctx), k(kernel)
 {
     if (!c->profiling) return;
-    if (c->profiling == 2 && kernel != MD_K_LJ && kernel != MD_K_DPD) return;
+    if (c->profiling == 2) {
+        if (kernel != MD_K_LJ && kernel != MD_K_DPD) return;
+        // MD_OPT_PROFILE_STRIDE: every S-th pair-force launch is bracketed (the events of every launch cost a 30 us step of
+        // 4,000 particles a third of its time)
+        if (c->prof_stride > 1 && (c->prof_count++ % c->prof_stride) != 0) return;
+    }
     e0 = prof_event(c);
     e1 = prof_event(c);
     cudaEventRecord(e0, c->stream);
@@ -1665,6 +1670,11 @@ extern "C" int md_set_option(md_ctx *c, int option, int64_t value)
     case MD_OPT_ACC_BLOCK:
         if (value != 1 && value != 8) { c->err = "md_set_option: accumulation block must be 1 or 8"; return MD_EINVAL; }
         c->acc_block = (int)value;
+        return MD_OK;
+    case MD_OPT_PROFILE_STRIDE:
+        if (value < 1) { c->err = "md_set_option: profile stride must be >= 1"; return MD_EINVAL; }
+        c->prof_stride = (uint64_t)value;
+        c->prof_count = 0;
         return MD_OK;
     case MD_OPT_RETUNE_PERIOD:
         if (value < 0) { c->err = "md_set_option: re-tune period must be >= 0"; return MD_EINVAL; }

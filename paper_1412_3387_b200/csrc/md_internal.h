@@ -208,6 +208,7 @@ struct md_ctx {
 
     // per-stage event timing (md_set_profiling)
     int profiling = 0;  // 0 off, 1 every stage, 2 pair-force stages only (md_set_profiling)
+    uint64_t prof_stride = 1, prof_count = 0;  // MD_OPT_PROFILE_STRIDE: mode 2 brackets every prof_stride-th pair-force launch
     std::vector<cudaEvent_t> ev_pool;
     struct Pending { int k; cudaEvent_t e0, e1; };
     std::vector<Pending> ev_pending;
