@@ -274,7 +274,7 @@ def run_ours(args):
             nvt["scheme"] = "mtk"
         w = dataclasses.replace(w, name=w.name + ("-nvt-mtk" if args.mtk else "-nvt"))
     angles = None
-    if args.angles and w.kind == "polymer":
+    if (args.angles or args.dihedrals) and w.kind == "polymer":
         # harmonic angles along the chains of the polymer melt (k = 5, theta0 = 2.0 rad); named in the
         # workload, not a BASELINE configuration
         import dataclasses
@@ -282,7 +282,11 @@ def run_ours(args):
         nc = w.N // L
         idx = (np.arange(nc, dtype=np.uint32)[:, None] * L + np.arange(L - 2, dtype=np.uint32)[None, :]).reshape(-1)
         angles = np.stack([idx, idx + 1, idx + 2], axis=1).astype(np.uint32)
-        w = dataclasses.replace(w, name=w.name + "-angles", params=dict(w.params, angle_k=5.0, angle_theta0=2.0))
+        # with dihedrals the angles are stiff (k = 50): the dihedral force grows as 1 / sin of the bond angles, and chains
+        # that may straighten (k = 5) throw particles across the skin in one step (dangerous builds)
+        ka = 50.0 if args.dihedrals else 5.0
+        w = dataclasses.replace(w, name=w.name + ("-angles%g" % ka if args.dihedrals else "-angles"),
+                                params=dict(w.params, angle_k=ka, angle_theta0=2.0))
     dihedrals = None
     if args.dihedrals and w.kind == "polymer":
         # periodic dihedrals along the chains, U = k/2 (1 + cos phi), k = 2 (R35); named in the workload
@@ -492,7 +496,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--r-buff", type=float, default=None, dest="r_buff",
                     help="override the configured skin r_buff = 0.4 (tuning sweep; not a reported configuration)")
-    ap.add_argument("--dihedrals", action="store_true", help="config 4 with periodic dihedrals along the chains (SURVEY 8(f) row 3)")
+    ap.add_argument("--dihedrals", action="store_true", help="config 4 with periodic dihedrals and stiff harmonic angles (k = 50) along the chains (SURVEY 8(f) row 3)")
     ap.add_argument("--angles", action="store_true", help="config 4 with harmonic angles along the chains (SURVEY 8(f) row 3)")
     ap.add_argument("--auto-rbuff", action="store_true", dest="auto_rbuff",
                     help="md_tune_rbuff: let the library choose the skin (tuning run; not a reported configuration)")
