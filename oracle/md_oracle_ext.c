@@ -16,13 +16,14 @@
  *                      finite-difference box rescale; symmetric tensor; DPD equation of state (weak, statistical)
  *   orc_forces_fene    closed form, gradient, divergence at r -> r0, Newton
  *   orc_virial_bonds   two-body closed form, -3 V dU/dV
- *   orc_forces_angles  zero force at theta0, closed form for a right angle, gradient, zero net force and torque
+ *   orc_forces_angles  zero force at theta0, closed form for a right angle, gradient, zero net force and torque; collinear
+ *                      triplets (theta = 0, pi) skipped, 1e-6 off the line finite and on the closed form
  *   orc_dihedral_angle hand-made quadruplets (cis 0, trans pi, +-pi/2 with the sign convention), quadruplets built from
  *                      internal coordinates (the angle put in comes back), invariance under rigid motion and the
  *                      periodic wrap
  *   orc_forces_dihedrals  energy k/2 (1 + s cos(n phi)) on built quadruplets for s = +-1, n = 1, 2, 3; F = -dU/dx by
  *                      central differences on all 12 coordinates; zero net force and torque; virial against
- *                      sum x_p (x) F_p; quarter-energy bookkeeping
+ *                      sum x_p (x) F_p; quarter-energy bookkeeping; quadruplets with three collinear particles skipped
  *   orc_langevin_u     the words of the KAT-pinned Philox for three (tag, step, seed) triples mapped by hand; range, mean,
  *                      variance 1/3, independence of components, steps and tags; not DPD's stream
  *   orc_forces_langevin  kT = 0 (pure drag), v = 0 (pure noise), gamma = 0 (off), component variance 2 gamma kT / dt;

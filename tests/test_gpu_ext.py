@@ -467,3 +467,39 @@ def test_mtk_nvt_single_factors_steps_and_reversal():
     bad = B.step_desc("lj", dt, dict(wl.params, langevin=dict(gamma=1.0, kT=1.0, seed=1)), nvt=nvt)
     with pytest.raises(B.MDError):
         r.step(bad, 1)
+
+
+def test_degenerate_and_empty_bonded_terms():
+    """Collinear triplets and quadruplets are skipped on the device exactly as in the oracle (no force, no NaN), next to regular
+    terms in the same call; empty term lists and particles without terms are no-ops."""
+    wl = inputs.lj_fcc(6, rc=2.5, r_buff=0.4, kT=1.0, jitter=0.05, pos_seed=31, vel_seed=32)      # N = 864
+    pos = wl.pos.copy()
+    base = pos[10].copy()
+    for k, x in enumerate((0.0, 1.0, 2.1)):                              # particles 10, 11, 12 on a line along x
+        pos[10 + k] = base + [x, 0.0, 0.0]
+    pos[13] = base + [3.0, 0.5, 0.0]
+    pos = oracle.wrap(pos, wl.box)
+    ang = np.array([[10, 11, 12], [11, 12, 13], [20, 21, 22], [12, 11, 10]], dtype=np.uint32)
+    dih = np.array([[10, 11, 12, 13], [13, 12, 11, 10], [20, 21, 22, 23], [30, 40, 50, 60]], dtype=np.uint32)
+    md = B.MD(wl.box, wl.N, wl.rc, wl.r_buff)
+    md.set_state(pos, wl.vel)
+    md.set_angles(ang); md.set_dihedrals(dih)
+    md.build_cells()
+    md.forces_angles(6.0, 1.9); md.forces_dihedrals(2.5, -1, 3)
+    F, E = md.get_forces()
+    Fr, Er, _ = oracle.forces_angles(pos, wl.box, ang, 6.0, 1.9)
+    oracle.forces_dihedrals(pos, wl.box, dih, 2.5, -1, 3, force=Fr, energy=Er)
+    assert np.isfinite(F).all() and np.isfinite(Fr).all()
+    assert force_rel_err(F, Fr) < 1e-10 and np.abs(E - Er).max() < 1e-11 * np.abs(Er).max()
+    assert np.abs(Fr[10]).max() == 0.0 and np.abs(F[10]).max() == 0.0    # 10 only takes part in skipped terms ...
+    assert np.abs(F[13]).max() > 0.0                                     # ... 13 also in the regular angle (11, 12, 13)
+    untouched = np.setdiff1d(np.arange(wl.N), np.unique(np.concatenate([ang.ravel(), dih.ravel()])))
+    assert np.abs(F[untouched]).max() == 0.0
+    pr = md.pressure(B.step_desc("none", wl.dt, dict(angle_k=6.0, angle_theta0=1.9, dihedral_k=2.5, dihedral_sign=-1, dihedral_n=3)))
+    Wr = oracle.forces_angles(pos, wl.box, ang, 6.0, 1.9)[2] + oracle.forces_dihedrals(pos, wl.box, dih, 2.5, -1, 3)[2]
+    assert np.isfinite(pr["virial"]).all() and np.abs(pr["virial"] - Wr).max() < 1e-10 * np.abs(Wr).max()
+    # empty lists: the calls and the step flags are no-ops
+    md.set_angles(None); md.set_dihedrals(None); md.set_bonds(None)
+    md.set_state(pos, wl.vel); md.build_cells()
+    md.forces_angles(6.0, 1.9); md.forces_dihedrals(2.5, -1, 3); md.forces_bonds(1.0, 1.0); md.forces_fene(1.0, 1.5)
+    assert np.abs(md.get_forces()[0]).max() == 0.0

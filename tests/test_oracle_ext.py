@@ -438,3 +438,31 @@ def test_bond_table_of_the_harmonic_bond_is_the_harmonic_bond():
     assert np.abs(Ft - Fh).max() < 1e-11 and np.abs(Wt - Wh).max() < 1e-11
     h = rk[1] - rk[0]
     assert 0.0 <= (Et - Eh).min() and (Et - Eh).max() <= 2 * 0.5 * k * h * h / 8 + 1e-12   # chord above a convex U; 2 bonds per bead
+
+
+# ---- degenerate bonded terms (R34, R35): collinear particles -----------------------------------------------------------
+def test_collinear_angle_and_dihedral_terms_are_skipped():
+    """theta = 0 or pi has no defined gradient direction (sin theta = 0), and a dihedral with three collinear particles no
+    defined angle: both terms are skipped (no force, no energy, no NaN), while the same particles moved off the line by
+    1e-6 give finite values that follow the closed forms."""
+    box = 20.0
+    line = np.array([[0.0, 0.0, 0.0], [1.0, 0.0, 0.0], [2.1, 0.0, 0.0], [3.0, 0.5, 0.0]])
+    F, E, W = oracle.forces_angles(line, box, np.array([[0, 1, 2]], dtype=np.uint32), 7.0, 2.0)
+    assert np.abs(F).max() == 0.0 and np.abs(E).max() == 0.0 and np.abs(W).max() == 0.0
+    fold = line.copy(); fold[2] = [0.4, 0.0, 0.0]                       # theta = 0: c folded back onto the a side
+    F, E, _ = oracle.forces_angles(fold, box, np.array([[0, 1, 2]], dtype=np.uint32), 7.0, 2.0)
+    assert np.abs(F).max() == 0.0 and np.abs(E).max() == 0.0
+    bent = line.copy(); bent[2, 1] = 1e-6
+    F, E, _ = oracle.forces_angles(bent, box, np.array([[0, 1, 2]], dtype=np.uint32), 7.0, 2.0)
+    th = math.pi - math.atan2(1e-6, 1.1)
+    assert np.isfinite(F).all() and abs(E.sum() - 0.5 * 7.0 * (th - 2.0) ** 2) < 1e-9
+    # dihedral: a, b, c collinear (A = F x G = 0), then b, c, d collinear (B = 0)
+    q = np.array([[0, 1, 2, 3]], dtype=np.uint32)
+    for pts in (line, line[::-1].copy()):
+        F, E, W = oracle.forces_dihedrals(pts, box, q, 3.0, 1, 2)
+        assert np.abs(F).max() == 0.0 and np.abs(E).max() == 0.0 and np.abs(W).max() == 0.0
+    off = line.copy(); off[0] = [0.0, 0.0, 1e-3]                        # a lifted out of the line: phi = +-pi/2 exactly
+    F, E, _ = oracle.forces_dihedrals(off, box, q, 3.0, 1, 2)
+    assert np.isfinite(F).all() and abs(abs(oracle.dihedral_angle(*off, box)) - 0.5 * math.pi) < 1e-12
+    assert abs(E.sum() - 0.5 * 3.0 * (1.0 + math.cos(math.pi))) < 1e-9  # U = k/2 (1 + cos(2 phi)) = 0 at phi = pi/2
+    assert abs(F.sum(axis=0)).max() < 1e-6 * np.abs(F).max()
