@@ -147,3 +147,55 @@ def test_mixed_bar_on_every_particle_of_config2():
     Fg, _ = mm.get_forces()
     errg = np.abs(Fg - F64).max(axis=1) / np.maximum(np.abs(F64).max(axis=1), 1e-3 * frms)
     assert errg.max() < 1e-4
+
+
+def test_full_size_bonded_terms_and_langevin_on_every_particle():
+    """SURVEY 8(f) row 3 at the size of configuration 4 (1.28 M beads, 1.26 M bonds, 1.24 M angles, 1.22 M dihedrals): the
+    bonded terms and the Langevin force are O(N) in the oracle as well, so the comparison is on EVERY particle, after the
+    polymer model with all of them has run 40 steps through md_step (rebuilds, batch scheduler, tuned launch sizes)."""
+    w = inputs.config(4)
+    L = 64
+    first = (np.arange(w.N // L, dtype=np.uint32)[:, None] * L)
+    i3 = (first + np.arange(L - 2, dtype=np.uint32)[None, :]).reshape(-1)
+    ang = np.stack([i3, i3 + 1, i3 + 2], axis=1).astype(np.uint32)
+    i4 = (first + np.arange(L - 3, dtype=np.uint32)[None, :]).reshape(-1)
+    dih = np.stack([i4, i4 + 1, i4 + 2, i4 + 3], axis=1).astype(np.uint32)
+    q = w.params
+    ka, th0, kd = 50.0, 2.0, 2.0
+    md = B.from_workload(w)
+    md.set_angles(ang); md.set_dihedrals(dih)
+    desc = B.step_desc("polymer", w.dt, dict(q, angle_k=ka, angle_theta0=th0, dihedral_k=kd, dihedral_sign=1, dihedral_n=1,
+                                            langevin=dict(gamma=0.5, kT=1.0, seed=77)))
+    assert desc.flags == B.MD_F_DPD | B.MD_F_BONDS | B.MD_F_ANGLES | B.MD_F_DIHEDRALS | B.MD_F_LANGEVIN
+    md.tune(desc)
+    md.step(desc, 40)
+    st = md.stats()
+    assert st["dangerous_builds"] == 0 and st["rebuilds"] >= 2
+    pos, vel, _ = md.get_state()
+    # the bonded terms and the thermostat force on the state the run left, term by term onto a cleared force array
+    md.set_state(pos, vel, None, 40)
+    md.set_angles(ang); md.set_dihedrals(dih)
+    md.build_cells()
+    md.forces_bonds(q["bond_k"], q["bond_r0"])
+    md.forces_angles(ka, th0)
+    md.forces_dihedrals(kd, 1, 1)
+    F, E = md.get_forces()
+    Fr, Er, Wr = oracle.forces_bonds_kind(pos, w.box, w.bonds, "harmonic", q["bond_k"], q["bond_r0"])
+    oracle.forces_angles(pos, w.box, ang, ka, th0, force=Fr, energy=Er, virial=Wr)
+    oracle.forces_dihedrals(pos, w.box, dih, kd, 1, 1, force=Fr, energy=Er, virial=Wr)
+    frms = np.sqrt(np.mean(np.sum(Fr * Fr, axis=1)))
+    err = np.abs(F - Fr).max(axis=1) / np.maximum(np.abs(Fr).max(axis=1), 1e-3 * frms)
+    assert err.max() < 1e-10, f"worst {err.max():.2e}"
+    assert np.abs(E - Er).max() < 1e-11 * np.abs(Er).max()
+    assert np.abs(F.sum(axis=0)).max() < 1e-9 * np.abs(F).sum()          # bonded terms carry no net force
+    # their virial through md_pressure (kinetic part checked as well)
+    pr = md.pressure(B.step_desc("bonds", w.dt, dict(bond_k=q["bond_k"], bond_r0=q["bond_r0"], angle_k=ka, angle_theta0=th0,
+                                                     dihedral_k=kd, dihedral_sign=1, dihedral_n=1)))
+    assert np.abs(pr["virial"] - Wr).max() < 1e-10 * np.abs(Wr).max()
+    assert abs(pr["kinetic"] - 0.5 * np.sum(vel * vel)) < 1e-12 * pr["kinetic"]
+    # Langevin force of all 1.28 M particles at a step index beyond 2^32: the same Philox words, the same operations
+    md.set_state(pos, vel); md.build_cells()
+    md.forces_langevin(0.5, 1.0, w.dt, (1 << 32) + 40, 77)
+    FL = md.get_forces()[0]
+    FLr = oracle.forces_langevin(vel, 0.5, 1.0, w.dt, (1 << 32) + 40, 77)
+    assert np.abs(FL - FLr).max() < 1e-12
