@@ -179,6 +179,29 @@ def pair_table(pos, box, r_min, r_max, U, F):
     return Fo, E, W
 
 
+def probe_pair_forces(pos, box, rc, kind, params, probes, energy_shift=1, table=None):
+    """Force and energy of the probe particles against all N (O(M N)); kind as pair_forces, or "table" with
+    table = (r_min, r_max, U, F) (R37)."""
+    pos, pp = _d(pos)
+    b, bp = _box(box)
+    pr, prp = _u(probes)
+    M = pr.shape[0]
+    Fo = np.zeros((M, 3)); E = np.zeros(M)
+    if kind == "table":
+        r_min, r_max, U, F = table
+        U, Up = _d(U); F, Fp = _d(F)
+        p, ppar = _p4(())
+        lib().orc_probe_pair_forces(pp, C.c_uint64(pos.shape[0]), bp, C.c_double(rc), C.c_int(4), ppar, C.c_int(0),
+                                    C.c_double(r_min), C.c_double(r_max), C.c_uint64(U.shape[0]), Up, Fp, prp, C.c_uint64(M),
+                                    Fo.ctypes.data_as(_dp), E.ctypes.data_as(_dp))
+    else:
+        p, ppar = _p4(params)
+        lib().orc_probe_pair_forces(pp, C.c_uint64(pos.shape[0]), bp, C.c_double(rc), C.c_int(PAIR_KINDS[kind]), ppar,
+                                    C.c_int(energy_shift), C.c_double(0.0), C.c_double(0.0), C.c_uint64(0), None, None, prp,
+                                    C.c_uint64(M), Fo.ctypes.data_as(_dp), E.ctypes.data_as(_dp))
+    return Fo, E
+
+
 def virial_pair(pos, box, rc, kind, params):
     """W (xx, yy, zz, xy, xz, yz) = sum over pairs of d (x) F."""
     pos, pp = _d(pos)

@@ -32,6 +32,7 @@
  *   orc_pair_table     table values at the nodes and the straight line between two nodes; tables linear in r reproduced
  *                      at any r; nothing outside [r_min, r_max), strict at r_max; tr W = r F(r); periodic wrap; a table
  *                      of the LJ closed forms against orc_forces_lj with second-order convergence in h
+ *   orc_probe_pair_forces  equal to the probes' rows of orc_pair_forces (four kinds, shifted and not) and orc_pair_table
  *   orc_bond_table     nodes and the straight line between them, NaN outside [r_min, r_max), accumulation, bond
  *                      direction, periodic wrap, tr W = r F(r); the table of a harmonic bond against
  *                      orc_forces_bonds_kind (forces exact, energies within k h^2 / 8 per bond, from above)
@@ -422,5 +423,46 @@ void orc_bond_table(const double *pos, uint64_t N, const double box[3], const ui
             for (int x = 0; x < 3; ++x) { force[3 * a + x] += Fv[x]; force[3 * b + x] -= Fv[x]; }
         if (energy) { energy[a] += 0.5 * u; energy[b] += 0.5 * u; }
         if (W) add_virial(W, d, Fv);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * Probe rows of the pair potentials (the O9 idea of md_oracle.c for R31 and R37): force and energy of M probe particles,
+ * each against ALL N particles by brute force -- O(M N), usable at the full sizes where the O(N^2) routines are not.
+ * Pinned as the rows of orc_pair_forces / orc_pair_table on a small system (tests/test_oracle_ext.py).
+ * kind 0..3: R31 with parameters p; kind 4: the table (r_min, r_max, M_tab, U, F) of R37, rc ignored.
+ * ---------------------------------------------------------------------------------------------------------------- */
+void orc_probe_pair_forces(const double *pos, uint64_t N, const double box[3], double rc, int kind, const double p[4],
+                           int energy_shift, double r_min, double r_max, uint64_t M_tab, const double *U, const double *F,
+                           const uint32_t *probes, uint64_t M, double *force, double *energy)
+{
+    double rc2 = kind == 4 ? r_max * r_max : rc * rc, uc = 0.0, d[3], u;
+    double h = kind == 4 ? (r_max - r_min) / (double)(M_tab - 1) : 0.0;
+    if (energy_shift && kind != 4) (void)pair_term(kind, rc2, p, &uc);
+    for (uint64_t q = 0; q < M; ++q) {
+        uint64_t a = probes[q];
+        double f3[3] = {0.0, 0.0, 0.0}, e = 0.0;
+        for (uint64_t b = 0; b < N; ++b) {
+            if (b == a) continue;
+            double r2 = sep(pos + 3 * a, pos + 3 * b, box, d);
+            if (!(r2 < rc2) || !(r2 > 0.0)) continue;
+            double f;
+            if (kind == 4) {
+                double r = sqrt(r2);
+                if (r < r_min) continue;
+                double s = (r - r_min) / h;
+                uint64_t k = (uint64_t)floor(s);
+                if (k > M_tab - 2) k = M_tab - 2;
+                double t = s - (double)k;
+                u = U[k] + t * (U[k + 1] - U[k]);
+                f = (F[k] + t * (F[k + 1] - F[k])) / r;
+            } else {
+                f = pair_term(kind, r2, p, &u);
+            }
+            for (int x = 0; x < 3; ++x) f3[x] += f * d[x];
+            e += 0.5 * (u - uc);
+        }
+        force[3 * q] = f3[0]; force[3 * q + 1] = f3[1]; force[3 * q + 2] = f3[2];
+        if (energy) energy[q] = e;
     }
 }

@@ -199,3 +199,30 @@ def test_full_size_bonded_terms_and_langevin_on_every_particle():
     FL = md.get_forces()[0]
     FLr = oracle.forces_langevin(vel, 0.5, 1.0, w.dt, (1 << 32) + 40, 77)
     assert np.abs(FL - FLr).max() < 1e-12
+
+
+@pytest.mark.parametrize("kind,p", [("yukawa", (2.0, 1.5)), ("morse", (1.7, 2.0, 1.0)), ("table", ())])
+def test_full_size_pair_potentials_on_probes(kind, p):
+    """SURVEY 8(f) row 3 at N = 1,048,576 (the positions of configuration 2 after 30 LJ steps): md_forces_pair on the tile
+    list against the oracle's O(M N) probe rows, 1e-10 (R11) on forces, 1e-11 on energies."""
+    w = inputs.config(2)
+    md = B.from_workload(w, precision=B.MD_FP64)
+    desc = B.step_desc(w.kind, w.dt, w.params)
+    md.step(desc, 30)
+    pos, vel, _ = md.get_state()
+    md.build_cells(); md.build_nlist()
+    probes = inputs.probe_tags(w.N, 128, seed=91)
+    table = None
+    if kind == "table":
+        rng = np.random.default_rng(17)
+        table = (0.85, 2.9, rng.normal(size=513), 3.0 * rng.normal(size=513))
+        md.set_pair_table(*table)
+        md.forces_pair("table")
+    else:
+        md.forces_pair(kind, p, 1)
+    F, E = md.get_forces()
+    Fo, Eo = oracle.probe_pair_forces(pos, w.box, w.rc, kind, p, probes, 1, table=table)
+    frms = np.sqrt(np.mean(np.sum(F * F, axis=1)))
+    assert _probe_err(F, Fo, probes, frms) < 1e-10
+    assert np.abs(E[probes] - Eo).max() < 1e-11 * np.abs(Eo).max()
+    assert np.abs(F.sum(axis=0)).max() < 1e-9 * np.abs(F).sum()              # Newton's third law over the whole list

@@ -466,3 +466,21 @@ def test_collinear_angle_and_dihedral_terms_are_skipped():
     assert np.isfinite(F).all() and abs(abs(oracle.dihedral_angle(*off, box)) - 0.5 * math.pi) < 1e-12
     assert abs(E.sum() - 0.5 * 3.0 * (1.0 + math.cos(math.pi))) < 1e-9  # U = k/2 (1 + cos(2 phi)) = 0 at phi = pi/2
     assert abs(F.sum(axis=0)).max() < 1e-6 * np.abs(F).max()
+
+
+def test_probe_pair_forces_are_the_rows_of_the_full_routines():
+    rng = np.random.default_rng(41)
+    n = 5
+    g = (np.stack(np.meshgrid(*[np.arange(n)] * 3, indexing="ij"), -1).reshape(-1, 3) + 0.5) * 1.25
+    pos = g + rng.uniform(-0.1, 0.1, size=g.shape)
+    box, rc = n * 1.25, 2.5
+    probes = np.array([0, 7, 63, 124], dtype=np.uint32)
+    for kind, p in (("yukawa", (2.0, 1.5)), ("gaussian", (3.0, 0.8)), ("morse", (1.7, 2.0, 1.0)), ("lj", (0.9, 1.05))):
+        for shift in (0, 1):
+            F, E = oracle.pair_forces(pos, box, rc, kind, p, shift)
+            Fp, Ep = oracle.probe_pair_forces(pos, box, rc, kind, p, probes, shift)
+            assert np.abs(Fp - F[probes]).max() < 1e-12 * np.abs(F).max() and np.abs(Ep - E[probes]).max() < 1e-12 * np.abs(E).max()
+    U, Ft = rng.normal(size=65), rng.normal(size=65)
+    F, E, _ = oracle.pair_table(pos, box, 0.6, 2.2, U, Ft)
+    Fp, Ep = oracle.probe_pair_forces(pos, box, rc, "table", (), probes, table=(0.6, 2.2, U, Ft))
+    assert np.abs(Fp - F[probes]).max() < 1e-12 * np.abs(F).max() and np.abs(Ep - E[probes]).max() < 1e-12 * np.abs(E).max()
