@@ -193,6 +193,25 @@ def test_full_size_bonded_terms_and_langevin_on_every_particle():
                                                      dihedral_k=kd, dihedral_sign=1, dihedral_n=1)))
     assert np.abs(pr["virial"] - Wr).max() < 1e-10 * np.abs(Wr).max()
     assert abs(pr["kinetic"] - 0.5 * np.sum(vel * vel)) < 1e-12 * pr["kinetic"]
+    # FENE and tabulated bonds on the same 1.26 M bonds
+    rng = np.random.default_rng(3)
+    Ut, Ft = rng.normal(size=257), 4.0 * rng.normal(size=257)
+    lens = np.linalg.norm((lambda d: d - w.box * np.round(d / w.box))(pos[w.bonds[:, 0]] - pos[w.bonds[:, 1]]), axis=1)
+    r_lo, r_hi = 0.9 * lens.min(), 1.1 * lens.max()
+    assert r_hi < 2.4                                                   # (FENE below needs r < r0 = 2.5 for every bond)
+    md.set_bond_table(r_lo, r_hi, Ut, Ft)
+    for which in ("fene", "table"):
+        md.set_state(pos, vel); md.build_cells()
+        if which == "fene":
+            md.forces_fene(30.0, 2.5)
+            Fb, Eb, _ = oracle.forces_bonds_kind(pos, w.box, w.bonds, "fene", 30.0, 2.5)
+        else:
+            md.forces_bond_table()
+            Fb, Eb, _ = oracle.bond_table(pos, w.box, w.bonds, r_lo, r_hi, Ut, Ft)
+        Fg, Eg = md.get_forces()
+        fr = np.sqrt(np.mean(np.sum(Fb * Fb, axis=1)))
+        eb = np.abs(Fg - Fb).max(axis=1) / np.maximum(np.abs(Fb).max(axis=1), 1e-3 * fr)
+        assert np.isfinite(Fb).all() and eb.max() < 1e-10 and np.abs(Eg - Eb).max() < 1e-11 * np.abs(Eb).max(), which
     # Langevin force of all 1.28 M particles at a step index beyond 2^32: the same Philox words, the same operations
     md.set_state(pos, vel); md.build_cells()
     md.forces_langevin(0.5, 1.0, w.dt, (1 << 32) + 40, 77)
