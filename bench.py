@@ -325,7 +325,10 @@ def run_ours(args):
         # the library picks the skin with the most steps per second (md_tune_rbuff); named in the
         # workload -- the reported BASELINE configuration keeps r_buff = 0.4
         import dataclasses
-        rb = md.tune_rbuff(desc, None, 200)
+        # the bursts must see the state the run will be in: first past the start-up transient (a melt built as random walks
+        # relaxes for ~100 steps with faster particles, which favours a larger skin than the steady state does)
+        md.step(desc, max(200, args.warmup))
+        rb = md.tune_rbuff(desc, None, 300)
         w = dataclasses.replace(w, r_buff=rb, name=w.name + "-autorbuff%g" % rb)
         if not args.no_tune:
             md.tune(desc, False)
